@@ -1,0 +1,298 @@
+"""fp64 CPU oracle for the Test-Time Speculation (TTS) distillation step.
+
+TEST INFRASTRUCTURE ONLY.  Only ``tests/``, ``__graft_entry__.smoke()`` and
+``bench.py``'s ``cpu_baseline`` / ``--impl reference`` legs may import this
+file.  It shares no code with the CUDA path (``paper_2605_09329_b200/``) and
+neither imports the other.  It is deliberately plain and slow: numpy in fp64,
+the formulas of the paper written out in the paper's order, no blocking or
+fusion beyond an optional split of the vocabulary into slabs (used only so
+that the 150K-row configurations fit in host memory; the arithmetic per
+element is unchanged).
+
+What it computes, with the passage each step follows
+(PAPER.md = /root/reference/PAPER.md, arxiv/paper_2605_09329):
+
+  * ``accept_mask``       greedy longest matching prefix; loop structure of the
+                          accept step, PAPER.md:97-101 (§4 step 2) and Alg. 1
+                          "Accept" PAPER.md:152.  Greedy variant per north_star
+                          (reading R8).
+  * ``row_weights``       w_k of PAPER.md:123-127 expanded per row, times the
+                          mask factor chosen by ``mask_mode`` (R2).
+  * ``loss_and_grads``    L_t = K~L(p||q) + lambda K~L(q_t||q), PAPER.md:119-125,
+                          Alg. 1; gradient evaluated at q = q_t
+                          (PAPER.md:158).
+  * ``sgd_update``        q <- q - eta grad L, Alg. 1 "Update" PAPER.md:158.
+  * ``adamw_update``      "an optimizer (Adam) step", PAPER.md:393 (App. C.1);
+                          hyper-parameter conventions per DESIGN.md R5.
+  * ``distill_step``      the whole step (dense, small shapes).
+  * ``distill_step_rows`` the same step restricted to a subset of vocabulary
+                          rows, given the full-vocabulary normalisers, so that a
+                          full-size configuration can be checked on samples.
+
+Pins (tests/test_oracle_pins.py): brute-force enumeration through the softmax
+Jacobian, central finite differences, closed forms (V=2, uniform draft,
+one-hot teacher, teacher == draft), invariants, and reduction to fp64
+torch autograd / torch.optim.  No function here is "parity unpinned".
+"""
+
+from __future__ import annotations
+
+import numpy as np
+
+# mask_mode values (R2)
+ROWS_ALL = 0
+ROWS_ACCEPTED = 1
+ROWS_ACCEPTED_PLUS_ONE = 2
+
+
+# ----------------------------------------------------------------------------
+# bf16 <-> fp32/fp64 bit conversions (the oracle's own; the CUDA path and the
+# input generators each have theirs)
+# ----------------------------------------------------------------------------
+
+def f32_to_bf16_bits(x: np.ndarray) -> np.ndarray:
+    """Round-to-nearest-even fp32 -> bf16, returned as uint16 bit patterns."""
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    u = x.view(np.uint32).astype(np.uint64)
+    lsb = (u >> 16) & 1
+    r = (u + 0x7FFF + lsb) >> 16
+    out = r.astype(np.uint16)
+    nan = np.isnan(x)
+    if nan.any():
+        out = np.where(nan, np.uint16(0x7FC0), out)
+    return out
+
+
+def bf16_bits_to_f64(b: np.ndarray) -> np.ndarray:
+    """Exact widening of bf16 bit patterns to fp64."""
+    b = np.ascontiguousarray(b, dtype=np.uint16)
+    return (b.astype(np.uint32) << 16).view(np.float32).astype(np.float64)
+
+
+def widen(x: np.ndarray) -> np.ndarray:
+    """Inputs arrive as the exact bits the GPU receives: uint16 = bf16 bits,
+    float32 or float64 arrays are widened exactly."""
+    if x.dtype == np.uint16:
+        return bf16_bits_to_f64(x)
+    return np.asarray(x, dtype=np.float64)
+
+
+# ----------------------------------------------------------------------------
+# a1: accepted-prefix mask (greedy variant)
+# ----------------------------------------------------------------------------
+
+def accept_mask(teacher_logits, draft_tokens, seg_len):
+    """Row k of ``teacher_logits`` judges ``draft_tokens[k]`` (R10).
+
+    am[r]   = argmax_v t[r, v], lowest index on ties (R11)
+    mask[r] = 1 while every earlier row of the same segment matched, else 0
+    tau[s]  = number of matched draft positions in segment s (0..seg_len) (R9)
+    """
+    t = widen(teacher_logits)
+    tok = np.asarray(draft_tokens, dtype=np.int64)
+    T = t.shape[0]
+    assert T % seg_len == 0 and tok.shape == (T,)
+    am = np.zeros(T, dtype=np.int32)
+    mask = np.zeros(T, dtype=np.uint8)
+    tau = np.zeros(T // seg_len, dtype=np.int32)
+    for s in range(T // seg_len):
+        alive = True                      # "if x_{t+k} rejected then break"
+        for k in range(seg_len):
+            r = s * seg_len + k
+            row = t[r]
+            # lowest index among the maxima, written out (not np.argmax) so the
+            # tie rule is visible
+            best_v = int(np.flatnonzero(row == row.max())[0])
+            am[r] = best_v
+            if alive and best_v == tok[r]:
+                mask[r] = 1
+                tau[s] += 1
+            else:
+                alive = False
+    return mask, tau, am
+
+
+# ----------------------------------------------------------------------------
+# a8 weights
+# ----------------------------------------------------------------------------
+
+def row_weights(pos_weight, mask, mask_mode, seg_len):
+    """omega_r = w_k times the mask factor.  ROWS_ALL: factor 1 (PAPER.md:123 sums
+    over every k = 1..C).  ROWS_ACCEPTED: factor mask[r].  ROWS_ACCEPTED_PLUS_ONE:
+    also the first rejected row of each segment."""
+    w = np.asarray(pos_weight, dtype=np.float64).copy()
+    if mask_mode == ROWS_ALL or mask is None:
+        return w
+    m = np.asarray(mask, dtype=np.float64).copy()
+    if mask_mode == ROWS_ACCEPTED_PLUS_ONE:
+        T = m.shape[0]
+        for s in range(T // seg_len):
+            seg = m[s * seg_len:(s + 1) * seg_len]
+            n = int(seg.sum())
+            if n < seg_len:
+                seg[n] = 1.0
+    return w * m
+
+
+# ----------------------------------------------------------------------------
+# a2-a6: loss and gradients
+# ----------------------------------------------------------------------------
+
+def logsumexp_rows(x):
+    m = x.max(axis=1, keepdims=True)
+    return (m + np.log(np.exp(x - m).sum(axis=1, keepdims=True)))[:, 0]
+
+
+def kl_rows_from_logits(a_logits, b_logits):
+    """KL(softmax(a) || softmax(b)) per row; terms with softmax(a)=0 dropped."""
+    la = a_logits - logsumexp_rows(a_logits)[:, None]
+    lb = b_logits - logsumexp_rows(b_logits)[:, None]
+    pa = np.exp(la)
+    with np.errstate(invalid="ignore"):
+        term = np.where(pa > 0.0, pa * (la - lb), 0.0)
+    return term.sum(axis=1)
+
+
+def loss_and_grads(teacher_logits, h, W, omega, loss_scale=1.0, lam=0.0, z_ref=None):
+    """Dense evaluation.  Returns dict(loss, kl_rows, z, lse_t, lse_z, dl, gW, gh).
+
+    1. z[r,v] = sum_j h[r,j] W[v,j]                      (q = q_t)
+    2. log p = t - lse(t), log q = z - lse(z)
+    3. KL_r = sum_v p (log p - log q)
+    4. loss = loss_scale * sum_r omega_r KL_r            (a sum)
+       + loss_scale * lam * sum_r omega_r KL(q_ref||q)_r
+    5. dl = loss_scale * omega_r [(q - p) + lam (q - q_ref)]
+    6. gW = dl^T h, gh = dl W
+    """
+    t = widen(teacher_logits)
+    hh = widen(h)
+    WW = widen(W)
+    om = np.asarray(omega, dtype=np.float64)
+    z = hh @ WW.T
+    lse_t = logsumexp_rows(t)
+    lse_z = logsumexp_rows(z)
+    p = np.exp(t - lse_t[:, None])
+    q = np.exp(z - lse_z[:, None])
+    kl = kl_rows_from_logits(t, z)
+    loss = loss_scale * float((om * kl).sum())
+    dl = (q - p)
+    if lam != 0.0:
+        zr = z if z_ref is None else np.asarray(z_ref, dtype=np.float64)
+        q_ref = np.exp(zr - logsumexp_rows(zr)[:, None])
+        kl_reg = kl_rows_from_logits(zr, z)
+        loss += loss_scale * lam * float((om * kl_reg).sum())
+        dl = dl + lam * (q - q_ref)
+    dl = loss_scale * om[:, None] * dl
+    gW = dl.T @ hh
+    gh = dl @ WW
+    return dict(loss=loss, kl_rows=kl, z=z, lse_t=lse_t, lse_z=lse_z, dl=dl, gW=gW, gh=gh)
+
+
+# ----------------------------------------------------------------------------
+# a7: updates
+# ----------------------------------------------------------------------------
+
+def sgd_update(M, g, lr):
+    """Alg. 1 'Update': M <- M - lr g."""
+    return np.asarray(M, dtype=np.float64) - lr * g
+
+
+def adamw_update(M, m, v, g, step, lr, beta1, beta2, eps, weight_decay):
+    """Adam with decoupled weight decay, bias correction on,
+    step counted from 1, eps outside the square root (R5)."""
+    M = np.asarray(M, dtype=np.float64)
+    m = np.asarray(m, dtype=np.float64)
+    v = np.asarray(v, dtype=np.float64)
+    M = M * (1.0 - lr * weight_decay)
+    m_new = beta1 * m + (1.0 - beta1) * g
+    v_new = beta2 * v + (1.0 - beta2) * g * g
+    m_hat = m_new / (1.0 - beta1 ** step)
+    v_hat = v_new / (1.0 - beta2 ** step)
+    M_new = M - lr * m_hat / (np.sqrt(v_hat) + eps)
+    return M_new, m_new, v_new
+
+
+def working_copy_bits(M_new):
+    """bf16 working copy = rn_bf16(rn_fp32(M_new)): the GPU's master is fp32."""
+    return f32_to_bf16_bits(np.asarray(M_new, dtype=np.float64).astype(np.float32))
+
+
+# ----------------------------------------------------------------------------
+# whole step
+# ----------------------------------------------------------------------------
+
+def distill_step(teacher_logits, h, W_in, W_master, adam_m, adam_v, pos_weight, mask,
+                 *, seg_len, mask_mode=ROWS_ALL, loss_scale=1.0, optimizer="adamw",
+                 lr=1e-5, beta1=0.9, beta2=0.999, eps=1e-8, weight_decay=0.0, step=1):
+    """One TTS update (Alg. 1 lines 'Loss' + 'Update'), dense.
+
+    W_in     : working weights that produced q_t (bf16 bits or fp32)
+    W_master : fp32 master (None when the parameters are fp32: W_in is the parameter)
+    Returns dict with loss, kl_rows, gW, gh, master, m, v (fp64) and W_out
+    (bf16 bits when a master exists, else fp32).
+    """
+    omega = row_weights(pos_weight, mask, mask_mode, seg_len)
+    r = loss_and_grads(teacher_logits, h, W_in, omega, loss_scale)
+    M = widen(W_master) if W_master is not None else widen(W_in)
+    if optimizer == "sgd":
+        M_new = sgd_update(M, r["gW"], lr)
+        m_new = v_new = None
+    else:
+        M_new, m_new, v_new = adamw_update(M, widen(adam_m), widen(adam_v), r["gW"], step,
+                                           lr, beta1, beta2, eps, weight_decay)
+    out = dict(r)
+    out.update(omega=omega, master=M_new, m=m_new, v=v_new)
+    if W_master is not None:
+        out["W_out"] = working_copy_bits(M_new)
+    else:
+        out["W_out"] = M_new.astype(np.float32)
+    return out
+
+
+def row_normalisers(teacher_logits, h, W_in, slab=8192):
+    """Full-vocabulary z, lse_t, lse_z, KL_r computed slab by slab over V (same
+    arithmetic as ``loss_and_grads`` steps 1-3; only the matmul is split)."""
+    t = widen(teacher_logits)
+    hh = widen(h)
+    V = W_in.shape[0]
+    z = np.empty((hh.shape[0], V), dtype=np.float64)
+    for v0 in range(0, V, slab):
+        z[:, v0:v0 + slab] = hh @ widen(W_in[v0:v0 + slab]).T
+    lse_t = logsumexp_rows(t)
+    lse_z = logsumexp_rows(z)
+    kl = kl_rows_from_logits(t, z)
+    return z, lse_t, lse_z, kl
+
+
+def distill_step_rows(rows, z, lse_t, lse_z, teacher_logits, h, W_in_rows, W_master_rows,
+                      adam_m_rows, adam_v_rows, omega, *, loss_scale=1.0, optimizer="adamw",
+                      lr=1e-5, beta1=0.9, beta2=0.999, eps=1e-8, weight_decay=0.0, step=1):
+    """The step for the vocabulary rows ``rows`` only (gW rows, updated state),
+    given the full-vocabulary normalisers from ``row_normalisers``."""
+    t = widen(teacher_logits)[:, rows]
+    hh = widen(h)
+    om = np.asarray(omega, dtype=np.float64)
+    p = np.exp(t - lse_t[:, None])
+    q = np.exp(z[:, rows] - lse_z[:, None])
+    dl = loss_scale * om[:, None] * (q - p)
+    gW = dl.T @ hh
+    M = widen(W_master_rows) if W_master_rows is not None else widen(W_in_rows)
+    if optimizer == "sgd":
+        M_new, m_new, v_new = sgd_update(M, gW, lr), None, None
+    else:
+        M_new, m_new, v_new = adamw_update(M, widen(adam_m_rows), widen(adam_v_rows), gW, step,
+                                           lr, beta1, beta2, eps, weight_decay)
+    return dict(dl=dl, gW=gW, master=M_new, m=m_new, v=v_new)
+
+
+def gh_full(z, lse_t, lse_z, teacher_logits, W_in, omega, loss_scale=1.0, slab=8192):
+    """gh = dl W accumulated slab by slab over V (a5)."""
+    t = widen(teacher_logits)
+    om = np.asarray(omega, dtype=np.float64)
+    V = W_in.shape[0]
+    gh = np.zeros((t.shape[0], W_in.shape[1]), dtype=np.float64)
+    for v0 in range(0, V, slab):
+        sl = slice(v0, min(V, v0 + slab))
+        dl = loss_scale * om[:, None] * (np.exp(z[:, sl] - lse_z[:, None]) - np.exp(t[:, sl] - lse_t[:, None]))
+        gh += dl @ widen(W_in[sl])
+    return gh
