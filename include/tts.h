@@ -1,0 +1,206 @@
+/*
+ * tts.h -- C ABI of the B200-native online-distillation step of Test-Time
+ * Speculation (TTS), arxiv/paper_2605_09329.  Citations are lines of
+ * /root/reference/PAPER.md ("PAPER.md:<line>") and readings R<n> of DESIGN.md.
+ *
+ * What the library does.  After a speculative-decoding round the caller holds
+ * the target's (teacher's) logits over the C canvas positions, the canvas
+ * tokens and the draft's state.  It wants
+ *   (i)  tau, the accepted-prefix length            (PAPER.md:115 step c, 152), and
+ *   (ii) the draft updated by ONE optimisation step on
+ *            L_t(q) = sum_k w_k KL(p_k || q_k) [+ lambda sum_k w_k KL(q_t,k || q_k)]
+ *        evaluated at q = q_t                        (Alg. 1 154-158),
+ *        off the critical path on a side stream.
+ * The trained parameters are the draft LM head W[V,d] (bf16 working copy + fp32
+ * master + optimiser state); the gradient w.r.t. the draft hidden states h is
+ * returned for whatever sits upstream.  At one step per round the lambda term is
+ * identically zero in loss and gradient (q = q_t), so it is not computed (R3).
+ *
+ * Conventions
+ *   - Plain C, no C++ exceptions cross the ABI.  Every function returns a status
+ *     (TTS_OK = 0) unless stated otherwise.
+ *   - Unless a parameter says "host", every data pointer is a DEVICE pointer on
+ *     the ctx's device, 16-byte aligned, row-major contiguous.  The caller owns
+ *     every tensor; the library owns only the scratch inside tts_ctx (allocated
+ *     in tts_ctx_create, never in a step).
+ *   - `stream` parameters are cudaStream_t handles passed as void* (so that this
+ *     header needs no CUDA include).  Step and mask calls only ENQUEUE work; they
+ *     never synchronise the host.  Device outputs are valid once the stream has
+ *     reached the step's done-event (tts_wait_step / tts_sync_step).
+ *   - One ctx per side stream.  Calls on one ctx are not thread-safe; distinct
+ *     ctxs are independent.
+ *   - There is no CPU fallback: on a machine without an sm_100 device
+ *     tts_ctx_create fails with TTS_ERR_ARCH / TTS_ERR_CUDA.
+ */
+#ifndef TTS_H_
+#define TTS_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* status codes */
+enum {
+  TTS_OK = 0,
+  TTS_ERR_INVALID_ARG = 1, /* NULL where data is required, T out of range, misaligned pointer */
+  TTS_ERR_UNSUPPORTED = 2, /* dtype / shape combination outside the supported set */
+  TTS_ERR_CUDA = 3,        /* a CUDA call failed; see tts_last_cuda_error */
+  TTS_ERR_ARCH = 4         /* device is not compute capability 10.x */
+};
+
+/* dtypes */
+enum { TTS_F32 = 0, TTS_BF16 = 1 };
+/* optimisers: Alg. 1 writes plain gradient descent; App. C.1 names Adam */
+enum { TTS_SGD = 0, TTS_ADAMW = 1 };
+/* which canvas rows enter the loss (R2).  The paper sums over all k = 1..C. */
+enum { TTS_ROWS_ALL = 0, TTS_ROWS_ACCEPTED = 1, TTS_ROWS_ACCEPTED_PLUS_ONE = 2 };
+/* kernel family.  AUTO: tcgen05/TMA kernels when param_dtype is bf16 and the shape
+ * qualifies (V % 128 == 0, d % 128 == 0, T <= 16 per step), CUDA-core kernels otherwise
+ * (fp32 parameters, e.g. BASELINE config 1; other shapes).  SIMT forces the CUDA-core kernels. */
+enum { TTS_PATH_AUTO = 0, TTS_PATH_SIMT = 1 };
+
+typedef struct tts_ctx tts_ctx;
+
+typedef struct {
+  int32_t V;            /* vocabulary size                                                    */
+  int32_t d;            /* draft hidden size                                                  */
+  int32_t T_max;        /* max rows (canvas positions x sequences) per step, <= 4096          */
+  int32_t seg_len;      /* C: rows per sequence; the prefix logic restarts every seg_len rows */
+  int32_t param_dtype;  /* TTS_BF16: bf16 working copy + fp32 master | TTS_F32: fp32 only     */
+  int32_t logits_dtype; /* teacher logits: TTS_BF16 | TTS_F32                                 */
+  int32_t optimizer;    /* TTS_SGD | TTS_ADAMW                                                */
+  float lr, beta1, beta2, eps, weight_decay; /* R5: eps outside the sqrt, bias correction on, */
+                                             /* decoupled decay M <- M (1 - lr wd)            */
+  int32_t mask_mode;    /* TTS_ROWS_*                                                         */
+  int32_t max_ctas;     /* 0 = one CTA per SM; else cap the persistent kernels' grids so the  */
+                        /* main stream keeps SMs while the step overlaps it    */
+  int32_t kernel_path;  /* TTS_PATH_*                                                         */
+} tts_config;
+
+const char* tts_status_string(int32_t status);
+/* library version, major*10000 + minor*100 + patch */
+int32_t tts_version(void);
+
+/* Creates a context on `device` (a CUDA ordinal) and allocates all scratch.
+ * Errors: INVALID_ARG (NULL, non-positive sizes, T_max % seg_len != 0), UNSUPPORTED,
+ * ARCH (not sm_10x), CUDA. */
+int32_t tts_ctx_create(const tts_config* cfg, int32_t device, tts_ctx** out);
+int32_t tts_ctx_destroy(tts_ctx* ctx);
+
+/* Hyper-parameters may change between steps. */
+int32_t tts_set_lr(tts_ctx* ctx, float lr);
+/* Adam's bias-correction step count n lives in the ctx: 0 after create, incremented at the
+ * start of every tts_distill_step (so the first step uses n = 1).  Set it to resume a stream
+ * or after restoring a snapshot (the paper resets the speculator between requests). */
+int32_t tts_set_step_count(tts_ctx* ctx, int64_t n);
+int64_t tts_get_step_count(const tts_ctx* ctx);   /* returns the count, not a status */
+/* CUDA error code (cudaError_t as int) of the last failed CUDA call on this ctx, 0 if none. */
+int32_t tts_last_cuda_error(const tts_ctx* ctx);
+/* 1 if the last tts_distill_step on this ctx ran the tcgen05/TMA kernels, 0 if CUDA-core. */
+int32_t tts_last_step_used_tensor_path(const tts_ctx* ctx);
+/* number of kernels the last tts_distill_step / tts_accept_mask enqueued (for bench.py's gpu_launches) */
+int32_t tts_last_launch_count(const tts_ctx* ctx);
+
+/*
+ * a1.  Greedy accepted-prefix mask: the accept loop of PAPER.md:97-101 / Alg. 1 "Accept"
+ * with the greedy rule "teacher argmax == draft token" in place of the
+ * stochastic min{1,p/q} test (north_star (4); R8).
+ *   am[r]   = argmax_v teacher_logits[r,v], LOWEST index on ties (R11), raw values compared
+ *   mask[r] = 1 iff rows s*C .. r of r's segment all have am == draft_tokens
+ *   tau[s]  = number of matched draft positions in segment s, 0..C.  The paper's acceptance
+ *             length (which counts the target's bonus token) is tau + 1 (R9).
+ * Row r of teacher_logits is the distribution that judges draft_tokens[r]; no shift is
+ * applied inside the library (R10).  Logits must be finite or -inf; NaN gives undefined
+ * results.  Integer/compare only: bit-exact.
+ */
+int32_t tts_accept_mask(tts_ctx* ctx,
+                        const void* teacher_logits,  /* [T,V] logits_dtype                     */
+                        const int32_t* draft_tokens, /* [T]   canvas tokens                    */
+                        int32_t T,                   /* multiple of seg_len, 1..T_max          */
+                        uint8_t* mask_out,           /* [T]   1 = inside the accepted prefix   */
+                        int32_t* tau_out,            /* [T/seg_len]                            */
+                        int32_t* teacher_argmax_out, /* [T] or NULL                            */
+                        void* stream);
+
+/*
+ * a2-a8.  One TTS update (Alg. 1 "Loss" + "Update"):
+ *   z      = h W_in^T                                   draft logits at q = q_t
+ *   KL_r   = KL(softmax(teacher_r) || softmax(z_r)), -inf teacher entries = p 0
+ *   omega_r= pos_weight[r] * maskfactor_r               (w_k of PAPER.md:123-127; R1, R2)
+ *   loss   = loss_scale * sum_r omega_r KL_r            a SUM, not a mean (R3')
+ *   dl     = loss_scale * omega_r (softmax(z_r) - softmax(teacher_r))
+ *   gW     = dl^T h,  gh = dl W_in
+ *   SGD    : M <- M - lr gW
+ *   AdamW  : M <- M (1 - lr wd); m <- b1 m + (1-b1) g; v <- b2 v + (1-b2) g^2;
+ *            M <- M - lr (m / (1-b1^n)) / (sqrt(v / (1-b2^n)) + eps)      (R5)
+ *   W_out  = rn_bf16(M)   (TTS_BF16)   |   W_out = M   (TTS_F32, W_master == NULL)
+ *
+ * Preconditions: for TTS_BF16, W_in == rn_bf16(W_master) element-wise at entry; teacher_logits
+ * and h must stay untouched until the done-event (the step consumes the buffers captured at
+ * dispatch time; R17); W_out may alias W_in, but when draft rounds keep reading
+ * W_in during the update pass distinct buffers and swap them at the barrier (R18).
+ * All kernels are enqueued on side_stream; a done-event is recorded after the last one.
+ */
+int32_t tts_distill_step(tts_ctx* ctx,
+                         const void* teacher_logits, /* [T,V] logits_dtype                                   */
+                         const void* h,              /* [T,d] param_dtype: draft hidden states               */
+                         const void* W_in,           /* [V,d] param_dtype: weights that produced q_t         */
+                         void* W_out,                /* [V,d] param_dtype: updated weights; may alias W_in   */
+                         float* W_master,            /* [V,d] fp32 in place; NULL iff TTS_F32                */
+                         float* adam_m,              /* [V,d] fp32 in place; NULL iff TTS_SGD                */
+                         float* adam_v,              /* [V,d] fp32 in place; NULL iff TTS_SGD                */
+                         const float* pos_weight,    /* [T]   w_k already expanded per row                   */
+                         const uint8_t* mask,        /* [T]   from tts_accept_mask; may be NULL for ROWS_ALL */
+                         int32_t T,                  /* multiple of seg_len, 1..T_max                        */
+                         float loss_scale,           /* multiplies the loss and every gradient               */
+                         float* loss_out,            /* [1]                                                  */
+                         float* kl_rows_out,         /* [T] unweighted KL_r, or NULL                         */
+                         float* gh_out,              /* [T,d] fp32, or NULL (then gh is not computed)        */
+                         float* gW_debug_out,        /* [V,d] fp32, or NULL (parity mode: extra 4 V d bytes) */
+                         void* side_stream);
+
+/*
+ * Per-phase device timing (for bench.py's roofline line).  When enabled, tts_distill_step records
+ * CUDA events on side_stream between its phases (no host synchronisation is added).  Phases:
+ *   0 = a2 draft logits, 1 = a3 row statistics + loss, 2 = a4 dlogits / operand preparation,
+ *   3 = a5 gh (0 when fused into phase 4), 4 = a6 + a7 gW contraction fused with the update.
+ * tts_profile_read synchronises with the last profiled step, writes the MEAN milliseconds per phase
+ * over the steps recorded since the last read (at most 256 are kept) into ms_out (HOST, [5]), stores
+ * the number of steps averaged in *n_steps_out (HOST, may be NULL) and resets the accumulation.
+ */
+enum { TTS_NUM_PHASES = 5 };
+int32_t tts_profile_enable(tts_ctx* ctx, int32_t enable);
+int32_t tts_profile_read(tts_ctx* ctx, float* ms_out, int32_t* n_steps_out);
+
+/* The paper's barrier after S-1 rounds: main_stream waits (on the device) for the
+ * last step's done-event. */
+int32_t tts_wait_step(tts_ctx* ctx, void* main_stream);
+/* Host blocks until the last step is done: the CPU-side barrier the paper needed in front of
+ * CUDA-graph replay. */
+int32_t tts_sync_step(tts_ctx* ctx);
+
+/*
+ * One whole round through HOST buffers (used for end-to-end timing): copies the round's inputs
+ * from (preferably pinned) host memory into ctx-owned staging buffers, runs tts_accept_mask and
+ * tts_distill_step on `stream`, copies loss / tau / mask back and synchronises the stream.
+ * The persistent draft state (W, master, m, v) stays resident on the device: device pointers.
+ */
+int32_t tts_round_host(tts_ctx* ctx,
+                       const void* teacher_logits_host, /* host [T,V] logits_dtype */
+                       const void* h_host,              /* host [T,d] param_dtype  */
+                       const int32_t* draft_tokens_host,/* host [T]                */
+                       const float* pos_weight_host,    /* host [T]                */
+                       int32_t T, float loss_scale,
+                       const void* W_in, void* W_out, float* W_master, float* adam_m, float* adam_v, /* device */
+                       float* gh_dev,                   /* device [T,d] or NULL    */
+                       float* loss_host,                /* host [1]                */
+                       int32_t* tau_host,               /* host [T/seg_len]        */
+                       uint8_t* mask_host,              /* host [T] or NULL        */
+                       void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TTS_H_ */

@@ -1,0 +1,294 @@
+// C-ABI entry points of libtts_b200.so (include/tts.h): context, validation, dispatch.
+// All arithmetic lives in the kernels (tts_mask.cu, tts_stats.cu, tts_simt.cu, tts_tc.cu).
+#include <math.h>
+#include <new>
+#include <stdlib.h>
+#include <string.h>
+
+#include "tts_internal.h"
+
+namespace {
+
+inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+inline int32_t cuda_fail(tts_ctx* c, cudaError_t e) {
+  if (c) c->last_cuda_error = static_cast<int>(e);
+  return TTS_ERR_CUDA;
+}
+
+size_t elem_size(int dtype) { return dtype == TTS_BF16 ? 2 : 4; }
+
+template <typename T>
+cudaError_t dmalloc(T** p, size_t n) {
+  *p = nullptr;
+  if (n == 0) return cudaSuccess;
+  return cudaMalloc(reinterpret_cast<void**>(p), n * sizeof(T));
+}
+
+void free_all(tts_ctx* c) {
+  if (!c) return;
+  tts::tc_destroy(c);
+  cudaFree(c->z); cudaFree(c->dl32); cudaFree(c->stat_part); cudaFree(c->row_stats);
+  cudaFree(c->arg_val); cudaFree(c->arg_idx); cudaFree(c->argmax_tmp);
+  cudaFree(c->st_teacher); cudaFree(c->st_h); cudaFree(c->st_tok); cudaFree(c->st_pw);
+  cudaFree(c->st_mask); cudaFree(c->st_tau); cudaFree(c->st_loss);
+  if (c->done_event) cudaEventDestroy(c->done_event);
+  if (c->prof_events) {
+    for (int i = 0; i < tts::kProfSlots * (TTS_NUM_PHASES + 1); ++i) cudaEventDestroy(c->prof_events[i]);
+    free(c->prof_events);
+  }
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* tts_status_string(int32_t s) {
+  switch (s) {
+    case TTS_OK: return "TTS_OK";
+    case TTS_ERR_INVALID_ARG: return "TTS_ERR_INVALID_ARG";
+    case TTS_ERR_UNSUPPORTED: return "TTS_ERR_UNSUPPORTED";
+    case TTS_ERR_CUDA: return "TTS_ERR_CUDA";
+    case TTS_ERR_ARCH: return "TTS_ERR_ARCH";
+    default: return "TTS_ERR_UNKNOWN";
+  }
+}
+
+int32_t tts_version(void) { return 100; /* 0.1.0 */ }
+
+int32_t tts_ctx_create(const tts_config* cfg, int32_t device, tts_ctx** out) {
+  if (!cfg || !out) return TTS_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (cfg->V <= 0 || cfg->d <= 0 || cfg->T_max <= 0 || cfg->seg_len <= 0) return TTS_ERR_INVALID_ARG;
+  if (cfg->T_max > 4096 || cfg->T_max % cfg->seg_len != 0) return TTS_ERR_INVALID_ARG;
+  if (cfg->param_dtype != TTS_F32 && cfg->param_dtype != TTS_BF16) return TTS_ERR_UNSUPPORTED;
+  if (cfg->logits_dtype != TTS_F32 && cfg->logits_dtype != TTS_BF16) return TTS_ERR_UNSUPPORTED;
+  if (cfg->optimizer != TTS_SGD && cfg->optimizer != TTS_ADAMW) return TTS_ERR_UNSUPPORTED;
+  if (cfg->mask_mode < TTS_ROWS_ALL || cfg->mask_mode > TTS_ROWS_ACCEPTED_PLUS_ONE) return TTS_ERR_UNSUPPORTED;
+  if (cfg->kernel_path != TTS_PATH_AUTO && cfg->kernel_path != TTS_PATH_SIMT) return TTS_ERR_UNSUPPORTED;
+  if (cfg->max_ctas < 0) return TTS_ERR_INVALID_ARG;
+  // rows of every [*, V] / [*, d] tensor must start 16-byte aligned
+  if ((static_cast<size_t>(cfg->V) * elem_size(cfg->logits_dtype)) % 16 != 0) return TTS_ERR_UNSUPPORTED;
+  if ((static_cast<size_t>(cfg->d) * elem_size(cfg->param_dtype)) % 16 != 0) return TTS_ERR_UNSUPPORTED;
+
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess) return TTS_ERR_CUDA;   // no driver / no device: there is no CPU fallback
+  if (device < 0 || device >= ndev) return TTS_ERR_INVALID_ARG;
+  cudaDeviceProp prop;
+  if ((e = cudaGetDeviceProperties(&prop, device)) != cudaSuccess) return TTS_ERR_CUDA;
+  if (prop.major != 10) return TTS_ERR_ARCH;
+  if ((e = cudaSetDevice(device)) != cudaSuccess) return TTS_ERR_CUDA;
+
+  tts_ctx* c = new (std::nothrow) tts_ctx();
+  if (!c) return TTS_ERR_INVALID_ARG;
+  memset(c, 0, sizeof(*c));
+  c->cfg = *cfg;
+  c->device = device;
+  c->sm_count = prop.multiProcessorCount;
+  c->T_pad_max = (cfg->T_max + 15) / 16 * 16;
+  c->tensor_ok = cfg->kernel_path == TTS_PATH_AUTO && tts::tc_supported(*cfg);
+
+  const size_t V = cfg->V, Tm = cfg->T_max, Tp = c->T_pad_max;
+  bool ok = true;
+  ok = ok && cudaEventCreateWithFlags(&c->done_event, cudaEventDisableTiming) == cudaSuccess;
+  ok = ok && dmalloc(&c->z, Tp * V) == cudaSuccess;
+  if (!c->tensor_ok) ok = ok && dmalloc(&c->dl32, Tm * V) == cudaSuccess;
+  ok = ok && dmalloc(&c->stat_part, Tm * tts::kStatSplitsMax * tts::kStatFields) == cudaSuccess;
+  ok = ok && dmalloc(&c->row_stats, 4 * Tm) == cudaSuccess;
+  ok = ok && dmalloc(&c->arg_val, Tm * tts::kArgSplitsMax) == cudaSuccess;
+  ok = ok && dmalloc(&c->arg_idx, Tm * tts::kArgSplitsMax) == cudaSuccess;
+  ok = ok && dmalloc(&c->argmax_tmp, Tm) == cudaSuccess;
+  // staging for tts_round_host
+  ok = ok && cudaMalloc(&c->st_teacher, Tm * V * elem_size(cfg->logits_dtype)) == cudaSuccess;
+  ok = ok && cudaMalloc(&c->st_h, Tm * cfg->d * elem_size(cfg->param_dtype)) == cudaSuccess;
+  ok = ok && dmalloc(&c->st_tok, Tm) == cudaSuccess;
+  ok = ok && dmalloc(&c->st_pw, Tm) == cudaSuccess;
+  ok = ok && dmalloc(&c->st_mask, Tm) == cudaSuccess;
+  ok = ok && dmalloc(&c->st_tau, Tm / cfg->seg_len) == cudaSuccess;
+  ok = ok && dmalloc(&c->st_loss, 1) == cudaSuccess;
+  if (ok && c->tensor_ok) ok = tts::tc_init(c) == cudaSuccess;
+  if (!ok) {
+    cudaGetLastError();
+    free_all(c);
+    delete c;
+    return TTS_ERR_CUDA;
+  }
+  *out = c;
+  return TTS_OK;
+}
+
+int32_t tts_ctx_destroy(tts_ctx* c) {
+  if (!c) return TTS_ERR_INVALID_ARG;
+  cudaSetDevice(c->device);
+  cudaDeviceSynchronize();
+  free_all(c);
+  delete c;
+  return TTS_OK;
+}
+
+int32_t tts_set_lr(tts_ctx* c, float lr) {
+  if (!c || !(lr >= 0.f)) return TTS_ERR_INVALID_ARG;
+  c->cfg.lr = lr;
+  return TTS_OK;
+}
+
+int32_t tts_set_step_count(tts_ctx* c, int64_t n) {
+  if (!c || n < 0) return TTS_ERR_INVALID_ARG;
+  c->step_count = n;
+  return TTS_OK;
+}
+
+int64_t tts_get_step_count(const tts_ctx* c) { return c ? c->step_count : -1; }
+int32_t tts_last_cuda_error(const tts_ctx* c) { return c ? c->last_cuda_error : 0; }
+int32_t tts_last_step_used_tensor_path(const tts_ctx* c) { return c ? c->last_used_tensor : 0; }
+int32_t tts_last_launch_count(const tts_ctx* c) { return c ? c->last_launches : 0; }
+
+int32_t tts_accept_mask(tts_ctx* c, const void* teacher, const int32_t* tok, int32_t T, uint8_t* mask_out,
+                        int32_t* tau_out, int32_t* am_out, void* stream) {
+  if (!c || !teacher || !tok || !mask_out || !tau_out) return TTS_ERR_INVALID_ARG;
+  if (T <= 0 || T > c->cfg.T_max || T % c->cfg.seg_len != 0) return TTS_ERR_INVALID_ARG;
+  if (!aligned16(teacher)) return TTS_ERR_INVALID_ARG;
+  int launches = 0;
+  cudaError_t e = tts::launch_accept_mask(c, teacher, tok, T, mask_out, tau_out, am_out,
+                                          static_cast<cudaStream_t>(stream), &launches);
+  c->last_launches = launches;
+  if (e != cudaSuccess) return cuda_fail(c, e);
+  return TTS_OK;
+}
+
+int32_t tts_distill_step(tts_ctx* c, const void* teacher, const void* h, const void* W_in, void* W_out,
+                         float* W_master, float* adam_m, float* adam_v, const float* pos_weight,
+                         const uint8_t* mask, int32_t T, float loss_scale, float* loss_out, float* kl_rows_out,
+                         float* gh_out, float* gW_debug_out, void* side_stream) {
+  if (!c || !teacher || !h || !W_in || !W_out || !pos_weight || !loss_out) return TTS_ERR_INVALID_ARG;
+  const tts_config& cfg = c->cfg;
+  if (T <= 0 || T > cfg.T_max || T % cfg.seg_len != 0) return TTS_ERR_INVALID_ARG;
+  if ((cfg.param_dtype == TTS_BF16) != (W_master != nullptr)) return TTS_ERR_INVALID_ARG;
+  if ((cfg.optimizer == TTS_ADAMW) != (adam_m != nullptr && adam_v != nullptr)) return TTS_ERR_INVALID_ARG;
+  if (cfg.optimizer == TTS_SGD && (adam_m || adam_v)) return TTS_ERR_INVALID_ARG;
+  if (cfg.mask_mode != TTS_ROWS_ALL && !mask) return TTS_ERR_INVALID_ARG;
+  if (!aligned16(teacher) || !aligned16(h) || !aligned16(W_in) || !aligned16(W_out) || !aligned16(W_master) ||
+      !aligned16(adam_m) || !aligned16(adam_v) || !aligned16(gh_out) || !aligned16(gW_debug_out))
+    return TTS_ERR_INVALID_ARG;
+
+  cudaStream_t s = static_cast<cudaStream_t>(side_stream);
+  c->step_count += 1;
+  const double n = static_cast<double>(c->step_count);
+  tts::StepArgs a;
+  a.teacher = teacher; a.h = h; a.W_in = W_in; a.W_out = W_out;
+  a.master = W_master; a.adam_m = adam_m; a.adam_v = adam_v;
+  a.pos_weight = pos_weight; a.mask = mask; a.T = T; a.loss_scale = loss_scale;
+  a.loss_out = loss_out; a.kl_rows_out = kl_rows_out; a.gh_out = gh_out; a.gW_debug = gW_debug_out;
+  a.lr = cfg.lr; a.beta1 = cfg.beta1; a.beta2 = cfg.beta2; a.eps = cfg.eps; a.wd = cfg.weight_decay;
+  a.inv_bc1 = static_cast<float>(1.0 / (1.0 - pow(static_cast<double>(cfg.beta1), n)));
+  a.inv_sqrt_bc2 = static_cast<float>(1.0 / sqrt(1.0 - pow(static_cast<double>(cfg.beta2), n)));
+
+  int launches = 0;
+  cudaError_t e;
+  tts::prof_mark(c, -1, s);
+  if (c->tensor_ok) {
+    c->last_used_tensor = 1;
+    e = tts::tc_step(c, a, s, &launches);
+  } else {
+    c->last_used_tensor = 0;
+    e = tts::simt_step(c, a, s, &launches);
+  }
+  c->last_launches = launches;
+  if (e != cudaSuccess) return cuda_fail(c, e);
+  if (c->prof_on) c->prof_count += 1;
+  if ((e = cudaEventRecord(c->done_event, s)) != cudaSuccess) return cuda_fail(c, e);
+  c->done_recorded = true;
+  return TTS_OK;
+}
+
+int32_t tts_profile_enable(tts_ctx* c, int32_t enable) {
+  if (!c) return TTS_ERR_INVALID_ARG;
+  if (enable && !c->prof_events) {
+    const int n = tts::kProfSlots * (TTS_NUM_PHASES + 1);
+    c->prof_events = static_cast<cudaEvent_t*>(calloc(n, sizeof(cudaEvent_t)));
+    if (!c->prof_events) return TTS_ERR_INVALID_ARG;
+    for (int i = 0; i < n; ++i) {
+      cudaError_t e = cudaEventCreate(&c->prof_events[i]);
+      if (e != cudaSuccess) return cuda_fail(c, e);
+    }
+  }
+  c->prof_on = enable != 0;
+  c->prof_count = 0;
+  return TTS_OK;
+}
+
+int32_t tts_profile_read(tts_ctx* c, float* ms_out, int32_t* n_steps_out) {
+  if (!c || !ms_out) return TTS_ERR_INVALID_ARG;
+  for (int p = 0; p < TTS_NUM_PHASES; ++p) ms_out[p] = 0.f;
+  const int n = c->prof_count < tts::kProfSlots ? c->prof_count : tts::kProfSlots;
+  if (n_steps_out) *n_steps_out = n;
+  if (n == 0 || !c->prof_events) return TTS_OK;
+  if (c->done_recorded) {
+    cudaError_t e = cudaEventSynchronize(c->done_event);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+  }
+  for (int i = 0; i < n; ++i) {
+    const cudaEvent_t* ev = c->prof_events + i * (TTS_NUM_PHASES + 1);
+    for (int p = 0; p < TTS_NUM_PHASES; ++p) {
+      float ms = 0.f;
+      cudaError_t e = cudaEventElapsedTime(&ms, ev[p], ev[p + 1]);
+      if (e != cudaSuccess) return cuda_fail(c, e);
+      ms_out[p] += ms / n;
+    }
+  }
+  c->prof_count = 0;
+  return TTS_OK;
+}
+
+int32_t tts_wait_step(tts_ctx* c, void* main_stream) {
+  if (!c) return TTS_ERR_INVALID_ARG;
+  if (!c->done_recorded) return TTS_OK;
+  cudaError_t e = cudaStreamWaitEvent(static_cast<cudaStream_t>(main_stream), c->done_event, 0);
+  return e == cudaSuccess ? TTS_OK : cuda_fail(c, e);
+}
+
+int32_t tts_sync_step(tts_ctx* c) {
+  if (!c) return TTS_ERR_INVALID_ARG;
+  if (!c->done_recorded) return TTS_OK;
+  cudaError_t e = cudaEventSynchronize(c->done_event);
+  return e == cudaSuccess ? TTS_OK : cuda_fail(c, e);
+}
+
+int32_t tts_round_host(tts_ctx* c, const void* teacher_host, const void* h_host, const int32_t* tok_host,
+                       const float* pw_host, int32_t T, float loss_scale, const void* W_in, void* W_out,
+                       float* W_master, float* adam_m, float* adam_v, float* gh_dev, float* loss_host,
+                       int32_t* tau_host, uint8_t* mask_host, void* stream) {
+  if (!c || !teacher_host || !h_host || !tok_host || !pw_host || !loss_host || !tau_host) return TTS_ERR_INVALID_ARG;
+  const tts_config& cfg = c->cfg;
+  if (T <= 0 || T > cfg.T_max || T % cfg.seg_len != 0) return TTS_ERR_INVALID_ARG;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const size_t V = cfg.V, d = cfg.d;
+  cudaError_t e;
+  if ((e = cudaMemcpyAsync(c->st_teacher, teacher_host, (size_t)T * V * elem_size(cfg.logits_dtype),
+                           cudaMemcpyHostToDevice, s)) != cudaSuccess) return cuda_fail(c, e);
+  if ((e = cudaMemcpyAsync(c->st_h, h_host, (size_t)T * d * elem_size(cfg.param_dtype),
+                           cudaMemcpyHostToDevice, s)) != cudaSuccess) return cuda_fail(c, e);
+  if ((e = cudaMemcpyAsync(c->st_tok, tok_host, (size_t)T * 4, cudaMemcpyHostToDevice, s)) != cudaSuccess)
+    return cuda_fail(c, e);
+  if ((e = cudaMemcpyAsync(c->st_pw, pw_host, (size_t)T * 4, cudaMemcpyHostToDevice, s)) != cudaSuccess)
+    return cuda_fail(c, e);
+  int32_t st = tts_accept_mask(c, c->st_teacher, c->st_tok, T, c->st_mask, c->st_tau, nullptr, stream);
+  if (st != TTS_OK) return st;
+  const int mask_launches = c->last_launches;
+  st = tts_distill_step(c, c->st_teacher, c->st_h, W_in, W_out, W_master, adam_m, adam_v, c->st_pw, c->st_mask, T,
+                        loss_scale, c->st_loss, nullptr, gh_dev, nullptr, stream);
+  if (st != TTS_OK) return st;
+  c->last_launches += mask_launches;
+  if ((e = cudaMemcpyAsync(loss_host, c->st_loss, 4, cudaMemcpyDeviceToHost, s)) != cudaSuccess) return cuda_fail(c, e);
+  if ((e = cudaMemcpyAsync(tau_host, c->st_tau, (size_t)(T / cfg.seg_len) * 4, cudaMemcpyDeviceToHost, s)) !=
+      cudaSuccess)
+    return cuda_fail(c, e);
+  if (mask_host &&
+      (e = cudaMemcpyAsync(mask_host, c->st_mask, (size_t)T, cudaMemcpyDeviceToHost, s)) != cudaSuccess)
+    return cuda_fail(c, e);
+  if ((e = cudaStreamSynchronize(s)) != cudaSuccess) return cuda_fail(c, e);
+  return TTS_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,102 @@
+// Internal declarations shared by the translation units of libtts_b200.so.
+// Not part of the ABI (include/tts.h is).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+#include <stdint.h>
+
+#include "../../include/tts.h"
+
+namespace tts {
+
+constexpr int kStatSplitsMax = 64;   // V-splits per row in the row-statistics sweep
+constexpr int kArgSplitsMax = 64;    // V-splits per row in the argmax sweep
+constexpr int kStatFields = 5;       // (m_t, s_t, a, m_z, s_z), SURVEY §8(a) a3
+constexpr int kProfSlots = 256;      // profiled steps kept between two tts_profile_read calls
+constexpr int kKPad = 64;            // K extent (bf16 elements) of one 128-byte swizzle atom
+
+struct StepArgs {
+  const void* teacher;
+  const void* h;
+  const void* W_in;
+  void* W_out;
+  float* master;
+  float* adam_m;
+  float* adam_v;
+  const float* pos_weight;
+  const uint8_t* mask;
+  int T;
+  float loss_scale;
+  float* loss_out;
+  float* kl_rows_out;
+  float* gh_out;
+  float* gW_debug;
+  // optimiser scalars for this step (bias corrections precomputed on the host in fp64)
+  float lr, beta1, beta2, eps, wd;
+  float inv_bc1;       // 1 / (1 - beta1^n)
+  float inv_sqrt_bc2;  // 1 / sqrt(1 - beta2^n)
+};
+
+}  // namespace tts
+
+struct tts_ctx {
+  tts_config cfg;
+  int device;
+  int sm_count;
+  int64_t step_count;
+  int last_cuda_error;
+  int last_used_tensor;
+  int last_launches;
+  int T_pad_max;          // T_max rounded up to 16
+  bool tensor_ok;         // shape/dtype qualifies for the tcgen05 kernels
+  cudaEvent_t done_event;
+  bool done_recorded;
+  // ---- scratch (device) ----
+  float* z;               // [T_pad_max, V] draft logits (fp32)
+  float* dl32;            // [T_max, V] fp32 dlogits                (CUDA-core path)
+  float* stat_part;       // [T_max, kStatSplitsMax, 5]
+  float* row_stats;       // [4, T_max]: lse_t, lse_z, kl, coef (= loss_scale * omega)
+  float* arg_val;         // [T_max, kArgSplitsMax]
+  int32_t* arg_idx;       // [T_max, kArgSplitsMax]
+  int32_t* argmax_tmp;    // [T_max]
+  // ---- staging for tts_round_host ----
+  void* st_teacher;
+  void* st_h;
+  int32_t* st_tok;
+  float* st_pw;
+  uint8_t* st_mask;
+  int32_t* st_tau;
+  float* st_loss;
+  // ---- per-phase profiling (tts_profile_*) ----
+  bool prof_on;
+  int prof_count;                                   // steps recorded since the last read
+  cudaEvent_t* prof_events;                         // [kProfSlots][TTS_NUM_PHASES + 1], created lazily
+  // ---- tensor-path state (opaque, owned by tts_tc.cu) ----
+  void* tc_state;
+};
+
+namespace tts {
+
+// Phase boundary: records the profiling event that ENDS phase `phase` (phase = -1: step start).
+inline void prof_mark(tts_ctx* c, int phase, cudaStream_t s) {
+  if (!c->prof_on || !c->prof_events) return;
+  const int slot = c->prof_count % kProfSlots;
+  cudaEventRecord(c->prof_events[slot * (TTS_NUM_PHASES + 1) + phase + 1], s);
+}
+
+// tts_mask.cu
+cudaError_t launch_accept_mask(tts_ctx* c, const void* teacher, const int32_t* tok, int T, uint8_t* mask,
+                               int32_t* tau, int32_t* am_out, cudaStream_t s, int* launches);
+// tts_stats.cu: row statistics + merge + loss (CUDA-core sweeps shared by both paths).
+// z_ld = leading dimension (row stride in floats) of the z scratch.
+cudaError_t launch_row_stats(tts_ctx* c, const StepArgs& a, int z_ld, cudaStream_t s, int* launches);
+// tts_simt.cu
+cudaError_t simt_step(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches);
+// tts_tc.cu
+bool tc_supported(const tts_config& cfg);
+cudaError_t tc_init(tts_ctx* c);
+void tc_destroy(tts_ctx* c);
+cudaError_t tc_step(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches);
+
+}  // namespace tts

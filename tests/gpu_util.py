@@ -1,0 +1,140 @@
+"""Helpers for the GPU parity tests: run the CUDA path (through the C ABI binding) on a seeded
+synthetic case and return numpy arrays; run the fp64 oracle on the same arrays.  Test
+infrastructure only."""
+from __future__ import annotations
+
+import numpy as np
+import torch
+
+from oracle import tts_oracle as O
+from paper_2605_09329_b200 import synth, tts
+
+
+def _dev(a, dtype=None):
+    """numpy -> cuda tensor; uint16 arrays are bf16 bit patterns."""
+    if a is None:
+        return None
+    if a.dtype == np.uint16:
+        return torch.from_numpy(a.view(np.int16).copy()).cuda().view(torch.bfloat16)
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def bits(t: torch.Tensor) -> np.ndarray:
+    """bf16 cuda tensor -> uint16 bit patterns."""
+    return t.view(torch.int16).cpu().numpy().view(np.uint16)
+
+
+def config_for(case, *, mask_mode=tts.TTS_ROWS_ALL, kernel_path=tts.TTS_PATH_AUTO, T_max=None, max_ctas=0):
+    c = case["cfg"]
+    return tts.make_config(case["V"], case["d"], T_max or case["T"], case["seg_len"], c["param"], c["logits"],
+                           c["optimizer"], c["lr"], c["beta1"], c["beta2"], c["eps"], c["weight_decay"], mask_mode,
+                           max_ctas, kernel_path)
+
+
+def run_gpu(case, *, mask_mode=tts.TTS_ROWS_ALL, kernel_path=tts.TTS_PATH_AUTO, want_gW=True, want_gh=True,
+            alias_w=False, side_stream=True, max_ctas=0):
+    """One tts_accept_mask + tts_distill_step on cuda:0.  Returns a dict of numpy results."""
+    T, V, d = case["T"], case["V"], case["d"]
+    bf = case["cfg"]["param"] == synth.BF16
+    ctx = tts.tts_ctx_create(config_for(case, mask_mode=mask_mode, kernel_path=kernel_path, max_ctas=max_ctas), 0)
+    try:
+        if case.get("step", 1) > 1:
+            tts.tts_set_step_count(ctx, case["step"] - 1)
+        teacher, h, tok = _dev(case["teacher"]), _dev(case["h"]), _dev(case["draft_tokens"])
+        W_in = _dev(case["W"])
+        W_out = W_in if alias_w else torch.empty_like(W_in)
+        master = _dev(case["master"]) if bf else None
+        m, v = _dev(case["m"]), _dev(case["v"])
+        pw = _dev(case["pos_weight"])
+        mask = torch.zeros(T, dtype=torch.uint8, device="cuda")
+        tau = torch.zeros(T // case["seg_len"], dtype=torch.int32, device="cuda")
+        am = torch.zeros(T, dtype=torch.int32, device="cuda")
+        loss = torch.zeros(1, dtype=torch.float32, device="cuda")
+        kl = torch.zeros(T, dtype=torch.float32, device="cuda")
+        gh = torch.full((T, d), float("nan"), dtype=torch.float32, device="cuda") if want_gh else None
+        gW = torch.full((V, d), float("nan"), dtype=torch.float32, device="cuda") if want_gW else None
+        torch.cuda.synchronize()
+        s = torch.cuda.Stream() if side_stream else torch.cuda.current_stream()
+        tts.tts_accept_mask(ctx, teacher, tok, T, mask, tau, am, s)
+        mask_launches = tts.tts_last_launch_count(ctx)
+        tts.tts_distill_step(ctx, teacher, h, W_in, W_out, master, m, v, pw, mask, T, case["loss_scale"], loss, kl,
+                             gh, gW, s)
+        step_launches = tts.tts_last_launch_count(ctx)
+        tts.tts_wait_step(ctx, torch.cuda.current_stream())
+        tts.tts_sync_step(ctx)
+        torch.cuda.synchronize()
+        out = dict(mask=mask.cpu().numpy(), tau=tau.cpu().numpy(), argmax=am.cpu().numpy(),
+                   loss=float(loss.item()), kl_rows=kl.cpu().numpy(),
+                   gh=gh.cpu().numpy() if want_gh else None, gW=gW.cpu().numpy() if want_gW else None,
+                   used_tensor=tts.tts_last_step_used_tensor_path(ctx), step_count=tts.tts_get_step_count(ctx),
+                   launches=mask_launches + step_launches)
+        if bf:
+            out["master"] = master.cpu().numpy()
+            out["W_out"] = bits(W_out)
+        else:
+            out["master"] = W_out.cpu().numpy()
+            out["W_out"] = out["master"]
+        out["m"] = m.cpu().numpy() if m is not None else None
+        out["v"] = v.cpu().numpy() if v is not None else None
+        return out
+    finally:
+        tts.tts_ctx_destroy(ctx)
+
+
+def run_oracle(case, *, mask_mode=O.ROWS_ALL):
+    c = case["cfg"]
+    mask, tau, am = O.accept_mask(case["teacher"], case["draft_tokens"], case["seg_len"])
+    r = O.distill_step(case["teacher"], case["h"], case["W"], case["master"], case["m"], case["v"],
+                       case["pos_weight"], mask, seg_len=case["seg_len"], mask_mode=mask_mode,
+                       loss_scale=case["loss_scale"], optimizer="sgd" if c["optimizer"] == synth.SGD else "adamw",
+                       lr=c["lr"], beta1=c["beta1"], beta2=c["beta2"], eps=c["eps"], weight_decay=c["weight_decay"],
+                       step=case.get("step", 1))
+    r.update(mask=mask, tau=tau, argmax=am)
+    return r
+
+
+def max_abs(x):
+    return float(np.max(np.abs(x))) if x.size else 0.0
+
+
+def check_step(g, o, case, *, fp32=False):
+    """Element-by-element comparison with the tolerances of BASELINE.json north_star (bf16 inputs,
+    fp32 accumulation: loss rel <= 1e-3, gW / gh / weights max abs err <= 2e-3 * max|ref|) or, for the
+    fp32 configuration, R21 (1e-5).  Mask, tau and argmax are bit-exact."""
+    c = case["cfg"]
+    np.testing.assert_array_equal(g["mask"], o["mask"])
+    np.testing.assert_array_equal(g["tau"], o["tau"])
+    np.testing.assert_array_equal(g["argmax"], o["argmax"])
+    rel, aabs, tol = (1e-5, 1e-9, 1e-5) if fp32 else (1e-3, 1e-6, 2e-3)
+    assert abs(g["loss"] - o["loss"]) <= rel * abs(o["loss"]) + aabs, (g["loss"], o["loss"])
+    klt = rel * np.abs(o["kl_rows"]) + max(aabs, 1e-6 if not fp32 else 1e-7) * 10
+    assert np.all(np.abs(g["kl_rows"] - o["kl_rows"]) <= klt), (g["kl_rows"], o["kl_rows"])
+    for name in ("gW", "gh", "master", "m", "v"):
+        if g.get(name) is None or o.get(name) is None:
+            continue
+        ref = o[name]
+        err = max_abs(g[name].astype(np.float64) - ref)
+        assert np.all(np.isfinite(g[name])), name
+        assert err <= tol * max_abs(ref) + 1e-30, (name, err, max_abs(ref))
+    # the update itself (R13): Delta M on elements with a sizeable gradient, and its sign everywhere
+    M_old = O.widen(case["master"]) if case["master"] is not None else O.widen(case["W"])
+    d_ref = o["master"] - M_old
+    d_gpu = g["master"].astype(np.float64) - M_old
+    lr = c["lr"]
+    if c["optimizer"] == synth.ADAMW:
+        big = np.abs(o["gW"]) >= 1e-2 * max_abs(o["gW"])
+        if big.any():
+            # fp32 master: one ulp of |M| ~ 0.1 is 7.5e-9, comparable to lr = 1e-5 * 0.02
+            ulp = np.spacing(np.abs(M_old[big]).astype(np.float32)).astype(np.float64)
+            assert np.all(np.abs(d_gpu[big] - d_ref[big]) <= 0.02 * lr + ulp)
+        moved = np.abs(d_ref) > 4 * np.spacing(np.abs(M_old).astype(np.float32)).astype(np.float64)
+        if moved.any():
+            bad = np.sign(d_gpu[moved]) != np.sign(d_ref[moved])
+            assert bad.mean() <= 1e-3, bad.mean()
+    else:
+        assert max_abs(d_gpu - d_ref) <= tol * lr * max_abs(o["gW"]) + float(np.spacing(np.float32(max_abs(M_old))))
+    if case["master"] is not None:
+        # working copy: bit-exactly rn_bf16 of the GPU's own master, and within 1 bf16 ulp of the oracle's (R12)
+        np.testing.assert_array_equal(g["W_out"], O.f32_to_bf16_bits(g["master"]))
+        diff = np.abs(g["W_out"].astype(np.int32) - o["W_out"].astype(np.int32))
+        assert diff.max() <= 1
