@@ -1,0 +1,361 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the TTS online-distillation step on B200 (one JSON line on stdout).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path over one round of synthetic input:
+tts_accept_mask (a1) + tts_distill_step (a2-a7) enqueued on a side stream, then the barrier (a8).
+Default workload: BASELINE.json configs[2], the Qwen3-8B-shaped draft head (V=151936, d=4096, T=16,
+bf16 weights + fp32 master, AdamW) -- the configuration the metric's >=70%-of-roofline target is
+quoted on.  Inputs are seeded and synthetic (paper_2605_09329_b200/synth.py).
+
+  value      steps/s with all inputs resident in HBM (CUDA events on the side stream, max over ranks)
+  e2e        the same metric through tts_round_host: the round's teacher logits / hidden states /
+             tokens / weights come from pinned HOST buffers and loss / tau / mask go back to the host
+             inside the timed region
+  roofline   dominant kernel (a6+a7, gW contraction fused with the AdamW update): ALGORITHMIC bytes per
+             launch / mean launch duration (CUDA events recorded on the launching stream by the library's
+             tts_profile_* calls) against MEASURED_PEAKS.json's copy bandwidth
+  cpu_baseline  the fp64 oracle (oracle/tts_oracle.py, as it stands) timed on this box's host cores on a
+             bounded vocabulary sample of the same workload
+
+N > 1: "replicas only": every rank runs an independent replica of the step on its
+own rounds, no data-path collective; value = steps of all ranks / max-over-ranks time.
+--impl reference: the oracle arm (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+FALLBACK_HBM_GBS = 6650.0   # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", type=int, default=3, choices=[2, 3, 4, 5])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--kernel-path", default="auto", choices=["auto", "simt"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--cpu-sample-rows", type=int, default=8192, help="vocabulary rows in the oracle sample")
+    return ap.parse_args()
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            with open(p) as f:
+                j = json.load(f)
+            return float(j["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def algorithmic_bytes(V, d, T, adam=True):
+    """SURVEY.md 8(d) / DESIGN.md "Algorithmic bytes": what the method must move per step."""
+    state = 12 if adam else 4                      # fp32 master (+ m, v)
+    step = V * d * (2 + state + state + 2)         # bf16 W read once, state read+written once, bf16 W written once
+    step += T * V * 2 + T * d * 2 + T * d * 4      # teacher logits, h, gh
+    update_kernel = V * d * (state + state + 2) + T * V * 2 + T * d * 2   # a6+a7 launch alone
+    return step, update_kernel
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clocks and throttle reasons with NVML while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.max_mhz = index, [], set(), None
+        self._stop_evt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception:
+            pass
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+                 nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap",
+                 nv.nvmlClocksThrottleReasonHwPowerBrakeSlowdown: "hw_power_brake"}
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._stop_evt.wait(0.02)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=2.0)
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2] if s else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(s)}
+
+
+def _np_bits(t):
+    """bf16 torch tensor -> uint16 numpy bit patterns (what the oracle consumes)."""
+    import numpy as np
+    import torch
+    return t.contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
+
+
+def host_sample(case, rows):
+    """The first ``rows`` vocabulary rows of a device case, as the oracle's numpy inputs."""
+    Vs = min(rows, case["V"])
+    return dict(teacher=_np_bits(case["teacher"][:, :Vs]), h=_np_bits(case["h"]), W=_np_bits(case["W"][:Vs]),
+                master=case["master"][:Vs].cpu().numpy(), m=case["m"][:Vs].cpu().numpy(),
+                v=case["v"][:Vs].cpu().numpy(), tok=case["draft_tokens"].cpu().numpy(),
+                pw=case["pos_weight"].cpu().numpy(), Vs=Vs)
+
+
+def time_oracle(case, sample, repeats=1):
+    """One oracle step (mask + loss + gradients + AdamW, fp64) on the vocabulary sample.  Returns seconds."""
+    from oracle import tts_oracle as O
+    c = case["cfg"]
+    best = None
+    for _ in range(repeats):
+        t0 = time.perf_counter()
+        mask, tau, am = O.accept_mask(sample["teacher"], sample["tok"], case["seg_len"])
+        O.distill_step(sample["teacher"], sample["h"], sample["W"], sample["master"], sample["m"], sample["v"],
+                       sample["pw"], mask, seg_len=case["seg_len"], loss_scale=case["loss_scale"],
+                       optimizer="adamw", lr=c["lr"], beta1=c["beta1"], beta2=c["beta2"], eps=c["eps"],
+                       weight_decay=c["weight_decay"], step=1)
+        dt = time.perf_counter() - t0
+        best = dt if best is None else min(best, dt)
+    return best
+
+
+def cpu_threads():
+    try:
+        from threadpoolctl import threadpool_info
+        n = max([p.get("num_threads", 1) for p in threadpool_info()] or [1])
+    except Exception:
+        n = 1
+    return max(1, min(n, len(os.sched_getaffinity(0))))   # BLAS threads the matmuls use; elementwise numpy is 1 thread
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the oracle as it stands on the host cores (rank 0 only)."""
+    if rank != 0:
+        return
+    import numpy as np
+    from paper_2605_09329_b200 import synth
+    cfgc = synth.CONFIGS[args.config]
+    V, d = cfgc["V"], cfgc["d"]
+    rows = min(args.cpu_sample_rows, 4096)   # ~1.5 s of oracle work per step
+    # the sample is a scaled-down draw of the same recipe (same d, T; first `rows` of the vocabulary)
+    case = synth.make_case(args.config, V=rows, n_seq=min(cfgc["n_seq"], 2) if args.config == 4 else None)
+    sample = dict(teacher=case["teacher"], h=case["h"], W=case["W"], master=case["master"], m=case["m"],
+                  v=case["v"], tok=case["draft_tokens"], pw=case["pos_weight"], Vs=rows)
+    for _ in range(args.warmup):
+        time_oracle(case, sample)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        time_oracle(case, sample)
+    dt = (time.perf_counter() - t0) / args.steps
+    scale = (V / rows) * (cfgc["n_seq"] * cfgc["seg_len"] / case["T"])
+    sps = 1.0 / (dt * scale)
+    cores = cpu_threads()
+    what = "vocabulary rows 0..%d of %d (full d=%d, T=%d of %d), time scaled by %.1f" % (
+        rows, V, d, case["T"], cfgc["n_seq"] * cfgc["seg_len"], scale)
+    line = {"impl": "reference", "metric": "distill_steps_per_sec", "value": sps, "unit": "steps/s",
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 / sps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": workload_config(args.config, world, "oracle-cpu"),
+            "cpu_baseline": {"value": sps, "unit": "steps/s", "cores": cores, "kind": "oracle", "sample": what},
+            "e2e": {"value": sps, "unit": "steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(cfg_id, world, path):
+    from paper_2605_09329_b200 import synth
+    c = synth.CONFIGS[cfg_id]
+    return {"workload": "BASELINE.json configs[%d] %s: V=%d d=%d T=%d (seg_len %d x %d seq), bf16 W + fp32 master, "
+                        "AdamW lr=1e-5" % (cfg_id - 1, c["name"], c["V"], c["d"], c["seg_len"] * c["n_seq"],
+                                           c["seg_len"], c["n_seq"]),
+            "V": c["V"], "d": c["d"], "T": c["seg_len"] * c["n_seq"], "optimizer": "adamw",
+            "parallelism": "replicas x%d (no data-path collective)" % world if world > 1 else "single GPU",
+            "kernel_path": path,
+            "l2": "working set per step (17 GB of weight state) exceeds the 126 MB L2: every step is L2-cold"}
+
+
+def run_ours(args, rank, world, local_rank):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2605_09329_b200 import synth, tts
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the distillation step has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = "cuda:%d" % local_rank
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    case = synth.make_case_device(args.config, dev, seed_offset=rank)
+    c = case["cfg"]
+    V, d, T, C = case["V"], case["d"], case["T"], case["seg_len"]
+    kpath = tts.TTS_PATH_AUTO if args.kernel_path == "auto" else tts.TTS_PATH_SIMT
+    cfg = tts.make_config(V, d, T, C, tts.TTS_BF16, tts.TTS_BF16, tts.TTS_ADAMW, c["lr"], c["beta1"], c["beta2"],
+                          c["eps"], c["weight_decay"], tts.TTS_ROWS_ALL, 0, kpath)
+    ctx = tts.tts_ctx_create(cfg, local_rank)
+    W = [case["W"], torch.empty_like(case["W"])]        # W_in / W_out double buffer, swapped at the barrier (R18)
+    master, m, v = case["master"], case["m"], case["v"]
+    teacher, h, tok, pw = case["teacher"], case["h"], case["draft_tokens"], case["pos_weight"]
+    mask = torch.zeros(T, dtype=torch.uint8, device=dev)
+    tau = torch.zeros(T // C, dtype=torch.int32, device=dev)
+    loss = torch.zeros(1, dtype=torch.float32, device=dev)
+    gh = torch.zeros(T, d, dtype=torch.float32, device=dev)
+    side = torch.cuda.Stream(device=dev)
+    main = torch.cuda.current_stream()
+    launches = [0]
+    cur = [0]
+
+    def step():
+        tts.tts_accept_mask(ctx, teacher, tok, T, mask, tau, None, side)
+        n = tts.tts_last_launch_count(ctx)
+        tts.tts_distill_step(ctx, teacher, h, W[cur[0]], W[1 - cur[0]], master, m, v, pw, mask, T,
+                             case["loss_scale"], loss, None, gh, None, side)
+        launches[0] += n + tts.tts_last_launch_count(ctx)
+        tts.tts_wait_step(ctx, main)      # the paper's barrier before the next draft round
+        cur[0] ^= 1
+
+    side.wait_stream(main)
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    used_tensor = tts.tts_last_step_used_tensor_path(ctx)
+    tts.tts_profile_enable(ctx, 1)
+    launches[0] = 0
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(side)
+    for _ in range(args.steps):
+        step()
+    e1.record(side)
+    barrier()
+    clocks = sampler.stop()
+    ms_total = e0.elapsed_time(e1)
+    phase_ms, n_prof = tts.tts_profile_read(ctx)
+    tts.tts_profile_enable(ctx, 0)
+    loss_val = float(loss.item())
+    tmax = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    ms_total = float(tmax.item())
+
+    # ---- end to end through HOST buffers: tts_round_host (H2D of the round's inputs, D2H of loss/tau/mask) ----
+    e2e = None
+    if not args.no_e2e:
+        ht = teacher.view(torch.int16).cpu().pin_memory()
+        hh = h.view(torch.int16).cpu().pin_memory()
+        htok, hpw = tok.cpu().pin_memory(), pw.cpu().pin_memory()
+        hloss = torch.zeros(1).pin_memory()
+        htau = torch.zeros(T // C, dtype=torch.int32).pin_memory()
+        hmask = torch.zeros(T, dtype=torch.uint8).pin_memory()
+
+        def round_host():
+            tts.tts_round_host(ctx, ht, hh, htok, hpw, T, case["loss_scale"], W[cur[0]], W[1 - cur[0]], master, m, v,
+                               gh, hloss, htau, hmask, side)
+            cur[0] ^= 1
+
+        for _ in range(max(3, args.warmup // 2)):
+            round_host()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            round_host()
+        barrier()
+        dt = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(dt, op=dist.ReduceOp.MAX)
+        e2e = {"value": world * args.steps / float(dt.item()), "unit": "steps/s",
+               "h2d_bytes_per_step": int(ht.numel() * 2 + hh.numel() * 2 + htok.numel() * 4 + hpw.numel() * 4),
+               "d2h_bytes_per_step": int(4 + htau.numel() * 4 + hmask.numel()),
+               "timing": "host clock around K tts_round_host calls (each ends with a stream synchronise)"}
+
+    # ---- CPU baseline: the oracle on a bounded vocabulary sample, rank 0 at N=1 only ----
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        sample = host_sample(case, args.cpu_sample_rows if T <= 64 else max(512, args.cpu_sample_rows // 8))
+        time_oracle(case, sample)
+        sec = time_oracle(case, sample, repeats=2)
+        scale = V / sample["Vs"]
+        cpu = {"value": 1.0 / (sec * scale), "unit": "steps/s", "cores": cpu_threads(), "kind": "oracle",
+               "sample": "vocabulary rows 0..%d of %d (full d=%d, T=%d): %.2f s, scaled by %.1f to the full step"
+                         % (sample["Vs"], V, d, T, sec, scale)}
+
+    tts.tts_ctx_destroy(ctx)
+    if rank != 0:
+        return
+    ms_step = ms_total / args.steps
+    sps = world * 1e3 / ms_step
+    step_bytes, upd_bytes = algorithmic_bytes(V, d, T)
+    peak, peak_src = measured_peaks()
+    upd_ms = phase_ms[4] if n_prof > 0 and phase_ms[4] > 0 else None
+    roof = {"bound": "hbm", "kernel": "a6+a7 gW contraction fused with AdamW update (phase 4)",
+            "achieved": (upd_bytes / (upd_ms * 1e-3) / 1e9) if upd_ms else None, "peak": peak, "unit": "GB/s",
+            "frac": (upd_bytes / (upd_ms * 1e-3) / 1e9 / peak) if upd_ms else None, "traffic": None,
+            "peak_source": peak_src, "algorithmic_bytes_per_launch": upd_bytes, "kernel_ms": upd_ms,
+            "step_algorithmic_bytes": step_bytes, "step_achieved": step_bytes / (ms_step * 1e-3) / 1e9,
+            "step_frac_of_measured_copy": step_bytes / (ms_step * 1e-3) / 1e9 / peak,
+            "step_frac_of_nominal_8TBs": step_bytes / (ms_step * 1e-3) / 1e9 / 8000.0,
+            "phase_ms": dict(zip(tts.PHASE_NAMES, phase_ms)), "profiled_steps": n_prof}
+    line = {"metric": "distill_steps_per_sec", "value": sps, "unit": "steps/s", "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+            "config": workload_config(args.config, world, "tcgen05+tma" if used_tensor else "cuda-core"),
+            "rows_V_per_sec": sps * T * V, "loss": loss_val, "clocks": clocks, "e2e": e2e,
+            "gpu_launches": launches[0], "roofline": roof, "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    args = parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

@@ -223,3 +223,68 @@ def planted_mask_cases(V: int, seg_len: int, seed: int = 11, dtype=BF16):
     expect_tau.append(1 if seg_len > 1 else 1)
     out_t = f32_to_bf16_bits(t) if dtype == BF16 else t
     return out_t, tok, np.array(expect_tau, dtype=np.int32)
+
+
+# ----------------------------------------------------------------------------
+# Full-size cases built ON THE DEVICE (bench.py and the full-size parity tests).
+# Same recipe as make_case, with torch's seeded device generator in place of numpy's
+# (the full-size host recipe needs minutes and ~10 GB of host memory per case).  Only
+# random draws, the draft-logit product the recipe needs, bf16 rounding, argmax for the
+# canvas tokens and the prefix planting: none of the method's arithmetic.
+# ----------------------------------------------------------------------------
+
+def make_case_device(cfg_id: int, device="cuda:0", *, seed_offset: int = 0, n_seq: int | None = None,
+                     V: int | None = None, d: int | None = None):
+    """Returns a dict of torch tensors on ``device``: teacher [T,V], h [T,d], W [V,d] (bf16),
+    master/m/v [V,d] fp32, draft_tokens [T] i32, pos_weight [T] f32, plus cfg, tau_star (host
+    numpy) and loss_scale.  ``seed_offset`` gives independent replicas (multi-GPU ranks)."""
+    import torch
+
+    c = dict(CONFIGS[cfg_id])
+    c.update(ADAM_DEFAULTS)
+    if n_seq is not None: c["n_seq"] = n_seq
+    if V is not None: c["V"] = V
+    if d is not None: c["d"] = d
+    V, d, C, S = c["V"], c["d"], c["seg_len"], c["n_seq"]
+    T = C * S
+    c["T"] = T
+    assert c["param"] == BF16 and c["logits"] == BF16
+    dev = torch.device(device)
+    g = torch.Generator(device=dev)
+    g.manual_seed(1000003 * (c["seed"] + 1) + seed_offset)
+    rng = np.random.Generator(np.random.PCG64(c["seed"] + 7919 * seed_offset))
+
+    master = torch.empty((V, d), dtype=torch.float32, device=dev)
+    master.normal_(0.0, 0.02, generator=g)
+    W = master.to(torch.bfloat16)
+    h = torch.empty((T, d), dtype=torch.float32, device=dev).normal_(0.0, 1.0, generator=g).to(torch.bfloat16)
+    z = (h.float() @ W.float().T) if T * V <= (1 << 24) else torch.cat(
+        [h[i:i + 64].float() @ W.float().T for i in range(0, T, 64)], 0)
+    kind = c["sigma"]
+    if kind[0] == "const":
+        sig = np.full(T, kind[1], dtype=np.float32)
+    else:
+        sig = rng.uniform(kind[1], kind[2], size=T).astype(np.float32)
+    noise = torch.empty((T, V), dtype=torch.float32, device=dev).normal_(0.0, 1.0, generator=g)
+    t = z + torch.from_numpy(sig).to(dev)[:, None] * noise
+    del noise
+    tok = torch.argmax(z, dim=1).to(torch.int32)
+    tau_star = None
+    if c["plant"]:
+        tau_star = np.minimum(rng.geometric(0.4, size=S), C).astype(np.int32)
+        rmax = t.max(dim=1).values
+        for s in range(S):
+            for k in range(C):
+                r = s * C + k
+                if k < tau_star[s]:
+                    t[r, tok[r]] = rmax[r] + 1.0
+                elif k == tau_star[s]:
+                    if int(torch.argmax(t[r])) == int(tok[r]):
+                        t[r, tok[r]] = torch.topk(t[r], 2).values[1] - 1.0
+    teacher = t.to(torch.bfloat16)
+    del t, z
+    pw = torch.from_numpy(position_weights(c["weights"], C, S)).to(dev)
+    out = dict(cfg=c, V=V, d=d, T=T, seg_len=C, tau_star=tau_star, teacher=teacher, h=h, W=W, master=master,
+               m=torch.zeros_like(master), v=torch.zeros_like(master), draft_tokens=tok, pos_weight=pw,
+               loss_scale=float(c["loss_scale"]), step=1)
+    return out
