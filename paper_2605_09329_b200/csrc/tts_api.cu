@@ -93,7 +93,7 @@ int32_t tts_ctx_create(const tts_config* cfg, int32_t device, tts_ctx** out) {
   bool ok = true;
   ok = ok && cudaEventCreateWithFlags(&c->done_event, cudaEventDisableTiming) == cudaSuccess;
   ok = ok && dmalloc(&c->z, Tp * V) == cudaSuccess;
-  if (!c->tensor_ok) ok = ok && dmalloc(&c->dl32, Tm * V) == cudaSuccess;
+  ok = ok && dmalloc(&c->dl32, Tm * V) == cudaSuccess;
   ok = ok && dmalloc(&c->stat_part, Tm * tts::kStatSplitsMax * tts::kStatFields) == cudaSuccess;
   ok = ok && dmalloc(&c->row_stats, 4 * Tm) == cudaSuccess;
   ok = ok && dmalloc(&c->arg_val, Tm * tts::kArgSplitsMax) == cudaSuccess;

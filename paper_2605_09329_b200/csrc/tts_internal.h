@@ -93,6 +93,8 @@ cudaError_t launch_accept_mask(tts_ctx* c, const void* teacher, const int32_t* t
 cudaError_t launch_row_stats(tts_ctx* c, const StepArgs& a, int z_ld, cudaStream_t s, int* launches);
 // tts_simt.cu
 cudaError_t simt_step(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches);
+cudaError_t simt_launch_logits(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches);
+cudaError_t simt_launch_gh(tts_ctx* c, const StepArgs& a, const float* dl32, cudaStream_t s, int* launches);
 // tts_tc.cu
 bool tc_supported(const tts_config& cfg);
 cudaError_t tc_init(tts_ctx* c);
