@@ -2,21 +2,20 @@
 // and optimiser state staged by TMA, mbarrier pipelines, warp-specialised persistent CTAs.
 //
 //   prep      (a4)     dl = coef_r (q - p) from z, teacher and the row normalisers; written as the bf16
-//                      operands of the two gradient contractions (hi/lo split: dl = hi + lo to 2^-16)
+//                      operands of the two gradient contractions (hi/lo split: dl = hi + lo to 2^-16):
+//                      dlT [V, Kp] (vocabulary-major, for gW) and dlR [2, P, V] (row-major planes, for gh)
 //   update    (a6+a7)  gW^T tile = h^T . dl   on the tensor cores (accumulator in TMEM, never in HBM),
 //                      epilogue = SGD / AdamW on the fp32 master + bf16 working-copy write-back; the
 //                      master / m / v tiles arrive by TMA, results leave by coalesced 128-byte stores
 //
 // Tile orientation of the update: TMEM lane = hidden column j, TMEM column = vocabulary row v, so that a
 // warp's 32 lanes touch 32 consecutive floats of one parameter row: every global access is a full line.
-#include <cuda.h>
-#include <cudaTypedefs.h>
 #include <new>
 #include <string.h>
 
 #include "tts_common.cuh"
-#include "tts_internal.h"
 #include "tts_tc_ptx.cuh"
+#include "tts_tc_state.h"
 
 namespace tts {
 namespace {
@@ -26,20 +25,11 @@ constexpr int kNV = 128;         // vocabulary rows per tile = MMA N = TMEM colu
 constexpr int kSV = 16;          // vocabulary rows per optimiser-state sub-tile (one pipeline stage)
 constexpr int kStages = 6;       // state ring depth
 constexpr int kOpStages = 2;     // operand ring depth
-constexpr int kKC = 64;          // bf16 elements per K chunk = one 128-byte swizzle row
 constexpr int kOpBytes = kMJ * kKC * 2;              // 16 KB per operand tile (A and B alike: kMJ == kNV)
 constexpr int kStateTileBytes = kSV * kMJ * 4;       // 8 KB per tensor per stage
 constexpr int kUpdThreads = 384; // warp 0 state TMA, 1 MMA, 2 TMEM alloc, 3 operand TMA, 4-11 epilogue
 constexpr int kTmemCols = 2 * kNV;
 constexpr int kUpdSmem = 1024 + 2 * kOpStages * kOpBytes + kStages * 3 * kStateTileBytes + 256;
-
-struct TcState {
-  __nv_bfloat16* dlT;   // [V, Kp]   B operand of gW: row v = (dl_hi[0..T16), dl_lo[0..T16)) of vocabulary row v
-  __nv_bfloat16* hTT;   // [d, Kp]   A operand of gW: row j = (h[0..T16, j], h[0..T16, j])
-  int Kp;               // allocated K extent (multiple of kKC)
-  CUtensorMap tm_dlT, tm_hTT;
-  PFN_cuTensorMapEncodeTiled_v12000 encode;
-};
 
 // ------------------------------------------------------------------ a4: operand preparation
 // One thread per vocabulary row v (coalesced over v for every canvas row r).
@@ -47,7 +37,8 @@ template <bool BF16>
 __global__ void __launch_bounds__(256) tc_prep_dl_kernel(const void* __restrict__ teacher, const float* __restrict__ z,
                                                          int V, int z_ld, int T, int T16, int Kp, int T_max,
                                                          const float* __restrict__ row_stats,
-                                                         __nv_bfloat16* __restrict__ dlT, float* __restrict__ dl32) {
+                                                         __nv_bfloat16* __restrict__ dlT,
+                                                         __nv_bfloat16* __restrict__ dlR, int P) {
   extern __shared__ float sh[];   // lse_t[T16], lse_z[T16], coef[T16]
   for (int r = threadIdx.x; r < T16; r += blockDim.x) {
     sh[r] = r < T ? row_stats[0 * T_max + r] : 0.f;
@@ -70,10 +61,13 @@ __global__ void __launch_bounds__(256) tc_prep_dl_kernel(const void* __restrict_
         const float q = expf(z[(size_t)r * z_ld + v] - sh[T16 + r]);
         const float p = expf(t - sh[r]);   // t = -inf -> 0
         dl = sh[2 * T16 + r] * (q - p);
-        if (dl32) dl32[(size_t)r * V + v] = dl;
       }
       const __nv_bfloat16 h = __float2bfloat16_rn(dl);
       const __nv_bfloat16 l = __float2bfloat16_rn(dl - __bfloat162float(h));
+      if (dlR) {   // row-major planes for the gh contraction (coalesced over v)
+        dlR[(size_t)r * V + v] = h;
+        dlR[(size_t)(P + r) * V + v] = l;
+      }
       const uint32_t hb = __bfloat16_as_ushort(h), lb = __bfloat16_as_ushort(l);
       if (u & 1) { hi[u >> 1] |= hb << 16; lo[u >> 1] |= lb << 16; }
       else       { hi[u >> 1] = hb;        lo[u >> 1] = lb; }
@@ -275,17 +269,6 @@ tc_update_kernel(const __grid_constant__ CUtensorMap tm_hTT, const __grid_consta
   }
 }
 
-// ------------------------------------------------------------------ host side
-CUresult make_map_2d(const TcState* st, CUtensorMap* m, CUtensorMapDataType dt, int esize, const void* base,
-                     uint64_t inner, uint64_t outer, uint32_t box_inner, uint32_t box_outer, CUtensorMapSwizzle sw) {
-  const cuuint64_t dims[2] = {inner, outer};
-  const cuuint64_t strides[1] = {inner * esize};
-  const cuuint32_t box[2] = {box_inner, box_outer};
-  const cuuint32_t estr[2] = {1, 1};
-  return st->encode(m, dt, 2, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, sw,
-                    CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-}
-
 }  // namespace
 
 bool tc_supported(const tts_config& cfg) {
@@ -308,6 +291,9 @@ cudaError_t tc_init(tts_ctx* c) {
   const size_t V = c->cfg.V, d = c->cfg.d;
   if ((e = cudaMalloc(&st->dlT, V * st->Kp * 2)) != cudaSuccess) return e;
   if ((e = cudaMalloc(&st->hTT, d * st->Kp * 2)) != cudaSuccess) return e;
+  st->P = T16 <= kGhNB ? T16 : (T16 + kGhNB - 1) / kGhNB * kGhNB;
+  if ((e = cudaMalloc(&st->dlR, (size_t)2 * st->P * V * 2)) != cudaSuccess) return e;
+  if ((e = cudaMemset(st->dlR, 0, (size_t)2 * st->P * V * 2)) != cudaSuccess) return e;
   if ((e = cudaMemset(st->dlT, 0, V * st->Kp * 2)) != cudaSuccess) return e;
   if ((e = cudaMemset(st->hTT, 0, d * st->Kp * 2)) != cudaSuccess) return e;
   if (make_map_2d(st, &st->tm_dlT, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, st->dlT, st->Kp, V, kKC, kNV,
@@ -322,7 +308,7 @@ cudaError_t tc_init(tts_ctx* c) {
   if ((e = cudaFuncSetAttribute(tc_update_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kUpdSmem)) !=
       cudaSuccess)
     return e;
-  return cudaSuccess;
+  return tc_gemm_init(c);
 }
 
 void tc_destroy(tts_ctx* c) {
@@ -330,6 +316,7 @@ void tc_destroy(tts_ctx* c) {
   if (!st) return;
   cudaFree(st->dlT);
   cudaFree(st->hTT);
+  cudaFree(st->dlR);
   delete st;
   c->tc_state = nullptr;
 }
@@ -341,29 +328,29 @@ cudaError_t tc_step(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches
   const bool adam = c->cfg.optimizer == TTS_ADAMW;
   cudaError_t e;
 
-  // a2: draft logits (CUDA-core kernel for now), a3: row statistics + loss
-  if ((e = simt_launch_logits(c, a, s, launches)) != cudaSuccess) return e;
+  // a2: draft logits on tcgen05, a3: row statistics + loss
+  if ((e = tc_launch_logits(c, a, s, launches)) != cudaSuccess) return e;
   prof_mark(c, 0, s);
   if ((e = launch_row_stats(c, a, V, s, launches)) != cudaSuccess) return e;
   prof_mark(c, 1, s);
 
   // a4: operands of the gradient contractions
-  float* dl32 = a.gh_out ? c->dl32 : nullptr;
+  __nv_bfloat16* dlR = a.gh_out ? st->dlR : nullptr;
   const size_t sh = 3 * T16 * sizeof(float);
   if (c->cfg.logits_dtype == TTS_BF16)
     tc_prep_dl_kernel<true><<<(V + 255) / 256, 256, sh, s>>>(a.teacher, c->z, V, V, T, T16, st->Kp, c->cfg.T_max,
-                                                               c->row_stats, st->dlT, dl32);
+                                                               c->row_stats, st->dlT, dlR, st->P);
   else
     tc_prep_dl_kernel<false><<<(V + 255) / 256, 256, sh, s>>>(a.teacher, c->z, V, V, T, T16, st->Kp, c->cfg.T_max,
-                                                                c->row_stats, st->dlT, dl32);
+                                                                c->row_stats, st->dlT, dlR, st->P);
   tc_prep_h_kernel<<<(d + 255) / 256, 256, 0, s>>>(static_cast<const __nv_bfloat16*>(a.h), d, T, T16, st->Kp,
                                                    st->hTT);
   *launches += 2;
   prof_mark(c, 2, s);
 
-  // a5: gh (CUDA-core kernel for now; reads W_in before the update may overwrite an aliased W_out)
+  // a5: gh on tcgen05 (reads W_in before the update may overwrite an aliased W_out)
   if (a.gh_out) {
-    if ((e = simt_launch_gh(c, a, dl32, s, launches)) != cudaSuccess) return e;
+    if ((e = tc_launch_gh(c, a, s, launches)) != cudaSuccess) return e;
   }
   prof_mark(c, 3, s);
 

@@ -1,0 +1,370 @@
+// The two W-streaming contractions of the distillation step on tcgen05 (sm_100a).  Both are strictly
+// W-bandwidth-bound at small T (16 flop per byte of W at T = 16): the kernels are persistent, one CTA per
+// SM, with a TMA producer warp keeping a deep ring of W tiles in flight, one MMA-issuing thread, and four
+// epilogue warps draining the TMEM accumulator of tile i while the ring already streams tile i + 1.
+//
+//   logits (a2)  z^T[v, r] = sum_j W_in[v, j] h[r, j]          M = 128 vocabulary rows, N = T16, K = d
+//                A = W_in tile, K-major (rows of W are contiguous in j);  B = h, K-major
+//   gh     (a5)  gh^T[j, r] = sum_v W_in[v, j] dl[r, v]        M = 128 hidden columns, N <= 128 rows, K = vocabulary
+//                A = W_in tile, MN-major (the same row-major W: j is contiguous, K = v strides by a row);
+//                B = dl planes [r, v], K-major.  dl = hi + lo (two bf16): both products accumulate into
+//                the same TMEM tile.  The vocabulary is split over CTAs; partial tiles are reduced with
+//                fp32 atomics into gh (zeroed first).
+#include <string.h>
+
+#include "tts_common.cuh"
+#include "tts_tc_ptx.cuh"
+#include "tts_tc_state.h"
+
+namespace tts {
+namespace {
+
+constexpr int kGemmThreads = 256;   // warp 0 TMA producer, 1 MMA issuer, 2 TMEM allocator, 3 idle, 4-7 epilogue
+constexpr int kATile = kTileMN * kKC * 2;   // 16 KB: [128 x 64] bf16 (K-major) or 2 x [64 k x 64 mn] (MN-major)
+constexpr int kMaxStages = 8;
+constexpr int kSmemBudget = 200 * 1024;
+constexpr int kNMax = 256;          // largest MMA N
+
+__host__ __device__ inline int pow2_cols(int n) {
+  int c = 32;
+  while (c < n) c <<= 1;
+  return c;
+}
+
+struct Bars {
+  uint64_t full[kMaxStages];
+  uint64_t empty[kMaxStages];
+  uint64_t acc_full[2];
+  uint64_t acc_empty[2];
+  uint32_t tmem_slot;
+};
+
+// ------------------------------------------------------------------ a2: draft logits
+struct LogitsParams {
+  float* z;
+  int z_ld;
+  int n_vt;        // V / 128
+  int k_chunks;    // d / 64
+  int T16;
+  int box_rows;    // rows per h box (<= 256)
+  int n_boxes;     // h boxes per stage
+  int stages;
+  int n_acc;       // TMEM accumulators (2 when 2 * T16 <= 512)
+  int tmem_cols;
+};
+
+__global__ void __launch_bounds__(kGemmThreads, 1)
+tc_logits_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant__ CUtensorMap tm_h,
+                 const LogitsParams p) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  const int b_bytes = p.n_boxes * p.box_rows * kKC * 2;
+  const int stage_bytes = kATile + b_bytes;
+  Bars* bars = reinterpret_cast<Bars*>(smem + p.stages * stage_bytes);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+  if (warp == 0 && lane == 0) {
+    ptx::prefetch_tensormap(&tm_W);
+    ptx::prefetch_tensormap(&tm_h);
+  }
+  if (warp == 1 && lane == 0) {
+    for (int i = 0; i < p.stages; ++i) { ptx::mbar_init(&bars->full[i], 1); ptx::mbar_init(&bars->empty[i], 1); }
+    for (int i = 0; i < 2; ++i) { ptx::mbar_init(&bars->acc_full[i], 1); ptx::mbar_init(&bars->acc_empty[i], 4); }
+    ptx::fence_barrier_init();
+  }
+  if (warp == 2) {
+    ptx::tmem_alloc(&bars->tmem_slot, p.tmem_cols);
+    ptx::tmem_relinquish();
+  }
+  ptx::tc_fence_before();
+  __syncthreads();
+  ptx::tc_fence_after();
+  const uint32_t tmem_base = bars->tmem_slot;
+
+  if (warp == 0) {
+    if (lane == 0) {
+      uint32_t n = 0;
+      for (int vt = blockIdx.x; vt < p.n_vt; vt += gridDim.x) {
+        for (int kc = 0; kc < p.k_chunks; ++kc, ++n) {
+          const int s = n % p.stages;
+          ptx::mbar_wait(&bars->empty[s], ((n / p.stages) & 1) ^ 1);
+          uint8_t* A = smem + s * stage_bytes;
+          ptx::mbar_expect_tx(&bars->full[s], stage_bytes);
+          ptx::tma_load_2d(A, &tm_W, &bars->full[s], kc * kKC, vt * kTileMN);
+          ptx::tma_load_2d(A + kATile / 2, &tm_W, &bars->full[s], kc * kKC, vt * kTileMN + 64);
+          for (int b = 0; b < p.n_boxes; ++b)
+            ptx::tma_load_2d(A + kATile + b * p.box_rows * kKC * 2, &tm_h, &bars->full[s], kc * kKC, b * p.box_rows);
+        }
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0) {
+      uint32_t n = 0, it = 0;
+      for (int vt = blockIdx.x; vt < p.n_vt; vt += gridDim.x, ++it) {
+        const int ab = it % p.n_acc;
+        ptx::mbar_wait(&bars->acc_empty[ab], ((it / p.n_acc) & 1) ^ 1);
+        ptx::tc_fence_after();
+        const uint32_t d_tmem = tmem_base + ab * p.T16;
+        for (int kc = 0; kc < p.k_chunks; ++kc, ++n) {
+          const int s = n % p.stages;
+          ptx::mbar_wait(&bars->full[s], (n / p.stages) & 1);
+          ptx::tc_fence_after();
+          const uint32_t a0 = ptx::smem_u32(smem + s * stage_bytes), b0 = a0 + kATile;
+#pragma unroll
+          for (int ks = 0; ks < kKC / 16; ++ks) {
+            const uint64_t ad = ptx::make_smem_desc(a0 + ks * 32, 16, 1024, ptx::kSwizzle128B);
+            for (int c0 = 0; c0 < p.T16; c0 += kNMax) {
+              const int nn = min(kNMax, p.T16 - c0);
+              const uint64_t bd = ptx::make_smem_desc(b0 + c0 * kKC * 2 + ks * 32, 16, 1024, ptx::kSwizzle128B);
+              ptx::mma_f16_ss(d_tmem + c0, ad, bd, ptx::make_idesc_bf16(kTileMN, nn, 0, 0), (kc | ks) != 0);
+            }
+          }
+          ptx::mma_commit(&bars->empty[s]);
+        }
+        ptx::mma_commit(&bars->acc_full[ab]);
+      }
+    }
+  } else if (warp >= 4) {
+    // epilogue: thread = one vocabulary row (TMEM lane); a warp's store of one canvas row is 128 contiguous bytes
+    const int q = warp & 3;
+    uint32_t it = 0;
+    for (int vt = blockIdx.x; vt < p.n_vt; vt += gridDim.x, ++it) {
+      const int ab = it % p.n_acc;
+      ptx::mbar_wait(&bars->acc_full[ab], (it / p.n_acc) & 1);
+      ptx::tc_fence_after();
+      float* zc = p.z + vt * kTileMN + q * 32 + lane;
+      for (int c0 = 0; c0 < p.T16; c0 += 16) {
+        uint32_t r[16];
+        ptx::tmem_ld_32x32b_x16(tmem_base + ab * p.T16 + c0 + (static_cast<uint32_t>(q * 32) << 16), r);
+        ptx::tmem_ld_wait();
+#pragma unroll
+        for (int i = 0; i < 16; ++i) zc[(size_t)(c0 + i) * p.z_ld] = __uint_as_float(r[i]);
+      }
+      ptx::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(&bars->acc_empty[ab]);
+    }
+  }
+  ptx::tc_fence_before();
+  __syncthreads();
+  if (warp == 2) {
+    ptx::tc_fence_after();
+    ptx::tmem_dealloc(tmem_base, p.tmem_cols);
+  }
+}
+
+// ------------------------------------------------------------------ a5: gh
+struct GhParams {
+  float* gh;
+  int T, d;
+  int n_jt;          // d / 128
+  int n_split;       // vocabulary splits
+  int chunks_split;  // K chunks (of 64 vocabulary rows) per split
+  int chunks_total;  // V / 64
+  int n_nb;          // accumulator blocks over the canvas rows
+  int NB;            // rows per block (MMA N)
+  int P;             // rows per dlR plane
+  int stages;
+  int tmem_cols;
+};
+
+__global__ void __launch_bounds__(kGemmThreads, 1)
+tc_gh_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant__ CUtensorMap tm_dl, const GhParams p) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  const int b_bytes = p.NB * kKC * 2;             // one plane
+  const int stage_bytes = kATile + 2 * b_bytes;
+  Bars* bars = reinterpret_cast<Bars*>(smem + p.stages * stage_bytes);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int n_units = p.n_jt * p.n_split;
+
+  if (warp == 0 && lane == 0) {
+    ptx::prefetch_tensormap(&tm_W);
+    ptx::prefetch_tensormap(&tm_dl);
+  }
+  if (warp == 1 && lane == 0) {
+    for (int i = 0; i < p.stages; ++i) { ptx::mbar_init(&bars->full[i], 1); ptx::mbar_init(&bars->empty[i], 1); }
+    for (int i = 0; i < 2; ++i) { ptx::mbar_init(&bars->acc_full[i], 1); ptx::mbar_init(&bars->acc_empty[i], 4); }
+    ptx::fence_barrier_init();
+  }
+  if (warp == 2) {
+    ptx::tmem_alloc(&bars->tmem_slot, p.tmem_cols);
+    ptx::tmem_relinquish();
+  }
+  ptx::tc_fence_before();
+  __syncthreads();
+  ptx::tc_fence_after();
+  const uint32_t tmem_base = bars->tmem_slot;
+
+  if (warp == 0) {
+    if (lane == 0) {
+      uint32_t n = 0;
+      for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
+        const int j0 = (u % p.n_jt) * kTileMN, sp = u / p.n_jt;
+        const int c_beg = sp * p.chunks_split, c_end = min(p.chunks_total, c_beg + p.chunks_split);
+        for (int nb = 0; nb < p.n_nb; ++nb) {
+          for (int kc = c_beg; kc < c_end; ++kc, ++n) {
+            const int s = n % p.stages;
+            ptx::mbar_wait(&bars->empty[s], ((n / p.stages) & 1) ^ 1);
+            uint8_t* A = smem + s * stage_bytes;
+            ptx::mbar_expect_tx(&bars->full[s], stage_bytes);
+            // W rows kc*64 .. +63 (K), columns j0 .. j0+127 (M) as two [64 k x 64 m] boxes
+            ptx::tma_load_2d(A, &tm_W, &bars->full[s], j0, kc * kKC);
+            ptx::tma_load_2d(A + kATile / 2, &tm_W, &bars->full[s], j0 + 64, kc * kKC);
+            ptx::tma_load_2d(A + kATile, &tm_dl, &bars->full[s], kc * kKC, nb * p.NB);
+            ptx::tma_load_2d(A + kATile + b_bytes, &tm_dl, &bars->full[s], kc * kKC, p.P + nb * p.NB);
+          }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0) {
+      const uint32_t idesc = ptx::make_idesc_bf16(kTileMN, p.NB, 1, 0);   // A MN-major, B K-major
+      uint32_t n = 0, it = 0;
+      for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
+        const int sp = u / p.n_jt;
+        const int c_beg = sp * p.chunks_split, c_end = min(p.chunks_total, c_beg + p.chunks_split);
+        for (int nb = 0; nb < p.n_nb; ++nb, ++it) {
+          const int ab = it & 1;
+          ptx::mbar_wait(&bars->acc_empty[ab], ((it >> 1) & 1) ^ 1);
+          ptx::tc_fence_after();
+          const uint32_t d_tmem = tmem_base + ab * p.NB;
+          for (int kc = c_beg; kc < c_end; ++kc, ++n) {
+            const int s = n % p.stages;
+            ptx::mbar_wait(&bars->full[s], (n / p.stages) & 1);
+            ptx::tc_fence_after();
+            const uint32_t a0 = ptx::smem_u32(smem + s * stage_bytes), b0 = a0 + kATile;
+#pragma unroll
+            for (int ks = 0; ks < kKC / 16; ++ks) {
+              // MN-major, 128-byte swizzle: 64 m per 128-byte row, one row per k; 8-row groups 1 KB apart (SBO),
+              // the second 64-m block kATile/2 further (LBO); 16 k per instruction = 2 KB
+              const uint64_t ad = ptx::make_smem_desc(a0 + ks * 2048, kATile / 2, 1024, ptx::kSwizzle128B);
+              const uint64_t bh = ptx::make_smem_desc(b0 + ks * 32, 16, 1024, ptx::kSwizzle128B);
+              const uint64_t bl = ptx::make_smem_desc(b0 + b_bytes + ks * 32, 16, 1024, ptx::kSwizzle128B);
+              ptx::mma_f16_ss(d_tmem, ad, bh, idesc, (kc != c_beg) || ks != 0);
+              ptx::mma_f16_ss(d_tmem, ad, bl, idesc, 1);
+            }
+            ptx::mma_commit(&bars->empty[s]);
+          }
+          ptx::mma_commit(&bars->acc_full[ab]);
+        }
+      }
+    }
+  } else if (warp >= 4) {
+    const int q = warp & 3;
+    uint32_t it = 0;
+    for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
+      const int j0 = (u % p.n_jt) * kTileMN;
+      for (int nb = 0; nb < p.n_nb; ++nb, ++it) {
+        const int ab = it & 1;
+        ptx::mbar_wait(&bars->acc_full[ab], (it >> 1) & 1);
+        ptx::tc_fence_after();
+        float* gc = p.gh + j0 + q * 32 + lane;
+        for (int c0 = 0; c0 < p.NB; c0 += 16) {
+          const int r0 = nb * p.NB + c0;
+          if (r0 >= p.T) break;
+          uint32_t r[16];
+          ptx::tmem_ld_32x32b_x16(tmem_base + ab * p.NB + c0 + (static_cast<uint32_t>(q * 32) << 16), r);
+          ptx::tmem_ld_wait();
+#pragma unroll
+          for (int i = 0; i < 16; ++i)
+            if (r0 + i < p.T) atomicAdd(gc + (size_t)(r0 + i) * p.d, __uint_as_float(r[i]));
+        }
+        ptx::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(&bars->acc_empty[ab]);
+      }
+    }
+  }
+  ptx::tc_fence_before();
+  __syncthreads();
+  if (warp == 2) {
+    ptx::tc_fence_after();
+    ptx::tmem_dealloc(tmem_base, p.tmem_cols);
+  }
+}
+
+int pick_stages(int stage_bytes) {
+  int s = (kSmemBudget - (int)sizeof(Bars) - 1024) / stage_bytes;
+  return s < 1 ? 1 : (s > kMaxStages ? kMaxStages : s);
+}
+
+}  // namespace
+
+cudaError_t tc_gemm_init(tts_ctx*) {
+  cudaError_t e;
+  const int smem_max = kSmemBudget + 16 * 1024;
+  if ((e = cudaFuncSetAttribute(tc_logits_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max)) !=
+      cudaSuccess)
+    return e;
+  return cudaFuncSetAttribute(tc_gh_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max);
+}
+
+cudaError_t tc_launch_logits(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches) {
+  TcState* st = static_cast<TcState*>(c->tc_state);
+  const int V = c->cfg.V, d = c->cfg.d, T = a.T;
+  const int T16 = (T + 15) / 16 * 16;
+  LogitsParams p;
+  p.z = c->z; p.z_ld = V;
+  p.n_vt = V / kTileMN; p.k_chunks = d / kKC; p.T16 = T16;
+  p.box_rows = T16 <= kNMax ? T16 : kNMax;
+  p.n_boxes = (T16 + p.box_rows - 1) / p.box_rows;
+  const int stage_bytes = kATile + p.n_boxes * p.box_rows * kKC * 2;
+  p.stages = pick_stages(stage_bytes);
+  p.n_acc = 2 * T16 <= 512 ? 2 : 1;
+  p.tmem_cols = pow2_cols(p.n_acc * T16);
+  CUtensorMap tm_W, tm_h;
+  if (make_map_2d(st, &tm_W, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, a.W_in, d, V, kKC, 64,
+                  CU_TENSOR_MAP_SWIZZLE_128B) != CUDA_SUCCESS)
+    return cudaErrorInvalidValue;
+  // rows >= T of a box are out of bounds: TMA fills them with zeros
+  if (make_map_2d(st, &tm_h, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, a.h, d, T, kKC, p.box_rows,
+                  CU_TENSOR_MAP_SWIZZLE_128B) != CUDA_SUCCESS)
+    return cudaErrorInvalidValue;
+  int grid = c->cfg.max_ctas > 0 ? c->cfg.max_ctas : c->sm_count;
+  if (grid > p.n_vt) grid = p.n_vt;
+  const size_t smem = 1024 + (size_t)p.stages * stage_bytes + sizeof(Bars);
+  tc_logits_kernel<<<grid, kGemmThreads, smem, s>>>(tm_W, tm_h, p);
+  *launches += 1;
+  return cudaGetLastError();
+}
+
+cudaError_t tc_launch_gh(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches) {
+  TcState* st = static_cast<TcState*>(c->tc_state);
+  const int V = c->cfg.V, d = c->cfg.d, T = a.T;
+  const int T16 = (T + 15) / 16 * 16;
+  cudaError_t e;
+  if ((e = cudaMemsetAsync(a.gh_out, 0, (size_t)T * d * sizeof(float), s)) != cudaSuccess) return e;
+  int grid = c->cfg.max_ctas > 0 ? c->cfg.max_ctas : c->sm_count;
+  GhParams p;
+  p.gh = a.gh_out; p.T = T; p.d = d;
+  p.n_jt = d / kTileMN;
+  p.chunks_total = V / kKC;
+  p.NB = T16 <= kGhNB ? T16 : kGhNB;
+  p.n_nb = (T16 + p.NB - 1) / p.NB;
+  p.P = st->P;
+  // about 8 units per CTA, each a contiguous run of vocabulary chunks for one 128-column tile of gh
+  int n_split = (8 * grid + p.n_jt - 1) / p.n_jt;
+  if (n_split > p.chunks_total) n_split = p.chunks_total;
+  if (n_split < 1) n_split = 1;
+  p.chunks_split = (p.chunks_total + n_split - 1) / n_split;
+  p.n_split = (p.chunks_total + p.chunks_split - 1) / p.chunks_split;
+  const int stage_bytes = kATile + 2 * p.NB * kKC * 2;
+  p.stages = pick_stages(stage_bytes);
+  p.tmem_cols = pow2_cols(2 * p.NB);
+  CUtensorMap tm_W, tm_dl;
+  if (make_map_2d(st, &tm_W, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, a.W_in, d, V, 64, kKC,
+                  CU_TENSOR_MAP_SWIZZLE_128B) != CUDA_SUCCESS)
+    return cudaErrorInvalidValue;
+  if (make_map_2d(st, &tm_dl, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, st->dlR, V, (uint64_t)2 * st->P, kKC, p.NB,
+                  CU_TENSOR_MAP_SWIZZLE_128B) != CUDA_SUCCESS)
+    return cudaErrorInvalidValue;
+  const int n_units = p.n_jt * p.n_split;
+  if (grid > n_units) grid = n_units;
+  const size_t smem = 1024 + (size_t)p.stages * stage_bytes + sizeof(Bars);
+  tc_gh_kernel<<<grid, kGemmThreads, smem, s>>>(tm_W, tm_dl, p);
+  *launches += 1;
+  return cudaGetLastError();
+}
+
+}  // namespace tts
