@@ -48,7 +48,7 @@ __global__ void __launch_bounds__(256) tc_prep_dl_kernel(const void* __restrict_
   __syncthreads();
   const int v = blockIdx.x * blockDim.x + threadIdx.x;
   if (v >= V) return;
-  uint4* out = reinterpret_cast<uint4*>(dlT + (size_t)v * Kp);
+  uint4* out = dlT ? reinterpret_cast<uint4*>(dlT + (size_t)v * Kp) : nullptr;
   for (int r0 = 0; r0 < T16; r0 += 8) {
     uint32_t hi[4], lo[4];
 #pragma unroll
@@ -72,8 +72,10 @@ __global__ void __launch_bounds__(256) tc_prep_dl_kernel(const void* __restrict_
       if (u & 1) { hi[u >> 1] |= hb << 16; lo[u >> 1] |= lb << 16; }
       else       { hi[u >> 1] = hb;        lo[u >> 1] = lb; }
     }
-    out[r0 / 8] = make_uint4(hi[0], hi[1], hi[2], hi[3]);
-    out[(T16 + r0) / 8] = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+    if (out) {
+      out[r0 / 8] = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+      out[(T16 + r0) / 8] = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+    }
   }
 }
 
@@ -308,7 +310,8 @@ cudaError_t tc_init(tts_ctx* c) {
   if ((e = cudaFuncSetAttribute(tc_update_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kUpdSmem)) !=
       cudaSuccess)
     return e;
-  return tc_gemm_init(c);
+  if ((e = tc_gemm_init(c)) != cudaSuccess) return e;
+  return tc_fused_init(c);
 }
 
 void tc_destroy(tts_ctx* c) {
@@ -335,19 +338,28 @@ cudaError_t tc_step(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches
   prof_mark(c, 1, s);
 
   // a4: operands of the gradient contractions
+  // small canvases with gh wanted: one fused pass (tts_tc_fused.cu) that needs only the dlR planes
+  const int fused_grid = a.gh_out ? tc_fused_grid(c, T16) : 0;
   __nv_bfloat16* dlR = a.gh_out ? st->dlR : nullptr;
+  __nv_bfloat16* dlT = fused_grid > 0 ? nullptr : st->dlT;
   const size_t sh = 3 * T16 * sizeof(float);
   if (c->cfg.logits_dtype == TTS_BF16)
     tc_prep_dl_kernel<true><<<(V + 255) / 256, 256, sh, s>>>(a.teacher, c->z, V, V, T, T16, st->Kp, c->cfg.T_max,
-                                                               c->row_stats, st->dlT, dlR, st->P);
+                                                               c->row_stats, dlT, dlR, st->P);
   else
     tc_prep_dl_kernel<false><<<(V + 255) / 256, 256, sh, s>>>(a.teacher, c->z, V, V, T, T16, st->Kp, c->cfg.T_max,
-                                                                c->row_stats, st->dlT, dlR, st->P);
+                                                                c->row_stats, dlT, dlR, st->P);
   tc_prep_h_kernel<<<(d + 255) / 256, 256, 0, s>>>(static_cast<const __nv_bfloat16*>(a.h), d, T, T16, st->Kp,
                                                    st->hTT);
   *launches += 2;
   prof_mark(c, 2, s);
 
+  if (fused_grid > 0) {
+    prof_mark(c, 3, s);
+    if ((e = tc_launch_update_fused(c, a, fused_grid, s, launches)) != cudaSuccess) return e;
+    prof_mark(c, 4, s);
+    return cudaGetLastError();
+  }
   // a5: gh on tcgen05 (reads W_in before the update may overwrite an aliased W_out)
   if (a.gh_out) {
     if ((e = tc_launch_gh(c, a, s, launches)) != cudaSuccess) return e;

@@ -43,4 +43,9 @@ cudaError_t tc_launch_logits(tts_ctx* c, const StepArgs& a, cudaStream_t s, int*
 // a5: gh[r, j] = sum_v (dl_hi + dl_lo)[r, v] W_in[v, j] on tcgen05, split over the vocabulary, fp32 atomics into gh
 cudaError_t tc_launch_gh(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches);
 
+// tts_tc_fused.cu: a5 + a6 + a7 in one pass over the optimiser state (T16 <= 32)
+cudaError_t tc_fused_init(tts_ctx* c);
+int tc_fused_grid(const tts_ctx* c, int T16);
+cudaError_t tc_launch_update_fused(tts_ctx* c, const StepArgs& a, int grid, cudaStream_t s, int* launches);
+
 }  // namespace tts
