@@ -320,6 +320,8 @@ void tc_destroy(tts_ctx* c) {
   cudaFree(st->dlT);
   cudaFree(st->hTT);
   cudaFree(st->dlR);
+  cudaFree(st->hTc);
+  cudaFree(st->dlC);
   delete st;
   c->tc_state = nullptr;
 }
@@ -338,28 +340,29 @@ cudaError_t tc_step(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches
   prof_mark(c, 1, s);
 
   // a4: operands of the gradient contractions
-  // small canvases with gh wanted: one fused pass (tts_tc_fused.cu) that needs only the dlR planes
-  const int fused_grid = a.gh_out ? tc_fused_grid(c, T16) : 0;
-  __nv_bfloat16* dlR = a.gh_out ? st->dlR : nullptr;
-  __nv_bfloat16* dlT = fused_grid > 0 ? nullptr : st->dlT;
-  const size_t sh = 3 * T16 * sizeof(float);
-  if (c->cfg.logits_dtype == TTS_BF16)
-    tc_prep_dl_kernel<true><<<(V + 255) / 256, 256, sh, s>>>(a.teacher, c->z, V, V, T, T16, st->Kp, c->cfg.T_max,
-                                                               c->row_stats, dlT, dlR, st->P);
-  else
-    tc_prep_dl_kernel<false><<<(V + 255) / 256, 256, sh, s>>>(a.teacher, c->z, V, V, T, T16, st->Kp, c->cfg.T_max,
-                                                                c->row_stats, dlT, dlR, st->P);
-  tc_prep_h_kernel<<<(d + 255) / 256, 256, 0, s>>>(static_cast<const __nv_bfloat16*>(a.h), d, T, T16, st->Kp,
-                                                   st->hTT);
-  *launches += 2;
-  prof_mark(c, 2, s);
-
+  // one canvas (T <= 16): one fused pass over the optimiser state (tts_tc_fused.cu) with its own pre-tiled operands
+  const int fused_grid = tc_fused_grid(c, T16);
   if (fused_grid > 0) {
+    if ((e = tc_launch_prep_fused(c, a, s, launches)) != cudaSuccess) return e;
+    prof_mark(c, 2, s);
     prof_mark(c, 3, s);
     if ((e = tc_launch_update_fused(c, a, fused_grid, s, launches)) != cudaSuccess) return e;
     prof_mark(c, 4, s);
     return cudaGetLastError();
   }
+  const size_t sh = 3 * T16 * sizeof(float);
+  __nv_bfloat16* dlR = a.gh_out ? st->dlR : nullptr;
+  if (c->cfg.logits_dtype == TTS_BF16)
+    tc_prep_dl_kernel<true><<<(V + 255) / 256, 256, sh, s>>>(a.teacher, c->z, V, V, T, T16, st->Kp, c->cfg.T_max,
+                                                               c->row_stats, st->dlT, dlR, st->P);
+  else
+    tc_prep_dl_kernel<false><<<(V + 255) / 256, 256, sh, s>>>(a.teacher, c->z, V, V, T, T16, st->Kp, c->cfg.T_max,
+                                                                c->row_stats, st->dlT, dlR, st->P);
+  *launches += 1;
+  tc_prep_h_kernel<<<(d + 255) / 256, 256, 0, s>>>(static_cast<const __nv_bfloat16*>(a.h), d, T, T16, st->Kp,
+                                                   st->hTT);
+  *launches += 1;
+  prof_mark(c, 2, s);
   // a5: gh on tcgen05 (reads W_in before the update may overwrite an aliased W_out)
   if (a.gh_out) {
     if ((e = tc_launch_gh(c, a, s, launches)) != cudaSuccess) return e;

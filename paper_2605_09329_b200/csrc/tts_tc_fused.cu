@@ -1,22 +1,30 @@
-// Pass B of the distillation step for small canvases (T16 <= 32): ONE persistent kernel per step that streams the
-// optimiser state exactly once and does, per [128 vocabulary rows x 128 hidden columns] tile,
+// Pass B of the distillation step for one canvas (T <= 16 rows): ONE persistent kernel per step that streams the
+// optimiser state exactly once and does, per tile of [16 vocabulary rows x 1024 hidden columns],
 //
-//   a6  gW^T tile = h^T . dl            tcgen05, accumulator in TMEM (never in HBM)
-//   a7  SGD / AdamW on the fp32 master  epilogue straight out of TMEM, state tiles staged by TMA,
-//       + bf16 working-copy write-back  results leave by coalesced 128-byte stores
-//   a5  gh^T[j, r] += W_in[v, j] dl[r, v]   tcgen05 as well: the bf16 tile of W_in is RE-DERIVED from the
-//                                       fp32 master tile the epilogue already holds in registers
-//                                       (precondition W_in == rn_bf16(W_master), include/tts.h), written to
-//                                       shared memory as the A operand, so bf16 W is not read from HBM again.
+//   a6  gW^T tile = h^T . dl            tcgen05, accumulators in TMEM (gW never exists in HBM)
+//   a7  SGD / AdamW on the fp32 master  epilogue straight out of TMEM; the master / m / v sub-tiles arrive by TMA, are
+//       + bf16 working-copy write-back  updated IN PLACE in shared memory and leave by TMA stores
+//   a5  gh^T[j, r] += W_in[v, j] dl[r, v]   tcgen05 as well: the bf16 tile of W_in is RE-DERIVED from the fp32
+//                                       master values the epilogue holds in registers (precondition
+//                                       W_in == rn_bf16(W_master), include/tts.h) and written to shared memory as
+//                                       the A operand, so bf16 W is not read from HBM again.  gh == NULL skips a5.
 //
-// gh accumulators persist in TMEM across a CTA's tiles: CTA b visits tiles t = b, b + grid, ..., whose hidden
-// tile index t mod n_jt takes only n_jt / gcd(grid, n_jt) distinct values (8 for grid 148, d = 4096), each
-// owning T16 TMEM columns next to the two gW accumulators; they are reduced into gh with fp32 atomics once,
-// at the end of the kernel.
+// Why this tile shape.  The pass is HBM-bound (26 bytes per parameter, 12 flop); what the memory system sees is
+// seven concurrent streams, three read and four written.  Measured on B200 with the same ring of TMA loads and
+// TMA stores and real (non-zero) data, only the shape of the sub-tile moved per pipeline stage changed:
+//     [128 cols x 16 rows] 5.65 TB/s   [256 x 8] 5.9   [512 x 4] 6.0   [1024 x 2] 6.7 (7 stages) / 6.4 (6 stages)
+// and per-thread 4-byte stores instead of TMA stores: 5.6 TB/s.  Long row segments (4 KB per tensor row) keep DRAM
+// pages open across the read and write streams.  So a pipeline stage is [2 rows x 1024 columns] of master, m
+// and v (24 KB), a tile is 8 stages, and a CTA owns ONE 1024-column stripe of the parameter matrix for the whole
+// kernel: its h^T operand (8 blocks of [128 j x 16 k]) is loaded once, and its gh accumulators (8 blocks of
+// [128 j x 16 r], 128 TMEM columns) persist in TMEM and are flushed once, with fp32 atomics, at the end.
 //
-// Operands: hTT [d, Kp] (K-major A of gW) and the dl planes dlR [2, P, V] (hi / lo bf16 split of dl).  One
-// shared-memory copy of the dlR tile serves both contractions: as the MN-major B of gW (N = vocabulary,
-// K = canvas row) and as the K-major B of gh (N = canvas row, K = vocabulary).
+// Operands, both pre-tiled by the a4 kernels in the canonical no-swizzle core-matrix order ([8 rows][16 bytes]
+// contiguous), so a tile is one contiguous bulk copy:
+//   hTc [d / 128][T16 / 8][16][8 j][8 k]                 A of gW, K-major (K = canvas row)
+//   dlC [V / 16][2 planes][T16 / 8][2][8 r][8 v]          dl = hi + lo (bf16 split).  One shared-memory copy serves
+//       both contractions: core matrices [8 r][8 v] are the MN-major B of gW (N = v, K = r) and the K-major B
+//       of gh (N = r, K = v); only the roles of the two descriptor strides swap.
 #include <string.h>
 
 #include "tts_common.cuh"
@@ -26,30 +34,38 @@
 namespace tts {
 namespace {
 
-constexpr int kMJ = 128;         // hidden columns per tile  = MMA M = TMEM lanes
-constexpr int kNV = 128;         // vocabulary rows per tile = MMA N of gW
-constexpr int kSV = 16;          // vocabulary rows per optimiser-state sub-tile (one pipeline stage)
-constexpr int kSubs = kNV / kSV;
-constexpr int kStages = 6;       // state ring depth
-constexpr int kOpStages = 2;     // operand ring depth
-constexpr int kWt = 4;           // ring of re-derived bf16 W sub-tiles (A operand of gh)
-constexpr int kHBytes = kMJ * kKC * 2;               // 16 KB hTT tile
-constexpr int kStateTileBytes = kSV * kMJ * 4;       // 8 KB per tensor per stage
-constexpr int kWtBytes = kMJ * kSV * 2;              // 4 KB
-constexpr int kThreads = 384;    // warp 0 state TMA, 1 MMA, 2 TMEM alloc, 3 operand TMA, 4-11 epilogue
-constexpr int kGhCol0 = 2 * kNV; // first TMEM column of the gh accumulators
+constexpr int kMJ = 128;         // hidden columns per MMA block = MMA M = TMEM lanes
+constexpr int kJB = 8;           // MMA blocks per stripe
+constexpr int kSW = kMJ * kJB;   // stripe width: 1024 hidden columns
+constexpr int kTV = 16;          // vocabulary rows per tile = MMA N of gW = MMA K of gh
+constexpr int kSV = 2;           // vocabulary rows per pipeline stage
+constexpr int kSubs = kTV / kSV; // 8 stages per tile
+constexpr int kBoxW = 256;       // TMA box width (elements): 4 boxes per tensor per stage
+constexpr int kBoxes = kSW / kBoxW;
+constexpr int kT16 = 16;         // canvas rows (padded)
+constexpr int kMaxStages = 6;    // state ring depth
+constexpr int kOpStages = 2;     // dl tile ring depth
+constexpr int kTensorBytes = kSV * kSW * 4;          // 8 KB per tensor per stage
+constexpr int kStageBytes = 3 * kTensorBytes;        // 24 KB
+constexpr int kWoBytes = kSV * kSW * 2;              // 4 KB: bf16 W_out staging of one sub-tile (one per group)
+constexpr int kHBytes = kSW * kT16 * 2;              // 32 KB: the stripe's h^T operand
+constexpr int kWtBytes = kSW * kTV * 2;              // 32 KB: re-derived bf16 W^T tile (A operand of gh)
+constexpr int kDlBytes = 2 * kT16 * kTV * 2;         // 1 KB: dl tile, both planes
+constexpr int kThreads = 384;    // warp 0 state TMA, 1 MMA, 2 TMEM alloc, 3 operand loads, 4-11 epilogue
+constexpr int kGhCol0 = 2 * kJB * kTV;               // 256: first TMEM column of the gh accumulators
 constexpr int kTmemCols = 512;
 
 struct FusedParams {
   float* master;
   float* am;
   float* av;
-  __nv_bfloat16* W_out;
   float* gW_debug;
-  float* gh;
-  int V, d, T, T16, P;
-  int n_jt;     // d / 128
-  int jt_gcd;   // gcd(grid, n_jt): the hidden tiles a CTA visits are congruent mod jt_gcd
+  float* gh;                  // NULL: a5 is skipped
+  const __nv_bfloat16* hTc;
+  const __nv_bfloat16* dlC;
+  int V, d, T;
+  int n_stripes;              // d / 1024
+  int stages;
   float lr, b1, b2, eps, decay, c1, inv_sqrt_bc2;   // decay = 1 - lr wd, c1 = lr / (1 - b1^n)
 };
 
@@ -58,49 +74,60 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
   return *reinterpret_cast<const uint32_t*>(&p);
 }
 
+// CTA b owns stripe b % n_stripes and every `peers`-th band of 16 vocabulary rows of it.
+struct Walk {
+  int stripe, first_band, peers, n_my;
+  __device__ Walk(int b, int grid, int n_stripes, int n_bands) {
+    stripe = b % n_stripes;
+    first_band = b / n_stripes;
+    peers = (grid - stripe + n_stripes - 1) / n_stripes;   // CTAs with this stripe
+    n_my = first_band < n_bands ? (n_bands - first_band + peers - 1) / peers : 0;
+  }
+};
+
 template <bool ADAM>
 __global__ void __launch_bounds__(kThreads, 1)
-tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_hTT, const __grid_constant__ CUtensorMap tm_dl,
-                    const __grid_constant__ CUtensorMap tm_master, const __grid_constant__ CUtensorMap tm_m,
-                    const __grid_constant__ CUtensorMap tm_v, const FusedParams p) {
+tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_constant__ CUtensorMap tm_m,
+                    const __grid_constant__ CUtensorMap tm_v, const __grid_constant__ CUtensorMap tm_wout,
+                    const FusedParams p) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-  const int box_bytes = p.T16 * kKC * 2;     // one dlR box: [T16 rows x 64 v]
-  const int dl_bytes = 4 * box_bytes;        // (hi, lo) x (v 0..63, v 64..127)
-  uint8_t* opA = smem;                                  // [kOpStages][16 KB]   hTT tiles (SW128, K-major)
-  uint8_t* opB = opA + kOpStages * kHBytes;             // [kOpStages][dl_bytes] dlR tiles (SW128)
-  uint8_t* st = opB + kOpStages * dl_bytes;             // [kStages][3][kSV][128] fp32
-  uint8_t* wt = st + kStages * 3 * kStateTileBytes;     // [kWt][2 k-groups][16 j-groups][8 x 16 B]
-  uint64_t* bars = reinterpret_cast<uint64_t*>(wt + kWt * kWtBytes);
-  uint64_t* op_full = bars;                  // [kOpStages]
-  uint64_t* op_empty = op_full + kOpStages;  // [kOpStages]
-  uint64_t* acc_full = op_empty + kOpStages; // [2]
-  uint64_t* acc_empty = acc_full + 2;        // [2]
-  uint64_t* st_full = acc_empty + 2;         // [kStages]
-  uint64_t* st_empty = st_full + kStages;    // [kStages]
-  uint64_t* wt_full = st_empty + kStages;    // [kWt]
-  uint64_t* wt_empty = wt_full + kWt;        // [kWt]
-  uint64_t* gh_full = wt_empty + kWt;        // [1]
+  const int kStages = p.stages;
+  uint8_t* st = smem;                                   // [kStages][3][4 boxes][2 v][256] fp32
+  uint8_t* hT = st + kStages * kStageBytes;             // [8 jb][2 k-groups][16 j-groups][8 j][8 k] bf16
+  uint8_t* wt = hT + kHBytes;                           // [8 jb][2 v-groups][16 j-groups][8 j][8 v] bf16
+  uint8_t* wo = wt + kWtBytes;                          // [2 groups][4 boxes][2 v][256] bf16
+  uint8_t* dl = wo + 2 * kWoBytes;                      // [kOpStages][2 planes][2 r-groups][2 v-groups][8 r][8 v] bf16
+  uint64_t* bars = reinterpret_cast<uint64_t*>(dl + kOpStages * kDlBytes);
+  uint64_t* st_full = bars;                    // [kMaxStages]
+  uint64_t* st_empty = st_full + kMaxStages;   // [kMaxStages]
+  uint64_t* op_full = st_empty + kMaxStages;   // [kOpStages]
+  uint64_t* op_empty = op_full + kOpStages;    // [kOpStages]
+  uint64_t* acc_full = op_empty + kOpStages;   // [2]
+  uint64_t* acc_empty = acc_full + 2;          // [2]
+  uint64_t* h_full = acc_empty + 2;            // [1]
+  uint64_t* wt_full = h_full + 1;              // [1]
+  uint64_t* wt_empty = wt_full + 1;            // [1]
+  uint64_t* gh_full = wt_empty + 1;            // [1]
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(gh_full + 1);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int n_jt = p.n_jt;
-  const int n_tiles = (p.V / kNV) * n_jt;
-  const int n_my = (n_tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+  const bool do_gh = p.gh != nullptr;
+  const Walk w(blockIdx.x, gridDim.x, p.n_stripes, p.V / kTV);
+  const int j_stripe = w.stripe * kSW;
 
   if (warp == 0 && lane == 0) {
     ptx::prefetch_tensormap(&tm_master);
     if (ADAM) { ptx::prefetch_tensormap(&tm_m); ptx::prefetch_tensormap(&tm_v); }
-  }
-  if (warp == 3 && lane == 0) {
-    ptx::prefetch_tensormap(&tm_hTT);
-    ptx::prefetch_tensormap(&tm_dl);
+    ptx::prefetch_tensormap(&tm_wout);
   }
   if (warp == 1 && lane == 0) {
+    for (int i = 0; i < kStages; ++i) { ptx::mbar_init(&st_full[i], 1); ptx::mbar_init(&st_empty[i], 1); }
     for (int i = 0; i < kOpStages; ++i) { ptx::mbar_init(&op_full[i], 1); ptx::mbar_init(&op_empty[i], 1); }
     for (int i = 0; i < 2; ++i) { ptx::mbar_init(&acc_full[i], 1); ptx::mbar_init(&acc_empty[i], 8); }
-    for (int i = 0; i < kStages; ++i) { ptx::mbar_init(&st_full[i], 1); ptx::mbar_init(&st_empty[i], 4); }
-    for (int i = 0; i < kWt; ++i) { ptx::mbar_init(&wt_full[i], 4); ptx::mbar_init(&wt_empty[i], 1); }
+    ptx::mbar_init(h_full, 1);
+    ptx::mbar_init(wt_full, 8);
+    ptx::mbar_init(wt_empty, 1);
     ptx::mbar_init(gh_full, 1);
     ptx::fence_barrier_init();
   }
@@ -114,180 +141,215 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_hTT, const __grid_con
   const uint32_t tmem_base = *tmem_slot;
 
   if (warp == 0) {
-    // ===== optimiser-state producer: master / m / v sub-tiles [kSV rows x 128 floats] by TMA =====
+    // ===== optimiser-state producer: [2 v x 1024 j] of master / m / v per stage, 4 boxes of [256 x 2] each =====
     if (lane == 0) {
       uint32_t n = 0;
-      for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
-        const int v0 = (t / n_jt) * kNV, j0 = (t % n_jt) * kMJ;
+      for (int i = 0; i < w.n_my; ++i) {
+        const int v0 = (w.first_band + i * w.peers) * kTV;
         for (int sub = 0; sub < kSubs; ++sub, ++n) {
           const int s = n % kStages;
           ptx::mbar_wait(&st_empty[s], ((n / kStages) & 1) ^ 1);
-          uint8_t* dst = st + s * 3 * kStateTileBytes;
-          ptx::mbar_expect_tx(&st_full[s], (ADAM ? 3 : 1) * kStateTileBytes);
-          ptx::tma_load_2d(dst, &tm_master, &st_full[s], j0, v0 + sub * kSV);
-          if (ADAM) {
-            ptx::tma_load_2d(dst + kStateTileBytes, &tm_m, &st_full[s], j0, v0 + sub * kSV);
-            ptx::tma_load_2d(dst + 2 * kStateTileBytes, &tm_v, &st_full[s], j0, v0 + sub * kSV);
+          uint8_t* dst = st + s * kStageBytes;
+          ptx::mbar_expect_tx(&st_full[s], (ADAM ? 3 : 1) * kTensorBytes);
+          const int r0 = v0 + sub * kSV;
+#pragma unroll
+          for (int b = 0; b < kBoxes; ++b) {
+            const int c0 = j_stripe + b * kBoxW, off = b * kSV * kBoxW * 4;
+            ptx::tma_load_2d(dst + off, &tm_master, &st_full[s], c0, r0);
+            if (ADAM) {
+              ptx::tma_load_2d(dst + kTensorBytes + off, &tm_m, &st_full[s], c0, r0);
+              ptx::tma_load_2d(dst + 2 * kTensorBytes + off, &tm_v, &st_full[s], c0, r0);
+            }
           }
         }
       }
     }
   } else if (warp == 3) {
-    // ===== operand producer: hTT tile [128 j x 64 k] and the dlR tile (4 boxes [T16 r x 64 v]) =====
-    if (lane == 0) {
-      uint32_t it = 0;
-      for (int t = blockIdx.x; t < n_tiles; t += gridDim.x, ++it) {
-        const int v0 = (t / n_jt) * kNV, j0 = (t % n_jt) * kMJ;
-        const int s = it % kOpStages;
-        ptx::mbar_wait(&op_empty[s], ((it / kOpStages) & 1) ^ 1);
-        ptx::mbar_expect_tx(&op_full[s], kHBytes + dl_bytes);
-        ptx::tma_load_2d(opA + s * kHBytes, &tm_hTT, &op_full[s], 0, j0);
-        uint8_t* b = opB + s * dl_bytes;
-        for (int pl = 0; pl < 2; ++pl)
-          for (int kh = 0; kh < 2; ++kh)
-            ptx::tma_load_2d(b + (pl * 2 + kh) * box_bytes, &tm_dl, &op_full[s], v0 + kh * kKC, pl * p.P);
+    // ===== operand loads: the stripe's h^T tiles once, then one 1 KB dl tile per band =====
+    if (lane == 0 && w.n_my > 0) {
+      ptx::mbar_expect_tx(h_full, kHBytes);
+      ptx::bulk_load_1d(hT, p.hTc + (size_t)j_stripe * kT16, kHBytes, h_full);
+      for (int i = 0; i < w.n_my; ++i) {
+        const int band = w.first_band + i * w.peers;
+        const int s = i % kOpStages;
+        ptx::mbar_wait(&op_empty[s], ((i / kOpStages) & 1) ^ 1);
+        ptx::mbar_expect_tx(&op_full[s], kDlBytes);
+        ptx::bulk_load_1d(dl + s * kDlBytes, p.dlC + (size_t)band * (kDlBytes / 2), kDlBytes, &op_full[s]);
       }
     }
   } else if (warp == 1) {
     // ===== MMA issuer =====
-    if (lane == 0 && n_my > 0) {
-      const uint32_t idesc_gw = ptx::make_idesc_bf16(kMJ, kNV, 0, 1);      // A = hTT K-major, B = dl MN-major
-      const uint32_t idesc_gh = ptx::make_idesc_bf16(kMJ, p.T16, 0, 0);    // A = W (re-derived) K-major, B = dl K-major
-      const int k_steps = p.T16 / 16;
-      // acc[j, v] = sum_r hTT[j, r] (dl_hi + dl_lo)[r, v]
-      auto issue_gw = [&](uint32_t it) {
-        const int ab = it & 1;
-        ptx::mbar_wait(&acc_empty[ab], ((it >> 1) & 1) ^ 1);
-        const int s = it % kOpStages;
-        ptx::mbar_wait(&op_full[s], (it / kOpStages) & 1);
+    if (lane == 0 && w.n_my > 0) {
+      constexpr uint32_t idesc_gw = ptx::make_idesc_bf16(kMJ, kTV, 0, 1);    // A = h^T K-major, B = dl MN-major
+      constexpr uint32_t idesc_gh = ptx::make_idesc_bf16(kMJ, kT16, 0, 0);   // A = W^T K-major, B = dl K-major
+      ptx::mbar_wait(h_full, 0);
+      // acc[jb][j, v] = sum_r h^T[j, r] (dl_hi + dl_lo)[r, v]
+      auto issue_gw = [&](int i) {
+        const int ab = i & 1, s = i % kOpStages;
+        ptx::mbar_wait(&acc_empty[ab], ((i >> 1) & 1) ^ 1);
+        ptx::mbar_wait(&op_full[s], (i / kOpStages) & 1);
         ptx::tc_fence_after();
-        const uint32_t a0 = ptx::smem_u32(opA + s * kHBytes), b0 = ptx::smem_u32(opB + s * dl_bytes);
-        uint32_t acc = 0;
-        for (int pl = 0; pl < 2; ++pl)
-          for (int kk = 0; kk < k_steps; ++kk) {
-            const uint64_t ad = ptx::make_smem_desc(a0 + kk * 32, 16, 1024, ptx::kSwizzle128B);
-            // MN-major: 64 v per 128-byte row, one row per canvas row; the second 64 v are one box further (LBO)
-            const uint64_t bd =
-                ptx::make_smem_desc(b0 + pl * 2 * box_bytes + kk * 2048, box_bytes, 1024, ptx::kSwizzle128B);
-            ptx::mma_f16_ss(tmem_base + ab * kNV, ad, bd, idesc_gw, acc);
-            acc = 1;
+        const uint32_t b0 = ptx::smem_u32(dl + s * kDlBytes);
+        for (int jb = 0; jb < kJB; ++jb) {
+          // A: K-major, no swizzle: core matrices [8 j x 8 k]; j-groups 128 B apart (SBO), k-groups 2 KB (LBO)
+          const uint64_t ad = ptx::make_smem_desc(ptx::smem_u32(hT + jb * 4096), 2048, 128, 0);
+          for (int pl = 0; pl < 2; ++pl) {
+            // B: MN-major, no swizzle: core matrices [8 r x 8 v]; v-groups 128 B apart (SBO), r-groups 256 B (LBO)
+            const uint64_t bd = ptx::make_smem_desc(b0 + pl * 512, 256, 128, 0);
+            ptx::mma_f16_ss(tmem_base + ab * (kJB * kTV) + jb * kTV, ad, bd, idesc_gw, pl);
           }
+        }
         ptx::mma_commit(&acc_full[ab]);
       };
-      uint32_t slot_mask = 0;
-      issue_gw(0);
-      for (uint32_t it = 0; it < (uint32_t)n_my; ++it) {
-        const int t = blockIdx.x + it * gridDim.x;
-        const int slot = (t % n_jt) / p.jt_gcd;
-        const int s = it % kOpStages;
-        const uint32_t b0 = ptx::smem_u32(opB + s * dl_bytes);
-        for (int sub = 0; sub < kSubs; ++sub) {
-          if (sub == 3 && it + 1 < (uint32_t)n_my) issue_gw(it + 1);
-          const uint32_t n = it * kSubs + sub;
-          const int buf = n % kWt;
-          ptx::mbar_wait(&wt_full[buf], (n / kWt) & 1);
-          ptx::tc_fence_after();
-          // A: K-major, no swizzle: core matrices [8 j x 8 v] of 128 B; j-groups 128 B apart (SBO), the two
-          // v-groups 2 KB apart (LBO)
-          const uint64_t ad = ptx::make_smem_desc(ptx::smem_u32(wt + buf * kWtBytes), 2048, 128, 0);
-          for (int pl = 0; pl < 2; ++pl) {
-            const uint64_t bd = ptx::make_smem_desc(b0 + (pl * 2 + (sub >> 2)) * box_bytes + (sub & 3) * 32, 16, 1024,
-                                                    ptx::kSwizzle128B);
-            ptx::mma_f16_ss(tmem_base + kGhCol0 + slot * p.T16, ad, bd, idesc_gh, ((slot_mask >> slot) & 1) | pl);
-          }
-          slot_mask |= 1u << slot;
-          ptx::mma_commit(&wt_empty[buf]);
+      if (!do_gh) {
+        for (int i = 0; i < w.n_my; ++i) {
+          issue_gw(i);
+          ptx::mma_commit(&op_empty[i % kOpStages]);
         }
-        ptx::mma_commit(&op_empty[s]);
+      } else {
+        issue_gw(0);
+        for (int i = 0; i < w.n_my; ++i) {
+          if (i + 1 < w.n_my) issue_gw(i + 1);
+          // the epilogue has re-derived the whole [16 v x 1024 j] bf16 tile of W_in
+          ptx::mbar_wait(wt_full, i & 1);
+          ptx::tc_fence_after();
+          const uint32_t b0 = ptx::smem_u32(dl + (i % kOpStages) * kDlBytes);
+          for (int jb = 0; jb < kJB; ++jb) {
+            // A: K-major, no swizzle: core matrices [8 j x 8 v]; j-groups 128 B apart (SBO), v-groups 2 KB (LBO)
+            const uint64_t ad = ptx::make_smem_desc(ptx::smem_u32(wt + jb * 4096), 2048, 128, 0);
+            for (int pl = 0; pl < 2; ++pl) {
+              // B: K-major, no swizzle: the same core matrices; v-groups 128 B apart (LBO), r-groups 256 B (SBO)
+              const uint64_t bd = ptx::make_smem_desc(b0 + pl * 512, 128, 256, 0);
+              ptx::mma_f16_ss(tmem_base + kGhCol0 + jb * kT16, ad, bd, idesc_gh, (i > 0) | pl);
+            }
+          }
+          ptx::mma_commit(wt_empty);
+          ptx::mma_commit(&op_empty[i % kOpStages]);
+        }
+        ptx::mma_commit(gh_full);
       }
-      ptx::mma_commit(gh_full);
     }
   } else if (warp >= 4) {
-    // ===== epilogue: 2 groups x 4 warps; group g takes sub-tiles sub % 2 == g; warp quarter q owns lanes 32q.. =====
+    // ===== epilogue: 2 groups x 4 warps; group g takes sub-tiles sub % 2 == g; warp quarter q owns TMEM lanes 32q.. =====
+    // thread (q, lane) <-> jj = 32 q + lane: hidden columns jb * 128 + jj of the stripe, jb = 0..7, both rows of a stage
     const int q = warp & 3, g = (warp - 4) >> 2;
-    const int col = q * 32 + lane;
-    uint8_t* wt_thr = wt + (col >> 3) * 128 + (col & 7) * 16;
-    uint32_t slot_mask = 0;
-    uint32_t it = 0;
-    for (int t = blockIdx.x; t < n_tiles; t += gridDim.x, ++it) {
-      const int v0 = (t / n_jt) * kNV, j0 = (t % n_jt) * kMJ;
-      slot_mask |= 1u << ((t % n_jt) / p.jt_gcd);
-      const int ab = it & 1;
-      ptx::mbar_wait(&acc_full[ab], (it >> 1) & 1);
+    const int jj = q * 32 + lane;
+    const bool leader = jj == 0;               // issues the group's TMA stores and releases its state stages
+    // element (v, jb) of a stage tensor sits in box jb / 2, row v, column (jb % 2) * 128 + jj
+    uint8_t* wt_thr = wt + (jj >> 3) * 128 + (jj & 7) * 16;   // + jb * 4096 + (v >> 3) * 2048 + (v & 7) * 2
+    __nv_bfloat16* wo_g = reinterpret_cast<__nv_bfloat16*>(wo + g * kWoBytes);
+    int prev_s = -1;                           // stage whose stores this group issued last
+    for (int i = 0; i < w.n_my; ++i) {
+      const int v0 = (w.first_band + i * w.peers) * kTV;
+      const int ab = i & 1;
+      ptx::mbar_wait(&acc_full[ab], (i >> 1) & 1);
       ptx::tc_fence_after();
       for (int sub = g; sub < kSubs; sub += 2) {
-        const uint32_t n = it * kSubs + sub;
+        const uint32_t n = (uint32_t)i * kSubs + sub;
         const int s = n % kStages;
-        uint32_t gr[kSV];
-        ptx::tmem_ld_32x32b_x16(tmem_base + ab * kNV + sub * kSV + (static_cast<uint32_t>(q * 32) << 16), gr);
+        // gradients: columns (2 sub, 2 sub + 1) of each of the 8 accumulator blocks
+        uint32_t gr[kJB][2];
+#pragma unroll
+        for (int jb = 0; jb < kJB; ++jb)
+          ptx::tmem_ld_32x32b_x2(tmem_base + ab * (kJB * kTV) + jb * kTV + sub * kSV +
+                                     (static_cast<uint32_t>(q * 32) << 16), gr[jb]);
         ptx::mbar_wait(&st_full[s], (n / kStages) & 1);
-        const float* sM = reinterpret_cast<const float*>(st + s * 3 * kStateTileBytes) + col;
-        float M[kSV], mm[kSV], vv[kSV];
+        float* sM = reinterpret_cast<float*>(st + s * kStageBytes) + jj;
+        float M[kJB][2], mm[kJB][2], vv[kJB][2];
 #pragma unroll
-        for (int r = 0; r < kSV; ++r) {
-          M[r] = sM[r * kMJ];
-          if (ADAM) { mm[r] = sM[kSV * kMJ + r * kMJ]; vv[r] = sM[2 * kSV * kMJ + r * kMJ]; }
-        }
-        __syncwarp();
-        if (lane == 0) ptx::mbar_arrive(&st_empty[s]);   // the stage's smem is in registers now
-        // a5 operand: W_in[v, j] = rn_bf16(master[v, j]) for this thread's column j, 16 consecutive v
-        const int buf = n % kWt;
-        ptx::mbar_wait(&wt_empty[buf], ((n / kWt) & 1) ^ 1);
-        {
-          uint4 w0, w1;
-          w0.x = pack_bf16(M[0], M[1]);   w0.y = pack_bf16(M[2], M[3]);
-          w0.z = pack_bf16(M[4], M[5]);   w0.w = pack_bf16(M[6], M[7]);
-          w1.x = pack_bf16(M[8], M[9]);   w1.y = pack_bf16(M[10], M[11]);
-          w1.z = pack_bf16(M[12], M[13]); w1.w = pack_bf16(M[14], M[15]);
-          uint8_t* dst = wt_thr + buf * kWtBytes;
-          *reinterpret_cast<uint4*>(dst) = w0;
-          *reinterpret_cast<uint4*>(dst + 2048) = w1;
-        }
-        ptx::fence_proxy_async_smem();
-        __syncwarp();
-        if (lane == 0) ptx::mbar_arrive(&wt_full[buf]);
-        ptx::tmem_ld_wait();
-        size_t idx = (size_t)(v0 + sub * kSV) * p.d + j0 + col;
+        for (int jb = 0; jb < kJB; ++jb)
 #pragma unroll
-        for (int r = 0; r < kSV; ++r, idx += p.d) {
-          const float gg = __uint_as_float(gr[r]);
-          float Mn;
-          if (ADAM) {
-            const float m1 = p.b1 * mm[r] + (1.f - p.b1) * gg;
-            const float v1 = p.b2 * vv[r] + (1.f - p.b2) * gg * gg;
-            const float den = __fsqrt_rn(v1) * p.inv_sqrt_bc2 + p.eps;
-            Mn = M[r] * p.decay - __fdividef(p.c1 * m1, den);
-            p.am[idx] = m1;
-            p.av[idx] = v1;
-          } else {
-            Mn = M[r] - p.lr * gg;
+          for (int v = 0; v < 2; ++v) {
+            const int e = (jb >> 1) * 512 + v * 256 + (jb & 1) * 128;
+            M[jb][v] = sM[e];
+            if (ADAM) { mm[jb][v] = sM[kSV * kSW + e]; vv[jb][v] = sM[2 * kSV * kSW + e]; }
           }
-          p.master[idx] = Mn;
-          p.W_out[idx] = __float2bfloat16_rn(Mn);
-          if (p.gW_debug) p.gW_debug[idx] = gg;
+        if (do_gh) {
+          // a5 operand: W_in[v, j] = rn_bf16(master[v, j]); rows (2 sub, 2 sub + 1) of this thread's 8 columns
+          if (sub < 2) ptx::mbar_wait(wt_empty, (i & 1) ^ 1);   // gh MMAs of the previous tile have read wt
+          uint8_t* dst = wt_thr + (sub >> 2) * 2048 + (sub & 3) * 4;
+#pragma unroll
+          for (int jb = 0; jb < kJB; ++jb) *reinterpret_cast<uint32_t*>(dst + jb * 4096) = pack_bf16(M[jb][0], M[jb][1]);
+          if (sub >= kSubs - 2) {               // the group's last sub-tile of this tile
+            ptx::fence_proxy_async_smem();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(wt_full);
+          }
         }
+        ptx::tmem_ld_wait();
+        // a7 in place: the thread rewrites exactly the shared-memory words it read
+#pragma unroll
+        for (int jb = 0; jb < kJB; ++jb)
+#pragma unroll
+          for (int v = 0; v < 2; ++v) {
+            const int e = (jb >> 1) * 512 + v * 256 + (jb & 1) * 128;
+            const float gg = __uint_as_float(gr[jb][v]);
+            if (ADAM) {
+              const float m1 = p.b1 * mm[jb][v] + (1.f - p.b1) * gg;
+              const float v1 = p.b2 * vv[jb][v] + (1.f - p.b2) * gg * gg;
+              const float den = __fsqrt_rn(v1) * p.inv_sqrt_bc2 + p.eps;
+              M[jb][v] = M[jb][v] * p.decay - __fdividef(p.c1 * m1, den);
+              sM[kSV * kSW + e] = m1;
+              sM[2 * kSV * kSW + e] = v1;
+            } else {
+              M[jb][v] = M[jb][v] - p.lr * gg;
+            }
+            sM[e] = M[jb][v];
+          }
+        if (p.gW_debug) {
+#pragma unroll
+          for (int jb = 0; jb < kJB; ++jb)
+#pragma unroll
+            for (int v = 0; v < 2; ++v)
+              p.gW_debug[(size_t)(v0 + sub * kSV + v) * p.d + j_stripe + jb * kMJ + jj] = __uint_as_float(gr[jb][v]);
+        }
+        // the group's previous stores have read their shared memory: release that stage, reuse the bf16 staging
+        if (leader) {
+          ptx::bulk_wait_group_read<0>();
+          if (prev_s >= 0) ptx::mbar_arrive(&st_empty[prev_s]);
+        }
+        ptx::named_barrier_sync(1 + g, 128);
+#pragma unroll
+        for (int jb = 0; jb < kJB; ++jb)
+#pragma unroll
+          for (int v = 0; v < 2; ++v)
+            wo_g[(jb >> 1) * 512 + v * 256 + (jb & 1) * 128 + jj] = __float2bfloat16_rn(M[jb][v]);
+        ptx::fence_proxy_async_smem();
+        ptx::named_barrier_sync(1 + g, 128);
+        if (leader) {
+          const int r0 = v0 + sub * kSV;
+          const float* sT = reinterpret_cast<const float*>(st + s * kStageBytes);
+#pragma unroll
+          for (int b = 0; b < kBoxes; ++b) {
+            const int c0 = j_stripe + b * kBoxW, off = b * kSV * kBoxW;
+            ptx::tma_store_2d(&tm_master, sT + off, c0, r0);
+            if (ADAM) {
+              ptx::tma_store_2d(&tm_m, sT + kSV * kSW + off, c0, r0);
+              ptx::tma_store_2d(&tm_v, sT + 2 * kSV * kSW + off, c0, r0);
+            }
+            ptx::tma_store_2d(&tm_wout, wo_g + off, c0, r0);
+          }
+          ptx::bulk_commit_group();
+        }
+        prev_s = s;
       }
       ptx::tc_fence_before();
       __syncwarp();
       if (lane == 0) ptx::mbar_arrive(&acc_empty[ab]);
     }
-    // ===== gh flush: the CTA's persistent accumulators -> fp32 atomics (group 0: one warp per lane quarter) =====
-    if (g == 0 && it > 0) {
+    if (leader) ptx::bulk_wait_group_read<0>();   // shared memory must outlive the last stores' reads
+    // ===== gh flush: the stripe's persistent accumulators -> fp32 atomics (group 0: one warp per lane quarter) =====
+    if (do_gh && g == 0 && w.n_my > 0) {
       ptx::mbar_wait(gh_full, 0);
       ptx::tc_fence_after();
-      const int n_slots = n_jt / p.jt_gcd;
-      for (int slot = 0; slot < n_slots; ++slot) {
-        if (!((slot_mask >> slot) & 1)) continue;
-        const int jt = (blockIdx.x % p.jt_gcd) + p.jt_gcd * slot;
-        float* gc = p.gh + jt * kMJ + col;
-        for (int c0 = 0; c0 < p.T16; c0 += 16) {
-          uint32_t r[16];
-          ptx::tmem_ld_32x32b_x16(tmem_base + kGhCol0 + slot * p.T16 + c0 + (static_cast<uint32_t>(q * 32) << 16), r);
-          ptx::tmem_ld_wait();
+      for (int jb = 0; jb < kJB; ++jb) {
+        float* gc = p.gh + j_stripe + jb * kMJ + jj;
+        uint32_t r[16];
+        ptx::tmem_ld_32x32b_x16(tmem_base + kGhCol0 + jb * kT16 + (static_cast<uint32_t>(q * 32) << 16), r);
+        ptx::tmem_ld_wait();
 #pragma unroll
-          for (int i = 0; i < 16; ++i)
-            if (c0 + i < p.T) atomicAdd(gc + (size_t)(c0 + i) * p.d, __uint_as_float(r[i]));
-        }
+        for (int k = 0; k < 16; ++k)
+          if (k < p.T) atomicAdd(gc + (size_t)k * p.d, __uint_as_float(r[k]));
       }
     }
   }
@@ -299,80 +361,136 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_hTT, const __grid_con
   }
 }
 
-int gcd_int(int a, int b) {
-  while (b) { const int t = a % b; a = b; b = t; }
-  return a;
+size_t fused_smem() {
+  return 1024 + (size_t)kMaxStages * kStageBytes + kHBytes + kWtBytes + 2 * (size_t)kWoBytes +
+         (size_t)kOpStages * kDlBytes + 512;
 }
 
-size_t fused_smem(int T16) {
-  return 1024 + (size_t)kOpStages * (kHBytes + 4 * T16 * kKC * 2) + (size_t)kStages * 3 * kStateTileBytes +
-         (size_t)kWt * kWtBytes + 512;
+// hTc[jt][k / 8][jj / 8][jj % 8][k % 8] = h[k, jt * 128 + jj] (rows k >= T are zero): the [128 j x 16 k] A tiles of
+// the gW contraction in the canonical no-swizzle K-major order.  One thread per hidden column j.
+__global__ void __launch_bounds__(256) tc_prep_hc_kernel(const __nv_bfloat16* __restrict__ h, int d, int T,
+                                                         __nv_bfloat16* __restrict__ hTc) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= d) return;
+  const int jt = j / kMJ, jj = j % kMJ;
+  __nv_bfloat16* tile = hTc + (size_t)jt * kMJ * kT16 + (jj >> 3) * 64 + (jj & 7) * 8;
+  for (int k = 0; k < kT16; ++k)
+    tile[(k >> 3) * 1024 + (k & 7)] = k < T ? h[(size_t)k * d + j] : __float2bfloat16_rn(0.f);
+}
+
+// a4 for this pass: dl = coef_r (q - p) from z, teacher and the row normalisers, split into two bf16 (dl = hi + lo
+// to 2^-16 relative) and written pre-tiled: dlC[v / 16][plane][r / 8][(v % 16) / 8][r % 8][v % 8].
+// One thread per vocabulary row v (loads coalesced over v for every canvas row r).
+template <bool BF16>
+__global__ void __launch_bounds__(256) tc_prep_dlc_kernel(const void* __restrict__ teacher, const float* __restrict__ z,
+                                                          int V, int z_ld, int T, int T_max,
+                                                          const float* __restrict__ row_stats,
+                                                          __nv_bfloat16* __restrict__ dlC) {
+  __shared__ float sh[3 * kT16];   // lse_t, lse_z, coef
+  if (threadIdx.x < kT16) {
+    const int r = threadIdx.x;
+    sh[r] = r < T ? row_stats[0 * T_max + r] : 0.f;
+    sh[kT16 + r] = r < T ? row_stats[1 * T_max + r] : 0.f;
+    sh[2 * kT16 + r] = r < T ? row_stats[3 * T_max + r] : 0.f;
+  }
+  __syncthreads();
+  const int v = blockIdx.x * blockDim.x + threadIdx.x;
+  if (v >= V) return;
+  __nv_bfloat16* tile = dlC + (size_t)(v / kTV) * (kDlBytes / 2) + ((v % kTV) >> 3) * 64 + (v & 7);
+#pragma unroll
+  for (int r = 0; r < kT16; ++r) {
+    float dl = 0.f;
+    if (r < T) {
+      const float t = BF16 ? __bfloat162float(static_cast<const __nv_bfloat16*>(teacher)[(size_t)r * V + v])
+                           : static_cast<const float*>(teacher)[(size_t)r * V + v];
+      const float qv = expf(z[(size_t)r * z_ld + v] - sh[kT16 + r]);
+      const float pv = expf(t - sh[r]);   // t = -inf -> 0
+      dl = sh[2 * kT16 + r] * (qv - pv);
+    }
+    const __nv_bfloat16 hi = __float2bfloat16_rn(dl);
+    const __nv_bfloat16 lo = __float2bfloat16_rn(dl - __bfloat162float(hi));
+    const int e = (r >> 3) * 128 + (r & 7) * 8;
+    tile[e] = hi;
+    tile[256 + e] = lo;
+  }
 }
 
 }  // namespace
 
-cudaError_t tc_fused_init(tts_ctx*) {
+cudaError_t tc_fused_init(tts_ctx* c) {
   cudaError_t e;
-  const int smem = (int)fused_smem(32);
+  TcState* st = static_cast<TcState*>(c->tc_state);
+  if ((e = cudaMalloc(&st->hTc, (size_t)c->cfg.d * kT16 * 2)) != cudaSuccess) return e;
+  if ((e = cudaMalloc(&st->dlC, (size_t)c->cfg.V * 2 * kT16 * 2)) != cudaSuccess) return e;
+  const int smem = (int)fused_smem();
   if ((e = cudaFuncSetAttribute(tc_update_gh_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) !=
       cudaSuccess)
     return e;
   return cudaFuncSetAttribute(tc_update_gh_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
 }
 
-// Largest grid <= the wanted one whose CTAs each visit few enough distinct hidden tiles for their gh
-// accumulators to fit the TMEM columns left beside the gW accumulators.  0: no such grid.
+// Grid of the fused pass, 0 when the shape does not qualify (T > 16 rows, d or V not a multiple of the tile).
 int tc_fused_grid(const tts_ctx* c, int T16) {
-  if (T16 > 32) return 0;
-  const int n_jt = c->cfg.d / kMJ;
-  const long n_tiles = (long)(c->cfg.V / kNV) * n_jt;
+  if (T16 > kT16 || c->cfg.d % kSW != 0 || c->cfg.V % kTV != 0) return 0;
+  const long n_tiles = (long)(c->cfg.V / kTV) * (c->cfg.d / kSW);
   int grid = c->cfg.max_ctas > 0 ? c->cfg.max_ctas : c->sm_count;
   if (grid > n_tiles) grid = (int)n_tiles;
-  for (; grid >= 1; --grid)
-    if ((n_jt / gcd_int(grid, n_jt)) * T16 <= kTmemCols - kGhCol0) return grid;
-  return 0;
+  return grid;
+}
+
+// a4: the operands of the fused pass (h^T tiles and the pre-tiled dl planes)
+cudaError_t tc_launch_prep_fused(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches) {
+  TcState* st = static_cast<TcState*>(c->tc_state);
+  const int V = c->cfg.V, d = c->cfg.d;
+  tc_prep_hc_kernel<<<(d + 255) / 256, 256, 0, s>>>(static_cast<const __nv_bfloat16*>(a.h), d, a.T, st->hTc);
+  if (c->cfg.logits_dtype == TTS_BF16)
+    tc_prep_dlc_kernel<true><<<(V + 255) / 256, 256, 0, s>>>(a.teacher, c->z, V, V, a.T, c->cfg.T_max, c->row_stats,
+                                                              st->dlC);
+  else
+    tc_prep_dlc_kernel<false><<<(V + 255) / 256, 256, 0, s>>>(a.teacher, c->z, V, V, a.T, c->cfg.T_max, c->row_stats,
+                                                               st->dlC);
+  *launches += 2;
+  return cudaGetLastError();
 }
 
 cudaError_t tc_launch_update_fused(tts_ctx* c, const StepArgs& a, int grid, cudaStream_t s, int* launches) {
   TcState* st = static_cast<TcState*>(c->tc_state);
   const int V = c->cfg.V, d = c->cfg.d, T = a.T;
-  const int T16 = (T + 15) / 16 * 16;
   const bool adam = c->cfg.optimizer == TTS_ADAMW;
   cudaError_t e;
-  if ((e = cudaMemsetAsync(a.gh_out, 0, (size_t)T * d * sizeof(float), s)) != cudaSuccess) return e;
-  CUtensorMap tm_master, tm_m, tm_v, tm_dl;
-  if (make_map_2d(st, &tm_master, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, a.master, d, V, kMJ, kSV,
+  if (a.gh_out && (e = cudaMemsetAsync(a.gh_out, 0, (size_t)T * d * sizeof(float), s)) != cudaSuccess) return e;
+  CUtensorMap tm_master, tm_m, tm_v, tm_wout;
+  if (make_map_2d(st, &tm_master, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, a.master, d, V, kBoxW, kSV,
+                  CU_TENSOR_MAP_SWIZZLE_NONE) != CUDA_SUCCESS)
+    return cudaErrorInvalidValue;
+  if (make_map_2d(st, &tm_wout, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, a.W_out, d, V, kBoxW, kSV,
                   CU_TENSOR_MAP_SWIZZLE_NONE) != CUDA_SUCCESS)
     return cudaErrorInvalidValue;
   tm_m = tm_master;
   tm_v = tm_master;
   if (adam) {
-    if (make_map_2d(st, &tm_m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, a.adam_m, d, V, kMJ, kSV,
+    if (make_map_2d(st, &tm_m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, a.adam_m, d, V, kBoxW, kSV,
                     CU_TENSOR_MAP_SWIZZLE_NONE) != CUDA_SUCCESS)
       return cudaErrorInvalidValue;
-    if (make_map_2d(st, &tm_v, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, a.adam_v, d, V, kMJ, kSV,
+    if (make_map_2d(st, &tm_v, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, a.adam_v, d, V, kBoxW, kSV,
                     CU_TENSOR_MAP_SWIZZLE_NONE) != CUDA_SUCCESS)
       return cudaErrorInvalidValue;
   }
-  if (make_map_2d(st, &tm_dl, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, st->dlR, V, (uint64_t)2 * st->P, kKC, T16,
-                  CU_TENSOR_MAP_SWIZZLE_128B) != CUDA_SUCCESS)
-    return cudaErrorInvalidValue;
   FusedParams p;
   p.master = a.master; p.am = a.adam_m; p.av = a.adam_v;
-  p.W_out = static_cast<__nv_bfloat16*>(a.W_out);
-  p.gW_debug = a.gW_debug; p.gh = a.gh_out;
-  p.V = V; p.d = d; p.T = T; p.T16 = T16; p.P = st->P;
-  p.n_jt = d / kMJ;
-  p.jt_gcd = gcd_int(grid, p.n_jt);
+  p.gW_debug = a.gW_debug; p.gh = a.gh_out; p.hTc = st->hTc; p.dlC = st->dlC;
+  p.V = V; p.d = d; p.T = T;
+  p.n_stripes = d / kSW;
+  p.stages = kMaxStages;
   p.lr = a.lr; p.b1 = a.beta1; p.b2 = a.beta2; p.eps = a.eps;
   p.decay = 1.f - a.lr * a.wd;
   p.c1 = a.lr * a.inv_bc1;
   p.inv_sqrt_bc2 = a.inv_sqrt_bc2;
-  const size_t smem = fused_smem(T16);
+  const size_t smem = fused_smem();
   if (adam)
-    tc_update_gh_kernel<true><<<grid, kThreads, smem, s>>>(st->tm_hTT, tm_dl, tm_master, tm_m, tm_v, p);
+    tc_update_gh_kernel<true><<<grid, kThreads, smem, s>>>(tm_master, tm_m, tm_v, tm_wout, p);
   else
-    tc_update_gh_kernel<false><<<grid, kThreads, smem, s>>>(st->tm_hTT, tm_dl, tm_master, tm_m, tm_v, p);
+    tc_update_gh_kernel<false><<<grid, kThreads, smem, s>>>(tm_master, tm_m, tm_v, tm_wout, p);
   *launches += 1;
   return cudaGetLastError();
 }

@@ -17,6 +17,8 @@ constexpr int kGhNB = 128;       // canvas rows (MMA N) per accumulator block of
 struct TcState {
   __nv_bfloat16* dlT;   // [V, Kp]        B operand of gW: row v = (dl_hi[0..T16), dl_lo[0..T16)) of vocabulary row v
   __nv_bfloat16* hTT;   // [d, Kp]        A operand of gW: row j = (h[0..T16, j], h[0..T16, j])
+  __nv_bfloat16* hTc;   // [d / 128][2][16][8][8]        A tiles of gW in core-matrix order (tts_tc_fused.cu, T <= 16)
+  __nv_bfloat16* dlC;   // [V / 16][2][2][2][8][8]        dl hi / lo planes, pre-tiled in core-matrix order (tts_tc_fused.cu)
   __nv_bfloat16* dlR;   // [2, P, V]      B operand of gh: plane 0 = dl_hi[r, v], plane 1 = dl_lo[r, v]
   int Kp;               // K extent of dlT / hTT (multiple of kKC)
   int P;                // rows per dlR plane (T_pad_max, rounded up to kGhNB when larger)
@@ -43,9 +45,10 @@ cudaError_t tc_launch_logits(tts_ctx* c, const StepArgs& a, cudaStream_t s, int*
 // a5: gh[r, j] = sum_v (dl_hi + dl_lo)[r, v] W_in[v, j] on tcgen05, split over the vocabulary, fp32 atomics into gh
 cudaError_t tc_launch_gh(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches);
 
-// tts_tc_fused.cu: a5 + a6 + a7 in one pass over the optimiser state (T16 <= 32)
+// tts_tc_fused.cu: a5 + a6 + a7 in one pass over the optimiser state (T <= 16, d % 1024 == 0, V % 16 == 0)
 cudaError_t tc_fused_init(tts_ctx* c);
 int tc_fused_grid(const tts_ctx* c, int T16);
+cudaError_t tc_launch_prep_fused(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches);   // a4: operands
 cudaError_t tc_launch_update_fused(tts_ctx* c, const StepArgs& a, int grid, cudaStream_t s, int* launches);
 
 }  // namespace tts
