@@ -51,8 +51,48 @@ struct LogitsParams {
   int stages;
   int n_acc;       // TMEM accumulators (2 when 2 * T16 <= 512)
   int tmem_cols;
+  int stream_k;    // 1: every CTA owns an equal, contiguous range of (tile, K chunk) units; tiles cut by a range
+                   // boundary are accumulated into the zeroed z with fp32 RED (exactly two addends: order-free)
 };
 
+// Work of CTA b: units [u_beg, u_end) of the n_vt * k_chunks (tile, chunk) units, walked tile by tile.
+struct LogitsWalk {
+  long u, u_end;
+  int k_chunks;
+  __device__ LogitsWalk(const LogitsParams& p) : k_chunks(p.k_chunks) {
+    if (p.stream_k) {
+      const long total = (long)p.n_vt * p.k_chunks;
+      u = total * blockIdx.x / gridDim.x;
+      u_end = total * (blockIdx.x + 1) / gridDim.x;
+    } else {   // whole tiles, round robin
+      u = (long)blockIdx.x * p.k_chunks;
+      u_end = (long)p.n_vt * p.k_chunks;
+    }
+  }
+  __device__ bool done() const { return u >= u_end; }
+  // current piece: tile vt, chunks [c_beg, c_end)
+  __device__ void piece(int& vt, int& c_beg, int& c_end) const {
+    vt = (int)(u / k_chunks);
+    c_beg = (int)(u - (long)vt * k_chunks);
+    const long rest = u_end - u;
+    c_end = rest < k_chunks - c_beg ? c_beg + (int)rest : k_chunks;
+  }
+  __device__ void next(const LogitsParams& p, int c_beg, int c_end) {
+    u += c_end - c_beg;
+    if (!p.stream_k) u += (long)(gridDim.x - 1) * k_chunks;
+  }
+};
+
+// Upper 32 bits of a K-major, 128-byte-swizzled operand descriptor: SBO = 1024 B, version 1, swizzle mode 2;
+// the lower 32 bits are (address >> 4) | LBO (16 B >> 4) << 16, so stepping 16 K elements (32 B) adds 2.
+constexpr uint32_t kDescHiSw128 = (1024u >> 4) | (1u << 14) | (ptx::kSwizzle128B << 29);
+__device__ __forceinline__ uint32_t desc_lo_sw128(uint32_t smem_addr) { return ((smem_addr >> 4) & 0x3FFFu) | (1u << 16); }
+__device__ __forceinline__ uint64_t desc64(uint32_t hi, uint32_t lo) { return (static_cast<uint64_t>(hi) << 32) | lo; }
+
+// WIDE = false: T16 <= 256, one MMA per 16-element K step.  The single issuing thread is the pipeline's narrowest
+// point at T = 16 (a [128 x 16 x 16] MMA finishes in a few cycles): with descriptors rebuilt per instruction the
+// kernel ran at 3.7 TB/s, MMA-issue-bound; the loop below is 2 integer adds per MMA.
+template <bool WIDE>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 tc_logits_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant__ CUtensorMap tm_h,
                  const LogitsParams p) {
@@ -82,10 +122,13 @@ tc_logits_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant
   const uint32_t tmem_base = bars->tmem_slot;
 
   if (warp == 0) {
+    // ===== TMA producer: one [128 v x 64 k] W tile (two 64-row boxes) + the matching h chunk per stage =====
     if (lane == 0) {
       uint32_t n = 0;
-      for (int vt = blockIdx.x; vt < p.n_vt; vt += gridDim.x) {
-        for (int kc = 0; kc < p.k_chunks; ++kc, ++n) {
+      int vt, c_beg, c_end;
+      for (LogitsWalk w(p); !w.done(); w.next(p, c_beg, c_end)) {
+        w.piece(vt, c_beg, c_end);
+        for (int kc = c_beg; kc < c_end; ++kc, ++n) {
           const int s = n % p.stages;
           ptx::mbar_wait(&bars->empty[s], ((n / p.stages) & 1) ^ 1);
           uint8_t* A = smem + s * stage_bytes;
@@ -98,37 +141,53 @@ tc_logits_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant
       }
     }
   } else if (warp == 1) {
-    if (lane == 0) {
-      uint32_t n = 0, it = 0;
-      for (int vt = blockIdx.x; vt < p.n_vt; vt += gridDim.x, ++it) {
-        const int ab = it % p.n_acc;
-        ptx::mbar_wait(&bars->acc_empty[ab], ((it / p.n_acc) & 1) ^ 1);
+    // ===== MMA issuer: the whole warp walks the pipeline, one elected lane issues =====
+    const uint32_t idesc = ptx::make_idesc_bf16(kTileMN, WIDE ? kNMax : p.T16, 0, 0);
+    const uint32_t smem0 = ptx::smem_u32(smem);
+    uint32_t n = 0, it = 0;
+    int vt, c_beg, c_end;
+    for (LogitsWalk w(p); !w.done(); w.next(p, c_beg, c_end), ++it) {
+      w.piece(vt, c_beg, c_end);
+      const int ab = it % p.n_acc;
+      ptx::mbar_wait(&bars->acc_empty[ab], ((it / p.n_acc) & 1) ^ 1);
+      ptx::tc_fence_after();
+      const uint32_t d_tmem = tmem_base + ab * p.T16;
+      for (int kc = c_beg; kc < c_end; ++kc, ++n) {
+        const int s = n % p.stages;
+        ptx::mbar_wait(&bars->full[s], (n / p.stages) & 1);
         ptx::tc_fence_after();
-        const uint32_t d_tmem = tmem_base + ab * p.T16;
-        for (int kc = 0; kc < p.k_chunks; ++kc, ++n) {
-          const int s = n % p.stages;
-          ptx::mbar_wait(&bars->full[s], (n / p.stages) & 1);
-          ptx::tc_fence_after();
-          const uint32_t a0 = ptx::smem_u32(smem + s * stage_bytes), b0 = a0 + kATile;
+        if (ptx::elect_one()) {
+          const uint32_t a_lo = desc_lo_sw128(smem0 + s * stage_bytes);
+          const uint32_t b_lo = desc_lo_sw128(smem0 + s * stage_bytes + kATile);
 #pragma unroll
           for (int ks = 0; ks < kKC / 16; ++ks) {
-            const uint64_t ad = ptx::make_smem_desc(a0 + ks * 32, 16, 1024, ptx::kSwizzle128B);
-            for (int c0 = 0; c0 < p.T16; c0 += kNMax) {
-              const int nn = min(kNMax, p.T16 - c0);
-              const uint64_t bd = ptx::make_smem_desc(b0 + c0 * kKC * 2 + ks * 32, 16, 1024, ptx::kSwizzle128B);
-              ptx::mma_f16_ss(d_tmem + c0, ad, bd, ptx::make_idesc_bf16(kTileMN, nn, 0, 0), (kc | ks) != 0);
+            if (!WIDE) {
+              ptx::mma_f16_ss(d_tmem, desc64(kDescHiSw128, a_lo + 2 * ks), desc64(kDescHiSw128, b_lo + 2 * ks), idesc,
+                              (kc != c_beg) | ks);
+            } else {
+              for (int c0 = 0; c0 < p.T16; c0 += kNMax) {
+                const int nn = min(kNMax, p.T16 - c0);
+                ptx::mma_f16_ss(d_tmem + c0, desc64(kDescHiSw128, a_lo + 2 * ks),
+                                desc64(kDescHiSw128, b_lo + (c0 * kKC * 2 >> 4) + 2 * ks),
+                                ptx::make_idesc_bf16(kTileMN, nn, 0, 0), (kc != c_beg) | ks);
+              }
             }
           }
           ptx::mma_commit(&bars->empty[s]);
         }
-        ptx::mma_commit(&bars->acc_full[ab]);
+        __syncwarp();
       }
+      if (ptx::elect_one()) ptx::mma_commit(&bars->acc_full[ab]);
+      __syncwarp();
     }
   } else if (warp >= 4) {
-    // epilogue: thread = one vocabulary row (TMEM lane); a warp's store of one canvas row is 128 contiguous bytes
+    // ===== epilogue: thread = one vocabulary row (TMEM lane); a warp's access to one canvas row is 128 contiguous bytes =====
     const int q = warp & 3;
     uint32_t it = 0;
-    for (int vt = blockIdx.x; vt < p.n_vt; vt += gridDim.x, ++it) {
+    int vt, c_beg, c_end;
+    for (LogitsWalk w(p); !w.done(); w.next(p, c_beg, c_end), ++it) {
+      w.piece(vt, c_beg, c_end);
+      const bool partial = c_end - c_beg < p.k_chunks;
       const int ab = it % p.n_acc;
       ptx::mbar_wait(&bars->acc_full[ab], (it / p.n_acc) & 1);
       ptx::tc_fence_after();
@@ -137,8 +196,13 @@ tc_logits_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant
         uint32_t r[16];
         ptx::tmem_ld_32x32b_x16(tmem_base + ab * p.T16 + c0 + (static_cast<uint32_t>(q * 32) << 16), r);
         ptx::tmem_ld_wait();
+        if (partial) {
 #pragma unroll
-        for (int i = 0; i < 16; ++i) zc[(size_t)(c0 + i) * p.z_ld] = __uint_as_float(r[i]);
+          for (int i = 0; i < 16; ++i) atomicAdd(zc + (size_t)(c0 + i) * p.z_ld, __uint_as_float(r[i]));
+        } else {
+#pragma unroll
+          for (int i = 0; i < 16; ++i) zc[(size_t)(c0 + i) * p.z_ld] = __uint_as_float(r[i]);
+        }
       }
       ptx::tc_fence_before();
       __syncwarp();
@@ -294,7 +358,10 @@ int pick_stages(int stage_bytes) {
 cudaError_t tc_gemm_init(tts_ctx*) {
   cudaError_t e;
   const int smem_max = kSmemBudget + 16 * 1024;
-  if ((e = cudaFuncSetAttribute(tc_logits_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max)) !=
+  if ((e = cudaFuncSetAttribute(tc_logits_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max)) !=
+      cudaSuccess)
+    return e;
+  if ((e = cudaFuncSetAttribute(tc_logits_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max)) !=
       cudaSuccess)
     return e;
   return cudaFuncSetAttribute(tc_gh_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max);
@@ -323,8 +390,19 @@ cudaError_t tc_launch_logits(tts_ctx* c, const StepArgs& a, cudaStream_t s, int*
     return cudaErrorInvalidValue;
   int grid = c->cfg.max_ctas > 0 ? c->cfg.max_ctas : c->sm_count;
   if (grid > p.n_vt) grid = p.n_vt;
+  // Stream-K for one canvas: 1187 tiles over 148 CTAs would quantise to 9 waves of 8.02; equal contiguous unit
+  // ranges keep every SM busy to the end.  A range spans >= k_chunks units (grid <= n_vt), so a tile is cut at most
+  // once: it receives exactly two partial sums (or one store), and 0 + a + b does not depend on the order.
+  p.stream_k = T16 <= 32 && p.n_vt % grid != 0;
+  if (p.stream_k) {
+    cudaError_t e = cudaMemsetAsync(c->z, 0, (size_t)T16 * V * sizeof(float), s);
+    if (e != cudaSuccess) return e;
+  }
   const size_t smem = 1024 + (size_t)p.stages * stage_bytes + sizeof(Bars);
-  tc_logits_kernel<<<grid, kGemmThreads, smem, s>>>(tm_W, tm_h, p);
+  if (T16 <= kNMax)
+    tc_logits_kernel<false><<<grid, kGemmThreads, smem, s>>>(tm_W, tm_h, p);
+  else
+    tc_logits_kernel<true><<<grid, kGemmThreads, smem, s>>>(tm_W, tm_h, p);
   *launches += 1;
   return cudaGetLastError();
 }
