@@ -187,6 +187,40 @@ def stream_mu(t: int, rounds: int = 4000, mu_max: float = 3.0) -> float:
     return mu_max * t / rounds
 
 
+def make_stream(*, V: int, d: int, rounds: int, seg_len: int = 16, seed: int = 4, mu_max: float = 3.0,
+                sigma: float = 1.5, total_rounds: int | None = None):
+    """Config 5 scaled down, on the host, for the round-by-round parity test (R16): a fixed initial head
+    (master ~ N(0,0.02), W0 = rn_bf16(master)), the drift direction u, and per round t
+        h_t ~ N(0,1) (bf16),  teacher_t = rn_bf16(h_t . W0^T + mu_t u + sigma eps_t),  tokens_t = argmax h_t . W0^T.
+    The teacher is built from the INITIAL weights so that the GPU path and the oracle, whose weights evolve
+    separately, consume identical bits at every round.  (bench.py's full-size stream builds it from the current
+    weights on the device instead, which is what a verifier would see; that run is timed, not compared.)
+    Returns (case0, rounds_list): case0 has cfg / W / master / m / v / pos_weight; rounds_list[t] = dict(teacher, h,
+    draft_tokens)."""
+    c = dict(CONFIGS[5])
+    c.update(ADAM_DEFAULTS)
+    c.update(V=V, d=d, seg_len=seg_len, T=seg_len, n_seq=1, seed=seed)
+    total = total_rounds or rounds
+    rng = np.random.Generator(np.random.PCG64(seed))
+    master = rng.standard_normal((V, d), dtype=np.float32) * np.float32(0.02)
+    W_bits = f32_to_bf16_bits(master)
+    W0 = bf16_bits_to_f32(W_bits)
+    u = stream_direction(V, seed)
+    out = []
+    for t in range(rounds):
+        r = np.random.Generator(np.random.PCG64([seed, t]))
+        h = bf16_bits_to_f32(f32_to_bf16_bits(r.standard_normal((seg_len, d), dtype=np.float32)))
+        z = h @ W0.T
+        tl = z + np.float32(stream_mu(t, total, mu_max)) * u[None, :] + np.float32(sigma) * r.standard_normal(
+            (seg_len, V), dtype=np.float32)
+        out.append(dict(teacher=f32_to_bf16_bits(tl), h=f32_to_bf16_bits(h),
+                        draft_tokens=np.argmax(z, axis=1).astype(np.int32)))
+    case0 = dict(cfg=c, V=V, d=d, T=seg_len, seg_len=seg_len, W=W_bits, master=master,
+                 m=np.zeros((V, d), dtype=np.float32), v=np.zeros((V, d), dtype=np.float32),
+                 pos_weight=position_weights(c["weights"], seg_len, 1), loss_scale=1.0)
+    return case0, out
+
+
 def planted_mask_cases(V: int, seg_len: int, seed: int = 11, dtype=BF16):
     """Teacher logits / tokens with planted tau in {0, 1, 3, seg_len}, ties at the
     maximum (lowest index must win) and -inf entries; one segment per case."""

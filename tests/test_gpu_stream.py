@@ -1,0 +1,86 @@
+"""Round-by-round parity of a scaled-down config-5 stream: the strided, asynchronous schedule of
+PAPER.md:397-426 driven through paper_2605_09329_b200.scheduler against the fp64 oracle applying the same sequence
+of updates.  Both sides consume identical seeded inputs every round (synth.make_stream builds the teacher from the
+INITIAL head, so neither side's evolving weights leak into the other's inputs)."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import tts_oracle as O
+from paper_2605_09329_b200 import synth, tts
+from paper_2605_09329_b200.scheduler import DraftHeadUpdater
+
+from gpu_util import _dev, bits, max_abs
+
+pytestmark = pytest.mark.gpu
+
+ROUNDS = 48
+
+
+def _oracle_stream(case0, rounds, stride):
+    c = case0["cfg"]
+    W, M, m, v = case0["W"], case0["master"].astype(np.float64), case0["m"].astype(np.float64), case0["v"].astype(np.float64)
+    losses, taus, n = [], [], 0
+    for t, rd in enumerate(rounds):
+        if t % stride != 0:
+            continue
+        n += 1
+        mask, tau, _ = O.accept_mask(rd["teacher"], rd["draft_tokens"], case0["seg_len"])
+        r = O.distill_step(rd["teacher"], rd["h"], W, M, m, v, case0["pos_weight"], mask, seg_len=case0["seg_len"],
+                           loss_scale=1.0, optimizer="adamw", lr=c["lr"], beta1=c["beta1"], beta2=c["beta2"],
+                           eps=c["eps"], weight_decay=c["weight_decay"], step=n)
+        W, M, m, v = r["W_out"], r["master"], r["m"], r["v"]
+        losses.append(r["loss"])
+        taus.append(int(tau[0]))
+    return dict(W=W, master=M, m=m, v=v, losses=np.array(losses), taus=taus, updates=n)
+
+
+@pytest.mark.parametrize("stride,host_barrier", [(1, False), (3, False), (4, True)])
+def test_stream_matches_oracle_round_by_round(stride, host_barrier):
+    V, d = 2048 + 16 * 3, 1024
+    case0, rounds = synth.make_stream(V=V, d=d, rounds=ROUNDS)
+    o = _oracle_stream(case0, rounds, stride)
+    c = case0["cfg"]
+    W0, master, m, v = _dev(case0["W"]), _dev(case0["master"]), _dev(case0["m"]), _dev(case0["v"])
+    pw = _dev(case0["pos_weight"])
+    up = DraftHeadUpdater(W0, master, m, v, seg_len=16, T_max=16, stride=stride, lr=c["lr"], beta1=c["beta1"],
+                          beta2=c["beta2"], eps=c["eps"], weight_decay=c["weight_decay"], host_barrier=host_barrier,
+                          keep_snapshot=True)
+    try:
+        dev_rounds = [dict(teacher=_dev(r["teacher"]), h=_dev(r["h"]), tok=_dev(r["draft_tokens"])) for r in rounds]
+        losses, taus = [], []
+        for t, rd in enumerate(dev_rounds):
+            w_before = up.weights().data_ptr()
+            if up.on_round_end(rd["teacher"], rd["h"], rd["tok"], pw, 16):
+                # the drafter keeps reading the OLD buffer until the barrier (R18)
+                if stride > 1:
+                    assert up.weights().data_ptr() == w_before
+                tts.tts_sync_step(up.ctx)
+                losses.append(float(up.loss.item()))
+                taus.append(int(up.tau[0].item()))
+        up.barrier()
+        torch.cuda.synchronize()
+        assert up.updates == o["updates"] and tts.tts_get_step_count(up.ctx) == o["updates"]
+        assert taus == o["taus"]
+        losses = np.array(losses)
+        assert np.all(np.abs(losses - o["losses"]) <= 1e-3 * np.abs(o["losses"]) + 1e-6)
+        g_master = master.cpu().numpy().astype(np.float64)
+        for name, gg, ref in (("master", g_master, o["master"]), ("m", m.cpu().numpy(), o["m"]),
+                              ("v", v.cpu().numpy(), o["v"])):
+            assert max_abs(gg.astype(np.float64) - ref) <= 2e-3 * max_abs(ref), name
+        # the accumulated movement is real and agrees (a no-op would pass the line above: lr * rounds << 2e-3 max|M|)
+        M0 = case0["master"].astype(np.float64)
+        d_ref, d_gpu = o["master"] - M0, g_master - M0
+        assert np.abs(d_ref).mean() > 0.2 * c["lr"] * o["updates"] ** 0.5
+        assert np.abs(d_gpu - d_ref).mean() <= 0.02 * np.abs(d_ref).mean()
+        # working copy in the CURRENT buffer: bit-exactly rn_bf16 of the GPU's own master
+        np.testing.assert_array_equal(bits(up.weights()), O.f32_to_bf16_bits(master.cpu().numpy()))
+        # reset between requests: state returns to the snapshot bit for bit, Adam's count to 0
+        up.restore()
+        torch.cuda.synchronize()
+        np.testing.assert_array_equal(bits(up.weights()), case0["W"])
+        np.testing.assert_array_equal(master.cpu().numpy(), case0["master"])
+        assert float(m.abs().max()) == 0.0 and float(v.abs().max()) == 0.0
+        assert tts.tts_get_step_count(up.ctx) == 0 and up.round == 0
+    finally:
+        up.close()
