@@ -50,6 +50,13 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-sample-rows", type=int, default=8192, help="vocabulary rows in the oracle sample")
+    ap.add_argument("--stream", action="store_true",
+                    help="also run the long-generation stream protocol (BASELINE.json configs[4]; use --config 5)")
+    ap.add_argument("--rounds", type=int, default=4000, help="--stream: speculation rounds per pass")
+    ap.add_argument("--strides", default="1,5", help="--stream: update strides S to run")
+    ap.add_argument("--standins", default="hbm,compute", help="--stream: stand-in verification kernels to run")
+    ap.add_argument("--standin-gb", type=float, default=64.0,
+                    help="--stream: bytes the HBM-bound stand-in reads per round (64 GB ~ one bf16 pass over a 32B target)")
     return ap.parse_args()
 
 
@@ -211,20 +218,17 @@ def workload_config(cfg_id, world, path):
 def run_ours(args, rank, world, local_rank):
     import numpy as np
     import torch
-    import torch.distributed as dist
-    from paper_2605_09329_b200 import synth, tts
+    from paper_2605_09329_b200 import dist_util, synth, tts
 
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: the distillation step has no CPU fallback")
     torch.cuda.set_device(local_rank)
     dev = "cuda:%d" % local_rank
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device(dev))
+    tdev = torch.device(dev)
+    dist_util.init("nccl", tdev)
 
     def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+        dist_util.barrier(tdev)
 
     case = synth.make_case_device(args.config, dev, seed_offset=rank)
     c = case["cfg"]
@@ -275,10 +279,7 @@ def run_ours(args, rank, world, local_rank):
     phase_ms, n_prof = tts.tts_profile_read(ctx)
     tts.tts_profile_enable(ctx, 0)
     loss_val = float(loss.item())
-    tmax = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    ms_total = float(tmax.item())
+    ms_total = dist_util.max_over_ranks(ms_total, tdev)
 
     # ---- end to end through HOST buffers: tts_round_host (H2D of the round's inputs, D2H of loss/tau/mask) ----
     e2e = None
@@ -302,10 +303,8 @@ def run_ours(args, rank, world, local_rank):
         for _ in range(args.steps):
             round_host()
         barrier()
-        dt = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(dt, op=dist.ReduceOp.MAX)
-        e2e = {"value": world * args.steps / float(dt.item()), "unit": "steps/s",
+        dt = dist_util.max_over_ranks(time.perf_counter() - t0, tdev)
+        e2e = {"value": world * args.steps / dt, "unit": "steps/s",
                "h2d_bytes_per_step": int(ht.numel() * 2 + hh.numel() * 2 + htok.numel() * 4 + hpw.numel() * 4),
                "d2h_bytes_per_step": int(4 + htau.numel() * 4 + hmask.numel()),
                "timing": "host clock around K tts_round_host calls (each ends with a stream synchronise)"}
@@ -322,6 +321,9 @@ def run_ours(args, rank, world, local_rank):
                          % (sample["Vs"], V, d, T, sec, scale)}
 
     tts.tts_ctx_destroy(ctx)
+    stream = None
+    if args.stream and world == 1:
+        stream = run_stream(args, case, dev)
     if rank != 0:
         return
     ms_step = ms_total / args.steps
@@ -343,7 +345,135 @@ def run_ours(args, rank, world, local_rank):
             "config": workload_config(args.config, world, "tcgen05+tma" if used_tensor else "cuda-core"),
             "rows_V_per_sec": sps * T * V, "loss": loss_val, "clocks": clocks, "e2e": e2e,
             "gpu_launches": launches[0], "roofline": roof, "cpu_baseline": cpu}
+    if stream is not None:
+        line["stream"] = stream
     print(json.dumps(line), flush=True)
+
+
+def run_stream(args, case, dev):
+    """BASELINE.json configs[4] / SURVEY 8(d): `rounds` consecutive speculation rounds on one head.  Per round the
+    harness (main stream) draws h_t, builds the round's teacher ON THE DEVICE from the CURRENT weights,
+    t_t = rn_bf16(h_t W_cur^T + mu_t u + 1.5 eps_t) (DESIGN.md R16), and runs a stand-in verification kernel;
+    scheduler.DraftHeadUpdater dispatches the TTS update on the side stream every S rounds and places the barrier
+    S-1 rounds later.  The harness ops (torch matmul / randn / sum) stand in for the drafter and the
+    verifier and are not the product; every step of the update runs in libtts_b200.so.
+
+    Reported per (stand-in, S): rounds/s with and without updates, steady-state update steps/s from device
+    timestamps recorded behind each step on the side stream (rounds >= 200), and the EXPOSED step time
+    (time with updates - time without) / number of updates.  Two stand-ins because they bracket the answer: an
+    HBM-bound verifier competes with the (HBM-bound) update for the same bandwidth, a tensor-bound one does not."""
+    import torch
+    from paper_2605_09329_b200 import synth, tts
+    from paper_2605_09329_b200.scheduler import DraftHeadUpdater
+
+    c = case["cfg"]
+    V, d, C = case["V"], case["d"], case["seg_len"]
+    T = C
+    tdev = torch.device(dev)
+    main = torch.cuda.current_stream()
+    W0, master0 = case["W"].clone(), case["master"].clone()
+    u = torch.from_numpy(synth.stream_direction(V, c["seed"])).to(tdev)
+    pw = case["pos_weight"][:T].contiguous()
+    rounds, skip = args.rounds, min(200, args.rounds // 4)
+    mu_max = c.get("mu_max", 3.0)
+
+    free, _ = torch.cuda.mem_get_info()
+    nbytes = int(min(args.standin_gb * 1e9, free - 8e9))
+    big = torch.empty(nbytes // 4, dtype=torch.float32, device=tdev)
+    big.zero_()
+    ga = torch.randn(8192, 8192, device=tdev, dtype=torch.bfloat16)
+    gb = torch.randn(8192, 8192, device=tdev, dtype=torch.bfloat16)
+    gc = torch.empty(8192, 8192, device=tdev, dtype=torch.bfloat16)
+    sink = torch.zeros(1, device=tdev)
+
+    def standin_hbm():
+        sink.add_(big.sum())
+
+    def time_of(fn, n=3):
+        fn()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(n):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / n
+
+    hbm_ms = time_of(standin_hbm)
+    mm_ms = time_of(lambda: torch.matmul(ga, gb, out=gc))
+    n_mm = max(1, int(round(hbm_ms / mm_ms)))      # same duration as the HBM-bound stand-in, tensor-bound instead
+
+    def standin_compute():
+        for _ in range(n_mm):
+            torch.matmul(ga, gb, out=gc)
+
+    standins = {"hbm": (standin_hbm, "%.1f GB read-reduce, %.2f ms alone" % (nbytes / 1e9, hbm_ms)),
+                "compute": (standin_compute, "%d x bf16 8192^3 matmul, %.2f ms alone" % (n_mm, n_mm * mm_ms))}
+    bufs = [dict(teacher=torch.empty(T, V, dtype=torch.bfloat16, device=tdev),
+                 h=torch.empty(T, d, dtype=torch.bfloat16, device=tdev),
+                 tok=torch.empty(T, dtype=torch.int32, device=tdev)) for _ in range(2)]
+    noise = torch.empty(T, V, dtype=torch.float32, device=tdev)
+    hf = torch.empty(T, d, dtype=torch.float32, device=tdev)
+
+    def one_pass(kind, stride, with_updates):
+        m, v = torch.zeros_like(master0), torch.zeros_like(master0)
+        master, W = master0.clone(), W0.clone()
+        up = DraftHeadUpdater(W, master, m, v, seg_len=C, T_max=T, stride=stride, lr=c["lr"], beta1=c["beta1"],
+                              beta2=c["beta2"], eps=c["eps"], weight_decay=c["weight_decay"], want_gh=True)
+        g = torch.Generator(device=tdev)
+        g.manual_seed(1000003 * (c["seed"] + 1))
+        fn = standins[kind][0]
+        marks = []
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        for t in range(rounds):
+            if t == skip:
+                e0.record(main)
+            b = bufs[0] if t % stride == 0 else bufs[1]     # a dispatching round's buffers rest until the barrier (R17)
+            hf.normal_(0.0, 1.0, generator=g)
+            b["h"].copy_(hf)
+            z = torch.matmul(b["h"], up.weights().T).float()            # the drafter's logits from the CURRENT head
+            noise.normal_(0.0, 1.0, generator=g)
+            b["tok"].copy_(torch.argmax(z, dim=1))
+            b["teacher"].copy_(z.add_(u, alpha=synth.stream_mu(t, rounds, mu_max)).add_(noise, alpha=1.5))
+            fn()                                                           # stand-in verification
+            if with_updates:
+                if up.on_round_end(b["teacher"], b["h"], b["tok"], pw, T, 1.0, main) and t >= skip:
+                    ev = torch.cuda.Event(enable_timing=True)
+                    ev.record(up.side)
+                    marks.append(ev)
+        up.barrier(main)
+        e1.record(main)
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        out = {"ms": ms, "updates_timed": len(marks)}
+        if with_updates:
+            out["steps_per_s"] = (len(marks) - 1) / (marks[0].elapsed_time(marks[-1]) * 1e-3) if len(marks) > 1 else None
+            out["launches"] = up.launches
+            out["final_loss"] = float(up.loss.item())
+            ok = bool(torch.isfinite(master).all()) and bool(torch.isfinite(m).all()) and bool(torch.isfinite(v).all())
+            ok = ok and bool((up.weights() == master.to(torch.bfloat16)).all())
+            ok = ok and tts.tts_get_step_count(up.ctx) == up.updates == (rounds + stride - 1) // stride
+            out["invariants_ok"] = ok
+        up.close()
+        return out
+
+    res = {"rounds": rounds, "timed_rounds": rounds - skip, "runs": []}
+    for kind in [k for k in args.standins.split(",") if k in standins]:
+        base = one_pass(kind, 1, False)
+        for S in [int(x) for x in args.strides.split(",")]:
+            w = one_pass(kind, S, True)
+            n_upd = w["updates_timed"]
+            res["runs"].append({
+                "standin": kind, "standin_desc": standins[kind][1], "stride": S,
+                "rounds_per_s_without_updates": (rounds - skip) / (base["ms"] * 1e-3),
+                "rounds_per_s_with_updates": (rounds - skip) / (w["ms"] * 1e-3),
+                "steady_state_steps_per_s": w["steps_per_s"],
+                "exposed_step_ms": (w["ms"] - base["ms"]) / max(1, n_upd),
+                "updates_timed": n_upd, "gpu_launches": w["launches"], "final_loss": w["final_loss"],
+                "invariants_ok": w["invariants_ok"]})
+    return res
 
 
 def main():
