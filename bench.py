@@ -50,6 +50,9 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-sample-rows", type=int, default=8192, help="vocabulary rows in the oracle sample")
+    ap.add_argument("--draft-logits", default="computed", choices=["computed", "given"],
+                    help="given: the drafter's own logits are passed in (tts_distill_step_ex, SURVEY 8(f) f1) and pass "
+                         "a2 is skipped; the default computes them, as BASELINE.json's north_star describes")
     ap.add_argument("--stream", action="store_true",
                     help="also run the long-generation stream protocol (BASELINE.json configs[4]; use --config 5)")
     ap.add_argument("--rounds", type=int, default=4000, help="--stream: speculation rounds per pass")
@@ -249,11 +252,19 @@ def run_ours(args, rank, world, local_rank):
     launches = [0]
     cur = [0]
 
+    z_given = None
+    if args.draft_logits == "given":      # what the drafter already holds after generating the canvas
+        z_given = torch.cat([h[i:i + 64].float() @ case["W"].float().T for i in range(0, T, 64)], 0).contiguous()
+
     def step():
         tts.tts_accept_mask(ctx, teacher, tok, T, mask, tau, None, side)
         n = tts.tts_last_launch_count(ctx)
-        tts.tts_distill_step(ctx, teacher, h, W[cur[0]], W[1 - cur[0]], master, m, v, pw, mask, T,
-                             case["loss_scale"], loss, None, gh, None, side)
+        if z_given is None:
+            tts.tts_distill_step(ctx, teacher, h, W[cur[0]], W[1 - cur[0]], master, m, v, pw, mask, T,
+                                 case["loss_scale"], loss, None, gh, None, side)
+        else:
+            tts.tts_distill_step_ex(ctx, teacher, h, W[cur[0]], W[1 - cur[0]], master, m, v, pw, mask, T,
+                                    case["loss_scale"], loss, None, gh, None, draft_logits=z_given, side_stream=side)
         launches[0] += n + tts.tts_last_launch_count(ctx)
         tts.tts_wait_step(ctx, main)      # the paper's barrier before the next draft round
         cur[0] ^= 1
@@ -329,6 +340,8 @@ def run_ours(args, rank, world, local_rank):
     ms_step = ms_total / args.steps
     sps = world * 1e3 / ms_step
     step_bytes, upd_bytes = algorithmic_bytes(V, d, T)
+    if z_given is not None:
+        step_bytes += T * V * 4 - V * d * 2      # fp32 draft logits read instead of the bf16 W pass
     peak, peak_src = measured_peaks()
     upd_ms = phase_ms[4] if n_prof > 0 and phase_ms[4] > 0 else None
     roof = {"bound": "hbm", "kernel": "a6+a7 gW contraction fused with AdamW update (phase 4)",
@@ -342,7 +355,8 @@ def run_ours(args, rank, world, local_rank):
     line = {"metric": "distill_steps_per_sec", "value": sps, "unit": "steps/s", "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-            "config": workload_config(args.config, world, "tcgen05+tma" if used_tensor else "cuda-core"),
+            "config": dict(workload_config(args.config, world, "tcgen05+tma" if used_tensor else "cuda-core"),
+                           draft_logits=args.draft_logits),
             "rows_V_per_sec": sps * T * V, "loss": loss_val, "clocks": clocks, "e2e": e2e,
             "gpu_launches": launches[0], "roofline": roof, "cpu_baseline": cpu}
     if stream is not None:

@@ -162,6 +162,51 @@ int32_t tts_distill_step(tts_ctx* ctx,
                          void* side_stream);
 
 /*
+ * f1.  The same step with optional extras (host struct, read during the call; NULL = tts_distill_step):
+ *   draft_logits      [T,V] fp32 device, row stride V, or NULL.  "each time a draft canvas is generated, we naturally
+ *                     have access to both the drafter's probabilities q and the target's probabilities p"
+ *                     (PAPER.md:109): the drafter's logits z of the canvas rows are taken as given and pass a2 (one
+ *                     read of the bf16 W, 7% of the step's bytes) is skipped.  They must be the logits of (h, W_in).
+ *   draft_logits_out  [T,V] fp32 device or NULL: a2 writes z here instead of the ctx scratch, so that the caller can
+ *                     pass it back as ref_logits of later inner steps.  Exclusive with draft_logits.
+ *   ref_logits, lambda  the regulariser  lambda * K~L(q_t || q)  of PAPER.md:119-121 with q_t = softmax(ref_logits):
+ *                       loss += loss_scale * lambda * sum_r omega_r KL(q_t,r || q_r)
+ *                       dl    = loss_scale * omega_r [(q - p) + lambda (q - q_t)]
+ *                     At q = q_t (one step per round, the paper's default) both vanish for every
+ *                     lambda (R3); the term matters for K > 1 inner steps.  ref_logits NULL or lambda 0 skips it.
+ *   kl_rows_out stays KL(p_r || q_r), the first term only.
+ */
+typedef struct {
+  const float* draft_logits;
+  float* draft_logits_out;
+  const float* ref_logits;
+  float lambda;
+} tts_step_extras;
+
+int32_t tts_distill_step_ex(tts_ctx* ctx, const void* teacher_logits, const void* h, const void* W_in, void* W_out,
+                            float* W_master, float* adam_m, float* adam_v, const float* pos_weight,
+                            const uint8_t* mask, int32_t T, float loss_scale, float* loss_out, float* kl_rows_out,
+                            float* gh_out, float* gW_debug_out,
+                            const tts_step_extras* extras, /* host, may be NULL */
+                            void* side_stream);
+
+/*
+ * K optimisation steps on the same round's signal (section 6.5; the paper's default and best is K = 1).
+ * Step 1 is tts_distill_step (q = q_t: the lambda term is inert) and keeps its draft logits as z_ref; steps 2..K
+ * recompute z from the weights step k-1 wrote and add lambda * K~L(q_t || q).  Step 1 reads W_in and writes W_out,
+ * later steps update W_out in place; master / m / v advance K times and Adam's count by K.
+ *   draft_logits  [T,V] fp32 device or NULL: the drafter's own logits for step 1 (and z_ref), as in tts_distill_step_ex
+ *   loss_out      [K] device: the loss of every inner step;  kl_rows_out [T] or NULL: step 1's KL rows;
+ *   gh_out        [T,d] or NULL: the LAST step's gradient w.r.t. h
+ * The first call with K > 1 on a ctx allocates the z_ref scratch (T_max x V fp32); nothing else allocates.
+ */
+int32_t tts_distill_inner_steps(tts_ctx* ctx, const void* teacher_logits, const void* h, const void* W_in, void* W_out,
+                                float* W_master, float* adam_m, float* adam_v, const float* pos_weight,
+                                const uint8_t* mask, int32_t T, float loss_scale, int32_t K, float lambda,
+                                const float* draft_logits, float* loss_out, float* kl_rows_out, float* gh_out,
+                                void* side_stream);
+
+/*
  * Per-phase device timing (for bench.py's roofline line).  When enabled, tts_distill_step records
  * CUDA events on side_stream between its phases (no host synchronisation is added).  Phases:
  *   0 = a2 draft logits, 1 = a3 row statistics + loss, 2 = a4 dlogits / operand preparation,

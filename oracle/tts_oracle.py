@@ -24,7 +24,9 @@ What it computes, with the passage each step follows
   * ``sgd_update``        q <- q - eta grad L, Alg. 1 "Update" PAPER.md:158.
   * ``adamw_update``      "an optimizer (Adam) step", PAPER.md:393 (App. C.1);
                           hyper-parameter conventions per DESIGN.md R5.
-  * ``distill_step``      the whole step (dense, small shapes).
+  * ``distill_step``      the whole step (dense, small shapes); optionally with the drafter's
+                          own logits taken as given and the lambda term.
+  * ``distill_inner_steps`` K steps on one round's signal (section 6.5).
   * ``distill_step_rows`` the same step restricted to a subset of vocabulary
                           rows, given the full-vocabulary normalisers, so that a
                           full-size configuration can be checked on samples.
@@ -153,10 +155,12 @@ def kl_rows_from_logits(a_logits, b_logits):
     return term.sum(axis=1)
 
 
-def loss_and_grads(teacher_logits, h, W, omega, loss_scale=1.0, lam=0.0, z_ref=None):
+def loss_and_grads(teacher_logits, h, W, omega, loss_scale=1.0, lam=0.0, z_ref=None, z=None):
     """Dense evaluation.  Returns dict(loss, kl_rows, z, lse_t, lse_z, dl, gW, gh).
 
     1. z[r,v] = sum_j h[r,j] W[v,j]                      (q = q_t)
+       or, when ``z`` is given, the drafter's own logits of the canvas rows: after a round "we naturally have
+       access to both the drafter's probabilities q and the target's probabilities p"
     2. log p = t - lse(t), log q = z - lse(z)
     3. KL_r = sum_v p (log p - log q)
     4. loss = loss_scale * sum_r omega_r KL_r            (a sum)
@@ -168,7 +172,7 @@ def loss_and_grads(teacher_logits, h, W, omega, loss_scale=1.0, lam=0.0, z_ref=N
     hh = widen(h)
     WW = widen(W)
     om = np.asarray(omega, dtype=np.float64)
-    z = hh @ WW.T
+    z = hh @ WW.T if z is None else np.asarray(z, dtype=np.float64)
     lse_t = logsumexp_rows(t)
     lse_z = logsumexp_rows(z)
     p = np.exp(t - lse_t[:, None])
@@ -223,8 +227,12 @@ def working_copy_bits(M_new):
 
 def distill_step(teacher_logits, h, W_in, W_master, adam_m, adam_v, pos_weight, mask,
                  *, seg_len, mask_mode=ROWS_ALL, loss_scale=1.0, optimizer="adamw",
-                 lr=1e-5, beta1=0.9, beta2=0.999, eps=1e-8, weight_decay=0.0, step=1):
+                 lr=1e-5, beta1=0.9, beta2=0.999, eps=1e-8, weight_decay=0.0, step=1,
+                 draft_logits=None, lam=0.0, z_ref=None):
     """One TTS update (Alg. 1 lines 'Loss' + 'Update'), dense.
+
+    draft_logits : the drafter's logits z, taken as given instead of h W_in^T
+    lam, z_ref   : the regulariser lam * K~L(q_t || q) with q_t = softmax(z_ref)
 
     W_in     : working weights that produced q_t (bf16 bits or fp32)
     W_master : fp32 master (None when the parameters are fp32: W_in is the parameter)
@@ -232,7 +240,7 @@ def distill_step(teacher_logits, h, W_in, W_master, adam_m, adam_v, pos_weight, 
     (bf16 bits when a master exists, else fp32).
     """
     omega = row_weights(pos_weight, mask, mask_mode, seg_len)
-    r = loss_and_grads(teacher_logits, h, W_in, omega, loss_scale)
+    r = loss_and_grads(teacher_logits, h, W_in, omega, loss_scale, lam=lam, z_ref=z_ref, z=draft_logits)
     M = widen(W_master) if W_master is not None else widen(W_in)
     if optimizer == "sgd":
         M_new = sgd_update(M, r["gW"], lr)
@@ -246,6 +254,33 @@ def distill_step(teacher_logits, h, W_in, W_master, adam_m, adam_v, pos_weight, 
         out["W_out"] = working_copy_bits(M_new)
     else:
         out["W_out"] = M_new.astype(np.float32)
+    return out
+
+
+def distill_inner_steps(teacher_logits, h, W_in, W_master, adam_m, adam_v, pos_weight, mask, *, K, lam,
+                        step=1, draft_logits=None, **kw):
+    """K optimisation steps on the same round's training signal (section 6.5).  q_t is the drafter
+    that produced the canvas: z_ref = the logits of step 1 (h W_in^T, or the drafter's own ``draft_logits``).
+    Step 1 is evaluated at q = q_t, where the lam term and its gradient vanish; steps 2..K recompute z from the
+    weights the previous step wrote and add lam * K~L(q_t || q).  With a master, the working
+    copy of step k is rn_bf16(rn_fp32(master_k)) and the GPU's master is fp32, so the master is rounded to fp32
+    between steps.  Returns the last step's dict plus ``losses`` (all K)."""
+    W, M, m, v = W_in, W_master, adam_m, adam_v
+    z_ref, losses, out, kl1 = None, [], None, None
+    for k in range(K):
+        if k == 0:
+            out = distill_step(teacher_logits, h, W, M, m, v, pos_weight, mask, step=step, draft_logits=draft_logits,
+                               **kw)
+            z_ref, kl1 = out["z"], out["kl_rows"]
+        else:
+            out = distill_step(teacher_logits, h, W, M, m, v, pos_weight, mask, step=step + k, lam=lam, z_ref=z_ref,
+                               **kw)
+        losses.append(out["loss"])
+        W = out["W_out"]
+        M = out["master"].astype(np.float32) if W_master is not None else None
+        m, v = out["m"], out["v"]
+    out = dict(out)
+    out.update(losses=np.array(losses), kl_rows_step1=kl1)
     return out
 
 

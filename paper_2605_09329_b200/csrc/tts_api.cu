@@ -28,7 +28,7 @@ cudaError_t dmalloc(T** p, size_t n) {
 void free_all(tts_ctx* c) {
   if (!c) return;
   tts::tc_destroy(c);
-  cudaFree(c->z); cudaFree(c->dl32); cudaFree(c->stat_part); cudaFree(c->row_stats);
+  cudaFree(c->z); cudaFree(c->z_ref_buf); cudaFree(c->dl32); cudaFree(c->stat_part); cudaFree(c->row_stats);
   cudaFree(c->arg_val); cudaFree(c->arg_idx); cudaFree(c->argmax_tmp);
   cudaFree(c->st_teacher); cudaFree(c->st_h); cudaFree(c->st_tok); cudaFree(c->st_pw);
   cudaFree(c->st_mask); cudaFree(c->st_tau); cudaFree(c->st_loss);
@@ -95,7 +95,7 @@ int32_t tts_ctx_create(const tts_config* cfg, int32_t device, tts_ctx** out) {
   ok = ok && dmalloc(&c->z, Tp * V) == cudaSuccess;
   ok = ok && dmalloc(&c->dl32, Tm * V) == cudaSuccess;
   ok = ok && dmalloc(&c->stat_part, Tm * tts::kStatSplitsMax * tts::kStatFields) == cudaSuccess;
-  ok = ok && dmalloc(&c->row_stats, 4 * Tm) == cudaSuccess;
+  ok = ok && dmalloc(&c->row_stats, tts::kRowStatFields * Tm) == cudaSuccess;
   ok = ok && dmalloc(&c->arg_val, Tm * tts::kArgSplitsMax) == cudaSuccess;
   ok = ok && dmalloc(&c->arg_idx, Tm * tts::kArgSplitsMax) == cudaSuccess;
   ok = ok && dmalloc(&c->argmax_tmp, Tm) == cudaSuccess;
@@ -161,7 +161,21 @@ int32_t tts_distill_step(tts_ctx* c, const void* teacher, const void* h, const v
                          float* W_master, float* adam_m, float* adam_v, const float* pos_weight,
                          const uint8_t* mask, int32_t T, float loss_scale, float* loss_out, float* kl_rows_out,
                          float* gh_out, float* gW_debug_out, void* side_stream) {
+  return tts_distill_step_ex(c, teacher, h, W_in, W_out, W_master, adam_m, adam_v, pos_weight, mask, T, loss_scale,
+                             loss_out, kl_rows_out, gh_out, gW_debug_out, nullptr, side_stream);
+}
+
+int32_t tts_distill_step_ex(tts_ctx* c, const void* teacher, const void* h, const void* W_in, void* W_out,
+                            float* W_master, float* adam_m, float* adam_v, const float* pos_weight,
+                            const uint8_t* mask, int32_t T, float loss_scale, float* loss_out, float* kl_rows_out,
+                            float* gh_out, float* gW_debug_out, const tts_step_extras* ex, void* side_stream) {
   if (!c || !teacher || !h || !W_in || !W_out || !pos_weight || !loss_out) return TTS_ERR_INVALID_ARG;
+  if (ex) {
+    if (!(ex->lambda >= 0.f)) return TTS_ERR_INVALID_ARG;
+    if (ex->draft_logits && ex->draft_logits_out) return TTS_ERR_INVALID_ARG;   // nothing is computed to write out
+    if (!aligned16(ex->draft_logits) || !aligned16(ex->draft_logits_out) || !aligned16(ex->ref_logits))
+      return TTS_ERR_INVALID_ARG;
+  }
   const tts_config& cfg = c->cfg;
   if (T <= 0 || T > cfg.T_max || T % cfg.seg_len != 0) return TTS_ERR_INVALID_ARG;
   if ((cfg.param_dtype == TTS_BF16) != (W_master != nullptr)) return TTS_ERR_INVALID_ARG;
@@ -180,6 +194,10 @@ int32_t tts_distill_step(tts_ctx* c, const void* teacher, const void* h, const v
   a.master = W_master; a.adam_m = adam_m; a.adam_v = adam_v;
   a.pos_weight = pos_weight; a.mask = mask; a.T = T; a.loss_scale = loss_scale;
   a.loss_out = loss_out; a.kl_rows_out = kl_rows_out; a.gh_out = gh_out; a.gW_debug = gW_debug_out;
+  a.z_given = ex ? ex->draft_logits : nullptr;
+  a.z_keep = ex ? ex->draft_logits_out : nullptr;
+  a.z_ref = (ex && ex->lambda > 0.f) ? ex->ref_logits : nullptr;   // lambda = 0: the term vanishes, skip its sweep
+  a.lambda = a.z_ref ? ex->lambda : 0.f;
   a.lr = cfg.lr; a.beta1 = cfg.beta1; a.beta2 = cfg.beta2; a.eps = cfg.eps; a.wd = cfg.weight_decay;
   a.inv_bc1 = static_cast<float>(1.0 / (1.0 - pow(static_cast<double>(cfg.beta1), n)));
   a.inv_sqrt_bc2 = static_cast<float>(1.0 / sqrt(1.0 - pow(static_cast<double>(cfg.beta2), n)));
@@ -199,6 +217,41 @@ int32_t tts_distill_step(tts_ctx* c, const void* teacher, const void* h, const v
   if (c->prof_on) c->prof_count += 1;
   if ((e = cudaEventRecord(c->done_event, s)) != cudaSuccess) return cuda_fail(c, e);
   c->done_recorded = true;
+  return TTS_OK;
+}
+
+int32_t tts_distill_inner_steps(tts_ctx* c, const void* teacher, const void* h, const void* W_in, void* W_out,
+                                float* W_master, float* adam_m, float* adam_v, const float* pos_weight,
+                                const uint8_t* mask, int32_t T, float loss_scale, int32_t K, float lambda,
+                                const float* draft_logits, float* loss_out, float* kl_rows_out, float* gh_out,
+                                void* side_stream) {
+  if (!c || K < 1 || !(lambda >= 0.f) || !loss_out) return TTS_ERR_INVALID_ARG;
+  if (K > 1 && !c->z_ref_buf) {   // the only allocation outside tts_ctx_create: first use of K > 1 on this ctx
+    cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&c->z_ref_buf),
+                               (size_t)c->T_pad_max * c->cfg.V * sizeof(float));
+    if (e != cudaSuccess) return cuda_fail(c, e);
+  }
+  int launches = 0;
+  for (int k = 0; k < K; ++k) {
+    tts_step_extras ex;
+    ex.draft_logits = nullptr; ex.draft_logits_out = nullptr; ex.ref_logits = nullptr; ex.lambda = 0.f;
+    if (k == 0) {
+      // step 1 at q = q_t: the lambda term and its gradient vanish (R3).  Its logits become z_ref.
+      if (draft_logits) ex.draft_logits = draft_logits;
+      else if (K > 1) ex.draft_logits_out = c->z_ref_buf;
+    } else {
+      ex.ref_logits = draft_logits ? draft_logits : c->z_ref_buf;
+      ex.lambda = lambda;
+    }
+    // step 1 reads W_in and writes W_out; later steps update W_out in place (W_out may alias W_in, include/tts.h)
+    const int32_t st = tts_distill_step_ex(c, teacher, h, k == 0 ? W_in : W_out, W_out, W_master, adam_m, adam_v,
+                                           pos_weight, mask, T, loss_scale, loss_out + k,
+                                           k == 0 ? kl_rows_out : nullptr, k == K - 1 ? gh_out : nullptr, nullptr,
+                                           &ex, side_stream);
+    if (st != TTS_OK) return st;
+    launches += c->last_launches;
+  }
+  c->last_launches = launches;
   return TTS_OK;
 }
 

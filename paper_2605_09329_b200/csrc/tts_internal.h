@@ -12,7 +12,8 @@ namespace tts {
 
 constexpr int kStatSplitsMax = 64;   // V-splits per row in the row-statistics sweep
 constexpr int kArgSplitsMax = 64;    // V-splits per row in the argmax sweep
-constexpr int kStatFields = 5;       // (m_t, s_t, a, m_z, s_z), SURVEY §8(a) a3
+constexpr int kStatFields = 8;       // (m_t, s_t, a, m_z, s_z) of SURVEY §8(a) a3 + (m_ref, s_ref, b) of the lambda term
+constexpr int kRowStatFields = 5;    // row_stats planes: lse_t, lse_z, kl, coef, lse_ref
 constexpr int kProfSlots = 256;      // profiled steps kept between two tts_profile_read calls
 constexpr int kKPad = 64;            // K extent (bf16 elements) of one 128-byte swizzle atom
 
@@ -32,11 +33,20 @@ struct StepArgs {
   float* kl_rows_out;
   float* gh_out;
   float* gW_debug;
+  // f1: optional extras of tts_distill_step_ex
+  const float* z_given;   // [T,V] fp32 draft logits supplied by the caller (a2 is skipped) or NULL
+  float* z_keep;          // [T,V] fp32: a2 writes z here instead of the ctx scratch (it becomes z_ref of later inner steps) or NULL
+  const float* z_ref;     // [T,V] fp32 logits of q_t for the lambda term or NULL
+  float lambda;           // weight of K~L(q_t || q)
   // optimiser scalars for this step (bias corrections precomputed on the host in fp64)
   float lr, beta1, beta2, eps, wd;
   float inv_bc1;       // 1 / (1 - beta1^n)
   float inv_sqrt_bc2;  // 1 / sqrt(1 - beta2^n)
 };
+
+// where a2 writes the draft logits, and where a3 / a4 read them
+inline float* z_dst(const StepArgs& a, float* scratch) { return a.z_keep ? a.z_keep : scratch; }
+inline const float* z_src(const StepArgs& a, float* scratch) { return a.z_given ? a.z_given : z_dst(a, scratch); }
 
 }  // namespace tts
 
@@ -56,7 +66,8 @@ struct tts_ctx {
   float* z;               // [T_pad_max, V] draft logits (fp32)
   float* dl32;            // [T_max, V] fp32 dlogits                (CUDA-core path)
   float* stat_part;       // [T_max, kStatSplitsMax, 5]
-  float* row_stats;       // [4, T_max]: lse_t, lse_z, kl, coef (= loss_scale * omega)
+  float* row_stats;       // [kRowStatFields, T_max]: lse_t, lse_z, kl, coef (= loss_scale * omega), lse_ref
+  float* z_ref_buf;       // [T_pad_max, V] fp32, allocated by the first tts_distill_inner_steps call
   float* arg_val;         // [T_max, kArgSplitsMax]
   int32_t* arg_idx;       // [T_max, kArgSplitsMax]
   int32_t* argmax_tmp;    // [T_max]
@@ -90,10 +101,9 @@ cudaError_t launch_accept_mask(tts_ctx* c, const void* teacher, const int32_t* t
                                int32_t* tau, int32_t* am_out, cudaStream_t s, int* launches);
 // tts_stats.cu: row statistics + merge + loss (CUDA-core sweeps shared by both paths).
 // z_ld = leading dimension (row stride in floats) of the z scratch.
-cudaError_t launch_row_stats(tts_ctx* c, const StepArgs& a, int z_ld, cudaStream_t s, int* launches);
+cudaError_t launch_row_stats(tts_ctx* c, const StepArgs& a, const float* z, int z_ld, cudaStream_t s, int* launches);
 // tts_simt.cu
 cudaError_t simt_step(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches);
-cudaError_t simt_launch_logits(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches);
 cudaError_t simt_launch_gh(tts_ctx* c, const StepArgs& a, const float* dl32, cudaStream_t s, int* launches);
 // tts_tc.cu
 bool tc_supported(const tts_config& cfg);

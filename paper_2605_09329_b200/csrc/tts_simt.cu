@@ -53,16 +53,20 @@ __global__ void __launch_bounds__(256) simt_logits_kernel(const PT* __restrict__
 // ---------------------------------------------------------------- a4: dl = coef_r (q - p)
 template <bool BF16>
 __global__ void __launch_bounds__(256) simt_dl_kernel(const void* __restrict__ teacher, const float* __restrict__ z,
-                                                      int V, int z_ld, int T_max, const float* __restrict__ row_stats,
+                                                      const float* __restrict__ z_ref, float lam, int V, int z_ld,
+                                                      int T_max, const float* __restrict__ row_stats,
                                                       float* __restrict__ dl) {
   const int r = blockIdx.y;
   const float lse_t = row_stats[0 * T_max + r], lse_z = row_stats[1 * T_max + r], coef = row_stats[3 * T_max + r];
+  const float lse_ref = row_stats[4 * T_max + r];
   for (int v = blockIdx.x * blockDim.x + threadIdx.x; v < V; v += gridDim.x * blockDim.x) {
     const float t = BF16 ? __bfloat162float(static_cast<const __nv_bfloat16*>(teacher)[(size_t)r * V + v])
                          : static_cast<const float*>(teacher)[(size_t)r * V + v];
     const float q = expf(z[(size_t)r * z_ld + v] - lse_z);
     const float p = expf(t - lse_t);   // t = -inf -> 0
-    dl[(size_t)r * V + v] = coef * (q - p);
+    float g = q - p;
+    if (z_ref) g += lam * (q - expf(z_ref[(size_t)r * z_ld + v] - lse_ref));   // + lambda (q - q_ref)
+    dl[(size_t)r * V + v] = coef * g;
   }
 }
 
@@ -170,18 +174,23 @@ static cudaError_t simt_step_t(tts_ctx* c, const StepArgs& a, cudaStream_t s, in
   PT* W_out = static_cast<PT*>(a.W_out);
   const bool bf_logits = c->cfg.logits_dtype == TTS_BF16;
 
-  simt_logits_kernel<PT><<<dim3((V + 63) / 64, (T + 15) / 16), 256, 0, s>>>(h, W_in, T, V, d, c->z, V);
-  *launches += 1;
+  const float* z = z_src(a, c->z);
+  if (!a.z_given) {
+    simt_logits_kernel<PT><<<dim3((V + 63) / 64, (T + 15) / 16), 256, 0, s>>>(h, W_in, T, V, d, z_dst(a, c->z), V);
+    *launches += 1;
+  }
   prof_mark(c, 0, s);
-  cudaError_t e = launch_row_stats(c, a, V, s, launches);
+  cudaError_t e = launch_row_stats(c, a, z, V, s, launches);
   if (e != cudaSuccess) return e;
   prof_mark(c, 1, s);
   {
     const int gx = max(1, min((V + 255) / 256, (4 * c->sm_count + T - 1) / T));
     if (bf_logits)
-      simt_dl_kernel<true><<<dim3(gx, T), 256, 0, s>>>(a.teacher, c->z, V, V, c->cfg.T_max, c->row_stats, c->dl32);
+      simt_dl_kernel<true><<<dim3(gx, T), 256, 0, s>>>(a.teacher, z, a.z_ref, a.lambda, V, V, c->cfg.T_max,
+                                                       c->row_stats, c->dl32);
     else
-      simt_dl_kernel<false><<<dim3(gx, T), 256, 0, s>>>(a.teacher, c->z, V, V, c->cfg.T_max, c->row_stats, c->dl32);
+      simt_dl_kernel<false><<<dim3(gx, T), 256, 0, s>>>(a.teacher, z, a.z_ref, a.lambda, V, V, c->cfg.T_max,
+                                                        c->row_stats, c->dl32);
     *launches += 1;
   }
   prof_mark(c, 2, s);
@@ -209,19 +218,7 @@ static cudaError_t simt_step_t(tts_ctx* c, const StepArgs& a, cudaStream_t s, in
   return cudaGetLastError();
 }
 
-// Stand-alone launchers used by the tensor path for the phases it has no tcgen05 kernel for yet.
-cudaError_t simt_launch_logits(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches) {
-  const int V = c->cfg.V, d = c->cfg.d, T = a.T;
-  if (c->cfg.param_dtype == TTS_BF16)
-    simt_logits_kernel<__nv_bfloat16><<<dim3((V + 63) / 64, (T + 15) / 16), 256, 0, s>>>(
-        static_cast<const __nv_bfloat16*>(a.h), static_cast<const __nv_bfloat16*>(a.W_in), T, V, d, c->z, V);
-  else
-    simt_logits_kernel<float><<<dim3((V + 63) / 64, (T + 15) / 16), 256, 0, s>>>(
-        static_cast<const float*>(a.h), static_cast<const float*>(a.W_in), T, V, d, c->z, V);
-  *launches += 1;
-  return cudaGetLastError();
-}
-
+// Stand-alone launcher kept for shapes the tensor path has no gh kernel for.
 cudaError_t simt_launch_gh(tts_ctx* c, const StepArgs& a, const float* dl32, cudaStream_t s, int* launches) {
   const int V = c->cfg.V, d = c->cfg.d, T = a.T;
   cudaError_t e;

@@ -14,10 +14,12 @@ namespace tts {
 
 struct RowStat {
   float mt, st, a, mz, sz;
+  float mr, sr, b;   // reference distribution q_ref = softmax(z_ref): max, sum e^{zr-mr}, sum e^{zr-mr} (zr - z)
 };
 
 __device__ __forceinline__ void stat_init(RowStat& s) {
   s.mt = -CUDART_INF_F; s.st = 0.f; s.a = 0.f; s.mz = -CUDART_INF_F; s.sz = 0.f;
+  s.mr = -CUDART_INF_F; s.sr = 0.f; s.b = 0.f;
 }
 
 // one element; teacher entries equal to -inf have p = 0 and are dropped (0 log 0 := 0)
@@ -31,6 +33,12 @@ __device__ __forceinline__ void stat_push(RowStat& s, float t, float z) {
   if (z > s.mz) { s.sz = s.sz * e + 1.f; s.mz = z; }
   else          { s.sz += e; }
 }
+// the lambda term's statistics: K~L(q_ref || q)_r = b / s_ref - lse_ref + lse_z
+__device__ __forceinline__ void stat_push_ref(RowStat& s, float zr, float z) {
+  const float e = expf(-fabsf(zr - s.mr));
+  if (zr > s.mr) { s.sr = s.sr * e + 1.f; s.b = s.b * e + (zr - z); s.mr = zr; }
+  else           { s.sr += e;             s.b += e * (zr - z); }
+}
 
 __device__ __forceinline__ RowStat stat_merge(const RowStat& x, const RowStat& y) {
   RowStat o;
@@ -43,6 +51,11 @@ __device__ __forceinline__ RowStat stat_merge(const RowStat& x, const RowStat& y
   const float fx = (x.mz == -CUDART_INF_F) ? 0.f : expf(x.mz - o.mz);
   const float fy = (y.mz == -CUDART_INF_F) ? 0.f : expf(y.mz - o.mz);
   o.sz = x.sz * fx + y.sz * fy;
+  o.mr = fmaxf(x.mr, y.mr);
+  const float gx = (x.mr == -CUDART_INF_F) ? 0.f : expf(x.mr - o.mr);
+  const float gy = (y.mr == -CUDART_INF_F) ? 0.f : expf(y.mr - o.mr);
+  o.sr = x.sr * gx + y.sr * gy;
+  o.b = x.b * gx + y.b * gy;
   return o;
 }
 
@@ -55,6 +68,9 @@ __device__ __forceinline__ RowStat warp_stat(RowStat s) {
     q.a = __shfl_xor_sync(0xffffffffu, s.a, o);
     q.mz = __shfl_xor_sync(0xffffffffu, s.mz, o);
     q.sz = __shfl_xor_sync(0xffffffffu, s.sz, o);
+    q.mr = __shfl_xor_sync(0xffffffffu, s.mr, o);
+    q.sr = __shfl_xor_sync(0xffffffffu, s.sr, o);
+    q.b = __shfl_xor_sync(0xffffffffu, s.b, o);
     s = stat_merge(s, q);
   }
   return s;
@@ -63,11 +79,13 @@ __device__ __forceinline__ RowStat warp_stat(RowStat s) {
 // grid (splits, T), 256 threads.  128-bit loads of the teacher (8 bf16 / 4 fp32) and of z (2 x / 1 x float4).
 template <bool BF16>
 __global__ void __launch_bounds__(256) row_stats_partial_kernel(const void* __restrict__ teacher,
-                                                                const float* __restrict__ z, int V, int z_ld,
+                                                                const float* __restrict__ z,
+                                                                const float* __restrict__ z_ref, int V, int z_ld,
                                                                 int chunk, float* __restrict__ part) {
   const int r = blockIdx.y, sp = blockIdx.x;
   const int v0 = sp * chunk, v1 = min(V, v0 + chunk);
   const float* zr = z + (size_t)r * z_ld;
+  const float* zf = z_ref ? z_ref + (size_t)r * z_ld : nullptr;
   RowStat s;
   stat_init(s);
   if (BF16) {
@@ -83,8 +101,18 @@ __global__ void __launch_bounds__(256) row_stats_partial_kernel(const void* __re
       const float zz[8] = {z0.x, z0.y, z0.z, z0.w, z1.x, z1.y, z1.z, z1.w};
 #pragma unroll
       for (int k = 0; k < 8; ++k) stat_push(s, f[k], zz[k]);
+      if (zf) {
+        const float4 r0 = __ldg(reinterpret_cast<const float4*>(zf + v0) + 2 * i);
+        const float4 r1 = __ldg(reinterpret_cast<const float4*>(zf + v0) + 2 * i + 1);
+        const float rr[8] = {r0.x, r0.y, r0.z, r0.w, r1.x, r1.y, r1.z, r1.w};
+#pragma unroll
+        for (int k = 0; k < 8; ++k) stat_push_ref(s, rr[k], zz[k]);
+      }
     }
-    for (int v = v0 + nvec * 8 + threadIdx.x; v < v1; v += blockDim.x) stat_push(s, __bfloat162float(row[v]), zr[v]);
+    for (int v = v0 + nvec * 8 + threadIdx.x; v < v1; v += blockDim.x) {
+      stat_push(s, __bfloat162float(row[v]), zr[v]);
+      if (zf) stat_push_ref(s, zf[v], zr[v]);
+    }
   } else {
     const float* row = static_cast<const float*>(teacher) + (size_t)r * V;
     const int nvec = (v1 - v0) / 4;
@@ -94,8 +122,16 @@ __global__ void __launch_bounds__(256) row_stats_partial_kernel(const void* __re
       const float4 q = __ldg(pt + i);
       const float4 z0 = __ldg(pz + i);
       stat_push(s, q.x, z0.x); stat_push(s, q.y, z0.y); stat_push(s, q.z, z0.z); stat_push(s, q.w, z0.w);
+      if (zf) {
+        const float4 r0 = __ldg(reinterpret_cast<const float4*>(zf + v0) + i);
+        stat_push_ref(s, r0.x, z0.x); stat_push_ref(s, r0.y, z0.y); stat_push_ref(s, r0.z, z0.z);
+        stat_push_ref(s, r0.w, z0.w);
+      }
     }
-    for (int v = v0 + nvec * 4 + threadIdx.x; v < v1; v += blockDim.x) stat_push(s, row[v], zr[v]);
+    for (int v = v0 + nvec * 4 + threadIdx.x; v < v1; v += blockDim.x) {
+      stat_push(s, row[v], zr[v]);
+      if (zf) stat_push_ref(s, zf[v], zr[v]);
+    }
   }
   __shared__ RowStat sh[8];
   s = warp_stat(s);
@@ -109,67 +145,87 @@ __global__ void __launch_bounds__(256) row_stats_partial_kernel(const void* __re
     q = warp_stat(q);
     if (lane == 0) {
       float* o = part + ((size_t)r * gridDim.x + sp) * kStatFields;
-      o[0] = q.mt; o[1] = q.st; o[2] = q.a; o[3] = q.mz; o[4] = q.sz;
+      o[0] = q.mt; o[1] = q.st; o[2] = q.a; o[3] = q.mz; o[4] = q.sz; o[5] = q.mr; o[6] = q.sr; o[7] = q.b;
     }
   }
 }
 
-// One CTA.  row_stats layout: [0]=lse_t, [1]=lse_z, [2]=kl, [3]=coef, each [T_max].
-__global__ void __launch_bounds__(256) row_stats_merge_kernel(const float* __restrict__ part, int splits, int T,
-                                                              int T_max, int seg_len, int mask_mode,
-                                                              const float* __restrict__ pos_weight,
-                                                              const uint8_t* __restrict__ mask, float loss_scale,
-                                                              float* __restrict__ row_stats,
-                                                              float* __restrict__ kl_rows_out,
-                                                              float* __restrict__ loss_out) {
-  __shared__ double red[256];
+// One CTA of 32 warps; a warp merges one row at a time with its lanes spread over the V-splits.
+// row_stats planes ([kRowStatFields][T_max]): 0 = lse_t, 1 = lse_z, 2 = kl, 3 = coef (= loss_scale * omega), 4 = lse_ref.
+// The maxima are exact in fp32; the rescaled sums and the final a / s_t - lse_t + lse_z (a difference of numbers
+// ~10 for a result that can be ~0.01) are formed in double.  With z_ref (has_ref) the loss gains
+// lambda * sum_r omega_r K~L(q_ref || q)_r.
+__global__ void __launch_bounds__(1024) row_stats_merge_kernel(const float* __restrict__ part, int splits, int T,
+                                                               int T_max, int seg_len, int mask_mode,
+                                                               const float* __restrict__ pos_weight,
+                                                               const uint8_t* __restrict__ mask, float loss_scale,
+                                                               int has_ref, float lambda,
+                                                               float* __restrict__ row_stats,
+                                                               float* __restrict__ kl_rows_out,
+                                                               float* __restrict__ loss_out) {
+  __shared__ double red[32];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
   double local = 0.0;
-  for (int r = threadIdx.x; r < T; r += blockDim.x) {
-    // merge in double: the partials are few and this fixes the cancellation in a/s_t - lse_t + lse_z
-    double mt = -CUDART_INF, st = 0.0, a = 0.0, mz = -CUDART_INF, sz = 0.0;
-    for (int s = 0; s < splits; ++s) {
-      const float* p = part + ((size_t)r * splits + s) * kStatFields;
-      const double pmt = p[0], pst = p[1], pa = p[2], pmz = p[3], psz = p[4];
-      if (pmt != -CUDART_INF) {
-        const double nm = fmax(mt, pmt);
-        const double e0 = (mt == -CUDART_INF) ? 0.0 : exp(mt - nm), e1 = exp(pmt - nm);
-        st = st * e0 + pst * e1; a = a * e0 + pa * e1; mt = nm;
+  for (int r = warp; r < T; r += n_warps) {
+    const float* pr = part + (size_t)r * splits * kStatFields;
+    float mt = -CUDART_INF_F, mz = -CUDART_INF_F, mr = -CUDART_INF_F;
+    for (int s = lane; s < splits; s += 32) {
+      const float* p = pr + s * kStatFields;
+      mt = fmaxf(mt, p[0]); mz = fmaxf(mz, p[3]); mr = fmaxf(mr, p[5]);
+    }
+    mt = warp_max(mt); mz = warp_max(mz); mr = warp_max(mr);
+    double st = 0.0, a = 0.0, sz = 0.0, sr = 0.0, b = 0.0;
+    for (int s = lane; s < splits; s += 32) {
+      const float* p = pr + s * kStatFields;
+      if (p[0] != -CUDART_INF_F) {
+        const double e = exp((double)p[0] - (double)mt);
+        st += (double)p[1] * e; a += (double)p[2] * e;
       }
-      if (pmz != -CUDART_INF) {
-        const double nm = fmax(mz, pmz);
-        const double e0 = (mz == -CUDART_INF) ? 0.0 : exp(mz - nm), e1 = exp(pmz - nm);
-        sz = sz * e0 + psz * e1; mz = nm;
+      if (p[3] != -CUDART_INF_F) sz += (double)p[4] * exp((double)p[3] - (double)mz);
+      if (has_ref && p[5] != -CUDART_INF_F) {
+        const double e = exp((double)p[5] - (double)mr);
+        sr += (double)p[6] * e; b += (double)p[7] * e;
       }
     }
-    const double lse_t = mt + log(st), lse_z = mz + log(sz);
-    const double kl = a / st - lse_t + lse_z;
-    // omega_r = w_k * mask factor (R2)
-    double f = 1.0;
-    if (mask_mode != TTS_ROWS_ALL) {
-      f = mask[r] ? 1.0 : 0.0;
-      if (mask_mode == TTS_ROWS_ACCEPTED_PLUS_ONE && !mask[r]) {
-        const int k = r % seg_len;
-        if (k == 0 || mask[r - 1]) f = 1.0;   // the first rejected row of the segment
+    st = warp_sum(st); a = warp_sum(a); sz = warp_sum(sz);
+    if (has_ref) { sr = warp_sum(sr); b = warp_sum(b); }
+    if (lane == 0) {
+      const double lse_t = (double)mt + log(st), lse_z = (double)mz + log(sz);
+      const double kl = a / st - lse_t + lse_z;
+      double lse_ref = 0.0, kl_ref = 0.0;
+      if (has_ref) {
+        lse_ref = (double)mr + log(sr);
+        kl_ref = b / sr - lse_ref + lse_z;
       }
+      // omega_r = w_k * mask factor (R2)
+      double f = 1.0;
+      if (mask_mode != TTS_ROWS_ALL) {
+        f = mask[r] ? 1.0 : 0.0;
+        if (mask_mode == TTS_ROWS_ACCEPTED_PLUS_ONE && !mask[r]) {
+          const int k = r % seg_len;
+          if (k == 0 || mask[r - 1]) f = 1.0;   // the first rejected row of the segment
+        }
+      }
+      const double omega = (double)pos_weight[r] * f;
+      row_stats[0 * T_max + r] = (float)lse_t;
+      row_stats[1 * T_max + r] = (float)lse_z;
+      row_stats[2 * T_max + r] = (float)kl;
+      row_stats[3 * T_max + r] = (float)((double)loss_scale * omega);
+      row_stats[4 * T_max + r] = (float)lse_ref;
+      if (kl_rows_out) kl_rows_out[r] = (float)kl;
+      local += omega * (kl + (double)lambda * kl_ref);
     }
-    const double omega = (double)pos_weight[r] * f;
-    row_stats[0 * T_max + r] = (float)lse_t;
-    row_stats[1 * T_max + r] = (float)lse_z;
-    row_stats[2 * T_max + r] = (float)kl;
-    row_stats[3 * T_max + r] = (float)((double)loss_scale * omega);
-    if (kl_rows_out) kl_rows_out[r] = (float)kl;
-    local += omega * kl;
   }
-  red[threadIdx.x] = local;
+  if (lane == 0) red[warp] = local;
   __syncthreads();
-  for (int o = 128; o > 0; o >>= 1) {
-    if (threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
-    __syncthreads();
+  if (threadIdx.x == 0) {
+    double sum = 0.0;
+    for (int w = 0; w < n_warps; ++w) sum += red[w];   // fixed order
+    loss_out[0] = (float)((double)loss_scale * sum);
   }
-  if (threadIdx.x == 0) loss_out[0] = (float)((double)loss_scale * red[0]);
 }
 
-cudaError_t launch_row_stats(tts_ctx* c, const StepArgs& a, int z_ld, cudaStream_t s, int* launches) {
+cudaError_t launch_row_stats(tts_ctx* c, const StepArgs& a, const float* z, int z_ld, cudaStream_t s, int* launches) {
   const int V = c->cfg.V, T = a.T;
   int splits = (2 * c->sm_count + T - 1) / T;
   splits = max(1, min(splits, kStatSplitsMax));
@@ -178,12 +234,13 @@ cudaError_t launch_row_stats(tts_ctx* c, const StepArgs& a, int z_ld, cudaStream
   splits = (V + chunk - 1) / chunk;
   dim3 grid(splits, T);
   if (c->cfg.logits_dtype == TTS_BF16)
-    row_stats_partial_kernel<true><<<grid, 256, 0, s>>>(a.teacher, c->z, V, z_ld, chunk, c->stat_part);
+    row_stats_partial_kernel<true><<<grid, 256, 0, s>>>(a.teacher, z, a.z_ref, V, z_ld, chunk, c->stat_part);
   else
-    row_stats_partial_kernel<false><<<grid, 256, 0, s>>>(a.teacher, c->z, V, z_ld, chunk, c->stat_part);
-  row_stats_merge_kernel<<<1, 256, 0, s>>>(c->stat_part, splits, T, c->cfg.T_max, c->cfg.seg_len, c->cfg.mask_mode,
-                                           a.pos_weight, a.mask, a.loss_scale, c->row_stats, a.kl_rows_out,
-                                           a.loss_out);
+    row_stats_partial_kernel<false><<<grid, 256, 0, s>>>(a.teacher, z, a.z_ref, V, z_ld, chunk, c->stat_part);
+  row_stats_merge_kernel<<<1, T >= 32 ? 1024 : 32 * T, 0, s>>>(c->stat_part, splits, T, c->cfg.T_max, c->cfg.seg_len,
+                                                              c->cfg.mask_mode, a.pos_weight, a.mask, a.loss_scale,
+                                                              a.z_ref != nullptr, a.lambda, c->row_stats,
+                                                              a.kl_rows_out, a.loss_out);
   *launches += 2;
   return cudaGetLastError();
 }

@@ -35,15 +35,17 @@ constexpr int kUpdSmem = 1024 + 2 * kOpStages * kOpBytes + kStages * 3 * kStateT
 // One thread per vocabulary row v (coalesced over v for every canvas row r).
 template <bool BF16>
 __global__ void __launch_bounds__(256) tc_prep_dl_kernel(const void* __restrict__ teacher, const float* __restrict__ z,
+                                                         const float* __restrict__ z_ref, float lam,
                                                          int V, int z_ld, int T, int T16, int Kp, int T_max,
                                                          const float* __restrict__ row_stats,
                                                          __nv_bfloat16* __restrict__ dlT,
                                                          __nv_bfloat16* __restrict__ dlR, int P) {
-  extern __shared__ float sh[];   // lse_t[T16], lse_z[T16], coef[T16]
+  extern __shared__ float sh[];   // lse_t[T16], lse_z[T16], coef[T16], lse_ref[T16]
   for (int r = threadIdx.x; r < T16; r += blockDim.x) {
     sh[r] = r < T ? row_stats[0 * T_max + r] : 0.f;
     sh[T16 + r] = r < T ? row_stats[1 * T_max + r] : 0.f;
     sh[2 * T16 + r] = r < T ? row_stats[3 * T_max + r] : 0.f;
+    sh[3 * T16 + r] = r < T ? row_stats[4 * T_max + r] : 0.f;
   }
   __syncthreads();
   const int v = blockIdx.x * blockDim.x + threadIdx.x;
@@ -60,7 +62,9 @@ __global__ void __launch_bounds__(256) tc_prep_dl_kernel(const void* __restrict_
                              : static_cast<const float*>(teacher)[(size_t)r * V + v];
         const float q = expf(z[(size_t)r * z_ld + v] - sh[T16 + r]);
         const float p = expf(t - sh[r]);   // t = -inf -> 0
-        dl = sh[2 * T16 + r] * (q - p);
+        float g = q - p;
+        if (z_ref) g += lam * (q - expf(z_ref[(size_t)r * z_ld + v] - sh[3 * T16 + r]));
+        dl = sh[2 * T16 + r] * g;
       }
       const __nv_bfloat16 h = __float2bfloat16_rn(dl);
       const __nv_bfloat16 l = __float2bfloat16_rn(dl - __bfloat162float(h));
@@ -333,30 +337,31 @@ cudaError_t tc_step(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches
   const bool adam = c->cfg.optimizer == TTS_ADAMW;
   cudaError_t e;
 
-  // a2: draft logits on tcgen05, a3: row statistics + loss
-  if ((e = tc_launch_logits(c, a, s, launches)) != cudaSuccess) return e;
+  // a2: draft logits on tcgen05 (skipped when the caller supplies them), a3: row statistics + loss
+  const float* z = z_src(a, c->z);
+  if (!a.z_given && (e = tc_launch_logits(c, a, z_dst(a, c->z), s, launches)) != cudaSuccess) return e;
   prof_mark(c, 0, s);
-  if ((e = launch_row_stats(c, a, V, s, launches)) != cudaSuccess) return e;
+  if ((e = launch_row_stats(c, a, z, V, s, launches)) != cudaSuccess) return e;
   prof_mark(c, 1, s);
 
   // a4: operands of the gradient contractions
   // one canvas (T <= 16): one fused pass over the optimiser state (tts_tc_fused.cu) with its own pre-tiled operands
   const int fused_grid = tc_fused_grid(c, T16);
   if (fused_grid > 0) {
-    if ((e = tc_launch_prep_fused(c, a, s, launches)) != cudaSuccess) return e;
+    if ((e = tc_launch_prep_fused(c, a, z, s, launches)) != cudaSuccess) return e;
     prof_mark(c, 2, s);
     prof_mark(c, 3, s);
     if ((e = tc_launch_update_fused(c, a, fused_grid, s, launches)) != cudaSuccess) return e;
     prof_mark(c, 4, s);
     return cudaGetLastError();
   }
-  const size_t sh = 3 * T16 * sizeof(float);
+  const size_t sh = 4 * T16 * sizeof(float);
   __nv_bfloat16* dlR = a.gh_out ? st->dlR : nullptr;
   if (c->cfg.logits_dtype == TTS_BF16)
-    tc_prep_dl_kernel<true><<<(V + 255) / 256, 256, sh, s>>>(a.teacher, c->z, V, V, T, T16, st->Kp, c->cfg.T_max,
+    tc_prep_dl_kernel<true><<<(V + 255) / 256, 256, sh, s>>>(a.teacher, z, a.z_ref, a.lambda, V, V, T, T16, st->Kp, c->cfg.T_max,
                                                                c->row_stats, st->dlT, dlR, st->P);
   else
-    tc_prep_dl_kernel<false><<<(V + 255) / 256, 256, sh, s>>>(a.teacher, c->z, V, V, T, T16, st->Kp, c->cfg.T_max,
+    tc_prep_dl_kernel<false><<<(V + 255) / 256, 256, sh, s>>>(a.teacher, z, a.z_ref, a.lambda, V, V, T, T16, st->Kp, c->cfg.T_max,
                                                                 c->row_stats, st->dlT, dlR, st->P);
   *launches += 1;
   tc_prep_h_kernel<<<(d + 255) / 256, 256, 0, s>>>(static_cast<const __nv_bfloat16*>(a.h), d, T, T16, st->Kp,

@@ -383,15 +383,17 @@ __global__ void __launch_bounds__(256) tc_prep_hc_kernel(const __nv_bfloat16* __
 // One thread per vocabulary row v (loads coalesced over v for every canvas row r).
 template <bool BF16>
 __global__ void __launch_bounds__(256) tc_prep_dlc_kernel(const void* __restrict__ teacher, const float* __restrict__ z,
+                                                          const float* __restrict__ z_ref, float lam,
                                                           int V, int z_ld, int T, int T_max,
                                                           const float* __restrict__ row_stats,
                                                           __nv_bfloat16* __restrict__ dlC) {
-  __shared__ float sh[3 * kT16];   // lse_t, lse_z, coef
+  __shared__ float sh[4 * kT16];   // lse_t, lse_z, coef, lse_ref
   if (threadIdx.x < kT16) {
     const int r = threadIdx.x;
     sh[r] = r < T ? row_stats[0 * T_max + r] : 0.f;
     sh[kT16 + r] = r < T ? row_stats[1 * T_max + r] : 0.f;
     sh[2 * kT16 + r] = r < T ? row_stats[3 * T_max + r] : 0.f;
+    sh[3 * kT16 + r] = r < T ? row_stats[4 * T_max + r] : 0.f;
   }
   __syncthreads();
   const int v = blockIdx.x * blockDim.x + threadIdx.x;
@@ -405,7 +407,9 @@ __global__ void __launch_bounds__(256) tc_prep_dlc_kernel(const void* __restrict
                            : static_cast<const float*>(teacher)[(size_t)r * V + v];
       const float qv = expf(z[(size_t)r * z_ld + v] - sh[kT16 + r]);
       const float pv = expf(t - sh[r]);   // t = -inf -> 0
-      dl = sh[2 * kT16 + r] * (qv - pv);
+      float g = qv - pv;
+      if (z_ref) g += lam * (qv - expf(z_ref[(size_t)r * z_ld + v] - sh[3 * kT16 + r]));
+      dl = sh[2 * kT16 + r] * g;
     }
     const __nv_bfloat16 hi = __float2bfloat16_rn(dl);
     const __nv_bfloat16 lo = __float2bfloat16_rn(dl - __bfloat162float(hi));
@@ -439,16 +443,16 @@ int tc_fused_grid(const tts_ctx* c, int T16) {
 }
 
 // a4: the operands of the fused pass (h^T tiles and the pre-tiled dl planes)
-cudaError_t tc_launch_prep_fused(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches) {
+cudaError_t tc_launch_prep_fused(tts_ctx* c, const StepArgs& a, const float* z, cudaStream_t s, int* launches) {
   TcState* st = static_cast<TcState*>(c->tc_state);
   const int V = c->cfg.V, d = c->cfg.d;
   tc_prep_hc_kernel<<<(d + 255) / 256, 256, 0, s>>>(static_cast<const __nv_bfloat16*>(a.h), d, a.T, st->hTc);
   if (c->cfg.logits_dtype == TTS_BF16)
-    tc_prep_dlc_kernel<true><<<(V + 255) / 256, 256, 0, s>>>(a.teacher, c->z, V, V, a.T, c->cfg.T_max, c->row_stats,
-                                                              st->dlC);
+    tc_prep_dlc_kernel<true><<<(V + 255) / 256, 256, 0, s>>>(a.teacher, z, a.z_ref, a.lambda, V, V, a.T, c->cfg.T_max,
+                                                              c->row_stats, st->dlC);
   else
-    tc_prep_dlc_kernel<false><<<(V + 255) / 256, 256, 0, s>>>(a.teacher, c->z, V, V, a.T, c->cfg.T_max, c->row_stats,
-                                                               st->dlC);
+    tc_prep_dlc_kernel<false><<<(V + 255) / 256, 256, 0, s>>>(a.teacher, z, a.z_ref, a.lambda, V, V, a.T, c->cfg.T_max,
+                                                               c->row_stats, st->dlC);
   *launches += 2;
   return cudaGetLastError();
 }

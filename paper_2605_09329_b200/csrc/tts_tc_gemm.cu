@@ -367,12 +367,12 @@ cudaError_t tc_gemm_init(tts_ctx*) {
   return cudaFuncSetAttribute(tc_gh_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max);
 }
 
-cudaError_t tc_launch_logits(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches) {
+cudaError_t tc_launch_logits(tts_ctx* c, const StepArgs& a, float* z_out, cudaStream_t s, int* launches) {
   TcState* st = static_cast<TcState*>(c->tc_state);
   const int V = c->cfg.V, d = c->cfg.d, T = a.T;
   const int T16 = (T + 15) / 16 * 16;
   LogitsParams p;
-  p.z = c->z; p.z_ld = V;
+  p.z = z_out; p.z_ld = V;
   p.n_vt = V / kTileMN; p.k_chunks = d / kKC; p.T16 = T16;
   p.box_rows = T16 <= kNMax ? T16 : kNMax;
   p.n_boxes = (T16 + p.box_rows - 1) / p.box_rows;
@@ -395,7 +395,7 @@ cudaError_t tc_launch_logits(tts_ctx* c, const StepArgs& a, cudaStream_t s, int*
   // once: it receives exactly two partial sums (or one store), and 0 + a + b does not depend on the order.
   p.stream_k = T16 <= 32 && p.n_vt % grid != 0;
   if (p.stream_k) {
-    cudaError_t e = cudaMemsetAsync(c->z, 0, (size_t)T16 * V * sizeof(float), s);
+    cudaError_t e = cudaMemsetAsync(z_out, 0, (size_t)T16 * V * sizeof(float), s);
     if (e != cudaSuccess) return e;
   }
   const size_t smem = 1024 + (size_t)p.stages * stage_bytes + sizeof(Bars);

@@ -41,14 +41,14 @@ inline CUresult make_map_2d(const TcState* st, CUtensorMap* m, CUtensorMapDataTy
 // tts_tc_gemm.cu
 cudaError_t tc_gemm_init(tts_ctx* c);
 // a2: z[r, v] = sum_j h[r, j] W_in[v, j] on tcgen05 (fp32 accumulation), z scratch [T16, V]
-cudaError_t tc_launch_logits(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches);
+cudaError_t tc_launch_logits(tts_ctx* c, const StepArgs& a, float* z_out, cudaStream_t s, int* launches);
 // a5: gh[r, j] = sum_v (dl_hi + dl_lo)[r, v] W_in[v, j] on tcgen05, split over the vocabulary, fp32 atomics into gh
 cudaError_t tc_launch_gh(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches);
 
 // tts_tc_fused.cu: a5 + a6 + a7 in one pass over the optimiser state (T <= 16, d % 1024 == 0, V % 16 == 0)
 cudaError_t tc_fused_init(tts_ctx* c);
 int tc_fused_grid(const tts_ctx* c, int T16);
-cudaError_t tc_launch_prep_fused(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches);   // a4: operands
+cudaError_t tc_launch_prep_fused(tts_ctx* c, const StepArgs& a, const float* z, cudaStream_t s, int* launches);   // a4: operands
 cudaError_t tc_launch_update_fused(tts_ctx* c, const StepArgs& a, int grid, cudaStream_t s, int* launches);
 
 }  // namespace tts

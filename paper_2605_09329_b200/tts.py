@@ -22,6 +22,11 @@ TTS_NUM_PHASES = 5
 PHASE_NAMES = ("a2_logits", "a3_row_stats", "a4_dlogits", "a5_gh", "a6a7_gW_update")
 
 
+class tts_step_extras(C.Structure):
+    _fields_ = [("draft_logits", C.c_void_p), ("draft_logits_out", C.c_void_p), ("ref_logits", C.c_void_p),
+                ("lambda_", C.c_float)]
+
+
 class tts_config(C.Structure):
     _fields_ = [("V", C.c_int32), ("d", C.c_int32), ("T_max", C.c_int32), ("seg_len", C.c_int32),
                 ("param_dtype", C.c_int32), ("logits_dtype", C.c_int32), ("optimizer", C.c_int32),
@@ -44,6 +49,9 @@ EXPORTS = {
     "tts_last_launch_count": (C.c_int32, [C.c_void_p]),
     "tts_accept_mask": (C.c_int32, [C.c_void_p] * 3 + [C.c_int32] + [C.c_void_p] * 4),
     "tts_distill_step": (C.c_int32, [C.c_void_p] * 10 + [C.c_int32, C.c_float] + [C.c_void_p] * 5),
+    "tts_distill_step_ex": (C.c_int32, [C.c_void_p] * 10 + [C.c_int32, C.c_float] + [C.c_void_p] * 6),
+    "tts_distill_inner_steps": (C.c_int32, [C.c_void_p] * 10 + [C.c_int32, C.c_float, C.c_int32, C.c_float] +
+                                [C.c_void_p] * 5),
     "tts_profile_enable": (C.c_int32, [C.c_void_p, C.c_int32]),
     "tts_profile_read": (C.c_int32, [C.c_void_p, C.POINTER(C.c_float), C.POINTER(C.c_int32)]),
     "tts_wait_step": (C.c_int32, [C.c_void_p, C.c_void_p]),
@@ -159,6 +167,27 @@ def tts_distill_step(ctx, teacher_logits, h, W_in, W_out, W_master, adam_m, adam
                                 _ptr(loss_out), _ptr(kl_rows_out), _ptr(gh_out), _ptr(gW_debug_out),
                                 _stream(side_stream))
     _check(ctx, st, "tts_distill_step")
+
+
+def tts_distill_step_ex(ctx, teacher_logits, h, W_in, W_out, W_master, adam_m, adam_v, pos_weight, mask, T, loss_scale,
+                        loss_out, kl_rows_out=None, gh_out=None, gW_debug_out=None, *, draft_logits=None,
+                        draft_logits_out=None, ref_logits=None, lam=0.0, side_stream=None):
+    ex = tts_step_extras(_ptr(draft_logits), _ptr(draft_logits_out), _ptr(ref_logits), lam)
+    st = lib().tts_distill_step_ex(ctx, _ptr(teacher_logits), _ptr(h), _ptr(W_in), _ptr(W_out), _ptr(W_master),
+                                   _ptr(adam_m), _ptr(adam_v), _ptr(pos_weight), _ptr(mask), T, loss_scale,
+                                   _ptr(loss_out), _ptr(kl_rows_out), _ptr(gh_out), _ptr(gW_debug_out),
+                                   C.addressof(ex), _stream(side_stream))
+    _check(ctx, st, "tts_distill_step_ex")
+
+
+def tts_distill_inner_steps(ctx, teacher_logits, h, W_in, W_out, W_master, adam_m, adam_v, pos_weight, mask, T,
+                            loss_scale, K, lam, draft_logits, loss_out, kl_rows_out=None, gh_out=None,
+                            side_stream=None):
+    st = lib().tts_distill_inner_steps(ctx, _ptr(teacher_logits), _ptr(h), _ptr(W_in), _ptr(W_out), _ptr(W_master),
+                                       _ptr(adam_m), _ptr(adam_v), _ptr(pos_weight), _ptr(mask), T, loss_scale, K,
+                                       lam, _ptr(draft_logits), _ptr(loss_out), _ptr(kl_rows_out), _ptr(gh_out),
+                                       _stream(side_stream))
+    _check(ctx, st, "tts_distill_inner_steps")
 
 
 def tts_profile_enable(ctx, enable: int):

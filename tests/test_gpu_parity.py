@@ -78,7 +78,8 @@ SMALL = [
     (3, 2048, 128, 1, 8, {}),                        # T = 8 (EAGLE-3 depth), padded to 16 rows
     (4, 2048, 256, 4, 16, {}),                       # batched: 64 rows, loss_scale 1/32
     (2, 1000, 72, 1, 16, {}),                        # shape outside the tensor-core tiles -> CUDA-core kernels
-    (3, 2048 + 16 * 5, 1024, 1, 16, {}),             # fused stripe kernel: one 1024-column stripe, ragged band count
+    (3, 2048 + 16 * 5, 1024, 1, 16, {}),             # V % 128 != 0: CUDA-core kernels at d = 1024
+    (3, 2048 + 128 * 3, 1024, 1, 16, {}),            # fused stripe kernel: one 1024-column stripe, 152 bands over 148 CTAs
     (3, 1024 + 128, 2048, 1, 8, {}),                 # fused stripe kernel: two stripes, T = 8 padded to 16 rows
 ]
 
@@ -149,10 +150,11 @@ def test_gh_and_gw_outputs_optional(d):
 def test_fused_kernel_with_capped_grid(max_ctas):
     """max_ctas (the SM budget the main stream keeps) changes how stripes and bands are walked,
     not the result.  3 and 7 are not multiples of the stripe count."""
-    case = synth.make_case(3, V=1024 + 16, d=2048, nonzero_state=True, step=2)
+    case = synth.make_case(3, V=1024 + 128, d=2048, nonzero_state=True, step=2)
     g = run_gpu(case, max_ctas=max_ctas)
     o = run_oracle(case)
     check_step(g, o, case)
+    assert g["used_tensor"] == 1
 
 
 def test_fused_kernel_sgd_alias_d1024():

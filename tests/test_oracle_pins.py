@@ -290,6 +290,55 @@ def test_sgd_matches_torch_optim():
     np.testing.assert_allclose(O.sgd_update(M, g, 1e-3), Mt.detach().numpy(), rtol=1e-15)
 
 
+def test_inner_steps_match_torch_autograd_adamw_loop():
+    """K steps with the lambda term against an fp64 torch loop: autograd on
+    sum_r w_r [KL(p||q) + lam KL(q_t||q)] + torch.optim.AdamW (the paper's own implementation is standard
+    PyTorch kernels).  fp32 parameters (no master) so no rounding sits between steps."""
+    T, V, d, K, lam = 4, 23, 6, 3, 0.7
+    t, h, W, om = _small(21, T, V, d)
+    W32, h32 = W.astype(np.float32), h.astype(np.float32)
+    Wt = torch.tensor(W32.astype(np.float64), requires_grad=True)
+    ht = torch.tensor(h32.astype(np.float64))
+    tt, omt = torch.tensor(t), torch.tensor(om)
+    opt = torch.optim.AdamW([Wt], lr=2e-3, betas=(0.9, 0.999), eps=1e-8, weight_decay=0.01)
+    with torch.no_grad():
+        q_t = torch.softmax(ht @ Wt.T, -1)
+    losses = []
+    for k in range(K):
+        opt.zero_grad()
+        logq = torch.log_softmax(ht @ Wt.T, -1)
+        kl = torch.nn.functional.kl_div(logq, torch.softmax(tt, -1), reduction="none").sum(-1)
+        reg = torch.nn.functional.kl_div(logq, q_t, reduction="none").sum(-1)
+        loss = 0.5 * (omt * (kl + lam * reg)).sum()
+        loss.backward()
+        opt.step()
+        losses.append(loss.item())
+    r = O.distill_inner_steps(t, h32, W32, None, np.zeros((V, d)), np.zeros((V, d)), om, None, K=K, lam=lam,
+                              seg_len=T, loss_scale=0.5, optimizer="adamw", lr=2e-3, weight_decay=0.01)
+    np.testing.assert_allclose(r["losses"], losses, rtol=1e-6)   # W_out is fp32-rounded between steps, torch is not
+    # W_out is fp32-rounded every step (the parameters ARE fp32 here): agreement to fp32 rounding of three steps
+    np.testing.assert_allclose(r["W_out"], Wt.detach().numpy(), rtol=0, atol=3e-7)
+    assert r["losses"][1] < r["losses"][0]            # the same signal again: the loss falls
+
+
+def test_given_draft_logits_replace_the_product():
+    """draft_logits given: identical to the computed path when they ARE h W^T; otherwise gW, gh
+    follow dl of the given logits (pinned through the chain rule: gW = dl^T h with dl from softmax(z_given))."""
+    T, V, d = 3, 11, 4
+    t, h, W, om = _small(22, T, V, d)
+    a = O.loss_and_grads(t, h, W, om)
+    b = O.loss_and_grads(t, h, W, om, z=h @ W.T)
+    for k in ("loss", "gW", "gh", "dl"):
+        np.testing.assert_allclose(b[k], a[k], rtol=1e-13, atol=1e-16)
+    zg = h @ W.T + 0.1 * _rng(5).standard_normal((T, V))
+    c = O.loss_and_grads(t, h, W, om, z=zg)
+    q = np.exp(zg - zg.max(1, keepdims=True)); q /= q.sum(1, keepdims=True)
+    p = np.exp(t - t.max(1, keepdims=True)); p /= p.sum(1, keepdims=True)
+    np.testing.assert_allclose(c["dl"], om[:, None] * (q - p), rtol=1e-12, atol=1e-15)
+    np.testing.assert_allclose(c["gW"], (om[:, None] * (q - p)).T @ h, rtol=1e-12, atol=1e-15)
+    assert c["loss"] == pytest.approx(float((om * (p * (np.log(p) - np.log(q))).sum(1)).sum()), rel=1e-12)
+
+
 def test_bf16_rounding_matches_torch():
     r = _rng(18)
     x = np.concatenate([r.standard_normal(20000).astype(np.float32) * 10.0 ** r.integers(-8, 4),
