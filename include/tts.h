@@ -125,6 +125,31 @@ int32_t tts_accept_mask(tts_ctx* ctx,
                         void* stream);
 
 /*
+ * f2.  The paper's own accept rule, "standard speculative rejection sampling" (Alg. 1):
+ * canvas tokens are considered left to right, x_{t+k} is accepted with probability min{1, p(x_{t+k}) / q(x_{t+k})},
+ * and the loop breaks at the first rejection.  p = softmax(teacher_logits[r]), q =
+ * softmax(draft_logits[r]) -- after a round both are at hand.  Randomness is the caller's:
+ *   uniforms[r]           U[0,1): row r is accepted iff every earlier row of its sequence was and
+ *                         uniforms[r] * q_r(tok_r) <= p_r(tok_r)            (fp32 products of fp64-normalised p, q)
+ *   uniforms_resample[s]  U[0,1): at the first rejected row of sequence s the replacement token is drawn from the
+ *                         residual distribution norm(max(0, p - q)) by inverse CDF over the vocabulary order: the
+ *                         smallest v with sum_{v' <= v} max(0, p - q) >= u * sum_v max(0, p - q)
+ *   next_token_out[s]     that token; -1 when the whole canvas was accepted (the bonus token needs the target's
+ *                         distribution at position C + 1, which this call does not see)
+ *   diag_out [T,4] or NULL: the diagnostics of the paper's section 3 (Fig. 4), free by-products of
+ *                         the same vocabulary sweep:  H(p_r) in nats,  -log q_r(argmax_v p_r),  p_r(tok_r),  q_r(tok_r)
+ * tau_out / mask_out as in tts_accept_mask.  draft_logits: [T,V] fp32, row stride V (V % 4 == 0).
+ */
+int32_t tts_accept_stochastic(tts_ctx* ctx,
+                              const void* teacher_logits,     /* [T,V] logits_dtype                  */
+                              const float* draft_logits,      /* [T,V] fp32                          */
+                              const int32_t* draft_tokens,    /* [T]                                 */
+                              const float* uniforms,          /* [T]                                 */
+                              const float* uniforms_resample, /* [T/seg_len]                         */
+                              int32_t T, uint8_t* mask_out, int32_t* tau_out, int32_t* next_token_out,
+                              float* diag_out, void* stream);
+
+/*
  * a2-a8.  One TTS update (Alg. 1 "Loss" + "Update"):
  *   z      = h W_in^T                                   draft logits at q = q_t
  *   KL_r   = KL(softmax(teacher_r) || softmax(z_r)), -inf teacher entries = p 0

@@ -30,6 +30,7 @@ void free_all(tts_ctx* c) {
   tts::tc_destroy(c);
   cudaFree(c->z); cudaFree(c->z_ref_buf); cudaFree(c->dl32); cudaFree(c->stat_part); cudaFree(c->row_stats);
   cudaFree(c->arg_val); cudaFree(c->arg_idx); cudaFree(c->argmax_tmp);
+  cudaFree(c->acc_rows); cudaFree(c->acc_rej); cudaFree(c->acc_rpart);
   cudaFree(c->st_teacher); cudaFree(c->st_h); cudaFree(c->st_tok); cudaFree(c->st_pw);
   cudaFree(c->st_mask); cudaFree(c->st_tau); cudaFree(c->st_loss);
   if (c->done_event) cudaEventDestroy(c->done_event);
@@ -99,6 +100,9 @@ int32_t tts_ctx_create(const tts_config* cfg, int32_t device, tts_ctx** out) {
   ok = ok && dmalloc(&c->arg_val, Tm * tts::kArgSplitsMax) == cudaSuccess;
   ok = ok && dmalloc(&c->arg_idx, Tm * tts::kArgSplitsMax) == cudaSuccess;
   ok = ok && dmalloc(&c->argmax_tmp, Tm) == cudaSuccess;
+  ok = ok && dmalloc(&c->acc_rows, 2 * Tm) == cudaSuccess;
+  ok = ok && dmalloc(&c->acc_rej, Tm / cfg->seg_len) == cudaSuccess;
+  ok = ok && dmalloc(&c->acc_rpart, (Tm / cfg->seg_len) * tts::kStatSplitsMax) == cudaSuccess;
   // staging for tts_round_host
   ok = ok && cudaMalloc(&c->st_teacher, Tm * V * elem_size(cfg->logits_dtype)) == cudaSuccess;
   ok = ok && cudaMalloc(&c->st_h, Tm * cfg->d * elem_size(cfg->param_dtype)) == cudaSuccess;
@@ -152,6 +156,24 @@ int32_t tts_accept_mask(tts_ctx* c, const void* teacher, const int32_t* tok, int
   int launches = 0;
   cudaError_t e = tts::launch_accept_mask(c, teacher, tok, T, mask_out, tau_out, am_out,
                                           static_cast<cudaStream_t>(stream), &launches);
+  c->last_launches = launches;
+  if (e != cudaSuccess) return cuda_fail(c, e);
+  return TTS_OK;
+}
+
+int32_t tts_accept_stochastic(tts_ctx* c, const void* teacher, const float* draft_logits, const int32_t* tok,
+                              const float* uniforms, const float* uniforms_resample, int32_t T, uint8_t* mask_out,
+                              int32_t* tau_out, int32_t* next_token_out, float* diag_out, void* stream) {
+  if (!c || !teacher || !draft_logits || !tok || !uniforms || !uniforms_resample || !mask_out || !tau_out ||
+      !next_token_out)
+    return TTS_ERR_INVALID_ARG;
+  if (T <= 0 || T > c->cfg.T_max || T % c->cfg.seg_len != 0) return TTS_ERR_INVALID_ARG;
+  if (!aligned16(teacher) || !aligned16(draft_logits)) return TTS_ERR_INVALID_ARG;
+  if ((static_cast<size_t>(c->cfg.V) * sizeof(float)) % 16 != 0) return TTS_ERR_UNSUPPORTED;
+  int launches = 0;
+  cudaError_t e = tts::launch_accept_stochastic(c, teacher, draft_logits, tok, uniforms, uniforms_resample, T,
+                                                mask_out, tau_out, next_token_out, diag_out,
+                                                static_cast<cudaStream_t>(stream), &launches);
   c->last_launches = launches;
   if (e != cudaSuccess) return cuda_fail(c, e);
   return TTS_OK;

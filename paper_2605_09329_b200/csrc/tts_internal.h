@@ -71,6 +71,9 @@ struct tts_ctx {
   float* arg_val;         // [T_max, kArgSplitsMax]
   int32_t* arg_idx;       // [T_max, kArgSplitsMax]
   int32_t* argmax_tmp;    // [T_max]
+  float* acc_rows;        // [T_max, 2] lse_t, lse_z of tts_accept_stochastic
+  int32_t* acc_rej;       // [T_max / seg_len] first rejected row per sequence
+  double* acc_rpart;      // [T_max / seg_len, kStatSplitsMax] residual mass per slice
   // ---- staging for tts_round_host ----
   void* st_teacher;
   void* st_h;
@@ -99,6 +102,10 @@ inline void prof_mark(tts_ctx* c, int phase, cudaStream_t s) {
 // tts_mask.cu
 cudaError_t launch_accept_mask(tts_ctx* c, const void* teacher, const int32_t* tok, int T, uint8_t* mask,
                                int32_t* tau, int32_t* am_out, cudaStream_t s, int* launches);
+// tts_accept.cu (f2)
+cudaError_t launch_accept_stochastic(tts_ctx* c, const void* teacher, const float* z, const int32_t* tok,
+                                     const float* u, const float* u2, int T, uint8_t* mask, int32_t* tau,
+                                     int32_t* next_tok, float* diag, cudaStream_t s, int* launches);
 // tts_stats.cu: row statistics + merge + loss (CUDA-core sweeps shared by both paths).
 // z_ld = leading dimension (row stride in floats) of the z scratch.
 cudaError_t launch_row_stats(tts_ctx* c, const StepArgs& a, const float* z, int z_ld, cudaStream_t s, int* launches);

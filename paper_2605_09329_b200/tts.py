@@ -48,6 +48,7 @@ EXPORTS = {
     "tts_last_step_used_tensor_path": (C.c_int32, [C.c_void_p]),
     "tts_last_launch_count": (C.c_int32, [C.c_void_p]),
     "tts_accept_mask": (C.c_int32, [C.c_void_p] * 3 + [C.c_int32] + [C.c_void_p] * 4),
+    "tts_accept_stochastic": (C.c_int32, [C.c_void_p] * 6 + [C.c_int32] + [C.c_void_p] * 5),
     "tts_distill_step": (C.c_int32, [C.c_void_p] * 10 + [C.c_int32, C.c_float] + [C.c_void_p] * 5),
     "tts_distill_step_ex": (C.c_int32, [C.c_void_p] * 10 + [C.c_int32, C.c_float] + [C.c_void_p] * 6),
     "tts_distill_inner_steps": (C.c_int32, [C.c_void_p] * 10 + [C.c_int32, C.c_float, C.c_int32, C.c_float] +
@@ -158,6 +159,14 @@ def tts_accept_mask(ctx, teacher_logits, draft_tokens, T, mask_out, tau_out, tea
     st = lib().tts_accept_mask(ctx, _ptr(teacher_logits), _ptr(draft_tokens), T, _ptr(mask_out), _ptr(tau_out),
                                _ptr(teacher_argmax_out), _stream(stream))
     _check(ctx, st, "tts_accept_mask")
+
+
+def tts_accept_stochastic(ctx, teacher_logits, draft_logits, draft_tokens, uniforms, uniforms_resample, T, mask_out,
+                          tau_out, next_token_out, diag_out=None, stream=None):
+    st = lib().tts_accept_stochastic(ctx, _ptr(teacher_logits), _ptr(draft_logits), _ptr(draft_tokens), _ptr(uniforms),
+                                     _ptr(uniforms_resample), T, _ptr(mask_out), _ptr(tau_out), _ptr(next_token_out),
+                                     _ptr(diag_out), _stream(stream))
+    _check(ctx, st, "tts_accept_stochastic")
 
 
 def tts_distill_step(ctx, teacher_logits, h, W_in, W_out, W_master, adam_m, adam_v, pos_weight, mask, T, loss_scale,

@@ -404,6 +404,71 @@ def test_accept_mask_against_python_reference_and_properties():
                 assert am[s * 8 + tau[s]] != tok[s * 8 + tau[s]]  # first 0 at the first mismatch
 
 
+def test_stochastic_acceptance_preserves_the_target_distribution():
+    """The defining property of speculative rejection sampling: with x ~ q, accept w.p. min{1, p/q}, else resample
+    from norm(max(0, p - q)), the emitted token is distributed exactly as p.  Evaluated through the oracle on a fine
+    midpoint grid of both uniforms (resolution 1/n), summed over x with weight q(x)."""
+    r = _rng(31)
+    V, n = 6, 150
+    t = r.standard_normal((1, V)) * 1.5
+    z = r.standard_normal((1, V)) * 1.5
+    p = np.exp(t[0] - t[0].max()); p /= p.sum()
+    q = np.exp(z[0] - z[0].max()); q /= q.sum()
+    grid = (np.arange(n) + 0.5) / n
+    out = np.zeros(V)
+    for x in range(V):
+        uu, vv = np.meshgrid(grid, grid, indexing="ij")
+        N = n * n
+        res = O.accept_stochastic(np.repeat(t, N, 0), np.repeat(z, N, 0), np.full(N, x), uu.ravel(), vv.ravel(), 1)
+        emitted = np.where(res["mask"] == 1, x, res["next_token"])
+        assert (emitted >= 0).all()
+        out += q[x] * np.bincount(emitted, minlength=V) / N
+    np.testing.assert_allclose(out, p, atol=2.5 / n)
+    # and the accept probability itself: sum_x q min(1, p/q) = sum_x min(p, q)
+    assert res["ratio"][0] == pytest.approx(p[V - 1] / q[V - 1], rel=1e-12)
+
+
+def test_stochastic_acceptance_loop_and_diagnostics():
+    r = _rng(32)
+    C, S, V = 4, 3, 17
+    t = r.standard_normal((C * S, V)) * 2.0
+    z = r.standard_normal((C * S, V))
+    t[5, 3] = -np.inf
+    tok = r.integers(0, V, size=C * S)
+    u = r.uniform(size=C * S)
+    u[0:C] = 0.0                       # sequence 0: u = 0 accepts everything (ratio > 0)
+    u2 = r.uniform(size=S)
+    res = O.accept_stochastic(t, z, tok, u, u2, C)
+    p = torch.softmax(torch.tensor(t), -1).numpy()
+    q = torch.softmax(torch.tensor(z), -1).numpy()
+    assert res["tau"][0] == C and res["next_token"][0] == -1
+    for s in range(S):                 # pure-Python restatement of the loop
+        n = 0
+        for k in range(C):
+            rr = s * C + k
+            if u[rr] <= min(1.0, p[rr, tok[rr]] / q[rr, tok[rr]]):
+                n += 1
+            else:
+                break
+        assert res["tau"][s] == n
+        np.testing.assert_array_equal(res["mask"][s * C:(s + 1) * C], [1] * n + [0] * (C - n))
+        if n < C:
+            rr = s * C + n
+            nt = res["next_token"][s]
+            assert p[rr, nt] > q[rr, nt]                       # inside the residual's support
+            resid = np.maximum(0, p[rr] - q[rr])
+            assert resid[:nt].sum() < u2[s] * resid.sum() <= resid[:nt + 1].sum() + 1e-15
+    import scipy.stats
+    for rr in range(C * S):
+        assert res["diag"][rr, 0] == pytest.approx(scipy.stats.entropy(p[rr]), rel=1e-10)
+        assert res["diag"][rr, 1] == pytest.approx(-math.log(q[rr, int(np.argmax(p[rr]))]), rel=1e-10)
+        assert res["diag"][rr, 2] == pytest.approx(p[rr, tok[rr]], rel=1e-10)
+        assert res["diag"][rr, 3] == pytest.approx(q[rr, tok[rr]], rel=1e-10)
+    # p == q: ratio 1, everything accepted for any u < 1
+    res = O.accept_stochastic(z, z, tok, np.full(C * S, 0.999999), u2, C)
+    assert (res["tau"] == C).all()
+
+
 def test_row_weights_modes():
     w = np.array([1.0, 0.9, 0.8, 0.7] * 2)
     mask = np.array([1, 1, 0, 0, 0, 0, 0, 0], dtype=np.uint8)
