@@ -433,11 +433,15 @@ cudaError_t tc_fused_init(tts_ctx* c) {
   return cudaFuncSetAttribute(tc_update_gh_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
 }
 
-// Grid of the fused pass, 0 when the shape does not qualify (T > 16 rows, d or V not a multiple of the tile).
+// Grid of the fused pass, 0 when the shape does not qualify (T > 16 rows, d or V not a multiple of the tile, or an
+// SM budget below one CTA per 1024-column stripe: a CTA owns exactly one stripe, so the general tile kernel, which
+// walks any grid, serves that case).
 int tc_fused_grid(const tts_ctx* c, int T16) {
   if (T16 > kT16 || c->cfg.d % kSW != 0 || c->cfg.V % kTV != 0) return 0;
-  const long n_tiles = (long)(c->cfg.V / kTV) * (c->cfg.d / kSW);
+  const int n_stripes = c->cfg.d / kSW;
+  const long n_tiles = (long)(c->cfg.V / kTV) * n_stripes;
   int grid = c->cfg.max_ctas > 0 ? c->cfg.max_ctas : c->sm_count;
+  if (grid < n_stripes) return 0;
   if (grid > n_tiles) grid = (int)n_tiles;
   return grid;
 }

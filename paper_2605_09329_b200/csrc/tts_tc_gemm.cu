@@ -5,11 +5,13 @@
 //
 //   logits (a2)  z^T[v, r] = sum_j W_in[v, j] h[r, j]          M = 128 vocabulary rows, N = T16, K = d
 //                A = W_in tile, K-major (rows of W are contiguous in j);  B = h, K-major
-//   gh     (a5)  gh^T[j, r] = sum_v W_in[v, j] dl[r, v]        M = 128 hidden columns, N <= 128 rows, K = vocabulary
+//   gh     (a5)  gh^T[j, r] = sum_v W_in[v, j] dl[r, v]        M = 128 hidden columns, N = T16 rows, K = vocabulary
 //                A = W_in tile, MN-major (the same row-major W: j is contiguous, K = v strides by a row);
-//                B = dl planes [r, v], K-major.  dl = hi + lo (two bf16): both products accumulate into
-//                the same TMEM tile.  The vocabulary is split over CTAs; partial tiles are reduced with
-//                fp32 atomics into gh (zeroed first).
+//                B = the fp16 plane S dl [r, v] of tts_tc_wide.cu, K-major; the W tile is rewritten as fp16 in
+//                shared memory (see the kernel); the epilogue multiplies by 1 / (16 S).  The vocabulary is split over CTAs; partial tiles are
+//                reduced with fp32 atomics into gh (zeroed first).  (One canvas with d % 1024 == 0 never comes
+//                here: tts_tc_fused.cu forms gh inside the update pass.)
+#include <cuda_fp16.h>
 #include <string.h>
 
 #include "tts_common.cuh"
@@ -20,6 +22,8 @@ namespace tts {
 namespace {
 
 constexpr int kGemmThreads = 256;   // warp 0 TMA producer, 1 MMA issuer, 2 TMEM allocator, 3 idle, 4-7 epilogue
+constexpr int kGhThreads = 384;     // gh: warps 8-11 convert the bf16 W tile of a stage to fp16 in place
+constexpr float kGhWScale = 16.f;   // bf16 -> fp16 scale of W: exact for 2^-18 <= |W| < 4094
 constexpr int kATile = kTileMN * kKC * 2;   // 16 KB: [128 x 64] bf16 (K-major) or 2 x [64 k x 64 mn] (MN-major)
 constexpr int kMaxStages = 8;
 constexpr int kSmemBudget = 200 * 1024;
@@ -36,6 +40,7 @@ struct Bars {
   uint64_t empty[kMaxStages];
   uint64_t acc_full[2];
   uint64_t acc_empty[2];
+  uint64_t conv[kMaxStages];   // gh: the stage's W tile is fp16 now
   uint32_t tmem_slot;
 };
 
@@ -220,24 +225,33 @@ tc_logits_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant
 // ------------------------------------------------------------------ a5: gh
 struct GhParams {
   float* gh;
-  int T, d;
+  const float* dl_scale;   // {S, 1 / S} of the fp16 dl plane
+  int T, d, T16;
+  int planes;        // dl planes stacked along N (2: rows T16 .. 2 T16 hold the lo plane)
+  int N;             // planes * T16: accumulator columns
   int n_jt;          // d / 128
   int n_split;       // vocabulary splits
   int chunks_split;  // K chunks (of 64 vocabulary rows) per split
   int chunks_total;  // V / 64
-  int n_nb;          // accumulator blocks over the canvas rows
-  int NB;            // rows per block (MMA N)
-  int P;             // rows per dlR plane
+  int box_rows;      // rows per dl box (<= 256)
+  int n_boxes;       // dl boxes per stage
+  int n_acc;         // TMEM accumulators (2 when 2 * T16 <= 512)
   int stages;
   int tmem_cols;
 };
 
-__global__ void __launch_bounds__(kGemmThreads, 1)
+// One accumulator [128 j x T16 r] per unit (j tile, vocabulary split): the W tile of a K chunk is read once and
+// multiplied with all canvas rows (MMA pieces of N <= 256), so bf16 W streams from HBM exactly once per step.
+// Operand formats: dl needs more than bf16's 8 significant bits (a row with one dominant entry would miss the
+// 2e-3 max|gh| bar), kind::f16 wants A and B in one format, and W arrives as bf16 from the caller's memory: so four
+// otherwise idle warps rewrite each W tile in shared memory as fp16(16 W) (element-wise, so the swizzle is
+// untouched; exact for 2^-18 <= |W| < 4094, values beyond are clamped) before the MMAs of that stage are issued.
+__global__ void __launch_bounds__(kGhThreads, 1)
 tc_gh_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant__ CUtensorMap tm_dl, const GhParams p) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-  const int b_bytes = p.NB * kKC * 2;             // one plane
-  const int stage_bytes = kATile + 2 * b_bytes;
+  const int b_bytes = p.n_boxes * p.box_rows * kKC * 2;
+  const int stage_bytes = kATile + b_bytes;
   Bars* bars = reinterpret_cast<Bars*>(smem + p.stages * stage_bytes);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int n_units = p.n_jt * p.n_split;
@@ -247,7 +261,9 @@ tc_gh_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant__ C
     ptx::prefetch_tensormap(&tm_dl);
   }
   if (warp == 1 && lane == 0) {
-    for (int i = 0; i < p.stages; ++i) { ptx::mbar_init(&bars->full[i], 1); ptx::mbar_init(&bars->empty[i], 1); }
+    for (int i = 0; i < p.stages; ++i) {
+      ptx::mbar_init(&bars->full[i], 1); ptx::mbar_init(&bars->empty[i], 1); ptx::mbar_init(&bars->conv[i], 128);
+    }
     for (int i = 0; i < 2; ++i) { ptx::mbar_init(&bars->acc_full[i], 1); ptx::mbar_init(&bars->acc_empty[i], 4); }
     ptx::fence_barrier_init();
   }
@@ -260,84 +276,115 @@ tc_gh_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant__ C
   ptx::tc_fence_after();
   const uint32_t tmem_base = bars->tmem_slot;
 
-  if (warp == 0) {
+  if (warp >= 8) {
+    // ===== W tile bf16 -> fp16(16 W), in place: 16 KB per stage, 8 x 16 bytes per thread =====
+    const int t = threadIdx.x - 256;
+    uint32_t n = 0;
+    for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
+      const int sp = u / p.n_jt;
+      const int c_beg = sp * p.chunks_split, c_end = min(p.chunks_total, c_beg + p.chunks_split);
+      for (int kc = c_beg; kc < c_end; ++kc, ++n) {
+        const int s = n % p.stages;
+        ptx::mbar_wait(&bars->full[s], (n / p.stages) & 1);
+        uint4* A = reinterpret_cast<uint4*>(smem + s * stage_bytes);
+#pragma unroll
+        for (int k = 0; k < kATile / 16 / 128; ++k) {
+          uint4 x = A[k * 128 + t];
+          uint32_t* w = reinterpret_cast<uint32_t*>(&x);
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const float lo = fminf(fmaxf(__uint_as_float(w[e] << 16) * kGhWScale, -65504.f), 65504.f);
+            const float hi = fminf(fmaxf(__uint_as_float(w[e] & 0xFFFF0000u) * kGhWScale, -65504.f), 65504.f);
+            const __half2 h2 = __floats2half2_rn(lo, hi);
+            w[e] = *reinterpret_cast<const uint32_t*>(&h2);
+          }
+          A[k * 128 + t] = x;
+        }
+        ptx::fence_proxy_async_smem();
+        ptx::mbar_arrive(&bars->conv[s]);
+      }
+    }
+  } else if (warp == 0) {
     if (lane == 0) {
       uint32_t n = 0;
       for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
         const int j0 = (u % p.n_jt) * kTileMN, sp = u / p.n_jt;
         const int c_beg = sp * p.chunks_split, c_end = min(p.chunks_total, c_beg + p.chunks_split);
-        for (int nb = 0; nb < p.n_nb; ++nb) {
-          for (int kc = c_beg; kc < c_end; ++kc, ++n) {
-            const int s = n % p.stages;
-            ptx::mbar_wait(&bars->empty[s], ((n / p.stages) & 1) ^ 1);
-            uint8_t* A = smem + s * stage_bytes;
-            ptx::mbar_expect_tx(&bars->full[s], stage_bytes);
-            // W rows kc*64 .. +63 (K), columns j0 .. j0+127 (M) as two [64 k x 64 m] boxes
-            ptx::tma_load_2d(A, &tm_W, &bars->full[s], j0, kc * kKC);
-            ptx::tma_load_2d(A + kATile / 2, &tm_W, &bars->full[s], j0 + 64, kc * kKC);
-            ptx::tma_load_2d(A + kATile, &tm_dl, &bars->full[s], kc * kKC, nb * p.NB);
-            ptx::tma_load_2d(A + kATile + b_bytes, &tm_dl, &bars->full[s], kc * kKC, p.P + nb * p.NB);
-          }
+        for (int kc = c_beg; kc < c_end; ++kc, ++n) {
+          const int s = n % p.stages;
+          ptx::mbar_wait(&bars->empty[s], ((n / p.stages) & 1) ^ 1);
+          uint8_t* A = smem + s * stage_bytes;
+          ptx::mbar_expect_tx(&bars->full[s], stage_bytes);
+          // W rows kc*64 .. +63 (K), columns j0 .. j0+127 (M) as two [64 k x 64 m] boxes
+          ptx::tma_load_2d(A, &tm_W, &bars->full[s], j0, kc * kKC);
+          ptx::tma_load_2d(A + kATile / 2, &tm_W, &bars->full[s], j0 + 64, kc * kKC);
+          for (int b = 0; b < p.n_boxes; ++b)   // rows beyond the scratch are out of bounds: zero fill
+            ptx::tma_load_2d(A + kATile + b * p.box_rows * kKC * 2, &tm_dl, &bars->full[s], kc * kKC, b * p.box_rows);
         }
       }
     }
   } else if (warp == 1) {
     if (lane == 0) {
-      const uint32_t idesc = ptx::make_idesc_bf16(kTileMN, p.NB, 1, 0);   // A MN-major, B K-major
       uint32_t n = 0, it = 0;
-      for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
+      for (int u = blockIdx.x; u < n_units; u += gridDim.x, ++it) {
         const int sp = u / p.n_jt;
         const int c_beg = sp * p.chunks_split, c_end = min(p.chunks_total, c_beg + p.chunks_split);
-        for (int nb = 0; nb < p.n_nb; ++nb, ++it) {
-          const int ab = it & 1;
-          ptx::mbar_wait(&bars->acc_empty[ab], ((it >> 1) & 1) ^ 1);
+        const int ab = it % p.n_acc;
+        ptx::mbar_wait(&bars->acc_empty[ab], ((it / p.n_acc) & 1) ^ 1);
+        ptx::tc_fence_after();
+        const uint32_t d_tmem = tmem_base + ab * p.N;
+        for (int kc = c_beg; kc < c_end; ++kc, ++n) {
+          const int s = n % p.stages;
+          ptx::mbar_wait(&bars->full[s], (n / p.stages) & 1);
+          ptx::mbar_wait(&bars->conv[s], (n / p.stages) & 1);
           ptx::tc_fence_after();
-          const uint32_t d_tmem = tmem_base + ab * p.NB;
-          for (int kc = c_beg; kc < c_end; ++kc, ++n) {
-            const int s = n % p.stages;
-            ptx::mbar_wait(&bars->full[s], (n / p.stages) & 1);
-            ptx::tc_fence_after();
-            const uint32_t a0 = ptx::smem_u32(smem + s * stage_bytes), b0 = a0 + kATile;
+          const uint32_t a0 = ptx::smem_u32(smem + s * stage_bytes), b0 = a0 + kATile;
 #pragma unroll
-            for (int ks = 0; ks < kKC / 16; ++ks) {
-              // MN-major, 128-byte swizzle: 64 m per 128-byte row, one row per k; 8-row groups 1 KB apart (SBO),
-              // the second 64-m block kATile/2 further (LBO); 16 k per instruction = 2 KB
-              const uint64_t ad = ptx::make_smem_desc(a0 + ks * 2048, kATile / 2, 1024, ptx::kSwizzle128B);
-              const uint64_t bh = ptx::make_smem_desc(b0 + ks * 32, 16, 1024, ptx::kSwizzle128B);
-              const uint64_t bl = ptx::make_smem_desc(b0 + b_bytes + ks * 32, 16, 1024, ptx::kSwizzle128B);
-              ptx::mma_f16_ss(d_tmem, ad, bh, idesc, (kc != c_beg) || ks != 0);
-              ptx::mma_f16_ss(d_tmem, ad, bl, idesc, 1);
+          for (int ks = 0; ks < kKC / 16; ++ks) {
+            // A (fp16 16 W, MN-major, 128-byte swizzle): 64 m per 128-byte row, one row per k; 8-row groups 1 KB apart
+            // (SBO), the second 64-m block kATile/2 further (LBO); 16 k per instruction = 2 KB
+            const uint64_t ad = ptx::make_smem_desc(a0 + ks * 2048, kATile / 2, 1024, ptx::kSwizzle128B);
+            for (int c0 = 0; c0 < p.N; c0 += kNMax) {
+              const int nn = min(kNMax, p.N - c0);
+              // B (fp16 S dl, K-major): rows r, 64 v per 128-byte row
+              const uint64_t bd = ptx::make_smem_desc(b0 + c0 * kKC * 2 + ks * 32, 16, 1024, ptx::kSwizzle128B);
+              ptx::mma_f16_ss(d_tmem + c0, ad, bd,
+                              ptx::make_idesc_f16(kTileMN, nn, ptx::kFmtF16, ptx::kFmtF16, 1, 0),
+                              (kc != c_beg) || ks != 0);
             }
-            ptx::mma_commit(&bars->empty[s]);
           }
-          ptx::mma_commit(&bars->acc_full[ab]);
+          ptx::mma_commit(&bars->empty[s]);
         }
+        ptx::mma_commit(&bars->acc_full[ab]);
       }
     }
   } else if (warp >= 4) {
     const int q = warp & 3;
+    const float inv_s = p.dl_scale[1] * (1.f / kGhWScale);
     uint32_t it = 0;
-    for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
+    for (int u = blockIdx.x; u < n_units; u += gridDim.x, ++it) {
       const int j0 = (u % p.n_jt) * kTileMN;
-      for (int nb = 0; nb < p.n_nb; ++nb, ++it) {
-        const int ab = it & 1;
-        ptx::mbar_wait(&bars->acc_full[ab], (it >> 1) & 1);
-        ptx::tc_fence_after();
-        float* gc = p.gh + j0 + q * 32 + lane;
-        for (int c0 = 0; c0 < p.NB; c0 += 16) {
-          const int r0 = nb * p.NB + c0;
-          if (r0 >= p.T) break;
-          uint32_t r[16];
-          ptx::tmem_ld_32x32b_x16(tmem_base + ab * p.NB + c0 + (static_cast<uint32_t>(q * 32) << 16), r);
-          ptx::tmem_ld_wait();
+      const int ab = it % p.n_acc;
+      ptx::mbar_wait(&bars->acc_full[ab], (it / p.n_acc) & 1);
+      ptx::tc_fence_after();
+      float* gc = p.gh + j0 + q * 32 + lane;
+      for (int c0 = 0; c0 < p.T16; c0 += 16) {
+        if (c0 >= p.T) break;
+        uint32_t r[16], r2[16];
+        ptx::tmem_ld_32x32b_x16(tmem_base + ab * p.N + c0 + (static_cast<uint32_t>(q * 32) << 16), r);
+        if (p.planes == 2)
+          ptx::tmem_ld_32x32b_x16(tmem_base + ab * p.N + p.T16 + c0 + (static_cast<uint32_t>(q * 32) << 16), r2);
+        ptx::tmem_ld_wait();
 #pragma unroll
-          for (int i = 0; i < 16; ++i)
-            if (r0 + i < p.T) atomicAdd(gc + (size_t)(r0 + i) * p.d, __uint_as_float(r[i]));
+        for (int i = 0; i < 16; ++i) {
+          float x = __uint_as_float(r[i]);
+          if (p.planes == 2) x += __uint_as_float(r2[i]);
+          if (c0 + i < p.T) atomicAdd(gc + (size_t)(c0 + i) * p.d, x * inv_s);
         }
-        ptx::tc_fence_before();
-        __syncwarp();
-        if (lane == 0) ptx::mbar_arrive(&bars->acc_empty[ab]);
       }
+      ptx::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(&bars->acc_empty[ab]);
     }
   }
   ptx::tc_fence_before();
@@ -415,32 +462,36 @@ cudaError_t tc_launch_gh(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* lau
   if ((e = cudaMemsetAsync(a.gh_out, 0, (size_t)T * d * sizeof(float), s)) != cudaSuccess) return e;
   int grid = c->cfg.max_ctas > 0 ? c->cfg.max_ctas : c->sm_count;
   GhParams p;
-  p.gh = a.gh_out; p.T = T; p.d = d;
+  p.gh = a.gh_out; p.dl_scale = st->dl_scale; p.T = T; p.d = d; p.T16 = T16;
   p.n_jt = d / kTileMN;
   p.chunks_total = V / kKC;
-  p.NB = T16 <= kGhNB ? T16 : kGhNB;
-  p.n_nb = (T16 + p.NB - 1) / p.NB;
-  p.P = st->P;
-  // about 8 units per CTA, each a contiguous run of vocabulary chunks for one 128-column tile of gh
-  int n_split = (8 * grid + p.n_jt - 1) / p.n_jt;
-  if (n_split > p.chunks_total) n_split = p.chunks_total;
+  p.planes = tc_wide_planes(T16);
+  p.N = p.planes * T16;
+  p.box_rows = p.N <= kNMax ? p.N : kNMax;
+  p.n_boxes = (p.N + p.box_rows - 1) / p.box_rows;
+  p.n_acc = 2 * p.N <= 512 ? 2 : 1;
+  p.tmem_cols = pow2_cols(p.n_acc * p.N);
+  // About two units per CTA: each is a contiguous run of vocabulary chunks for one 128-column tile of gh, flushed
+  // with fp32 RED (256 KB per unit at T = 512: more units would make the flush the bottleneck).  Units of one
+  // vocabulary split run side by side on consecutive CTAs, so a dl chunk is fetched into L2 once for all j tiles.
+  int n_split = (2 * grid) / p.n_jt;
   if (n_split < 1) n_split = 1;
+  if (n_split > p.chunks_total) n_split = p.chunks_total;
   p.chunks_split = (p.chunks_total + n_split - 1) / n_split;
   p.n_split = (p.chunks_total + p.chunks_split - 1) / p.chunks_split;
-  const int stage_bytes = kATile + 2 * p.NB * kKC * 2;
+  const int stage_bytes = kATile + p.n_boxes * p.box_rows * kKC * 2;
   p.stages = pick_stages(stage_bytes);
-  p.tmem_cols = pow2_cols(2 * p.NB);
   CUtensorMap tm_W, tm_dl;
   if (make_map_2d(st, &tm_W, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, a.W_in, d, V, 64, kKC,
                   CU_TENSOR_MAP_SWIZZLE_128B) != CUDA_SUCCESS)
     return cudaErrorInvalidValue;
-  if (make_map_2d(st, &tm_dl, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, st->dlR, V, (uint64_t)2 * st->P, kKC, p.NB,
+  if (make_map_2d(st, &tm_dl, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, st->dlR, V, (uint64_t)st->P, kKC, p.box_rows,
                   CU_TENSOR_MAP_SWIZZLE_128B) != CUDA_SUCCESS)
     return cudaErrorInvalidValue;
   const int n_units = p.n_jt * p.n_split;
   if (grid > n_units) grid = n_units;
   const size_t smem = 1024 + (size_t)p.stages * stage_bytes + sizeof(Bars);
-  tc_gh_kernel<<<grid, kGemmThreads, smem, s>>>(tm_W, tm_dl, p);
+  tc_gh_kernel<<<grid, kGhThreads, smem, s>>>(tm_W, tm_dl, p);
   *launches += 1;
   return cudaGetLastError();
 }

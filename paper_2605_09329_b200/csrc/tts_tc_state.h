@@ -12,17 +12,16 @@ namespace tts {
 
 constexpr int kKC = 64;          // bf16 elements per K chunk = one 128-byte swizzle row
 constexpr int kTileMN = 128;     // MMA M of every tensor-path kernel (vocabulary rows or hidden columns per tile)
-constexpr int kGhNB = 128;       // canvas rows (MMA N) per accumulator block of the gh contraction
 
 struct TcState {
-  __nv_bfloat16* dlT;   // [V, Kp]        B operand of gW: row v = (dl_hi[0..T16), dl_lo[0..T16)) of vocabulary row v
-  __nv_bfloat16* hTT;   // [d, Kp]        A operand of gW: row j = (h[0..T16, j], h[0..T16, j])
+  void* dlT;            // [V, Kp] fp16   B operand of gW (wide path): row v = S dl[0..Kp, v], this step's Kp as row pitch
+  void* hTT;            // [d, Kp] fp16   A operand of gW (wide path): row j = S_h h[0..Kp, j]
   __nv_bfloat16* hTc;   // [d / 128][2][16][8][8]        A tiles of gW in core-matrix order (tts_tc_fused.cu, T <= 16)
   __nv_bfloat16* dlC;   // [V / 16][2][2][2][8][8]        dl hi / lo planes, pre-tiled in core-matrix order (tts_tc_fused.cu)
-  __nv_bfloat16* dlR;   // [2, P, V]      B operand of gh: plane 0 = dl_hi[r, v], plane 1 = dl_lo[r, v]
-  int Kp;               // K extent of dlT / hTT (multiple of kKC)
-  int P;                // rows per dlR plane (T_pad_max, rounded up to kGhNB when larger)
-  CUtensorMap tm_dlT, tm_hTT;
+  void* dlR;            // [P, V] fp16    B operand of gh: S dl[r, v] (rows T16 .. 2 T16: the lo plane when there are two)
+  float* dl_scale;      // {S, 1 / S, S_h, 1 / S_h, bits of max|h|}: power-of-two scales of the fp16 dl and h^T planes (a4 kernels)
+  int Kp;               // largest K extent of dlT / hTT (T_pad_max rounded up to kKC)
+  int P;                // rows of dlR (T_pad_max, twice that up to 32 rows)
   PFN_cuTensorMapEncodeTiled_v12000 encode;
 };
 
@@ -42,7 +41,7 @@ inline CUresult make_map_2d(const TcState* st, CUtensorMap* m, CUtensorMapDataTy
 cudaError_t tc_gemm_init(tts_ctx* c);
 // a2: z[r, v] = sum_j h[r, j] W_in[v, j] on tcgen05 (fp32 accumulation), z scratch [T16, V]
 cudaError_t tc_launch_logits(tts_ctx* c, const StepArgs& a, float* z_out, cudaStream_t s, int* launches);
-// a5: gh[r, j] = sum_v (dl_hi + dl_lo)[r, v] W_in[v, j] on tcgen05, split over the vocabulary, fp32 atomics into gh
+// a5: gh[r, j] = sum_v dl[r, v] W_in[v, j] on tcgen05, split over the vocabulary, fp32 atomics into gh
 cudaError_t tc_launch_gh(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches);
 
 // tts_tc_fused.cu: a5 + a6 + a7 in one pass over the optimiser state (T <= 16, d % 1024 == 0, V % 16 == 0)
@@ -50,5 +49,11 @@ cudaError_t tc_fused_init(tts_ctx* c);
 int tc_fused_grid(const tts_ctx* c, int T16);
 cudaError_t tc_launch_prep_fused(tts_ctx* c, const StepArgs& a, const float* z, cudaStream_t s, int* launches);   // a4: operands
 cudaError_t tc_launch_update_fused(tts_ctx* c, const StepArgs& a, int grid, cudaStream_t s, int* launches);
+
+// tts_tc_wide.cu: a4 operands (h^T rows, fp16 dl planes) and a6 + a7 for T <= 512
+cudaError_t tc_wide_init(tts_ctx* c);
+int tc_wide_planes(int T16);   // 2: dl S = hi + lo (T16 <= 32), 1: one fp16 plane
+cudaError_t tc_launch_prep_wide(tts_ctx* c, const StepArgs& a, const float* z, cudaStream_t s, int* launches);
+cudaError_t tc_launch_update_wide(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches);
 
 }  // namespace tts

@@ -1,0 +1,569 @@
+// Pass B of the distillation step for MORE than one canvas (16 < T <= 512 rows, SURVEY 8(a) a4 + a6 + a7), and for
+// one-canvas shapes whose hidden size is not a multiple of the fused kernel's 1024-column stripe.
+//
+// Why it differs from tts_tc_fused.cu.  gW = dl^T h is a rank-T update: at T = 512 every [128 j x N v] tile of gW
+// needs (128 + N) x 512 operand values, and an operand that is re-fetched per tile costs as much L2 -> SM traffic as
+// the optimiser state itself costs HBM traffic (the first version of this kernel re-read 512 KB of operands per
+// 426 KB of state and ran at 4.1 TB/s).  So here
+//   * a CTA owns one 128-column stripe of the parameter matrix at a time and keeps the stripe's h^T operand
+//     [128 j x Kp] RESIDENT: in tensor memory (256 of the 512 columns at T = 512; A_TMEM), which leaves all of
+//     shared memory to the state ring, or in shared memory (the variant kept for comparison);
+//   * dl is ONE 16-bit plane: fp16 with a power-of-two scale chosen from the row coefficients (|dl S| <= 2^14), i.e.
+//     11 significant bits against bf16's 8 (one bf16 plane misses the 2e-3 max|gW| bar on rows with a dominant
+//     entry; the hi/lo bf16 split of the one-canvas kernel would double K).  kind::f16 wants A and B in the same
+//     format (a bf16 x fp16 MMA traps as an illegal instruction on sm_100a), so h^T is converted to fp16 as well:
+//     exact for bf16 inputs after a power-of-two scale S_h from max|h| (|h S_h| <= 2^14; only values below
+//     2^-28 max|h| lose bits).  The epilogue multiplies the accumulator by 1 / (S S_h) (exact);
+//   * per band of NV vocabulary rows the only operand traffic is the band's dl rows [NV x Kp] (8 B per parameter
+//     at T = 512 against 26 B of state);
+//   * work is cut as windowed stream-K: the vocabulary is cut into windows whose dl rows (<= 12 MB) stay in L2
+//     (evict_last) while every stripe passes over them; inside a window the (stripe, band) units, stripe-major, are
+//     split into gridDim equal contiguous ranges, so the grid is balanced to one band for any SM budget and a CTA
+//     changes stripe (reloads A) at most twice per window.
+// The state moves as in the fused kernel: TMA loads of [8 v x 128 j] sub-tiles of master / m / v into a ring,
+// AdamW applied in place in shared memory, TMA stores of the three tensors and the bf16 working copy.
+#include <cuda_fp16.h>
+#include <string.h>
+
+#include "tts_common.cuh"
+#include "tts_tc_ptx.cuh"
+#include "tts_tc_state.h"
+
+namespace tts {
+namespace {
+
+constexpr int kWJ = 128;                 // stripe width = MMA M = TMEM lanes
+constexpr int kWSV = 8;                  // vocabulary rows per state stage
+constexpr int kWTensorBytes = kWSV * kWJ * 4;   // 4 KB per tensor per stage
+constexpr int kWStageBytes = 3 * kWTensorBytes; // 12 KB
+constexpr int kWWoBytes = kWSV * kWJ * 2;       // 2 KB: bf16 staging of one sub-tile (one per epilogue group)
+constexpr int kWThreads = 384;           // warp 0 state TMA, 1 MMA, 2 TMEM alloc, 3 operand TMA, 4-11 epilogue
+constexpr int kWMaxStages = 16;
+constexpr int kWOpStages = 2;            // dl band ring
+constexpr int kWSmemBudget = 225 * 1024;
+constexpr int kWAccCols = 64;            // TMEM columns reserved for the two gW accumulators (NV <= 32)
+constexpr long kWWindowBytes = 12l << 20;
+
+struct WideParams {
+  float* gW_debug;
+  const uint16_t* hTT;        // [d, Kp] fp16 bits
+  const float* dl_scale;      // {S, 1 / S, S_h, 1 / S_h}
+  int V, d, Kp;
+  int n_stripes, n_bands, n_win, stages;
+  float lr, b1, b2, eps, decay, c1, inv_sqrt_bc2;   // decay = 1 - lr wd, c1 = lr / (1 - b1^n)
+};
+
+struct WideBars {
+  uint64_t st_full[kWMaxStages];
+  uint64_t st_empty[kWMaxStages];
+  uint64_t op_full[kWOpStages];
+  uint64_t op_empty[kWOpStages];
+  uint64_t acc_full[2];
+  uint64_t acc_empty[2];
+  uint64_t a_full;
+  uint64_t a_empty;
+  uint32_t tmem_slot;
+};
+
+// The sequence of (stripe, band) units of this CTA: window by window, a contiguous range of each window's units.
+struct WideWalk {
+  int n_stripes, n_bands, n_win;
+  int win, wb0, wbn;
+  long u, u_end;
+  __device__ WideWalk(const WideParams& p) : n_stripes(p.n_stripes), n_bands(p.n_bands), n_win(p.n_win), win(-1),
+                                             wb0(0), wbn(1), u(0), u_end(0) {}
+  __device__ bool get(int& stripe, int& band) {
+    while (u >= u_end) {
+      if (++win >= n_win) return false;
+      wb0 = (int)((long)n_bands * win / n_win);
+      wbn = (int)((long)n_bands * (win + 1) / n_win) - wb0;
+      const long units = (long)n_stripes * wbn;
+      u = units * blockIdx.x / gridDim.x;
+      u_end = units * (blockIdx.x + 1) / gridDim.x;
+    }
+    stripe = (int)(u / wbn);
+    band = wb0 + (int)(u - (long)stripe * wbn);
+    ++u;
+    return true;
+  }
+};
+
+constexpr uint32_t kDescHiSw128 = (1024u >> 4) | (1u << 14) | (ptx::kSwizzle128B << 29);
+__device__ __forceinline__ uint32_t desc_lo_sw128(uint32_t smem_addr) { return ((smem_addr >> 4) & 0x3FFFu) | (1u << 16); }
+__device__ __forceinline__ uint64_t desc64(uint32_t hi, uint32_t lo) { return (static_cast<uint64_t>(hi) << 32) | lo; }
+
+template <bool ADAM, bool A_TMEM, int NV>
+__global__ void __launch_bounds__(kWThreads, 1)
+tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_hTT, const __grid_constant__ CUtensorMap tm_dlT,
+                      const __grid_constant__ CUtensorMap tm_master, const __grid_constant__ CUtensorMap tm_m,
+                      const __grid_constant__ CUtensorMap tm_v, const __grid_constant__ CUtensorMap tm_wout,
+                      const WideParams p) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  constexpr int kSubs = NV / kWSV;
+  const int a_bytes = A_TMEM ? 0 : p.Kp * kWJ * 2;     // [Kp / 64][128 j][64 k] bf16, 128-byte swizzle
+  const int b_bytes = NV * p.Kp * 2;                   // [Kp / 64][NV v][64 k] fp16, 128-byte swizzle
+  uint8_t* sA = smem;
+  uint8_t* sB = sA + a_bytes;
+  uint8_t* st = sB + kWOpStages * b_bytes;             // [stages][3][8 v][128 j] fp32
+  uint8_t* wo = st + p.stages * kWStageBytes;          // [2 groups][8 v][128 j] bf16
+  WideBars* bars = reinterpret_cast<WideBars*>(wo + 2 * kWWoBytes);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int nks = p.Kp / 16;                           // MMA K steps per band
+
+  if (warp == 0 && lane == 0) {
+    ptx::prefetch_tensormap(&tm_master);
+    if (ADAM) { ptx::prefetch_tensormap(&tm_m); ptx::prefetch_tensormap(&tm_v); }
+    ptx::prefetch_tensormap(&tm_wout);
+  }
+  if (warp == 3 && lane == 0) {
+    ptx::prefetch_tensormap(&tm_dlT);
+    if (!A_TMEM) ptx::prefetch_tensormap(&tm_hTT);
+  }
+  if (warp == 1 && lane == 0) {
+    for (int i = 0; i < p.stages; ++i) { ptx::mbar_init(&bars->st_full[i], 1); ptx::mbar_init(&bars->st_empty[i], 1); }
+    for (int i = 0; i < kWOpStages; ++i) { ptx::mbar_init(&bars->op_full[i], 1); ptx::mbar_init(&bars->op_empty[i], 1); }
+    for (int i = 0; i < 2; ++i) { ptx::mbar_init(&bars->acc_full[i], 1); ptx::mbar_init(&bars->acc_empty[i], 8); }
+    ptx::mbar_init(&bars->a_full, A_TMEM ? 8 : 1);
+    ptx::mbar_init(&bars->a_empty, 1);
+    ptx::fence_barrier_init();
+  }
+  if (warp == 2) {
+    ptx::tmem_alloc(&bars->tmem_slot, 512);
+    ptx::tmem_relinquish();
+  }
+  ptx::tc_fence_before();
+  __syncthreads();
+  ptx::tc_fence_after();
+  const uint32_t tmem_base = bars->tmem_slot;
+  const uint32_t tmem_A = tmem_base + kWAccCols;       // Kp / 2 columns: h^T of the stripe, K packed in pairs
+
+  if (warp == 0) {
+    // ===== optimiser-state producer: [8 v x 128 j] of master / m / v per stage =====
+    if (lane == 0) {
+      const uint64_t pol = ptx::policy_evict_first();
+      WideWalk w(p);
+      uint32_t n = 0;
+      int stripe, band;
+      while (w.get(stripe, band)) {
+        const int j0 = stripe * kWJ, v0 = band * NV;
+        for (int sub = 0; sub < kSubs; ++sub, ++n) {
+          const int s = n % p.stages;
+          ptx::mbar_wait(&bars->st_empty[s], ((n / p.stages) & 1) ^ 1);
+          uint8_t* dst = st + s * kWStageBytes;
+          ptx::mbar_expect_tx(&bars->st_full[s], (ADAM ? 3 : 1) * kWTensorBytes);
+          const int r0 = v0 + sub * kWSV;
+          ptx::tma_load_2d_hint(dst, &tm_master, &bars->st_full[s], j0, r0, pol);
+          if (ADAM) {
+            ptx::tma_load_2d_hint(dst + kWTensorBytes, &tm_m, &bars->st_full[s], j0, r0, pol);
+            ptx::tma_load_2d_hint(dst + 2 * kWTensorBytes, &tm_v, &bars->st_full[s], j0, r0, pol);
+          }
+        }
+      }
+    }
+  } else if (warp == 3) {
+    // ===== operand producer: the band's dl rows [NV v x Kp] (and, A in shared memory, the stripe's h^T) =====
+    if (lane == 0) {
+      const uint64_t pol = ptx::policy_evict_last();
+      WideWalk w(p);
+      uint32_t i = 0, a_loads = 0;
+      int stripe, band, cur = -1;
+      while (w.get(stripe, band)) {
+        if (!A_TMEM && stripe != cur) {
+          ptx::mbar_wait(&bars->a_empty, (a_loads & 1) ^ 1);     // the MMAs that read the old stripe are complete
+          ptx::mbar_expect_tx(&bars->a_full, a_bytes);
+          for (int c = 0; c < p.Kp / kKC; ++c)
+            ptx::tma_load_2d_hint(sA + c * (kWJ * 128), &tm_hTT, &bars->a_full, c * kKC, stripe * kWJ, pol);
+          ++a_loads;
+          cur = stripe;
+        }
+        const int s = i % kWOpStages;
+        ptx::mbar_wait(&bars->op_empty[s], ((i / kWOpStages) & 1) ^ 1);
+        ptx::mbar_expect_tx(&bars->op_full[s], b_bytes);
+        for (int c = 0; c < p.Kp / kKC; ++c)
+          ptx::tma_load_2d_hint(sB + s * b_bytes + c * (NV * 128), &tm_dlT, &bars->op_full[s], c * kKC, band * NV, pol);
+        ++i;
+      }
+    }
+  } else if (warp == 1) {
+    // ===== MMA issuer: acc[j, v] = sum_r h^T[j, r] (S dl)[r, v]   (M = 128, N = NV, K = 16 per instruction) =====
+    if (lane == 0) {
+      constexpr uint32_t idesc = ptx::make_idesc_f16(kWJ, NV, ptx::kFmtF16, ptx::kFmtF16, 0, 0);
+      const uint32_t sA0 = ptx::smem_u32(sA), sB0 = ptx::smem_u32(sB);
+      WideWalk w(p);
+      uint32_t i = 0, a_n = 0;
+      int stripe, band, cur = -1;
+      while (w.get(stripe, band)) {
+        if (stripe != cur) {
+          if (!A_TMEM && cur >= 0) ptx::mma_commit(&bars->a_empty);
+          ptx::mbar_wait(&bars->a_full, a_n & 1);
+          ptx::tc_fence_after();
+          ++a_n;
+          cur = stripe;
+        }
+        const int ab = i & 1, s = i % kWOpStages;
+        ptx::mbar_wait(&bars->acc_empty[ab], ((i >> 1) & 1) ^ 1);
+        ptx::mbar_wait(&bars->op_full[s], (i / kWOpStages) & 1);
+        ptx::tc_fence_after();
+        const uint32_t d_tmem = tmem_base + ab * NV;
+        const uint32_t b_base = sB0 + s * b_bytes;
+        for (int ks = 0; ks < nks; ++ks) {
+          const uint32_t b_lo = desc_lo_sw128(b_base + (ks >> 2) * (NV * 128)) + 2 * (ks & 3);
+          if (A_TMEM) {
+            ptx::mma_f16_ts(d_tmem, tmem_A + ks * 8, desc64(kDescHiSw128, b_lo), idesc, ks);
+          } else {
+            const uint32_t a_lo = desc_lo_sw128(sA0 + (ks >> 2) * (kWJ * 128)) + 2 * (ks & 3);
+            ptx::mma_f16_ss(d_tmem, desc64(kDescHiSw128, a_lo), desc64(kDescHiSw128, b_lo), idesc, ks);
+          }
+        }
+        ptx::mma_commit(&bars->op_empty[s]);
+        ptx::mma_commit(&bars->acc_full[ab]);
+        ++i;
+      }
+    }
+  } else if (warp >= 4) {
+    // ===== epilogue: 2 groups x 4 warps; group g takes sub-tiles sub % 2 == g; warp quarter q owns TMEM lanes 32q.. =====
+    const int q = warp & 3, g = (warp - 4) >> 2;
+    const int jj = q * 32 + lane;              // hidden column of the stripe = TMEM lane
+    const bool leader = jj == 0;               // issues the group's TMA stores and releases its state stages
+    const uint32_t lane_bits = static_cast<uint32_t>(q * 32) << 16;
+    __nv_bfloat16* wo_g = reinterpret_cast<__nv_bfloat16*>(wo + g * kWWoBytes);
+    const float inv_s = p.dl_scale[1] * p.dl_scale[3];
+    WideWalk w(p);
+    uint32_t i = 0;
+    int stripe, band, cur = -1, prev_s = -1;
+    while (w.get(stripe, band)) {
+      const int j0 = stripe * kWJ, v0 = band * NV;
+      if (A_TMEM && stripe != cur) {
+        // every MMA that read the old stripe is complete: this warp has waited on the previous band's acc_full.
+        // Row jj of hTT is K-contiguous; this group writes half of the K steps.
+        const uint4* row = reinterpret_cast<const uint4*>(p.hTT + (size_t)(j0 + jj) * p.Kp);
+        for (int ks = g * (nks / 2); ks < (g + 1) * (nks / 2); ++ks) {
+          const uint4 lo = row[2 * ks], hi = row[2 * ks + 1];
+          const uint32_t r[8] = {lo.x, lo.y, lo.z, lo.w, hi.x, hi.y, hi.z, hi.w};
+          ptx::tmem_st_32x32b_x8(tmem_A + ks * 8 + lane_bits, r);
+        }
+        ptx::tmem_st_wait();
+        ptx::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(&bars->a_full);
+        cur = stripe;
+      }
+      const int ab = i & 1;
+      ptx::mbar_wait(&bars->acc_full[ab], (i >> 1) & 1);
+      ptx::tc_fence_after();
+      for (int sub = g; sub < kSubs; sub += 2) {
+        const uint32_t n = i * kSubs + sub;
+        const int s = n % p.stages;
+        uint32_t gr[kWSV];
+        ptx::tmem_ld_32x32b_x8(tmem_base + ab * NV + sub * kWSV + lane_bits, gr);
+        ptx::mbar_wait(&bars->st_full[s], (n / p.stages) & 1);
+        float* sM = reinterpret_cast<float*>(st + s * kWStageBytes) + jj;
+        float M[kWSV], mm[kWSV], vv[kWSV];
+#pragma unroll
+        for (int r = 0; r < kWSV; ++r) {
+          M[r] = sM[r * kWJ];
+          if (ADAM) { mm[r] = sM[kWSV * kWJ + r * kWJ]; vv[r] = sM[2 * kWSV * kWJ + r * kWJ]; }
+        }
+        ptx::tmem_ld_wait();
+        // a7 in place: the thread rewrites exactly the shared-memory words it read
+#pragma unroll
+        for (int r = 0; r < kWSV; ++r) {
+          const float gg = __uint_as_float(gr[r]) * inv_s;
+          gr[r] = __float_as_uint(gg);
+          if (ADAM) {
+            const float m1 = p.b1 * mm[r] + (1.f - p.b1) * gg;
+            const float v1 = p.b2 * vv[r] + (1.f - p.b2) * gg * gg;
+            const float den = __fsqrt_rn(v1) * p.inv_sqrt_bc2 + p.eps;
+            M[r] = M[r] * p.decay - __fdividef(p.c1 * m1, den);
+            sM[kWSV * kWJ + r * kWJ] = m1;
+            sM[2 * kWSV * kWJ + r * kWJ] = v1;
+          } else {
+            M[r] = M[r] - p.lr * gg;
+          }
+          sM[r * kWJ] = M[r];
+        }
+        if (p.gW_debug) {
+#pragma unroll
+          for (int r = 0; r < kWSV; ++r)
+            p.gW_debug[(size_t)(v0 + sub * kWSV + r) * p.d + j0 + jj] = __uint_as_float(gr[r]);
+        }
+        // the group's previous stores have read their shared memory: release that stage, reuse the bf16 staging
+        if (leader) {
+          ptx::bulk_wait_group_read<0>();
+          if (prev_s >= 0) ptx::mbar_arrive(&bars->st_empty[prev_s]);
+        }
+        ptx::named_barrier_sync(1 + g, 128);
+#pragma unroll
+        for (int r = 0; r < kWSV; ++r) wo_g[r * kWJ + jj] = __float2bfloat16_rn(M[r]);
+        ptx::fence_proxy_async_smem();
+        ptx::named_barrier_sync(1 + g, 128);
+        if (leader) {
+          const int r0 = v0 + sub * kWSV;
+          const float* sT = reinterpret_cast<const float*>(st + s * kWStageBytes);
+          ptx::tma_store_2d(&tm_master, sT, j0, r0);
+          if (ADAM) {
+            ptx::tma_store_2d(&tm_m, sT + kWSV * kWJ, j0, r0);
+            ptx::tma_store_2d(&tm_v, sT + 2 * kWSV * kWJ, j0, r0);
+          }
+          ptx::tma_store_2d(&tm_wout, wo_g, j0, r0);
+          ptx::bulk_commit_group();
+        }
+        prev_s = s;
+      }
+      ptx::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(&bars->acc_empty[ab]);
+      ++i;
+    }
+    if (leader) ptx::bulk_wait_group_read<0>();   // shared memory must outlive the last stores' reads
+  }
+  ptx::tc_fence_before();
+  __syncthreads();
+  if (warp == 2) {
+    ptx::tc_fence_after();
+    ptx::tmem_dealloc(tmem_base, 512);
+  }
+}
+
+// ------------------------------------------------------------------ a4: operands
+// Power-of-two scale of a 16-bit fp16 plane whose entries are bounded by `bound`: S = 2^(14 - e) with bound <= 2^e.
+__device__ __forceinline__ float pow2_scale_from_bound(float bound) {
+  if (!(bound > 0.f) || !isfinite(bound)) return 1.f;
+  int e;
+  frexpf(bound, &e);          // bound = m 2^e, m in [0.5, 1)
+  int k = 14 - e;
+  k = k > 100 ? 100 : (k < -100 ? -100 : k);
+  return ldexpf(1.f, k);
+}
+
+// max |h| over the T x d hidden states, as the bit pattern of a non-negative float (atomicMax on the zeroed slot)
+__global__ void __launch_bounds__(256) tc_h_absmax_kernel(const __nv_bfloat16* __restrict__ h, size_t n,
+                                                          unsigned int* __restrict__ out_bits) {
+  __shared__ float red[32];
+  float m = 0.f;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+    m = fmaxf(m, fabsf(__bfloat162float(h[i])));
+  m = block_max(m, red);
+  if (threadIdx.x == 0) atomicMax(out_bits, __float_as_uint(m));
+}
+
+// hTT[j, k] = fp16(S_h h[k, j]) for k < T (and again at k + T16 with two dl planes), 0 elsewhere up to Kp.  32 x 32 transpose tiles through shared memory.
+__global__ void __launch_bounds__(256) tc_prep_hT_kernel(const __nv_bfloat16* __restrict__ h, int d, int T, int T16,
+                                                         int planes, int Kp,
+                                                         const unsigned int* __restrict__ absmax_bits,
+                                                         uint16_t* __restrict__ hTT, float* __restrict__ dl_scale) {
+  __shared__ uint16_t tile[32][33];
+  const float Sh = pow2_scale_from_bound(__uint_as_float(*absmax_bits));
+  if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) { dl_scale[2] = Sh; dl_scale[3] = 1.f / Sh; }
+  const int j0 = blockIdx.x * 32, k0 = blockIdx.y * 32;
+  const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+  for (int k = ty; k < 32; k += 8) {
+    const int kk = k0 + k;
+    const int r = (planes == 2 && kk >= T16) ? kk - T16 : kk;       // the lo plane of dl meets the same rows of h
+    const float x = (r < T && kk < planes * T16 && j0 + tx < d) ? __bfloat162float(h[(size_t)r * d + j0 + tx]) : 0.f;
+    tile[k][tx] = __half_as_ushort(__float2half_rn(x * Sh));
+  }
+  __syncthreads();
+  for (int j = ty; j < 32; j += 8)
+    if (j0 + j < d && k0 + tx < Kp) hTT[(size_t)(j0 + j) * Kp + k0 + tx] = tile[tx][j];
+}
+
+// dl = coef_r ((q - p) + lambda (q - q_ref)) from z, teacher and the row normalisers, scaled by S and rounded to fp16;
+// one [64 v x 64 k] tile per block.  Up to 32 rows the 64-wide K chunk has room for a second plane, so dl S is
+// split hi + lo (two fp16, 2^-22) at no cost in operand bytes or MMAs and the h^T operand repeats its rows.  Written twice, both coalesced: dlT[v, r] (r contiguous: the K-major B operand
+// of gW; transposed through shared memory, 128-byte row segments) and dlR[r, v] (the K-major B operand of gh).
+template <bool BF16>
+__global__ void __launch_bounds__(256) tc_prep_dl_wide_kernel(const void* __restrict__ teacher, const float* __restrict__ z,
+                                                              const float* __restrict__ z_ref, float lam, int V,
+                                                              int z_ld, int T, int T16, int planes, int Kp, int T_max,
+                                                              const float* __restrict__ row_stats,
+                                                              uint16_t* __restrict__ dlT, uint16_t* __restrict__ dlR,
+                                                              float* __restrict__ dl_scale) {
+  constexpr int kPitch = 68;                      // halves: 34 words per row, 8-byte aligned rows
+  __shared__ __align__(16) uint16_t tile[64 * kPitch];
+  __shared__ float sh[4 * 64];                    // lse_t, lse_z, coef, lse_ref of the tile's rows
+  __shared__ float red[32];
+  const int v0 = blockIdx.x * 64, r0 = blockIdx.y * 64;
+  float cmax = 0.f;
+  for (int r = threadIdx.x; r < T; r += blockDim.x) cmax = fmaxf(cmax, fabsf(row_stats[3 * T_max + r]));
+  cmax = block_max(cmax, red);
+  const float S = pow2_scale_from_bound(cmax * (1.f + (z_ref ? lam : 0.f)));
+  if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) { dl_scale[0] = S; dl_scale[1] = 1.f / S; }
+  // K index k of the operand -> canvas row: k < T16 is the (hi) plane of row k; with two planes (2 T16 <= 64) k in
+  // [T16, 2 T16) is the lo plane of row k - T16
+  if (threadIdx.x < 64) {
+    const int k = r0 + threadIdx.x;
+    const int r = (planes == 2 && k >= T16) ? k - T16 : k;
+    const bool ok = r < T && k < planes * T16;
+    sh[threadIdx.x] = ok ? row_stats[0 * T_max + r] : 0.f;
+    sh[64 + threadIdx.x] = ok ? row_stats[1 * T_max + r] : 0.f;
+    sh[128 + threadIdx.x] = ok ? row_stats[3 * T_max + r] : 0.f;
+    sh[192 + threadIdx.x] = ok ? row_stats[4 * T_max + r] : 0.f;
+  }
+  __syncthreads();
+  const int vv = threadIdx.x & 63;
+  const int v = v0 + vv;
+  for (int rr = threadIdx.x >> 6; rr < 64; rr += 4) {
+    const int k = r0 + rr;
+    const bool lo_plane = planes == 2 && k >= T16;
+    const int r = lo_plane ? k - T16 : k;
+    float dl = 0.f;
+    if (r < T && k < planes * T16) {
+      const float t = BF16 ? __bfloat162float(static_cast<const __nv_bfloat16*>(teacher)[(size_t)r * V + v])
+                           : static_cast<const float*>(teacher)[(size_t)r * V + v];
+      const float qv = expf(z[(size_t)r * z_ld + v] - sh[64 + rr]);
+      const float pv = expf(t - sh[rr]);   // t = -inf -> 0
+      float g = qv - pv;
+      if (z_ref) g += lam * (qv - expf(z_ref[(size_t)r * z_ld + v] - sh[192 + rr]));
+      dl = sh[128 + rr] * g * S;
+    }
+    __half hq = __float2half_rn(dl);
+    if (lo_plane) hq = __float2half_rn(dl - __half2float(hq));   // dl S = hi + lo to 2^-22
+    const uint16_t hv = __half_as_ushort(hq);
+    tile[vv * kPitch + rr] = hv;
+    if (dlR && k < planes * T16) dlR[(size_t)k * V + v] = hv;   // rows T .. T16 of a plane are zero
+  }
+  __syncthreads();
+  // 8 threads per vocabulary row: 16 bytes each -> one 128-byte segment of dlT per row
+  const int seg = threadIdx.x & 7;
+  for (int row = threadIdx.x >> 3; row < 64; row += 32) {
+    const uint2* src = reinterpret_cast<const uint2*>(tile + row * kPitch + seg * 8);
+    const uint2 a = src[0], b = src[1];
+    *reinterpret_cast<uint4*>(dlT + (size_t)(v0 + row) * Kp + r0 + seg * 8) = make_uint4(a.x, a.y, b.x, b.y);
+  }
+}
+
+template <bool ADAM, bool A_TMEM, int NV>
+cudaError_t launch_wide(int grid, size_t smem, cudaStream_t s, const CUtensorMap& tm_hTT, const CUtensorMap& tm_dlT,
+                        const CUtensorMap& tm_master, const CUtensorMap& tm_m, const CUtensorMap& tm_v,
+                        const CUtensorMap& tm_wout, const WideParams& p) {
+  tc_update_wide_kernel<ADAM, A_TMEM, NV><<<grid, kWThreads, smem, s>>>(tm_hTT, tm_dlT, tm_master, tm_m, tm_v, tm_wout, p);
+  return cudaGetLastError();
+}
+
+
+template <bool ADAM, bool A_TMEM, int NV>
+cudaError_t wide_attr() {
+  return cudaFuncSetAttribute(tc_update_wide_kernel<ADAM, A_TMEM, NV>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              kWSmemBudget + 2048);
+}
+
+}  // namespace
+
+cudaError_t tc_wide_init(tts_ctx*) {
+  cudaError_t e;
+  if ((e = wide_attr<true, true, 32>()) != cudaSuccess) return e;
+  if ((e = wide_attr<false, true, 32>()) != cudaSuccess) return e;
+  if ((e = wide_attr<true, false, 16>()) != cudaSuccess) return e;
+  return wide_attr<false, false, 16>();
+}
+
+// dl planes of the wide path: hi + lo while both fit the 64-wide K chunk (T16 <= 32), one plane beyond
+int tc_wide_planes(int T16) { return 2 * T16 <= kKC ? 2 : 1; }
+
+int tc_wide_a_in_tmem() {
+  static int v = -1;
+  if (v < 0) {
+    const char* e = getenv("TTS_WIDE_A_SMEM");   // measurement switch: keep the stripe's h^T in shared memory
+    v = (e && e[0] == '1') ? 0 : 1;
+  }
+  return v;
+}
+
+// a4 of the wide path: h^T rows and the fp16 dl planes
+cudaError_t tc_launch_prep_wide(tts_ctx* c, const StepArgs& a, const float* z, cudaStream_t s, int* launches) {
+  TcState* st = static_cast<TcState*>(c->tc_state);
+  const int V = c->cfg.V, d = c->cfg.d, T = a.T;
+  const int T16 = (T + 15) / 16 * 16;
+  const int Kp = (T16 + kKC - 1) / kKC * kKC;
+  unsigned int* absmax = reinterpret_cast<unsigned int*>(st->dl_scale + 4);
+  cudaError_t e = cudaMemsetAsync(absmax, 0, sizeof(unsigned int), s);
+  if (e != cudaSuccess) return e;
+  const __nv_bfloat16* h = static_cast<const __nv_bfloat16*>(a.h);
+  tc_h_absmax_kernel<<<64, 256, 0, s>>>(h, (size_t)T * d, absmax);
+  const int planes = tc_wide_planes(T16);
+  tc_prep_hT_kernel<<<dim3((d + 31) / 32, Kp / 32), 256, 0, s>>>(h, d, T, T16, planes, Kp, absmax,
+                                                                  static_cast<uint16_t*>(st->hTT), st->dl_scale);
+  uint16_t* dlT = static_cast<uint16_t*>(st->dlT);
+  uint16_t* dlR = a.gh_out ? static_cast<uint16_t*>(st->dlR) : nullptr;
+  const dim3 grid(V / 64, Kp / 64);
+  if (c->cfg.logits_dtype == TTS_BF16)
+    tc_prep_dl_wide_kernel<true><<<grid, 256, 0, s>>>(a.teacher, z, a.z_ref, a.lambda, V, V, T, T16, planes, Kp, c->cfg.T_max,
+                                                       c->row_stats, dlT, dlR, st->dl_scale);
+  else
+    tc_prep_dl_wide_kernel<false><<<grid, 256, 0, s>>>(a.teacher, z, a.z_ref, a.lambda, V, V, T, T16, planes, Kp, c->cfg.T_max,
+                                                        c->row_stats, dlT, dlR, st->dl_scale);
+  *launches += 3;
+  return cudaGetLastError();
+}
+
+// a6 + a7 of the wide path
+cudaError_t tc_launch_update_wide(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches) {
+  TcState* st = static_cast<TcState*>(c->tc_state);
+  const int V = c->cfg.V, d = c->cfg.d, T = a.T;
+  const int T16 = (T + 15) / 16 * 16;
+  const int Kp = (T16 + kKC - 1) / kKC * kKC;
+  const bool adam = c->cfg.optimizer == TTS_ADAMW;
+  const bool a_tmem = tc_wide_a_in_tmem() != 0;
+  const int NV = a_tmem ? 32 : 16;
+  CUtensorMap tm_hTT, tm_dlT, tm_master, tm_m, tm_v, tm_wout;
+  // the operand maps depend on this step's Kp (row pitch of the scratch)
+  if (make_map_2d(st, &tm_hTT, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, st->hTT, Kp, d, kKC, kWJ,
+                  CU_TENSOR_MAP_SWIZZLE_128B) != CUDA_SUCCESS)
+    return cudaErrorInvalidValue;
+  if (make_map_2d(st, &tm_dlT, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, st->dlT, Kp, V, kKC, NV,
+                  CU_TENSOR_MAP_SWIZZLE_128B) != CUDA_SUCCESS)
+    return cudaErrorInvalidValue;
+  if (make_map_2d(st, &tm_master, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, a.master, d, V, kWJ, kWSV,
+                  CU_TENSOR_MAP_SWIZZLE_NONE) != CUDA_SUCCESS)
+    return cudaErrorInvalidValue;
+  if (make_map_2d(st, &tm_wout, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, a.W_out, d, V, kWJ, kWSV,
+                  CU_TENSOR_MAP_SWIZZLE_NONE) != CUDA_SUCCESS)
+    return cudaErrorInvalidValue;
+  tm_m = tm_master;
+  tm_v = tm_master;
+  if (adam) {
+    if (make_map_2d(st, &tm_m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, a.adam_m, d, V, kWJ, kWSV,
+                    CU_TENSOR_MAP_SWIZZLE_NONE) != CUDA_SUCCESS)
+      return cudaErrorInvalidValue;
+    if (make_map_2d(st, &tm_v, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, a.adam_v, d, V, kWJ, kWSV,
+                    CU_TENSOR_MAP_SWIZZLE_NONE) != CUDA_SUCCESS)
+      return cudaErrorInvalidValue;
+  }
+  WideParams p;
+  p.gW_debug = a.gW_debug;
+  p.hTT = static_cast<const uint16_t*>(st->hTT);
+  p.dl_scale = st->dl_scale;
+  p.V = V; p.d = d; p.Kp = Kp;
+  p.n_stripes = d / kWJ;
+  p.n_bands = V / NV;
+  const long dl_bytes = (long)V * Kp * 2;
+  p.n_win = (int)((dl_bytes + kWWindowBytes - 1) / kWWindowBytes);
+  if (p.n_win < 1) p.n_win = 1;
+  if (p.n_win > p.n_bands) p.n_win = p.n_bands;
+  const int fixed = 1024 + (a_tmem ? 0 : Kp * kWJ * 2) + kWOpStages * NV * Kp * 2 + 2 * kWWoBytes + (int)sizeof(WideBars);
+  p.stages = (kWSmemBudget - fixed) / kWStageBytes;
+  if (p.stages > kWMaxStages) p.stages = kWMaxStages;
+  if (p.stages < 2) return cudaErrorInvalidConfiguration;
+  p.lr = a.lr; p.b1 = a.beta1; p.b2 = a.beta2; p.eps = a.eps;
+  p.decay = 1.f - a.lr * a.wd;
+  p.c1 = a.lr * a.inv_bc1;
+  p.inv_sqrt_bc2 = a.inv_sqrt_bc2;
+  const long units = (long)p.n_stripes * (p.n_bands / p.n_win);
+  int grid = c->cfg.max_ctas > 0 ? c->cfg.max_ctas : c->sm_count;
+  if (grid > units) grid = (int)units;
+  const size_t smem = (size_t)fixed + (size_t)p.stages * kWStageBytes;
+  cudaError_t e;
+  if (a_tmem)
+    e = adam ? launch_wide<true, true, 32>(grid, smem, s, tm_hTT, tm_dlT, tm_master, tm_m, tm_v, tm_wout, p)
+             : launch_wide<false, true, 32>(grid, smem, s, tm_hTT, tm_dlT, tm_master, tm_m, tm_v, tm_wout, p);
+  else
+    e = adam ? launch_wide<true, false, 16>(grid, smem, s, tm_hTT, tm_dlT, tm_master, tm_m, tm_v, tm_wout, p)
+             : launch_wide<false, false, 16>(grid, smem, s, tm_hTT, tm_dlT, tm_master, tm_m, tm_v, tm_wout, p);
+  *launches += 1;
+  return e;
+}
+
+}  // namespace tts

@@ -97,8 +97,12 @@ def make_case(cfg_id: int, *, V: int | None = None, d: int | None = None, n_seq:
     scaled down (V, d, n_seq, seg_len overrides keep the recipe).  Returns a dict of
     numpy arrays (bf16 as uint16 bits) plus the hyper-parameters.
 
-    nonzero_state: draw Adam moments as if ``step-1`` steps had happened (m ~ 1e-5 N(0,1),
-    v ~ 1e-10 chi^2) instead of the configs' m = v = 0, to exercise the general update.
+    nonzero_state: draw Adam moments as if ``step-1`` steps had happened instead of the configs'
+    m = v = 0, to exercise the general update: v ~ 1e-10 chi^2, m = sqrt(v) U(-3, 3).  The pair is drawn
+    so that it CAN be an Adam state: moments that are exponential averages of one gradient sequence
+    satisfy m^2 <= (1-b1)^2 / ((1-b2) (1 - b1^2/b2)) v = 52.8 v (Cauchy-Schwarz, b = 0.9 / 0.999).  Independent
+    draws of m and v do not (|m| / sqrt(v) is Cauchy-tailed), and where m^2 >> v the step is hundreds of lr and
+    ill-conditioned in g: a regime no run of the optimiser reaches (R12).
     """
     c = dict(CONFIGS[cfg_id])
     c.update(ADAM_DEFAULTS)
@@ -167,8 +171,8 @@ def make_case(cfg_id: int, *, V: int | None = None, d: int | None = None, n_seq:
     if c["optimizer"] == ADAMW:
         if nonzero_state:
             rs = np.random.Generator(np.random.PCG64(c["seed"] + 77))
-            out["m"] = (1e-5 * rs.standard_normal((V, d), dtype=np.float32)).astype(np.float32)
             out["v"] = (1e-10 * rs.standard_normal((V, d), dtype=np.float32) ** 2).astype(np.float32)
+            out["m"] = (np.sqrt(out["v"]) * rs.uniform(-3.0, 3.0, (V, d)).astype(np.float32)).astype(np.float32)
         else:
             out["m"] = np.zeros((V, d), dtype=np.float32)
             out["v"] = np.zeros((V, d), dtype=np.float32)
