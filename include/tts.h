@@ -270,6 +270,53 @@ int32_t tts_round_host(tts_ctx* ctx,
                        uint8_t* mask_host,              /* host [T] or NULL        */
                        void* stream);
 
+/*
+ * f4.  The step sharded over the VOCABULARY across n_shards GPUs, one process per GPU.  Shard g owns
+ * cfg.V consecutive rows [v_offset, v_offset + cfg.V) of W / master / m / v (each process creates its ctx with its
+ * own local V) and the matching columns of the teacher logits as a contiguous [T, cfg.V] tensor -- the way a
+ * tensor-parallel target delivers them.  h, pos_weight, mask and the draft tokens are replicated.  The paper's TTS
+ * runs on one GPU; the shard axis follows from the step's algebra: every quantity that couples
+ * vocabulary rows is a per-canvas-row reduction, so the exchange is tiny and the 28 bytes per parameter stay local.
+ *   1. tts_shard_begin_step   a2 + this shard's a3 sweep; stats_out [T, 8] fp32 = per row the online tuple
+ *                             (m_t, s_t, a, m_z, s_z, m_ref, s_ref, b) of SURVEY 8(a) a3 over the shard's columns
+ *   2. the caller all-gathers the tuples -> stats_all [n_shards, T, 8]           (32 T bytes per rank)
+ *   3. tts_shard_finish_step  merges the tuples (associative: same rule as between CTAs) into the GLOBAL lse_t,
+ *                             lse_z, KL_r and loss -- identical on every shard -- then a4 .. a7 on the shard's rows
+ *                             with no further communication; gh_partial_out [T, d] = this shard's sum over its rows
+ *   4. the caller all-reduces (sum) gh_partial_out                               (4 T d bytes)
+ * Between 1 and 3 the ctx keeps the shard's draft logits: call them in pairs, with the same T and extras, on the
+ * same stream.  Adam's step count advances in tts_shard_finish_step.  With n_shards = 1 the pair equals
+ * tts_distill_step_ex.  For the mask, tts_shard_argmax gives this shard's (max value, GLOBAL index = local index +
+ * v_offset; 0x7fffffff for an all -inf slice) per row, the caller all-gathers both [T] arrays, and
+ * tts_shard_accept_mask applies the lowest-global-index rule (R11) and the prefix logic of tts_accept_mask.
+ */
+enum { TTS_SHARD_STAT_FIELDS = 8 };
+int32_t tts_shard_begin_step(tts_ctx* ctx,
+                             const void* teacher_logits_local, /* [T, cfg.V] logits_dtype                   */
+                             const void* h,                    /* [T, d]                                   */
+                             const void* W_in_local,           /* [cfg.V, d]                               */
+                             int32_t T,
+                             const tts_step_extras* extras,    /* host, may be NULL; logits pointers are local [T, cfg.V] */
+                             float* stats_out,                 /* [T, 8]                                   */
+                             void* side_stream);
+int32_t tts_shard_finish_step(tts_ctx* ctx,
+                              const float* stats_all,          /* [n_shards, T, 8], own shard included     */
+                              int32_t n_shards,                /* 1..1024                                  */
+                              const void* teacher_logits_local, const void* h, const void* W_in_local,
+                              void* W_out_local, float* W_master_local, float* adam_m_local, float* adam_v_local,
+                              const float* pos_weight, const uint8_t* mask, int32_t T, float loss_scale,
+                              float* loss_out,                 /* [1] the GLOBAL loss                      */
+                              float* kl_rows_out,              /* [T] global KL_r, or NULL                 */
+                              float* gh_partial_out,           /* [T, d] this shard's part of gh, or NULL  */
+                              float* gW_debug_out,             /* [cfg.V, d] or NULL                       */
+                              const tts_step_extras* extras, void* side_stream);
+int32_t tts_shard_argmax(tts_ctx* ctx, const void* teacher_logits_local, int32_t T, int32_t v_offset,
+                         float* val_out /* [T] */, int32_t* idx_out /* [T] */, void* stream);
+int32_t tts_shard_accept_mask(tts_ctx* ctx, const float* val_all /* [n_shards, T] */,
+                              const int32_t* idx_all /* [n_shards, T] */, int32_t n_shards,
+                              const int32_t* draft_tokens, int32_t T, uint8_t* mask_out, int32_t* tau_out,
+                              int32_t* teacher_argmax_out /* [T] or NULL */, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -33,6 +33,10 @@ What it computes, with the passage each step follows
                           rows, given the full-vocabulary normalisers, so that a
                           full-size configuration can be checked on samples.
 
+  * ``shard_row_stats`` / ``merge_shard_stats``  the per-row online tuple (m_t, s_t, a, m_z, s_z) over a slice of
+                          the vocabulary and its associative merge: what vocabulary shards exchange (SURVEY 8(e));
+                          pinned against the plain logsumexp / KL of the whole row.
+
 Pins (tests/test_oracle_pins.py): brute-force enumeration through the softmax
 Jacobian, central finite differences, closed forms (V=2, uniform draft,
 one-hot teacher, teacher == draft), invariants, and reduction to fp64
@@ -394,3 +398,46 @@ def gh_full(z, lse_t, lse_z, teacher_logits, W_in, omega, loss_scale=1.0, slab=8
         dl = loss_scale * om[:, None] * (np.exp(z[:, sl] - lse_z[:, None]) - np.exp(t[:, sl] - lse_t[:, None]))
         gh += dl @ widen(W_in[sl])
     return gh
+
+
+# ----------------------------------------------------------------------------
+# what vocabulary shards exchange
+# ----------------------------------------------------------------------------
+
+def shard_row_stats(teacher_cols, z_cols):
+    """Per row, over the columns of one vocabulary slice:
+        m_t = max t,  s_t = sum e^{t - m_t},  a = sum e^{t - m_t} (t - z),  m_z = max z,  s_z = sum e^{z - m_z}
+    Teacher entries equal to -inf have p = 0 and are dropped (0 log 0 := 0); a slice whose teacher entries are all
+    -inf gives (m_t, s_t, a) = (-inf, 0, 0).  Returns [T, 5] fp64."""
+    t = widen(teacher_cols)
+    z = np.asarray(z_cols, dtype=np.float64)
+    T = t.shape[0]
+    out = np.zeros((T, 5), dtype=np.float64)
+    for r in range(T):
+        keep = t[r] != -np.inf
+        if keep.any():
+            mt = t[r][keep].max()
+            e = np.exp(t[r][keep] - mt)
+            out[r, 0], out[r, 1], out[r, 2] = mt, e.sum(), (e * (t[r][keep] - z[r][keep])).sum()
+        else:
+            out[r, 0] = -np.inf
+        mz = z[r].max()
+        out[r, 3], out[r, 4] = mz, np.exp(z[r] - mz).sum()
+    return out
+
+
+def merge_shard_stats(stats_all):
+    """stats_all [G, T, 5] -> (lse_t, lse_z, KL_r) of the whole rows: rescale every slice to the common maximum,
+    add, then  lse_t = m_t + log s_t,  lse_z = m_z + log s_z,  KL_r = a / s_t - lse_t + lse_z."""
+    st = np.asarray(stats_all, dtype=np.float64)
+    mt = st[:, :, 0].max(axis=0)
+    mz = st[:, :, 3].max(axis=0)
+    with np.errstate(invalid="ignore"):
+        et = np.where(st[:, :, 0] == -np.inf, 0.0, np.exp(st[:, :, 0] - mt[None, :]))
+    ez = np.exp(st[:, :, 3] - mz[None, :])
+    s_t = (st[:, :, 1] * et).sum(axis=0)
+    a = (st[:, :, 2] * et).sum(axis=0)
+    s_z = (st[:, :, 4] * ez).sum(axis=0)
+    lse_t = mt + np.log(s_t)
+    lse_z = mz + np.log(s_z)
+    return lse_t, lse_z, a / s_t - lse_t + lse_z

@@ -187,11 +187,16 @@ int32_t tts_distill_step(tts_ctx* c, const void* teacher, const void* h, const v
                              loss_out, kl_rows_out, gh_out, gW_debug_out, nullptr, side_stream);
 }
 
-int32_t tts_distill_step_ex(tts_ctx* c, const void* teacher, const void* h, const void* W_in, void* W_out,
-                            float* W_master, float* adam_m, float* adam_v, const float* pos_weight,
-                            const uint8_t* mask, int32_t T, float loss_scale, float* loss_out, float* kl_rows_out,
-                            float* gh_out, float* gW_debug_out, const tts_step_extras* ex, void* side_stream) {
-  if (!c || !teacher || !h || !W_in || !W_out || !pos_weight || !loss_out) return TTS_ERR_INVALID_ARG;
+// The step of include/tts.h in one piece (phase 0) or as the two halves of the vocabulary-sharded step.
+static int32_t run_step(tts_ctx* c, const void* teacher, const void* h, const void* W_in, void* W_out,
+                        float* W_master, float* adam_m, float* adam_v, const float* pos_weight,
+                        const uint8_t* mask, int32_t T, float loss_scale, float* loss_out, float* kl_rows_out,
+                        float* gh_out, float* gW_debug_out, const tts_step_extras* ex, void* side_stream, int phase,
+                        float* stats_out, const float* stats_all, int32_t n_shards) {
+  if (!c || !teacher || !h || !W_in) return TTS_ERR_INVALID_ARG;
+  if (phase != tts::kPhaseBegin && (!W_out || !pos_weight || !loss_out)) return TTS_ERR_INVALID_ARG;
+  if (phase == tts::kPhaseBegin && !stats_out) return TTS_ERR_INVALID_ARG;
+  if (phase == tts::kPhaseFinish && (!stats_all || n_shards < 1 || n_shards > 1024)) return TTS_ERR_INVALID_ARG;
   if (ex) {
     if (!(ex->lambda >= 0.f)) return TTS_ERR_INVALID_ARG;
     if (ex->draft_logits && ex->draft_logits_out) return TTS_ERR_INVALID_ARG;   // nothing is computed to write out
@@ -200,18 +205,21 @@ int32_t tts_distill_step_ex(tts_ctx* c, const void* teacher, const void* h, cons
   }
   const tts_config& cfg = c->cfg;
   if (T <= 0 || T > cfg.T_max || T % cfg.seg_len != 0) return TTS_ERR_INVALID_ARG;
-  if ((cfg.param_dtype == TTS_BF16) != (W_master != nullptr)) return TTS_ERR_INVALID_ARG;
-  if ((cfg.optimizer == TTS_ADAMW) != (adam_m != nullptr && adam_v != nullptr)) return TTS_ERR_INVALID_ARG;
-  if (cfg.optimizer == TTS_SGD && (adam_m || adam_v)) return TTS_ERR_INVALID_ARG;
-  if (cfg.mask_mode != TTS_ROWS_ALL && !mask) return TTS_ERR_INVALID_ARG;
+  if (phase != tts::kPhaseBegin) {
+    if ((cfg.param_dtype == TTS_BF16) != (W_master != nullptr)) return TTS_ERR_INVALID_ARG;
+    if ((cfg.optimizer == TTS_ADAMW) != (adam_m != nullptr && adam_v != nullptr)) return TTS_ERR_INVALID_ARG;
+    if (cfg.optimizer == TTS_SGD && (adam_m || adam_v)) return TTS_ERR_INVALID_ARG;
+    if (cfg.mask_mode != TTS_ROWS_ALL && !mask) return TTS_ERR_INVALID_ARG;
+  }
   if (!aligned16(teacher) || !aligned16(h) || !aligned16(W_in) || !aligned16(W_out) || !aligned16(W_master) ||
       !aligned16(adam_m) || !aligned16(adam_v) || !aligned16(gh_out) || !aligned16(gW_debug_out))
     return TTS_ERR_INVALID_ARG;
 
   cudaStream_t s = static_cast<cudaStream_t>(side_stream);
-  c->step_count += 1;
-  const double n = static_cast<double>(c->step_count);
+  if (phase != tts::kPhaseBegin) c->step_count += 1;     // Adam's count advances once per step: in the second half
+  const double n = static_cast<double>(c->step_count > 0 ? c->step_count : 1);
   tts::StepArgs a;
+  a.phase = phase; a.shard_stats_out = stats_out; a.shard_stats_all = stats_all; a.n_shards = n_shards;
   a.teacher = teacher; a.h = h; a.W_in = W_in; a.W_out = W_out;
   a.master = W_master; a.adam_m = adam_m; a.adam_v = adam_v;
   a.pos_weight = pos_weight; a.mask = mask; a.T = T; a.loss_scale = loss_scale;
@@ -226,6 +234,8 @@ int32_t tts_distill_step_ex(tts_ctx* c, const void* teacher, const void* h, cons
 
   int launches = 0;
   cudaError_t e;
+  const bool prof_saved = c->prof_on;
+  if (phase != tts::kPhaseAll) c->prof_on = false;       // the phase events describe whole steps only
   tts::prof_mark(c, -1, s);
   if (c->tensor_ok) {
     c->last_used_tensor = 1;
@@ -235,11 +245,60 @@ int32_t tts_distill_step_ex(tts_ctx* c, const void* teacher, const void* h, cons
     e = tts::simt_step(c, a, s, &launches);
   }
   c->last_launches = launches;
-  if (e != cudaSuccess) return cuda_fail(c, e);
+  if (e != cudaSuccess) { c->prof_on = prof_saved; return cuda_fail(c, e); }
   if (c->prof_on) c->prof_count += 1;
+  c->prof_on = prof_saved;
   if ((e = cudaEventRecord(c->done_event, s)) != cudaSuccess) return cuda_fail(c, e);
   c->done_recorded = true;
   return TTS_OK;
+}
+
+int32_t tts_distill_step_ex(tts_ctx* c, const void* teacher, const void* h, const void* W_in, void* W_out,
+                            float* W_master, float* adam_m, float* adam_v, const float* pos_weight,
+                            const uint8_t* mask, int32_t T, float loss_scale, float* loss_out, float* kl_rows_out,
+                            float* gh_out, float* gW_debug_out, const tts_step_extras* ex, void* side_stream) {
+  return run_step(c, teacher, h, W_in, W_out, W_master, adam_m, adam_v, pos_weight, mask, T, loss_scale, loss_out,
+                  kl_rows_out, gh_out, gW_debug_out, ex, side_stream, tts::kPhaseAll, nullptr, nullptr, 0);
+}
+
+int32_t tts_shard_begin_step(tts_ctx* c, const void* teacher_local, const void* h, const void* W_in_local, int32_t T,
+                             const tts_step_extras* ex, float* stats_out, void* side_stream) {
+  if (stats_out && !aligned16(stats_out)) return TTS_ERR_INVALID_ARG;
+  return run_step(c, teacher_local, h, W_in_local, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, T, 1.f, nullptr,
+                  nullptr, nullptr, nullptr, ex, side_stream, tts::kPhaseBegin, stats_out, nullptr, 0);
+}
+
+int32_t tts_shard_finish_step(tts_ctx* c, const float* stats_all, int32_t n_shards, const void* teacher_local,
+                              const void* h, const void* W_in_local, void* W_out_local, float* W_master_local,
+                              float* adam_m_local, float* adam_v_local, const float* pos_weight, const uint8_t* mask,
+                              int32_t T, float loss_scale, float* loss_out, float* kl_rows_out, float* gh_partial_out,
+                              float* gW_debug_out, const tts_step_extras* ex, void* side_stream) {
+  return run_step(c, teacher_local, h, W_in_local, W_out_local, W_master_local, adam_m_local, adam_v_local, pos_weight,
+                  mask, T, loss_scale, loss_out, kl_rows_out, gh_partial_out, gW_debug_out, ex, side_stream,
+                  tts::kPhaseFinish, nullptr, stats_all, n_shards);
+}
+
+int32_t tts_shard_argmax(tts_ctx* c, const void* teacher_local, int32_t T, int32_t v_offset, float* val_out,
+                         int32_t* idx_out, void* stream) {
+  if (!c || !teacher_local || !val_out || !idx_out || v_offset < 0) return TTS_ERR_INVALID_ARG;
+  if (T <= 0 || T > c->cfg.T_max || T % c->cfg.seg_len != 0 || !aligned16(teacher_local)) return TTS_ERR_INVALID_ARG;
+  int launches = 0;
+  cudaError_t e = tts::launch_shard_argmax(c, teacher_local, T, v_offset, val_out, idx_out,
+                                           static_cast<cudaStream_t>(stream), &launches);
+  c->last_launches = launches;
+  return e == cudaSuccess ? TTS_OK : cuda_fail(c, e);
+}
+
+int32_t tts_shard_accept_mask(tts_ctx* c, const float* val_all, const int32_t* idx_all, int32_t n_shards,
+                              const int32_t* tok, int32_t T, uint8_t* mask_out, int32_t* tau_out, int32_t* am_out,
+                              void* stream) {
+  if (!c || !val_all || !idx_all || !tok || !mask_out || !tau_out || n_shards < 1) return TTS_ERR_INVALID_ARG;
+  if (T <= 0 || T > c->cfg.T_max || T % c->cfg.seg_len != 0) return TTS_ERR_INVALID_ARG;
+  int launches = 0;
+  cudaError_t e = tts::launch_shard_mask(c, val_all, idx_all, n_shards, tok, T, mask_out, tau_out, am_out,
+                                         static_cast<cudaStream_t>(stream), &launches);
+  c->last_launches = launches;
+  return e == cudaSuccess ? TTS_OK : cuda_fail(c, e);
 }
 
 int32_t tts_distill_inner_steps(tts_ctx* c, const void* teacher, const void* h, const void* W_in, void* W_out,

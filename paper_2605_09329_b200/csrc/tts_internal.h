@@ -38,6 +38,12 @@ struct StepArgs {
   float* z_keep;          // [T,V] fp32: a2 writes z here instead of the ctx scratch (it becomes z_ref of later inner steps) or NULL
   const float* z_ref;     // [T,V] fp32 logits of q_t for the lambda term or NULL
   float lambda;           // weight of K~L(q_t || q)
+  // SURVEY 8(e), the step sharded over the vocabulary: phase 1 = a2 + this shard's a3 sweep -> shard_stats_out;
+  // phase 2 = merge of all shards' tuples -> a4 .. a7 on this shard; 0 = the whole step on one GPU
+  int phase;
+  float* shard_stats_out;        // [T, kStatFields]            (phase 1)
+  const float* shard_stats_all;  // [n_shards, T, kStatFields]  (phase 2)
+  int n_shards;
   // optimiser scalars for this step (bias corrections precomputed on the host in fp64)
   float lr, beta1, beta2, eps, wd;
   float inv_bc1;       // 1 / (1 - beta1^n)
@@ -102,6 +108,11 @@ inline void prof_mark(tts_ctx* c, int phase, cudaStream_t s) {
 // tts_mask.cu
 cudaError_t launch_accept_mask(tts_ctx* c, const void* teacher, const int32_t* tok, int T, uint8_t* mask,
                                int32_t* tau, int32_t* am_out, cudaStream_t s, int* launches);
+cudaError_t launch_shard_argmax(tts_ctx* c, const void* teacher, int T, int v_offset, float* val, int32_t* idx,
+                                cudaStream_t s, int* launches);
+cudaError_t launch_shard_mask(tts_ctx* c, const float* val_all, const int32_t* idx_all, int n_shards,
+                              const int32_t* tok, int T, uint8_t* mask, int32_t* tau, int32_t* am_out, cudaStream_t s,
+                              int* launches);
 // tts_accept.cu (f2)
 cudaError_t launch_accept_stochastic(tts_ctx* c, const void* teacher, const float* z, const int32_t* tok,
                                      const float* u, const float* u2, int T, uint8_t* mask, int32_t* tau,
@@ -109,6 +120,12 @@ cudaError_t launch_accept_stochastic(tts_ctx* c, const void* teacher, const floa
 // tts_stats.cu: row statistics + merge + loss (CUDA-core sweeps shared by both paths).
 // z_ld = leading dimension (row stride in floats) of the z scratch.
 cudaError_t launch_row_stats(tts_ctx* c, const StepArgs& a, const float* z, int z_ld, cudaStream_t s, int* launches);
+cudaError_t launch_row_stats_shard(tts_ctx* c, const StepArgs& a, const float* z, int z_ld, float* stats_out,
+                                   cudaStream_t s, int* launches);
+cudaError_t launch_row_stats_merge_shards(tts_ctx* c, const StepArgs& a, const float* stats_all, int n_shards,
+                                          cudaStream_t s, int* launches);
+// a2 + a3 of either path for the phase of `a`: returns after phase 1, or leaves the row normalisers in c->row_stats
+enum { kPhaseAll = 0, kPhaseBegin = 1, kPhaseFinish = 2 };
 // tts_simt.cu
 cudaError_t simt_step(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches);
 cudaError_t simt_launch_gh(tts_ctx* c, const StepArgs& a, const float* dl32, cudaStream_t s, int* launches);

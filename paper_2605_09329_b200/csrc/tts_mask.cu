@@ -90,14 +90,29 @@ __global__ void __launch_bounds__(256) argmax_partial_kernel(const void* __restr
   }
 }
 
+// the splits of one row merged into this shard's (max value, GLOBAL index = local index + v_offset)
+__global__ void __launch_bounds__(256) argmax_reduce_kernel(const float* __restrict__ pv, const int* __restrict__ pi,
+                                                            int splits, int T, int v_offset, float* __restrict__ val,
+                                                            int32_t* __restrict__ idx) {
+  for (int r = blockIdx.x * blockDim.x + threadIdx.x; r < T; r += gridDim.x * blockDim.x) {
+    ArgPair best{-CUDART_INF_F, 0x7fffffff};
+    for (int s = 0; s < splits; ++s) best = arg_better(best, ArgPair{pv[(size_t)r * splits + s], pi[(size_t)r * splits + s]});
+    val[r] = best.v;
+    idx[r] = best.i == 0x7fffffff ? 0x7fffffff : best.i + v_offset;
+  }
+}
+
+// pv / pi hold `splits` candidates per row: element (r, s) at r * row_stride + s * split_stride
 __global__ void __launch_bounds__(256) mask_finalize_kernel(const float* __restrict__ pv, const int* __restrict__ pi,
-                                                            int splits, const int32_t* __restrict__ tok, int T,
+                                                            int splits, long row_stride, long split_stride,
+                                                            const int32_t* __restrict__ tok, int T,
                                                             int seg_len, uint8_t* __restrict__ mask,
                                                             int32_t* __restrict__ tau, int32_t* __restrict__ am_out,
                                                             int32_t* __restrict__ am_tmp) {
   for (int r = threadIdx.x; r < T; r += blockDim.x) {
     ArgPair best{-CUDART_INF_F, 0x7fffffff};
-    for (int s = 0; s < splits; ++s) best = arg_better(best, ArgPair{pv[(size_t)r * splits + s], pi[(size_t)r * splits + s]});
+    for (int s = 0; s < splits; ++s)
+      best = arg_better(best, ArgPair{pv[r * row_stride + s * split_stride], pi[r * row_stride + s * split_stride]});
     // a row of only -inf (or an empty slice everywhere) resolves to index 0, like the lowest-index rule
     const int am = best.i == 0x7fffffff ? 0 : best.i;
     am_tmp[r] = am;
@@ -118,8 +133,7 @@ __global__ void __launch_bounds__(256) mask_finalize_kernel(const float* __restr
   }
 }
 
-cudaError_t launch_accept_mask(tts_ctx* c, const void* teacher, const int32_t* tok, int T, uint8_t* mask,
-                               int32_t* tau, int32_t* am_out, cudaStream_t s, int* launches) {
+static int launch_argmax_partial(tts_ctx* c, const void* teacher, int T, cudaStream_t s) {
   const int V = c->cfg.V;
   const bool bf = c->cfg.logits_dtype == TTS_BF16;
   // enough CTAs to fill the machine at small T, at most kArgSplitsMax per row, slices a multiple of 8
@@ -133,9 +147,34 @@ cudaError_t launch_accept_mask(tts_ctx* c, const void* teacher, const int32_t* t
     argmax_partial_kernel<true><<<grid, 256, 0, s>>>(teacher, V, chunk, c->arg_val, c->arg_idx);
   else
     argmax_partial_kernel<false><<<grid, 256, 0, s>>>(teacher, V, chunk, c->arg_val, c->arg_idx);
-  mask_finalize_kernel<<<1, 256, 0, s>>>(c->arg_val, c->arg_idx, splits, tok, T, c->cfg.seg_len, mask, tau, am_out,
-                                         c->argmax_tmp);
+  return splits;
+}
+
+cudaError_t launch_accept_mask(tts_ctx* c, const void* teacher, const int32_t* tok, int T, uint8_t* mask,
+                               int32_t* tau, int32_t* am_out, cudaStream_t s, int* launches) {
+  const int splits = launch_argmax_partial(c, teacher, T, s);
+  mask_finalize_kernel<<<1, 256, 0, s>>>(c->arg_val, c->arg_idx, splits, splits, 1, tok, T, c->cfg.seg_len, mask, tau,
+                                         am_out, c->argmax_tmp);
   *launches += 2;
+  return cudaGetLastError();
+}
+
+// shard: (max, global index) of this shard's columns per row
+cudaError_t launch_shard_argmax(tts_ctx* c, const void* teacher, int T, int v_offset, float* val, int32_t* idx,
+                                cudaStream_t s, int* launches) {
+  const int splits = launch_argmax_partial(c, teacher, T, s);
+  argmax_reduce_kernel<<<(T + 255) / 256, 256, 0, s>>>(c->arg_val, c->arg_idx, splits, T, v_offset, val, idx);
+  *launches += 2;
+  return cudaGetLastError();
+}
+
+// shard: candidates of all shards [n_shards, T] -> mask, tau (lowest global index wins ties, as on one GPU)
+cudaError_t launch_shard_mask(tts_ctx* c, const float* val_all, const int32_t* idx_all, int n_shards,
+                              const int32_t* tok, int T, uint8_t* mask, int32_t* tau, int32_t* am_out, cudaStream_t s,
+                              int* launches) {
+  mask_finalize_kernel<<<1, 256, 0, s>>>(val_all, idx_all, n_shards, 1, T, tok, T, c->cfg.seg_len, mask, tau, am_out,
+                                         c->argmax_tmp);
+  *launches += 1;
   return cudaGetLastError();
 }
 

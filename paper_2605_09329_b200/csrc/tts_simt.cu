@@ -175,12 +175,19 @@ static cudaError_t simt_step_t(tts_ctx* c, const StepArgs& a, cudaStream_t s, in
   const bool bf_logits = c->cfg.logits_dtype == TTS_BF16;
 
   const float* z = z_src(a, c->z);
-  if (!a.z_given) {
-    simt_logits_kernel<PT><<<dim3((V + 63) / 64, (T + 15) / 16), 256, 0, s>>>(h, W_in, T, V, d, z_dst(a, c->z), V);
-    *launches += 1;
+  cudaError_t e;
+  if (a.phase != kPhaseFinish) {
+    if (!a.z_given) {
+      simt_logits_kernel<PT><<<dim3((V + 63) / 64, (T + 15) / 16), 256, 0, s>>>(h, W_in, T, V, d, z_dst(a, c->z), V);
+      *launches += 1;
+    }
+    prof_mark(c, 0, s);
+    if (a.phase == kPhaseBegin) return launch_row_stats_shard(c, a, z, V, a.shard_stats_out, s, launches);
+    e = launch_row_stats(c, a, z, V, s, launches);
+  } else {
+    prof_mark(c, 0, s);
+    e = launch_row_stats_merge_shards(c, a, a.shard_stats_all, a.n_shards, s, launches);
   }
-  prof_mark(c, 0, s);
-  cudaError_t e = launch_row_stats(c, a, z, V, s, launches);
   if (e != cudaSuccess) return e;
   prof_mark(c, 1, s);
   {

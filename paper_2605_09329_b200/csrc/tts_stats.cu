@@ -155,7 +155,8 @@ __global__ void __launch_bounds__(256) row_stats_partial_kernel(const void* __re
 // The maxima are exact in fp32; the rescaled sums and the final a / s_t - lse_t + lse_z (a difference of numbers
 // ~10 for a result that can be ~0.01) are formed in double.  With z_ref (has_ref) the loss gains
 // lambda * sum_r omega_r K~L(q_ref || q)_r.
-__global__ void __launch_bounds__(1024) row_stats_merge_kernel(const float* __restrict__ part, int splits, int T,
+__global__ void __launch_bounds__(1024) row_stats_merge_kernel(const float* __restrict__ part, int splits,
+                                                               long row_stride, long split_stride, int T,
                                                                int T_max, int seg_len, int mask_mode,
                                                                const float* __restrict__ pos_weight,
                                                                const uint8_t* __restrict__ mask, float loss_scale,
@@ -167,16 +168,16 @@ __global__ void __launch_bounds__(1024) row_stats_merge_kernel(const float* __re
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
   double local = 0.0;
   for (int r = warp; r < T; r += n_warps) {
-    const float* pr = part + (size_t)r * splits * kStatFields;
+    const float* pr = part + (size_t)r * row_stride;
     float mt = -CUDART_INF_F, mz = -CUDART_INF_F, mr = -CUDART_INF_F;
     for (int s = lane; s < splits; s += 32) {
-      const float* p = pr + s * kStatFields;
+      const float* p = pr + s * split_stride;
       mt = fmaxf(mt, p[0]); mz = fmaxf(mz, p[3]); mr = fmaxf(mr, p[5]);
     }
     mt = warp_max(mt); mz = warp_max(mz); mr = warp_max(mr);
     double st = 0.0, a = 0.0, sz = 0.0, sr = 0.0, b = 0.0;
     for (int s = lane; s < splits; s += 32) {
-      const float* p = pr + s * kStatFields;
+      const float* p = pr + s * split_stride;
       if (p[0] != -CUDART_INF_F) {
         const double e = exp((double)p[0] - (double)mt);
         st += (double)p[1] * e; a += (double)p[2] * e;
@@ -225,7 +226,43 @@ __global__ void __launch_bounds__(1024) row_stats_merge_kernel(const float* __re
   }
 }
 
-cudaError_t launch_row_stats(tts_ctx* c, const StepArgs& a, const float* z, int z_ld, cudaStream_t s, int* launches) {
+// the splits of one row merged into ONE tuple (m_t, s_t, a, m_z, s_z, m_ref, s_ref, b) instead of the
+// normalisers: what a vocabulary shard hands to the other shards.  Same arithmetic as the merge kernel (maxima exact,
+// rescaled sums in double), so merging the shards' tuples equals merging all their splits up to fp32 rounding of
+// the eight numbers.  One warp per row.
+__global__ void __launch_bounds__(1024) row_stats_reduce_kernel(const float* __restrict__ part, int splits, int T,
+                                                                float* __restrict__ out) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
+  for (int r = warp; r < T; r += n_warps) {
+    const float* pr = part + (size_t)r * splits * kStatFields;
+    float mt = -CUDART_INF_F, mz = -CUDART_INF_F, mr = -CUDART_INF_F;
+    for (int s = lane; s < splits; s += 32) {
+      const float* p = pr + s * kStatFields;
+      mt = fmaxf(mt, p[0]); mz = fmaxf(mz, p[3]); mr = fmaxf(mr, p[5]);
+    }
+    mt = warp_max(mt); mz = warp_max(mz); mr = warp_max(mr);
+    double st = 0.0, a = 0.0, sz = 0.0, sr = 0.0, b = 0.0;
+    for (int s = lane; s < splits; s += 32) {
+      const float* p = pr + s * kStatFields;
+      if (p[0] != -CUDART_INF_F) {
+        const double e = exp((double)p[0] - (double)mt);
+        st += (double)p[1] * e; a += (double)p[2] * e;
+      }
+      if (p[3] != -CUDART_INF_F) sz += (double)p[4] * exp((double)p[3] - (double)mz);
+      if (p[5] != -CUDART_INF_F) {
+        const double e = exp((double)p[5] - (double)mr);
+        sr += (double)p[6] * e; b += (double)p[7] * e;
+      }
+    }
+    st = warp_sum(st); a = warp_sum(a); sz = warp_sum(sz); sr = warp_sum(sr); b = warp_sum(b);
+    if (lane == 0) {
+      float* o = out + (size_t)r * kStatFields;
+      o[0] = mt; o[1] = (float)st; o[2] = (float)a; o[3] = mz; o[4] = (float)sz; o[5] = mr; o[6] = (float)sr; o[7] = (float)b;
+    }
+  }
+}
+
+static int launch_partial(tts_ctx* c, const StepArgs& a, const float* z, int z_ld, cudaStream_t s) {
   const int V = c->cfg.V, T = a.T;
   int splits = (2 * c->sm_count + T - 1) / T;
   splits = max(1, min(splits, kStatSplitsMax));
@@ -237,11 +274,39 @@ cudaError_t launch_row_stats(tts_ctx* c, const StepArgs& a, const float* z, int 
     row_stats_partial_kernel<true><<<grid, 256, 0, s>>>(a.teacher, z, a.z_ref, V, z_ld, chunk, c->stat_part);
   else
     row_stats_partial_kernel<false><<<grid, 256, 0, s>>>(a.teacher, z, a.z_ref, V, z_ld, chunk, c->stat_part);
-  row_stats_merge_kernel<<<1, T >= 32 ? 1024 : 32 * T, 0, s>>>(c->stat_part, splits, T, c->cfg.T_max, c->cfg.seg_len,
-                                                              c->cfg.mask_mode, a.pos_weight, a.mask, a.loss_scale,
-                                                              a.z_ref != nullptr, a.lambda, c->row_stats,
+  return splits;
+}
+
+static void launch_merge(tts_ctx* c, const StepArgs& a, const float* part, int splits, long row_stride,
+                         long split_stride, cudaStream_t s) {
+  const int T = a.T;
+  row_stats_merge_kernel<<<1, T >= 32 ? 1024 : 32 * T, 0, s>>>(part, splits, row_stride, split_stride, T, c->cfg.T_max,
+                                                              c->cfg.seg_len, c->cfg.mask_mode, a.pos_weight, a.mask,
+                                                              a.loss_scale, a.z_ref != nullptr, a.lambda, c->row_stats,
                                                               a.kl_rows_out, a.loss_out);
+}
+
+cudaError_t launch_row_stats(tts_ctx* c, const StepArgs& a, const float* z, int z_ld, cudaStream_t s, int* launches) {
+  const int splits = launch_partial(c, a, z, z_ld, s);
+  launch_merge(c, a, c->stat_part, splits, (long)splits * kStatFields, kStatFields, s);
   *launches += 2;
+  return cudaGetLastError();
+}
+
+// shard: this shard's sweep, one tuple per row into stats_out [T, kStatFields]
+cudaError_t launch_row_stats_shard(tts_ctx* c, const StepArgs& a, const float* z, int z_ld, float* stats_out,
+                                   cudaStream_t s, int* launches) {
+  const int splits = launch_partial(c, a, z, z_ld, s);
+  row_stats_reduce_kernel<<<1, a.T >= 32 ? 1024 : 32 * a.T, 0, s>>>(c->stat_part, splits, a.T, stats_out);
+  *launches += 2;
+  return cudaGetLastError();
+}
+
+// shard: the tuples of all shards, stats_all [n_shards, T, kStatFields] -> normalisers, KL, omega, loss
+cudaError_t launch_row_stats_merge_shards(tts_ctx* c, const StepArgs& a, const float* stats_all, int n_shards,
+                                          cudaStream_t s, int* launches) {
+  launch_merge(c, a, stats_all, n_shards, kStatFields, (long)a.T * kStatFields, s);
+  *launches += 1;
   return cudaGetLastError();
 }
 

@@ -62,9 +62,15 @@ cudaError_t tc_step(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches
 
   // a2: draft logits on tcgen05 (skipped when the caller supplies them), a3: row statistics + loss
   const float* z = z_src(a, c->z);
-  if (!a.z_given && (e = tc_launch_logits(c, a, z_dst(a, c->z), s, launches)) != cudaSuccess) return e;
-  prof_mark(c, 0, s);
-  if ((e = launch_row_stats(c, a, z, V, s, launches)) != cudaSuccess) return e;
+  if (a.phase != kPhaseFinish) {
+    if (!a.z_given && (e = tc_launch_logits(c, a, z_dst(a, c->z), s, launches)) != cudaSuccess) return e;
+    prof_mark(c, 0, s);
+    if (a.phase == kPhaseBegin) return launch_row_stats_shard(c, a, z, V, a.shard_stats_out, s, launches);
+    if ((e = launch_row_stats(c, a, z, V, s, launches)) != cudaSuccess) return e;
+  } else {
+    prof_mark(c, 0, s);
+    if ((e = launch_row_stats_merge_shards(c, a, a.shard_stats_all, a.n_shards, s, launches)) != cudaSuccess) return e;
+  }
   prof_mark(c, 1, s);
 
   // a4: operands of the gradient contractions

@@ -19,6 +19,7 @@ TTS_SGD, TTS_ADAMW = 0, 1
 TTS_ROWS_ALL, TTS_ROWS_ACCEPTED, TTS_ROWS_ACCEPTED_PLUS_ONE = 0, 1, 2
 TTS_PATH_AUTO, TTS_PATH_SIMT = 0, 1
 TTS_NUM_PHASES = 5
+TTS_SHARD_STAT_FIELDS = 8
 PHASE_NAMES = ("a2_logits", "a3_row_stats", "a4_dlogits", "a5_gh", "a6a7_gW_update")
 
 
@@ -58,6 +59,11 @@ EXPORTS = {
     "tts_wait_step": (C.c_int32, [C.c_void_p, C.c_void_p]),
     "tts_sync_step": (C.c_int32, [C.c_void_p]),
     "tts_round_host": (C.c_int32, [C.c_void_p] * 5 + [C.c_int32, C.c_float] + [C.c_void_p] * 10),
+    "tts_shard_begin_step": (C.c_int32, [C.c_void_p] * 4 + [C.c_int32] + [C.c_void_p] * 3),
+    "tts_shard_finish_step": (C.c_int32, [C.c_void_p] * 2 + [C.c_int32] + [C.c_void_p] * 9 + [C.c_int32, C.c_float] +
+                              [C.c_void_p] * 6),
+    "tts_shard_argmax": (C.c_int32, [C.c_void_p] * 2 + [C.c_int32, C.c_int32] + [C.c_void_p] * 3),
+    "tts_shard_accept_mask": (C.c_int32, [C.c_void_p] * 3 + [C.c_int32, C.c_void_p, C.c_int32] + [C.c_void_p] * 4),
 }
 
 _lib = None
@@ -226,6 +232,44 @@ def tts_round_host(ctx, teacher_logits_host, h_host, draft_tokens_host, pos_weig
                               _ptr(adam_m), _ptr(adam_v), _ptr(gh_dev), _ptr(loss_host), _ptr(tau_host),
                               _ptr(mask_host), _stream(stream))
     _check(ctx, st, "tts_round_host")
+
+
+def _extras(draft_logits, draft_logits_out, ref_logits, lam):
+    return tts_step_extras(_ptr(draft_logits), _ptr(draft_logits_out), _ptr(ref_logits), lam)
+
+
+def tts_shard_begin_step(ctx, teacher_logits_local, h, W_in_local, T, stats_out, *, draft_logits=None,
+                         draft_logits_out=None, ref_logits=None, lam=0.0, side_stream=None):
+    ex = _extras(draft_logits, draft_logits_out, ref_logits, lam)
+    st = lib().tts_shard_begin_step(ctx, _ptr(teacher_logits_local), _ptr(h), _ptr(W_in_local), T, C.addressof(ex),
+                                    _ptr(stats_out), _stream(side_stream))
+    _check(ctx, st, "tts_shard_begin_step")
+
+
+def tts_shard_finish_step(ctx, stats_all, n_shards, teacher_logits_local, h, W_in_local, W_out_local, W_master_local,
+                          adam_m_local, adam_v_local, pos_weight, mask, T, loss_scale, loss_out, kl_rows_out=None,
+                          gh_partial_out=None, gW_debug_out=None, *, draft_logits=None, draft_logits_out=None,
+                          ref_logits=None, lam=0.0, side_stream=None):
+    ex = _extras(draft_logits, draft_logits_out, ref_logits, lam)
+    st = lib().tts_shard_finish_step(ctx, _ptr(stats_all), n_shards, _ptr(teacher_logits_local), _ptr(h),
+                                     _ptr(W_in_local), _ptr(W_out_local), _ptr(W_master_local), _ptr(adam_m_local),
+                                     _ptr(adam_v_local), _ptr(pos_weight), _ptr(mask), T, loss_scale, _ptr(loss_out),
+                                     _ptr(kl_rows_out), _ptr(gh_partial_out), _ptr(gW_debug_out), C.addressof(ex),
+                                     _stream(side_stream))
+    _check(ctx, st, "tts_shard_finish_step")
+
+
+def tts_shard_argmax(ctx, teacher_logits_local, T, v_offset, val_out, idx_out, stream=None):
+    st = lib().tts_shard_argmax(ctx, _ptr(teacher_logits_local), T, v_offset, _ptr(val_out), _ptr(idx_out),
+                                _stream(stream))
+    _check(ctx, st, "tts_shard_argmax")
+
+
+def tts_shard_accept_mask(ctx, val_all, idx_all, n_shards, draft_tokens, T, mask_out, tau_out, teacher_argmax_out=None,
+                          stream=None):
+    st = lib().tts_shard_accept_mask(ctx, _ptr(val_all), _ptr(idx_all), n_shards, _ptr(draft_tokens), T, _ptr(mask_out),
+                                     _ptr(tau_out), _ptr(teacher_argmax_out), _stream(stream))
+    _check(ctx, st, "tts_shard_accept_mask")
 
 
 def make_config(V, d, T_max, seg_len, param_dtype=TTS_BF16, logits_dtype=TTS_BF16, optimizer=TTS_ADAMW, lr=1e-5,

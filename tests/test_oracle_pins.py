@@ -523,3 +523,27 @@ def test_golden_config1_regression():
     assert int(vals["tau"]) == int(tau[0])
     assert float(np.abs(r["gW"]).max()) == pytest.approx(float(vals["gW_absmax"]), rel=1e-12)
     assert float(np.abs(r["gh"]).max()) == pytest.approx(float(vals["gh_absmax"]), rel=1e-12)
+
+
+def test_shard_tuples_merge_to_the_whole_row_normalisers():
+    """the per-slice tuples (m_t, s_t, a, m_z, s_z), merged, give the plain logsumexp of the whole teacher
+    and draft rows and the plain KL -- for uneven slices, -inf teacher entries and a slice that is all -inf."""
+    rng = np.random.Generator(np.random.PCG64(21))
+    T, V = 5, 97
+    t = 3.0 * rng.standard_normal((T, V))
+    z = 2.0 * rng.standard_normal((T, V))
+    t[:, 7::11] = -np.inf
+    t[2, 40:70] = -np.inf                          # row 2: the middle slice has no finite teacher entry
+    want_t, want_z, want_kl = O.logsumexp_rows(t), O.logsumexp_rows(z), O.kl_rows_from_logits(t, z)
+    for cuts in ([0, V], [0, 40, 70, V], [0, 1, 2, 50, V]):
+        st = np.stack([O.shard_row_stats(t[:, a:b], z[:, a:b]) for a, b in zip(cuts[:-1], cuts[1:])])
+        lse_t, lse_z, kl = O.merge_shard_stats(st)
+        np.testing.assert_allclose(lse_t, want_t, rtol=1e-13)
+        np.testing.assert_allclose(lse_z, want_z, rtol=1e-13)
+        np.testing.assert_allclose(kl, want_kl, rtol=1e-11, atol=1e-13)
+    # brute force on one row, literal definitions
+    r = 1
+    p = np.exp(t[r]) / np.exp(t[r]).sum()
+    q = np.exp(z[r]) / np.exp(z[r]).sum()
+    kl_lit = sum(p[v] * (np.log(p[v]) - np.log(q[v])) for v in range(V) if p[v] > 0)
+    assert abs(kl[r] - kl_lit) < 1e-12
