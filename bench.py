@@ -53,6 +53,10 @@ def parse_args():
     ap.add_argument("--draft-logits", default="computed", choices=["computed", "given"],
                     help="given: the drafter's own logits are passed in (tts_distill_step_ex, SURVEY 8(f) f1) and pass "
                          "a2 is skipped; the default computes them, as BASELINE.json's north_star describes")
+    ap.add_argument("--parallelism", default="replicas", choices=["replicas", "vocab"],
+                    help="N > 1: independent replicas of the step (weak scaling, no data-path collective), or ONE step "
+                         "sharded over the vocabulary (strong scaling; SURVEY 8(e): all-gather of [T,8] row tuples and "
+                         "all-reduce of gh [T,d] per step over NCCL)")
     ap.add_argument("--stream", action="store_true",
                     help="also run the long-generation stream protocol (BASELINE.json configs[4]; use --config 5)")
     ap.add_argument("--rounds", type=int, default=4000, help="--stream: speculation rounds per pass")
@@ -73,6 +77,26 @@ def measured_peaks():
         except Exception:
             pass
     return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def profiled_traffic(cfg_id):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed
+    `ncu --set full` capture of this workload (profiles/r1c_README.md has the command); None when there is none."""
+    import csv
+    p = os.path.join(ROOT, "profiles", "r1c_ncu_full_config%d.csv" % cfg_id)
+    if not os.path.exists(p):
+        return None
+    try:
+        rows = list(csv.reader(open(p)))
+        hdr, units = rows[0], rows[1]
+        ki, ri, wi = hdr.index("Kernel Name"), hdr.index("dram__bytes_read.sum"), hdr.index("dram__bytes_write.sum")
+        mult = {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0}
+        for r in rows[2:]:
+            if "tc_update" in r[ki]:
+                return int(float(r[ri]) * mult[units[ri]] + float(r[wi]) * mult[units[wi]])
+    except Exception:
+        return None
+    return None
 
 
 def algorithmic_bytes(V, d, T, adam=True):
@@ -206,14 +230,18 @@ def run_reference(args, rank, world):
     print(json.dumps(line), flush=True)
 
 
-def workload_config(cfg_id, world, path):
+def workload_config(cfg_id, world, path, parallelism="replicas"):
     from paper_2605_09329_b200 import synth
     c = synth.CONFIGS[cfg_id]
+    par = "single GPU"
+    if world > 1:
+        par = ("replicas x%d (no data-path collective)" % world if parallelism == "replicas" else
+               "vocabulary shards x%d (all-gather [T,8] row tuples + all-reduce gh [T,d] per step, NCCL)" % world)
     return {"workload": "BASELINE.json configs[%d] %s: V=%d d=%d T=%d (seg_len %d x %d seq), bf16 W + fp32 master, "
                         "AdamW lr=1e-5" % (cfg_id - 1, c["name"], c["V"], c["d"], c["seg_len"] * c["n_seq"],
                                            c["seg_len"], c["n_seq"]),
             "V": c["V"], "d": c["d"], "T": c["seg_len"] * c["n_seq"], "optimizer": "adamw",
-            "parallelism": "replicas x%d (no data-path collective)" % world if world > 1 else "single GPU",
+            "parallelism": par,
             "kernel_path": path,
             "l2": "working set per step (17 GB of weight state) exceeds the 126 MB L2: every step is L2-cold"}
 
@@ -233,13 +261,24 @@ def run_ours(args, rank, world, local_rank):
     def barrier():
         dist_util.barrier(tdev)
 
-    case = synth.make_case_device(args.config, dev, seed_offset=rank)
+    vocab = world > 1 and args.parallelism == "vocab"
+    V_full = synth.CONFIGS[args.config]["V"]
+    if vocab:
+        # one step, every rank owns a slice of the vocabulary (rows of W / master / m / v, columns of the teacher)
+        import torch.distributed as dist
+        from paper_2605_09329_b200 import sharded
+        v0, v1 = sharded.shard_range(V_full, rank, world)
+        case = synth.make_case_device(args.config, dev, seed_offset=rank, V=v1 - v0, shared_h=True)
+        dist.broadcast(case["draft_tokens"], 0)      # replicated inputs: canvas tokens (global ids), h, pos_weight
+    else:
+        case = synth.make_case_device(args.config, dev, seed_offset=rank)
     c = case["cfg"]
     V, d, T, C = case["V"], case["d"], case["T"], case["seg_len"]
     kpath = tts.TTS_PATH_AUTO if args.kernel_path == "auto" else tts.TTS_PATH_SIMT
     cfg = tts.make_config(V, d, T, C, tts.TTS_BF16, tts.TTS_BF16, tts.TTS_ADAMW, c["lr"], c["beta1"], c["beta2"],
                           c["eps"], c["weight_decay"], tts.TTS_ROWS_ALL, 0, kpath)
-    ctx = tts.tts_ctx_create(cfg, local_rank)
+    shard = sharded.VocabShardedStep(cfg, v0, local_rank) if vocab else None
+    ctx = shard.ctx if vocab else tts.tts_ctx_create(cfg, local_rank)
     W = [case["W"], torch.empty_like(case["W"])]        # W_in / W_out double buffer, swapped at the barrier (R18)
     master, m, v = case["master"], case["m"], case["v"]
     teacher, h, tok, pw = case["teacher"], case["h"], case["draft_tokens"], case["pos_weight"]
@@ -256,7 +295,18 @@ def run_ours(args, rank, world, local_rank):
     if args.draft_logits == "given":      # what the drafter already holds after generating the canvas
         z_given = torch.cat([h[i:i + 64].float() @ case["W"].float().T for i in range(0, T, 64)], 0).contiguous()
 
+    def step_vocab():
+        shard.accept_mask(teacher, tok, T, mask, tau, None, side)
+        launches[0] += 3
+        shard.distill_step(teacher, h, W[cur[0]], W[1 - cur[0]], master, m, v, pw, mask, T, case["loss_scale"], loss,
+                           None, gh, None, side)
+        launches[0] += 2 + tts.tts_last_launch_count(ctx)      # begin (logits + sweep) + finish
+        tts.tts_wait_step(ctx, main)
+        cur[0] ^= 1
+
     def step():
+        if vocab:
+            return step_vocab()
         tts.tts_accept_mask(ctx, teacher, tok, T, mask, tau, None, side)
         n = tts.tts_last_launch_count(ctx)
         if z_given is None:
@@ -274,7 +324,8 @@ def run_ours(args, rank, world, local_rank):
         step()
     barrier()
     used_tensor = tts.tts_last_step_used_tensor_path(ctx)
-    tts.tts_profile_enable(ctx, 1)
+    if not vocab:
+        tts.tts_profile_enable(ctx, 1)
     launches[0] = 0
     sampler = ClockSampler(local_rank)
     sampler.start()
@@ -287,14 +338,14 @@ def run_ours(args, rank, world, local_rank):
     barrier()
     clocks = sampler.stop()
     ms_total = e0.elapsed_time(e1)
-    phase_ms, n_prof = tts.tts_profile_read(ctx)
+    phase_ms, n_prof = tts.tts_profile_read(ctx) if not vocab else ([0.0] * tts.TTS_NUM_PHASES, 0)
     tts.tts_profile_enable(ctx, 0)
     loss_val = float(loss.item())
     ms_total = dist_util.max_over_ranks(ms_total, tdev)
 
     # ---- end to end through HOST buffers: tts_round_host (H2D of the round's inputs, D2H of loss/tau/mask) ----
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not vocab:
         ht = teacher.view(torch.int16).cpu().pin_memory()
         hh = h.view(torch.int16).cpu().pin_memory()
         htok, hpw = tok.cpu().pin_memory(), pw.cpu().pin_memory()
@@ -338,15 +389,20 @@ def run_ours(args, rank, world, local_rank):
     if rank != 0:
         return
     ms_step = ms_total / args.steps
-    sps = world * 1e3 / ms_step
+    sps = (1 if vocab else world) * 1e3 / ms_step          # shards: all ranks together take ONE step
+    if vocab:
+        V = V_full
     step_bytes, upd_bytes = algorithmic_bytes(V, d, T)
+    if vocab:
+        step_bytes //= world
     if z_given is not None:
         step_bytes += T * V * 4 - V * d * 2      # fp32 draft logits read instead of the bf16 W pass
     peak, peak_src = measured_peaks()
     upd_ms = phase_ms[4] if n_prof > 0 and phase_ms[4] > 0 else None
     roof = {"bound": "hbm", "kernel": "a6+a7 gW contraction fused with AdamW update (phase 4)",
             "achieved": (upd_bytes / (upd_ms * 1e-3) / 1e9) if upd_ms else None, "peak": peak, "unit": "GB/s",
-            "frac": (upd_bytes / (upd_ms * 1e-3) / 1e9 / peak) if upd_ms else None, "traffic": None,
+            "frac": (upd_bytes / (upd_ms * 1e-3) / 1e9 / peak) if upd_ms else None,
+            "traffic": profiled_traffic(args.config) if (z_given is None and not vocab) else None,
             "peak_source": peak_src, "algorithmic_bytes_per_launch": upd_bytes, "kernel_ms": upd_ms,
             "step_algorithmic_bytes": step_bytes, "step_achieved": step_bytes / (ms_step * 1e-3) / 1e9,
             "step_frac_of_measured_copy": step_bytes / (ms_step * 1e-3) / 1e9 / peak,
@@ -354,8 +410,9 @@ def run_ours(args, rank, world, local_rank):
             "phase_ms": dict(zip(tts.PHASE_NAMES, phase_ms)), "profiled_steps": n_prof}
     line = {"metric": "distill_steps_per_sec", "value": sps, "unit": "steps/s", "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-            "config": dict(workload_config(args.config, world, "tcgen05+tma" if used_tensor else "cuda-core"),
+            "scaling": "strong" if vocab else "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+            "config": dict(workload_config(args.config, world, "tcgen05+tma" if used_tensor else "cuda-core",
+                                           args.parallelism),
                            draft_logits=args.draft_logits),
             "rows_V_per_sec": sps * T * V, "loss": loss_val, "clocks": clocks, "e2e": e2e,
             "gpu_launches": launches[0], "roofline": roof, "cpu_baseline": cpu}

@@ -272,10 +272,11 @@ def planted_mask_cases(V: int, seg_len: int, seed: int = 11, dtype=BF16):
 # ----------------------------------------------------------------------------
 
 def make_case_device(cfg_id: int, device="cuda:0", *, seed_offset: int = 0, n_seq: int | None = None,
-                     V: int | None = None, d: int | None = None):
+                     V: int | None = None, d: int | None = None, shared_h: bool = False):
     """Returns a dict of torch tensors on ``device``: teacher [T,V], h [T,d], W [V,d] (bf16),
     master/m/v [V,d] fp32, draft_tokens [T] i32, pos_weight [T] f32, plus cfg, tau_star (host
-    numpy) and loss_scale.  ``seed_offset`` gives independent replicas (multi-GPU ranks)."""
+    numpy) and loss_scale.  ``seed_offset`` gives independent replicas (multi-GPU ranks); with ``shared_h`` the hidden
+    states do not depend on it (vocabulary shards: every rank holds the same h and its own rows of W)."""
     import torch
 
     c = dict(CONFIGS[cfg_id])
@@ -295,7 +296,11 @@ def make_case_device(cfg_id: int, device="cuda:0", *, seed_offset: int = 0, n_se
     master = torch.empty((V, d), dtype=torch.float32, device=dev)
     master.normal_(0.0, 0.02, generator=g)
     W = master.to(torch.bfloat16)
-    h = torch.empty((T, d), dtype=torch.float32, device=dev).normal_(0.0, 1.0, generator=g).to(torch.bfloat16)
+    gh_ = g
+    if shared_h:
+        gh_ = torch.Generator(device=dev)
+        gh_.manual_seed(1000003 * (c["seed"] + 1) + 999983)
+    h = torch.empty((T, d), dtype=torch.float32, device=dev).normal_(0.0, 1.0, generator=gh_).to(torch.bfloat16)
     z = (h.float() @ W.float().T) if T * V <= (1 << 24) else torch.cat(
         [h[i:i + 64].float() @ W.float().T for i in range(0, T, 64)], 0)
     kind = c["sigma"]
