@@ -167,16 +167,20 @@ __global__ void __launch_bounds__(1024) row_stats_merge_kernel(const float* __re
   __shared__ double red[32];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
   double local = 0.0;
-  for (int r = warp; r < T; r += n_warps) {
+  // many rows, few splits (several canvases; vocabulary shards): a THREAD per row, otherwise a warp per row
+  const bool thread_rows = splits <= 8 && T > n_warps;
+  const int r_first = thread_rows ? (int)threadIdx.x : warp, r_step = thread_rows ? (int)blockDim.x : n_warps;
+  const int l_first = thread_rows ? 0 : lane, l_step = thread_rows ? 1 : 32;
+  for (int r = r_first; r < T; r += r_step) {
     const float* pr = part + (size_t)r * row_stride;
     float mt = -CUDART_INF_F, mz = -CUDART_INF_F, mr = -CUDART_INF_F;
-    for (int s = lane; s < splits; s += 32) {
+    for (int s = l_first; s < splits; s += l_step) {
       const float* p = pr + s * split_stride;
       mt = fmaxf(mt, p[0]); mz = fmaxf(mz, p[3]); mr = fmaxf(mr, p[5]);
     }
-    mt = warp_max(mt); mz = warp_max(mz); mr = warp_max(mr);
+    if (!thread_rows) { mt = warp_max(mt); mz = warp_max(mz); mr = warp_max(mr); }
     double st = 0.0, a = 0.0, sz = 0.0, sr = 0.0, b = 0.0;
-    for (int s = lane; s < splits; s += 32) {
+    for (int s = l_first; s < splits; s += l_step) {
       const float* p = pr + s * split_stride;
       if (p[0] != -CUDART_INF_F) {
         const double e = exp((double)p[0] - (double)mt);
@@ -188,9 +192,11 @@ __global__ void __launch_bounds__(1024) row_stats_merge_kernel(const float* __re
         sr += (double)p[6] * e; b += (double)p[7] * e;
       }
     }
-    st = warp_sum(st); a = warp_sum(a); sz = warp_sum(sz);
-    if (has_ref) { sr = warp_sum(sr); b = warp_sum(b); }
-    if (lane == 0) {
+    if (!thread_rows) {
+      st = warp_sum(st); a = warp_sum(a); sz = warp_sum(sz);
+      if (has_ref) { sr = warp_sum(sr); b = warp_sum(b); }
+    }
+    if (thread_rows || lane == 0) {
       const double lse_t = (double)mt + log(st), lse_z = (double)mz + log(sz);
       const double kl = a / st - lse_t + lse_z;
       double lse_ref = 0.0, kl_ref = 0.0;
@@ -217,6 +223,7 @@ __global__ void __launch_bounds__(1024) row_stats_merge_kernel(const float* __re
       local += omega * (kl + (double)lambda * kl_ref);
     }
   }
+  if (thread_rows) local = warp_sum(local);   // fixed shuffle tree: deterministic
   if (lane == 0) red[warp] = local;
   __syncthreads();
   if (threadIdx.x == 0) {

@@ -39,6 +39,7 @@ cudaError_t tc_init(tts_ctx* c) {
   if ((e = cudaMemset(st->hTT, 0, d * st->Kp * 2)) != cudaSuccess) return e;
   if ((e = tc_gemm_init(c)) != cudaSuccess) return e;
   if ((e = tc_wide_init(c)) != cudaSuccess) return e;
+  if ((e = tc_pair_init(c)) != cudaSuccess) return e;
   return tc_fused_init(c);
 }
 
@@ -63,7 +64,11 @@ cudaError_t tc_step(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches
   // a2: draft logits on tcgen05 (skipped when the caller supplies them), a3: row statistics + loss
   const float* z = z_src(a, c->z);
   if (a.phase != kPhaseFinish) {
-    if (!a.z_given && (e = tc_launch_logits(c, a, z_dst(a, c->z), s, launches)) != cudaSuccess) return e;
+    if (!a.z_given) {
+      e = tc_pair_eligible(c, T16) ? tc_launch_logits_pair(c, a, z_dst(a, c->z), s, launches)
+                                   : tc_launch_logits(c, a, z_dst(a, c->z), s, launches);
+      if (e != cudaSuccess) return e;
+    }
     prof_mark(c, 0, s);
     if (a.phase == kPhaseBegin) return launch_row_stats_shard(c, a, z, V, a.shard_stats_out, s, launches);
     if ((e = launch_row_stats(c, a, z, V, s, launches)) != cudaSuccess) return e;

@@ -56,4 +56,9 @@ int tc_wide_planes(int T16);   // 2: dl S = hi + lo (T16 <= 32), 1: one fp16 pla
 cudaError_t tc_launch_prep_wide(tts_ctx* c, const StepArgs& a, const float* z, cudaStream_t s, int* launches);
 cudaError_t tc_launch_update_wide(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches);
 
+// tts_tc_pair.cu: CTA-pair (cta_group::2) a2 for 256 < T16 <= 512
+cudaError_t tc_pair_init(tts_ctx* c);
+int tc_pair_eligible(const tts_ctx* c, int T16);
+cudaError_t tc_launch_logits_pair(tts_ctx* c, const StepArgs& a, float* z_out, cudaStream_t s, int* launches);
+
 }  // namespace tts

@@ -343,7 +343,15 @@ __global__ void __launch_bounds__(256) tc_h_absmax_kernel(const __nv_bfloat16* _
                                                           unsigned int* __restrict__ out_bits) {
   __shared__ float red[32];
   float m = 0.f;
-  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+  const size_t nvec = n / 8;                     // rows of h start 16-byte aligned (d % 128 == 0 on this path)
+  const uint4* hv = reinterpret_cast<const uint4*>(h);
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x) {
+    float f[8];
+    unpack_bf16x8(__ldg(hv + i), f);
+#pragma unroll
+    for (int k = 0; k < 8; ++k) m = fmaxf(m, fabsf(f[k]));
+  }
+  for (size_t i = nvec * 8 + (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
     m = fmaxf(m, fabsf(__bfloat162float(h[i])));
   m = block_max(m, red);
   if (threadIdx.x == 0) atomicMax(out_bits, __float_as_uint(m));
@@ -374,7 +382,8 @@ __global__ void __launch_bounds__(256) tc_prep_hT_kernel(const __nv_bfloat16* __
 // one [64 v x 64 k] tile per block.  Up to 32 rows the 64-wide K chunk has room for a second plane, so dl S is
 // split hi + lo (two fp16, 2^-22) at no cost in operand bytes or MMAs and the h^T operand repeats its rows.  Written twice, both coalesced: dlT[v, r] (r contiguous: the K-major B operand
 // of gW; transposed through shared memory, 128-byte row segments) and dlR[r, v] (the K-major B operand of gh).
-template <bool BF16>
+// FAST (one fp16 plane, 2^-12): ex2.approx-based __expf, error ~|x| 1e-7, far inside the plane's rounding.
+template <bool BF16, bool FAST>
 __global__ void __launch_bounds__(256) tc_prep_dl_wide_kernel(const void* __restrict__ teacher, const float* __restrict__ z,
                                                               const float* __restrict__ z_ref, float lam, int V,
                                                               int z_ld, int T, int T16, int planes, int Kp, int T_max,
@@ -413,10 +422,14 @@ __global__ void __launch_bounds__(256) tc_prep_dl_wide_kernel(const void* __rest
     if (r < T && k < planes * T16) {
       const float t = BF16 ? __bfloat162float(static_cast<const __nv_bfloat16*>(teacher)[(size_t)r * V + v])
                            : static_cast<const float*>(teacher)[(size_t)r * V + v];
-      const float qv = expf(z[(size_t)r * z_ld + v] - sh[64 + rr]);
-      const float pv = expf(t - sh[rr]);   // t = -inf -> 0
+      const float az = z[(size_t)r * z_ld + v] - sh[64 + rr], at = t - sh[rr];
+      const float qv = FAST ? __expf(az) : expf(az);
+      const float pv = FAST ? __expf(at) : expf(at);   // t = -inf -> 0
       float g = qv - pv;
-      if (z_ref) g += lam * (qv - expf(z_ref[(size_t)r * z_ld + v] - sh[192 + rr]));
+      if (z_ref) {
+        const float ar = z_ref[(size_t)r * z_ld + v] - sh[192 + rr];
+        g += lam * (qv - (FAST ? __expf(ar) : expf(ar)));
+      }
       dl = sh[128 + rr] * g * S;
     }
     __half hq = __float2half_rn(dl);
@@ -482,19 +495,21 @@ cudaError_t tc_launch_prep_wide(tts_ctx* c, const StepArgs& a, const float* z, c
   cudaError_t e = cudaMemsetAsync(absmax, 0, sizeof(unsigned int), s);
   if (e != cudaSuccess) return e;
   const __nv_bfloat16* h = static_cast<const __nv_bfloat16*>(a.h);
-  tc_h_absmax_kernel<<<64, 256, 0, s>>>(h, (size_t)T * d, absmax);
+  const size_t n_h = (size_t)T * d;
+  int ab_grid = (int)((n_h / 8 + 255) / 256);
+  ab_grid = ab_grid < 1 ? 1 : (ab_grid > 4 * c->sm_count ? 4 * c->sm_count : ab_grid);
+  tc_h_absmax_kernel<<<ab_grid, 256, 0, s>>>(h, n_h, absmax);
   const int planes = tc_wide_planes(T16);
   tc_prep_hT_kernel<<<dim3((d + 31) / 32, Kp / 32), 256, 0, s>>>(h, d, T, T16, planes, Kp, absmax,
                                                                   static_cast<uint16_t*>(st->hTT), st->dl_scale);
   uint16_t* dlT = static_cast<uint16_t*>(st->dlT);
   uint16_t* dlR = a.gh_out ? static_cast<uint16_t*>(st->dlR) : nullptr;
   const dim3 grid(V / 64, Kp / 64);
-  if (c->cfg.logits_dtype == TTS_BF16)
-    tc_prep_dl_wide_kernel<true><<<grid, 256, 0, s>>>(a.teacher, z, a.z_ref, a.lambda, V, V, T, T16, planes, Kp, c->cfg.T_max,
-                                                       c->row_stats, dlT, dlR, st->dl_scale);
-  else
-    tc_prep_dl_wide_kernel<false><<<grid, 256, 0, s>>>(a.teacher, z, a.z_ref, a.lambda, V, V, T, T16, planes, Kp, c->cfg.T_max,
-                                                        c->row_stats, dlT, dlR, st->dl_scale);
+  const bool bf = c->cfg.logits_dtype == TTS_BF16, fast = planes == 1;
+  auto kern = bf ? (fast ? tc_prep_dl_wide_kernel<true, true> : tc_prep_dl_wide_kernel<true, false>)
+                 : (fast ? tc_prep_dl_wide_kernel<false, true> : tc_prep_dl_wide_kernel<false, false>);
+  kern<<<grid, 256, 0, s>>>(a.teacher, z, a.z_ref, a.lambda, V, V, T, T16, planes, Kp, c->cfg.T_max, c->row_stats, dlT,
+                            dlR, st->dl_scale);
   *launches += 3;
   return cudaGetLastError();
 }

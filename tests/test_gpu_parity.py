@@ -81,6 +81,8 @@ SMALL = [
     (3, 2048 + 16 * 5, 1024, 1, 16, {}),             # V % 128 != 0: CUDA-core kernels at d = 1024
     (3, 2048 + 128 * 3, 1024, 1, 16, {}),            # fused stripe kernel: one 1024-column stripe, 152 bands over 148 CTAs
     (3, 1024 + 128, 2048, 1, 8, {}),                 # fused stripe kernel: two stripes, T = 8 padded to 16 rows
+    (4, 2048 + 128, 256, 32, 16, {}),                # 512 rows: CTA-pair logits (17 tiles of 128: the last pair tile is half empty), full-TMEM gh
+    (4, 1024, 384, 20, 16, {}),                      # 320 rows: pair pieces of 256 + 64 rows
 ]
 
 
