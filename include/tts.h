@@ -91,11 +91,12 @@ int32_t tts_ctx_destroy(tts_ctx* ctx);
 
 /* Hyper-parameters may change between steps. */
 int32_t tts_set_lr(tts_ctx* ctx, float lr);
-/* Adam's bias-correction step count n lives in the ctx: 0 after create, incremented at the
- * start of every tts_distill_step (so the first step uses n = 1).  Set it to resume a stream
- * or after restoring a snapshot (the paper resets the speculator between requests). */
+/* Adam's bias-correction step count n lives in DEVICE memory of the ctx: 0 after create, incremented by the first
+ * kernel of every tts_distill_step on the step's stream (so the first step uses n = 1, and a replayed CUDA graph of
+ * the step keeps counting).  Set it to resume a stream or after restoring a snapshot (the paper resets the
+ * speculator between requests).  Both calls synchronise the device. */
 int32_t tts_set_step_count(tts_ctx* ctx, int64_t n);
-int64_t tts_get_step_count(const tts_ctx* ctx);   /* returns the count, not a status */
+int64_t tts_get_step_count(const tts_ctx* ctx);   /* returns the count (-1 on error), not a status */
 /* CUDA error code (cudaError_t as int) of the last failed CUDA call on this ctx, 0 if none. */
 int32_t tts_last_cuda_error(const tts_ctx* ctx);
 /* 1 if the last tts_distill_step on this ctx ran the tcgen05/TMA kernels, 0 if CUDA-core. */
@@ -243,6 +244,19 @@ int32_t tts_distill_inner_steps(tts_ctx* ctx, const void* teacher_logits, const 
 enum { TTS_NUM_PHASES = 5 };
 int32_t tts_profile_enable(tts_ctx* ctx, int32_t enable);
 int32_t tts_profile_read(tts_ctx* ctx, float* ms_out, int32_t* n_steps_out);
+
+/*
+ * f3: CUDA-graph capture.  tts_accept_mask and tts_distill_step[_ex] may be called while their stream
+ * is being captured (cudaStreamBeginCapture .. EndCapture): they allocate nothing, never synchronise, and every
+ * step-dependent scalar (Adam's count and bias corrections) is read from device memory.  What is baked into the
+ * captured graph: all pointer arguments (so a W_in / W_out double buffer needs one graph per parity, or W_out ==
+ * W_in), T, loss_scale and the ctx's hyper-parameters at capture time (re-capture after tts_set_lr).  Inside a
+ * capture no done-event is recorded and the phase profile is off; after cudaGraphLaunch on a stream call
+ * tts_record_done on that stream, then tts_wait_step / tts_sync_step as usual (graph replay ignores
+ * cross-stream events recorded elsewhere, hence the paper's CPU-side barrier = tts_sync_step).
+ * tts_distill_inner_steps with K > 1 allocates on its first call and must not be captured first.
+ */
+int32_t tts_record_done(tts_ctx* ctx, void* stream);
 
 /* The paper's barrier after S-1 rounds: main_stream waits (on the device) for the
  * last step's done-event. */

@@ -28,6 +28,7 @@ cudaError_t dmalloc(T** p, size_t n) {
 void free_all(tts_ctx* c) {
   if (!c) return;
   tts::tc_destroy(c);
+  cudaFree(c->step_count_dev); cudaFree(c->step_scalars);
   cudaFree(c->z); cudaFree(c->z_ref_buf); cudaFree(c->dl32); cudaFree(c->stat_part); cudaFree(c->row_stats);
   cudaFree(c->arg_val); cudaFree(c->arg_idx); cudaFree(c->argmax_tmp);
   cudaFree(c->acc_rows); cudaFree(c->acc_rej); cudaFree(c->acc_rpart);
@@ -93,6 +94,9 @@ int32_t tts_ctx_create(const tts_config* cfg, int32_t device, tts_ctx** out) {
   const size_t V = cfg->V, Tm = cfg->T_max, Tp = c->T_pad_max;
   bool ok = true;
   ok = ok && cudaEventCreateWithFlags(&c->done_event, cudaEventDisableTiming) == cudaSuccess;
+  ok = ok && dmalloc(&c->step_count_dev, 1) == cudaSuccess;
+  ok = ok && dmalloc(&c->step_scalars, 2) == cudaSuccess;
+  ok = ok && cudaMemset(c->step_count_dev, 0, sizeof(unsigned long long)) == cudaSuccess;
   ok = ok && dmalloc(&c->z, Tp * V) == cudaSuccess;
   ok = ok && dmalloc(&c->dl32, Tm * V) == cudaSuccess;
   ok = ok && dmalloc(&c->stat_part, Tm * tts::kStatSplitsMax * tts::kStatFields) == cudaSuccess;
@@ -139,11 +143,21 @@ int32_t tts_set_lr(tts_ctx* c, float lr) {
 
 int32_t tts_set_step_count(tts_ctx* c, int64_t n) {
   if (!c || n < 0) return TTS_ERR_INVALID_ARG;
-  c->step_count = n;
-  return TTS_OK;
+  const unsigned long long v = static_cast<unsigned long long>(n);
+  cudaError_t e = cudaSetDevice(c->device);
+  if (e == cudaSuccess) e = cudaDeviceSynchronize();
+  if (e == cudaSuccess) e = cudaMemcpy(c->step_count_dev, &v, sizeof(v), cudaMemcpyHostToDevice);
+  return e == cudaSuccess ? TTS_OK : cuda_fail(c, e);
 }
 
-int64_t tts_get_step_count(const tts_ctx* c) { return c ? c->step_count : -1; }
+int64_t tts_get_step_count(const tts_ctx* c) {
+  if (!c) return -1;
+  unsigned long long v = 0;
+  if (cudaSetDevice(c->device) != cudaSuccess || cudaDeviceSynchronize() != cudaSuccess ||
+      cudaMemcpy(&v, c->step_count_dev, sizeof(v), cudaMemcpyDeviceToHost) != cudaSuccess)
+    return -1;
+  return static_cast<int64_t>(v);
+}
 int32_t tts_last_cuda_error(const tts_ctx* c) { return c ? c->last_cuda_error : 0; }
 int32_t tts_last_step_used_tensor_path(const tts_ctx* c) { return c ? c->last_used_tensor : 0; }
 int32_t tts_last_launch_count(const tts_ctx* c) { return c ? c->last_launches : 0; }
@@ -216,9 +230,12 @@ static int32_t run_step(tts_ctx* c, const void* teacher, const void* h, const vo
     return TTS_ERR_INVALID_ARG;
 
   cudaStream_t s = static_cast<cudaStream_t>(side_stream);
-  if (phase != tts::kPhaseBegin) c->step_count += 1;     // Adam's count advances once per step: in the second half
-  const double n = static_cast<double>(c->step_count > 0 ? c->step_count : 1);
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  cudaError_t e = cudaStreamIsCapturing(s, &cap);
+  if (e != cudaSuccess) return cuda_fail(c, e);
+  const bool capturing = cap != cudaStreamCaptureStatusNone;
   tts::StepArgs a;
+  a.step_scalars = c->step_scalars;
   a.phase = phase; a.shard_stats_out = stats_out; a.shard_stats_all = stats_all; a.n_shards = n_shards;
   a.teacher = teacher; a.h = h; a.W_in = W_in; a.W_out = W_out;
   a.master = W_master; a.adam_m = adam_m; a.adam_v = adam_v;
@@ -229,13 +246,15 @@ static int32_t run_step(tts_ctx* c, const void* teacher, const void* h, const vo
   a.z_ref = (ex && ex->lambda > 0.f) ? ex->ref_logits : nullptr;   // lambda = 0: the term vanishes, skip its sweep
   a.lambda = a.z_ref ? ex->lambda : 0.f;
   a.lr = cfg.lr; a.beta1 = cfg.beta1; a.beta2 = cfg.beta2; a.eps = cfg.eps; a.wd = cfg.weight_decay;
-  a.inv_bc1 = static_cast<float>(1.0 / (1.0 - pow(static_cast<double>(cfg.beta1), n)));
-  a.inv_sqrt_bc2 = static_cast<float>(1.0 / sqrt(1.0 - pow(static_cast<double>(cfg.beta2), n)));
 
   int launches = 0;
-  cudaError_t e;
   const bool prof_saved = c->prof_on;
-  if (phase != tts::kPhaseAll) c->prof_on = false;       // the phase events describe whole steps only
+  if (phase != tts::kPhaseAll || capturing) c->prof_on = false;   // the phase events describe whole, eager steps only
+  // Adam's count advances once per step (in the second half of a sharded step), ON THE DEVICE
+  if (phase != tts::kPhaseBegin && (e = tts::launch_step_advance(c, s, &launches)) != cudaSuccess) {
+    c->prof_on = prof_saved;
+    return cuda_fail(c, e);
+  }
   tts::prof_mark(c, -1, s);
   if (c->tensor_ok) {
     c->last_used_tensor = 1;
@@ -248,7 +267,16 @@ static int32_t run_step(tts_ctx* c, const void* teacher, const void* h, const vo
   if (e != cudaSuccess) { c->prof_on = prof_saved; return cuda_fail(c, e); }
   if (c->prof_on) c->prof_count += 1;
   c->prof_on = prof_saved;
+  if (capturing) return TTS_OK;   // an event recorded inside a capture cannot be waited on outside: tts_record_done
   if ((e = cudaEventRecord(c->done_event, s)) != cudaSuccess) return cuda_fail(c, e);
+  c->done_recorded = true;
+  return TTS_OK;
+}
+
+int32_t tts_record_done(tts_ctx* c, void* stream) {
+  if (!c) return TTS_ERR_INVALID_ARG;
+  cudaError_t e = cudaEventRecord(c->done_event, static_cast<cudaStream_t>(stream));
+  if (e != cudaSuccess) return cuda_fail(c, e);
   c->done_recorded = true;
   return TTS_OK;
 }

@@ -46,8 +46,9 @@ struct StepArgs {
   int n_shards;
   // optimiser scalars for this step (bias corrections precomputed on the host in fp64)
   float lr, beta1, beta2, eps, wd;
-  float inv_bc1;       // 1 / (1 - beta1^n)
-  float inv_sqrt_bc2;  // 1 / sqrt(1 - beta2^n)
+  const float* step_scalars;   // device: {1 / (1 - beta1^n), 1 / sqrt(1 - beta2^n)} of THIS step, written by the
+                               // step-advance kernel on the same stream (so a captured CUDA graph of the step
+                               // advances Adam's count on every replay)
 };
 
 // where a2 writes the draft logits, and where a3 / a4 read them
@@ -60,7 +61,8 @@ struct tts_ctx {
   tts_config cfg;
   int device;
   int sm_count;
-  int64_t step_count;
+  unsigned long long* step_count_dev;   // Adam's step count n lives on the device (see step_scalars)
+  float* step_scalars;                  // [2]
   int last_cuda_error;
   int last_used_tensor;
   int last_launches;
@@ -105,6 +107,8 @@ inline void prof_mark(tts_ctx* c, int phase, cudaStream_t s) {
   cudaEventRecord(c->prof_events[slot * (TTS_NUM_PHASES + 1) + phase + 1], s);
 }
 
+// tts_stats.cu: n <- n + 1, bias corrections of step n (one thread)
+cudaError_t launch_step_advance(tts_ctx* c, cudaStream_t s, int* launches);
 // tts_mask.cu
 cudaError_t launch_accept_mask(tts_ctx* c, const void* teacher, const int32_t* tok, int T, uint8_t* mask,
                                int32_t* tau, int32_t* am_out, cudaStream_t s, int* launches);

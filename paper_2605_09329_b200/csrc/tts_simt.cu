@@ -118,7 +118,8 @@ __global__ void __launch_bounds__(128) simt_update_kernel(const float* __restric
                                                           PT* __restrict__ W_out, float* __restrict__ master,
                                                           float* __restrict__ am, float* __restrict__ av,
                                                           float* __restrict__ gW_debug, float lr, float b1, float b2,
-                                                          float eps, float wd, float inv_bc1, float inv_sqrt_bc2) {
+                                                          float eps, float wd, const float* __restrict__ step_scalars) {
+  const float inv_bc1 = ADAM ? step_scalars[0] : 1.f, inv_sqrt_bc2 = ADAM ? step_scalars[1] : 1.f;
   constexpr int VT = 8;
   __shared__ float dls[16][VT];
   const int j = blockIdx.x * 128 + threadIdx.x;
@@ -214,12 +215,12 @@ static cudaError_t simt_step_t(tts_ctx* c, const StepArgs& a, cudaStream_t s, in
   dim3 grid((d + 127) / 128, (V + 7) / 8);
   if (c->cfg.optimizer == TTS_ADAMW)
     simt_update_kernel<PT, true><<<grid, 128, 0, s>>>(c->dl32, h, T, V, d, W_in, W_out, a.master, a.adam_m, a.adam_v,
-                                                      a.gW_debug, a.lr, a.beta1, a.beta2, a.eps, a.wd, a.inv_bc1,
-                                                      a.inv_sqrt_bc2);
+                                                      a.gW_debug, a.lr, a.beta1, a.beta2, a.eps, a.wd,
+                                                      a.step_scalars);
   else
     simt_update_kernel<PT, false><<<grid, 128, 0, s>>>(c->dl32, h, T, V, d, W_in, W_out, a.master, nullptr, nullptr,
-                                                       a.gW_debug, a.lr, a.beta1, a.beta2, a.eps, a.wd, a.inv_bc1,
-                                                       a.inv_sqrt_bc2);
+                                                       a.gW_debug, a.lr, a.beta1, a.beta2, a.eps, a.wd,
+                                                       a.step_scalars);
   *launches += 1;
   prof_mark(c, 4, s);
   return cudaGetLastError();

@@ -317,4 +317,19 @@ cudaError_t launch_row_stats_merge_shards(tts_ctx* c, const StepArgs& a, const f
   return cudaGetLastError();
 }
 
+// Adam's count and bias corrections on the device: n <- n + 1; {1 / (1 - b1^n), 1 / sqrt(1 - b2^n)} in double.
+__global__ void step_advance_kernel(unsigned long long* __restrict__ count, float* __restrict__ scal, float b1,
+                                    float b2) {
+  const unsigned long long n = *count + 1ull;
+  *count = n;
+  scal[0] = (float)(1.0 / (1.0 - pow((double)b1, (double)n)));
+  scal[1] = (float)(1.0 / sqrt(1.0 - pow((double)b2, (double)n)));
+}
+
+cudaError_t launch_step_advance(tts_ctx* c, cudaStream_t s, int* launches) {
+  step_advance_kernel<<<1, 1, 0, s>>>(c->step_count_dev, c->step_scalars, c->cfg.beta1, c->cfg.beta2);
+  *launches += 1;
+  return cudaGetLastError();
+}
+
 }  // namespace tts

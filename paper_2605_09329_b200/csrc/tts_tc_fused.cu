@@ -66,7 +66,8 @@ struct FusedParams {
   int V, d, T;
   int n_stripes;              // d / 1024
   int stages;
-  float lr, b1, b2, eps, decay, c1, inv_sqrt_bc2;   // decay = 1 - lr wd, c1 = lr / (1 - b1^n)
+  const float* step_scalars;  // device {1 / (1 - b1^n), 1 / sqrt(1 - b2^n)} of this step
+  float lr, b1, b2, eps, decay;   // decay = 1 - lr wd
 };
 
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
@@ -235,6 +236,7 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
     const int q = warp & 3, g = (warp - 4) >> 2;
     const int jj = q * 32 + lane;
     const bool leader = jj == 0;               // issues the group's TMA stores and releases its state stages
+    const float c1 = ADAM ? p.lr * p.step_scalars[0] : 0.f, inv_sqrt_bc2 = ADAM ? p.step_scalars[1] : 0.f;
     // element (v, jb) of a stage tensor sits in box jb / 2, row v, column (jb % 2) * 128 + jj
     uint8_t* wt_thr = wt + (jj >> 3) * 128 + (jj & 7) * 16;   // + jb * 4096 + (v >> 3) * 2048 + (v & 7) * 2
     __nv_bfloat16* wo_g = reinterpret_cast<__nv_bfloat16*>(wo + g * kWoBytes);
@@ -287,8 +289,8 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
             if (ADAM) {
               const float m1 = p.b1 * mm[jb][v] + (1.f - p.b1) * gg;
               const float v1 = p.b2 * vv[jb][v] + (1.f - p.b2) * gg * gg;
-              const float den = __fsqrt_rn(v1) * p.inv_sqrt_bc2 + p.eps;
-              M[jb][v] = M[jb][v] * p.decay - __fdividef(p.c1 * m1, den);
+              const float den = __fsqrt_rn(v1) * inv_sqrt_bc2 + p.eps;
+              M[jb][v] = M[jb][v] * p.decay - __fdividef(c1 * m1, den);
               sM[kSV * kSW + e] = m1;
               sM[2 * kSV * kSW + e] = v1;
             } else {
@@ -492,8 +494,7 @@ cudaError_t tc_launch_update_fused(tts_ctx* c, const StepArgs& a, int grid, cuda
   p.stages = kMaxStages;
   p.lr = a.lr; p.b1 = a.beta1; p.b2 = a.beta2; p.eps = a.eps;
   p.decay = 1.f - a.lr * a.wd;
-  p.c1 = a.lr * a.inv_bc1;
-  p.inv_sqrt_bc2 = a.inv_sqrt_bc2;
+  p.step_scalars = a.step_scalars;
   const size_t smem = fused_smem();
   if (adam)
     tc_update_gh_kernel<true><<<grid, kThreads, smem, s>>>(tm_master, tm_m, tm_v, tm_wout, p);

@@ -50,7 +50,8 @@ struct WideParams {
   const float* dl_scale;      // {S, 1 / S, S_h, 1 / S_h}
   int V, d, Kp;
   int n_stripes, n_bands, n_win, stages;
-  float lr, b1, b2, eps, decay, c1, inv_sqrt_bc2;   // decay = 1 - lr wd, c1 = lr / (1 - b1^n)
+  const float* step_scalars;  // device {1 / (1 - b1^n), 1 / sqrt(1 - b2^n)} of this step
+  float lr, b1, b2, eps, decay;   // decay = 1 - lr wd
 };
 
 struct WideBars {
@@ -230,6 +231,7 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_hTT, const __grid_c
     const uint32_t lane_bits = static_cast<uint32_t>(q * 32) << 16;
     __nv_bfloat16* wo_g = reinterpret_cast<__nv_bfloat16*>(wo + g * kWWoBytes);
     const float inv_s = p.dl_scale[1] * p.dl_scale[3];
+    const float c1 = ADAM ? p.lr * p.step_scalars[0] : 0.f, inv_sqrt_bc2 = ADAM ? p.step_scalars[1] : 0.f;
     WideWalk w(p);
     uint32_t i = 0;
     int stripe, band, cur = -1, prev_s = -1;
@@ -275,8 +277,8 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_hTT, const __grid_c
           if (ADAM) {
             const float m1 = p.b1 * mm[r] + (1.f - p.b1) * gg;
             const float v1 = p.b2 * vv[r] + (1.f - p.b2) * gg * gg;
-            const float den = __fsqrt_rn(v1) * p.inv_sqrt_bc2 + p.eps;
-            M[r] = M[r] * p.decay - __fdividef(p.c1 * m1, den);
+            const float den = __fsqrt_rn(v1) * inv_sqrt_bc2 + p.eps;
+            M[r] = M[r] * p.decay - __fdividef(c1 * m1, den);
             sM[kWSV * kWJ + r * kWJ] = m1;
             sM[2 * kWSV * kWJ + r * kWJ] = v1;
           } else {
@@ -564,8 +566,7 @@ cudaError_t tc_launch_update_wide(tts_ctx* c, const StepArgs& a, cudaStream_t s,
   if (p.stages < 2) return cudaErrorInvalidConfiguration;
   p.lr = a.lr; p.b1 = a.beta1; p.b2 = a.beta2; p.eps = a.eps;
   p.decay = 1.f - a.lr * a.wd;
-  p.c1 = a.lr * a.inv_bc1;
-  p.inv_sqrt_bc2 = a.inv_sqrt_bc2;
+  p.step_scalars = a.step_scalars;
   const long units = (long)p.n_stripes * (p.n_bands / p.n_win);
   int grid = c->cfg.max_ctas > 0 ? c->cfg.max_ctas : c->sm_count;
   if (grid > units) grid = (int)units;

@@ -21,7 +21,8 @@ from . import tts
 class DraftHeadUpdater:
     def __init__(self, W, master, adam_m, adam_v, *, seg_len, T_max, stride=1, lr=1e-5, beta1=0.9, beta2=0.999,
                  eps=1e-8, weight_decay=0.0, optimizer=tts.TTS_ADAMW, logits_dtype=tts.TTS_BF16,
-                 mask_mode=tts.TTS_ROWS_ALL, max_ctas=0, host_barrier=False, want_gh=True, keep_snapshot=False):
+                 mask_mode=tts.TTS_ROWS_ALL, max_ctas=0, host_barrier=False, want_gh=True, keep_snapshot=False,
+                 use_graph=False):
         assert stride >= 1
         V, d = W.shape
         self.V, self.d, self.seg_len, self.T_max, self.stride = V, d, seg_len, T_max, int(stride)
@@ -39,6 +40,10 @@ class DraftHeadUpdater:
         self.loss = torch.zeros(1, dtype=torch.float32, device=self.device)
         self.kl_rows = torch.zeros(T_max, dtype=torch.float32, device=self.device)
         self.gh = torch.zeros(T_max, d, dtype=torch.float32, device=self.device) if want_gh else None
+        # CUDA-graph replay of the whole step (include/tts.h "CUDA-graph capture"): one captured graph
+        # per parity of the W double buffer, fed from static input buffers; captured lazily for (T, loss_scale)
+        self.use_graph = bool(use_graph)
+        self._graphs, self._graph_key, self._static = None, None, None
         self.round = 0                 # rounds seen since the last reset
         self.pending_since = None      # round index at which the in-flight update was dispatched
         self.updates = 0
@@ -64,19 +69,50 @@ class DraftHeadUpdater:
         dispatched = False
         if r % self.stride == 0:
             assert self.pending_since is None
-            self.side.wait_stream(main)            # the round's signal exists once main reaches this point
-            tts.tts_accept_mask(self.ctx, teacher_logits, draft_tokens, T, self.mask, self.tau, None, self.side)
-            n = tts.tts_last_launch_count(self.ctx)
-            tts.tts_distill_step(self.ctx, teacher_logits, h, self.W[self.cur], self.W[1 - self.cur], self.master,
-                                 self.m, self.v, pos_weight, self.mask, T, loss_scale, self.loss, self.kl_rows,
-                                 self.gh, None, self.side)
-            self.launches += n + tts.tts_last_launch_count(self.ctx)
+            if self.use_graph:
+                self._dispatch_graph(teacher_logits, h, draft_tokens, pos_weight, T, loss_scale, main)
+            else:
+                self.side.wait_stream(main)        # the round's signal exists once main reaches this point
+                self._enqueue(teacher_logits, h, draft_tokens, pos_weight, T, loss_scale, self.cur)
             self.pending_since = r
             self.updates += 1
             dispatched = True
         if self.pending_since is not None and r - self.pending_since == self.stride - 1:
             self.barrier(main)
         return dispatched
+
+    def _enqueue(self, teacher_logits, h, draft_tokens, pos_weight, T, loss_scale, parity):
+        tts.tts_accept_mask(self.ctx, teacher_logits, draft_tokens, T, self.mask, self.tau, None, self.side)
+        n = tts.tts_last_launch_count(self.ctx)
+        tts.tts_distill_step(self.ctx, teacher_logits, h, self.W[parity], self.W[1 - parity], self.master, self.m,
+                             self.v, pos_weight, self.mask, T, loss_scale, self.loss, self.kl_rows, self.gh, None,
+                             self.side)
+        self._launches_per_step = n + tts.tts_last_launch_count(self.ctx)
+        self.launches += self._launches_per_step
+
+    def _dispatch_graph(self, teacher_logits, h, draft_tokens, pos_weight, T, loss_scale, main):
+        key = (T, float(loss_scale), teacher_logits.dtype)
+        if self._graph_key != key:
+            st = dict(teacher=torch.empty_like(teacher_logits[:T]), h=torch.empty_like(h[:T]),
+                      tok=torch.empty_like(draft_tokens[:T]), pw=torch.empty_like(pos_weight[:T]))
+            graphs = []
+            for parity in (0, 1):
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g, stream=self.side):
+                    self._enqueue(st["teacher"], st["h"], st["tok"], st["pw"], T, loss_scale, parity)
+                self.launches -= self._launches_per_step      # captured, not launched
+                graphs.append(g)
+            self._graphs, self._graph_key, self._static = graphs, key, st
+        self.side.wait_stream(main)
+        st = self._static
+        with torch.cuda.stream(self.side):                    # the round's signal -> the graph's static inputs
+            st["teacher"].copy_(teacher_logits[:T], non_blocking=True)
+            st["h"].copy_(h[:T], non_blocking=True)
+            st["tok"].copy_(draft_tokens[:T], non_blocking=True)
+            st["pw"].copy_(pos_weight[:T], non_blocking=True)
+            self._graphs[self.cur].replay()
+        tts.tts_record_done(self.ctx, self.side)
+        self.launches += self._launches_per_step
 
     def barrier(self, main_stream=None):
         """The paper's barrier: the main stream (or, with host_barrier, the CPU) waits for the in-flight update;

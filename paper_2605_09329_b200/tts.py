@@ -58,6 +58,7 @@ EXPORTS = {
     "tts_profile_read": (C.c_int32, [C.c_void_p, C.POINTER(C.c_float), C.POINTER(C.c_int32)]),
     "tts_wait_step": (C.c_int32, [C.c_void_p, C.c_void_p]),
     "tts_sync_step": (C.c_int32, [C.c_void_p]),
+    "tts_record_done": (C.c_int32, [C.c_void_p, C.c_void_p]),
     "tts_round_host": (C.c_int32, [C.c_void_p] * 5 + [C.c_int32, C.c_float] + [C.c_void_p] * 10),
     "tts_shard_begin_step": (C.c_int32, [C.c_void_p] * 4 + [C.c_int32] + [C.c_void_p] * 3),
     "tts_shard_finish_step": (C.c_int32, [C.c_void_p] * 2 + [C.c_int32] + [C.c_void_p] * 9 + [C.c_int32, C.c_float] +
@@ -219,6 +220,10 @@ def tts_profile_read(ctx):
 
 def tts_wait_step(ctx, main_stream=None):
     _check(ctx, lib().tts_wait_step(ctx, _stream(main_stream)), "tts_wait_step")
+
+
+def tts_record_done(ctx, stream=None):
+    _check(ctx, lib().tts_record_done(ctx, _stream(stream)), "tts_record_done")
 
 
 def tts_sync_step(ctx):

@@ -35,8 +35,11 @@ def _oracle_stream(case0, rounds, stride):
     return dict(W=W, master=M, m=m, v=v, losses=np.array(losses), taus=taus, updates=n)
 
 
-@pytest.mark.parametrize("stride,host_barrier", [(1, False), (3, False), (4, True)])
-def test_stream_matches_oracle_round_by_round(stride, host_barrier):
+@pytest.mark.parametrize("stride,host_barrier,use_graph", [(1, False, False), (3, False, False), (4, True, False),
+                                                           (1, False, True), (3, True, True)])
+def test_stream_matches_oracle_round_by_round(stride, host_barrier, use_graph):
+    """use_graph: the whole step replayed from a captured CUDA graph (one per parity of the W double buffer); Adam's
+    count advances on the device with every replay (include/tts.h "CUDA-graph capture")."""
     V, d = 2048 + 16 * 3, 1024
     case0, rounds = synth.make_stream(V=V, d=d, rounds=ROUNDS)
     o = _oracle_stream(case0, rounds, stride)
@@ -45,7 +48,7 @@ def test_stream_matches_oracle_round_by_round(stride, host_barrier):
     pw = _dev(case0["pos_weight"])
     up = DraftHeadUpdater(W0, master, m, v, seg_len=16, T_max=16, stride=stride, lr=c["lr"], beta1=c["beta1"],
                           beta2=c["beta2"], eps=c["eps"], weight_decay=c["weight_decay"], host_barrier=host_barrier,
-                          keep_snapshot=True)
+                          keep_snapshot=True, use_graph=use_graph)
     try:
         dev_rounds = [dict(teacher=_dev(r["teacher"]), h=_dev(r["h"]), tok=_dev(r["draft_tokens"])) for r in rounds]
         losses, taus = [], []
