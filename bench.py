@@ -57,6 +57,9 @@ def parse_args():
                     help="N > 1: independent replicas of the step (weak scaling, no data-path collective), or ONE step "
                          "sharded over the vocabulary (strong scaling; SURVEY 8(e): all-gather of [T,8] row tuples and "
                          "all-reduce of gh [T,d] per step over NCCL)")
+    ap.add_argument("--max-ctas", type=int, default=0,
+                    help="SM budget of the step's persistent kernels (tts_config.max_ctas; 0 = all SMs): what the main "
+                         "stream keeps while the update overlaps it (PAPER.md:426)")
     ap.add_argument("--stream", action="store_true",
                     help="also run the long-generation stream protocol (BASELINE.json configs[4]; use --config 5)")
     ap.add_argument("--rounds", type=int, default=4000, help="--stream: speculation rounds per pass")
@@ -276,7 +279,7 @@ def run_ours(args, rank, world, local_rank):
     V, d, T, C = case["V"], case["d"], case["T"], case["seg_len"]
     kpath = tts.TTS_PATH_AUTO if args.kernel_path == "auto" else tts.TTS_PATH_SIMT
     cfg = tts.make_config(V, d, T, C, tts.TTS_BF16, tts.TTS_BF16, tts.TTS_ADAMW, c["lr"], c["beta1"], c["beta2"],
-                          c["eps"], c["weight_decay"], tts.TTS_ROWS_ALL, 0, kpath)
+                          c["eps"], c["weight_decay"], tts.TTS_ROWS_ALL, args.max_ctas, kpath)
     shard = sharded.VocabShardedStep(cfg, v0, local_rank) if vocab else None
     ctx = shard.ctx if vocab else tts.tts_ctx_create(cfg, local_rank)
     W = [case["W"], torch.empty_like(case["W"])]        # W_in / W_out double buffer, swapped at the barrier (R18)
@@ -491,7 +494,8 @@ def run_stream(args, case, dev):
         m, v = torch.zeros_like(master0), torch.zeros_like(master0)
         master, W = master0.clone(), W0.clone()
         up = DraftHeadUpdater(W, master, m, v, seg_len=C, T_max=T, stride=stride, lr=c["lr"], beta1=c["beta1"],
-                              beta2=c["beta2"], eps=c["eps"], weight_decay=c["weight_decay"], want_gh=True)
+                              beta2=c["beta2"], eps=c["eps"], weight_decay=c["weight_decay"], want_gh=True,
+                              max_ctas=args.max_ctas)
         g = torch.Generator(device=tdev)
         g.manual_seed(1000003 * (c["seed"] + 1))
         fn = standins[kind][0]

@@ -6,8 +6,9 @@
 // the optimiser state itself costs HBM traffic (the first version of this kernel re-read 512 KB of operands per
 // 426 KB of state and ran at 4.1 TB/s).  So here
 //   * a CTA owns one 128-column stripe of the parameter matrix at a time and keeps the stripe's h^T operand
-//     [128 j x Kp] RESIDENT: in tensor memory (256 of the 512 columns at T = 512; A_TMEM), which leaves all of
-//     shared memory to the state ring, or in shared memory (the variant kept for comparison);
+//     [128 j x Kp] RESIDENT in tensor memory (tcgen05.mma with A from TMEM; 256 of the 512 columns at T = 512), which
+//     leaves all of shared memory to the state ring (resident in shared memory instead, the ring shrinks to two
+//     stages: measured 4.35 ms against 3.07);
 //   * dl is ONE 16-bit plane: fp16 with a power-of-two scale chosen from the row coefficients (|dl S| <= 2^14), i.e.
 //     11 significant bits against bf16's 8 (one bf16 plane misses the 2e-3 max|gW| bar on rows with a dominant
 //     entry; the hi/lo bf16 split of the one-canvas kernel would double K).  kind::f16 wants A and B in the same
@@ -39,7 +40,7 @@ constexpr int kWStageBytes = 3 * kWTensorBytes; // 12 KB
 constexpr int kWWoBytes = kWSV * kWJ * 2;       // 2 KB: bf16 staging of one sub-tile (one per epilogue group)
 constexpr int kWThreads = 384;           // warp 0 state TMA, 1 MMA, 2 TMEM alloc, 3 operand TMA, 4-11 epilogue
 constexpr int kWMaxStages = 16;
-constexpr int kWOpStages = 2;            // dl band ring
+constexpr int kWOpStagesMax = 4;         // dl band ring (depth chosen per launch)
 constexpr int kWSmemBudget = 225 * 1024;
 constexpr int kWAccCols = 64;            // TMEM columns reserved for the two gW accumulators (NV <= 32)
 constexpr long kWWindowBytes = 12l << 20;
@@ -49,7 +50,7 @@ struct WideParams {
   const uint16_t* hTT;        // [d, Kp] fp16 bits
   const float* dl_scale;      // {S, 1 / S, S_h, 1 / S_h}
   int V, d, Kp;
-  int n_stripes, n_bands, n_win, stages;
+  int n_stripes, n_bands, n_win, stages, op_stages;
   const float* step_scalars;  // device {1 / (1 - b1^n), 1 / sqrt(1 - b2^n)} of this step
   float lr, b1, b2, eps, decay;   // decay = 1 - lr wd
 };
@@ -57,34 +58,37 @@ struct WideParams {
 struct WideBars {
   uint64_t st_full[kWMaxStages];
   uint64_t st_empty[kWMaxStages];
-  uint64_t op_full[kWOpStages];
-  uint64_t op_empty[kWOpStages];
+  uint64_t op_full[kWOpStagesMax];
+  uint64_t op_empty[kWOpStagesMax];
   uint64_t acc_full[2];
   uint64_t acc_empty[2];
   uint64_t a_full;
-  uint64_t a_empty;
   uint32_t tmem_slot;
 };
 
-// The sequence of (stripe, band) units of this CTA: window by window, a contiguous range of each window's units.
+// The sequence of (stripe, band) units of this CTA: window by window, a contiguous range of each window's units --
+// the SAME relative range in every window, walked forwards in even windows and backwards in odd ones, so that a
+// window ends in the stripe the next one starts in and h^T is reloaded only where a range crosses a stripe boundary.
 struct WideWalk {
   int n_stripes, n_bands, n_win;
   int win, wb0, wbn;
-  long u, u_end;
+  long u_lo, u_hi, k;      // range [u_lo, u_hi) of the current window, k units of it already handed out
   __device__ WideWalk(const WideParams& p) : n_stripes(p.n_stripes), n_bands(p.n_bands), n_win(p.n_win), win(-1),
-                                             wb0(0), wbn(1), u(0), u_end(0) {}
+                                             wb0(0), wbn(1), u_lo(0), u_hi(0), k(0) {}
   __device__ bool get(int& stripe, int& band) {
-    while (u >= u_end) {
+    while (u_lo + k >= u_hi) {
       if (++win >= n_win) return false;
       wb0 = (int)((long)n_bands * win / n_win);
       wbn = (int)((long)n_bands * (win + 1) / n_win) - wb0;
       const long units = (long)n_stripes * wbn;
-      u = units * blockIdx.x / gridDim.x;
-      u_end = units * (blockIdx.x + 1) / gridDim.x;
+      u_lo = units * blockIdx.x / gridDim.x;
+      u_hi = units * (blockIdx.x + 1) / gridDim.x;
+      k = 0;
     }
+    const long u = (win & 1) ? u_hi - 1 - k : u_lo + k;
     stripe = (int)(u / wbn);
     band = wb0 + (int)(u - (long)stripe * wbn);
-    ++u;
+    ++k;
     return true;
   }
 };
@@ -93,19 +97,18 @@ constexpr uint32_t kDescHiSw128 = (1024u >> 4) | (1u << 14) | (ptx::kSwizzle128B
 __device__ __forceinline__ uint32_t desc_lo_sw128(uint32_t smem_addr) { return ((smem_addr >> 4) & 0x3FFFu) | (1u << 16); }
 __device__ __forceinline__ uint64_t desc64(uint32_t hi, uint32_t lo) { return (static_cast<uint64_t>(hi) << 32) | lo; }
 
-template <bool ADAM, bool A_TMEM, int NV>
+template <bool ADAM, int NV>
 __global__ void __launch_bounds__(kWThreads, 1)
-tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_hTT, const __grid_constant__ CUtensorMap tm_dlT,
+tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
                       const __grid_constant__ CUtensorMap tm_master, const __grid_constant__ CUtensorMap tm_m,
                       const __grid_constant__ CUtensorMap tm_v, const __grid_constant__ CUtensorMap tm_wout,
                       const WideParams p) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   constexpr int kSubs = NV / kWSV;
-  const int a_bytes = A_TMEM ? 0 : p.Kp * kWJ * 2;     // [Kp / 64][128 j][64 k] bf16, 128-byte swizzle
   const int b_bytes = NV * p.Kp * 2;                   // [Kp / 64][NV v][64 k] fp16, 128-byte swizzle
-  uint8_t* sA = smem;
-  uint8_t* sB = sA + a_bytes;
+  uint8_t* sB = smem;
+  const int kWOpStages = p.op_stages;
   uint8_t* st = sB + kWOpStages * b_bytes;             // [stages][3][8 v][128 j] fp32
   uint8_t* wo = st + p.stages * kWStageBytes;          // [2 groups][8 v][128 j] bf16
   WideBars* bars = reinterpret_cast<WideBars*>(wo + 2 * kWWoBytes);
@@ -120,14 +123,12 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_hTT, const __grid_c
   }
   if (warp == 3 && lane == 0) {
     ptx::prefetch_tensormap(&tm_dlT);
-    if (!A_TMEM) ptx::prefetch_tensormap(&tm_hTT);
   }
   if (warp == 1 && lane == 0) {
     for (int i = 0; i < p.stages; ++i) { ptx::mbar_init(&bars->st_full[i], 1); ptx::mbar_init(&bars->st_empty[i], 1); }
     for (int i = 0; i < kWOpStages; ++i) { ptx::mbar_init(&bars->op_full[i], 1); ptx::mbar_init(&bars->op_empty[i], 1); }
     for (int i = 0; i < 2; ++i) { ptx::mbar_init(&bars->acc_full[i], 1); ptx::mbar_init(&bars->acc_empty[i], 8); }
-    ptx::mbar_init(&bars->a_full, A_TMEM ? 8 : 1);
-    ptx::mbar_init(&bars->a_empty, 1);
+    ptx::mbar_init(&bars->a_full, 8);
     ptx::fence_barrier_init();
   }
   if (warp == 2) {
@@ -164,21 +165,13 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_hTT, const __grid_c
       }
     }
   } else if (warp == 3) {
-    // ===== operand producer: the band's dl rows [NV v x Kp] (and, A in shared memory, the stripe's h^T) =====
+    // ===== operand producer: the band's dl rows [NV v x Kp] =====
     if (lane == 0) {
       const uint64_t pol = ptx::policy_evict_last();
       WideWalk w(p);
-      uint32_t i = 0, a_loads = 0;
-      int stripe, band, cur = -1;
+      uint32_t i = 0;
+      int stripe, band;
       while (w.get(stripe, band)) {
-        if (!A_TMEM && stripe != cur) {
-          ptx::mbar_wait(&bars->a_empty, (a_loads & 1) ^ 1);     // the MMAs that read the old stripe are complete
-          ptx::mbar_expect_tx(&bars->a_full, a_bytes);
-          for (int c = 0; c < p.Kp / kKC; ++c)
-            ptx::tma_load_2d_hint(sA + c * (kWJ * 128), &tm_hTT, &bars->a_full, c * kKC, stripe * kWJ, pol);
-          ++a_loads;
-          cur = stripe;
-        }
         const int s = i % kWOpStages;
         ptx::mbar_wait(&bars->op_empty[s], ((i / kWOpStages) & 1) ^ 1);
         ptx::mbar_expect_tx(&bars->op_full[s], b_bytes);
@@ -191,13 +184,12 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_hTT, const __grid_c
     // ===== MMA issuer: acc[j, v] = sum_r h^T[j, r] (S dl)[r, v]   (M = 128, N = NV, K = 16 per instruction) =====
     if (lane == 0) {
       constexpr uint32_t idesc = ptx::make_idesc_f16(kWJ, NV, ptx::kFmtF16, ptx::kFmtF16, 0, 0);
-      const uint32_t sA0 = ptx::smem_u32(sA), sB0 = ptx::smem_u32(sB);
+      const uint32_t sB0 = ptx::smem_u32(sB);
       WideWalk w(p);
       uint32_t i = 0, a_n = 0;
       int stripe, band, cur = -1;
       while (w.get(stripe, band)) {
         if (stripe != cur) {
-          if (!A_TMEM && cur >= 0) ptx::mma_commit(&bars->a_empty);
           ptx::mbar_wait(&bars->a_full, a_n & 1);
           ptx::tc_fence_after();
           ++a_n;
@@ -211,12 +203,7 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_hTT, const __grid_c
         const uint32_t b_base = sB0 + s * b_bytes;
         for (int ks = 0; ks < nks; ++ks) {
           const uint32_t b_lo = desc_lo_sw128(b_base + (ks >> 2) * (NV * 128)) + 2 * (ks & 3);
-          if (A_TMEM) {
-            ptx::mma_f16_ts(d_tmem, tmem_A + ks * 8, desc64(kDescHiSw128, b_lo), idesc, ks);
-          } else {
-            const uint32_t a_lo = desc_lo_sw128(sA0 + (ks >> 2) * (kWJ * 128)) + 2 * (ks & 3);
-            ptx::mma_f16_ss(d_tmem, desc64(kDescHiSw128, a_lo), desc64(kDescHiSw128, b_lo), idesc, ks);
-          }
+          ptx::mma_f16_ts(d_tmem, tmem_A + ks * 8, desc64(kDescHiSw128, b_lo), idesc, ks);
         }
         ptx::mma_commit(&bars->op_empty[s]);
         ptx::mma_commit(&bars->acc_full[ab]);
@@ -237,14 +224,26 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_hTT, const __grid_c
     int stripe, band, cur = -1, prev_s = -1;
     while (w.get(stripe, band)) {
       const int j0 = stripe * kWJ, v0 = band * NV;
-      if (A_TMEM && stripe != cur) {
+      if (stripe != cur) {
         // every MMA that read the old stripe is complete: this warp has waited on the previous band's acc_full.
-        // Row jj of hTT is K-contiguous; this group writes half of the K steps.
-        const uint4* row = reinterpret_cast<const uint4*>(p.hTT + (size_t)(j0 + jj) * p.Kp);
-        for (int ks = g * (nks / 2); ks < (g + 1) * (nks / 2); ++ks) {
-          const uint4 lo = row[2 * ks], hi = row[2 * ks + 1];
-          const uint32_t r[8] = {lo.x, lo.y, lo.z, lo.w, hi.x, hi.y, hi.z, hi.w};
-          ptx::tmem_st_32x32b_x8(tmem_A + ks * 8 + lane_bits, r);
+        // hTT is tiled [stripe][K step][128 j][16 k]: a warp reads 1 KB contiguous per K step; this group writes
+        // half of the K steps.
+        const uint4* tile = reinterpret_cast<const uint4*>(p.hTT + ((size_t)stripe * nks * kWJ + jj) * 16);
+        const int ks_end = (g + 1) * (nks / 2);
+        for (int ks0 = g * (nks / 2); ks0 < ks_end; ks0 += 4) {     // four K steps of loads in flight per thread
+          uint4 lo[4], hi[4];
+#pragma unroll
+          for (int u = 0; u < 4; ++u)
+            if (ks0 + u < ks_end) {
+              lo[u] = __ldg(tile + (size_t)(ks0 + u) * kWJ * 2);
+              hi[u] = __ldg(tile + (size_t)(ks0 + u) * kWJ * 2 + 1);
+            }
+#pragma unroll
+          for (int u = 0; u < 4; ++u)
+            if (ks0 + u < ks_end) {
+              const uint32_t r[8] = {lo[u].x, lo[u].y, lo[u].z, lo[u].w, hi[u].x, hi[u].y, hi[u].z, hi[u].w};
+              ptx::tmem_st_32x32b_x8(tmem_A + (ks0 + u) * 8 + lane_bits, r);
+            }
         }
         ptx::tmem_st_wait();
         ptx::tc_fence_before();
@@ -359,7 +358,8 @@ __global__ void __launch_bounds__(256) tc_h_absmax_kernel(const __nv_bfloat16* _
   if (threadIdx.x == 0) atomicMax(out_bits, __float_as_uint(m));
 }
 
-// hTT[j, k] = fp16(S_h h[k, j]) for k < T (and again at k + T16 with two dl planes), 0 elsewhere up to Kp.  32 x 32 transpose tiles through shared memory.
+// hTT = fp16(S_h h[k, j]) for k < T (and again at k + T16 with two dl planes), 0 elsewhere up to Kp, tiled
+// [j / 128][k / 16][j % 128][k % 16]: the order in which a stripe's rows go to tensor memory.  32 x 32 transpose tiles through shared memory.
 __global__ void __launch_bounds__(256) tc_prep_hT_kernel(const __nv_bfloat16* __restrict__ h, int d, int T, int T16,
                                                          int planes, int Kp,
                                                          const unsigned int* __restrict__ absmax_bits,
@@ -377,7 +377,10 @@ __global__ void __launch_bounds__(256) tc_prep_hT_kernel(const __nv_bfloat16* __
   }
   __syncthreads();
   for (int j = ty; j < 32; j += 8)
-    if (j0 + j < d && k0 + tx < Kp) hTT[(size_t)(j0 + j) * Kp + k0 + tx] = tile[tx][j];
+    if (j0 + j < d && k0 + tx < Kp) {
+      const int jg = j0 + j, kg = k0 + tx;
+      hTT[(((size_t)(jg / 128) * (Kp / 16) + kg / 16) * 128 + jg % 128) * 16 + kg % 16] = tile[tx][j];
+    }
 }
 
 // dl = coef_r ((q - p) + lambda (q - q_ref)) from z, teacher and the row normalisers, scaled by S and rounded to fp16;
@@ -450,18 +453,18 @@ __global__ void __launch_bounds__(256) tc_prep_dl_wide_kernel(const void* __rest
   }
 }
 
-template <bool ADAM, bool A_TMEM, int NV>
-cudaError_t launch_wide(int grid, size_t smem, cudaStream_t s, const CUtensorMap& tm_hTT, const CUtensorMap& tm_dlT,
+template <bool ADAM, int NV>
+cudaError_t launch_wide(int grid, size_t smem, cudaStream_t s, const CUtensorMap& tm_dlT,
                         const CUtensorMap& tm_master, const CUtensorMap& tm_m, const CUtensorMap& tm_v,
                         const CUtensorMap& tm_wout, const WideParams& p) {
-  tc_update_wide_kernel<ADAM, A_TMEM, NV><<<grid, kWThreads, smem, s>>>(tm_hTT, tm_dlT, tm_master, tm_m, tm_v, tm_wout, p);
+  tc_update_wide_kernel<ADAM, NV><<<grid, kWThreads, smem, s>>>(tm_dlT, tm_master, tm_m, tm_v, tm_wout, p);
   return cudaGetLastError();
 }
 
 
-template <bool ADAM, bool A_TMEM, int NV>
+template <bool ADAM, int NV>
 cudaError_t wide_attr() {
-  return cudaFuncSetAttribute(tc_update_wide_kernel<ADAM, A_TMEM, NV>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  return cudaFuncSetAttribute(tc_update_wide_kernel<ADAM, NV>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                               kWSmemBudget + 2048);
 }
 
@@ -469,23 +472,12 @@ cudaError_t wide_attr() {
 
 cudaError_t tc_wide_init(tts_ctx*) {
   cudaError_t e;
-  if ((e = wide_attr<true, true, 32>()) != cudaSuccess) return e;
-  if ((e = wide_attr<false, true, 32>()) != cudaSuccess) return e;
-  if ((e = wide_attr<true, false, 16>()) != cudaSuccess) return e;
-  return wide_attr<false, false, 16>();
+  if ((e = wide_attr<true, 32>()) != cudaSuccess) return e;
+  return wide_attr<false, 32>();
 }
 
 // dl planes of the wide path: hi + lo while both fit the 64-wide K chunk (T16 <= 32), one plane beyond
 int tc_wide_planes(int T16) { return 2 * T16 <= kKC ? 2 : 1; }
-
-int tc_wide_a_in_tmem() {
-  static int v = -1;
-  if (v < 0) {
-    const char* e = getenv("TTS_WIDE_A_SMEM");   // measurement switch: keep the stripe's h^T in shared memory
-    v = (e && e[0] == '1') ? 0 : 1;
-  }
-  return v;
-}
 
 // a4 of the wide path: h^T rows and the fp16 dl planes
 cudaError_t tc_launch_prep_wide(tts_ctx* c, const StepArgs& a, const float* z, cudaStream_t s, int* launches) {
@@ -523,13 +515,9 @@ cudaError_t tc_launch_update_wide(tts_ctx* c, const StepArgs& a, cudaStream_t s,
   const int T16 = (T + 15) / 16 * 16;
   const int Kp = (T16 + kKC - 1) / kKC * kKC;
   const bool adam = c->cfg.optimizer == TTS_ADAMW;
-  const bool a_tmem = tc_wide_a_in_tmem() != 0;
-  const int NV = a_tmem ? 32 : 16;
-  CUtensorMap tm_hTT, tm_dlT, tm_master, tm_m, tm_v, tm_wout;
-  // the operand maps depend on this step's Kp (row pitch of the scratch)
-  if (make_map_2d(st, &tm_hTT, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, st->hTT, Kp, d, kKC, kWJ,
-                  CU_TENSOR_MAP_SWIZZLE_128B) != CUDA_SUCCESS)
-    return cudaErrorInvalidValue;
+  constexpr int NV = 32;
+  CUtensorMap tm_dlT, tm_master, tm_m, tm_v, tm_wout;
+  // the operand map depends on this step's Kp (row pitch of the scratch)
   if (make_map_2d(st, &tm_dlT, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, st->dlT, Kp, V, kKC, NV,
                   CU_TENSOR_MAP_SWIZZLE_128B) != CUDA_SUCCESS)
     return cudaErrorInvalidValue;
@@ -560,7 +548,8 @@ cudaError_t tc_launch_update_wide(tts_ctx* c, const StepArgs& a, cudaStream_t s,
   p.n_win = (int)((dl_bytes + kWWindowBytes - 1) / kWWindowBytes);
   if (p.n_win < 1) p.n_win = 1;
   if (p.n_win > p.n_bands) p.n_win = p.n_bands;
-  const int fixed = 1024 + (a_tmem ? 0 : Kp * kWJ * 2) + kWOpStages * NV * Kp * 2 + 2 * kWWoBytes + (int)sizeof(WideBars);
+  p.op_stages = 2;
+  const int fixed = 1024 + p.op_stages * NV * Kp * 2 + 2 * kWWoBytes + (int)sizeof(WideBars);
   p.stages = (kWSmemBudget - fixed) / kWStageBytes;
   if (p.stages > kWMaxStages) p.stages = kWMaxStages;
   if (p.stages < 2) return cudaErrorInvalidConfiguration;
@@ -572,12 +561,8 @@ cudaError_t tc_launch_update_wide(tts_ctx* c, const StepArgs& a, cudaStream_t s,
   if (grid > units) grid = (int)units;
   const size_t smem = (size_t)fixed + (size_t)p.stages * kWStageBytes;
   cudaError_t e;
-  if (a_tmem)
-    e = adam ? launch_wide<true, true, 32>(grid, smem, s, tm_hTT, tm_dlT, tm_master, tm_m, tm_v, tm_wout, p)
-             : launch_wide<false, true, 32>(grid, smem, s, tm_hTT, tm_dlT, tm_master, tm_m, tm_v, tm_wout, p);
-  else
-    e = adam ? launch_wide<true, false, 16>(grid, smem, s, tm_hTT, tm_dlT, tm_master, tm_m, tm_v, tm_wout, p)
-             : launch_wide<false, false, 16>(grid, smem, s, tm_hTT, tm_dlT, tm_master, tm_m, tm_v, tm_wout, p);
+  e = adam ? launch_wide<true, NV>(grid, smem, s, tm_dlT, tm_master, tm_m, tm_v, tm_wout, p)
+           : launch_wide<false, NV>(grid, smem, s, tm_dlT, tm_master, tm_m, tm_v, tm_wout, p);
   *launches += 1;
   return e;
 }
