@@ -21,7 +21,9 @@
 //
 // Operands, both pre-tiled by the a4 kernels in the canonical no-swizzle core-matrix order ([8 rows][16 bytes]
 // contiguous), so a tile is one contiguous bulk copy:
-//   hTc [d / 128][T16 / 8][16][8 j][8 k]                 A of gW, K-major (K = canvas row)
+//   hTc [d][16 k]                                        A of gW: copied once per CTA into TENSOR MEMORY (lane = hidden
+//       column, 8 columns = 16 canvas rows packed in pairs); tcgen05.mma reads A from there, shared memory keeps a
+//       seventh state stage instead (ring depth is what the pass's bandwidth scales with)
 //   dlC [V / 16][2 planes][T16 / 8][2][8 r][8 v]          dl = hi + lo (bf16 split).  One shared-memory copy serves
 //       both contractions: core matrices [8 r][8 v] are the MN-major B of gW (N = v, K = r) and the K-major B
 //       of gh (N = r, K = v); only the roles of the two descriptor strides swap.
@@ -43,16 +45,16 @@ constexpr int kSubs = kTV / kSV; // 8 stages per tile
 constexpr int kBoxW = 256;       // TMA box width (elements): 4 boxes per tensor per stage
 constexpr int kBoxes = kSW / kBoxW;
 constexpr int kT16 = 16;         // canvas rows (padded)
-constexpr int kMaxStages = 6;    // state ring depth
+constexpr int kMaxStages = 7;    // state ring depth (168 KB; h^T lives in tensor memory, not shared memory)
 constexpr int kOpStages = 2;     // dl tile ring depth
 constexpr int kTensorBytes = kSV * kSW * 4;          // 8 KB per tensor per stage
 constexpr int kStageBytes = 3 * kTensorBytes;        // 24 KB
 constexpr int kWoBytes = kSV * kSW * 2;              // 4 KB: bf16 W_out staging of one sub-tile (one per group)
-constexpr int kHBytes = kSW * kT16 * 2;              // 32 KB: the stripe's h^T operand
 constexpr int kWtBytes = kSW * kTV * 2;              // 32 KB: re-derived bf16 W^T tile (A operand of gh)
 constexpr int kDlBytes = 2 * kT16 * kTV * 2;         // 1 KB: dl tile, both planes
 constexpr int kThreads = 384;    // warp 0 state TMA, 1 MMA, 2 TMEM alloc, 3 operand loads, 4-11 epilogue
 constexpr int kGhCol0 = 2 * kJB * kTV;               // 256: first TMEM column of the gh accumulators
+constexpr int kHtCol0 = kGhCol0 + kJB * kT16;        // 384: h^T of the stripe, 8 blocks x 8 columns (16 k packed in pairs)
 constexpr int kTmemCols = 512;
 
 struct FusedParams {
@@ -95,8 +97,7 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const int kStages = p.stages;
   uint8_t* st = smem;                                   // [kStages][3][4 boxes][2 v][256] fp32
-  uint8_t* hT = st + kStages * kStageBytes;             // [8 jb][2 k-groups][16 j-groups][8 j][8 k] bf16
-  uint8_t* wt = hT + kHBytes;                           // [8 jb][2 v-groups][16 j-groups][8 j][8 v] bf16
+  uint8_t* wt = st + kStages * kStageBytes;                         // [8 jb][2 v-groups][16 j-groups][8 j][8 v] bf16
   uint8_t* wo = wt + kWtBytes;                          // [2 groups][4 boxes][2 v][256] bf16
   uint8_t* dl = wo + 2 * kWoBytes;                      // [kOpStages][2 planes][2 r-groups][2 v-groups][8 r][8 v] bf16
   uint64_t* bars = reinterpret_cast<uint64_t*>(dl + kOpStages * kDlBytes);
@@ -126,7 +127,7 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
     for (int i = 0; i < kStages; ++i) { ptx::mbar_init(&st_full[i], 1); ptx::mbar_init(&st_empty[i], 1); }
     for (int i = 0; i < kOpStages; ++i) { ptx::mbar_init(&op_full[i], 1); ptx::mbar_init(&op_empty[i], 1); }
     for (int i = 0; i < 2; ++i) { ptx::mbar_init(&acc_full[i], 1); ptx::mbar_init(&acc_empty[i], 8); }
-    ptx::mbar_init(h_full, 1);
+    ptx::mbar_init(h_full, 8);
     ptx::mbar_init(wt_full, 8);
     ptx::mbar_init(wt_empty, 1);
     ptx::mbar_init(gh_full, 1);
@@ -168,8 +169,6 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
   } else if (warp == 3) {
     // ===== operand loads: the stripe's h^T tiles once, then one 1 KB dl tile per band =====
     if (lane == 0 && w.n_my > 0) {
-      ptx::mbar_expect_tx(h_full, kHBytes);
-      ptx::bulk_load_1d(hT, p.hTc + (size_t)j_stripe * kT16, kHBytes, h_full);
       for (int i = 0; i < w.n_my; ++i) {
         const int band = w.first_band + i * w.peers;
         const int s = i % kOpStages;
@@ -192,12 +191,11 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
         ptx::tc_fence_after();
         const uint32_t b0 = ptx::smem_u32(dl + s * kDlBytes);
         for (int jb = 0; jb < kJB; ++jb) {
-          // A: K-major, no swizzle: core matrices [8 j x 8 k]; j-groups 128 B apart (SBO), k-groups 2 KB (LBO)
-          const uint64_t ad = ptx::make_smem_desc(ptx::smem_u32(hT + jb * 4096), 2048, 128, 0);
           for (int pl = 0; pl < 2; ++pl) {
             // B: MN-major, no swizzle: core matrices [8 r x 8 v]; v-groups 128 B apart (SBO), r-groups 256 B (LBO)
             const uint64_t bd = ptx::make_smem_desc(b0 + pl * 512, 256, 128, 0);
-            ptx::mma_f16_ss(tmem_base + ab * (kJB * kTV) + jb * kTV, ad, bd, idesc_gw, pl);
+            // A = the block's h^T rows from tensor memory (lane = hidden column, 8 columns = 16 canvas rows)
+            ptx::mma_f16_ts(tmem_base + ab * (kJB * kTV) + jb * kTV, tmem_base + kHtCol0 + jb * 8, bd, idesc_gw, pl);
           }
         }
         ptx::mma_commit(&acc_full[ab]);
@@ -241,6 +239,20 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
     uint8_t* wt_thr = wt + (jj >> 3) * 128 + (jj & 7) * 16;   // + jb * 4096 + (v >> 3) * 2048 + (v & 7) * 2
     __nv_bfloat16* wo_g = reinterpret_cast<__nv_bfloat16*>(wo + g * kWoBytes);
     int prev_s = -1;                           // stage whose stores this group issued last
+    if (w.n_my > 0) {
+      // the stripe's h^T operand -> tensor memory, once per kernel: hTc row j holds h[0..16, j] (32 bytes); this
+      // group writes four of the eight 128-column blocks
+      for (int jb = 4 * g; jb < 4 * g + 4; ++jb) {
+        const uint4* row = reinterpret_cast<const uint4*>(p.hTc + (size_t)(j_stripe + jb * kMJ + jj) * kT16);
+        const uint4 lo = __ldg(row), hi = __ldg(row + 1);
+        const uint32_t r[8] = {lo.x, lo.y, lo.z, lo.w, hi.x, hi.y, hi.z, hi.w};
+        ptx::tmem_st_32x32b_x8(tmem_base + kHtCol0 + jb * 8 + (static_cast<uint32_t>(q * 32) << 16), r);
+      }
+      ptx::tmem_st_wait();
+      ptx::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(h_full);
+    }
     for (int i = 0; i < w.n_my; ++i) {
       const int v0 = (w.first_band + i * w.peers) * kTV;
       const int ab = i & 1;
@@ -364,20 +376,18 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
 }
 
 size_t fused_smem() {
-  return 1024 + (size_t)kMaxStages * kStageBytes + kHBytes + kWtBytes + 2 * (size_t)kWoBytes +
+  return 1024 + (size_t)kMaxStages * kStageBytes + kWtBytes + 2 * (size_t)kWoBytes +
          (size_t)kOpStages * kDlBytes + 512;
 }
 
-// hTc[jt][k / 8][jj / 8][jj % 8][k % 8] = h[k, jt * 128 + jj] (rows k >= T are zero): the [128 j x 16 k] A tiles of
-// the gW contraction in the canonical no-swizzle K-major order.  One thread per hidden column j.
+// hTc[j][k] = h[k, j] for k < 16 (rows k >= T are zero): 32 bytes per hidden column, the order in which the epilogue
+// warps of the fused pass copy a stripe's h^T into tensor memory.  One thread per hidden column j.
 __global__ void __launch_bounds__(256) tc_prep_hc_kernel(const __nv_bfloat16* __restrict__ h, int d, int T,
                                                          __nv_bfloat16* __restrict__ hTc) {
   const int j = blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= d) return;
-  const int jt = j / kMJ, jj = j % kMJ;
-  __nv_bfloat16* tile = hTc + (size_t)jt * kMJ * kT16 + (jj >> 3) * 64 + (jj & 7) * 8;
-  for (int k = 0; k < kT16; ++k)
-    tile[(k >> 3) * 1024 + (k & 7)] = k < T ? h[(size_t)k * d + j] : __float2bfloat16_rn(0.f);
+  __nv_bfloat16* row = hTc + (size_t)j * kT16;
+  for (int k = 0; k < kT16; ++k) row[k] = k < T ? h[(size_t)k * d + j] : __float2bfloat16_rn(0.f);
 }
 
 // a4 for this pass: dl = coef_r (q - p) from z, teacher and the row normalisers, split into two bf16 (dl = hi + lo

@@ -16,7 +16,7 @@ constexpr int kTileMN = 128;     // MMA M of every tensor-path kernel (vocabular
 struct TcState {
   void* dlT;            // [V, Kp] fp16   B operand of gW (wide path): row v = S dl[0..Kp, v], this step's Kp as row pitch
   void* hTT;            // [d, Kp] fp16   A operand of gW (wide path): row j = S_h h[0..Kp, j]
-  __nv_bfloat16* hTc;   // [d / 128][2][16][8][8]        A tiles of gW in core-matrix order (tts_tc_fused.cu, T <= 16)
+  __nv_bfloat16* hTc;   // [d][16]        h^T rows, the A operand of gW (tts_tc_fused.cu, T <= 16; copied into tensor memory)
   __nv_bfloat16* dlC;   // [V / 16][2][2][2][8][8]        dl hi / lo planes, pre-tiled in core-matrix order (tts_tc_fused.cu)
   void* dlR;            // [P, V] fp16    B operand of gh: S dl[r, v] (rows T16 .. 2 T16: the lo plane when there are two)
   float* dl_scale;      // {S, 1 / S, S_h, 1 / S_h, bits of max|h|}: power-of-two scales of the fp16 dl and h^T planes (a4 kernels)
