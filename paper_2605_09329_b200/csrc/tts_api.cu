@@ -250,11 +250,7 @@ static int32_t run_step(tts_ctx* c, const void* teacher, const void* h, const vo
   int launches = 0;
   const bool prof_saved = c->prof_on;
   if (phase != tts::kPhaseAll || capturing) c->prof_on = false;   // the phase events describe whole, eager steps only
-  // Adam's count advances once per step (in the second half of a sharded step), ON THE DEVICE
-  if (phase != tts::kPhaseBegin && (e = tts::launch_step_advance(c, s, &launches)) != cudaSuccess) {
-    c->prof_on = prof_saved;
-    return cuda_fail(c, e);
-  }
+  // Adam's count advances once per step, ON THE DEVICE: in the merge kernel of a3 (second half of a sharded step)
   tts::prof_mark(c, -1, s);
   if (c->tensor_ok) {
     c->last_used_tensor = 1;

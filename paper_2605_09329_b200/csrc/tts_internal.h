@@ -47,7 +47,7 @@ struct StepArgs {
   // optimiser scalars for this step (bias corrections precomputed on the host in fp64)
   float lr, beta1, beta2, eps, wd;
   const float* step_scalars;   // device: {1 / (1 - beta1^n), 1 / sqrt(1 - beta2^n)} of THIS step, written by the
-                               // step-advance kernel on the same stream (so a captured CUDA graph of the step
+                               // row-statistics merge kernel earlier in the same stream (so a captured CUDA graph of the step
                                // advances Adam's count on every replay)
 };
 
@@ -107,8 +107,6 @@ inline void prof_mark(tts_ctx* c, int phase, cudaStream_t s) {
   cudaEventRecord(c->prof_events[slot * (TTS_NUM_PHASES + 1) + phase + 1], s);
 }
 
-// tts_stats.cu: n <- n + 1, bias corrections of step n (one thread)
-cudaError_t launch_step_advance(tts_ctx* c, cudaStream_t s, int* launches);
 // tts_mask.cu
 cudaError_t launch_accept_mask(tts_ctx* c, const void* teacher, const int32_t* tok, int T, uint8_t* mask,
                                int32_t* tau, int32_t* am_out, cudaStream_t s, int* launches);

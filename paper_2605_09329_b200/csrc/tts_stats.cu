@@ -6,7 +6,7 @@
 // without ever storing a [T,V] probability tensor.  Partial tuples from different CTAs merge
 // associatively (rescale to the larger maximum).  The merge kernel also forms the row weights
 // omega_r (mask_mode per DESIGN.md R2), coef_r = loss_scale * omega_r and
-// loss = loss_scale * sum_r omega_r KL_r  (a sum).
+// loss = loss_scale * sum_r omega_r KL_r  (a sum), and advances Adam's step count.
 #include "tts_common.cuh"
 #include "tts_internal.h"
 
@@ -163,8 +163,18 @@ __global__ void __launch_bounds__(1024) row_stats_merge_kernel(const float* __re
                                                                int has_ref, float lambda,
                                                                float* __restrict__ row_stats,
                                                                float* __restrict__ kl_rows_out,
-                                                               float* __restrict__ loss_out) {
+                                                               float* __restrict__ loss_out,
+                                                               unsigned long long* __restrict__ step_count,
+                                                               float* __restrict__ step_scalars, float b1, float b2) {
   __shared__ double red[32];
+  if (threadIdx.x == 0) {
+    // Adam's count and bias corrections live on the device (a replayed CUDA graph of the step keeps counting):
+    // n <- n + 1, {1 / (1 - b1^n), 1 / sqrt(1 - b2^n)} in double, read by the update kernel later in the stream
+    const unsigned long long n = *step_count + 1ull;
+    *step_count = n;
+    step_scalars[0] = (float)(1.0 / (1.0 - pow((double)b1, (double)n)));
+    step_scalars[1] = (float)(1.0 / sqrt(1.0 - pow((double)b2, (double)n)));
+  }
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
   double local = 0.0;
   // many rows, few splits (several canvases; vocabulary shards): a THREAD per row, otherwise a warp per row
@@ -290,7 +300,8 @@ static void launch_merge(tts_ctx* c, const StepArgs& a, const float* part, int s
   row_stats_merge_kernel<<<1, T >= 32 ? 1024 : 32 * T, 0, s>>>(part, splits, row_stride, split_stride, T, c->cfg.T_max,
                                                               c->cfg.seg_len, c->cfg.mask_mode, a.pos_weight, a.mask,
                                                               a.loss_scale, a.z_ref != nullptr, a.lambda, c->row_stats,
-                                                              a.kl_rows_out, a.loss_out);
+                                                              a.kl_rows_out, a.loss_out, c->step_count_dev,
+                                                              c->step_scalars, c->cfg.beta1, c->cfg.beta2);
 }
 
 cudaError_t launch_row_stats(tts_ctx* c, const StepArgs& a, const float* z, int z_ld, cudaStream_t s, int* launches) {
@@ -313,21 +324,6 @@ cudaError_t launch_row_stats_shard(tts_ctx* c, const StepArgs& a, const float* z
 cudaError_t launch_row_stats_merge_shards(tts_ctx* c, const StepArgs& a, const float* stats_all, int n_shards,
                                           cudaStream_t s, int* launches) {
   launch_merge(c, a, stats_all, n_shards, kStatFields, (long)a.T * kStatFields, s);
-  *launches += 1;
-  return cudaGetLastError();
-}
-
-// Adam's count and bias corrections on the device: n <- n + 1; {1 / (1 - b1^n), 1 / sqrt(1 - b2^n)} in double.
-__global__ void step_advance_kernel(unsigned long long* __restrict__ count, float* __restrict__ scal, float b1,
-                                    float b2) {
-  const unsigned long long n = *count + 1ull;
-  *count = n;
-  scal[0] = (float)(1.0 / (1.0 - pow((double)b1, (double)n)));
-  scal[1] = (float)(1.0 / sqrt(1.0 - pow((double)b2, (double)n)));
-}
-
-cudaError_t launch_step_advance(tts_ctx* c, cudaStream_t s, int* launches) {
-  step_advance_kernel<<<1, 1, 0, s>>>(c->step_count_dev, c->step_scalars, c->cfg.beta1, c->cfg.beta2);
   *launches += 1;
   return cudaGetLastError();
 }
