@@ -57,7 +57,7 @@ enum { TTS_SGD = 0, TTS_ADAMW = 1 };
 /* which canvas rows enter the loss (R2).  The paper sums over all k = 1..C. */
 enum { TTS_ROWS_ALL = 0, TTS_ROWS_ACCEPTED = 1, TTS_ROWS_ACCEPTED_PLUS_ONE = 2 };
 /* kernel family.  AUTO: tcgen05/TMA kernels when param_dtype is bf16 and the shape
- * qualifies (V % 128 == 0, d % 128 == 0, T <= 16 per step), CUDA-core kernels otherwise
+ * qualifies (V % 128 == 0, d % 128 == 0, T_max <= 512), CUDA-core kernels otherwise
  * (fp32 parameters, e.g. BASELINE config 1; other shapes).  SIMT forces the CUDA-core kernels. */
 enum { TTS_PATH_AUTO = 0, TTS_PATH_SIMT = 1 };
 

@@ -159,6 +159,17 @@ def test_fused_kernel_with_capped_grid(max_ctas):
     assert g["used_tensor"] == 1
 
 
+@pytest.mark.parametrize("max_ctas", [1, 3, 8])
+def test_several_canvases_with_capped_grid(max_ctas):
+    """512 rows under an SM budget: 1 CTA takes the one-CTA-per-tile logits kernel, 3 CTAs one CTA pair (+ an idle
+    SM), 8 CTAs four pairs; the wide update's stream-K ranges then span many stripes per CTA."""
+    case = synth.make_case(4, V=1024 + 128, d=256, n_seq=32, seg_len=16)
+    g = run_gpu(case, max_ctas=max_ctas)
+    o = run_oracle(case)
+    check_step(g, o, case)
+    assert g["used_tensor"] == 1
+
+
 def test_fused_kernel_sgd_alias_d1024():
     case = synth.make_case(2, V=1024, d=1024)
     case["cfg"]["optimizer"] = synth.SGD

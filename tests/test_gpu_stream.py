@@ -87,3 +87,56 @@ def test_stream_matches_oracle_round_by_round(stride, host_barrier, use_graph):
         assert tts.tts_get_step_count(up.ctx) == 0 and up.round == 0
     finally:
         up.close()
+
+
+@pytest.mark.parametrize("n_seq,d", [(32, 256), (4, 256), (1, 1024)])
+def test_captured_step_replays_like_eager_steps(n_seq, d):
+    """f3: tts_accept_mask + tts_distill_step captured into a CUDA graph on their stream (512-row case: cluster launch
+    of the CTA-pair logits kernel, memsets and the wide kernels inside the capture) and replayed twice must leave the
+    state two EAGER steps leave, bit for bit -- Adam's count advances on the device with every replay."""
+    from gpu_util import config_for
+    case = synth.make_case(4 if n_seq > 1 else 3, V=1024, d=d, n_seq=n_seq, seg_len=16)
+    T = case["T"]
+    outs = []
+    for graph in (False, True):
+        ctx = tts.tts_ctx_create(config_for(case), 0)
+        try:
+            t = dict(teacher=_dev(case["teacher"]), h=_dev(case["h"]), tok=_dev(case["draft_tokens"]),
+                     W=_dev(case["W"]), master=_dev(case["master"]), m=_dev(case["m"]), v=_dev(case["v"]),
+                     pw=_dev(case["pos_weight"]))
+            mask = torch.zeros(T, dtype=torch.uint8, device="cuda")
+            tau = torch.zeros(T // 16, dtype=torch.int32, device="cuda")
+            loss = torch.zeros(1, device="cuda")
+            gh = torch.zeros(T, d, device="cuda")
+            s = torch.cuda.Stream()
+
+            def enqueue():
+                tts.tts_accept_mask(ctx, t["teacher"], t["tok"], T, mask, tau, None, s)
+                tts.tts_distill_step(ctx, t["teacher"], t["h"], t["W"], t["W"], t["master"], t["m"], t["v"], t["pw"],
+                                     mask, T, case["loss_scale"], loss, None, gh, None, s)    # W_out aliases W_in
+            torch.cuda.synchronize()
+            if graph:
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g, stream=s):
+                    enqueue()
+                assert tts.tts_get_step_count(ctx) == 0          # captured, not run
+                with torch.cuda.stream(s):
+                    g.replay()
+                    g.replay()
+                tts.tts_record_done(ctx, s)
+            else:
+                enqueue()
+                enqueue()
+            tts.tts_sync_step(ctx)
+            torch.cuda.synchronize()
+            assert tts.tts_get_step_count(ctx) == 2
+            outs.append(dict(master=t["master"].cpu().numpy(), m=t["m"].cpu().numpy(), v=t["v"].cpu().numpy(),
+                             W=bits(t["W"]), loss=float(loss.item()), tau=tau.cpu().numpy()))
+        finally:
+            tts.tts_ctx_destroy(ctx)
+    a, b = outs
+    np.testing.assert_array_equal(a["tau"], b["tau"])
+    assert a["loss"] == b["loss"]
+    for k in ("m", "v", "master", "W"):
+        # gh's fp32 RED order may differ between runs, the weight state may not
+        np.testing.assert_array_equal(a[k], b[k])
