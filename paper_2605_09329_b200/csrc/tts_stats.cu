@@ -40,6 +40,31 @@ __device__ __forceinline__ void stat_push_ref(RowStat& s, float zr, float z) {
   else           { s.sr += e;             s.b += e * (zr - z); }
 }
 
+// N elements at once: one rescale of the running sums to the new maxima, then one exp per element (the per-element
+// form above costs a compare / select chain and an exp of the correction per element).  Same quantities.
+template <int N>
+__device__ __forceinline__ void stat_push_vec(RowStat& s, const float (&t)[N], const float (&z)[N]) {
+  float mt = s.mt, mz = s.mz;
+#pragma unroll
+  for (int k = 0; k < N; ++k) { mt = fmaxf(mt, t[k]); mz = fmaxf(mz, z[k]); }
+  if (mt != -CUDART_INF_F) {          // all teacher entries so far -inf: nothing to add (p = 0)
+    const float c = s.mt == -CUDART_INF_F ? 0.f : expf(s.mt - mt);
+    float st = s.st * c, a = s.a * c;
+#pragma unroll
+    for (int k = 0; k < N; ++k) {
+      const float e = expf(t[k] - mt);   // t = -inf -> 0
+      st += e;
+      a += t[k] == -CUDART_INF_F ? 0.f : e * (t[k] - z[k]);
+    }
+    s.st = st; s.a = a; s.mt = mt;
+  }
+  const float cz = s.mz == -CUDART_INF_F ? 0.f : expf(s.mz - mz);
+  float sz = s.sz * cz;
+#pragma unroll
+  for (int k = 0; k < N; ++k) sz += expf(z[k] - mz);
+  s.sz = sz; s.mz = mz;
+}
+
 __device__ __forceinline__ RowStat stat_merge(const RowStat& x, const RowStat& y) {
   RowStat o;
   o.mt = fmaxf(x.mt, y.mt);
@@ -99,8 +124,7 @@ __global__ void __launch_bounds__(256) row_stats_partial_kernel(const void* __re
       float f[8];
       unpack_bf16x8(q, f);
       const float zz[8] = {z0.x, z0.y, z0.z, z0.w, z1.x, z1.y, z1.z, z1.w};
-#pragma unroll
-      for (int k = 0; k < 8; ++k) stat_push(s, f[k], zz[k]);
+      stat_push_vec<8>(s, f, zz);
       if (zf) {
         const float4 r0 = __ldg(reinterpret_cast<const float4*>(zf + v0) + 2 * i);
         const float4 r1 = __ldg(reinterpret_cast<const float4*>(zf + v0) + 2 * i + 1);
@@ -121,7 +145,10 @@ __global__ void __launch_bounds__(256) row_stats_partial_kernel(const void* __re
     for (int i = threadIdx.x; i < nvec; i += blockDim.x) {
       const float4 q = __ldg(pt + i);
       const float4 z0 = __ldg(pz + i);
-      stat_push(s, q.x, z0.x); stat_push(s, q.y, z0.y); stat_push(s, q.z, z0.z); stat_push(s, q.w, z0.w);
+      {
+        const float tq[4] = {q.x, q.y, q.z, q.w}, zq[4] = {z0.x, z0.y, z0.z, z0.w};
+        stat_push_vec<4>(s, tq, zq);
+      }
       if (zf) {
         const float4 r0 = __ldg(reinterpret_cast<const float4*>(zf + v0) + i);
         stat_push_ref(s, r0.x, z0.x); stat_push_ref(s, r0.y, z0.y); stat_push_ref(s, r0.z, z0.z);

@@ -384,7 +384,7 @@ __global__ void __launch_bounds__(256) tc_prep_hT_kernel(const __nv_bfloat16* __
 }
 
 // dl = coef_r ((q - p) + lambda (q - q_ref)) from z, teacher and the row normalisers, scaled by S and rounded to fp16;
-// one [64 v x 64 k] tile per block.  Up to 32 rows the 64-wide K chunk has room for a second plane, so dl S is
+// one [128 v x 64 k] tile per block, two adjacent vocabulary rows per thread.  Up to 32 rows the 64-wide K chunk has room for a second plane, so dl S is
 // split hi + lo (two fp16, 2^-22) at no cost in operand bytes or MMAs and the h^T operand repeats its rows.  Written twice, both coalesced: dlT[v, r] (r contiguous: the K-major B operand
 // of gW; transposed through shared memory, 128-byte row segments) and dlR[r, v] (the K-major B operand of gh).
 // FAST (one fp16 plane, 2^-12): ex2.approx-based __expf, error ~|x| 1e-7, far inside the plane's rounding.
@@ -395,11 +395,12 @@ __global__ void __launch_bounds__(256) tc_prep_dl_wide_kernel(const void* __rest
                                                               const float* __restrict__ row_stats,
                                                               uint16_t* __restrict__ dlT, uint16_t* __restrict__ dlR,
                                                               float* __restrict__ dl_scale) {
-  constexpr int kPitch = 68;                      // halves: 34 words per row, 8-byte aligned rows
-  __shared__ __align__(16) uint16_t tile[64 * kPitch];
+  constexpr int kTileV = 128;                     // vocabulary rows per block: two adjacent ones per thread
+  constexpr int kPitch = 66;                      // halves: 33 words per row (phase-1 stores 2-way conflicted at most)
+  __shared__ __align__(16) uint16_t tile[kTileV * kPitch];
   __shared__ float sh[4 * 64];                    // lse_t, lse_z, coef, lse_ref of the tile's rows
   __shared__ float red[32];
-  const int v0 = blockIdx.x * 64, r0 = blockIdx.y * 64;
+  const int v0 = blockIdx.x * kTileV, r0 = blockIdx.y * 64;
   float cmax = 0.f;
   for (int r = threadIdx.x; r < T; r += blockDim.x) cmax = fmaxf(cmax, fabsf(row_stats[3 * T_max + r]));
   cmax = block_max(cmax, red);
@@ -417,39 +418,56 @@ __global__ void __launch_bounds__(256) tc_prep_dl_wide_kernel(const void* __rest
     sh[192 + threadIdx.x] = ok ? row_stats[4 * T_max + r] : 0.f;
   }
   __syncthreads();
-  const int vv = threadIdx.x & 63;
+  const int vv = 2 * (threadIdx.x & 63);          // V % 128 == 0 on this path: v, v + 1 < V, 8-byte aligned pairs
   const int v = v0 + vv;
   for (int rr = threadIdx.x >> 6; rr < 64; rr += 4) {
     const int k = r0 + rr;
     const bool lo_plane = planes == 2 && k >= T16;
     const int r = lo_plane ? k - T16 : k;
-    float dl = 0.f;
+    float dl[2] = {0.f, 0.f};
     if (r < T && k < planes * T16) {
-      const float t = BF16 ? __bfloat162float(static_cast<const __nv_bfloat16*>(teacher)[(size_t)r * V + v])
-                           : static_cast<const float*>(teacher)[(size_t)r * V + v];
-      const float az = z[(size_t)r * z_ld + v] - sh[64 + rr], at = t - sh[rr];
-      const float qv = FAST ? __expf(az) : expf(az);
-      const float pv = FAST ? __expf(at) : expf(at);   // t = -inf -> 0
-      float g = qv - pv;
-      if (z_ref) {
-        const float ar = z_ref[(size_t)r * z_ld + v] - sh[192 + rr];
-        g += lam * (qv - (FAST ? __expf(ar) : expf(ar)));
+      float t[2];
+      if (BF16) {
+        const uint32_t tb = *reinterpret_cast<const uint32_t*>(static_cast<const __nv_bfloat16*>(teacher) + (size_t)r * V + v);
+        t[0] = __uint_as_float(tb << 16); t[1] = __uint_as_float(tb & 0xFFFF0000u);
+      } else {
+        const float2 tf = *reinterpret_cast<const float2*>(static_cast<const float*>(teacher) + (size_t)r * V + v);
+        t[0] = tf.x; t[1] = tf.y;
       }
-      dl = sh[128 + rr] * g * S;
+      const float2 zz = *reinterpret_cast<const float2*>(z + (size_t)r * z_ld + v);
+      float2 zr = make_float2(0.f, 0.f);
+      if (z_ref) zr = *reinterpret_cast<const float2*>(z_ref + (size_t)r * z_ld + v);
+      const float zv[2] = {zz.x, zz.y}, zrv[2] = {zr.x, zr.y};
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        const float az = zv[e] - sh[64 + rr], at = t[e] - sh[rr];
+        const float qv = FAST ? __expf(az) : expf(az);
+        const float pv = FAST ? __expf(at) : expf(at);   // t = -inf -> 0
+        float g = qv - pv;
+        if (z_ref) {
+          const float ar = zrv[e] - sh[192 + rr];
+          g += lam * (qv - (FAST ? __expf(ar) : expf(ar)));
+        }
+        dl[e] = sh[128 + rr] * g * S;
+      }
     }
-    __half hq = __float2half_rn(dl);
-    if (lo_plane) hq = __float2half_rn(dl - __half2float(hq));   // dl S = hi + lo to 2^-22
-    const uint16_t hv = __half_as_ushort(hq);
-    tile[vv * kPitch + rr] = hv;
-    if (dlR && k < planes * T16) dlR[(size_t)k * V + v] = hv;   // rows T .. T16 of a plane are zero
+    uint16_t hv[2];
+#pragma unroll
+    for (int e = 0; e < 2; ++e) {
+      __half hq = __float2half_rn(dl[e]);
+      if (lo_plane) hq = __float2half_rn(dl[e] - __half2float(hq));   // dl S = hi + lo to 2^-22
+      hv[e] = __half_as_ushort(hq);
+      tile[(vv + e) * kPitch + rr] = hv[e];
+    }
+    if (dlR && k < planes * T16)   // rows T .. T16 of a plane are zero
+      *reinterpret_cast<uint32_t*>(dlR + (size_t)k * V + v) = (uint32_t)hv[0] | ((uint32_t)hv[1] << 16);
   }
   __syncthreads();
   // 8 threads per vocabulary row: 16 bytes each -> one 128-byte segment of dlT per row
   const int seg = threadIdx.x & 7;
-  for (int row = threadIdx.x >> 3; row < 64; row += 32) {
-    const uint2* src = reinterpret_cast<const uint2*>(tile + row * kPitch + seg * 8);
-    const uint2 a = src[0], b = src[1];
-    *reinterpret_cast<uint4*>(dlT + (size_t)(v0 + row) * Kp + r0 + seg * 8) = make_uint4(a.x, a.y, b.x, b.y);
+  for (int row = threadIdx.x >> 3; row < kTileV; row += 32) {
+    const uint32_t* src = reinterpret_cast<const uint32_t*>(tile + row * kPitch + seg * 8);
+    *reinterpret_cast<uint4*>(dlT + (size_t)(v0 + row) * Kp + r0 + seg * 8) = make_uint4(src[0], src[1], src[2], src[3]);
   }
 }
 
@@ -498,7 +516,7 @@ cudaError_t tc_launch_prep_wide(tts_ctx* c, const StepArgs& a, const float* z, c
                                                                   static_cast<uint16_t*>(st->hTT), st->dl_scale);
   uint16_t* dlT = static_cast<uint16_t*>(st->dlT);
   uint16_t* dlR = a.gh_out ? static_cast<uint16_t*>(st->dlR) : nullptr;
-  const dim3 grid(V / 64, Kp / 64);
+  const dim3 grid(V / 128, Kp / 64);
   const bool bf = c->cfg.logits_dtype == TTS_BF16, fast = planes == 1;
   auto kern = bf ? (fast ? tc_prep_dl_wide_kernel<true, true> : tc_prep_dl_wide_kernel<true, false>)
                  : (fast ? tc_prep_dl_wide_kernel<false, true> : tc_prep_dl_wide_kernel<false, false>);
