@@ -83,6 +83,10 @@ SMALL = [
     (3, 1024 + 128, 2048, 1, 8, {}),                 # fused stripe kernel: two stripes, T = 8 padded to 16 rows
     (4, 2048 + 128, 256, 32, 16, {}),                # 512 rows: CTA-pair logits (17 tiles of 128: the last pair tile is half empty), full-TMEM gh
     (4, 1024, 384, 20, 16, {}),                      # 320 rows: pair pieces of 256 + 64 rows
+    (4, 1024, 256, 17, 16, {}),                      # 272 rows: second pair piece of 16 rows (8 per CTA)
+    (4, 1024, 128, 3, 16, {}),                       # 48 rows: one fp16 dl plane, K padded to 64
+    (4, 1024, 128, 2, 16, {}),                       # 32 rows: hi + lo fp16 planes fill the 64-wide K chunk
+    (4, 1024, 128, 12, 16, {}),                      # 192 rows: gh accumulators double-buffered, K = 192
 ]
 
 
