@@ -53,6 +53,41 @@ struct PairLogitsParams {
   int T16;
   int n_pieces;    // ceil(T16 / 256)
   int stages;
+  // work split: `n_rounds` rounds of whole tiles (tile = pair + round * n_pairs, below n_main), then the `n_left`
+  // tiles from n_main on are cut along K into n_pairs equal unit ranges (594 tiles over 74 pairs would otherwise be
+  // 8.03 waves rounding to 9); their partial sums are accumulated into the zeroed z columns with fp32 RED
+  int n_rounds, n_main, n_left;
+};
+
+struct PairItem {
+  int pt, c_beg, c_end;
+  bool partial;
+};
+
+struct PairWalk {
+  int pair, n_pairs, round;
+  long u, u_end;
+  __device__ PairWalk(const PairLogitsParams& p, int pair_, int n_pairs_) : pair(pair_), n_pairs(n_pairs_), round(0) {
+    const long U = (long)p.n_left * p.k_chunks;
+    u = U * pair / n_pairs;
+    u_end = U * (pair + 1) / n_pairs;
+  }
+  __device__ bool next(const PairLogitsParams& p, PairItem& w) {
+    while (round < p.n_rounds) {
+      const int pt = pair + round * n_pairs;
+      ++round;
+      if (pt < p.n_main) { w.pt = pt; w.c_beg = 0; w.c_end = p.k_chunks; w.partial = false; return true; }
+    }
+    if (u >= u_end) return false;
+    const int t = (int)(u / p.k_chunks);
+    w.c_beg = (int)(u - (long)t * p.k_chunks);
+    const long rest = u_end - u;
+    w.c_end = rest < p.k_chunks - w.c_beg ? w.c_beg + (int)rest : p.k_chunks;
+    w.pt = p.n_main + t;
+    w.partial = true;
+    u += w.c_end - w.c_beg;
+    return true;
+  }
 };
 
 constexpr uint32_t kDescHiSw128 = (1024u >> 4) | (1u << 14) | (ptx::kSwizzle128B << 29);
@@ -94,9 +129,11 @@ tc_logits_pair_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_con
     // ===== TMA producer (both CTAs): own W rows + own half of every h piece; bytes counted on the leader's barrier =====
     if (lane == 0) {
       uint32_t n = 0;
-      for (int pt = pair; pt < p.n_pt; pt += n_pairs) {
-        const int v0 = pt * 256 + (int)cta * 128;             // rows beyond V: zero fill
-        for (int kc = 0; kc < p.k_chunks; ++kc, ++n) {
+      PairWalk walk(p, pair, n_pairs);
+      PairItem w;
+      while (walk.next(p, w)) {
+        const int v0 = w.pt * 256 + (int)cta * 128;           // rows beyond V: zero fill
+        for (int kc = w.c_beg; kc < w.c_end; ++kc, ++n) {
           const int s = n % p.stages;
           ptx::mbar_wait(&bars->empty[s], ((n / p.stages) & 1) ^ 1);
           uint8_t* A = smem + s * stage_bytes;
@@ -116,10 +153,12 @@ tc_logits_pair_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_con
     if (cta == 0 && lane == 0) {
       const uint32_t smem0 = ptx::smem_u32(smem);
       uint32_t n = 0, it = 0;
-      for (int pt = pair; pt < p.n_pt; pt += n_pairs, ++it) {
+      PairWalk walk(p, pair, n_pairs);
+      PairItem w;
+      for (; walk.next(p, w); ++it) {
         ptx::mbar_wait_cluster(&bars->acc_empty, (it & 1) ^ 1);
         ptx::tc_fence_after();
-        for (int kc = 0; kc < p.k_chunks; ++kc, ++n) {
+        for (int kc = w.c_beg; kc < w.c_end; ++kc, ++n) {
           const int s = n % p.stages;
           ptx::mbar_wait(&bars->full[s], (n / p.stages) & 1);
           ptx::tc_fence_after();
@@ -131,7 +170,7 @@ tc_logits_pair_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_con
               const uint32_t b_lo = desc_lo_sw128(smem0 + s * stage_bytes + kPATile + q * piece_bytes);
               ptx::mma_f16_ss_pair(tmem_base + q * kPNMax, desc64(kDescHiSw128, a_lo + 2 * ks),
                                    desc64(kDescHiSw128, b_lo + 2 * ks), ptx::make_idesc_bf16(256, nn, 0, 0),
-                                   (kc | ks) != 0);
+                                   (kc != w.c_beg) | ks);
             }
           }
           ptx::mma_commit_pair(&bars->empty[s]);
@@ -143,18 +182,25 @@ tc_logits_pair_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_con
     // ===== epilogue (both CTAs): thread = one vocabulary row of this CTA's half of the tile =====
     const int q4 = warp & 3;
     uint32_t it = 0;
-    for (int pt = pair; pt < p.n_pt; pt += n_pairs, ++it) {
+    PairWalk walk(p, pair, n_pairs);
+    PairItem w;
+    for (; walk.next(p, w); ++it) {
       ptx::mbar_wait(&bars->acc_full, it & 1);
       ptx::tc_fence_after();
-      const int v = pt * 256 + (int)cta * 128 + q4 * 32 + lane;
+      const int v = w.pt * 256 + (int)cta * 128 + q4 * 32 + lane;
       float* zc = p.z + v;
       for (int c0 = 0; c0 < p.T16; c0 += 16) {
         uint32_t r[16];
         ptx::tmem_ld_32x32b_x16(tmem_base + c0 + (static_cast<uint32_t>(q4 * 32) << 16), r);
         ptx::tmem_ld_wait();
         if (v < p.V) {
+          if (w.partial) {
 #pragma unroll
-          for (int i = 0; i < 16; ++i) zc[(size_t)(c0 + i) * p.z_ld] = __uint_as_float(r[i]);
+            for (int i = 0; i < 16; ++i) atomicAdd(zc + (size_t)(c0 + i) * p.z_ld, __uint_as_float(r[i]));
+          } else {
+#pragma unroll
+            for (int i = 0; i < 16; ++i) zc[(size_t)(c0 + i) * p.z_ld] = __uint_as_float(r[i]);
+          }
         }
       }
       ptx::tc_fence_before();
@@ -213,6 +259,17 @@ cudaError_t tc_launch_logits_pair(tts_ctx* c, const StepArgs& a, float* z_out, c
   int grid = c->cfg.max_ctas > 0 ? c->cfg.max_ctas : c->sm_count;
   grid &= ~1;
   if (grid > 2 * p.n_pt) grid = 2 * p.n_pt;
+  const int n_pairs = grid / 2;
+  p.n_rounds = p.n_pt / n_pairs;
+  p.n_left = p.n_pt % n_pairs;
+  if (p.n_left > n_pairs / 2) { p.n_rounds += 1; p.n_left = 0; }   // a nearly full last round: whole tiles
+  p.n_main = p.n_pt - p.n_left;
+  if (p.n_left > 0) {
+    // the K-split tiles accumulate into zeroed columns [256 n_main, V) of z
+    const size_t v_left = (size_t)p.n_main * 256;
+    cudaError_t e = cudaMemset2DAsync(z_out + v_left, (size_t)V * sizeof(float), 0, (V - v_left) * sizeof(float), T16, s);
+    if (e != cudaSuccess) return e;
+  }
   cudaLaunchConfig_t cfg;
   memset(&cfg, 0, sizeof(cfg));
   cfg.gridDim = dim3(grid);
