@@ -230,6 +230,7 @@ struct GhParams {
   int planes;        // dl planes stacked along N (2: rows T16 .. 2 T16 hold the lo plane)
   int N;             // planes * T16: accumulator columns
   int n_jt;          // d / 128
+  int n_ju;          // units along j: n_jt, or ceil(n_jt / 2) cluster units with MC
   int n_split;       // vocabulary splits
   int chunks_split;  // K chunks (of 64 vocabulary rows) per split
   int chunks_total;  // V / 64
@@ -246,6 +247,11 @@ struct GhParams {
 // 2e-3 max|gh| bar), kind::f16 wants A and B in one format, and W arrives as bf16 from the caller's memory: so four
 // otherwise idle warps rewrite each W tile in shared memory as fp16(16 W) (element-wise, so the swizzle is
 // untouched; exact for 2^-18 <= |W| < 4094, values beyond are clamped) before the MMAs of that stage are issued.
+// MC (T16 > 256): a cluster of two CTAs takes two adjacent j tiles of the same vocabulary split; each CTA loads ONE of
+// the two 256-row dl boxes of a stage and TMA multicasts it to both, so a dl chunk leaves L2 once per two j tiles
+// (this kernel runs at the L2 slice throughput: 6.2 GB at 8.5 TB/s without it).  Everything else stays per CTA; a
+// stage is reused when BOTH CTAs' MMAs have read it (empty[s] collects both commits, each multicast to both CTAs).
+template <bool MC>
 __global__ void __launch_bounds__(kGhThreads, 1)
 tc_gh_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant__ CUtensorMap tm_dl, const GhParams p) {
   extern __shared__ uint8_t smem_raw[];
@@ -254,7 +260,11 @@ tc_gh_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant__ C
   const int stage_bytes = kATile + b_bytes;
   Bars* bars = reinterpret_cast<Bars*>(smem + p.stages * stage_bytes);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int n_units = p.n_jt * p.n_split;
+  const int n_units = p.n_ju * p.n_split;
+  const int cta = MC ? (int)ptx::cluster_ctarank() : 0;
+  const int u_first = MC ? (int)(blockIdx.x >> 1) : (int)blockIdx.x, u_step = MC ? (int)(gridDim.x >> 1) : (int)gridDim.x;
+  // unit u -> first hidden column of this CTA's tile (beyond d with MC and an odd tile count: zero fill, nothing flushed)
+  auto unit_j0 = [&](int u) { return ((u % p.n_ju) * (MC ? 2 : 1) + cta) * kTileMN; };
 
   if (warp == 0 && lane == 0) {
     ptx::prefetch_tensormap(&tm_W);
@@ -262,7 +272,7 @@ tc_gh_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant__ C
   }
   if (warp == 1 && lane == 0) {
     for (int i = 0; i < p.stages; ++i) {
-      ptx::mbar_init(&bars->full[i], 1); ptx::mbar_init(&bars->empty[i], 1); ptx::mbar_init(&bars->conv[i], 128);
+      ptx::mbar_init(&bars->full[i], 1); ptx::mbar_init(&bars->empty[i], MC ? 2 : 1); ptx::mbar_init(&bars->conv[i], 128);
     }
     for (int i = 0; i < 2; ++i) { ptx::mbar_init(&bars->acc_full[i], 1); ptx::mbar_init(&bars->acc_empty[i], 4); }
     ptx::fence_barrier_init();
@@ -272,7 +282,7 @@ tc_gh_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant__ C
     ptx::tmem_relinquish();
   }
   ptx::tc_fence_before();
-  __syncthreads();
+  if (MC) ptx::cluster_sync(); else __syncthreads();
   ptx::tc_fence_after();
   const uint32_t tmem_base = bars->tmem_slot;
 
@@ -280,8 +290,8 @@ tc_gh_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant__ C
     // ===== W tile bf16 -> fp16(16 W), in place: 16 KB per stage, 8 x 16 bytes per thread =====
     const int t = threadIdx.x - 256;
     uint32_t n = 0;
-    for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
-      const int sp = u / p.n_jt;
+    for (int u = u_first; u < n_units; u += u_step) {
+      const int sp = u / p.n_ju;
       const int c_beg = sp * p.chunks_split, c_end = min(p.chunks_total, c_beg + p.chunks_split);
       for (int kc = c_beg; kc < c_end; ++kc, ++n) {
         const int s = n % p.stages;
@@ -307,8 +317,8 @@ tc_gh_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant__ C
   } else if (warp == 0) {
     if (lane == 0) {
       uint32_t n = 0;
-      for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
-        const int j0 = (u % p.n_jt) * kTileMN, sp = u / p.n_jt;
+      for (int u = u_first; u < n_units; u += u_step) {
+        const int j0 = unit_j0(u), sp = u / p.n_ju;
         const int c_beg = sp * p.chunks_split, c_end = min(p.chunks_total, c_beg + p.chunks_split);
         for (int kc = c_beg; kc < c_end; ++kc, ++n) {
           const int s = n % p.stages;
@@ -318,16 +328,21 @@ tc_gh_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant__ C
           // W rows kc*64 .. +63 (K), columns j0 .. j0+127 (M) as two [64 k x 64 m] boxes
           ptx::tma_load_2d(A, &tm_W, &bars->full[s], j0, kc * kKC);
           ptx::tma_load_2d(A + kATile / 2, &tm_W, &bars->full[s], j0 + 64, kc * kKC);
-          for (int b = 0; b < p.n_boxes; ++b)   // rows beyond the scratch are out of bounds: zero fill
-            ptx::tma_load_2d(A + kATile + b * p.box_rows * kKC * 2, &tm_dl, &bars->full[s], kc * kKC, b * p.box_rows);
+          if (MC) {   // this CTA's one of the two dl boxes, to both CTAs
+            ptx::tma_load_2d_multicast(A + kATile + cta * p.box_rows * kKC * 2, &tm_dl, &bars->full[s], kc * kKC,
+                                       cta * p.box_rows, 3);
+          } else {
+            for (int b = 0; b < p.n_boxes; ++b)   // rows beyond the scratch are out of bounds: zero fill
+              ptx::tma_load_2d(A + kATile + b * p.box_rows * kKC * 2, &tm_dl, &bars->full[s], kc * kKC, b * p.box_rows);
+          }
         }
       }
     }
   } else if (warp == 1) {
     if (lane == 0) {
       uint32_t n = 0, it = 0;
-      for (int u = blockIdx.x; u < n_units; u += gridDim.x, ++it) {
-        const int sp = u / p.n_jt;
+      for (int u = u_first; u < n_units; u += u_step, ++it) {
+        const int sp = u / p.n_ju;
         const int c_beg = sp * p.chunks_split, c_end = min(p.chunks_total, c_beg + p.chunks_split);
         const int ab = it % p.n_acc;
         ptx::mbar_wait(&bars->acc_empty[ab], ((it / p.n_acc) & 1) ^ 1);
@@ -353,7 +368,7 @@ tc_gh_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant__ C
                               (kc != c_beg) || ks != 0);
             }
           }
-          ptx::mma_commit(&bars->empty[s]);
+          if (MC) ptx::mma_commit_multicast(&bars->empty[s], 3); else ptx::mma_commit(&bars->empty[s]);
         }
         ptx::mma_commit(&bars->acc_full[ab]);
       }
@@ -362,8 +377,8 @@ tc_gh_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant__ C
     const int q = warp & 3;
     const float inv_s = p.dl_scale[1] * (1.f / kGhWScale);
     uint32_t it = 0;
-    for (int u = blockIdx.x; u < n_units; u += gridDim.x, ++it) {
-      const int j0 = (u % p.n_jt) * kTileMN;
+    for (int u = u_first; u < n_units; u += u_step, ++it) {
+      const int j0 = unit_j0(u);
       const int ab = it % p.n_acc;
       ptx::mbar_wait(&bars->acc_full[ab], (it / p.n_acc) & 1);
       ptx::tc_fence_after();
@@ -379,7 +394,7 @@ tc_gh_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant__ C
         for (int i = 0; i < 16; ++i) {
           float x = __uint_as_float(r[i]);
           if (p.planes == 2) x += __uint_as_float(r2[i]);
-          if (c0 + i < p.T) atomicAdd(gc + (size_t)(c0 + i) * p.d, x * inv_s);
+          if (c0 + i < p.T && j0 < p.d) atomicAdd(gc + (size_t)(c0 + i) * p.d, x * inv_s);
         }
       }
       ptx::tc_fence_before();
@@ -388,7 +403,7 @@ tc_gh_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant__ C
     }
   }
   ptx::tc_fence_before();
-  __syncthreads();
+  if (MC) ptx::cluster_sync(); else __syncthreads();
   if (warp == 2) {
     ptx::tc_fence_after();
     ptx::tmem_dealloc(tmem_base, p.tmem_cols);
@@ -411,7 +426,10 @@ cudaError_t tc_gemm_init(tts_ctx*) {
   if ((e = cudaFuncSetAttribute(tc_logits_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max)) !=
       cudaSuccess)
     return e;
-  return cudaFuncSetAttribute(tc_gh_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max);
+  if ((e = cudaFuncSetAttribute(tc_gh_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max)) !=
+      cudaSuccess)
+    return e;
+  return cudaFuncSetAttribute(tc_gh_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max);
 }
 
 cudaError_t tc_launch_logits(tts_ctx* c, const StepArgs& a, float* z_out, cudaStream_t s, int* launches) {
@@ -471,10 +489,17 @@ cudaError_t tc_launch_gh(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* lau
   p.n_boxes = (p.N + p.box_rows - 1) / p.box_rows;
   p.n_acc = 2 * p.N <= 512 ? 2 : 1;
   p.tmem_cols = pow2_cols(p.n_acc * p.N);
-  // About two units per CTA: each is a contiguous run of vocabulary chunks for one 128-column tile of gh, flushed
-  // with fp32 RED (256 KB per unit at T = 512: more units would make the flush the bottleneck).  Units of one
-  // vocabulary split run side by side on consecutive CTAs, so a dl chunk is fetched into L2 once for all j tiles.
-  int n_split = (2 * grid) / p.n_jt;
+  // MC: clusters of two CTAs on adjacent j tiles share every dl box by TMA multicast (two boxes: 256 < T16 <= 512)
+  static int mc_off = -1;
+  if (mc_off < 0) { const char* e = getenv("TTS_NO_GH_MC"); mc_off = (e && e[0] == '1') ? 1 : 0; }   // measurement switch
+  const bool mc = !mc_off && p.n_boxes == 2 && grid >= 2;
+  if (mc) grid &= ~1;
+  const int n_cl = mc ? grid / 2 : grid;
+  p.n_ju = mc ? (p.n_jt + 1) / 2 : p.n_jt;
+  // About two units per CTA (cluster): each is a contiguous run of vocabulary chunks for one 128-column tile of gh,
+  // flushed with fp32 RED (256 KB per unit at T = 512: more units would make the flush the bottleneck).  Units of
+  // one vocabulary split run side by side on consecutive CTAs, so a dl chunk is fetched into L2 once for all j tiles.
+  int n_split = (2 * n_cl) / p.n_ju;
   if (n_split < 1) n_split = 1;
   if (n_split > p.chunks_total) n_split = p.chunks_total;
   p.chunks_split = (p.chunks_total + n_split - 1) / n_split;
@@ -488,10 +513,26 @@ cudaError_t tc_launch_gh(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* lau
   if (make_map_2d(st, &tm_dl, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, st->dlR, V, (uint64_t)st->P, kKC, p.box_rows,
                   CU_TENSOR_MAP_SWIZZLE_128B) != CUDA_SUCCESS)
     return cudaErrorInvalidValue;
-  const int n_units = p.n_jt * p.n_split;
-  if (grid > n_units) grid = n_units;
+  const int n_units = p.n_ju * p.n_split;
   const size_t smem = 1024 + (size_t)p.stages * stage_bytes + sizeof(Bars);
-  tc_gh_kernel<<<grid, kGhThreads, smem, s>>>(tm_W, tm_dl, p);
+  if (!mc) {
+    if (grid > n_units) grid = n_units;
+    tc_gh_kernel<false><<<grid, kGhThreads, smem, s>>>(tm_W, tm_dl, p);
+  } else {
+    if (grid > 2 * n_units) grid = 2 * n_units;
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(kGhThreads);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = s;
+    cudaLaunchAttribute attr;
+    attr.id = cudaLaunchAttributeClusterDimension;
+    attr.val.clusterDim.x = 2; attr.val.clusterDim.y = 1; attr.val.clusterDim.z = 1;
+    cfg.attrs = &attr;
+    cfg.numAttrs = 1;
+    if ((e = cudaLaunchKernelEx(&cfg, tc_gh_kernel<true>, tm_W, tm_dl, p)) != cudaSuccess) return e;
+  }
   *launches += 1;
   return cudaGetLastError();
 }
