@@ -446,7 +446,7 @@ cudaError_t tc_fused_init(tts_ctx* c) {
 }
 
 // Grid of the fused pass, 0 when the shape does not qualify (T > 16 rows, d or V not a multiple of the tile, or an
-// SM budget below one CTA per 1024-column stripe: a CTA owns exactly one stripe, so the general tile kernel, which
+// SM budget below one CTA per 1024-column stripe: a CTA owns exactly one stripe, so the wide kernel (tts_tc_wide.cu), which
 // walks any grid, serves that case).
 int tc_fused_grid(const tts_ctx* c, int T16) {
   if (T16 > kT16 || c->cfg.d % kSW != 0 || c->cfg.V % kTV != 0) return 0;

@@ -8,9 +8,10 @@
 //   gh     (a5)  gh^T[j, r] = sum_v W_in[v, j] dl[r, v]        M = 128 hidden columns, N = T16 rows, K = vocabulary
 //                A = W_in tile, MN-major (the same row-major W: j is contiguous, K = v strides by a row);
 //                B = the fp16 plane S dl [r, v] of tts_tc_wide.cu, K-major; the W tile is rewritten as fp16 in
-//                shared memory (see the kernel); the epilogue multiplies by 1 / (16 S).  The vocabulary is split over CTAs; partial tiles are
-//                reduced with fp32 atomics into gh (zeroed first).  (One canvas with d % 1024 == 0 never comes
-//                here: tts_tc_fused.cu forms gh inside the update pass.)
+//                shared memory (see the kernel); the epilogue multiplies by 1 / (16 S).  The vocabulary is split
+//                over CTAs; partial tiles are reduced with fp32 atomics into gh (zeroed first).  (One canvas with
+//                d % 1024 == 0 never comes here: tts_tc_fused.cu forms gh inside the update pass.  Beyond 256 rows
+//                the logits pass is served by the CTA-pair kernel of tts_tc_pair.cu.)
 #include <cuda_fp16.h>
 #include <string.h>
 
