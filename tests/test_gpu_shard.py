@@ -137,3 +137,57 @@ def test_mask_ties_across_shards_take_the_lowest_global_index():
     np.testing.assert_array_equal(g["mask"], mask)
     np.testing.assert_array_equal(g["tau"], tau)
     assert am[:4].tolist() == [100, 513, 800, 0]
+
+
+def test_sharded_step_with_given_logits_and_lambda_term():
+    """f1 extras through the shard calls: every shard passes ITS columns of the drafter's logits and of the reference
+    logits; the (m_ref, s_ref, b) fields of the exchanged tuples must merge to the whole-row regulariser."""
+    case = synth.make_case(3, V=2048, d=256, nonzero_state=True, step=3)
+    G, T, V, d = 2, case["T"], case["V"], case["d"]
+    rng = np.random.Generator(np.random.PCG64(9))
+    W = O.widen(case["W"]); hh = O.widen(case["h"])
+    z_given = (hh @ W.T + 0.05 * rng.standard_normal((T, V))).astype(np.float32)
+    z_ref = (hh @ W.T + 0.8 * rng.standard_normal((T, V))).astype(np.float32)
+    lam = 0.6
+    c = case["cfg"]
+    mask, _, _ = O.accept_mask(case["teacher"], case["draft_tokens"], case["seg_len"])
+    o = O.distill_step(case["teacher"], case["h"], case["W"], case["master"], case["m"], case["v"], case["pos_weight"],
+                       mask, seg_len=case["seg_len"], loss_scale=case["loss_scale"], optimizer="adamw", lr=c["lr"],
+                       beta1=c["beta1"], beta2=c["beta2"], eps=c["eps"], weight_decay=c["weight_decay"], step=3,
+                       draft_logits=z_given, lam=lam, z_ref=z_ref)
+    h, pw = _dev(case["h"]), _dev(case["pos_weight"])
+    shards = []
+    for g in range(G):
+        v0, v1 = sharded.shard_range(V, g, G)
+        cfg = tts.make_config(v1 - v0, d, T, case["seg_len"], c["param"], c["logits"], c["optimizer"], c["lr"],
+                              c["beta1"], c["beta2"], c["eps"], c["weight_decay"])
+        ctx = tts.tts_ctx_create(cfg, 0)
+        tts.tts_set_step_count(ctx, 2)
+        shards.append(dict(ctx=ctx, teacher=_dev(np.ascontiguousarray(case["teacher"][:, v0:v1])),
+                           W=_dev(case["W"][v0:v1]), master=_dev(case["master"][v0:v1]), m=_dev(case["m"][v0:v1]),
+                           v=_dev(case["v"][v0:v1]), zg=_dev(np.ascontiguousarray(z_given[:, v0:v1])),
+                           zr=_dev(np.ascontiguousarray(z_ref[:, v0:v1])), stats=torch.zeros(T, 8, device="cuda"),
+                           loss=torch.zeros(1, device="cuda"), kl=torch.zeros(T, device="cuda"),
+                           gh=torch.zeros(T, d, device="cuda")))
+    try:
+        for sh in shards:
+            tts.tts_shard_begin_step(sh["ctx"], sh["teacher"], h, sh["W"], T, sh["stats"], draft_logits=sh["zg"],
+                                     ref_logits=sh["zr"], lam=lam)
+        stats_all = torch.stack([sh["stats"] for sh in shards]).contiguous()
+        for sh in shards:
+            tts.tts_shard_finish_step(sh["ctx"], stats_all, G, sh["teacher"], h, sh["W"], sh["W"], sh["master"], sh["m"],
+                                      sh["v"], pw, None, T, case["loss_scale"], sh["loss"], sh["kl"], sh["gh"], None,
+                                      draft_logits=sh["zg"], ref_logits=sh["zr"], lam=lam)
+        torch.cuda.synchronize()
+        loss = float(shards[0]["loss"].item())
+        assert loss == float(shards[1]["loss"].item())
+        assert abs(loss - o["loss"]) <= 1e-3 * abs(o["loss"]) + 1e-6
+        assert np.all(np.abs(shards[0]["kl"].cpu().numpy() - o["kl_rows"]) <= 1e-3 * np.abs(o["kl_rows"]) + 1e-5)
+        cat = lambda k: np.concatenate([sh[k].cpu().numpy() for sh in shards]).astype(np.float64)
+        for name, gg, ref in (("master", cat("master"), o["master"]), ("m", cat("m"), o["m"]), ("v", cat("v"), o["v"]),
+                              ("gh", sum(sh["gh"] for sh in shards).cpu().numpy().astype(np.float64), o["gh"])):
+            assert np.abs(gg - ref).max() <= 2e-3 * np.abs(ref).max(), name
+        assert [tts.tts_get_step_count(sh["ctx"]) for sh in shards] == [3, 3]
+    finally:
+        for sh in shards:
+            tts.tts_ctx_destroy(sh["ctx"])
