@@ -44,7 +44,7 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=30)
     ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--config", type=int, default=3, choices=[2, 3, 4, 5])
+    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--kernel-path", default="auto", choices=["auto", "simt"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -183,8 +183,8 @@ def time_oracle(case, sample, repeats=1):
         mask, tau, am = O.accept_mask(sample["teacher"], sample["tok"], case["seg_len"])
         O.distill_step(sample["teacher"], sample["h"], sample["W"], sample["master"], sample["m"], sample["v"],
                        sample["pw"], mask, seg_len=case["seg_len"], loss_scale=case["loss_scale"],
-                       optimizer="adamw", lr=c["lr"], beta1=c["beta1"], beta2=c["beta2"], eps=c["eps"],
-                       weight_decay=c["weight_decay"], step=1)
+                       optimizer="sgd" if sample["m"] is None else "adamw", lr=c["lr"], beta1=c["beta1"],
+                       beta2=c["beta2"], eps=c["eps"], weight_decay=c["weight_decay"], step=1)
         dt = time.perf_counter() - t0
         best = dt if best is None else min(best, dt)
     return best
@@ -207,7 +207,7 @@ def run_reference(args, rank, world):
     from paper_2605_09329_b200 import synth
     cfgc = synth.CONFIGS[args.config]
     V, d = cfgc["V"], cfgc["d"]
-    rows = min(args.cpu_sample_rows, 4096)   # ~1.5 s of oracle work per step
+    rows = min(args.cpu_sample_rows, 4096, V)   # ~1.5 s of oracle work per step (config 1: the whole problem)
     # the sample is a scaled-down draw of the same recipe (same d, T; first `rows` of the vocabulary)
     case = synth.make_case(args.config, V=rows, n_seq=min(cfgc["n_seq"], 2) if args.config == 4 else None)
     sample = dict(teacher=case["teacher"], h=case["h"], W=case["W"], master=case["master"], m=case["m"],
@@ -240,10 +240,11 @@ def workload_config(cfg_id, world, path, parallelism="replicas"):
     if world > 1:
         par = ("replicas x%d (no data-path collective)" % world if parallelism == "replicas" else
                "vocabulary shards x%d (all-gather [T,8] row tuples + all-reduce gh [T,d] per step, NCCL)" % world)
-    return {"workload": "BASELINE.json configs[%d] %s: V=%d d=%d T=%d (seg_len %d x %d seq), bf16 W + fp32 master, "
-                        "AdamW lr=1e-5" % (cfg_id - 1, c["name"], c["V"], c["d"], c["seg_len"] * c["n_seq"],
-                                           c["seg_len"], c["n_seq"]),
-            "V": c["V"], "d": c["d"], "T": c["seg_len"] * c["n_seq"], "optimizer": "adamw",
+    kind = ("fp32 throughout, plain SGD lr=1e-3" if c["param"] == synth.F32 else "bf16 W + fp32 master, AdamW lr=1e-5")
+    return {"workload": "BASELINE.json configs[%d] %s: V=%d d=%d T=%d (seg_len %d x %d seq), %s"
+                        % (cfg_id - 1, c["name"], c["V"], c["d"], c["seg_len"] * c["n_seq"], c["seg_len"], c["n_seq"], kind),
+            "V": c["V"], "d": c["d"], "T": c["seg_len"] * c["n_seq"],
+            "optimizer": "sgd" if c["optimizer"] == synth.SGD else "adamw",
             "parallelism": par,
             "kernel_path": path,
             "l2": "working set per step (17 GB of weight state) exceeds the 126 MB L2: every step is L2-cold"}
@@ -551,6 +552,102 @@ def run_stream(args, case, dev):
     return res
 
 
+def run_tiny(args):
+    """BASELINE.json configs[0]: V=1024, d=64, T=8, fp32 throughout, plain SGD -- the CUDA-core kernels.  786 KB of
+    state: the step is launch-latency-bound ("report us/step only"), so the roofline object carries the
+    step's bytes over its time for the record and says so; the numbers that mean something are ms_per_step, the
+    number of launches and the oracle's time on the same (whole) problem."""
+    import numpy as np
+    import torch
+    from paper_2605_09329_b200 import synth, tts
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the distillation step has no CPU fallback")
+    case = synth.make_case(1)
+    c = case["cfg"]
+    V, d, T, C = case["V"], case["d"], case["T"], case["seg_len"]
+    cfg = tts.make_config(V, d, T, C, tts.TTS_F32, tts.TTS_F32, tts.TTS_SGD, c["lr"], max_ctas=args.max_ctas)
+    ctx = tts.tts_ctx_create(cfg, 0)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    teacher, h, tok, pw = dev(case["teacher"]), dev(case["h"]), dev(case["draft_tokens"]), dev(case["pos_weight"])
+    W = [dev(case["W"]), torch.empty(V, d, device="cuda")]
+    mask = torch.zeros(T, dtype=torch.uint8, device="cuda")
+    tau = torch.zeros(T // C, dtype=torch.int32, device="cuda")
+    loss = torch.zeros(1, device="cuda")
+    gh = torch.zeros(T, d, device="cuda")
+    side, main = torch.cuda.Stream(), torch.cuda.current_stream()
+    cur, launches = [0], [0]
+
+    def step():
+        tts.tts_accept_mask(ctx, teacher, tok, T, mask, tau, None, side)
+        n = tts.tts_last_launch_count(ctx)
+        tts.tts_distill_step(ctx, teacher, h, W[cur[0]], W[1 - cur[0]], None, None, None, pw, mask, T, 1.0, loss, None,
+                             gh, None, side)
+        launches[0] += n + tts.tts_last_launch_count(ctx)
+        tts.tts_wait_step(ctx, main)
+        cur[0] ^= 1
+
+    side.wait_stream(main)
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    launches[0] = 0
+    sampler = ClockSampler(0)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(side)
+    for _ in range(args.steps):
+        step()
+    e1.record(side)
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms_step = e0.elapsed_time(e1) / args.steps
+    # end to end through host buffers
+    ht, hh = case["teacher"], case["h"]
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    pt, ph, ptok, ppw = pin(ht), pin(hh), pin(case["draft_tokens"]), pin(case["pos_weight"])
+    hloss, htau, hmask = torch.zeros(1).pin_memory(), torch.zeros(T // C, dtype=torch.int32).pin_memory(), torch.zeros(T, dtype=torch.uint8).pin_memory()
+    for _ in range(3):
+        tts.tts_round_host(ctx, pt, ph, ptok, ppw, T, 1.0, W[cur[0]], W[1 - cur[0]], None, None, None, gh, hloss, htau, hmask, side)
+        cur[0] ^= 1
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        tts.tts_round_host(ctx, pt, ph, ptok, ppw, T, 1.0, W[cur[0]], W[1 - cur[0]], None, None, None, gh, hloss, htau, hmask, side)
+        cur[0] ^= 1
+    dt = time.perf_counter() - t0
+    tts.tts_ctx_destroy(ctx)
+    # the oracle on the whole problem
+    from oracle import tts_oracle as O
+    def oracle_step():
+        m_, _, _ = O.accept_mask(case["teacher"], case["draft_tokens"], C)
+        O.distill_step(case["teacher"], case["h"], case["W"], None, None, None, case["pos_weight"], m_, seg_len=C,
+                       loss_scale=1.0, optimizer="sgd", lr=c["lr"])
+    oracle_step()
+    t0 = time.perf_counter()
+    for _ in range(20):
+        oracle_step()
+    osec = (time.perf_counter() - t0) / 20
+    step_bytes = V * d * (4 + 4 + 4) + T * V * 4 + T * d * 8
+    peak, peak_src = measured_peaks()
+    ach = step_bytes / (ms_step * 1e-3) / 1e9
+    line = {"metric": "distill_steps_per_sec", "value": 1e3 / ms_step, "unit": "steps/s", "n_gpus": 1, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": "BASELINE.json configs[0] tiny_fp32: V=1024 d=64 T=8, fp32 throughout, plain SGD lr=1e-3",
+                       "V": V, "d": d, "T": T, "optimizer": "sgd", "parallelism": "single GPU", "kernel_path": "cuda-core",
+                       "l2": "786 KB of state: L2-resident, the step is launch-latency-bound"},
+            "rows_V_per_sec": 1e3 / ms_step * T * V, "loss": float(loss.item()), "clocks": clocks,
+            "e2e": {"value": args.steps / dt, "unit": "steps/s", "h2d_bytes_per_step": int(pt.numel() * 4 + ph.numel() * 4 + T * 8),
+                    "d2h_bytes_per_step": int(4 + T // C * 4 + T),
+                    "timing": "host clock around K tts_round_host calls (each ends with a stream synchronise)"},
+            "gpu_launches": launches[0],
+            "roofline": {"bound": "hbm", "kernel": "whole step (latency-bound: %d launches of CUDA-core kernels over 786 KB)" % (launches[0] // max(args.steps, 1)),
+                         "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None, "peak_source": peak_src,
+                         "algorithmic_bytes_per_launch": step_bytes, "kernel_ms": ms_step},
+            "cpu_baseline": {"value": 1.0 / osec, "unit": "steps/s", "cores": cpu_threads(), "kind": "oracle",
+                             "sample": "the whole configuration (V=1024, d=64, T=8): %.2f ms per oracle step" % (osec * 1e3)}}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     args = parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -558,6 +655,9 @@ def main():
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
         run_reference(args, rank, world)
+    elif args.config == 1:
+        if rank == 0:
+            run_tiny(args)
     else:
         run_ours(args, rank, world, local_rank)
 
