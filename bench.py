@@ -601,6 +601,28 @@ def run_tiny(args):
     torch.cuda.synchronize()
     clocks = sampler.stop()
     ms_step = e0.elapsed_time(e1) / args.steps
+    # the same steps replayed from CUDA graphs (one per parity of the W double buffer): at 786 KB the step is nothing
+    # but launch latency, which is what capture removes (include/tts.h "CUDA-graph capture")
+    graphs = []
+    for parity in (0, 1):
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side):
+            tts.tts_accept_mask(ctx, teacher, tok, T, mask, tau, None, side)
+            tts.tts_distill_step(ctx, teacher, h, W[parity], W[1 - parity], None, None, None, pw, mask, T, 1.0, loss, None,
+                                 gh, None, side)
+        graphs.append(g)
+    with torch.cuda.stream(side):
+        for i in range(4):
+            graphs[(cur[0] + i) & 1].replay()
+        torch.cuda.synchronize()
+        e0.record(side)
+        for i in range(args.steps):
+            graphs[(cur[0] + i) & 1].replay()
+        e1.record(side)
+    tts.tts_record_done(ctx, side)
+    torch.cuda.synchronize()
+    cur[0] = (cur[0] + 4 + args.steps) & 1
+    ms_graph = e0.elapsed_time(e1) / args.steps
     # end to end through host buffers
     ht, hh = case["teacher"], case["h"]
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
@@ -636,6 +658,7 @@ def run_tiny(args):
                        "V": V, "d": d, "T": T, "optimizer": "sgd", "parallelism": "single GPU", "kernel_path": "cuda-core",
                        "l2": "786 KB of state: L2-resident, the step is launch-latency-bound"},
             "rows_V_per_sec": 1e3 / ms_step * T * V, "loss": float(loss.item()), "clocks": clocks,
+            "graph_replay_ms_per_step": ms_graph,
             "e2e": {"value": args.steps / dt, "unit": "steps/s", "h2d_bytes_per_step": int(pt.numel() * 4 + ph.numel() * 4 + T * 8),
                     "d2h_bytes_per_step": int(4 + T // C * 4 + T),
                     "timing": "host clock around K tts_round_host calls (each ends with a stream synchronise)"},
