@@ -98,7 +98,7 @@ int32_t tts_ctx_create(const tts_config* cfg, int32_t device, tts_ctx** out) {
   ok = ok && dmalloc(&c->step_scalars, 2) == cudaSuccess;
   ok = ok && cudaMemset(c->step_count_dev, 0, sizeof(unsigned long long)) == cudaSuccess;
   ok = ok && dmalloc(&c->z, Tp * V) == cudaSuccess;
-  ok = ok && dmalloc(&c->dl32, Tm * V) == cudaSuccess;
+  if (!c->tensor_ok) ok = ok && dmalloc(&c->dl32, Tm * V) == cudaSuccess;   // fp32 dlogits: CUDA-core kernels only
   ok = ok && dmalloc(&c->stat_part, Tm * tts::kStatSplitsMax * tts::kStatFields) == cudaSuccess;
   ok = ok && dmalloc(&c->row_stats, tts::kRowStatFields * Tm) == cudaSuccess;
   ok = ok && dmalloc(&c->arg_val, Tm * tts::kArgSplitsMax) == cudaSuccess;

@@ -130,7 +130,6 @@ cudaError_t launch_row_stats_merge_shards(tts_ctx* c, const StepArgs& a, const f
 enum { kPhaseAll = 0, kPhaseBegin = 1, kPhaseFinish = 2 };
 // tts_simt.cu
 cudaError_t simt_step(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches);
-cudaError_t simt_launch_gh(tts_ctx* c, const StepArgs& a, const float* dl32, cudaStream_t s, int* launches);
 // tts_tc.cu
 bool tc_supported(const tts_config& cfg);
 cudaError_t tc_init(tts_ctx* c);

@@ -226,25 +226,6 @@ static cudaError_t simt_step_t(tts_ctx* c, const StepArgs& a, cudaStream_t s, in
   return cudaGetLastError();
 }
 
-// Stand-alone launcher kept for shapes the tensor path has no gh kernel for.
-cudaError_t simt_launch_gh(tts_ctx* c, const StepArgs& a, const float* dl32, cudaStream_t s, int* launches) {
-  const int V = c->cfg.V, d = c->cfg.d, T = a.T;
-  cudaError_t e;
-  if ((e = cudaMemsetAsync(a.gh_out, 0, (size_t)T * d * sizeof(float), s)) != cudaSuccess) return e;
-  const int jb = (d + 127) / 128, rb = (T + 15) / 16;
-  int vs = max(1, (4 * c->sm_count) / (jb * rb));
-  int vchunk = ((V + vs - 1) / vs + 63) / 64 * 64;
-  vs = (V + vchunk - 1) / vchunk;
-  if (c->cfg.param_dtype == TTS_BF16)
-    simt_gh_kernel<__nv_bfloat16><<<dim3(jb, vs, rb), 128, 0, s>>>(dl32, static_cast<const __nv_bfloat16*>(a.W_in), T,
-                                                                   V, d, vchunk, a.gh_out);
-  else
-    simt_gh_kernel<float><<<dim3(jb, vs, rb), 128, 0, s>>>(dl32, static_cast<const float*>(a.W_in), T, V, d, vchunk,
-                                                           a.gh_out);
-  *launches += 1;
-  return cudaGetLastError();
-}
-
 cudaError_t simt_step(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches) {
   if (c->cfg.param_dtype == TTS_BF16) return simt_step_t<__nv_bfloat16>(c, a, s, launches);
   return simt_step_t<float>(c, a, s, launches);
