@@ -77,18 +77,43 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
   return *reinterpret_cast<const uint32_t*>(&p);
 }
 
-// CTA b owns stripe b % n_stripes and every `peers`-th band of 16 vocabulary rows of it.
+// The bands of this CTA, as at most two segments (stripe, first band, step, count).
+//   grid % n_stripes == 0 (configs 2, 3: 148 = 4 x 37): CTA b owns stripe b % n_stripes and every peers-th band of it.
+//   otherwise (d = 5120: 5 stripes over 148 CTAs would be 30 / 29 peers; any SM budget): the n_stripes x n_bands units,
+//   stripe-major, are cut into gridDim equal contiguous ranges; grid >= n_stripes, so a range spans at most two
+//   stripes.  A CTA that crosses re-loads h^T into tensor memory and flushes its gh accumulators once more.
+struct Seg {
+  int stripe, first, step, n;
+};
 struct Walk {
-  int stripe, first_band, peers, n_my;
-  __device__ Walk(int b, int grid, int n_stripes, int n_bands) {
-    stripe = b % n_stripes;
-    first_band = b / n_stripes;
-    peers = (grid - stripe + n_stripes - 1) / n_stripes;   // CTAs with this stripe
-    n_my = first_band < n_bands ? (n_bands - first_band + peers - 1) / peers : 0;
+  Seg s0, s1;      // scalars, selected with seg(): an indexed array would live in local memory
+  int n_seg, n_my;
+  __device__ Walk(int b, int grid, int n_stripes, int n_bands) : s0{0, 0, 1, 0}, s1{0, 0, 1, 0}, n_seg(0), n_my(0) {
+    if (grid % n_stripes == 0) {
+      const int peers = grid / n_stripes, first = b / n_stripes;
+      const int n = first < n_bands ? (n_bands - first + peers - 1) / peers : 0;
+      if (n > 0) { s0 = Seg{b % n_stripes, first, peers, n}; n_seg = 1; n_my = n; }
+    } else {
+      const long U = (long)n_stripes * n_bands;
+      const long u0 = U * b / grid, u1 = U * (b + 1) / grid;
+      if (u0 < u1) {
+        const int st = (int)(u0 / n_bands);
+        const long end = u1 < (long)(st + 1) * n_bands ? u1 : (long)(st + 1) * n_bands;
+        s0 = Seg{st, (int)(u0 - (long)st * n_bands), 1, (int)(end - u0)};
+        n_seg = 1;
+        if (end < u1) { s1 = Seg{st + 1, 0, 1, (int)(u1 - end)}; n_seg = 2; }
+        n_my = (int)(u1 - u0);
+      }
+    }
   }
+  template <bool SK>
+  __device__ __forceinline__ Seg seg(int sg) const { return (!SK || sg == 0) ? s0 : s1; }
+  template <bool SK>
+  __device__ __forceinline__ int segs() const { return SK ? n_seg : (n_seg > 0 ? 1 : 0); }
 };
 
-template <bool ADAM>
+// SK: the stream-K walk (up to two segments); false: one segment, known at compile time (grid % n_stripes == 0)
+template <bool ADAM, bool SK>
 __global__ void __launch_bounds__(kThreads, 1)
 tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_constant__ CUtensorMap tm_m,
                     const __grid_constant__ CUtensorMap tm_v, const __grid_constant__ CUtensorMap tm_wout,
@@ -111,12 +136,12 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
   uint64_t* wt_full = h_full + 1;              // [1]
   uint64_t* wt_empty = wt_full + 1;            // [1]
   uint64_t* gh_full = wt_empty + 1;            // [1]
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(gh_full + 1);
+  uint64_t* gh_empty = gh_full + 1;            // [1]
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(gh_empty + 1);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const bool do_gh = p.gh != nullptr;
   const Walk w(blockIdx.x, gridDim.x, p.n_stripes, p.V / kTV);
-  const int j_stripe = w.stripe * kSW;
 
   if (warp == 0 && lane == 0) {
     ptx::prefetch_tensormap(&tm_master);
@@ -131,6 +156,7 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
     ptx::mbar_init(wt_full, 8);
     ptx::mbar_init(wt_empty, 1);
     ptx::mbar_init(gh_full, 1);
+    ptx::mbar_init(gh_empty, 4);
     ptx::fence_barrier_init();
   }
   if (warp == 2) {
@@ -146,8 +172,11 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
     // ===== optimiser-state producer: [2 v x 1024 j] of master / m / v per stage, 4 boxes of [256 x 2] each =====
     if (lane == 0) {
       uint32_t n = 0;
-      for (int i = 0; i < w.n_my; ++i) {
-        const int v0 = (w.first_band + i * w.peers) * kTV;
+      for (int sg = 0; sg < w.template segs<SK>(); ++sg) {
+      const Seg cs = w.template seg<SK>(sg);
+      const int j_stripe = cs.stripe * kSW;
+      for (int k = 0; k < cs.n; ++k) {
+        const int v0 = (cs.first + k * cs.step) * kTV;
         for (int sub = 0; sub < kSubs; ++sub, ++n) {
           const int s = n % kStages;
           ptx::mbar_wait(&st_empty[s], ((n / kStages) & 1) ^ 1);
@@ -165,24 +194,28 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
           }
         }
       }
+      }   // segments
     }
   } else if (warp == 3) {
-    // ===== operand loads: the stripe's h^T tiles once, then one 1 KB dl tile per band =====
+    // ===== operand loads: one 1 KB dl tile per band =====
     if (lane == 0 && w.n_my > 0) {
-      for (int i = 0; i < w.n_my; ++i) {
-        const int band = w.first_band + i * w.peers;
+      int i = 0;
+      for (int sg = 0; sg < w.template segs<SK>(); ++sg) {
+      const Seg cs = w.template seg<SK>(sg);
+      for (int k = 0; k < cs.n; ++k, ++i) {
+        const int band = cs.first + k * cs.step;
         const int s = i % kOpStages;
         ptx::mbar_wait(&op_empty[s], ((i / kOpStages) & 1) ^ 1);
         ptx::mbar_expect_tx(&op_full[s], kDlBytes);
         ptx::bulk_load_1d(dl + s * kDlBytes, p.dlC + (size_t)band * (kDlBytes / 2), kDlBytes, &op_full[s]);
       }
+      }   // segments
     }
   } else if (warp == 1) {
     // ===== MMA issuer =====
     if (lane == 0 && w.n_my > 0) {
       constexpr uint32_t idesc_gw = ptx::make_idesc_bf16(kMJ, kTV, 0, 1);    // A = h^T K-major, B = dl MN-major
       constexpr uint32_t idesc_gh = ptx::make_idesc_bf16(kMJ, kT16, 0, 0);   // A = W^T K-major, B = dl K-major
-      ptx::mbar_wait(h_full, 0);
       // acc[jb][j, v] = sum_r h^T[j, r] (dl_hi + dl_lo)[r, v]
       auto issue_gw = [&](int i) {
         const int ab = i & 1, s = i % kOpStages;
@@ -200,15 +233,25 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
         }
         ptx::mma_commit(&acc_full[ab]);
       };
-      if (!do_gh) {
-        for (int i = 0; i < w.n_my; ++i) {
-          issue_gw(i);
-          ptx::mma_commit(&op_empty[i % kOpStages]);
+      int i = 0;   // bands issued so far (ring and accumulator phases run on over the segments)
+      for (int sg = 0; sg < w.template segs<SK>(); ++sg) {
+        const int n = w.template seg<SK>(sg).n;
+        ptx::mbar_wait(h_full, sg & 1);          // this segment's h^T is in tensor memory
+        ptx::tc_fence_after();
+        if (!do_gh) {
+          for (int k = 0; k < n; ++k, ++i) {
+            issue_gw(i);
+            ptx::mma_commit(&op_empty[i % kOpStages]);
+          }
+          continue;
         }
-      } else {
-        issue_gw(0);
-        for (int i = 0; i < w.n_my; ++i) {
-          if (i + 1 < w.n_my) issue_gw(i + 1);
+        if (sg > 0) {                            // the previous segment's gh accumulators have been flushed
+          ptx::mbar_wait(gh_empty, (sg - 1) & 1);
+          ptx::tc_fence_after();
+        }
+        issue_gw(i);
+        for (int k = 0; k < n; ++k, ++i) {
+          if (k + 1 < n) issue_gw(i + 1);
           // the epilogue has re-derived the whole [16 v x 1024 j] bf16 tile of W_in
           ptx::mbar_wait(wt_full, i & 1);
           ptx::tc_fence_after();
@@ -219,7 +262,7 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
             for (int pl = 0; pl < 2; ++pl) {
               // B: K-major, no swizzle: the same core matrices; v-groups 128 B apart (LBO), r-groups 256 B (SBO)
               const uint64_t bd = ptx::make_smem_desc(b0 + pl * 512, 128, 256, 0);
-              ptx::mma_f16_ss(tmem_base + kGhCol0 + jb * kT16, ad, bd, idesc_gh, (i > 0) | pl);
+              ptx::mma_f16_ss(tmem_base + kGhCol0 + jb * kT16, ad, bd, idesc_gh, (k > 0) | pl);
             }
           }
           ptx::mma_commit(wt_empty);
@@ -239,9 +282,13 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
     uint8_t* wt_thr = wt + (jj >> 3) * 128 + (jj & 7) * 16;   // + jb * 4096 + (v >> 3) * 2048 + (v & 7) * 2
     __nv_bfloat16* wo_g = reinterpret_cast<__nv_bfloat16*>(wo + g * kWoBytes);
     int prev_s = -1;                           // stage whose stores this group issued last
-    if (w.n_my > 0) {
-      // the stripe's h^T operand -> tensor memory, once per kernel: hTc row j holds h[0..16, j] (32 bytes); this
-      // group writes four of the eight 128-column blocks
+    int i = 0;   // bands processed so far
+    for (int sg = 0; sg < w.template segs<SK>(); ++sg) {
+    const Seg cs = w.template seg<SK>(sg);
+    const int j_stripe = cs.stripe * kSW;
+    {
+      // the segment's h^T operand -> tensor memory: hTc row j holds h[0..16, j] (32 bytes); this group writes four of
+      // the eight 128-column blocks.  (Every gW MMA of the previous segment is complete: its accumulators were read.)
       for (int jb = 4 * g; jb < 4 * g + 4; ++jb) {
         const uint4* row = reinterpret_cast<const uint4*>(p.hTc + (size_t)(j_stripe + jb * kMJ + jj) * kT16);
         const uint4 lo = __ldg(row), hi = __ldg(row + 1);
@@ -253,8 +300,8 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
       __syncwarp();
       if (lane == 0) ptx::mbar_arrive(h_full);
     }
-    for (int i = 0; i < w.n_my; ++i) {
-      const int v0 = (w.first_band + i * w.peers) * kTV;
+    for (int k = 0; k < cs.n; ++k, ++i) {
+      const int v0 = (cs.first + k * cs.step) * kTV;
       const int ab = i & 1;
       ptx::mbar_wait(&acc_full[ab], (i >> 1) & 1);
       ptx::tc_fence_after();
@@ -351,10 +398,9 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
       __syncwarp();
       if (lane == 0) ptx::mbar_arrive(&acc_empty[ab]);
     }
-    if (leader) ptx::bulk_wait_group_read<0>();   // shared memory must outlive the last stores' reads
-    // ===== gh flush: the stripe's persistent accumulators -> fp32 atomics (group 0: one warp per lane quarter) =====
-    if (do_gh && g == 0 && w.n_my > 0) {
-      ptx::mbar_wait(gh_full, 0);
+    // ===== gh flush: the segment's accumulators -> fp32 atomics (group 0: one warp per lane quarter) =====
+    if (do_gh && g == 0) {
+      ptx::mbar_wait(gh_full, sg & 1);
       ptx::tc_fence_after();
       for (int jb = 0; jb < kJB; ++jb) {
         float* gc = p.gh + j_stripe + jb * kMJ + jj;
@@ -362,10 +408,15 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
         ptx::tmem_ld_32x32b_x16(tmem_base + kGhCol0 + jb * kT16 + (static_cast<uint32_t>(q * 32) << 16), r);
         ptx::tmem_ld_wait();
 #pragma unroll
-        for (int k = 0; k < 16; ++k)
-          if (k < p.T) atomicAdd(gc + (size_t)k * p.d, __uint_as_float(r[k]));
+        for (int kk = 0; kk < 16; ++kk)
+          if (kk < p.T) atomicAdd(gc + (size_t)kk * p.d, __uint_as_float(r[kk]));
       }
+      ptx::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(gh_empty);   // the next segment may overwrite the accumulators
     }
+    }   // segments
+    if (leader) ptx::bulk_wait_group_read<0>();   // shared memory must outlive the last stores' reads
   }
   ptx::tc_fence_before();
   __syncthreads();
@@ -439,10 +490,16 @@ cudaError_t tc_fused_init(tts_ctx* c) {
   if ((e = cudaMalloc(&st->hTc, (size_t)c->cfg.d * kT16 * 2)) != cudaSuccess) return e;
   if ((e = cudaMalloc(&st->dlC, (size_t)c->cfg.V * 2 * kT16 * 2)) != cudaSuccess) return e;
   const int smem = (int)fused_smem();
-  if ((e = cudaFuncSetAttribute(tc_update_gh_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) !=
+  if ((e = cudaFuncSetAttribute(tc_update_gh_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) !=
       cudaSuccess)
     return e;
-  return cudaFuncSetAttribute(tc_update_gh_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  if ((e = cudaFuncSetAttribute(tc_update_gh_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) !=
+      cudaSuccess)
+    return e;
+  if ((e = cudaFuncSetAttribute(tc_update_gh_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) !=
+      cudaSuccess)
+    return e;
+  return cudaFuncSetAttribute(tc_update_gh_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
 }
 
 // Grid of the fused pass, 0 when the shape does not qualify (T > 16 rows, d or V not a multiple of the tile, or an
@@ -506,10 +563,14 @@ cudaError_t tc_launch_update_fused(tts_ctx* c, const StepArgs& a, int grid, cuda
   p.decay = 1.f - a.lr * a.wd;
   p.step_scalars = a.step_scalars;
   const size_t smem = fused_smem();
-  if (adam)
-    tc_update_gh_kernel<true><<<grid, kThreads, smem, s>>>(tm_master, tm_m, tm_v, tm_wout, p);
-  else
-    tc_update_gh_kernel<false><<<grid, kThreads, smem, s>>>(tm_master, tm_m, tm_v, tm_wout, p);
+  const bool sk = grid % p.n_stripes != 0;
+  if (adam) {
+    if (sk) tc_update_gh_kernel<true, true><<<grid, kThreads, smem, s>>>(tm_master, tm_m, tm_v, tm_wout, p);
+    else tc_update_gh_kernel<true, false><<<grid, kThreads, smem, s>>>(tm_master, tm_m, tm_v, tm_wout, p);
+  } else {
+    if (sk) tc_update_gh_kernel<false, true><<<grid, kThreads, smem, s>>>(tm_master, tm_m, tm_v, tm_wout, p);
+    else tc_update_gh_kernel<false, false><<<grid, kThreads, smem, s>>>(tm_master, tm_m, tm_v, tm_wout, p);
+  }
   *launches += 1;
   return cudaGetLastError();
 }
