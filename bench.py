@@ -57,6 +57,9 @@ def parse_args():
                     help="N > 1: independent replicas of the step (weak scaling, no data-path collective), or ONE step "
                          "sharded over the vocabulary (strong scaling; SURVEY 8(e): all-gather of [T,8] row tuples and "
                          "all-reduce of gh [T,d] per step over NCCL)")
+    ap.add_argument("--n-seq", type=int, default=0,
+                    help="override the number of concurrent sequences (rows = 16 x n_seq <= 512): the T-scaling of the "
+                         "batched shape between BASELINE configs[2] (1 sequence) and configs[3] (32)")
     ap.add_argument("--max-ctas", type=int, default=0,
                     help="SM budget of the step's persistent kernels (tts_config.max_ctas; 0 = all SMs): what the main "
                          "stream keeps while the update overlaps it (PAPER.md:426)")
@@ -275,7 +278,7 @@ def run_ours(args, rank, world, local_rank):
         case = synth.make_case_device(args.config, dev, seed_offset=rank, V=v1 - v0, shared_h=True)
         dist.broadcast(case["draft_tokens"], 0)      # replicated inputs: canvas tokens (global ids), h, pos_weight
     else:
-        case = synth.make_case_device(args.config, dev, seed_offset=rank)
+        case = synth.make_case_device(args.config, dev, seed_offset=rank, n_seq=args.n_seq or None)
     c = case["cfg"]
     V, d, T, C = case["V"], case["d"], case["T"], case["seg_len"]
     kpath = tts.TTS_PATH_AUTO if args.kernel_path == "auto" else tts.TTS_PATH_SIMT
@@ -416,7 +419,7 @@ def run_ours(args, rank, world, local_rank):
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
             "scaling": "strong" if vocab else "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
             "config": dict(workload_config(args.config, world, "tcgen05+tma" if used_tensor else "cuda-core",
-                                           args.parallelism),
+                                           args.parallelism), **({"T": T, "n_seq_override": args.n_seq} if args.n_seq else {}),
                            draft_logits=args.draft_logits),
             "rows_V_per_sec": sps * T * V, "loss": loss_val, "clocks": clocks, "e2e": e2e,
             "gpu_launches": launches[0], "roofline": roof, "cpu_baseline": cpu}
