@@ -93,7 +93,7 @@ cudaError_t tc_step(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches
   if ((e = tc_launch_prep_wide(c, a, z, s, launches)) != cudaSuccess) return e;
   prof_mark(c, 2, s);
   // a5: gh on tcgen05 (reads W_in before the update may overwrite an aliased W_out)
-  if (a.gh_out) {
+  if (a.gh_out && !tc_wide_fuses_gh(T16)) {
     if ((e = tc_launch_gh(c, a, s, launches)) != cudaSuccess) return e;
   }
   prof_mark(c, 3, s);

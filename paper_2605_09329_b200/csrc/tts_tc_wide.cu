@@ -44,11 +44,16 @@ constexpr int kWOpStagesMax = 4;         // dl band ring (depth chosen per launc
 constexpr int kWSmemBudget = 225 * 1024;
 constexpr int kWAccCols = 64;            // TMEM columns reserved for the two gW accumulators (NV <= 32)
 constexpr long kWWindowBytes = 12l << 20;
+constexpr int kWGhCol0 = 192;            // GH: first TMEM column of the gh accumulators (h^T ends at 64 + 96 = 160)
+constexpr int kWGhMaxN = 192;            // GH: most canvas rows (x dl planes) whose gh accumulators fit next to h^T
+constexpr int kWWtBytes = kWJ * 32 * 2;  // GH: the band's W^T tile [128 j x 32 v] fp16 (A operand of gh), 8 KB
 
 struct WideParams {
   float* gW_debug;
   const uint16_t* hTT;        // [d, Kp] fp16 bits
   const float* dl_scale;      // {S, 1 / S, S_h, 1 / S_h}
+  float* gh;                  // GH: [T, d] fp32, zeroed; this kernel adds its parts with fp32 RED
+  int T, T16, planes;         // GH: rows, padded rows, dl planes stacked along K (the gh accumulators have planes * T16 columns)
   int V, d, Kp;
   int n_stripes, n_bands, n_win, stages, op_stages;
   const float* step_scalars;  // device {1 / (1 - b1^n), 1 / sqrt(1 - b2^n)} of this step
@@ -63,6 +68,7 @@ struct WideBars {
   uint64_t acc_full[2];
   uint64_t acc_empty[2];
   uint64_t a_full;
+  uint64_t wt_full, wt_empty, gh_full, gh_empty;   // GH
   uint32_t tmem_slot;
 };
 
@@ -97,7 +103,12 @@ constexpr uint32_t kDescHiSw128 = (1024u >> 4) | (1u << 14) | (ptx::kSwizzle128B
 __device__ __forceinline__ uint32_t desc_lo_sw128(uint32_t smem_addr) { return ((smem_addr >> 4) & 0x3FFFu) | (1u << 16); }
 __device__ __forceinline__ uint64_t desc64(uint32_t hi, uint32_t lo) { return (static_cast<uint64_t>(hi) << 32) | lo; }
 
-template <bool ADAM, int NV>
+// GH (planes * T16 <= 192): gh^T[j, r] += W_in[v, j] dl[r, v] is formed here as well, as in the one-canvas kernel: the
+// band's W_in tile is re-derived from the master values the epilogue holds (precondition W_in == rn_bf16(W_master)),
+// written to shared memory as fp16(16 W) (the A operand), the dl band already in shared memory is read a second
+// time as the MN-major B operand, and the stripe's accumulators [128 j x planes T16] persist in tensor memory until
+// the CTA leaves the stripe.  No gh kernel, no second pass over W.
+template <bool ADAM, int NV, bool GH>
 __global__ void __launch_bounds__(kWThreads, 1)
 tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
                       const __grid_constant__ CUtensorMap tm_master, const __grid_constant__ CUtensorMap tm_m,
@@ -111,7 +122,8 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
   const int kWOpStages = p.op_stages;
   uint8_t* st = sB + kWOpStages * b_bytes;             // [stages][3][8 v][128 j] fp32
   uint8_t* wo = st + p.stages * kWStageBytes;          // [2 groups][8 v][128 j] bf16
-  WideBars* bars = reinterpret_cast<WideBars*>(wo + 2 * kWWoBytes);
+  uint8_t* wt = wo + 2 * kWWoBytes;                    // GH: [4 v-groups][16 j-groups][8 j][8 v] fp16, K-major core matrices
+  WideBars* bars = reinterpret_cast<WideBars*>(wt + (GH ? kWWtBytes : 0));
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int nks = p.Kp / 16;                           // MMA K steps per band
@@ -129,6 +141,10 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
     for (int i = 0; i < kWOpStages; ++i) { ptx::mbar_init(&bars->op_full[i], 1); ptx::mbar_init(&bars->op_empty[i], 1); }
     for (int i = 0; i < 2; ++i) { ptx::mbar_init(&bars->acc_full[i], 1); ptx::mbar_init(&bars->acc_empty[i], 8); }
     ptx::mbar_init(&bars->a_full, 8);
+    ptx::mbar_init(&bars->wt_full, 8);
+    ptx::mbar_init(&bars->wt_empty, 1);
+    ptx::mbar_init(&bars->gh_full, 1);
+    ptx::mbar_init(&bars->gh_empty, 4);
     ptx::fence_barrier_init();
   }
   if (warp == 2) {
@@ -188,10 +204,44 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
       WideWalk w(p);
       uint32_t i = 0, a_n = 0;
       int stripe, band, cur = -1;
+      // GH: gh MMAs of band i are issued after the gW MMAs of band i + 1 (the epilogue produces their A operand while
+      // it drains band i's accumulator), and before the CTA leaves a stripe
+      const int n_gh = p.planes * p.T16;
+      const uint32_t idesc_gh = ptx::make_idesc_f16(kWJ, n_gh, ptx::kFmtF16, ptx::kFmtF16, 0, 1);   // A K-major, B MN-major
+      const uint32_t wt0 = ptx::smem_u32(wt);
+      bool pending = false, first_gh = true;
+      uint32_t i_prev = 0;
+      auto issue_gh = [&]() {
+        ptx::mbar_wait(&bars->wt_full, i_prev & 1);
+        ptx::tc_fence_after();
+        const uint32_t b_base = sB0 + (i_prev % kWOpStages) * b_bytes;
+#pragma unroll
+        for (int ks = 0; ks < NV / 16; ++ks) {
+          // A: W^T tile, K-major, no swizzle: core matrices [8 j x 8 v]; j-groups 128 B apart (SBO), v-groups 2 KB (LBO)
+          const uint64_t ad = ptx::make_smem_desc(wt0 + ks * 4096, 2048, 128, 0);
+          // B: the dl band read MN-major (N = canvas row, contiguous in the 128-byte rows; K = vocabulary row):
+          // 16 k rows = 2 KB per step, 8-row groups 1 KB apart (SBO), 64-row blocks of N one K chunk apart (LBO)
+          const uint64_t bd = ptx::make_smem_desc(b_base + ks * 2048, NV * 128, 1024, ptx::kSwizzle128B);
+          ptx::mma_f16_ss(tmem_base + kWGhCol0, ad, bd, idesc_gh, (first_gh ? 0u : 1u) | ks);
+        }
+        first_gh = false;
+        ptx::mma_commit(&bars->wt_empty);
+        ptx::mma_commit(&bars->op_empty[i_prev % kWOpStages]);
+        pending = false;
+      };
       while (w.get(stripe, band)) {
         if (stripe != cur) {
+          if (GH && cur >= 0) {
+            if (pending) issue_gh();
+            ptx::mma_commit(&bars->gh_full);             // the old stripe's accumulators are complete
+          }
           ptx::mbar_wait(&bars->a_full, a_n & 1);
           ptx::tc_fence_after();
+          if (GH && cur >= 0) {                          // ... and flushed: the new stripe starts from zero
+            ptx::mbar_wait(&bars->gh_empty, (a_n - 1) & 1);
+            ptx::tc_fence_after();
+            first_gh = true;
+          }
           ++a_n;
           cur = stripe;
         }
@@ -205,9 +255,18 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
           const uint32_t b_lo = desc_lo_sw128(b_base + (ks >> 2) * (NV * 128)) + 2 * (ks & 3);
           ptx::mma_f16_ts(d_tmem, tmem_A + ks * 8, desc64(kDescHiSw128, b_lo), idesc, ks);
         }
-        ptx::mma_commit(&bars->op_empty[s]);
+        if (!GH) ptx::mma_commit(&bars->op_empty[s]);
         ptx::mma_commit(&bars->acc_full[ab]);
+        if (GH) {
+          if (pending) issue_gh();
+          i_prev = i;
+          pending = true;
+        }
         ++i;
+      }
+      if (GH && cur >= 0) {
+        if (pending) issue_gh();
+        ptx::mma_commit(&bars->gh_full);
       }
     }
   } else if (warp >= 4) {
@@ -220,11 +279,38 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
     const float inv_s = p.dl_scale[1] * p.dl_scale[3];
     const float c1 = ADAM ? p.lr * p.step_scalars[0] : 0.f, inv_sqrt_bc2 = ADAM ? p.step_scalars[1] : 0.f;
     WideWalk w(p);
-    uint32_t i = 0;
+    uint32_t i = 0, n_flush = 0;
     int stripe, band, cur = -1, prev_s = -1;
+    uint8_t* wt_thr = wt + (jj >> 3) * 128 + (jj & 7) * 16;   // + (v >> 3) * 2048: this thread's 16-byte chunk of 8 v
+    // GH: the stripe's gh accumulators -> fp32 RED (group 0: one warp per lane quarter), then the issuer may reuse them
+    auto flush_gh = [&](int stripe_done) {
+      if (g != 0) return;
+      ptx::mbar_wait(&bars->gh_full, n_flush & 1);
+      ptx::tc_fence_after();
+      const float inv_gh = p.dl_scale[1] * (1.f / 16.f);
+      float* gc = p.gh + stripe_done * kWJ + jj;
+      for (int c0 = 0; c0 < p.T16; c0 += 16) {
+        if (c0 >= p.T) break;
+        uint32_t r[16], r2[16];
+        ptx::tmem_ld_32x32b_x16(tmem_base + kWGhCol0 + c0 + lane_bits, r);
+        if (p.planes == 2) ptx::tmem_ld_32x32b_x16(tmem_base + kWGhCol0 + p.T16 + c0 + lane_bits, r2);
+        ptx::tmem_ld_wait();
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+          float x = __uint_as_float(r[k]);
+          if (p.planes == 2) x += __uint_as_float(r2[k]);
+          if (c0 + k < p.T) atomicAdd(gc + (size_t)(c0 + k) * p.d, x * inv_gh);
+        }
+      }
+      ptx::tc_fence_before();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(&bars->gh_empty);
+      ++n_flush;
+    };
     while (w.get(stripe, band)) {
       const int j0 = stripe * kWJ, v0 = band * NV;
       if (stripe != cur) {
+        if (GH && cur >= 0) flush_gh(cur);
         // every MMA that read the old stripe is complete: this warp has waited on the previous band's acc_full.
         // hTT is tiled [stripe][K step][128 j][16 k]: a warp reads 1 KB contiguous per K step; this group writes
         // half of the K steps.
@@ -266,6 +352,25 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
         for (int r = 0; r < kWSV; ++r) {
           M[r] = sM[r * kWJ];
           if (ADAM) { mm[r] = sM[kWSV * kWJ + r * kWJ]; vv[r] = sM[2 * kWSV * kWJ + r * kWJ]; }
+        }
+        if (GH) {
+          // a5 operand: W_in[v, j] = rn_bf16(master[v, j]), as fp16(16 W): rows 8 sub .. 8 sub + 7 of this thread's column
+          ptx::mbar_wait(&bars->wt_empty, (i & 1) ^ 1);          // the gh MMAs of the previous band have read wt
+          uint32_t pk[4];
+#pragma unroll
+          for (int r = 0; r < 4; ++r) {
+            const __nv_bfloat162 b2 = __floats2bfloat162_rn(M[2 * r], M[2 * r + 1]);       // W_in = rn_bf16(master)
+            const uint32_t bb = *reinterpret_cast<const uint32_t*>(&b2);
+            const float lo = __uint_as_float(bb << 16) * 16.f, hi = __uint_as_float(bb & 0xFFFF0000u) * 16.f;
+            // fp16(16 W), saturating (|W| >= 4094 clamps, as in tts_tc_gemm.cu)
+            asm("cvt.rn.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(pk[r]) : "f"(hi), "f"(lo));
+          }
+          *reinterpret_cast<uint4*>(wt_thr + sub * 2048) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+          if (sub >= kSubs - 2) {                                // the group's last sub-tile of this band
+            ptx::fence_proxy_async_smem();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(&bars->wt_full);
+          }
         }
         ptx::tmem_ld_wait();
         // a7 in place: the thread rewrites exactly the shared-memory words it read
@@ -318,6 +423,7 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
       if (lane == 0) ptx::mbar_arrive(&bars->acc_empty[ab]);
       ++i;
     }
+    if (GH && cur >= 0) flush_gh(cur);
     if (leader) ptx::bulk_wait_group_read<0>();   // shared memory must outlive the last stores' reads
   }
   ptx::tc_fence_before();
@@ -471,18 +577,18 @@ __global__ void __launch_bounds__(256) tc_prep_dl_wide_kernel(const void* __rest
   }
 }
 
-template <bool ADAM, int NV>
+template <bool ADAM, int NV, bool GH>
 cudaError_t launch_wide(int grid, size_t smem, cudaStream_t s, const CUtensorMap& tm_dlT,
                         const CUtensorMap& tm_master, const CUtensorMap& tm_m, const CUtensorMap& tm_v,
                         const CUtensorMap& tm_wout, const WideParams& p) {
-  tc_update_wide_kernel<ADAM, NV><<<grid, kWThreads, smem, s>>>(tm_dlT, tm_master, tm_m, tm_v, tm_wout, p);
+  tc_update_wide_kernel<ADAM, NV, GH><<<grid, kWThreads, smem, s>>>(tm_dlT, tm_master, tm_m, tm_v, tm_wout, p);
   return cudaGetLastError();
 }
 
 
-template <bool ADAM, int NV>
+template <bool ADAM, int NV, bool GH>
 cudaError_t wide_attr() {
-  return cudaFuncSetAttribute(tc_update_wide_kernel<ADAM, NV>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  return cudaFuncSetAttribute(tc_update_wide_kernel<ADAM, NV, GH>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                               kWSmemBudget + 2048);
 }
 
@@ -490,12 +596,21 @@ cudaError_t wide_attr() {
 
 cudaError_t tc_wide_init(tts_ctx*) {
   cudaError_t e;
-  if ((e = wide_attr<true, 32>()) != cudaSuccess) return e;
-  return wide_attr<false, 32>();
+  if ((e = wide_attr<true, 32, false>()) != cudaSuccess) return e;
+  if ((e = wide_attr<false, 32, false>()) != cudaSuccess) return e;
+  if ((e = wide_attr<true, 32, true>()) != cudaSuccess) return e;
+  return wide_attr<false, 32, true>();
 }
 
 // dl planes of the wide path: hi + lo while both fit the 64-wide K chunk (T16 <= 32), one plane beyond
 int tc_wide_planes(int T16) { return 2 * T16 <= kKC ? 2 : 1; }
+
+// 1 when the wide update kernel forms gh itself (its accumulators fit next to h^T in tensor memory)
+int tc_wide_fuses_gh(int T16) {
+  static int off = -1;
+  if (off < 0) { const char* e = getenv("TTS_WIDE_NO_GH"); off = (e && e[0] == '1') ? 1 : 0; }   // measurement switch
+  return !off && tc_wide_planes(T16) * T16 <= kWGhMaxN;
+}
 
 // a4 of the wide path: h^T rows and the fp16 dl planes
 cudaError_t tc_launch_prep_wide(tts_ctx* c, const StepArgs& a, const float* z, cudaStream_t s, int* launches) {
@@ -515,7 +630,8 @@ cudaError_t tc_launch_prep_wide(tts_ctx* c, const StepArgs& a, const float* z, c
   tc_prep_hT_kernel<<<dim3((d + 31) / 32, Kp / 32), 256, 0, s>>>(h, d, T, T16, planes, Kp, absmax,
                                                                   static_cast<uint16_t*>(st->hTT), st->dl_scale);
   uint16_t* dlT = static_cast<uint16_t*>(st->dlT);
-  uint16_t* dlR = a.gh_out ? static_cast<uint16_t*>(st->dlR) : nullptr;
+  // the row-major plane is the gh KERNEL's operand: not needed when the update kernel forms gh itself
+  uint16_t* dlR = (a.gh_out && !tc_wide_fuses_gh(T16)) ? static_cast<uint16_t*>(st->dlR) : nullptr;
   const dim3 grid(V / 128, Kp / 64);
   const bool bf = c->cfg.logits_dtype == TTS_BF16, fast = planes == 1;
   auto kern = bf ? (fast ? tc_prep_dl_wide_kernel<true, true> : tc_prep_dl_wide_kernel<true, false>)
@@ -566,8 +682,13 @@ cudaError_t tc_launch_update_wide(tts_ctx* c, const StepArgs& a, cudaStream_t s,
   p.n_win = (int)((dl_bytes + kWWindowBytes - 1) / kWWindowBytes);
   if (p.n_win < 1) p.n_win = 1;
   if (p.n_win > p.n_bands) p.n_win = p.n_bands;
-  p.op_stages = 2;
-  const int fixed = 1024 + p.op_stages * NV * Kp * 2 + 2 * kWWoBytes + (int)sizeof(WideBars);
+  cudaError_t e;
+  const bool gh_here = a.gh_out != nullptr && tc_wide_fuses_gh(T16);
+  p.gh = gh_here ? a.gh_out : nullptr;
+  p.T = T; p.T16 = T16; p.planes = tc_wide_planes(T16);
+  if (gh_here && (e = cudaMemsetAsync(a.gh_out, 0, (size_t)T * d * sizeof(float), s)) != cudaSuccess) return e;
+  p.op_stages = gh_here ? 3 : 2;   // with gh a band's dl rows stay until the gh MMAs issued one band later have read them
+  const int fixed = 1024 + p.op_stages * NV * Kp * 2 + 2 * kWWoBytes + (gh_here ? kWWtBytes : 0) + (int)sizeof(WideBars);
   p.stages = (kWSmemBudget - fixed) / kWStageBytes;
   if (p.stages > kWMaxStages) p.stages = kWMaxStages;
   if (p.stages < 2) return cudaErrorInvalidConfiguration;
@@ -578,9 +699,12 @@ cudaError_t tc_launch_update_wide(tts_ctx* c, const StepArgs& a, cudaStream_t s,
   int grid = c->cfg.max_ctas > 0 ? c->cfg.max_ctas : c->sm_count;
   if (grid > units) grid = (int)units;
   const size_t smem = (size_t)fixed + (size_t)p.stages * kWStageBytes;
-  cudaError_t e;
-  e = adam ? launch_wide<true, NV>(grid, smem, s, tm_dlT, tm_master, tm_m, tm_v, tm_wout, p)
-           : launch_wide<false, NV>(grid, smem, s, tm_dlT, tm_master, tm_m, tm_v, tm_wout, p);
+  if (gh_here)
+    e = adam ? launch_wide<true, NV, true>(grid, smem, s, tm_dlT, tm_master, tm_m, tm_v, tm_wout, p)
+             : launch_wide<false, NV, true>(grid, smem, s, tm_dlT, tm_master, tm_m, tm_v, tm_wout, p);
+  else
+    e = adam ? launch_wide<true, NV, false>(grid, smem, s, tm_dlT, tm_master, tm_m, tm_v, tm_wout, p)
+             : launch_wide<false, NV, false>(grid, smem, s, tm_dlT, tm_master, tm_m, tm_v, tm_wout, p);
   *launches += 1;
   return e;
 }
