@@ -78,23 +78,31 @@ struct WideBars {
 struct WideWalk {
   int n_stripes, n_bands, n_win;
   int win, wb0, wbn;
-  long u_lo, u_hi, k;      // range [u_lo, u_hi) of the current window, k units of it already handed out
+  int left;            // units of the current window still to hand out
+  int cs, cb, dir;     // next unit: stripe, band within the window, direction (+1 even windows, -1 odd ones)
   __device__ WideWalk(const WideParams& p) : n_stripes(p.n_stripes), n_bands(p.n_bands), n_win(p.n_win), win(-1),
-                                             wb0(0), wbn(1), u_lo(0), u_hi(0), k(0) {}
+                                             wb0(0), wbn(1), left(0), cs(0), cb(0), dir(1) {}
+  // one 64-bit division per window; inside a window the walk is increments only (every role calls this once per band,
+  // the epilogue threads included)
   __device__ bool get(int& stripe, int& band) {
-    while (u_lo + k >= u_hi) {
+    while (left == 0) {
       if (++win >= n_win) return false;
       wb0 = (int)((long)n_bands * win / n_win);
       wbn = (int)((long)n_bands * (win + 1) / n_win) - wb0;
       const long units = (long)n_stripes * wbn;
-      u_lo = units * blockIdx.x / gridDim.x;
-      u_hi = units * (blockIdx.x + 1) / gridDim.x;
-      k = 0;
+      const long u_lo = units * blockIdx.x / gridDim.x, u_hi = units * (blockIdx.x + 1) / gridDim.x;
+      left = (int)(u_hi - u_lo);
+      dir = (win & 1) ? -1 : 1;
+      const long u = dir > 0 ? u_lo : u_hi - 1;
+      cs = (int)(u / wbn);
+      cb = (int)(u - (long)cs * wbn);
     }
-    const long u = (win & 1) ? u_hi - 1 - k : u_lo + k;
-    stripe = (int)(u / wbn);
-    band = wb0 + (int)(u - (long)stripe * wbn);
-    ++k;
+    stripe = cs;
+    band = wb0 + cb;
+    cb += dir;
+    if (cb == wbn) { cb = 0; ++cs; }
+    else if (cb < 0) { cb = wbn - 1; --cs; }
+    --left;
     return true;
   }
 };
