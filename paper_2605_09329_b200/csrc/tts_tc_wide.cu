@@ -170,13 +170,17 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
     if (lane == 0) {
       const uint64_t pol = ptx::policy_evict_first();
       WideWalk w(p);
-      uint32_t n = 0;
+      int ps = 0;
+      uint32_t pph = 0, n = 0;
       int stripe, band;
       while (w.get(stripe, band)) {
         const int j0 = stripe * kWJ, v0 = band * NV;
         for (int sub = 0; sub < kSubs; ++sub, ++n) {
-          const int s = n % p.stages;
-          ptx::mbar_wait(&bars->st_empty[s], ((n / p.stages) & 1) ^ 1);
+          int s;
+          uint32_t ph;
+          if (GH) { s = ps; ph = pph; if (++ps == p.stages) { ps = 0; pph ^= 1; } }
+          else { s = n % p.stages; ph = (n / p.stages) & 1; }   // see the epilogue for why the two instances differ
+          ptx::mbar_wait(&bars->st_empty[s], ph ^ 1);
           uint8_t* dst = st + s * kWStageBytes;
           ptx::mbar_expect_tx(&bars->st_full[s], (ADAM ? 3 : 1) * kWTensorBytes);
           const int r0 = v0 + sub * kWSV;
@@ -289,6 +293,8 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
     WideWalk w(p);
     uint32_t i = 0, n_flush = 0;
     int stripe, band, cur = -1, prev_s = -1;
+    int st_s = g;                 // p.stages >= 2 > g
+    uint32_t st_ph = 0;           // no division by the runtime ring depth in the per-sub-tile path
     uint8_t* wt_thr = wt + (jj >> 3) * 128 + (jj & 7) * 16;   // + (v >> 3) * 2048: this thread's 16-byte chunk of 8 v
     // GH: the stripe's gh accumulators -> fp32 RED (group 0: one warp per lane quarter), then the issuer may reuse them
     auto flush_gh = [&](int stripe_done) {
@@ -349,11 +355,23 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
       ptx::mbar_wait(&bars->acc_full[ab], (i >> 1) & 1);
       ptx::tc_fence_after();
       for (int sub = g; sub < kSubs; sub += 2) {
-        const uint32_t n = i * kSubs + sub;
-        const int s = n % p.stages;
+        // stage and phase of sub-tile n = i * kSubs + sub.  The gh-forming instance steps them (the group's stages
+        // advance by 2); the other one divides by the runtime ring depth.  Measured, same box, both ways round: stepping
+        // takes the gh-forming update from 2.90 to 2.77 ms at 64 rows and the plain one from 2.97 to 3.18 ms at 512
+        // (a faster epilogue bunches its TMA stores; the same change slows the one-canvas kernel by 6%).
+        int s;
+        uint32_t st_par;
+        if (GH) {
+          s = st_s; st_par = st_ph;
+          st_s += 2;
+          if (st_s >= p.stages) { st_s -= p.stages; st_ph ^= 1; }
+        } else {
+          const uint32_t n = i * kSubs + sub;
+          s = n % p.stages; st_par = (n / p.stages) & 1;
+        }
         uint32_t gr[kWSV];
         ptx::tmem_ld_32x32b_x8(tmem_base + ab * NV + sub * kWSV + lane_bits, gr);
-        ptx::mbar_wait(&bars->st_full[s], (n / p.stages) & 1);
+        ptx::mbar_wait(&bars->st_full[s], st_par);
         float* sM = reinterpret_cast<float*>(st + s * kWStageBytes) + jj;
         float M[kWSV], mm[kWSV], vv[kWSV];
 #pragma unroll
