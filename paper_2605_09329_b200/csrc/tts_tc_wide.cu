@@ -358,7 +358,8 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
         // stage and phase of sub-tile n = i * kSubs + sub.  The gh-forming instance steps them (the group's stages
         // advance by 2); the other one divides by the runtime ring depth.  Measured, same box, both ways round: stepping
         // takes the gh-forming update from 2.90 to 2.77 ms at 64 rows and the plain one from 2.97 to 3.18 ms at 512
-        // (a faster epilogue bunches its TMA stores; the same change slows the one-canvas kernel by 6%).
+        // (an explicit delay only slows the kernels, so it is ptxas' schedule of the two codings, not pacing; the same
+        // change slows the one-canvas kernel by 6%).
         int s;
         uint32_t st_par;
         if (GH) {
