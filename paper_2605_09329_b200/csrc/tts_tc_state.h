@@ -53,7 +53,7 @@ cudaError_t tc_launch_update_fused(tts_ctx* c, const StepArgs& a, int grid, cuda
 // tts_tc_wide.cu: a4 operands (h^T rows, fp16 dl planes) and a6 + a7 for T <= 512
 cudaError_t tc_wide_init(tts_ctx* c);
 int tc_wide_planes(int T16);   // 2: dl S = hi + lo (T16 <= 32), 1: one fp16 plane
-int tc_wide_fuses_gh(int T16); // 1: the wide update kernel forms gh itself (planes * T16 <= 192): no gh kernel
+int tc_wide_fuses_gh(int T16); // 1: the wide update kernel forms gh itself (planes * T16 <= 256): no gh kernel
 cudaError_t tc_launch_prep_wide(tts_ctx* c, const StepArgs& a, const float* z, cudaStream_t s, int* launches);
 cudaError_t tc_launch_update_wide(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches);
 

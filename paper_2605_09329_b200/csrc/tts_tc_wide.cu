@@ -44,8 +44,8 @@ constexpr int kWOpStagesMax = 4;         // dl band ring (depth chosen per launc
 constexpr int kWSmemBudget = 225 * 1024;
 constexpr int kWAccCols = 64;            // TMEM columns reserved for the two gW accumulators (NV <= 32)
 constexpr long kWWindowBytes = 12l << 20;
-constexpr int kWGhCol0 = 192;            // GH: first TMEM column of the gh accumulators (h^T ends at 64 + 96 = 160)
-constexpr int kWGhMaxN = 192;            // GH: most canvas rows (x dl planes) whose gh accumulators fit next to h^T
+constexpr int kWGhCol0 = 192;            // GH: first TMEM column of the gh accumulators (h^T ends at 64 + 128 = 192)
+constexpr int kWGhMaxN = 256;            // GH: most canvas rows (x dl planes) whose gh accumulators fit next to h^T
 constexpr int kWWtBytes = kWJ * 32 * 2;  // GH: the band's W^T tile [128 j x 32 v] fp16 (A operand of gh), 8 KB
 
 struct WideParams {
@@ -111,7 +111,7 @@ constexpr uint32_t kDescHiSw128 = (1024u >> 4) | (1u << 14) | (ptx::kSwizzle128B
 __device__ __forceinline__ uint32_t desc_lo_sw128(uint32_t smem_addr) { return ((smem_addr >> 4) & 0x3FFFu) | (1u << 16); }
 __device__ __forceinline__ uint64_t desc64(uint32_t hi, uint32_t lo) { return (static_cast<uint64_t>(hi) << 32) | lo; }
 
-// GH (planes * T16 <= 192): gh^T[j, r] += W_in[v, j] dl[r, v] is formed here as well, as in the one-canvas kernel: the
+// GH (planes * T16 <= 256): gh^T[j, r] += W_in[v, j] dl[r, v] is formed here as well, as in the one-canvas kernel: the
 // band's W_in tile is re-derived from the master values the epilogue holds (precondition W_in == rn_bf16(W_master)),
 // written to shared memory as fp16(16 W) (the A operand), the dl band already in shared memory is read a second
 // time as the MN-major B operand, and the stripe's accumulators [128 j x planes T16] persist in tensor memory until

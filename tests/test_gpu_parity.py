@@ -86,7 +86,8 @@ SMALL = [
     (4, 1024, 256, 17, 16, {}),                      # 272 rows: second pair piece of 16 rows (8 per CTA)
     (4, 1024, 128, 3, 16, {}),                       # 48 rows: one fp16 dl plane, K padded to 64
     (4, 1024, 128, 2, 16, {}),                       # 32 rows: hi + lo fp16 planes fill the 64-wide K chunk
-    (4, 1024, 128, 12, 16, {}),                      # 192 rows: gh accumulators double-buffered, K = 192
+    (4, 1024, 128, 12, 16, {}),                      # 192 rows: gh formed inside the wide update kernel, K = 192
+    (4, 1024 + 128, 256, 16, 16, {}),                # 256 rows: the most the wide kernel's tensor memory holds next to h^T
 ]
 
 
