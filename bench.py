@@ -7,7 +7,7 @@ A "step" is one pass of the whole hot path over one round of synthetic input (SU
 tts_accept_mask (a1) + tts_distill_step (a2-a7) enqueued on a side stream, then the barrier (a8).
 Default workload: BASELINE.json configs[2], the Qwen3-8B-shaped draft head (V=151936, d=4096, T=16,
 bf16 weights + fp32 master, AdamW) -- the configuration the metric's >=70%-of-roofline target is
-quoted on.  Inputs are seeded and synthetic (paper_2605_09329_b200/synth.py).
+quoted on.  Inputs are seeded and synthetic (workloads/synth.py).
 
   value      steps/s with all inputs resident in HBM (CUDA events on the side stream, max over ranks)
   e2e        the same metric through tts_round_host: the round's teacher logits / hidden states /
@@ -207,7 +207,7 @@ def run_reference(args, rank, world):
     if rank != 0:
         return
     import numpy as np
-    from paper_2605_09329_b200 import synth
+    from workloads import synth
     cfgc = synth.CONFIGS[args.config]
     V, d = cfgc["V"], cfgc["d"]
     rows = min(args.cpu_sample_rows, 4096, V)   # ~1.5 s of oracle work per step (config 1: the whole problem)
@@ -237,7 +237,7 @@ def run_reference(args, rank, world):
 
 
 def workload_config(cfg_id, world, path, parallelism="replicas"):
-    from paper_2605_09329_b200 import synth
+    from workloads import synth
     c = synth.CONFIGS[cfg_id]
     par = "single GPU"
     if world > 1:
@@ -256,7 +256,8 @@ def workload_config(cfg_id, world, path, parallelism="replicas"):
 def run_ours(args, rank, world, local_rank):
     import numpy as np
     import torch
-    from paper_2605_09329_b200 import dist_util, synth, tts
+    from paper_2605_09329_b200 import dist_util, tts
+    from workloads import synth
 
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: the distillation step has no CPU fallback")
@@ -441,7 +442,8 @@ def run_stream(args, case, dev):
     (time with updates - time without) / number of updates.  Two stand-ins because they bracket the answer: an
     HBM-bound verifier competes with the (HBM-bound) update for the same bandwidth, a tensor-bound one does not."""
     import torch
-    from paper_2605_09329_b200 import synth, tts
+    from paper_2605_09329_b200 import tts
+    from workloads import synth
     from paper_2605_09329_b200.scheduler import DraftHeadUpdater
 
     c = case["cfg"]
@@ -562,7 +564,8 @@ def run_tiny(args):
     number of launches and the oracle's time on the same (whole) problem."""
     import numpy as np
     import torch
-    from paper_2605_09329_b200 import synth, tts
+    from paper_2605_09329_b200 import tts
+    from workloads import synth
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: the distillation step has no CPU fallback")
     case = synth.make_case(1)

@@ -1,6 +1,6 @@
 """Writes tests/golden/config1_tiny.txt: oracle results on BASELINE.json configs[0]
 (V=1024, d=64, T=8, fp32, seed 0, one SGD step lr=1e-3).  Calls only oracle/ and
-the input recipe (paper_2605_09329_b200.synth holds no method arithmetic); never
+the input recipe (workloads.synth holds no method arithmetic); never
 the CUDA path.  The paper prints no worked example for this path, so this is a
 regression fixture of the pinned oracle, not a paper value.
 
@@ -14,7 +14,7 @@ import numpy as np
 ROOT = os.path.dirname(os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
 sys.path.insert(0, ROOT)
 from oracle import tts_oracle as O  # noqa: E402
-from paper_2605_09329_b200 import synth  # noqa: E402
+from workloads import synth  # noqa: E402
 
 c = synth.make_case(1)
 mask, tau, am = O.accept_mask(c["teacher"], c["draft_tokens"], c["seg_len"])

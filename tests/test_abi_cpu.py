@@ -61,7 +61,8 @@ def test_config_struct_matches_header():
 
 
 def test_enums_match_header():
-    from paper_2605_09329_b200 import synth, tts
+    from paper_2605_09329_b200 import tts
+    from workloads import synth
     src = open(os.path.join(ROOT, "include", "tts.h")).read()
     for m in re.finditer(r"enum\s*\{(.*?)\}", src, flags=re.S):
         body = re.sub(r"/\*.*?\*/", "", m.group(1), flags=re.S)

@@ -6,7 +6,8 @@ import pytest
 import torch
 
 from oracle import tts_oracle as O
-from paper_2605_09329_b200 import synth, tts
+from paper_2605_09329_b200 import tts
+from workloads import synth
 
 from gpu_util import _dev, bits, config_for, max_abs
 

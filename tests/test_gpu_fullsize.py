@@ -16,7 +16,8 @@ import pytest
 import torch
 
 from oracle import tts_oracle as O
-from paper_2605_09329_b200 import synth, tts
+from paper_2605_09329_b200 import tts
+from workloads import synth
 
 from gpu_util import bits, max_abs
 

@@ -8,7 +8,8 @@ import pytest
 import torch
 
 from oracle import tts_oracle as O
-from paper_2605_09329_b200 import synth, tts
+from paper_2605_09329_b200 import tts
+from workloads import synth
 
 from gpu_util import _dev, check_step, run_gpu, run_oracle
 

@@ -6,7 +6,7 @@ import random
 
 import pytest
 
-from paper_2605_09329_b200 import synth
+from workloads import synth
 
 from gpu_util import check_step, run_gpu, run_oracle
 

@@ -7,7 +7,8 @@ import pytest
 import torch
 
 from oracle import tts_oracle as O
-from paper_2605_09329_b200 import synth, tts
+from paper_2605_09329_b200 import tts
+from workloads import synth
 from paper_2605_09329_b200.scheduler import DraftHeadUpdater
 
 from gpu_util import _dev, bits, max_abs

@@ -385,7 +385,7 @@ def _mask_ref(t, tok, C):
 
 
 def test_accept_mask_against_python_reference_and_properties():
-    from paper_2605_09329_b200 import synth
+    from workloads import synth
     for dtype in (synth.F32, synth.BF16):
         t, tok, exp_tau = synth.planted_mask_cases(257, 8, seed=3, dtype=dtype)
         mask, tau, am = O.accept_mask(t, tok, 8)
@@ -481,7 +481,7 @@ def test_row_weights_modes():
 
 # ---------------------------------------------------------------- 8. whole step / slab pieces
 def test_step_pieces_agree_with_dense_step():
-    from paper_2605_09329_b200 import synth
+    from workloads import synth
     c = synth.make_case(3, V=640, d=64, nonzero_state=True, step=3)
     mask, tau, _ = O.accept_mask(c["teacher"], c["draft_tokens"], c["seg_len"])
     np.testing.assert_array_equal(tau, c["tau_star"])
@@ -506,7 +506,7 @@ def test_golden_config1_regression():
     """tests/golden/config1_tiny.txt was written by tests/golden/make_golden.py,
     which calls only oracle/ and the input recipe."""
     import os
-    from paper_2605_09329_b200 import synth
+    from workloads import synth
     path = os.path.join(os.path.dirname(__file__), "golden", "config1_tiny.txt")
     vals = {}
     for line in open(path):

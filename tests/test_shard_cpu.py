@@ -47,7 +47,8 @@ def _worker(rank, world, port, q):
                       MASTER_PORT=str(port))
     import torch.distributed as dist
     from oracle import tts_oracle as O
-    from paper_2605_09329_b200 import dist_util as D, synth
+    from paper_2605_09329_b200 import dist_util as D
+    from workloads import synth
     D.init("gloo")
     case = synth.make_case(3, V=1024, d=64)            # every rank draws the same seeded case
     T, V = case["T"], case["V"]
@@ -83,7 +84,7 @@ def _worker(rank, world, port, q):
 
 def test_two_rank_exchange_reproduces_the_unsharded_step():
     from oracle import tts_oracle as O
-    from paper_2605_09329_b200 import synth
+    from workloads import synth
     world, port = 2, _free_port()
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
