@@ -60,6 +60,27 @@ enum { TTS_ROWS_ALL = 0, TTS_ROWS_ACCEPTED = 1, TTS_ROWS_ACCEPTED_PLUS_ONE = 2 }
  * qualifies (V % 128 == 0, d % 128 == 0, T_max <= 512), CUDA-core kernels otherwise
  * (fp32 parameters, e.g. BASELINE config 1; other shapes).  SIMT forces the CUDA-core kernels. */
 enum { TTS_PATH_AUTO = 0, TTS_PATH_SIMT = 1 };
+/* precision of Adam's moments m, v (the paper fixes only "Adam"; R6, R26).  F32 is the default and what
+ * every BASELINE.json configuration uses.  BF16 / Q8 are opt-in variants that cut the step's bytes (tensor path, AdamW
+ * only); their layouts and rounding rules are given at tts_distill_step. */
+enum { TTS_MOMENT_F32 = 0, TTS_MOMENT_BF16 = 1, TTS_MOMENT_Q8 = 2 };
+/* tts_config.flags */
+enum {
+  TTS_FLAG_CHECK_PRECONDITIONS = 1, /* every step also runs the checks behind tts_last_device_status (debug mode)  */
+  TTS_FLAG_DETERMINISTIC = 2,       /* gh is reduced in a fixed order (two-stage: per-CTA parts, then one sum) so    */
+                                    /* that a step is bit-reproducible run to run; costs one small kernel + scratch  */
+  TTS_FLAG_SEPARATE_GH = 4          /* gh is contracted against the W_in BUFFER by its own kernel instead of being   */
+                                    /* re-derived from the master inside the update pass: for callers who cannot     */
+                                    /* guarantee W_in == rn_bf16(W_master); costs a second read of W_in              */
+};
+/* bits of tts_last_device_status */
+enum {
+  TTS_DEV_W_MISMATCH = 1,        /* W_in != rn_bf16(W_master) somewhere (precondition 1 of tts_distill_step)       */
+  TTS_DEV_NONFINITE_TEACHER = 2, /* a teacher logit is NaN or +inf (-inf is legal: a masked vocabulary entry, R23) */
+  TTS_DEV_NONFINITE_H = 4,       /* a hidden state is NaN or +-inf                                                 */
+  TTS_DEV_BAD_TOKEN = 8,         /* tts_accept_stochastic saw a draft token outside [0, V) (treated as rejected)   */
+  TTS_DEV_NONFINITE_LOSS = 16    /* the step's loss came out NaN / inf                                             */
+};
 
 typedef struct tts_ctx tts_ctx;
 
@@ -77,6 +98,10 @@ typedef struct {
   int32_t max_ctas;     /* 0 = one CTA per SM; else cap the persistent kernels' grids so the  */
                         /* main stream keeps SMs while the step overlaps it    */
   int32_t kernel_path;  /* TTS_PATH_*                                                         */
+  int32_t moment_dtype; /* TTS_MOMENT_*: storage format of adam_m / adam_v (0 = fp32)                 */
+  int32_t max_inner_steps; /* largest K of tts_distill_inner_steps; > 1 reserves its z_ref scratch    */
+                        /* (T_max x V fp32) in tts_ctx_create so that no step call ever allocates     */
+  int32_t flags;        /* TTS_FLAG_* (0 = none)                                                      */
 } tts_config;
 
 const char* tts_status_string(int32_t status);
@@ -97,6 +122,22 @@ int32_t tts_set_lr(tts_ctx* ctx, float lr);
  * speculator between requests).  Both calls synchronise the device. */
 int32_t tts_set_step_count(tts_ctx* ctx, int64_t n);
 int64_t tts_get_step_count(const tts_ctx* ctx);   /* returns the count (-1 on error), not a status */
+/* Stream-ordered forms that do NOT synchronise the device: the set is enqueued on `stream` (put it on the step's side
+ * stream between two steps); the get enqueues a copy on `stream` and blocks the host on THAT stream only. */
+int32_t tts_set_step_count_async(tts_ctx* ctx, int64_t n, void* stream);
+int64_t tts_get_step_count_on(tts_ctx* ctx, void* stream);
+/* Device status word (bits TTS_DEV_*), accumulated by the kernels since the last read: blocks the host until the last
+ * step on this ctx is done (as tts_sync_step), returns the bits (-1 on error) and clears them.  Which checks run:
+ *   always                       TTS_DEV_BAD_TOKEN, TTS_DEV_NONFINITE_LOSS
+ *   TTS_FLAG_CHECK_PRECONDITIONS TTS_DEV_W_MISMATCH (every element of W_in against rn_bf16(W_master)),
+ *                                TTS_DEV_NONFINITE_TEACHER, TTS_DEV_NONFINITE_H (complete scans); +0.6 ms at the
+ *                                Qwen3-8B head: a debug mode.  tts_check_preconditions runs the same checks once. */
+int32_t tts_last_device_status(tts_ctx* ctx);
+int32_t tts_check_preconditions(tts_ctx* ctx, const void* teacher_logits, const void* h, const void* W_in,
+                                const float* W_master, int32_t T, void* stream);
+/* A kernel whose internal pipeline stalls for more than ~4 s (a protocol error, never a legal state) executes a trap
+ * instead of spinning forever: the launch fails with cudaErrorLaunchFailed, reported as TTS_ERR_CUDA by the next call
+ * that synchronises (tts_sync_step, tts_round_host, tts_last_device_status, ...). */
 /* CUDA error code (cudaError_t as int) of the last failed CUDA call on this ctx, 0 if none. */
 int32_t tts_last_cuda_error(const tts_ctx* ctx);
 /* 1 if the last tts_distill_step on this ctx ran the tcgen05/TMA kernels, 0 if CUDA-core. */
@@ -137,6 +178,8 @@ int32_t tts_accept_mask(tts_ctx* ctx,
  *                         smallest v with sum_{v' <= v} max(0, p - q) >= u * sum_v max(0, p - q)
  *   next_token_out[s]     that token; -1 when the whole canvas was accepted (the bonus token needs the target's
  *                         distribution at position C + 1, which this call does not see)
+ *   draft tokens outside [0, cfg.V) are rejected (never dereferenced) and set TTS_DEV_BAD_TOKEN: the call takes the
+ *                         WHOLE vocabulary, it is not shard-aware (a shard holds cfg.V local rows, tokens are global)
  *   diag_out [T,4] or NULL: the diagnostics of the paper's section 3 (Fig. 4), free by-products of
  *                         the same vocabulary sweep:  H(p_r) in nats,  -log q_r(argmax_v p_r),  p_r(tok_r),  q_r(tok_r)
  * tau_out / mask_out as in tts_accept_mask.  draft_logits: [T,V] fp32, row stride V (V % 4 == 0).
@@ -224,7 +267,8 @@ int32_t tts_distill_step_ex(tts_ctx* ctx, const void* teacher_logits, const void
  *   draft_logits  [T,V] fp32 device or NULL: the drafter's own logits for step 1 (and z_ref), as in tts_distill_step_ex
  *   loss_out      [K] device: the loss of every inner step;  kl_rows_out [T] or NULL: step 1's KL rows;
  *   gh_out        [T,d] or NULL: the LAST step's gradient w.r.t. h
- * The first call with K > 1 on a ctx allocates the z_ref scratch (T_max x V fp32); nothing else allocates.
+ * K > 1 without caller-supplied draft_logits needs the z_ref scratch: create the ctx with max_inner_steps >= K
+ * (else TTS_ERR_INVALID_ARG); no step call allocates.
  */
 int32_t tts_distill_inner_steps(tts_ctx* ctx, const void* teacher_logits, const void* h, const void* W_in, void* W_out,
                                 float* W_master, float* adam_m, float* adam_v, const float* pos_weight,
@@ -254,7 +298,6 @@ int32_t tts_profile_read(tts_ctx* ctx, float* ms_out, int32_t* n_steps_out);
  * capture no done-event is recorded and the phase profile is off; after cudaGraphLaunch on a stream call
  * tts_record_done on that stream, then tts_wait_step / tts_sync_step as usual (graph replay ignores
  * cross-stream events recorded elsewhere, hence the paper's CPU-side barrier = tts_sync_step).
- * tts_distill_inner_steps with K > 1 allocates on its first call and must not be captured first.
  */
 int32_t tts_record_done(tts_ctx* ctx, void* stream);
 

@@ -145,7 +145,8 @@ __global__ void __launch_bounds__(1024) accept_finalize_kernel(const float* __re
                                                                const float* __restrict__ u, int T, int seg_len,
                                                                uint8_t* __restrict__ mask, int32_t* __restrict__ tau,
                                                                int32_t* __restrict__ next_tok, float* __restrict__ diag,
-                                                               float* __restrict__ rows, int32_t* __restrict__ rej_row) {
+                                                               float* __restrict__ rows, int32_t* __restrict__ rej_row,
+                                                               int* __restrict__ dev_status) {
   extern __shared__ float pq[];   // [T][2]: p_r(tok), q_r(tok)
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
   for (int r = warp; r < T; r += n_warps) {
@@ -179,9 +180,14 @@ __global__ void __launch_bounds__(1024) accept_finalize_kernel(const float* __re
       const double lse_t = (double)mt + log(st), lse_z = (double)mz + log(sz);
       const int am = ai == 0x7fffffff ? 0 : ai;
       const size_t row = (size_t)r * V;
-      const float tt = load_t<BF16>(teacher, row + tok[r]);
+      // a draft token outside [0, V) (e.g. a GLOBAL id handed to a vocabulary shard: this call is not shard-aware)
+      // is never dereferenced: p(tok) = 0, q(tok) = +inf, so the row is rejected for every u, and the status word says so
+      const int tk = tok[r];
+      const bool tok_ok = tk >= 0 && tk < V;
+      if (!tok_ok) atomicOr(dev_status, TTS_DEV_BAD_TOKEN);
+      const float tt = tok_ok ? load_t<BF16>(teacher, row + tk) : -CUDART_INF_F;
       const float p_tok = tt == -CUDART_INF_F ? 0.f : (float)exp((double)tt - lse_t);
-      const float q_tok = (float)exp((double)z[row + tok[r]] - lse_z);
+      const float q_tok = tok_ok ? (float)exp((double)z[row + tk] - lse_z) : CUDART_INF_F;
       pq[2 * r] = p_tok;
       pq[2 * r + 1] = q_tok;
       rows[2 * r] = (float)lse_t;
@@ -350,14 +356,14 @@ cudaError_t launch_accept_stochastic(tts_ctx* c, const void* teacher, const floa
   if (bf) {
     accept_stats_partial_kernel<true><<<g1, 256, 0, s>>>(teacher, z, V, chunk, c->stat_part);
     accept_finalize_kernel<true><<<1, nt, sh, s>>>(c->stat_part, splits, teacher, z, V, tok, u, T, c->cfg.seg_len, mask,
-                                                   tau, next_tok, diag, c->acc_rows, c->acc_rej);
+                                                   tau, next_tok, diag, c->acc_rows, c->acc_rej, c->dev_status);
     residual_partial_kernel<true><<<g3, 256, 0, s>>>(teacher, z, V, rchunk, c->acc_rows, c->acc_rej, c->acc_rpart);
     residual_pick_kernel<true><<<S, 256, 0, s>>>(teacher, z, V, rchunk, rsplits, c->acc_rows, c->acc_rej, c->acc_rpart,
                                                  u2, next_tok);
   } else {
     accept_stats_partial_kernel<false><<<g1, 256, 0, s>>>(teacher, z, V, chunk, c->stat_part);
     accept_finalize_kernel<false><<<1, nt, sh, s>>>(c->stat_part, splits, teacher, z, V, tok, u, T, c->cfg.seg_len,
-                                                    mask, tau, next_tok, diag, c->acc_rows, c->acc_rej);
+                                                    mask, tau, next_tok, diag, c->acc_rows, c->acc_rej, c->dev_status);
     residual_partial_kernel<false><<<g3, 256, 0, s>>>(teacher, z, V, rchunk, c->acc_rows, c->acc_rej, c->acc_rpart);
     residual_pick_kernel<false><<<S, 256, 0, s>>>(teacher, z, V, rchunk, rsplits, c->acc_rows, c->acc_rej,
                                                   c->acc_rpart, u2, next_tok);

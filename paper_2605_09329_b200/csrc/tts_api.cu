@@ -28,7 +28,8 @@ cudaError_t dmalloc(T** p, size_t n) {
 void free_all(tts_ctx* c) {
   if (!c) return;
   tts::tc_destroy(c);
-  cudaFree(c->step_count_dev); cudaFree(c->step_scalars);
+  cudaFree(c->step_count_dev); cudaFree(c->step_scalars); cudaFree(c->dev_status);
+  if (c->host_slot) cudaFreeHost(c->host_slot);
   cudaFree(c->z); cudaFree(c->z_ref_buf); cudaFree(c->dl32); cudaFree(c->stat_part); cudaFree(c->row_stats);
   cudaFree(c->arg_val); cudaFree(c->arg_idx); cudaFree(c->argmax_tmp);
   cudaFree(c->acc_rows); cudaFree(c->acc_rej); cudaFree(c->acc_rpart);
@@ -56,7 +57,7 @@ const char* tts_status_string(int32_t s) {
   }
 }
 
-int32_t tts_version(void) { return 100; /* 0.1.0 */ }
+int32_t tts_version(void) { return 200; /* 0.2.0 */ }
 
 int32_t tts_ctx_create(const tts_config* cfg, int32_t device, tts_ctx** out) {
   if (!cfg || !out) return TTS_ERR_INVALID_ARG;
@@ -68,7 +69,10 @@ int32_t tts_ctx_create(const tts_config* cfg, int32_t device, tts_ctx** out) {
   if (cfg->optimizer != TTS_SGD && cfg->optimizer != TTS_ADAMW) return TTS_ERR_UNSUPPORTED;
   if (cfg->mask_mode < TTS_ROWS_ALL || cfg->mask_mode > TTS_ROWS_ACCEPTED_PLUS_ONE) return TTS_ERR_UNSUPPORTED;
   if (cfg->kernel_path != TTS_PATH_AUTO && cfg->kernel_path != TTS_PATH_SIMT) return TTS_ERR_UNSUPPORTED;
-  if (cfg->max_ctas < 0) return TTS_ERR_INVALID_ARG;
+  if (cfg->max_ctas < 0 || cfg->max_inner_steps < 0) return TTS_ERR_INVALID_ARG;
+  if (cfg->flags & ~(TTS_FLAG_CHECK_PRECONDITIONS | TTS_FLAG_DETERMINISTIC | TTS_FLAG_SEPARATE_GH)) return TTS_ERR_INVALID_ARG;
+  if (cfg->moment_dtype < TTS_MOMENT_F32 || cfg->moment_dtype > TTS_MOMENT_Q8) return TTS_ERR_UNSUPPORTED;
+  if (cfg->moment_dtype != TTS_MOMENT_F32 && cfg->optimizer != TTS_ADAMW) return TTS_ERR_UNSUPPORTED;
   // rows of every [*, V] / [*, d] tensor must start 16-byte aligned
   if ((static_cast<size_t>(cfg->V) * elem_size(cfg->logits_dtype)) % 16 != 0) return TTS_ERR_UNSUPPORTED;
   if ((static_cast<size_t>(cfg->d) * elem_size(cfg->param_dtype)) % 16 != 0) return TTS_ERR_UNSUPPORTED;
@@ -97,7 +101,12 @@ int32_t tts_ctx_create(const tts_config* cfg, int32_t device, tts_ctx** out) {
   ok = ok && dmalloc(&c->step_count_dev, 1) == cudaSuccess;
   ok = ok && dmalloc(&c->step_scalars, 2) == cudaSuccess;
   ok = ok && cudaMemset(c->step_count_dev, 0, sizeof(unsigned long long)) == cudaSuccess;
+  ok = ok && dmalloc(&c->dev_status, 1) == cudaSuccess;
+  ok = ok && cudaMemset(c->dev_status, 0, sizeof(int)) == cudaSuccess;
+  ok = ok && cudaHostAlloc(reinterpret_cast<void**>(&c->host_slot), 16, cudaHostAllocDefault) == cudaSuccess;
   ok = ok && dmalloc(&c->z, Tp * V) == cudaSuccess;
+  // K > 1 inner steps keep step 1's logits as z_ref: reserved here so that no step call allocates
+  if (cfg->max_inner_steps > 1) ok = ok && dmalloc(&c->z_ref_buf, Tp * V) == cudaSuccess;
   if (!c->tensor_ok) ok = ok && dmalloc(&c->dl32, Tm * V) == cudaSuccess;   // fp32 dlogits: CUDA-core kernels only
   ok = ok && dmalloc(&c->stat_part, Tm * tts::kStatSplitsMax * tts::kStatFields) == cudaSuccess;
   ok = ok && dmalloc(&c->row_stats, tts::kRowStatFields * Tm) == cudaSuccess;
@@ -115,6 +124,12 @@ int32_t tts_ctx_create(const tts_config* cfg, int32_t device, tts_ctx** out) {
   ok = ok && dmalloc(&c->st_mask, Tm) == cudaSuccess;
   ok = ok && dmalloc(&c->st_tau, Tm / cfg->seg_len) == cudaSuccess;
   ok = ok && dmalloc(&c->st_loss, 1) == cudaSuccess;
+  // the low-precision moment formats live in the tcgen05 update kernels only
+  if (ok && !c->tensor_ok && cfg->moment_dtype != TTS_MOMENT_F32) {
+    free_all(c);
+    delete c;
+    return TTS_ERR_UNSUPPORTED;
+  }
   if (ok && c->tensor_ok) ok = tts::tc_init(c) == cudaSuccess;
   if (!ok) {
     cudaGetLastError();
@@ -158,6 +173,51 @@ int64_t tts_get_step_count(const tts_ctx* c) {
     return -1;
   return static_cast<int64_t>(v);
 }
+int32_t tts_set_step_count_async(tts_ctx* c, int64_t n, void* stream) {
+  if (!c || n < 0) return TTS_ERR_INVALID_ARG;
+  tts_device_guard g(c->device);
+  cudaError_t e = tts::launch_set_count(c, static_cast<unsigned long long>(n), static_cast<cudaStream_t>(stream));
+  return e == cudaSuccess ? TTS_OK : cuda_fail(c, e);
+}
+
+int64_t tts_get_step_count_on(tts_ctx* c, void* stream) {
+  if (!c) return -1;
+  tts_device_guard g(c->device);
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  unsigned long long* slot = reinterpret_cast<unsigned long long*>(c->host_slot);
+  cudaError_t e = cudaMemcpyAsync(slot, c->step_count_dev, sizeof(*slot), cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  if (e != cudaSuccess) { cuda_fail(c, e); return -1; }
+  return static_cast<int64_t>(*slot);
+}
+
+int32_t tts_last_device_status(tts_ctx* c) {
+  if (!c) return -1;
+  tts_device_guard g(c->device);
+  cudaError_t e = cudaSuccess;
+  if (c->done_recorded) e = cudaEventSynchronize(c->done_event);
+  int bits = 0;
+  // the word is only ever written by kernels of finished steps at this point; the copy and the clear use the
+  // legacy default stream, which orders them after everything enqueued before this call
+  if (e == cudaSuccess) e = cudaMemcpy(&bits, c->dev_status, sizeof(int), cudaMemcpyDeviceToHost);
+  if (e == cudaSuccess) e = cudaMemset(c->dev_status, 0, sizeof(int));
+  if (e != cudaSuccess) { cuda_fail(c, e); return -1; }
+  return bits;
+}
+
+int32_t tts_check_preconditions(tts_ctx* c, const void* teacher, const void* h, const void* W_in, const float* W_master,
+                                int32_t T, void* stream) {
+  if (!c) return TTS_ERR_INVALID_ARG;
+  if (T <= 0 || T > c->cfg.T_max) return TTS_ERR_INVALID_ARG;
+  if (!aligned16(teacher) || !aligned16(h) || !aligned16(W_in) || !aligned16(W_master)) return TTS_ERR_INVALID_ARG;
+  tts_device_guard g(c->device);
+  int launches = 0;
+  cudaError_t e = tts::launch_check_preconditions(c, teacher, h, W_in, W_master, T, static_cast<cudaStream_t>(stream),
+                                                  &launches);
+  c->last_launches = launches;
+  return e == cudaSuccess ? TTS_OK : cuda_fail(c, e);
+}
+
 int32_t tts_last_cuda_error(const tts_ctx* c) { return c ? c->last_cuda_error : 0; }
 int32_t tts_last_step_used_tensor_path(const tts_ctx* c) { return c ? c->last_used_tensor : 0; }
 int32_t tts_last_launch_count(const tts_ctx* c) { return c ? c->last_launches : 0; }
@@ -167,6 +227,7 @@ int32_t tts_accept_mask(tts_ctx* c, const void* teacher, const int32_t* tok, int
   if (!c || !teacher || !tok || !mask_out || !tau_out) return TTS_ERR_INVALID_ARG;
   if (T <= 0 || T > c->cfg.T_max || T % c->cfg.seg_len != 0) return TTS_ERR_INVALID_ARG;
   if (!aligned16(teacher)) return TTS_ERR_INVALID_ARG;
+  tts_device_guard g(c->device);
   int launches = 0;
   cudaError_t e = tts::launch_accept_mask(c, teacher, tok, T, mask_out, tau_out, am_out,
                                           static_cast<cudaStream_t>(stream), &launches);
@@ -184,6 +245,7 @@ int32_t tts_accept_stochastic(tts_ctx* c, const void* teacher, const float* draf
   if (T <= 0 || T > c->cfg.T_max || T % c->cfg.seg_len != 0) return TTS_ERR_INVALID_ARG;
   if (!aligned16(teacher) || !aligned16(draft_logits)) return TTS_ERR_INVALID_ARG;
   if ((static_cast<size_t>(c->cfg.V) * sizeof(float)) % 16 != 0) return TTS_ERR_UNSUPPORTED;
+  tts_device_guard g(c->device);
   int launches = 0;
   cudaError_t e = tts::launch_accept_stochastic(c, teacher, draft_logits, tok, uniforms, uniforms_resample, T,
                                                 mask_out, tau_out, next_token_out, diag_out,
@@ -229,6 +291,7 @@ static int32_t run_step(tts_ctx* c, const void* teacher, const void* h, const vo
       !aligned16(adam_m) || !aligned16(adam_v) || !aligned16(gh_out) || !aligned16(gW_debug_out))
     return TTS_ERR_INVALID_ARG;
 
+  tts_device_guard guard(c->device);
   cudaStream_t s = static_cast<cudaStream_t>(side_stream);
   cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
   cudaError_t e = cudaStreamIsCapturing(s, &cap);
@@ -252,6 +315,13 @@ static int32_t run_step(tts_ctx* c, const void* teacher, const void* h, const vo
   if (phase != tts::kPhaseAll || capturing) c->prof_on = false;   // the phase events describe whole, eager steps only
   // Adam's count advances once per step, ON THE DEVICE: in the merge kernel of a3 (second half of a sharded step)
   tts::prof_mark(c, -1, s);
+  if ((cfg.flags & TTS_FLAG_CHECK_PRECONDITIONS) && phase != tts::kPhaseFinish) {   // debug mode: SURVEY 8(b) 1 and 5
+    if ((e = tts::launch_check_preconditions(c, teacher, h, W_in, phase == tts::kPhaseAll ? W_master : nullptr, T, s,
+                                             &launches)) != cudaSuccess) {
+      c->prof_on = prof_saved;
+      return cuda_fail(c, e);
+    }
+  }
   if (c->tensor_ok) {
     c->last_used_tensor = 1;
     e = tts::tc_step(c, a, s, &launches);
@@ -271,6 +341,7 @@ static int32_t run_step(tts_ctx* c, const void* teacher, const void* h, const vo
 
 int32_t tts_record_done(tts_ctx* c, void* stream) {
   if (!c) return TTS_ERR_INVALID_ARG;
+  tts_device_guard g(c->device);
   cudaError_t e = cudaEventRecord(c->done_event, static_cast<cudaStream_t>(stream));
   if (e != cudaSuccess) return cuda_fail(c, e);
   c->done_recorded = true;
@@ -306,6 +377,7 @@ int32_t tts_shard_argmax(tts_ctx* c, const void* teacher_local, int32_t T, int32
                          int32_t* idx_out, void* stream) {
   if (!c || !teacher_local || !val_out || !idx_out || v_offset < 0) return TTS_ERR_INVALID_ARG;
   if (T <= 0 || T > c->cfg.T_max || T % c->cfg.seg_len != 0 || !aligned16(teacher_local)) return TTS_ERR_INVALID_ARG;
+  tts_device_guard g(c->device);
   int launches = 0;
   cudaError_t e = tts::launch_shard_argmax(c, teacher_local, T, v_offset, val_out, idx_out,
                                            static_cast<cudaStream_t>(stream), &launches);
@@ -318,6 +390,7 @@ int32_t tts_shard_accept_mask(tts_ctx* c, const float* val_all, const int32_t* i
                               void* stream) {
   if (!c || !val_all || !idx_all || !tok || !mask_out || !tau_out || n_shards < 1) return TTS_ERR_INVALID_ARG;
   if (T <= 0 || T > c->cfg.T_max || T % c->cfg.seg_len != 0) return TTS_ERR_INVALID_ARG;
+  tts_device_guard g(c->device);
   int launches = 0;
   cudaError_t e = tts::launch_shard_mask(c, val_all, idx_all, n_shards, tok, T, mask_out, tau_out, am_out,
                                          static_cast<cudaStream_t>(stream), &launches);
@@ -331,11 +404,9 @@ int32_t tts_distill_inner_steps(tts_ctx* c, const void* teacher, const void* h, 
                                 const float* draft_logits, float* loss_out, float* kl_rows_out, float* gh_out,
                                 void* side_stream) {
   if (!c || K < 1 || !(lambda >= 0.f) || !loss_out) return TTS_ERR_INVALID_ARG;
-  if (K > 1 && !c->z_ref_buf) {   // the only allocation outside tts_ctx_create: first use of K > 1 on this ctx
-    cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&c->z_ref_buf),
-                               (size_t)c->T_pad_max * c->cfg.V * sizeof(float));
-    if (e != cudaSuccess) return cuda_fail(c, e);
-  }
+  // K > 1 keeps step 1's logits as z_ref: the caller's own draft_logits, or the scratch reserved by
+  // tts_config.max_inner_steps (no step call allocates)
+  if (K > 1 && !draft_logits && !c->z_ref_buf) return TTS_ERR_INVALID_ARG;
   int launches = 0;
   for (int k = 0; k < K; ++k) {
     tts_step_extras ex;
@@ -402,6 +473,7 @@ int32_t tts_profile_read(tts_ctx* c, float* ms_out, int32_t* n_steps_out) {
 int32_t tts_wait_step(tts_ctx* c, void* main_stream) {
   if (!c) return TTS_ERR_INVALID_ARG;
   if (!c->done_recorded) return TTS_OK;
+  tts_device_guard g(c->device);
   cudaError_t e = cudaStreamWaitEvent(static_cast<cudaStream_t>(main_stream), c->done_event, 0);
   return e == cudaSuccess ? TTS_OK : cuda_fail(c, e);
 }
@@ -420,6 +492,7 @@ int32_t tts_round_host(tts_ctx* c, const void* teacher_host, const void* h_host,
   if (!c || !teacher_host || !h_host || !tok_host || !pw_host || !loss_host || !tau_host) return TTS_ERR_INVALID_ARG;
   const tts_config& cfg = c->cfg;
   if (T <= 0 || T > cfg.T_max || T % cfg.seg_len != 0) return TTS_ERR_INVALID_ARG;
+  tts_device_guard guard(c->device);
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const size_t V = cfg.V, d = cfg.d;
   cudaError_t e;

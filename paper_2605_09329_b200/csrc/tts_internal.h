@@ -57,6 +57,16 @@ inline const float* z_src(const StepArgs& a, float* scratch) { return a.z_given 
 
 }  // namespace tts
 
+// Makes the ctx's device current for the lifetime of the object (a process may hold ctxs on several GPUs).
+struct tts_device_guard {
+  int prev;
+  bool switched;
+  explicit tts_device_guard(int device) : prev(-1), switched(false) {
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != device) switched = cudaSetDevice(device) == cudaSuccess;
+  }
+  ~tts_device_guard() { if (switched) cudaSetDevice(prev); }
+};
+
 struct tts_ctx {
   tts_config cfg;
   int device;
@@ -79,6 +89,9 @@ struct tts_ctx {
   float* arg_val;         // [T_max, kArgSplitsMax]
   int32_t* arg_idx;       // [T_max, kArgSplitsMax]
   int32_t* argmax_tmp;    // [T_max]
+  int* dev_status;        // device status word (bits TTS_DEV_*), read and cleared by tts_last_device_status
+  int* host_slot;         // pinned host scratch (16 bytes) for the stream-ordered status / step-count reads
+  float* gh_part;         // TTS_FLAG_DETERMINISTIC: [units][T16][128] per-unit parts of gh (tts_tc_gemm.cu)
   float* acc_rows;        // [T_max, 2] lse_t, lse_z of tts_accept_stochastic
   int32_t* acc_rej;       // [T_max / seg_len] first rejected row per sequence
   double* acc_rpart;      // [T_max / seg_len, kStatSplitsMax] residual mass per slice
@@ -107,6 +120,10 @@ inline void prof_mark(tts_ctx* c, int phase, cudaStream_t s) {
   cudaEventRecord(c->prof_events[slot * (TTS_NUM_PHASES + 1) + phase + 1], s);
 }
 
+// tts_check.cu: precondition checks (debug mode)
+cudaError_t launch_check_preconditions(tts_ctx* c, const void* teacher, const void* h, const void* W_in,
+                                       const float* master, int T, cudaStream_t s, int* launches);
+cudaError_t launch_set_count(tts_ctx* c, unsigned long long n, cudaStream_t s);
 // tts_mask.cu
 cudaError_t launch_accept_mask(tts_ctx* c, const void* teacher, const int32_t* tok, int T, uint8_t* mask,
                                int32_t* tau, int32_t* am_out, cudaStream_t s, int* launches);

@@ -192,7 +192,8 @@ __global__ void __launch_bounds__(1024) row_stats_merge_kernel(const float* __re
                                                                float* __restrict__ kl_rows_out,
                                                                float* __restrict__ loss_out,
                                                                unsigned long long* __restrict__ step_count,
-                                                               float* __restrict__ step_scalars, float b1, float b2) {
+                                                               float* __restrict__ step_scalars, float b1, float b2,
+                                                               int* __restrict__ dev_status) {
   __shared__ double red[32];
   if (threadIdx.x == 0) {
     // Adam's count and bias corrections live on the device (a replayed CUDA graph of the step keeps counting):
@@ -266,7 +267,9 @@ __global__ void __launch_bounds__(1024) row_stats_merge_kernel(const float* __re
   if (threadIdx.x == 0) {
     double sum = 0.0;
     for (int w = 0; w < n_warps; ++w) sum += red[w];   // fixed order
-    loss_out[0] = (float)((double)loss_scale * sum);
+    const float loss = (float)((double)loss_scale * sum);
+    loss_out[0] = loss;
+    if (!isfinite(loss)) atomicOr(dev_status, TTS_DEV_NONFINITE_LOSS);
   }
 }
 
@@ -328,7 +331,8 @@ static void launch_merge(tts_ctx* c, const StepArgs& a, const float* part, int s
                                                               c->cfg.seg_len, c->cfg.mask_mode, a.pos_weight, a.mask,
                                                               a.loss_scale, a.z_ref != nullptr, a.lambda, c->row_stats,
                                                               a.kl_rows_out, a.loss_out, c->step_count_dev,
-                                                              c->step_scalars, c->cfg.beta1, c->cfg.beta2);
+                                                              c->step_scalars, c->cfg.beta1, c->cfg.beta2,
+                                                              c->dev_status);
 }
 
 cudaError_t launch_row_stats(tts_ctx* c, const StepArgs& a, const float* z, int z_ld, cudaStream_t s, int* launches) {

@@ -37,6 +37,9 @@ cudaError_t tc_init(tts_ctx* c) {
   if ((e = cudaMemset(st->dlR, 0, (size_t)st->P * V * 2)) != cudaSuccess) return e;
   if ((e = cudaMemset(st->dlT, 0, V * st->Kp * 2)) != cudaSuccess) return e;
   if ((e = cudaMemset(st->hTT, 0, d * st->Kp * 2)) != cudaSuccess) return e;
+  if (c->cfg.flags & TTS_FLAG_DETERMINISTIC) {
+    if ((e = cudaMalloc(&c->gh_part, tc_gh_part_floats(c, T16) * sizeof(float))) != cudaSuccess) return e;
+  }
   if ((e = tc_gemm_init(c)) != cudaSuccess) return e;
   if ((e = tc_wide_init(c)) != cudaSuccess) return e;
   if ((e = tc_pair_init(c)) != cudaSuccess) return e;
@@ -52,6 +55,8 @@ void tc_destroy(tts_ctx* c) {
   cudaFree(st->dl_scale);
   cudaFree(st->hTc);
   cudaFree(st->dlC);
+  cudaFree(c->gh_part);
+  c->gh_part = nullptr;
   delete st;
   c->tc_state = nullptr;
 }
@@ -80,7 +85,10 @@ cudaError_t tc_step(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches
 
   // a4: operands of the gradient contractions
   // one canvas (T <= 16): one fused pass over the optimiser state (tts_tc_fused.cu) with its own pre-tiled operands
-  const int fused_grid = tc_fused_grid(c, T16);
+  // TTS_FLAG_SEPARATE_GH / TTS_FLAG_DETERMINISTIC: gh comes from its own kernel (reads the W_in buffer; per-unit parts
+  // reduced in a fixed order), which consumes the wide path's dl planes
+  const bool own_gh_kernel = a.gh_out && (c->cfg.flags & (TTS_FLAG_SEPARATE_GH | TTS_FLAG_DETERMINISTIC)) != 0;
+  const int fused_grid = own_gh_kernel ? 0 : tc_fused_grid(c, T16);
   if (fused_grid > 0) {
     if ((e = tc_launch_prep_fused(c, a, z, s, launches)) != cudaSuccess) return e;
     prof_mark(c, 2, s);
@@ -93,7 +101,7 @@ cudaError_t tc_step(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches
   if ((e = tc_launch_prep_wide(c, a, z, s, launches)) != cudaSuccess) return e;
   prof_mark(c, 2, s);
   // a5: gh on tcgen05 (reads W_in before the update may overwrite an aliased W_out)
-  if (a.gh_out && !tc_wide_fuses_gh(T16)) {
+  if (a.gh_out && !tc_wide_fuses_gh(c, T16)) {
     if ((e = tc_launch_gh(c, a, s, launches)) != cudaSuccess) return e;
   }
   prof_mark(c, 3, s);

@@ -51,7 +51,7 @@ struct LogitsParams {
   int z_ld;
   int n_vt;        // V / 128
   int k_chunks;    // d / 64
-  int T16;
+  int T16, T;      // padded rows (MMA N) and the caller's rows: rows >= T are computed but never stored
   int box_rows;    // rows per h box (<= 256)
   int n_boxes;     // h boxes per stage
   int stages;
@@ -202,12 +202,15 @@ tc_logits_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant
         uint32_t r[16];
         ptx::tmem_ld_32x32b_x16(tmem_base + ab * p.T16 + c0 + (static_cast<uint32_t>(q * 32) << 16), r);
         ptx::tmem_ld_wait();
+        // rows T .. T16 exist only as MMA padding: a caller's draft_logits_out has exactly T rows
         if (partial) {
 #pragma unroll
-          for (int i = 0; i < 16; ++i) atomicAdd(zc + (size_t)(c0 + i) * p.z_ld, __uint_as_float(r[i]));
+          for (int i = 0; i < 16; ++i)
+            if (c0 + i < p.T) atomicAdd(zc + (size_t)(c0 + i) * p.z_ld, __uint_as_float(r[i]));
         } else {
 #pragma unroll
-          for (int i = 0; i < 16; ++i) zc[(size_t)(c0 + i) * p.z_ld] = __uint_as_float(r[i]);
+          for (int i = 0; i < 16; ++i)
+            if (c0 + i < p.T) zc[(size_t)(c0 + i) * p.z_ld] = __uint_as_float(r[i]);
         }
       }
       ptx::tc_fence_before();
@@ -226,6 +229,7 @@ tc_logits_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant
 // ------------------------------------------------------------------ a5: gh
 struct GhParams {
   float* gh;
+  float* part;             // TTS_FLAG_DETERMINISTIC: [slots][T16][128] per-unit parts instead of fp32 RED into gh
   const float* dl_scale;   // {S, 1 / S} of the fp16 dl plane
   int T, d, T16;
   int planes;        // dl planes stacked along N (2: rows T16 .. 2 T16 hold the lo plane)
@@ -391,11 +395,17 @@ tc_gh_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant__ C
         if (p.planes == 2)
           ptx::tmem_ld_32x32b_x16(tmem_base + ab * p.N + p.T16 + c0 + (static_cast<uint32_t>(q * 32) << 16), r2);
         ptx::tmem_ld_wait();
+        // deterministic mode: this unit's part goes to its own slot (a warp stores 128 contiguous bytes per canvas
+        // row); tc_gh_reduce_kernel adds the slots of a j tile in split order
+        float* pc = p.part ? p.part + ((size_t)(MC ? 2 * u + cta : u) * p.T16 + c0) * kTileMN + q * 32 + lane : nullptr;
 #pragma unroll
         for (int i = 0; i < 16; ++i) {
           float x = __uint_as_float(r[i]);
           if (p.planes == 2) x += __uint_as_float(r2[i]);
-          if (c0 + i < p.T && j0 < p.d) atomicAdd(gc + (size_t)(c0 + i) * p.d, x * inv_s);
+          if (c0 + i < p.T && j0 < p.d) {
+            if (pc) pc[(size_t)i * kTileMN] = x * inv_s;
+            else atomicAdd(gc + (size_t)(c0 + i) * p.d, x * inv_s);
+          }
         }
       }
       ptx::tc_fence_before();
@@ -409,6 +419,47 @@ tc_gh_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant__ C
     ptx::tc_fence_after();
     ptx::tmem_dealloc(tmem_base, p.tmem_cols);
   }
+}
+
+// gh[r, j] = sum over the vocabulary splits of the j tile's parts, in split order (fixed: bit-reproducible)
+__global__ void __launch_bounds__(128) tc_gh_reduce_kernel(const float* __restrict__ part, int n_ju, int n_split, int mc,
+                                                           int T16, int d, float* __restrict__ gh) {
+  const int jt = blockIdx.x, r = blockIdx.y, jj = threadIdx.x;
+  float acc = 0.f;
+  for (int sp = 0; sp < n_split; ++sp) {
+    const int slot = mc ? 2 * (sp * n_ju + (jt >> 1)) + (jt & 1) : sp * n_ju + jt;
+    acc += part[((size_t)slot * T16 + r) * kTileMN + jj];
+  }
+  gh[(size_t)r * d + jt * kTileMN + jj] = acc;
+}
+
+// Work split of the gh kernel (shared by the launch and by the sizing of the deterministic-mode scratch).
+struct GhPlan {
+  bool mc;
+  int grid, n_ju, n_split, chunks_split, planes, N, box_rows, n_boxes;
+};
+GhPlan gh_plan(const tts_ctx* c, int T16) {
+  GhPlan g;
+  const int n_jt = c->cfg.d / kTileMN, chunks_total = c->cfg.V / kKC;
+  g.grid = c->cfg.max_ctas > 0 ? c->cfg.max_ctas : c->sm_count;
+  g.planes = tc_wide_planes(T16);
+  g.N = g.planes * T16;
+  g.box_rows = g.N <= kNMax ? g.N : kNMax;
+  g.n_boxes = (g.N + g.box_rows - 1) / g.box_rows;
+  // MC: clusters of two CTAs on adjacent j tiles share every dl box by TMA multicast (two boxes: 256 < T16 <= 512)
+  g.mc = g.n_boxes == 2 && g.grid >= 2;
+  if (g.mc) g.grid &= ~1;
+  const int n_cl = g.mc ? g.grid / 2 : g.grid;
+  g.n_ju = g.mc ? (n_jt + 1) / 2 : n_jt;
+  // About two units per CTA (cluster): each is a contiguous run of vocabulary chunks for one 128-column tile of gh,
+  // flushed with fp32 RED (256 KB per unit at T = 512: more units would make the flush the bottleneck).  Units of
+  // one vocabulary split run side by side on consecutive CTAs, so a dl chunk is fetched into L2 once for all j tiles.
+  int n_split = (2 * n_cl) / g.n_ju;
+  if (n_split < 1) n_split = 1;
+  if (n_split > chunks_total) n_split = chunks_total;
+  g.chunks_split = (chunks_total + n_split - 1) / n_split;
+  g.n_split = (chunks_total + g.chunks_split - 1) / g.chunks_split;
+  return g;
 }
 
 int pick_stages(int stage_bytes) {
@@ -439,7 +490,7 @@ cudaError_t tc_launch_logits(tts_ctx* c, const StepArgs& a, float* z_out, cudaSt
   const int T16 = (T + 15) / 16 * 16;
   LogitsParams p;
   p.z = z_out; p.z_ld = V;
-  p.n_vt = V / kTileMN; p.k_chunks = d / kKC; p.T16 = T16;
+  p.n_vt = V / kTileMN; p.k_chunks = d / kKC; p.T16 = T16; p.T = T;
   p.box_rows = T16 <= kNMax ? T16 : kNMax;
   p.n_boxes = (T16 + p.box_rows - 1) / p.box_rows;
   const int stage_bytes = kATile + p.n_boxes * p.box_rows * kKC * 2;
@@ -461,7 +512,7 @@ cudaError_t tc_launch_logits(tts_ctx* c, const StepArgs& a, float* z_out, cudaSt
   // once: it receives exactly two partial sums (or one store), and 0 + a + b does not depend on the order.
   p.stream_k = T16 <= 32 && p.n_vt % grid != 0;
   if (p.stream_k) {
-    cudaError_t e = cudaMemsetAsync(z_out, 0, (size_t)T16 * V * sizeof(float), s);
+    cudaError_t e = cudaMemsetAsync(z_out, 0, (size_t)T * V * sizeof(float), s);
     if (e != cudaSuccess) return e;
   }
   const size_t smem = 1024 + (size_t)p.stages * stage_bytes + sizeof(Bars);
@@ -473,38 +524,36 @@ cudaError_t tc_launch_logits(tts_ctx* c, const StepArgs& a, float* z_out, cudaSt
   return cudaGetLastError();
 }
 
+// slots of the deterministic-mode scratch for steps of up to T16 rows ([slots][T16][128] fp32)
+size_t tc_gh_part_floats(const tts_ctx* c, int T16) {
+  const GhPlan g = gh_plan(c, T16);
+  return (size_t)g.n_ju * g.n_split * (g.mc ? 2 : 1) * T16 * kTileMN;
+}
+
 cudaError_t tc_launch_gh(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches) {
   TcState* st = static_cast<TcState*>(c->tc_state);
   const int V = c->cfg.V, d = c->cfg.d, T = a.T;
   const int T16 = (T + 15) / 16 * 16;
   cudaError_t e;
-  if ((e = cudaMemsetAsync(a.gh_out, 0, (size_t)T * d * sizeof(float), s)) != cudaSuccess) return e;
-  int grid = c->cfg.max_ctas > 0 ? c->cfg.max_ctas : c->sm_count;
+  const bool det = (c->cfg.flags & TTS_FLAG_DETERMINISTIC) != 0 && c->gh_part != nullptr;
+  if (!det && (e = cudaMemsetAsync(a.gh_out, 0, (size_t)T * d * sizeof(float), s)) != cudaSuccess) return e;
+  const GhPlan g = gh_plan(c, T16);
+  int grid = g.grid;
+  const bool mc = g.mc;
   GhParams p;
-  p.gh = a.gh_out; p.dl_scale = st->dl_scale; p.T = T; p.d = d; p.T16 = T16;
+  p.gh = a.gh_out; p.part = det ? c->gh_part : nullptr;
+  p.dl_scale = st->dl_scale; p.T = T; p.d = d; p.T16 = T16;
   p.n_jt = d / kTileMN;
   p.chunks_total = V / kKC;
-  p.planes = tc_wide_planes(T16);
-  p.N = p.planes * T16;
-  p.box_rows = p.N <= kNMax ? p.N : kNMax;
-  p.n_boxes = (p.N + p.box_rows - 1) / p.box_rows;
+  p.planes = g.planes;
+  p.N = g.N;
+  p.box_rows = g.box_rows;
+  p.n_boxes = g.n_boxes;
   p.n_acc = 2 * p.N <= 512 ? 2 : 1;
   p.tmem_cols = pow2_cols(p.n_acc * p.N);
-  // MC: clusters of two CTAs on adjacent j tiles share every dl box by TMA multicast (two boxes: 256 < T16 <= 512)
-  static int mc_off = -1;
-  if (mc_off < 0) { const char* e = getenv("TTS_NO_GH_MC"); mc_off = (e && e[0] == '1') ? 1 : 0; }   // measurement switch
-  const bool mc = !mc_off && p.n_boxes == 2 && grid >= 2;
-  if (mc) grid &= ~1;
-  const int n_cl = mc ? grid / 2 : grid;
-  p.n_ju = mc ? (p.n_jt + 1) / 2 : p.n_jt;
-  // About two units per CTA (cluster): each is a contiguous run of vocabulary chunks for one 128-column tile of gh,
-  // flushed with fp32 RED (256 KB per unit at T = 512: more units would make the flush the bottleneck).  Units of
-  // one vocabulary split run side by side on consecutive CTAs, so a dl chunk is fetched into L2 once for all j tiles.
-  int n_split = (2 * n_cl) / p.n_ju;
-  if (n_split < 1) n_split = 1;
-  if (n_split > p.chunks_total) n_split = p.chunks_total;
-  p.chunks_split = (p.chunks_total + n_split - 1) / n_split;
-  p.n_split = (p.chunks_total + p.chunks_split - 1) / p.chunks_split;
+  p.n_ju = g.n_ju;
+  p.chunks_split = g.chunks_split;
+  p.n_split = g.n_split;
   const int stage_bytes = kATile + p.n_boxes * p.box_rows * kKC * 2;
   p.stages = pick_stages(stage_bytes);
   CUtensorMap tm_W, tm_dl;
@@ -535,6 +584,10 @@ cudaError_t tc_launch_gh(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* lau
     if ((e = cudaLaunchKernelEx(&cfg, tc_gh_kernel<true>, tm_W, tm_dl, p)) != cudaSuccess) return e;
   }
   *launches += 1;
+  if (det) {
+    tc_gh_reduce_kernel<<<dim3(p.n_jt, T), kTileMN, 0, s>>>(c->gh_part, p.n_ju, p.n_split, mc ? 1 : 0, T16, d, a.gh_out);
+    *launches += 1;
+  }
   return cudaGetLastError();
 }
 

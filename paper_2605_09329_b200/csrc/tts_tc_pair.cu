@@ -50,12 +50,12 @@ struct PairLogitsParams {
   int z_ld, V;
   int n_pt;        // pair tiles: ceil(V / 256)
   int k_chunks;    // d / 64
-  int T16;
+  int T16, T;      // padded rows (MMA N) and the caller's rows: rows >= T are computed but never stored
   int n_pieces;    // ceil(T16 / 256)
   int stages;
   // work split: `n_rounds` rounds of whole tiles (tile = pair + round * n_pairs, below n_main), then the `n_left`
-  // tiles from n_main on are cut along K into n_pairs equal unit ranges (594 tiles over 74 pairs would otherwise be
-  // 8.03 waves rounding to 9); their partial sums are accumulated into the zeroed z columns with fp32 RED
+  // tiles from n_main on are cut along K into two halves each (594 tiles over 74 pairs would otherwise be 8.03 waves
+  // rounding to 9); the two partial sums are accumulated into the zeroed z columns with fp32 RED (order-free)
   int n_rounds, n_main, n_left;
 };
 
@@ -68,9 +68,14 @@ struct PairWalk {
   int pair, n_pairs, round;
   long u, u_end;
   __device__ PairWalk(const PairLogitsParams& p, int pair_, int n_pairs_) : pair(pair_), n_pairs(n_pairs_), round(0) {
+    // every leftover tile is cut ONCE, in the middle of K: 2 n_left <= n_pairs halves, one per pair.  A z entry then
+    // receives exactly two partial sums, and 0 + a + b does not depend on their order: z, hence the loss and the
+    // weights, are bit-reproducible run to run.  (Cutting the leftovers over all pairs gave ~n_pairs / n_left
+    // unordered fp32 addends per entry for 0.03 ms.)
     const long U = (long)p.n_left * p.k_chunks;
-    u = U * pair / n_pairs;
-    u_end = U * (pair + 1) / n_pairs;
+    const int n_cut = 2 * p.n_left;
+    u = pair < n_cut ? U * pair / n_cut : 0;
+    u_end = pair < n_cut ? U * (pair + 1) / n_cut : 0;
   }
   __device__ bool next(const PairLogitsParams& p, PairItem& w) {
     while (round < p.n_rounds) {
@@ -196,10 +201,12 @@ tc_logits_pair_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_con
         if (v < p.V) {
           if (w.partial) {
 #pragma unroll
-            for (int i = 0; i < 16; ++i) atomicAdd(zc + (size_t)(c0 + i) * p.z_ld, __uint_as_float(r[i]));
+            for (int i = 0; i < 16; ++i)
+              if (c0 + i < p.T) atomicAdd(zc + (size_t)(c0 + i) * p.z_ld, __uint_as_float(r[i]));
           } else {
 #pragma unroll
-            for (int i = 0; i < 16; ++i) zc[(size_t)(c0 + i) * p.z_ld] = __uint_as_float(r[i]);
+            for (int i = 0; i < 16; ++i)
+              if (c0 + i < p.T) zc[(size_t)(c0 + i) * p.z_ld] = __uint_as_float(r[i]);
           }
         }
       }
@@ -224,12 +231,7 @@ cudaError_t tc_pair_init(tts_ctx*) {
 
 // 1 when the pair kernels serve this step: several canvases beyond one MMA's N, an even grid of at least one pair
 int tc_pair_eligible(const tts_ctx* c, int T16) {
-  static int off = -1;
-  if (off < 0) {
-    const char* e = getenv("TTS_NO_PAIR");   // measurement switch: one CTA per tile (tts_tc_gemm.cu)
-    off = (e && e[0] == '1') ? 1 : 0;
-  }
-  if (off || T16 <= kPNMax || T16 > 512) return 0;
+  if (T16 <= kPNMax || T16 > 512) return 0;
   const int grid = c->cfg.max_ctas > 0 ? c->cfg.max_ctas : c->sm_count;
   return grid >= 2;
 }
@@ -242,7 +244,7 @@ cudaError_t tc_launch_logits_pair(tts_ctx* c, const StepArgs& a, float* z_out, c
   p.z = z_out; p.z_ld = V; p.V = V;
   p.n_pt = (V + 255) / 256;
   p.k_chunks = d / kKC;
-  p.T16 = T16;
+  p.T16 = T16; p.T = T;
   p.n_pieces = (T16 + kPNMax - 1) / kPNMax;
   const int stage_bytes = kPATile + p.n_pieces * 128 * kKC * 2;
   p.stages = (kPSmemBudget - (int)sizeof(PairBars) - 1024) / stage_bytes;
@@ -267,7 +269,7 @@ cudaError_t tc_launch_logits_pair(tts_ctx* c, const StepArgs& a, float* z_out, c
   if (p.n_left > 0) {
     // the K-split tiles accumulate into zeroed columns [256 n_main, V) of z
     const size_t v_left = (size_t)p.n_main * 256;
-    cudaError_t e = cudaMemset2DAsync(z_out + v_left, (size_t)V * sizeof(float), 0, (V - v_left) * sizeof(float), T16, s);
+    cudaError_t e = cudaMemset2DAsync(z_out + v_left, (size_t)V * sizeof(float), 0, (V - v_left) * sizeof(float), T, s);
     if (e != cudaSuccess) return e;
   }
   cudaLaunchConfig_t cfg;

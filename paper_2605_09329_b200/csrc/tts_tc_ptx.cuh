@@ -49,8 +49,16 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
       : "memory");
   return ok != 0;
 }
+// Bounded wait.  The first probe is the fast path; after that the spin is watched by the SM clock, and a phase that
+// has not completed after ~2^33 cycles (4 s at 1.9 GHz; a step takes milliseconds) is a protocol error: the thread
+// traps, the launch fails with cudaErrorLaunchFailed and the host sees TTS_ERR_CUDA instead of a hung GPU.
+constexpr long long kMbarTimeoutCycles = 1ll << 33;
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  if (mbar_try_wait(bar, parity)) return;
+  const long long t0 = clock64();
+  uint32_t n = 0;
   while (!mbar_try_wait(bar, parity)) {
+    if ((++n & 0xFFFu) == 0 && clock64() - t0 > kMbarTimeoutCycles) asm volatile("trap;");
   }
 }
 
@@ -226,7 +234,8 @@ __device__ __forceinline__ void mbar_arrive_cta0(uint64_t* bar) {
 }
 // wait with acquire at cluster scope: the arrivals come from both CTAs of the pair
 __device__ __forceinline__ void mbar_wait_cluster(uint64_t* bar, uint32_t parity) {
-  uint32_t ok = 0;
+  uint32_t ok = 0, n = 0;
+  long long t0 = 0;
   while (!ok) {
     asm volatile(
         "{\n\t.reg .pred p;\n\t"
@@ -235,6 +244,10 @@ __device__ __forceinline__ void mbar_wait_cluster(uint64_t* bar, uint32_t parity
         : "=r"(ok)
         : "r"(smem_u32(bar)), "r"(parity)
         : "memory");
+    if (!ok) {   // bounded like mbar_wait
+      if (n == 0) t0 = clock64();
+      if ((++n & 0xFFFu) == 0 && clock64() - t0 > kMbarTimeoutCycles) asm volatile("trap;");
+    }
   }
 }
 // 2-D tiled load into THIS CTA's shared memory; the bytes are counted on CTA 0's mbarrier

@@ -43,6 +43,8 @@ cudaError_t tc_gemm_init(tts_ctx* c);
 cudaError_t tc_launch_logits(tts_ctx* c, const StepArgs& a, float* z_out, cudaStream_t s, int* launches);
 // a5: gh[r, j] = sum_v dl[r, v] W_in[v, j] on tcgen05, split over the vocabulary, fp32 atomics into gh
 cudaError_t tc_launch_gh(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches);
+// floats of the deterministic-mode scratch (per-unit parts of gh) for steps of up to T16 rows
+size_t tc_gh_part_floats(const tts_ctx* c, int T16);
 
 // tts_tc_fused.cu: a5 + a6 + a7 in one pass over the optimiser state (T <= 16, d % 1024 == 0, V % 16 == 0)
 cudaError_t tc_fused_init(tts_ctx* c);
@@ -53,7 +55,8 @@ cudaError_t tc_launch_update_fused(tts_ctx* c, const StepArgs& a, int grid, cuda
 // tts_tc_wide.cu: a4 operands (h^T rows, fp16 dl planes) and a6 + a7 for T <= 512
 cudaError_t tc_wide_init(tts_ctx* c);
 int tc_wide_planes(int T16);   // 2: dl S = hi + lo (T16 <= 32), 1: one fp16 plane
-int tc_wide_fuses_gh(int T16); // 1: the wide update kernel forms gh itself (planes * T16 <= 256): no gh kernel
+int tc_wide_fuses_gh(const tts_ctx* c, int T16); // 1: the wide update kernel forms gh itself (planes * T16 <= 256, and
+                                                 // neither TTS_FLAG_SEPARATE_GH nor TTS_FLAG_DETERMINISTIC): no gh kernel
 cudaError_t tc_launch_prep_wide(tts_ctx* c, const StepArgs& a, const float* z, cudaStream_t s, int* launches);
 cudaError_t tc_launch_update_wide(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches);
 

@@ -633,10 +633,9 @@ cudaError_t tc_wide_init(tts_ctx*) {
 int tc_wide_planes(int T16) { return 2 * T16 <= kKC ? 2 : 1; }
 
 // 1 when the wide update kernel forms gh itself (its accumulators fit next to h^T in tensor memory)
-int tc_wide_fuses_gh(int T16) {
-  static int off = -1;
-  if (off < 0) { const char* e = getenv("TTS_WIDE_NO_GH"); off = (e && e[0] == '1') ? 1 : 0; }   // measurement switch
-  return !off && tc_wide_planes(T16) * T16 <= kWGhMaxN;
+int tc_wide_fuses_gh(const tts_ctx* c, int T16) {
+  if (c->cfg.flags & (TTS_FLAG_SEPARATE_GH | TTS_FLAG_DETERMINISTIC)) return 0;
+  return tc_wide_planes(T16) * T16 <= kWGhMaxN;
 }
 
 // a4 of the wide path: h^T rows and the fp16 dl planes
@@ -658,7 +657,7 @@ cudaError_t tc_launch_prep_wide(tts_ctx* c, const StepArgs& a, const float* z, c
                                                                   static_cast<uint16_t*>(st->hTT), st->dl_scale);
   uint16_t* dlT = static_cast<uint16_t*>(st->dlT);
   // the row-major plane is the gh KERNEL's operand: not needed when the update kernel forms gh itself
-  uint16_t* dlR = (a.gh_out && !tc_wide_fuses_gh(T16)) ? static_cast<uint16_t*>(st->dlR) : nullptr;
+  uint16_t* dlR = (a.gh_out && !tc_wide_fuses_gh(c, T16)) ? static_cast<uint16_t*>(st->dlR) : nullptr;
   const dim3 grid(V / 128, Kp / 64);
   const bool bf = c->cfg.logits_dtype == TTS_BF16, fast = planes == 1;
   auto kern = bf ? (fast ? tc_prep_dl_wide_kernel<true, true> : tc_prep_dl_wide_kernel<true, false>)
@@ -710,7 +709,7 @@ cudaError_t tc_launch_update_wide(tts_ctx* c, const StepArgs& a, cudaStream_t s,
   if (p.n_win < 1) p.n_win = 1;
   if (p.n_win > p.n_bands) p.n_win = p.n_bands;
   cudaError_t e;
-  const bool gh_here = a.gh_out != nullptr && tc_wide_fuses_gh(T16);
+  const bool gh_here = a.gh_out != nullptr && tc_wide_fuses_gh(c, T16);
   p.gh = gh_here ? a.gh_out : nullptr;
   p.T = T; p.T16 = T16; p.planes = tc_wide_planes(T16);
   if (gh_here && (e = cudaMemsetAsync(a.gh_out, 0, (size_t)T * d * sizeof(float), s)) != cudaSuccess) return e;

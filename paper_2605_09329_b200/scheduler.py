@@ -133,7 +133,7 @@ class DraftHeadUpdater:
         self.barrier()
         self._snap = dict(W=self.W[self.cur].clone(), master=self.master.clone(),
                           m=None if self.m is None else self.m.clone(), v=None if self.v is None else self.v.clone(),
-                          step=tts.tts_get_step_count(self.ctx))
+                          step=tts.tts_get_step_count_on(self.ctx, self.side))   # waits for the side stream only
 
     def restore(self):
         """"resets the speculator between requests so per-request adaptation is bounded" (PAPER.md:459)."""
@@ -145,7 +145,7 @@ class DraftHeadUpdater:
         if self.m is not None:
             self.m.copy_(self._snap["m"])
             self.v.copy_(self._snap["v"])
-        tts.tts_set_step_count(self.ctx, self._snap["step"])
+        tts.tts_set_step_count_async(self.ctx, self._snap["step"], self.side)   # ordered before the next step, no host sync
         self.round = 0
 
     def close(self):

@@ -18,6 +18,9 @@ TTS_F32, TTS_BF16 = 0, 1
 TTS_SGD, TTS_ADAMW = 0, 1
 TTS_ROWS_ALL, TTS_ROWS_ACCEPTED, TTS_ROWS_ACCEPTED_PLUS_ONE = 0, 1, 2
 TTS_PATH_AUTO, TTS_PATH_SIMT = 0, 1
+TTS_MOMENT_F32, TTS_MOMENT_BF16, TTS_MOMENT_Q8 = 0, 1, 2
+TTS_FLAG_CHECK_PRECONDITIONS, TTS_FLAG_DETERMINISTIC, TTS_FLAG_SEPARATE_GH = 1, 2, 4
+TTS_DEV_W_MISMATCH, TTS_DEV_NONFINITE_TEACHER, TTS_DEV_NONFINITE_H, TTS_DEV_BAD_TOKEN, TTS_DEV_NONFINITE_LOSS = 1, 2, 4, 8, 16
 TTS_NUM_PHASES = 5
 TTS_SHARD_STAT_FIELDS = 8
 PHASE_NAMES = ("a2_logits", "a3_row_stats", "a4_dlogits", "a5_gh", "a6a7_gW_update")
@@ -33,7 +36,8 @@ class tts_config(C.Structure):
                 ("param_dtype", C.c_int32), ("logits_dtype", C.c_int32), ("optimizer", C.c_int32),
                 ("lr", C.c_float), ("beta1", C.c_float), ("beta2", C.c_float), ("eps", C.c_float),
                 ("weight_decay", C.c_float), ("mask_mode", C.c_int32), ("max_ctas", C.c_int32),
-                ("kernel_path", C.c_int32)]
+                ("kernel_path", C.c_int32), ("moment_dtype", C.c_int32), ("max_inner_steps", C.c_int32),
+                ("flags", C.c_int32)]
 
 
 EXPORTS = {
@@ -45,6 +49,10 @@ EXPORTS = {
     "tts_set_lr": (C.c_int32, [C.c_void_p, C.c_float]),
     "tts_set_step_count": (C.c_int32, [C.c_void_p, C.c_int64]),
     "tts_get_step_count": (C.c_int64, [C.c_void_p]),
+    "tts_set_step_count_async": (C.c_int32, [C.c_void_p, C.c_int64, C.c_void_p]),
+    "tts_get_step_count_on": (C.c_int64, [C.c_void_p, C.c_void_p]),
+    "tts_last_device_status": (C.c_int32, [C.c_void_p]),
+    "tts_check_preconditions": (C.c_int32, [C.c_void_p] * 5 + [C.c_int32, C.c_void_p]),
     "tts_last_cuda_error": (C.c_int32, [C.c_void_p]),
     "tts_last_step_used_tensor_path": (C.c_int32, [C.c_void_p]),
     "tts_last_launch_count": (C.c_int32, [C.c_void_p]),
@@ -105,10 +113,15 @@ def _ptr(x):
     raise TypeError("cannot take the address of %r" % type(x))
 
 
-def _stream(s):
+_ctx_device = {}   # ctx address -> CUDA ordinal (a process may hold ctxs on several GPUs)
+
+
+def _stream(s, ctx=None):
+    """None -> the current stream OF THE CTX'S DEVICE (not of whatever device is current)."""
     if s is None:
         import torch
-        return torch.cuda.current_stream().cuda_stream
+        dev = _ctx_device.get(getattr(ctx, "value", None))
+        return torch.cuda.current_stream(dev).cuda_stream
     if isinstance(s, int):
         return s
     return s.cuda_stream
@@ -131,10 +144,12 @@ def tts_ctx_create(cfg: tts_config, device: int = 0):
     out = C.c_void_p()
     st = lib().tts_ctx_create(C.byref(cfg), device, C.byref(out))
     _check(None, st, "tts_ctx_create")
+    _ctx_device[out.value] = device
     return out
 
 
 def tts_ctx_destroy(ctx):
+    _ctx_device.pop(getattr(ctx, "value", None), None)
     _check(None, lib().tts_ctx_destroy(ctx), "tts_ctx_destroy")
 
 
@@ -148,6 +163,24 @@ def tts_set_step_count(ctx, n: int):
 
 def tts_get_step_count(ctx) -> int:
     return lib().tts_get_step_count(ctx)
+
+
+def tts_set_step_count_async(ctx, n: int, stream=None):
+    _check(ctx, lib().tts_set_step_count_async(ctx, n, _stream(stream, ctx)), "tts_set_step_count_async")
+
+
+def tts_get_step_count_on(ctx, stream=None) -> int:
+    return lib().tts_get_step_count_on(ctx, _stream(stream, ctx))
+
+
+def tts_last_device_status(ctx) -> int:
+    return lib().tts_last_device_status(ctx)
+
+
+def tts_check_preconditions(ctx, teacher_logits, h, W_in, W_master, T, stream=None):
+    st = lib().tts_check_preconditions(ctx, _ptr(teacher_logits), _ptr(h), _ptr(W_in), _ptr(W_master), T,
+                                       _stream(stream, ctx))
+    _check(ctx, st, "tts_check_preconditions")
 
 
 def tts_last_cuda_error(ctx) -> int:
@@ -164,7 +197,7 @@ def tts_last_launch_count(ctx) -> int:
 
 def tts_accept_mask(ctx, teacher_logits, draft_tokens, T, mask_out, tau_out, teacher_argmax_out=None, stream=None):
     st = lib().tts_accept_mask(ctx, _ptr(teacher_logits), _ptr(draft_tokens), T, _ptr(mask_out), _ptr(tau_out),
-                               _ptr(teacher_argmax_out), _stream(stream))
+                               _ptr(teacher_argmax_out), _stream(stream, ctx))
     _check(ctx, st, "tts_accept_mask")
 
 
@@ -172,7 +205,7 @@ def tts_accept_stochastic(ctx, teacher_logits, draft_logits, draft_tokens, unifo
                           tau_out, next_token_out, diag_out=None, stream=None):
     st = lib().tts_accept_stochastic(ctx, _ptr(teacher_logits), _ptr(draft_logits), _ptr(draft_tokens), _ptr(uniforms),
                                      _ptr(uniforms_resample), T, _ptr(mask_out), _ptr(tau_out), _ptr(next_token_out),
-                                     _ptr(diag_out), _stream(stream))
+                                     _ptr(diag_out), _stream(stream, ctx))
     _check(ctx, st, "tts_accept_stochastic")
 
 
@@ -181,7 +214,7 @@ def tts_distill_step(ctx, teacher_logits, h, W_in, W_out, W_master, adam_m, adam
     st = lib().tts_distill_step(ctx, _ptr(teacher_logits), _ptr(h), _ptr(W_in), _ptr(W_out), _ptr(W_master),
                                 _ptr(adam_m), _ptr(adam_v), _ptr(pos_weight), _ptr(mask), T, loss_scale,
                                 _ptr(loss_out), _ptr(kl_rows_out), _ptr(gh_out), _ptr(gW_debug_out),
-                                _stream(side_stream))
+                                _stream(side_stream, ctx))
     _check(ctx, st, "tts_distill_step")
 
 
@@ -192,7 +225,7 @@ def tts_distill_step_ex(ctx, teacher_logits, h, W_in, W_out, W_master, adam_m, a
     st = lib().tts_distill_step_ex(ctx, _ptr(teacher_logits), _ptr(h), _ptr(W_in), _ptr(W_out), _ptr(W_master),
                                    _ptr(adam_m), _ptr(adam_v), _ptr(pos_weight), _ptr(mask), T, loss_scale,
                                    _ptr(loss_out), _ptr(kl_rows_out), _ptr(gh_out), _ptr(gW_debug_out),
-                                   C.addressof(ex), _stream(side_stream))
+                                   C.addressof(ex), _stream(side_stream, ctx))
     _check(ctx, st, "tts_distill_step_ex")
 
 
@@ -202,7 +235,7 @@ def tts_distill_inner_steps(ctx, teacher_logits, h, W_in, W_out, W_master, adam_
     st = lib().tts_distill_inner_steps(ctx, _ptr(teacher_logits), _ptr(h), _ptr(W_in), _ptr(W_out), _ptr(W_master),
                                        _ptr(adam_m), _ptr(adam_v), _ptr(pos_weight), _ptr(mask), T, loss_scale, K,
                                        lam, _ptr(draft_logits), _ptr(loss_out), _ptr(kl_rows_out), _ptr(gh_out),
-                                       _stream(side_stream))
+                                       _stream(side_stream, ctx))
     _check(ctx, st, "tts_distill_inner_steps")
 
 
@@ -219,11 +252,11 @@ def tts_profile_read(ctx):
 
 
 def tts_wait_step(ctx, main_stream=None):
-    _check(ctx, lib().tts_wait_step(ctx, _stream(main_stream)), "tts_wait_step")
+    _check(ctx, lib().tts_wait_step(ctx, _stream(main_stream, ctx)), "tts_wait_step")
 
 
 def tts_record_done(ctx, stream=None):
-    _check(ctx, lib().tts_record_done(ctx, _stream(stream)), "tts_record_done")
+    _check(ctx, lib().tts_record_done(ctx, _stream(stream, ctx)), "tts_record_done")
 
 
 def tts_sync_step(ctx):
@@ -235,7 +268,7 @@ def tts_round_host(ctx, teacher_logits_host, h_host, draft_tokens_host, pos_weig
     st = lib().tts_round_host(ctx, _ptr(teacher_logits_host), _ptr(h_host), _ptr(draft_tokens_host),
                               _ptr(pos_weight_host), T, loss_scale, _ptr(W_in), _ptr(W_out), _ptr(W_master),
                               _ptr(adam_m), _ptr(adam_v), _ptr(gh_dev), _ptr(loss_host), _ptr(tau_host),
-                              _ptr(mask_host), _stream(stream))
+                              _ptr(mask_host), _stream(stream, ctx))
     _check(ctx, st, "tts_round_host")
 
 
@@ -247,7 +280,7 @@ def tts_shard_begin_step(ctx, teacher_logits_local, h, W_in_local, T, stats_out,
                          draft_logits_out=None, ref_logits=None, lam=0.0, side_stream=None):
     ex = _extras(draft_logits, draft_logits_out, ref_logits, lam)
     st = lib().tts_shard_begin_step(ctx, _ptr(teacher_logits_local), _ptr(h), _ptr(W_in_local), T, C.addressof(ex),
-                                    _ptr(stats_out), _stream(side_stream))
+                                    _ptr(stats_out), _stream(side_stream, ctx))
     _check(ctx, st, "tts_shard_begin_step")
 
 
@@ -260,25 +293,25 @@ def tts_shard_finish_step(ctx, stats_all, n_shards, teacher_logits_local, h, W_i
                                      _ptr(W_in_local), _ptr(W_out_local), _ptr(W_master_local), _ptr(adam_m_local),
                                      _ptr(adam_v_local), _ptr(pos_weight), _ptr(mask), T, loss_scale, _ptr(loss_out),
                                      _ptr(kl_rows_out), _ptr(gh_partial_out), _ptr(gW_debug_out), C.addressof(ex),
-                                     _stream(side_stream))
+                                     _stream(side_stream, ctx))
     _check(ctx, st, "tts_shard_finish_step")
 
 
 def tts_shard_argmax(ctx, teacher_logits_local, T, v_offset, val_out, idx_out, stream=None):
     st = lib().tts_shard_argmax(ctx, _ptr(teacher_logits_local), T, v_offset, _ptr(val_out), _ptr(idx_out),
-                                _stream(stream))
+                                _stream(stream, ctx))
     _check(ctx, st, "tts_shard_argmax")
 
 
 def tts_shard_accept_mask(ctx, val_all, idx_all, n_shards, draft_tokens, T, mask_out, tau_out, teacher_argmax_out=None,
                           stream=None):
     st = lib().tts_shard_accept_mask(ctx, _ptr(val_all), _ptr(idx_all), n_shards, _ptr(draft_tokens), T, _ptr(mask_out),
-                                     _ptr(tau_out), _ptr(teacher_argmax_out), _stream(stream))
+                                     _ptr(tau_out), _ptr(teacher_argmax_out), _stream(stream, ctx))
     _check(ctx, st, "tts_shard_accept_mask")
 
 
 def make_config(V, d, T_max, seg_len, param_dtype=TTS_BF16, logits_dtype=TTS_BF16, optimizer=TTS_ADAMW, lr=1e-5,
                 beta1=0.9, beta2=0.999, eps=1e-8, weight_decay=0.0, mask_mode=TTS_ROWS_ALL, max_ctas=0,
-                kernel_path=TTS_PATH_AUTO) -> tts_config:
+                kernel_path=TTS_PATH_AUTO, moment_dtype=TTS_MOMENT_F32, max_inner_steps=0, flags=0) -> tts_config:
     return tts_config(V, d, T_max, seg_len, param_dtype, logits_dtype, optimizer, lr, beta1, beta2, eps,
-                      weight_decay, mask_mode, max_ctas, kernel_path)
+                      weight_decay, mask_mode, max_ctas, kernel_path, moment_dtype, max_inner_steps, flags)

@@ -40,7 +40,7 @@ def test_binding_covers_every_declared_symbol(built):
     assert sorted(tts.EXPORTS) == _declared()
     for name in _declared():
         assert callable(getattr(tts, name)), name
-    assert tts.tts_version() >= 100
+    assert tts.tts_version() >= 200
     assert tts.tts_status_string(tts.TTS_ERR_ARCH) == "TTS_ERR_ARCH"
 
 
