@@ -25,19 +25,21 @@ def bits(t: torch.Tensor) -> np.ndarray:
     return t.view(torch.int16).cpu().numpy().view(np.uint16)
 
 
-def config_for(case, *, mask_mode=tts.TTS_ROWS_ALL, kernel_path=tts.TTS_PATH_AUTO, T_max=None, max_ctas=0):
+def config_for(case, *, mask_mode=tts.TTS_ROWS_ALL, kernel_path=tts.TTS_PATH_AUTO, T_max=None, max_ctas=0,
+               moment_dtype=tts.TTS_MOMENT_F32, max_inner_steps=0, flags=0):
     c = case["cfg"]
     return tts.make_config(case["V"], case["d"], T_max or case["T"], case["seg_len"], c["param"], c["logits"],
                            c["optimizer"], c["lr"], c["beta1"], c["beta2"], c["eps"], c["weight_decay"], mask_mode,
-                           max_ctas, kernel_path)
+                           max_ctas, kernel_path, moment_dtype, max_inner_steps, flags)
 
 
 def run_gpu(case, *, mask_mode=tts.TTS_ROWS_ALL, kernel_path=tts.TTS_PATH_AUTO, want_gW=True, want_gh=True,
-            alias_w=False, side_stream=True, max_ctas=0):
+            alias_w=False, side_stream=True, max_ctas=0, flags=0):
     """One tts_accept_mask + tts_distill_step on cuda:0.  Returns a dict of numpy results."""
     T, V, d = case["T"], case["V"], case["d"]
     bf = case["cfg"]["param"] == synth.BF16
-    ctx = tts.tts_ctx_create(config_for(case, mask_mode=mask_mode, kernel_path=kernel_path, max_ctas=max_ctas), 0)
+    ctx = tts.tts_ctx_create(config_for(case, mask_mode=mask_mode, kernel_path=kernel_path, max_ctas=max_ctas,
+                                        flags=flags), 0)
     try:
         if case.get("step", 1) > 1:
             tts.tts_set_step_count(ctx, case["step"] - 1)
@@ -68,7 +70,7 @@ def run_gpu(case, *, mask_mode=tts.TTS_ROWS_ALL, kernel_path=tts.TTS_PATH_AUTO, 
                    loss=float(loss.item()), kl_rows=kl.cpu().numpy(),
                    gh=gh.cpu().numpy() if want_gh else None, gW=gW.cpu().numpy() if want_gW else None,
                    used_tensor=tts.tts_last_step_used_tensor_path(ctx), step_count=tts.tts_get_step_count(ctx),
-                   launches=mask_launches + step_launches)
+                   launches=mask_launches + step_launches, dev_status=tts.tts_last_device_status(ctx))
         if bf:
             out["master"] = master.cpu().numpy()
             out["W_out"] = bits(W_out)

@@ -1,0 +1,209 @@
+"""Boundary behaviour of the C-ABI library on the GPU: buffers are written exactly as declared, the
+debug-mode precondition checks report into the device status word, the stream-ordered step-count calls, the
+no-allocation contract of K > 1 inner steps, and the two flags that change how gh is formed
+(TTS_FLAG_SEPARATE_GH: contracted against the W_in buffer; TTS_FLAG_DETERMINISTIC: bit-reproducible)."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import tts_oracle as O
+from paper_2605_09329_b200 import tts
+from workloads import synth
+
+from gpu_util import _dev, check_step, config_for, max_abs, run_gpu, run_oracle
+
+pytestmark = pytest.mark.gpu
+
+
+def _buffers(case):
+    t = dict(teacher=_dev(case["teacher"]), h=_dev(case["h"]), tok=_dev(case["draft_tokens"]), W_in=_dev(case["W"]),
+             master=_dev(case["master"]), m=_dev(case["m"]), v=_dev(case["v"]), pw=_dev(case["pos_weight"]))
+    t["W_out"] = torch.empty_like(t["W_in"])
+    t["loss"] = torch.zeros(1, device="cuda")
+    t["gh"] = torch.zeros(case["T"], case["d"], device="cuda")
+    return t
+
+
+@pytest.mark.parametrize("V,d,T", [(2048 + 128, 1024, 8), (4096, 256, 8), (4096, 256, 24), (1000, 72, 8)])
+def test_draft_logits_out_holds_exactly_T_rows(V, d, T):
+    """T % 16 != 0 (T = 8 is the EAGLE-3 depth): the tensor-path logits kernels compute ceil16(T) rows
+    as MMA padding but must store only T of them into the caller's draft_logits_out [T, V]."""
+    case = synth.make_case(3, V=V, d=d, seg_len=8, n_seq=T // 8)
+    ctx = tts.tts_ctx_create(config_for(case), 0)
+    try:
+        t = _buffers(case)
+        guard = 4 * V
+        buf = torch.full((T * V + guard,), 12345.0, device="cuda")
+        z_out = buf[:T * V].view(T, V)
+        tts.tts_distill_step_ex(ctx, t["teacher"], t["h"], t["W_in"], t["W_out"], t["master"], t["m"], t["v"], t["pw"],
+                                None, T, 1.0, t["loss"], None, t["gh"], None, draft_logits_out=z_out)
+        tts.tts_sync_step(ctx)
+        assert bool((buf[T * V:] == 12345.0).all()), "rows beyond T were written"
+        z_ref = O.widen(case["h"]) @ O.widen(case["W"]).T
+        assert max_abs(z_out.cpu().numpy() - z_ref) <= 2e-3 * max_abs(z_ref)
+        o = run_oracle(case)
+        assert abs(float(t["loss"].item()) - o["loss"]) <= 1e-3 * abs(o["loss"]) + 1e-6
+    finally:
+        tts.tts_ctx_destroy(ctx)
+
+
+def test_precondition_checks_report_into_the_status_word():
+    case = synth.make_case(3, V=4096, d=1024)
+    ctx = tts.tts_ctx_create(config_for(case, flags=tts.TTS_FLAG_CHECK_PRECONDITIONS), 0)
+    try:
+        T = case["T"]
+
+        def step(t):
+            tts.tts_distill_step(ctx, t["teacher"], t["h"], t["W_in"], t["W_out"], t["master"], t["m"], t["v"], t["pw"],
+                                 None, T, 1.0, t["loss"], None, t["gh"], None)
+            return tts.tts_last_device_status(ctx)
+
+        t = _buffers(case)
+        t["teacher"][3, 17] = float("-inf")           # a masked vocabulary entry is legal (R23)
+        assert step(t) == 0
+        assert tts.tts_last_device_status(ctx) == 0
+        t = _buffers(case)
+        w = t["W_in"].view(torch.int16)
+        w[1234, 77] ^= 1                              # one bf16 ulp off rn_bf16(master)
+        assert step(t) == tts.TTS_DEV_W_MISMATCH
+        assert tts.tts_last_device_status(ctx) == 0   # read-and-clear
+        t = _buffers(case)
+        t["teacher"][5, 4000] = float("nan")
+        assert step(t) & tts.TTS_DEV_NONFINITE_TEACHER
+        t = _buffers(case)
+        t["teacher"][0, 0] = float("inf")
+        st = step(t)
+        assert st & tts.TTS_DEV_NONFINITE_TEACHER and st & tts.TTS_DEV_NONFINITE_LOSS
+        t = _buffers(case)
+        t["h"][2, 5] = float("inf")
+        assert step(t) & tts.TTS_DEV_NONFINITE_H
+        # the same checks as one explicit call, no step
+        t = _buffers(case)
+        t["W_in"].view(torch.int16)[0, 0] ^= 1
+        tts.tts_check_preconditions(ctx, t["teacher"], t["h"], t["W_in"], t["master"], T)
+        assert tts.tts_last_device_status(ctx) == tts.TTS_DEV_W_MISMATCH
+    finally:
+        tts.tts_ctx_destroy(ctx)
+
+
+def test_checks_are_off_by_default_and_loss_bit_is_always_on():
+    case = synth.make_case(3, V=2048, d=256)
+    ctx = tts.tts_ctx_create(config_for(case), 0)
+    try:
+        t = _buffers(case)
+        t["W_in"].view(torch.int16)[0, 0] ^= 1
+        tts.tts_distill_step(ctx, t["teacher"], t["h"], t["W_in"], t["W_out"], t["master"], t["m"], t["v"], t["pw"],
+                             None, case["T"], 1.0, t["loss"], None, t["gh"], None)
+        assert tts.tts_last_device_status(ctx) == 0
+        t = _buffers(case)
+        t["teacher"][0, 0] = float("nan")
+        tts.tts_distill_step(ctx, t["teacher"], t["h"], t["W_in"], t["W_out"], t["master"], t["m"], t["v"], t["pw"],
+                             None, case["T"], 1.0, t["loss"], None, t["gh"], None)
+        assert tts.tts_last_device_status(ctx) == tts.TTS_DEV_NONFINITE_LOSS
+    finally:
+        tts.tts_ctx_destroy(ctx)
+
+
+def test_stream_ordered_step_count():
+    case = synth.make_case(3, V=2048, d=256)
+    ctx = tts.tts_ctx_create(config_for(case), 0)
+    try:
+        side = torch.cuda.Stream()
+        t = _buffers(case)
+        assert tts.tts_get_step_count_on(ctx, side) == 0
+        tts.tts_set_step_count_async(ctx, 41, side)
+        tts.tts_distill_step(ctx, t["teacher"], t["h"], t["W_in"], t["W_out"], t["master"], t["m"], t["v"], t["pw"],
+                             None, case["T"], 1.0, t["loss"], None, t["gh"], None, side)
+        assert tts.tts_get_step_count_on(ctx, side) == 42
+        assert tts.tts_get_step_count(ctx) == 42
+        # the step really ran with n = 42: compare m against the oracle at that count (m does not depend on n, the
+        # master does)
+        case2 = dict(case, step=42)
+        o = run_oracle(case2)
+        err = max_abs(t["master"].cpu().numpy().astype(np.float64) - o["master"])
+        assert err <= 2e-3 * max_abs(o["master"])
+        d_ref = o["master"] - O.widen(case["master"])
+        d_gpu = t["master"].cpu().numpy().astype(np.float64) - O.widen(case["master"])
+        big = np.abs(o["gW"]) >= 1e-2 * max_abs(o["gW"])
+        assert np.all(np.abs(d_gpu[big] - d_ref[big]) <= 0.02 * case["cfg"]["lr"] + 1e-8)
+    finally:
+        tts.tts_ctx_destroy(ctx)
+
+
+def test_inner_steps_never_allocate():
+    case = synth.make_case(3, V=2048, d=256)
+    t = _buffers(case)
+    losses = torch.zeros(3, device="cuda")
+    ctx = tts.tts_ctx_create(config_for(case), 0)             # max_inner_steps = 0: no z_ref scratch
+    try:
+        with pytest.raises(tts.TTSError) as e:
+            tts.tts_distill_inner_steps(ctx, t["teacher"], t["h"], t["W_in"], t["W_out"], t["master"], t["m"], t["v"],
+                                        t["pw"], None, case["T"], 1.0, 3, 0.5, None, losses)
+        assert e.value.status == tts.TTS_ERR_INVALID_ARG
+        # with the drafter's own logits as z_ref no scratch is needed
+        z = torch.from_numpy((O.widen(case["h"]) @ O.widen(case["W"]).T).astype(np.float32)).cuda()
+        tts.tts_distill_inner_steps(ctx, t["teacher"], t["h"], t["W_in"], t["W_out"], t["master"], t["m"], t["v"],
+                                    t["pw"], None, case["T"], 1.0, 3, 0.5, z, losses)
+        tts.tts_sync_step(ctx)
+        assert bool(torch.isfinite(losses).all()) and float(losses[0]) > 0
+    finally:
+        tts.tts_ctx_destroy(ctx)
+    ctx = tts.tts_ctx_create(config_for(case, max_inner_steps=3), 0)
+    try:
+        t = _buffers(case)
+        free0, _ = torch.cuda.mem_get_info()
+        tts.tts_distill_inner_steps(ctx, t["teacher"], t["h"], t["W_in"], t["W_out"], t["master"], t["m"], t["v"],
+                                    t["pw"], None, case["T"], 1.0, 3, 0.5, None, losses)
+        tts.tts_sync_step(ctx)
+        free1, _ = torch.cuda.mem_get_info()
+        assert free1 == free0, "a step call allocated device memory"
+    finally:
+        tts.tts_ctx_destroy(ctx)
+
+
+@pytest.mark.parametrize("V,d,n_seq", [(4096, 1024, 1), (4096 + 128, 256, 4), (2048, 512, 24)])
+@pytest.mark.parametrize("flag", [tts.TTS_FLAG_SEPARATE_GH, tts.TTS_FLAG_DETERMINISTIC])
+def test_gh_from_its_own_kernel_matches_oracle(V, d, n_seq, flag):
+    case = synth.make_case(4 if n_seq > 1 else 3, V=V, d=d, n_seq=n_seq)
+    g, o = run_gpu(case, flags=flag), run_oracle(case)
+    check_step(g, o, case)
+
+
+def test_separate_gh_reads_the_W_in_buffer():
+    """With TTS_FLAG_SEPARATE_GH a W_in that is NOT rn_bf16(master) still gives gh = dl . W_in (the default path would
+    contract against rn_bf16(master) instead: precondition 1)."""
+    case = synth.make_case(3, V=4096, d=1024)
+    rng = np.random.Generator(np.random.PCG64(3))
+    case["master"] = (case["master"] * (1.0 + 0.05 * rng.standard_normal(case["master"].shape))).astype(np.float32)
+    o = run_oracle(case)                       # the oracle's z and gh use W_in; its update starts from the master
+    g = run_gpu(case, flags=tts.TTS_FLAG_SEPARATE_GH)
+    assert max_abs(g["gh"] - o["gh"]) <= 2e-3 * max_abs(o["gh"])
+    assert abs(g["loss"] - o["loss"]) <= 1e-3 * abs(o["loss"]) + 1e-6
+    g0 = run_gpu(case)                         # default: gh from rn_bf16(master), visibly different here
+    assert max_abs(g0["gh"] - o["gh"]) > 2e-3 * max_abs(o["gh"])
+
+
+@pytest.mark.parametrize("V,d,n_seq", [(19072, 256, 32), (4096 + 384, 512, 32), (4096, 1024, 1), (8192, 256, 8)])
+def test_deterministic_mode_is_bit_reproducible(V, d, n_seq):
+    """Two runs of the same step give bit-identical loss, gh, master, m, v and W_out, including at 512 rows with a
+    vocabulary whose pair-tile count does not divide the number of CTA pairs (leftover tiles cut along K), which is
+    where the draft logits used to collect ~37 unordered fp32 addends per entry."""
+    case = synth.make_case(4 if n_seq > 1 else 3, V=V, d=d, n_seq=n_seq)
+    a = run_gpu(case, flags=tts.TTS_FLAG_DETERMINISTIC, want_gW=False)
+    for _ in range(2):
+        b = run_gpu(case, flags=tts.TTS_FLAG_DETERMINISTIC, want_gW=False)
+        assert a["loss"] == b["loss"]
+        for k in ("gh", "master", "m", "v", "W_out", "kl_rows"):
+            np.testing.assert_array_equal(a[k], b[k], err_msg=k)
+
+
+@pytest.mark.parametrize("V,d,n_seq", [(19072, 256, 32), (4096 + 384, 512, 32)])
+def test_default_mode_weights_are_bit_reproducible(V, d, n_seq):
+    """Without the flag only gh (fp32 RED from many CTAs) may differ between runs; z, the loss and every weight-state
+    tensor are order-free."""
+    case = synth.make_case(4, V=V, d=d, n_seq=n_seq)
+    a = run_gpu(case, want_gW=False)
+    b = run_gpu(case, want_gW=False)
+    assert a["loss"] == b["loss"]
+    for k in ("master", "m", "v", "W_out", "kl_rows"):
+        np.testing.assert_array_equal(a[k], b[k], err_msg=k)

@@ -15,7 +15,7 @@ pytestmark = pytest.mark.gpu
 
 
 def _setup(case, kernel_path=tts.TTS_PATH_AUTO):
-    ctx = tts.tts_ctx_create(config_for(case, kernel_path=kernel_path), 0)
+    ctx = tts.tts_ctx_create(config_for(case, kernel_path=kernel_path, max_inner_steps=8), 0)
     bf = case["cfg"]["param"] == synth.BF16
     t = dict(teacher=_dev(case["teacher"]), h=_dev(case["h"]), tok=_dev(case["draft_tokens"]), W_in=_dev(case["W"]),
              master=_dev(case["master"]) if bf else None, m=_dev(case["m"]), v=_dev(case["v"]),
