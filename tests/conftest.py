@@ -25,3 +25,18 @@ def pytest_collection_modifyitems(config, items):
     for it in items:
         if "gpu" in it.keywords:
             it.add_marker(skip)
+
+
+def pytest_sessionfinish(session, exitstatus):
+    """Observed parity figures of the GPU tests (tests/gpu_util.check_step) -> gpurun_out/parity_metrics.json, so that
+    the tolerances can be read against what was measured."""
+    try:
+        import json
+        import gpu_util
+        if gpu_util.METRICS:
+            out = os.path.join(ROOT, "gpurun_out")
+            os.makedirs(out, exist_ok=True)
+            with open(os.path.join(out, "parity_metrics.json"), "w") as f:
+                json.dump(gpu_util.METRICS, f, indent=1)
+    except Exception:
+        pass

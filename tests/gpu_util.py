@@ -96,6 +96,9 @@ def run_oracle(case, *, mask_mode=O.ROWS_ALL):
     return r
 
 
+METRICS = []   # observed error figures of every check_step call; conftest.py writes them to gpurun_out/ at session end
+
+
 def max_abs(x):
     return float(np.max(np.abs(x))) if x.size else 0.0
 
@@ -105,10 +108,13 @@ def check_step(g, o, case, *, fp32=False):
     fp32 accumulation: loss rel <= 1e-3, gW / gh / weights max abs err <= 2e-3 * max|ref|) or, for the
     fp32 configuration, R21 (1e-5).  Mask, tau and argmax are bit-exact."""
     c = case["cfg"]
+    obs = dict(V=case["V"], d=case["d"], T=case["T"], step=case.get("step", 1))
+    METRICS.append(obs)
     np.testing.assert_array_equal(g["mask"], o["mask"])
     np.testing.assert_array_equal(g["tau"], o["tau"])
     np.testing.assert_array_equal(g["argmax"], o["argmax"])
     rel, aabs, tol = (1e-5, 1e-9, 1e-5) if fp32 else (1e-3, 1e-6, 2e-3)
+    obs["loss_rel"] = abs(g["loss"] - o["loss"]) / max(abs(o["loss"]), 1e-30)
     assert abs(g["loss"] - o["loss"]) <= rel * abs(o["loss"]) + aabs, (g["loss"], o["loss"])
     klt = rel * np.abs(o["kl_rows"]) + max(aabs, 1e-6 if not fp32 else 1e-7) * 10
     assert np.all(np.abs(g["kl_rows"] - o["kl_rows"]) <= klt), (g["kl_rows"], o["kl_rows"])
@@ -118,6 +124,7 @@ def check_step(g, o, case, *, fp32=False):
         ref = o[name]
         err = max_abs(g[name].astype(np.float64) - ref)
         assert np.all(np.isfinite(g[name])), name
+        obs[name + "_err_over_max"] = err / max(max_abs(ref), 1e-300)
         assert err <= tol * max_abs(ref) + 1e-30, (name, err, max_abs(ref))
     # the update itself (R13): Delta M on elements with a sizeable gradient, and its sign everywhere
     M_old = O.widen(case["master"]) if case["master"] is not None else O.widen(case["W"])
@@ -129,10 +136,13 @@ def check_step(g, o, case, *, fp32=False):
         if big.any():
             # fp32 master: one ulp of |M| ~ 0.1 is 7.5e-9, comparable to lr = 1e-5 * 0.02
             ulp = np.spacing(np.abs(M_old[big]).astype(np.float32)).astype(np.float64)
+            obs["dM_big_err_over_lr"] = float(np.max(np.abs(d_gpu[big] - d_ref[big]) - ulp)) / lr
             assert np.all(np.abs(d_gpu[big] - d_ref[big]) <= 0.02 * lr + ulp)
         moved = np.abs(d_ref) > 4 * np.spacing(np.abs(M_old).astype(np.float32)).astype(np.float64)
         if moved.any():
             bad = np.sign(d_gpu[moved]) != np.sign(d_ref[moved])
+            obs["dM_sign_mismatch_frac"] = float(bad.mean())
+            obs["dM_all_err_over_lr"] = float(np.max(np.abs(d_gpu - d_ref))) / lr
             assert bad.mean() <= 1e-3, bad.mean()
     else:
         assert max_abs(d_gpu - d_ref) <= tol * lr * max_abs(o["gW"]) + float(np.spacing(np.float32(max_abs(M_old))))
@@ -148,4 +158,6 @@ def check_step(g, o, case, *, fp32=False):
         ulp = 2.0 ** (np.floor(np.log2(mag)) - 7)
         assert np.all(np.abs(wg - wo) <= ulp + np.abs(g["master"].astype(np.float64) - o["master"]))
         diff = np.abs(g["W_out"].astype(np.int32) - o["W_out"].astype(np.int32))
+        obs["W_out_gt1ulp_frac"] = float((diff > 1).mean())
+        obs["W_out_ne_frac"] = float((diff > 0).mean())
         assert (diff > 1).mean() <= 1e-4

@@ -18,8 +18,9 @@ pytestmark = pytest.mark.gpu
 ROUNDS = 48
 
 
-def _oracle_stream(case0, rounds, stride):
+def _oracle_stream(case0, rounds, stride, checkpoints=()):
     c = case0["cfg"]
+    snaps = {}
     W, M, m, v = case0["W"], case0["master"].astype(np.float64), case0["m"].astype(np.float64), case0["v"].astype(np.float64)
     losses, taus, n = [], [], 0
     for t, rd in enumerate(rounds):
@@ -33,7 +34,9 @@ def _oracle_stream(case0, rounds, stride):
         W, M, m, v = r["W_out"], r["master"], r["m"], r["v"]
         losses.append(r["loss"])
         taus.append(int(tau[0]))
-    return dict(W=W, master=M, m=m, v=v, losses=np.array(losses), taus=taus, updates=n)
+        if n in checkpoints:
+            snaps[n] = dict(master=M.copy(), m=m.copy(), v=v.copy())
+    return dict(W=W, master=M, m=m, v=v, losses=np.array(losses), taus=taus, updates=n, snaps=snaps)
 
 
 @pytest.mark.parametrize("stride,host_barrier,use_graph", [(1, False, False), (3, False, False), (4, True, False),
@@ -86,6 +89,54 @@ def test_stream_matches_oracle_round_by_round(stride, host_barrier, use_graph):
         np.testing.assert_array_equal(master.cpu().numpy(), case0["master"])
         assert float(m.abs().max()) == 0.0 and float(v.abs().max()) == 0.0
         assert tts.tts_get_step_count(up.ctx) == 0 and up.round == 0
+    finally:
+        up.close()
+
+
+@pytest.mark.parametrize("d", [256, 1024])
+def test_300_round_stream_drift_stays_bounded(d):
+    """SURVEY 8(d), config 5 scaled down (V = 4096, 300 rounds; d = 256 takes the wide update kernel, d = 1024 the
+    one-canvas stripe kernel): the regime the paper describes is thousands of rounds on one sequence, so
+    the GPU stream is compared with the oracle's round by round -- the loss of EVERY round, and at every 50th update
+    the whole state with a tolerance that grows with the number of updates n:
+        max |M_gpu - M_ref| <= 0.05 lr n   (each side moves at most ~lr per step; conditioned elements agree to 2% of lr
+                                            per step, ill-conditioned ones random-walk)
+        mean |dM_gpu - dM_ref| <= 0.02 mean |dM_ref|,   m and v at 2e-3 max|ref|."""
+    V, rounds_n = 4096, 300
+    case0, rounds = synth.make_stream(V=V, d=d, rounds=rounds_n)
+    cps = tuple(range(50, rounds_n + 1, 50))
+    o = _oracle_stream(case0, rounds, 1, checkpoints=cps)
+    c = case0["cfg"]
+    lr = c["lr"]
+    W0, master, m, v = _dev(case0["W"]), _dev(case0["master"]), _dev(case0["m"]), _dev(case0["v"])
+    pw = _dev(case0["pos_weight"])
+    up = DraftHeadUpdater(W0, master, m, v, seg_len=16, T_max=16, stride=1, lr=lr, beta1=c["beta1"], beta2=c["beta2"],
+                          eps=c["eps"], weight_decay=c["weight_decay"])
+    M0 = case0["master"].astype(np.float64)
+    try:
+        worst = []
+        for t, r in enumerate(rounds):
+            rd = (_dev(r["teacher"]), _dev(r["h"]), _dev(r["draft_tokens"]))   # alive until the step is done (R17)
+            up.on_round_end(rd[0], rd[1], rd[2], pw, 16)
+            tts.tts_sync_step(up.ctx)
+            loss = float(up.loss.item())
+            assert abs(loss - o["losses"][t]) <= 1e-3 * abs(o["losses"][t]) + 1e-6, (t, loss, o["losses"][t])
+            assert int(up.tau[0].item()) == o["taus"][t]
+            n = t + 1
+            if n in cps:
+                torch.cuda.synchronize()
+                ref = o["snaps"][n]
+                g_master = master.cpu().numpy().astype(np.float64)
+                err = max_abs(g_master - ref["master"])
+                worst.append((n, err / lr))
+                assert err <= 0.05 * lr * n, (n, err / lr)
+                d_ref, d_gpu = ref["master"] - M0, g_master - M0
+                assert np.abs(d_gpu - d_ref).mean() <= 0.02 * np.abs(d_ref).mean(), n
+                for name, gg in (("m", m), ("v", v)):
+                    assert max_abs(gg.cpu().numpy().astype(np.float64) - ref[name]) <= 2e-3 * max_abs(ref[name]), (name, n)
+        assert tts.tts_get_step_count(up.ctx) == rounds_n
+        np.testing.assert_array_equal(bits(up.weights()), O.f32_to_bf16_bits(master.cpu().numpy()))
+        print("max |M_gpu - M_ref| / lr at updates", worst)
     finally:
         up.close()
 

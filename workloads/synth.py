@@ -97,12 +97,15 @@ def make_case(cfg_id: int, *, V: int | None = None, d: int | None = None, n_seq:
     scaled down (V, d, n_seq, seg_len overrides keep the recipe).  Returns a dict of
     numpy arrays (bf16 as uint16 bits) plus the hyper-parameters.
 
-    nonzero_state: draw Adam moments as if ``step-1`` steps had happened instead of the configs'
-    m = v = 0, to exercise the general update: v ~ 1e-10 chi^2, m = sqrt(v) U(-3, 3).  The pair is drawn
-    so that it CAN be an Adam state: moments that are exponential averages of one gradient sequence
-    satisfy m^2 <= (1-b1)^2 / ((1-b2) (1 - b1^2/b2)) v = 52.8 v (Cauchy-Schwarz, b = 0.9 / 0.999).  Independent
-    draws of m and v do not (|m| / sqrt(v) is Cauchy-tailed), and where m^2 >> v the step is hundreds of lr and
-    ill-conditioned in g: a regime no run of the optimiser reaches (R12).
+    nonzero_state: draw Adam moments as if earlier steps had happened instead of the configs' m = v = 0, to exercise
+    the general update.  Every recipe stays inside the set an optimiser run can reach: moments that are exponential
+    averages of ONE gradient sequence satisfy m^2 <= (1-b1)^2 / ((1-b2) (1 - b1^2/b2)) v = 52.8 v (Cauchy-Schwarz,
+    b = 0.9 / 0.999), i.e. |m| / sqrt(v) <= 7.27 (R12); independent draws of m and v do not.
+        True / "mix"   element (v, j) takes recipe (v + j) % 4 of: "uniform", "const2", "const10", "const1000"
+        "uniform"      v ~ 1e-10 chi^2,  m = sqrt(v) U(-7.2, 7.2): the whole reachable band of |m| / sqrt(v)
+        "const<n>"     the state after n steps of a CONSTANT gradient g0 ~ 1e-5 N(0,1) (the most ordinary Adam
+                       state): m = g0 (1 - b1^n), v = g0^2 (1 - b2^n); |m| / sqrt(v) = 4.25 / 6.52 / 1.26 at
+                       n = 2 / 10 / 1000.  Pass step = n + 1 for the matching bias corrections.
     """
     c = dict(CONFIGS[cfg_id])
     c.update(ADAM_DEFAULTS)
@@ -170,15 +173,42 @@ def make_case(cfg_id: int, *, V: int | None = None, d: int | None = None, n_seq:
         out["master"] = None
     if c["optimizer"] == ADAMW:
         if nonzero_state:
-            rs = np.random.Generator(np.random.PCG64(c["seed"] + 77))
-            out["v"] = (1e-10 * rs.standard_normal((V, d), dtype=np.float32) ** 2).astype(np.float32)
-            out["m"] = (np.sqrt(out["v"]) * rs.uniform(-3.0, 3.0, (V, d)).astype(np.float32)).astype(np.float32)
+            out["m"], out["v"] = adam_state(V, d, "mix" if nonzero_state is True else nonzero_state, c["seed"] + 77,
+                                            c["beta1"], c["beta2"])
         else:
             out["m"] = np.zeros((V, d), dtype=np.float32)
             out["v"] = np.zeros((V, d), dtype=np.float32)
     else:
         out["m"] = out["v"] = None
     return out
+
+
+def adam_state(V: int, d: int, kind: str, seed: int, beta1: float = 0.9, beta2: float = 0.999):
+    """Non-zero Adam moments (m, v) of the recipes documented at make_case (all inside |m| / sqrt(v) <= 7.27)."""
+    rs = np.random.Generator(np.random.PCG64(seed))
+
+    def uniform():
+        v = (1e-10 * rs.standard_normal((V, d), dtype=np.float32) ** 2).astype(np.float32)
+        m = (np.sqrt(v) * rs.uniform(-7.2, 7.2, (V, d)).astype(np.float32)).astype(np.float32)
+        return m, v
+
+    def const(n):
+        g0 = (1e-5 * rs.standard_normal((V, d), dtype=np.float32)).astype(np.float64)
+        return ((g0 * (1.0 - beta1 ** n)).astype(np.float32), (g0 * g0 * (1.0 - beta2 ** n)).astype(np.float32))
+
+    if kind == "uniform":
+        return uniform()
+    if kind.startswith("const"):
+        return const(int(kind[5:]))
+    assert kind == "mix", kind
+    parts = [uniform(), const(2), const(10), const(1000)]
+    sel = (np.arange(V)[:, None] + np.arange(d)[None, :]) % 4
+    m = np.empty((V, d), dtype=np.float32)
+    v = np.empty((V, d), dtype=np.float32)
+    for k, (pm, pv) in enumerate(parts):
+        m[sel == k] = pm[sel == k]
+        v[sel == k] = pv[sel == k]
+    return m, v
 
 
 def stream_direction(V: int, seed: int = 4) -> np.ndarray:
