@@ -33,6 +33,11 @@ What it computes, with the passage each step follows
                           rows, given the full-vocabulary normalisers, so that a
                           full-size configuration can be checked on samples.
 
+  * ``adamw_update_lowp`` the same Adam step with the moments STORED in bf16 (f4, an opt-in variant; the paper fixes
+                          only "Adam"): dequantise -> update in full precision -> requantise, m by
+                          round-to-nearest-even, v by stochastic rounding with the counter-based bits of
+                          ``sr_bits16`` (R26).
+
   * ``shard_row_stats`` / ``merge_shard_stats``  the per-row online tuple (m_t, s_t, a, m_z, s_z) over a slice of
                           the vocabulary and its associative merge: what vocabulary shards exchange (SURVEY 8(e));
                           pinned against the plain logsumexp / KL of the whole row.
@@ -283,6 +288,60 @@ def adamw_update(M, m, v, g, step, lr, beta1, beta2, eps, weight_decay):
     return M_new, m_new, v_new
 
 
+# ----------------------------------------------------------------------------
+# f4: Adam with low-precision moment storage (R26; PAPER.md:393 names only "Adam")
+# ----------------------------------------------------------------------------
+
+def sr_bits16(idx, step, seed):
+    """16 pseudo-random bits per element for stochastic rounding: a counter-based generator, so that the GPU and the
+    oracle draw the same bits without exchanging them (each side implements it on its own).  Key: the element's
+    linear index idx = v * d + j (64-bit), Adam's count n of the step being taken, a caller seed.
+
+        x = lo32(idx) ^ (n * 0x9E3779B9) ^ (seed * 0x85EBCA6B) ^ (hi32(idx) * 0xC2B2AE35)        (mod 2^32)
+        x ^= x >> 16;  x *= 0x7FEB352D;  x ^= x >> 15;  x *= 0x846CA68B;  x ^= x >> 16           (an integer mixer)
+        bits = x >> 16
+    """
+    idx = np.asarray(idx, dtype=np.uint64)
+    m32 = np.uint64(0xFFFFFFFF)
+    lo = idx & m32
+    hi = idx >> np.uint64(32)
+    x = lo ^ ((np.uint64(step) * np.uint64(0x9E3779B9)) & m32) ^ ((np.uint64(seed) * np.uint64(0x85EBCA6B)) & m32) \
+        ^ ((hi * np.uint64(0xC2B2AE35)) & m32)
+    x ^= x >> np.uint64(16)
+    x = (x * np.uint64(0x7FEB352D)) & m32
+    x ^= x >> np.uint64(15)
+    x = (x * np.uint64(0x846CA68B)) & m32
+    x ^= x >> np.uint64(16)
+    return (x >> np.uint64(16)).astype(np.uint32)
+
+
+def f32_to_bf16_bits_sr(x, r16):
+    """Stochastic rounding fp32 -> bf16 with 16 random bits r per element: the 16 discarded mantissa bits f of x
+    round up with probability f / 65536 (up iff f + r >= 65536), so that E_r[result] = x exactly for uniform r."""
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    u = x.view(np.uint32).astype(np.uint64)
+    return ((u + np.asarray(r16, dtype=np.uint64)) >> np.uint64(16)).astype(np.uint16)
+
+
+def adamw_update_lowp(M, m_bits, v_bits, g, step, lr, beta1, beta2, eps, weight_decay, *, idx, seed):
+    """Adam (conventions of ``adamw_update``, R5) with m and v STORED as bf16 (R26):
+
+      1. dequantise        m = widen(m_bits), v = widen(v_bits)                      (exact)
+      2. update            M, m_new, v_new exactly as adamw_update: the parameter step uses the UNROUNDED m_new, v_new
+      3. requantise        m_bits' = rn_bf16(rn_fp32(m_new))                         round to nearest even
+                           v_bits' = sr_bf16(rn_fp32(v_new), sr_bits16(idx, step, seed))   stochastic rounding:
+                           beta2 = 0.999 decays v by 0.1% per step, below half a bf16 ulp (0.2-0.4%), so nearest
+                           rounding would freeze v whenever g^2 << v; stochastic rounding keeps E[v] exact.
+    The quantisation decisions are taken on the fp32 value (the precision the kernel computes in).
+    Returns (M_new fp64, m_bits' uint16, v_bits' uint16, m_new fp64, v_new fp64)."""
+    m = bf16_bits_to_f64(m_bits)
+    v = bf16_bits_to_f64(v_bits)
+    M_new, m_new, v_new = adamw_update(M, m, v, g, step, lr, beta1, beta2, eps, weight_decay)
+    m_q = f32_to_bf16_bits(m_new.astype(np.float32))
+    v_q = f32_to_bf16_bits_sr(v_new.astype(np.float32), sr_bits16(idx, step, seed))
+    return M_new, m_q, v_q, m_new, v_new
+
+
 def working_copy_bits(M_new):
     """bf16 working copy = rn_bf16(rn_fp32(M_new)): the GPU's master is fp32."""
     return f32_to_bf16_bits(np.asarray(M_new, dtype=np.float64).astype(np.float32))
@@ -295,8 +354,12 @@ def working_copy_bits(M_new):
 def distill_step(teacher_logits, h, W_in, W_master, adam_m, adam_v, pos_weight, mask,
                  *, seg_len, mask_mode=ROWS_ALL, loss_scale=1.0, optimizer="adamw",
                  lr=1e-5, beta1=0.9, beta2=0.999, eps=1e-8, weight_decay=0.0, step=1,
-                 draft_logits=None, lam=0.0, z_ref=None):
+                 draft_logits=None, lam=0.0, z_ref=None, moments="f32", sr_seed=0):
     """One TTS update (Alg. 1 lines 'Loss' + 'Update'), dense.
+
+    moments      : "f32" (default) or "bf16": adam_m / adam_v are uint16 bf16 bit patterns, updated by
+                   ``adamw_update_lowp`` (the element index of W[v, j] is v * d + j); the result then also carries
+                   ``m_bits`` / ``v_bits`` (what is stored) next to the unrounded ``m`` / ``v``
 
     draft_logits : the drafter's logits z, taken as given instead of h W_in^T
     lam, z_ref   : the regulariser lam * K~L(q_t || q) with q_t = softmax(z_ref)
@@ -312,11 +375,18 @@ def distill_step(teacher_logits, h, W_in, W_master, adam_m, adam_v, pos_weight, 
     if optimizer == "sgd":
         M_new = sgd_update(M, r["gW"], lr)
         m_new = v_new = None
+    elif moments == "bf16":
+        V_, d_ = M.shape
+        idx = np.arange(V_, dtype=np.uint64)[:, None] * np.uint64(d_) + np.arange(d_, dtype=np.uint64)[None, :]
+        M_new, m_q, v_q, m_new, v_new = adamw_update_lowp(M, adam_m, adam_v, r["gW"], step, lr, beta1, beta2, eps,
+                                                          weight_decay, idx=idx, seed=sr_seed)
     else:
         M_new, m_new, v_new = adamw_update(M, widen(adam_m), widen(adam_v), r["gW"], step,
                                            lr, beta1, beta2, eps, weight_decay)
     out = dict(r)
     out.update(omega=omega, master=M_new, m=m_new, v=v_new)
+    if optimizer != "sgd" and moments == "bf16":
+        out.update(m_bits=m_q, v_bits=v_q)
     if W_master is not None:
         out["W_out"] = working_copy_bits(M_new)
     else:
@@ -368,7 +438,7 @@ def row_normalisers(teacher_logits, h, W_in, slab=8192):
 
 def distill_step_rows(rows, z, lse_t, lse_z, teacher_logits, h, W_in_rows, W_master_rows,
                       adam_m_rows, adam_v_rows, omega, *, loss_scale=1.0, optimizer="adamw",
-                      lr=1e-5, beta1=0.9, beta2=0.999, eps=1e-8, weight_decay=0.0, step=1):
+                      lr=1e-5, beta1=0.9, beta2=0.999, eps=1e-8, weight_decay=0.0, step=1, moments="f32", sr_seed=0):
     """The step for the vocabulary rows ``rows`` only (gW rows, updated state),
     given the full-vocabulary normalisers from ``row_normalisers``."""
     t = widen(teacher_logits)[:, rows]
@@ -379,12 +449,20 @@ def distill_step_rows(rows, z, lse_t, lse_z, teacher_logits, h, W_in_rows, W_mas
     dl = loss_scale * om[:, None] * (q - p)
     gW = dl.T @ hh
     M = widen(W_master_rows) if W_master_rows is not None else widen(W_in_rows)
+    out = {}
     if optimizer == "sgd":
         M_new, m_new, v_new = sgd_update(M, gW, lr), None, None
+    elif moments == "bf16":
+        d_ = M.shape[1]
+        idx = np.asarray(rows, dtype=np.uint64)[:, None] * np.uint64(d_) + np.arange(d_, dtype=np.uint64)[None, :]
+        M_new, m_q, v_q, m_new, v_new = adamw_update_lowp(M, adam_m_rows, adam_v_rows, gW, step, lr, beta1, beta2, eps,
+                                                          weight_decay, idx=idx, seed=sr_seed)
+        out.update(m_bits=m_q, v_bits=v_q)
     else:
         M_new, m_new, v_new = adamw_update(M, widen(adam_m_rows), widen(adam_v_rows), gW, step,
                                            lr, beta1, beta2, eps, weight_decay)
-    return dict(dl=dl, gW=gW, master=M_new, m=m_new, v=v_new)
+    out.update(dl=dl, gW=gW, master=M_new, m=m_new, v=v_new)
+    return out
 
 
 def gh_full(z, lse_t, lse_z, teacher_logits, W_in, omega, loss_scale=1.0, slab=8192):

@@ -547,3 +547,135 @@ def test_shard_tuples_merge_to_the_whole_row_normalisers():
     q = np.exp(z[r]) / np.exp(z[r]).sum()
     kl_lit = sum(p[v] * (np.log(p[v]) - np.log(q[v])) for v in range(V) if p[v] > 0)
     assert abs(kl[r] - kl_lit) < 1e-12
+
+
+# ----------------------------------------------------------------------------
+# f4: Adam with bf16 moment storage (R26).  Pins of adamw_update_lowp / sr_bits16 / f32_to_bf16_bits_sr
+# ----------------------------------------------------------------------------
+
+def _bf16_bits_py(x):
+    """fp32 -> (bits of the bf16 at or below |x|, the 16 discarded bits), through struct: independent of numpy views."""
+    import struct
+    u = struct.unpack("<I", struct.pack("<f", x))[0]
+    return u >> 16, u & 0xFFFF
+
+
+def _bf16_val_py(b):
+    import struct
+    return struct.unpack("<f", struct.pack("<I", (b & 0xFFFF) << 16))[0]
+
+
+def test_stochastic_rounding_is_exactly_unbiased_over_all_16_bit_draws():
+    """E_r[sr(x, r)] = x EXACTLY when r runs over all 65536 values: the discarded fraction f rounds up for exactly f of
+    them.  Also: every result is one of the two bf16 neighbours of x, and r = 0 truncates."""
+    rs = np.arange(65536, dtype=np.uint32)
+    for x in (1.2345678, 3.0e-11, 0.999, 65504.0, -0.3333333, 1.0, 7.0e-39):
+        x32 = np.float32(x)
+        q = O.f32_to_bf16_bits_sr(np.full(65536, x32, dtype=np.float32), rs)
+        vals = O.bf16_bits_to_f64(q)
+        lo_bits, f = _bf16_bits_py(float(x32))
+        lo, hi = _bf16_val_py(lo_bits), _bf16_val_py(lo_bits + 1)
+        assert set(np.unique(q).tolist()) <= {lo_bits, lo_bits + 1}
+        assert int((q == lo_bits + 1).sum()) == f                     # rounds away from zero for exactly f draws
+        assert q[0] == lo_bits
+        assert vals.mean() == pytest.approx(float(x32), rel=1e-15, abs=0.0) or f == 0
+        # mean = lo + (hi - lo) f / 65536 = x, term by term
+        assert lo + (hi - lo) * f / 65536.0 == pytest.approx(float(x32), rel=1e-15)
+
+
+def test_sr_bits_are_uniform_and_decorrelated():
+    """The counter-based generator has no paper value to hit; what the method needs from it is uniform 16-bit draws that
+    are independent across elements, steps and seeds."""
+    n = 1 << 20
+    idx = np.arange(n, dtype=np.uint64)
+    a = O.sr_bits16(idx, 1, 0).astype(np.float64)
+    assert a.min() >= 0 and a.max() <= 65535
+    assert abs(a.mean() - 32767.5) < 4 * 18918.0 / np.sqrt(n)        # sd of U{0..65535} = 18918
+    counts = np.bincount((a.astype(np.int64) >> 8), minlength=256)    # chi-square over the top byte
+    chi2 = ((counts - n / 256.0) ** 2 / (n / 256.0)).sum()
+    assert chi2 < 255 + 6 * np.sqrt(2 * 255)
+    for bit in range(16):                                             # every bit is fair
+        assert abs(((a.astype(np.int64) >> bit) & 1).mean() - 0.5) < 4 * 0.5 / np.sqrt(n)
+    b = O.sr_bits16(idx, 2, 0).astype(np.float64)                     # next step, same elements
+    c = O.sr_bits16(idx, 1, 1).astype(np.float64)                     # another seed
+    d = O.sr_bits16(idx + np.uint64(1), 1, 0).astype(np.float64)      # neighbouring elements
+    e = O.sr_bits16(idx + np.uint64(1 << 32), 1, 0).astype(np.float64)  # beyond 2^32 elements: the high word counts
+    for other in (b, c, d, e):
+        assert abs(np.corrcoef(a, other)[0, 1]) < 5.0 / np.sqrt(n)
+        assert (a == other).mean() < 4.0 / 65536
+
+
+def test_lowp_adam_matches_a_scalar_loop_in_the_stated_order():
+    """dequantise -> update with the unrounded moments -> requantise (m nearest-even, v stochastic), element by element
+    in plain Python floats with struct-based bf16 conversions."""
+    rng = np.random.Generator(np.random.PCG64(31))
+    V, d = 7, 5
+    M = rng.standard_normal((V, d)) * 0.02
+    g = rng.standard_normal((V, d)) * 1e-3
+    m_bits = O.f32_to_bf16_bits((rng.standard_normal((V, d)) * 1e-4).astype(np.float32))
+    v_bits = O.f32_to_bf16_bits((rng.standard_normal((V, d)) ** 2 * 1e-8).astype(np.float32))
+    idx = np.arange(V, dtype=np.uint64)[:, None] * np.uint64(d) + np.arange(d, dtype=np.uint64)[None, :]
+    lr, b1, b2, eps, wd, n, seed = 1e-3, 0.9, 0.999, 1e-8, 0.01, 4, 9
+    Mn, mq, vq, m_new, v_new = O.adamw_update_lowp(M, m_bits, v_bits, g, n, lr, b1, b2, eps, wd, idx=idx, seed=seed)
+    bits = O.sr_bits16(idx, n, seed)
+    for i in range(V):
+        for j in range(d):
+            m0, v0 = _bf16_val_py(int(m_bits[i, j])), _bf16_val_py(int(v_bits[i, j]))
+            Mw = M[i, j] * (1.0 - lr * wd)
+            m1 = b1 * m0 + (1.0 - b1) * g[i, j]
+            v1 = b2 * v0 + (1.0 - b2) * g[i, j] * g[i, j]
+            want = Mw - lr * (m1 / (1.0 - b1 ** n)) / ((v1 / (1.0 - b2 ** n)) ** 0.5 + eps)
+            assert Mn[i, j] == pytest.approx(want, rel=1e-13)
+            assert m_new[i, j] == pytest.approx(m1, rel=1e-14) and v_new[i, j] == pytest.approx(v1, rel=1e-14)
+            # m: nearest even on the fp32 value
+            lo_b, f = _bf16_bits_py(float(np.float32(m1)))
+            up = f > 0x8000 or (f == 0x8000 and (lo_b & 1))
+            assert int(mq[i, j]) == lo_b + (1 if up else 0)
+            # v: up iff the discarded bits plus the element's draw carry
+            lo_b, f = _bf16_bits_py(float(np.float32(v1)))
+            assert int(vq[i, j]) == lo_b + (1 if f + int(bits[i, j]) >= 65536 else 0)
+
+
+def test_lowp_v_decays_in_expectation_where_nearest_rounding_freezes():
+    """Why v is rounded stochastically: with zero gradients v must decay as beta2^n.  Nearest rounding leaves a bf16 v
+    unchanged for ever (0.1% per step is below half an ulp); the stochastic rule follows beta2^n in the mean."""
+    nel, steps, b2 = 20000, 200, 0.999
+    idx = np.arange(nel, dtype=np.uint64)[None, :]
+    v0 = np.full((1, nel), 1.0e-6, dtype=np.float32)
+    v_bits = O.f32_to_bf16_bits(v0)
+    v_rne = v_bits.copy()
+    m_bits = np.zeros((1, nel), dtype=np.uint16)
+    M = np.zeros((1, nel))
+    g = np.zeros((1, nel))
+    start = O.bf16_bits_to_f64(v_bits).mean()
+    for n in range(1, steps + 1):
+        _, m_bits, v_bits, _, _ = O.adamw_update_lowp(M, m_bits, v_bits, g, n, 1e-5, 0.9, b2, 1e-8, 0.0, idx=idx, seed=3)
+        v_rne = O.f32_to_bf16_bits((b2 * O.bf16_bits_to_f64(v_rne)).astype(np.float32))
+    got = O.bf16_bits_to_f64(v_bits).mean() / start
+    assert got == pytest.approx(b2 ** steps, rel=5e-3)               # 0.8186
+    assert O.bf16_bits_to_f64(v_rne).mean() / start == 1.0            # frozen
+
+
+def test_lowp_step_uses_unrounded_moments_for_the_parameter_update():
+    from workloads import synth
+    c = synth.make_case(3, V=384, d=64, nonzero_state="mix", step=5)
+    mask, _, _ = O.accept_mask(c["teacher"], c["draft_tokens"], c["seg_len"])
+    mb, vb = O.f32_to_bf16_bits(c["m"]), O.f32_to_bf16_bits(c["v"])
+    kw = dict(seg_len=c["seg_len"], lr=1e-5, step=5)
+    lo = O.distill_step(c["teacher"], c["h"], c["W"], c["master"], mb, vb, c["pos_weight"], mask, moments="bf16",
+                        sr_seed=1, **kw)
+    hi = O.distill_step(c["teacher"], c["h"], c["W"], c["master"], O.bf16_bits_to_f64(mb), O.bf16_bits_to_f64(vb),
+                        c["pos_weight"], mask, **kw)
+    np.testing.assert_array_equal(lo["master"], hi["master"])          # same dequantised moments in, same step out
+    np.testing.assert_array_equal(lo["m"], hi["m"])
+    # what is stored lies within one bf16 ulp of the unrounded moments (half an ulp for m)
+    m_err = np.abs(O.bf16_bits_to_f64(lo["m_bits"]) - lo["m"])
+    v_err = np.abs(O.bf16_bits_to_f64(lo["v_bits"]) - lo["v"])
+    assert np.all(m_err <= 2.0 ** -8 * np.abs(lo["m"]) + 1e-45)
+    assert np.all(v_err <= 2.0 ** -7 * np.abs(lo["v"]) + 1e-45)
+    rows = np.array([3, 100, 383])
+    z, lse_t, lse_z, _ = O.row_normalisers(c["teacher"], c["h"], c["W"])
+    part = O.distill_step_rows(rows, z, lse_t, lse_z, c["teacher"], c["h"], c["W"][rows], c["master"][rows], mb[rows],
+                               vb[rows], lo["omega"], lr=1e-5, step=5, moments="bf16", sr_seed=1)
+    np.testing.assert_array_equal(part["v_bits"], lo["v_bits"][rows])   # the draws are keyed by the GLOBAL element index
+    np.testing.assert_array_equal(part["m_bits"], lo["m_bits"][rows])
