@@ -62,6 +62,9 @@ def parse_args():
     ap.add_argument("--n-seq", type=int, default=0,
                     help="override the number of concurrent sequences (rows = 16 x n_seq <= 512): the T-scaling of the "
                          "batched shape between BASELINE configs[2] (1 sequence) and configs[3] (32)")
+    ap.add_argument("--moments", default="f32", choices=["f32", "bf16"],
+                    help="storage format of Adam's moments: f32 (every BASELINE.json configuration) or the opt-in bf16 "
+                         "variant (TTS_MOMENT_BF16, SURVEY 8(f) f4: 20 instead of 28 bytes per parameter per step)")
     ap.add_argument("--max-ctas", type=int, default=0,
                     help="SM budget of the step's persistent kernels (tts_config.max_ctas; 0 = all SMs): what the main "
                          "stream keeps while the update overlaps it (PAPER.md:426)")
@@ -107,9 +110,9 @@ def profiled_traffic(cfg_id):
     return None
 
 
-def algorithmic_bytes(V, d, T, adam=True):
+def algorithmic_bytes(V, d, T, adam=True, moments="f32"):
     """SURVEY.md 8(d) / DESIGN.md "Algorithmic bytes": what the method must move per step."""
-    state = 12 if adam else 4                      # fp32 master (+ m, v)
+    state = (12 if moments == "f32" else 8) if adam else 4     # fp32 master (+ m, v in fp32 or bf16)
     step = V * d * (2 + state + state + 2)         # bf16 W read once, state read+written once, bf16 W written once
     step += T * V * 2 + T * d * 2 + T * d * 4      # teacher logits, h, gh
     update_kernel = V * d * (state + state + 2) + T * V * 2 + T * d * 2   # a6+a7 launch alone
@@ -173,8 +176,8 @@ def host_sample(case, rows):
     """The first ``rows`` vocabulary rows of a device case, as the oracle's numpy inputs."""
     Vs = min(rows, case["V"])
     return dict(teacher=_np_bits(case["teacher"][:, :Vs]), h=_np_bits(case["h"]), W=_np_bits(case["W"][:Vs]),
-                master=case["master"][:Vs].cpu().numpy(), m=case["m"][:Vs].cpu().numpy(),
-                v=case["v"][:Vs].cpu().numpy(), tok=case["draft_tokens"].cpu().numpy(),
+                master=case["master"][:Vs].cpu().numpy(), m=case["m"][:Vs].float().cpu().numpy(),
+                v=case["v"][:Vs].float().cpu().numpy(), tok=case["draft_tokens"].cpu().numpy(),
                 pw=case["pos_weight"].cpu().numpy(), Vs=Vs)
 
 
@@ -356,7 +359,10 @@ def run_ours(args, rank, world, local_rank):
     V, d, T, C = case["V"], case["d"], case["T"], case["seg_len"]
     kpath = tts.TTS_PATH_AUTO if args.kernel_path == "auto" else tts.TTS_PATH_SIMT
     cfg = tts.make_config(V, d, T, C, tts.TTS_BF16, tts.TTS_BF16, tts.TTS_ADAMW, c["lr"], c["beta1"], c["beta2"],
-                          c["eps"], c["weight_decay"], tts.TTS_ROWS_ALL, args.max_ctas, kpath)
+                          c["eps"], c["weight_decay"], tts.TTS_ROWS_ALL, args.max_ctas, kpath,
+                          moment_dtype=tts.TTS_MOMENT_BF16 if args.moments == "bf16" else tts.TTS_MOMENT_F32)
+    if args.moments == "bf16":
+        case["m"], case["v"] = case["m"].to(torch.bfloat16), case["v"].to(torch.bfloat16)
     shard = sharded.VocabShardedStep(cfg, v0, local_rank) if vocab else None
     ctx = shard.ctx if vocab else tts.tts_ctx_create(cfg, local_rank)
     W = [case["W"], torch.empty_like(case["W"])]        # W_in / W_out double buffer, swapped at the barrier (R18)
@@ -461,7 +467,7 @@ def run_ours(args, rank, world, local_rank):
         scale = V / sample["Vs"]
         sampled = {"value": 1.0 / (sec * scale), "sample": "vocabulary rows 0..%d of %d (full d=%d, T=%d): %.2f s, "
                    "scaled by %.1f (an extrapolation)" % (sample["Vs"], V, d, T, sec, scale)}
-        if T <= 64 and not args.cpu_sampled_only:
+        if T <= 64 and not args.cpu_sampled_only and args.moments == "f32":
             # the inputs of the step the GPU just timed would need its PRE-step state; the oracle's time does not
             # depend on the values, so it runs on the state as it is now (same shapes, same bits the GPU holds)
             full_s, _ = oracle_full_step(case, host_full(case))
@@ -483,7 +489,7 @@ def run_ours(args, rank, world, local_rank):
     sps = (1 if vocab else world) * 1e3 / ms_step          # shards: all ranks together take ONE step
     if vocab:
         V = V_full
-    step_bytes, upd_bytes = algorithmic_bytes(V, d, T)
+    step_bytes, upd_bytes = algorithmic_bytes(V, d, T, moments=args.moments)
     if vocab:
         step_bytes //= world
     if z_given is not None:
@@ -493,7 +499,7 @@ def run_ours(args, rank, world, local_rank):
     roof = {"bound": "hbm", "kernel": "a6+a7 gW contraction fused with AdamW update (phase 4)",
             "achieved": (upd_bytes / (upd_ms * 1e-3) / 1e9) if upd_ms else None, "peak": peak, "unit": "GB/s",
             "frac": (upd_bytes / (upd_ms * 1e-3) / 1e9 / peak) if upd_ms else None,
-            "traffic": profiled_traffic(args.config) if (z_given is None and not vocab) else None,
+            "traffic": profiled_traffic(args.config) if (z_given is None and not vocab and args.moments == "f32") else None,
             "peak_source": peak_src, "algorithmic_bytes_per_launch": upd_bytes, "kernel_ms": upd_ms,
             "step_algorithmic_bytes": step_bytes, "step_achieved": step_bytes / (ms_step * 1e-3) / 1e9,
             "step_frac_of_measured_copy": step_bytes / (ms_step * 1e-3) / 1e9 / peak,
@@ -504,7 +510,7 @@ def run_ours(args, rank, world, local_rank):
             "scaling": "strong" if vocab else "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
             "config": dict(workload_config(args.config, world, "tcgen05+tma" if used_tensor else "cuda-core",
                                            args.parallelism), **({"T": T, "n_seq_override": args.n_seq} if args.n_seq else {}),
-                           draft_logits=args.draft_logits),
+                           draft_logits=args.draft_logits, adam_moments=args.moments),
             "rows_V_per_sec": sps * T * V, "loss": loss_val, "clocks": clocks, "e2e": e2e,
             "gpu_launches": launches[0], "roofline": roof, "cpu_baseline": cpu}
     if stream is not None:

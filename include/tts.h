@@ -102,6 +102,7 @@ typedef struct {
   int32_t max_inner_steps; /* largest K of tts_distill_inner_steps; > 1 reserves its z_ref scratch    */
                         /* (T_max x V fp32) in tts_ctx_create so that no step call ever allocates     */
   int32_t flags;        /* TTS_FLAG_* (0 = none)                                                      */
+  int32_t sr_seed;      /* TTS_MOMENT_BF16: seed of the stochastic-rounding draws of v                */
 } tts_config;
 
 const char* tts_status_string(int32_t status);
@@ -135,9 +136,13 @@ int64_t tts_get_step_count_on(tts_ctx* ctx, void* stream);
 int32_t tts_last_device_status(tts_ctx* ctx);
 int32_t tts_check_preconditions(tts_ctx* ctx, const void* teacher_logits, const void* h, const void* W_in,
                                 const float* W_master, int32_t T, void* stream);
-/* A kernel whose internal pipeline stalls for more than ~4 s (a protocol error, never a legal state) executes a trap
- * instead of spinning forever: the launch fails with cudaErrorLaunchFailed, reported as TTS_ERR_CUDA by the next call
- * that synchronises (tts_sync_step, tts_round_host, tts_last_device_status, ...). */
+/* A tensor-path kernel whose internal pipeline stalls (a protocol error, never a legal state) does not hang the GPU:
+ * a watchdog warp in every persistent kernel traps after ~9 s without progress, the launch fails with
+ * cudaErrorLaunchFailed and the next call that synchronises (tts_sync_step, tts_round_host, tts_last_device_status, ...)
+ * returns TTS_ERR_CUDA.  tts_debug_trip_watchdog proves it: it launches a deliberately stalled pipeline on `stream`,
+ * blocks until the launch has failed and returns TTS_ERR_CUDA; the process's CUDA context is unusable afterwards
+ * (run it in a process of its own). */
+int32_t tts_debug_trip_watchdog(tts_ctx* ctx, void* stream);
 /* CUDA error code (cudaError_t as int) of the last failed CUDA call on this ctx, 0 if none. */
 int32_t tts_last_cuda_error(const tts_ctx* ctx);
 /* 1 if the last tts_distill_step on this ctx ran the tcgen05/TMA kernels, 0 if CUDA-core. */
@@ -205,6 +210,15 @@ int32_t tts_accept_stochastic(tts_ctx* ctx,
  *   AdamW  : M <- M (1 - lr wd); m <- b1 m + (1-b1) g; v <- b2 v + (1-b2) g^2;
  *            M <- M - lr (m / (1-b1^n)) / (sqrt(v / (1-b2^n)) + eps)      (R5)
  *   W_out  = rn_bf16(M)   (TTS_BF16)   |   W_out = M   (TTS_F32, W_master == NULL)
+ *   TTS_MOMENT_BF16 (opt-in, R26): adam_m / adam_v hold bf16 [V,d] (18 instead of 26 bytes per parameter in the update
+ *            pass).  Per element: widen m, v exactly; update as above with the UNROUNDED new moments; store
+ *            m = rn_bf16(m_new) and v = bf16 by STOCHASTIC rounding of v_new (beta2 = 0.999 decays v by 0.1% per
+ *            step, below half a bf16 ulp: nearest rounding would freeze it): the 16 discarded fp32 bits f round
+ *            away from zero iff f + r >= 65536, r = the 16 bits of a counter-based generator keyed by the element
+ *            index v * d + j (LOCAL rows on a vocabulary shard), Adam's count n and cfg.sr_seed:
+ *              x = lo32(idx) ^ (n * 0x9E3779B9) ^ (sr_seed * 0x85EBCA6B) ^ (hi32(idx) * 0xC2B2AE35)
+ *              x ^= x >> 16; x *= 0x7FEB352D; x ^= x >> 15; x *= 0x846CA68B; x ^= x >> 16;  r = x >> 16
+ *            TTS_MOMENT_Q8 (8-bit block-scaled moments) is reserved: tts_ctx_create returns TTS_ERR_UNSUPPORTED.
  *
  * Preconditions: for TTS_BF16, W_in == rn_bf16(W_master) element-wise at entry; teacher_logits
  * and h must stay untouched until the done-event (the step consumes the buffers captured at
@@ -218,8 +232,8 @@ int32_t tts_distill_step(tts_ctx* ctx,
                          const void* W_in,           /* [V,d] param_dtype: weights that produced q_t         */
                          void* W_out,                /* [V,d] param_dtype: updated weights; may alias W_in   */
                          float* W_master,            /* [V,d] fp32 in place; NULL iff TTS_F32                */
-                         float* adam_m,              /* [V,d] fp32 in place; NULL iff TTS_SGD                */
-                         float* adam_v,              /* [V,d] fp32 in place; NULL iff TTS_SGD                */
+                         void* adam_m,               /* [V,d] moment_dtype in place; NULL iff TTS_SGD        */
+                         void* adam_v,               /* [V,d] moment_dtype in place; NULL iff TTS_SGD        */
                          const float* pos_weight,    /* [T]   w_k already expanded per row                   */
                          const uint8_t* mask,        /* [T]   from tts_accept_mask; may be NULL for ROWS_ALL */
                          int32_t T,                  /* multiple of seg_len, 1..T_max                        */
@@ -253,7 +267,7 @@ typedef struct {
 } tts_step_extras;
 
 int32_t tts_distill_step_ex(tts_ctx* ctx, const void* teacher_logits, const void* h, const void* W_in, void* W_out,
-                            float* W_master, float* adam_m, float* adam_v, const float* pos_weight,
+                            float* W_master, void* adam_m, void* adam_v, const float* pos_weight,
                             const uint8_t* mask, int32_t T, float loss_scale, float* loss_out, float* kl_rows_out,
                             float* gh_out, float* gW_debug_out,
                             const tts_step_extras* extras, /* host, may be NULL */
@@ -271,7 +285,7 @@ int32_t tts_distill_step_ex(tts_ctx* ctx, const void* teacher_logits, const void
  * (else TTS_ERR_INVALID_ARG); no step call allocates.
  */
 int32_t tts_distill_inner_steps(tts_ctx* ctx, const void* teacher_logits, const void* h, const void* W_in, void* W_out,
-                                float* W_master, float* adam_m, float* adam_v, const float* pos_weight,
+                                float* W_master, void* adam_m, void* adam_v, const float* pos_weight,
                                 const uint8_t* mask, int32_t T, float loss_scale, int32_t K, float lambda,
                                 const float* draft_logits, float* loss_out, float* kl_rows_out, float* gh_out,
                                 void* side_stream);
@@ -320,7 +334,7 @@ int32_t tts_round_host(tts_ctx* ctx,
                        const int32_t* draft_tokens_host,/* host [T]                */
                        const float* pos_weight_host,    /* host [T]                */
                        int32_t T, float loss_scale,
-                       const void* W_in, void* W_out, float* W_master, float* adam_m, float* adam_v, /* device */
+                       const void* W_in, void* W_out, float* W_master, void* adam_m, void* adam_v, /* device */
                        float* gh_dev,                   /* device [T,d] or NULL    */
                        float* loss_host,                /* host [1]                */
                        int32_t* tau_host,               /* host [T/seg_len]        */
@@ -360,7 +374,7 @@ int32_t tts_shard_finish_step(tts_ctx* ctx,
                               const float* stats_all,          /* [n_shards, T, 8], own shard included     */
                               int32_t n_shards,                /* 1..1024                                  */
                               const void* teacher_logits_local, const void* h, const void* W_in_local,
-                              void* W_out_local, float* W_master_local, float* adam_m_local, float* adam_v_local,
+                              void* W_out_local, float* W_master_local, void* adam_m_local, void* adam_v_local,
                               const float* pos_weight, const uint8_t* mask, int32_t T, float loss_scale,
                               float* loss_out,                 /* [1] the GLOBAL loss                      */
                               float* kl_rows_out,              /* [T] global KL_r, or NULL                 */

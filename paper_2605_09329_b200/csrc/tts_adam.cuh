@@ -1,0 +1,29 @@
+// Low-precision moment storage of the AdamW update (include/tts.h TTS_MOMENT_BF16; R26): the counter-based
+// draws of the stochastic rounding of v and the two fp32 -> bf16 conversions.  The fp64 oracle has its own
+// implementation of the same generator (nothing is shared): both follow the definition written out here.
+#pragma once
+
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace tts {
+
+// 16 pseudo-random bits for element idx = v * d + j at Adam count n:
+//   x = lo32(idx) ^ (n * 0x9E3779B9) ^ (seed * 0x85EBCA6B) ^ (hi32(idx) * 0xC2B2AE35)
+//   x ^= x >> 16;  x *= 0x7FEB352D;  x ^= x >> 15;  x *= 0x846CA68B;  x ^= x >> 16;   bits = x >> 16
+// `key` = (n * 0x9E3779B9) ^ (seed * 0x85EBCA6B) is formed once per thread.
+__device__ __forceinline__ uint32_t sr_key(uint32_t n, uint32_t seed) { return (n * 0x9E3779B9u) ^ (seed * 0x85EBCA6Bu); }
+__device__ __forceinline__ uint32_t sr_bits16(unsigned long long idx, uint32_t key) {
+  uint32_t x = static_cast<uint32_t>(idx) ^ key ^ (static_cast<uint32_t>(idx >> 32) * 0xC2B2AE35u);
+  x ^= x >> 16; x *= 0x7FEB352Du; x ^= x >> 15; x *= 0x846CA68Bu; x ^= x >> 16;
+  return x >> 16;
+}
+// stochastic rounding: the 16 discarded bits f round away from zero iff f + r >= 65536, so E_r[result] = x
+__device__ __forceinline__ uint16_t bf16_bits_sr(float x, uint32_t r16) {
+  return static_cast<uint16_t>((__float_as_uint(x) + r16) >> 16);
+}
+__device__ __forceinline__ uint16_t bf16_bits_rn(float x) { return __bfloat16_as_ushort(__float2bfloat16_rn(x)); }
+__device__ __forceinline__ float bf16_bits_widen(uint16_t b) { return __uint_as_float(static_cast<uint32_t>(b) << 16); }
+
+}  // namespace tts

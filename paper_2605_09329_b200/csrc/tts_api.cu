@@ -71,7 +71,7 @@ int32_t tts_ctx_create(const tts_config* cfg, int32_t device, tts_ctx** out) {
   if (cfg->kernel_path != TTS_PATH_AUTO && cfg->kernel_path != TTS_PATH_SIMT) return TTS_ERR_UNSUPPORTED;
   if (cfg->max_ctas < 0 || cfg->max_inner_steps < 0) return TTS_ERR_INVALID_ARG;
   if (cfg->flags & ~(TTS_FLAG_CHECK_PRECONDITIONS | TTS_FLAG_DETERMINISTIC | TTS_FLAG_SEPARATE_GH)) return TTS_ERR_INVALID_ARG;
-  if (cfg->moment_dtype < TTS_MOMENT_F32 || cfg->moment_dtype > TTS_MOMENT_Q8) return TTS_ERR_UNSUPPORTED;
+  if (cfg->moment_dtype != TTS_MOMENT_F32 && cfg->moment_dtype != TTS_MOMENT_BF16) return TTS_ERR_UNSUPPORTED;   // Q8: reserved
   if (cfg->moment_dtype != TTS_MOMENT_F32 && cfg->optimizer != TTS_ADAMW) return TTS_ERR_UNSUPPORTED;
   // rows of every [*, V] / [*, d] tensor must start 16-byte aligned
   if ((static_cast<size_t>(cfg->V) * elem_size(cfg->logits_dtype)) % 16 != 0) return TTS_ERR_UNSUPPORTED;
@@ -218,6 +218,15 @@ int32_t tts_check_preconditions(tts_ctx* c, const void* teacher, const void* h, 
   return e == cudaSuccess ? TTS_OK : cuda_fail(c, e);
 }
 
+int32_t tts_debug_trip_watchdog(tts_ctx* c, void* stream) {
+  if (!c) return TTS_ERR_INVALID_ARG;
+  tts_device_guard g(c->device);
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  cudaError_t e = tts::launch_stalled_pipeline(s);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  return e == cudaSuccess ? TTS_OK : cuda_fail(c, e);
+}
+
 int32_t tts_last_cuda_error(const tts_ctx* c) { return c ? c->last_cuda_error : 0; }
 int32_t tts_last_step_used_tensor_path(const tts_ctx* c) { return c ? c->last_used_tensor : 0; }
 int32_t tts_last_launch_count(const tts_ctx* c) { return c ? c->last_launches : 0; }
@@ -256,7 +265,7 @@ int32_t tts_accept_stochastic(tts_ctx* c, const void* teacher, const float* draf
 }
 
 int32_t tts_distill_step(tts_ctx* c, const void* teacher, const void* h, const void* W_in, void* W_out,
-                         float* W_master, float* adam_m, float* adam_v, const float* pos_weight,
+                         float* W_master, void* adam_m, void* adam_v, const float* pos_weight,
                          const uint8_t* mask, int32_t T, float loss_scale, float* loss_out, float* kl_rows_out,
                          float* gh_out, float* gW_debug_out, void* side_stream) {
   return tts_distill_step_ex(c, teacher, h, W_in, W_out, W_master, adam_m, adam_v, pos_weight, mask, T, loss_scale,
@@ -265,7 +274,7 @@ int32_t tts_distill_step(tts_ctx* c, const void* teacher, const void* h, const v
 
 // The step of include/tts.h in one piece (phase 0) or as the two halves of the vocabulary-sharded step.
 static int32_t run_step(tts_ctx* c, const void* teacher, const void* h, const void* W_in, void* W_out,
-                        float* W_master, float* adam_m, float* adam_v, const float* pos_weight,
+                        float* W_master, void* adam_m, void* adam_v, const float* pos_weight,
                         const uint8_t* mask, int32_t T, float loss_scale, float* loss_out, float* kl_rows_out,
                         float* gh_out, float* gW_debug_out, const tts_step_extras* ex, void* side_stream, int phase,
                         float* stats_out, const float* stats_all, int32_t n_shards) {
@@ -349,7 +358,7 @@ int32_t tts_record_done(tts_ctx* c, void* stream) {
 }
 
 int32_t tts_distill_step_ex(tts_ctx* c, const void* teacher, const void* h, const void* W_in, void* W_out,
-                            float* W_master, float* adam_m, float* adam_v, const float* pos_weight,
+                            float* W_master, void* adam_m, void* adam_v, const float* pos_weight,
                             const uint8_t* mask, int32_t T, float loss_scale, float* loss_out, float* kl_rows_out,
                             float* gh_out, float* gW_debug_out, const tts_step_extras* ex, void* side_stream) {
   return run_step(c, teacher, h, W_in, W_out, W_master, adam_m, adam_v, pos_weight, mask, T, loss_scale, loss_out,
@@ -365,7 +374,7 @@ int32_t tts_shard_begin_step(tts_ctx* c, const void* teacher_local, const void* 
 
 int32_t tts_shard_finish_step(tts_ctx* c, const float* stats_all, int32_t n_shards, const void* teacher_local,
                               const void* h, const void* W_in_local, void* W_out_local, float* W_master_local,
-                              float* adam_m_local, float* adam_v_local, const float* pos_weight, const uint8_t* mask,
+                              void* adam_m_local, void* adam_v_local, const float* pos_weight, const uint8_t* mask,
                               int32_t T, float loss_scale, float* loss_out, float* kl_rows_out, float* gh_partial_out,
                               float* gW_debug_out, const tts_step_extras* ex, void* side_stream) {
   return run_step(c, teacher_local, h, W_in_local, W_out_local, W_master_local, adam_m_local, adam_v_local, pos_weight,
@@ -399,7 +408,7 @@ int32_t tts_shard_accept_mask(tts_ctx* c, const float* val_all, const int32_t* i
 }
 
 int32_t tts_distill_inner_steps(tts_ctx* c, const void* teacher, const void* h, const void* W_in, void* W_out,
-                                float* W_master, float* adam_m, float* adam_v, const float* pos_weight,
+                                float* W_master, void* adam_m, void* adam_v, const float* pos_weight,
                                 const uint8_t* mask, int32_t T, float loss_scale, int32_t K, float lambda,
                                 const float* draft_logits, float* loss_out, float* kl_rows_out, float* gh_out,
                                 void* side_stream) {
@@ -487,7 +496,7 @@ int32_t tts_sync_step(tts_ctx* c) {
 
 int32_t tts_round_host(tts_ctx* c, const void* teacher_host, const void* h_host, const int32_t* tok_host,
                        const float* pw_host, int32_t T, float loss_scale, const void* W_in, void* W_out,
-                       float* W_master, float* adam_m, float* adam_v, float* gh_dev, float* loss_host,
+                       float* W_master, void* adam_m, void* adam_v, float* gh_dev, float* loss_host,
                        int32_t* tau_host, uint8_t* mask_host, void* stream) {
   if (!c || !teacher_host || !h_host || !tok_host || !pw_host || !loss_host || !tau_host) return TTS_ERR_INVALID_ARG;
   const tts_config& cfg = c->cfg;

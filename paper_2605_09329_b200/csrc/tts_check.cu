@@ -7,6 +7,7 @@
 //   precondition 5   teacher logits finite or -inf (R23), hidden states finite.
 #include "tts_common.cuh"
 #include "tts_internal.h"
+#include "tts_tc_ptx.cuh"
 
 namespace tts {
 namespace {
@@ -35,6 +36,23 @@ __global__ void __launch_bounds__(256) check_finite_kernel(const T* __restrict__
     bad |= !(isfinite(f) || (allow_neg_inf && f == -CUDART_INF_F));
   }
   if (__any_sync(0xffffffffu, bad) && (threadIdx.x & 31) == 0) atomicOr(status, bit);
+}
+
+// A pipeline that never completes: warp 1 waits on an mbarrier nobody arrives at (the shape of a protocol slip in the
+// tensor-path kernels), so the "epilogue" never reports and the watchdog warp must trap.
+__global__ void __launch_bounds__(96) stalled_pipeline_kernel() {
+  __shared__ uint64_t bar;
+  __shared__ uint32_t done_ctr;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (threadIdx.x == 0) { ptx::mbar_init(&bar, 1); done_ctr = 0; ptx::fence_barrier_init(); }
+  __syncthreads();
+  if (warp == 1) {
+    ptx::mbar_wait(&bar, 0);
+    if (lane == 0) ptx::watchdog_arrive(&done_ctr);
+  } else if (warp == 2) {
+    ptx::watchdog_wait(&done_ctr, 1);
+  }
+  __syncthreads();
 }
 
 __global__ void set_count_kernel(unsigned long long* p, unsigned long long n) { *p = n; }
@@ -68,6 +86,11 @@ cudaError_t launch_check_preconditions(tts_ctx* c, const void* teacher, const vo
                                              c->dev_status);
     *launches += 1;
   }
+  return cudaGetLastError();
+}
+
+cudaError_t launch_stalled_pipeline(cudaStream_t s) {
+  stalled_pipeline_kernel<<<1, 96, 0, s>>>();
   return cudaGetLastError();
 }
 

@@ -23,8 +23,8 @@ struct StepArgs {
   const void* W_in;
   void* W_out;
   float* master;
-  float* adam_m;
-  float* adam_v;
+  void* adam_m;   // [V,d] cfg.moment_dtype (fp32, or bf16 bits with TTS_MOMENT_BF16)
+  void* adam_v;
   const float* pos_weight;
   const uint8_t* mask;
   int T;
@@ -124,6 +124,7 @@ inline void prof_mark(tts_ctx* c, int phase, cudaStream_t s) {
 cudaError_t launch_check_preconditions(tts_ctx* c, const void* teacher, const void* h, const void* W_in,
                                        const float* master, int T, cudaStream_t s, int* launches);
 cudaError_t launch_set_count(tts_ctx* c, unsigned long long n, cudaStream_t s);
+cudaError_t launch_stalled_pipeline(cudaStream_t s);
 // tts_mask.cu
 cudaError_t launch_accept_mask(tts_ctx* c, const void* teacher, const int32_t* tok, int T, uint8_t* mask,
                                int32_t* tau, int32_t* am_out, cudaStream_t s, int* launches);

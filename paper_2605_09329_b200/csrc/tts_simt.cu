@@ -214,7 +214,7 @@ static cudaError_t simt_step_t(tts_ctx* c, const StepArgs& a, cudaStream_t s, in
   prof_mark(c, 3, s);
   dim3 grid((d + 127) / 128, (V + 7) / 8);
   if (c->cfg.optimizer == TTS_ADAMW)
-    simt_update_kernel<PT, true><<<grid, 128, 0, s>>>(c->dl32, h, T, V, d, W_in, W_out, a.master, a.adam_m, a.adam_v,
+    simt_update_kernel<PT, true><<<grid, 128, 0, s>>>(c->dl32, h, T, V, d, W_in, W_out, a.master, static_cast<float*>(a.adam_m), static_cast<float*>(a.adam_v),
                                                       a.gW_debug, a.lr, a.beta1, a.beta2, a.eps, a.wd,
                                                       a.step_scalars);
   else

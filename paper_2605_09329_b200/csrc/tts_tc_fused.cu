@@ -29,6 +29,7 @@
 //       of gh (N = r, K = v); only the roles of the two descriptor strides swap.
 #include <string.h>
 
+#include "tts_adam.cuh"
 #include "tts_common.cuh"
 #include "tts_tc_ptx.cuh"
 #include "tts_tc_state.h"
@@ -45,10 +46,13 @@ constexpr int kSubs = kTV / kSV; // 8 stages per tile
 constexpr int kBoxW = 256;       // TMA box width (elements): 4 boxes per tensor per stage
 constexpr int kBoxes = kSW / kBoxW;
 constexpr int kT16 = 16;         // canvas rows (padded)
-constexpr int kMaxStages = 7;    // state ring depth (168 KB; h^T lives in tensor memory, not shared memory)
+constexpr int kMaxStages = 10;   // state ring depth: 7 x 24 KB with fp32 moments, 10 x 16 KB with bf16 moments (h^T lives in
+                                 // tensor memory, not shared memory)
 constexpr int kOpStages = 2;     // dl tile ring depth
-constexpr int kTensorBytes = kSV * kSW * 4;          // 8 KB per tensor per stage
-constexpr int kStageBytes = 3 * kTensorBytes;        // 24 KB
+constexpr int kTensorBytes = kSV * kSW * 4;          // 8 KB per fp32 tensor per stage
+constexpr int kStageBytes = 3 * kTensorBytes;        // 24 KB (fp32 moments)
+constexpr int kMomBytesLp = kSV * kSW * 2;           // 4 KB per bf16 moment tensor per stage
+constexpr int kStageBytesLp = kTensorBytes + 2 * kMomBytesLp;   // 16 KB (bf16 moments)
 constexpr int kWoBytes = kSV * kSW * 2;              // 4 KB: bf16 W_out staging of one sub-tile (one per group)
 constexpr int kWtBytes = kSW * kTV * 2;              // 32 KB: re-derived bf16 W^T tile (A operand of gh)
 constexpr int kDlBytes = 2 * kT16 * kTV * 2;         // 1 KB: dl tile, both planes
@@ -59,8 +63,6 @@ constexpr int kTmemCols = 512;
 
 struct FusedParams {
   float* master;
-  float* am;
-  float* av;
   float* gW_debug;
   float* gh;                  // NULL: a5 is skipped
   const __nv_bfloat16* hTc;
@@ -69,6 +71,8 @@ struct FusedParams {
   int n_stripes;              // d / 1024
   int stages;
   const float* step_scalars;  // device {1 / (1 - b1^n), 1 / sqrt(1 - b2^n)} of this step
+  const unsigned long long* step_count;   // device: Adam's count n of this step (keys the stochastic rounding of v)
+  uint32_t sr_seed;
   float lr, b1, b2, eps, decay;   // decay = 1 - lr wd
 };
 
@@ -113,7 +117,9 @@ struct Walk {
 };
 
 // SK: the stream-K walk (up to two segments); false: one segment, known at compile time (grid % n_stripes == 0)
-template <bool ADAM, bool SK>
+// MOM: 1 = Adam's moments are stored as bf16 (TTS_MOMENT_BF16: a stage is 16 KB, the ring 10 deep; m is written back
+// round-to-nearest-even, v with stochastic rounding keyed by (element index, Adam count, seed): tts_adam.cuh)
+template <bool ADAM, bool SK, int MOM>
 __global__ void __launch_bounds__(kThreads, 1)
 tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_constant__ CUtensorMap tm_m,
                     const __grid_constant__ CUtensorMap tm_v, const __grid_constant__ CUtensorMap tm_wout,
@@ -121,8 +127,11 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const int kStages = p.stages;
-  uint8_t* st = smem;                                   // [kStages][3][4 boxes][2 v][256] fp32
-  uint8_t* wt = st + kStages * kStageBytes;                         // [8 jb][2 v-groups][16 j-groups][8 j][8 v] bf16
+  constexpr int kStageB = MOM ? kStageBytesLp : kStageBytes;
+  constexpr int kMomB = MOM ? kMomBytesLp : kTensorBytes;            // bytes of one moment tensor in a stage
+  constexpr int kMomE = MOM ? 2 : 4;                                  // bytes per moment element
+  uint8_t* st = smem;                                   // [kStages]{master [4 boxes][2 v][256] fp32, m, v likewise}
+  uint8_t* wt = st + kStages * kStageB;                             // [8 jb][2 v-groups][16 j-groups][8 j][8 v] bf16
   uint8_t* wo = wt + kWtBytes;                          // [2 groups][4 boxes][2 v][256] bf16
   uint8_t* dl = wo + 2 * kWoBytes;                      // [kOpStages][2 planes][2 r-groups][2 v-groups][8 r][8 v] bf16
   uint64_t* bars = reinterpret_cast<uint64_t*>(dl + kOpStages * kDlBytes);
@@ -138,6 +147,7 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
   uint64_t* gh_full = wt_empty + 1;            // [1]
   uint64_t* gh_empty = gh_full + 1;            // [1]
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(gh_empty + 1);
+  uint32_t* done_ctr = tmem_slot + 1;          // epilogue warps finished (watchdog)
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const bool do_gh = p.gh != nullptr;
@@ -157,6 +167,7 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
     ptx::mbar_init(wt_empty, 1);
     ptx::mbar_init(gh_full, 1);
     ptx::mbar_init(gh_empty, 4);
+    *done_ctr = 0;
     ptx::fence_barrier_init();
   }
   if (warp == 2) {
@@ -180,16 +191,16 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
         for (int sub = 0; sub < kSubs; ++sub, ++n) {
           const int s = n % kStages;
           ptx::mbar_wait(&st_empty[s], ((n / kStages) & 1) ^ 1);
-          uint8_t* dst = st + s * kStageBytes;
-          ptx::mbar_expect_tx(&st_full[s], (ADAM ? 3 : 1) * kTensorBytes);
+          uint8_t* dst = st + s * kStageB;
+          ptx::mbar_expect_tx(&st_full[s], ADAM ? kTensorBytes + 2 * kMomB : kTensorBytes);
           const int r0 = v0 + sub * kSV;
 #pragma unroll
           for (int b = 0; b < kBoxes; ++b) {
-            const int c0 = j_stripe + b * kBoxW, off = b * kSV * kBoxW * 4;
+            const int c0 = j_stripe + b * kBoxW, off = b * kSV * kBoxW * 4, off_m = b * kSV * kBoxW * kMomE;
             ptx::tma_load_2d(dst + off, &tm_master, &st_full[s], c0, r0);
             if (ADAM) {
-              ptx::tma_load_2d(dst + kTensorBytes + off, &tm_m, &st_full[s], c0, r0);
-              ptx::tma_load_2d(dst + 2 * kTensorBytes + off, &tm_v, &st_full[s], c0, r0);
+              ptx::tma_load_2d(dst + kTensorBytes + off_m, &tm_m, &st_full[s], c0, r0);
+              ptx::tma_load_2d(dst + kTensorBytes + kMomB + off_m, &tm_v, &st_full[s], c0, r0);
             }
           }
         }
@@ -278,6 +289,7 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
     const int jj = q * 32 + lane;
     const bool leader = jj == 0;               // issues the group's TMA stores and releases its state stages
     const float c1 = ADAM ? p.lr * p.step_scalars[0] : 0.f, inv_sqrt_bc2 = ADAM ? p.step_scalars[1] : 0.f;
+    const uint32_t key = MOM ? sr_key(static_cast<uint32_t>(*p.step_count), p.sr_seed) : 0u;
     // element (v, jb) of a stage tensor sits in box jb / 2, row v, column (jb % 2) * 128 + jj
     uint8_t* wt_thr = wt + (jj >> 3) * 128 + (jj & 7) * 16;   // + jb * 4096 + (v >> 3) * 2048 + (v & 7) * 2
     __nv_bfloat16* wo_g = reinterpret_cast<__nv_bfloat16*>(wo + g * kWoBytes);
@@ -315,7 +327,9 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
           ptx::tmem_ld_32x32b_x2(tmem_base + ab * (kJB * kTV) + jb * kTV + sub * kSV +
                                      (static_cast<uint32_t>(q * 32) << 16), gr[jb]);
         ptx::mbar_wait(&st_full[s], (n / kStages) & 1);
-        float* sM = reinterpret_cast<float*>(st + s * kStageBytes) + jj;
+        float* sM = reinterpret_cast<float*>(st + s * kStageB) + jj;
+        uint16_t* sLm = reinterpret_cast<uint16_t*>(st + s * kStageB + kTensorBytes) + jj;   // MOM: bf16 m, then v
+        uint16_t* sLv = reinterpret_cast<uint16_t*>(st + s * kStageB + kTensorBytes + kMomB) + jj;
         float M[kJB][2], mm[kJB][2], vv[kJB][2];
 #pragma unroll
         for (int jb = 0; jb < kJB; ++jb)
@@ -323,7 +337,10 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
           for (int v = 0; v < 2; ++v) {
             const int e = (jb >> 1) * 512 + v * 256 + (jb & 1) * 128;
             M[jb][v] = sM[e];
-            if (ADAM) { mm[jb][v] = sM[kSV * kSW + e]; vv[jb][v] = sM[2 * kSV * kSW + e]; }
+            if (ADAM) {
+              if (MOM) { mm[jb][v] = bf16_bits_widen(sLm[e]); vv[jb][v] = bf16_bits_widen(sLv[e]); }
+              else { mm[jb][v] = sM[kSV * kSW + e]; vv[jb][v] = sM[2 * kSV * kSW + e]; }
+            }
           }
         if (do_gh) {
           // a5 operand: W_in[v, j] = rn_bf16(master[v, j]); rows (2 sub, 2 sub + 1) of this thread's 8 columns
@@ -349,9 +366,16 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
               const float m1 = p.b1 * mm[jb][v] + (1.f - p.b1) * gg;
               const float v1 = p.b2 * vv[jb][v] + (1.f - p.b2) * gg * gg;
               const float den = __fsqrt_rn(v1) * inv_sqrt_bc2 + p.eps;
-              M[jb][v] = M[jb][v] * p.decay - __fdividef(c1 * m1, den);
-              sM[kSV * kSW + e] = m1;
-              sM[2 * kSV * kSW + e] = v1;
+              M[jb][v] = M[jb][v] * p.decay - __fdividef(c1 * m1, den);     // the step uses the unrounded moments
+              if (MOM) {
+                const unsigned long long idx =
+                    (unsigned long long)(v0 + sub * kSV + v) * (unsigned long long)p.d + (j_stripe + jb * kMJ + jj);
+                sLm[e] = bf16_bits_rn(m1);
+                sLv[e] = bf16_bits_sr(v1, sr_bits16(idx, key));
+              } else {
+                sM[kSV * kSW + e] = m1;
+                sM[2 * kSV * kSW + e] = v1;
+              }
             } else {
               M[jb][v] = M[jb][v] - p.lr * gg;
             }
@@ -379,14 +403,14 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
         ptx::named_barrier_sync(1 + g, 128);
         if (leader) {
           const int r0 = v0 + sub * kSV;
-          const float* sT = reinterpret_cast<const float*>(st + s * kStageBytes);
+          const uint8_t* sT = st + s * kStageB;
 #pragma unroll
           for (int b = 0; b < kBoxes; ++b) {
             const int c0 = j_stripe + b * kBoxW, off = b * kSV * kBoxW;
-            ptx::tma_store_2d(&tm_master, sT + off, c0, r0);
+            ptx::tma_store_2d(&tm_master, sT + off * 4, c0, r0);
             if (ADAM) {
-              ptx::tma_store_2d(&tm_m, sT + kSV * kSW + off, c0, r0);
-              ptx::tma_store_2d(&tm_v, sT + 2 * kSV * kSW + off, c0, r0);
+              ptx::tma_store_2d(&tm_m, sT + kTensorBytes + off * kMomE, c0, r0);
+              ptx::tma_store_2d(&tm_v, sT + kTensorBytes + kMomB + off * kMomE, c0, r0);
             }
             ptx::tma_store_2d(&tm_wout, wo_g + off, c0, r0);
           }
@@ -417,6 +441,9 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
     }
     }   // segments
     if (leader) ptx::bulk_wait_group_read<0>();   // shared memory must outlive the last stores' reads
+    if (lane == 0) ptx::watchdog_arrive(done_ctr);
+  } else if (warp == 2) {
+    ptx::watchdog_wait(done_ctr, 8);
   }
   ptx::tc_fence_before();
   __syncthreads();
@@ -426,9 +453,10 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
   }
 }
 
-size_t fused_smem() {
-  return 1024 + (size_t)kMaxStages * kStageBytes + kWtBytes + 2 * (size_t)kWoBytes +
-         (size_t)kOpStages * kDlBytes + 512;
+constexpr int kStagesF32 = 7, kStagesLp = 10;
+size_t fused_smem(bool lowp) {
+  return 1024 + (lowp ? (size_t)kStagesLp * kStageBytesLp : (size_t)kStagesF32 * kStageBytes) + kWtBytes +
+         2 * (size_t)kWoBytes + (size_t)kOpStages * kDlBytes + 512;
 }
 
 // hTc[j][k] = h[k, j] for k < 16 (rows k >= T are zero): 32 bytes per hidden column, the order in which the epilogue
@@ -489,17 +517,14 @@ cudaError_t tc_fused_init(tts_ctx* c) {
   TcState* st = static_cast<TcState*>(c->tc_state);
   if ((e = cudaMalloc(&st->hTc, (size_t)c->cfg.d * kT16 * 2)) != cudaSuccess) return e;
   if ((e = cudaMalloc(&st->dlC, (size_t)c->cfg.V * 2 * kT16 * 2)) != cudaSuccess) return e;
-  const int smem = (int)fused_smem();
-  if ((e = cudaFuncSetAttribute(tc_update_gh_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) !=
-      cudaSuccess)
-    return e;
-  if ((e = cudaFuncSetAttribute(tc_update_gh_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) !=
-      cudaSuccess)
-    return e;
-  if ((e = cudaFuncSetAttribute(tc_update_gh_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) !=
-      cudaSuccess)
-    return e;
-  return cudaFuncSetAttribute(tc_update_gh_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  const int smem = (int)fused_smem(false), smem_lp = (int)fused_smem(true);
+  const auto attr = cudaFuncAttributeMaxDynamicSharedMemorySize;
+  if ((e = cudaFuncSetAttribute(tc_update_gh_kernel<true, false, 0>, attr, smem)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(tc_update_gh_kernel<true, true, 0>, attr, smem)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(tc_update_gh_kernel<false, true, 0>, attr, smem)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(tc_update_gh_kernel<false, false, 0>, attr, smem)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(tc_update_gh_kernel<true, false, 1>, attr, smem_lp)) != cudaSuccess) return e;
+  return cudaFuncSetAttribute(tc_update_gh_kernel<true, true, 1>, attr, smem_lp);
 }
 
 // Grid of the fused pass, 0 when the shape does not qualify (T > 16 rows, d or V not a multiple of the tile, or an
@@ -545,31 +570,37 @@ cudaError_t tc_launch_update_fused(tts_ctx* c, const StepArgs& a, int grid, cuda
     return cudaErrorInvalidValue;
   tm_m = tm_master;
   tm_v = tm_master;
+  const bool lowp = adam && c->cfg.moment_dtype == TTS_MOMENT_BF16;
   if (adam) {
-    if (make_map_2d(st, &tm_m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, a.adam_m, d, V, kBoxW, kSV,
-                    CU_TENSOR_MAP_SWIZZLE_NONE) != CUDA_SUCCESS)
+    const CUtensorMapDataType mdt = lowp ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
+    const int msz = lowp ? 2 : 4;
+    if (make_map_2d(st, &tm_m, mdt, msz, a.adam_m, d, V, kBoxW, kSV, CU_TENSOR_MAP_SWIZZLE_NONE) != CUDA_SUCCESS)
       return cudaErrorInvalidValue;
-    if (make_map_2d(st, &tm_v, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, a.adam_v, d, V, kBoxW, kSV,
-                    CU_TENSOR_MAP_SWIZZLE_NONE) != CUDA_SUCCESS)
+    if (make_map_2d(st, &tm_v, mdt, msz, a.adam_v, d, V, kBoxW, kSV, CU_TENSOR_MAP_SWIZZLE_NONE) != CUDA_SUCCESS)
       return cudaErrorInvalidValue;
   }
   FusedParams p;
-  p.master = a.master; p.am = a.adam_m; p.av = a.adam_v;
+  p.master = a.master;
   p.gW_debug = a.gW_debug; p.gh = a.gh_out; p.hTc = st->hTc; p.dlC = st->dlC;
   p.V = V; p.d = d; p.T = T;
   p.n_stripes = d / kSW;
-  p.stages = kMaxStages;
+  p.stages = lowp ? kStagesLp : kStagesF32;
   p.lr = a.lr; p.b1 = a.beta1; p.b2 = a.beta2; p.eps = a.eps;
   p.decay = 1.f - a.lr * a.wd;
   p.step_scalars = a.step_scalars;
-  const size_t smem = fused_smem();
+  p.step_count = c->step_count_dev;
+  p.sr_seed = static_cast<uint32_t>(c->cfg.sr_seed);
+  const size_t smem = fused_smem(lowp);
   const bool sk = grid % p.n_stripes != 0;
-  if (adam) {
-    if (sk) tc_update_gh_kernel<true, true><<<grid, kThreads, smem, s>>>(tm_master, tm_m, tm_v, tm_wout, p);
-    else tc_update_gh_kernel<true, false><<<grid, kThreads, smem, s>>>(tm_master, tm_m, tm_v, tm_wout, p);
+  if (lowp) {
+    if (sk) tc_update_gh_kernel<true, true, 1><<<grid, kThreads, smem, s>>>(tm_master, tm_m, tm_v, tm_wout, p);
+    else tc_update_gh_kernel<true, false, 1><<<grid, kThreads, smem, s>>>(tm_master, tm_m, tm_v, tm_wout, p);
+  } else if (adam) {
+    if (sk) tc_update_gh_kernel<true, true, 0><<<grid, kThreads, smem, s>>>(tm_master, tm_m, tm_v, tm_wout, p);
+    else tc_update_gh_kernel<true, false, 0><<<grid, kThreads, smem, s>>>(tm_master, tm_m, tm_v, tm_wout, p);
   } else {
-    if (sk) tc_update_gh_kernel<false, true><<<grid, kThreads, smem, s>>>(tm_master, tm_m, tm_v, tm_wout, p);
-    else tc_update_gh_kernel<false, false><<<grid, kThreads, smem, s>>>(tm_master, tm_m, tm_v, tm_wout, p);
+    if (sk) tc_update_gh_kernel<false, true, 0><<<grid, kThreads, smem, s>>>(tm_master, tm_m, tm_v, tm_wout, p);
+    else tc_update_gh_kernel<false, false, 0><<<grid, kThreads, smem, s>>>(tm_master, tm_m, tm_v, tm_wout, p);
   }
   *launches += 1;
   return cudaGetLastError();

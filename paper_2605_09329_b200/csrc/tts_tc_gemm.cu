@@ -43,6 +43,7 @@ struct Bars {
   uint64_t acc_empty[2];
   uint64_t conv[kMaxStages];   // gh: the stage's W tile is fp16 now
   uint32_t tmem_slot;
+  uint32_t done_ctr;           // epilogue warps finished (watchdog)
 };
 
 // ------------------------------------------------------------------ a2: draft logits
@@ -116,6 +117,7 @@ tc_logits_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant
   if (warp == 1 && lane == 0) {
     for (int i = 0; i < p.stages; ++i) { ptx::mbar_init(&bars->full[i], 1); ptx::mbar_init(&bars->empty[i], 1); }
     for (int i = 0; i < 2; ++i) { ptx::mbar_init(&bars->acc_full[i], 1); ptx::mbar_init(&bars->acc_empty[i], 4); }
+    bars->done_ctr = 0;
     ptx::fence_barrier_init();
   }
   if (warp == 2) {
@@ -217,6 +219,9 @@ tc_logits_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant
       __syncwarp();
       if (lane == 0) ptx::mbar_arrive(&bars->acc_empty[ab]);
     }
+    if (lane == 0) ptx::watchdog_arrive(&bars->done_ctr);
+  } else if (warp == 2) {
+    ptx::watchdog_wait(&bars->done_ctr, 4);
   }
   ptx::tc_fence_before();
   __syncthreads();
@@ -280,6 +285,7 @@ tc_gh_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant__ C
       ptx::mbar_init(&bars->full[i], 1); ptx::mbar_init(&bars->empty[i], MC ? 2 : 1); ptx::mbar_init(&bars->conv[i], 128);
     }
     for (int i = 0; i < 2; ++i) { ptx::mbar_init(&bars->acc_full[i], 1); ptx::mbar_init(&bars->acc_empty[i], 4); }
+    bars->done_ctr = 0;
     ptx::fence_barrier_init();
   }
   if (warp == 2) {
@@ -412,6 +418,9 @@ tc_gh_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant__ C
       __syncwarp();
       if (lane == 0) ptx::mbar_arrive(&bars->acc_empty[ab]);
     }
+    if (lane == 0) ptx::watchdog_arrive(&bars->done_ctr);
+  } else if (warp == 2) {
+    ptx::watchdog_wait(&bars->done_ctr, 4);
   }
   ptx::tc_fence_before();
   if (MC) ptx::cluster_sync(); else __syncthreads();

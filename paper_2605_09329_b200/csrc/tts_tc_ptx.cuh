@@ -49,16 +49,25 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
       : "memory");
   return ok != 0;
 }
-// Bounded wait.  The first probe is the fast path; after that the spin is watched by the SM clock, and a phase that
-// has not completed after ~2^33 cycles (4 s at 1.9 GHz; a step takes milliseconds) is a protocol error: the thread
-// traps, the launch fails with cudaErrorLaunchFailed and the host sees TTS_ERR_CUDA instead of a hung GPU.
-constexpr long long kMbarTimeoutCycles = 1ll << 33;
+// The pipeline waits are plain spins: every bounded form tried (a clock check in the loop, an out-of-line slow path,
+// an iteration counter) cost the one-canvas update kernel 1.7 - 5% through ptxas' schedule of its epilogue (measured
+// A/B on one box, profiles/r2_README.md).  A stalled pipeline is caught by a WATCHDOG instead: the warp that only
+// allocates tensor memory sleeps until every epilogue warp (the last stage of each kernel's pipeline) has finished, and
+// traps if that takes more than ~2^34 cycles (8.7 s at 1.965 GHz; a step takes milliseconds).  The launch then fails
+// with cudaErrorLaunchFailed and the host sees TTS_ERR_CUDA instead of a hung GPU.
+constexpr long long kWatchdogCycles = 1ll << 34;
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-  if (mbar_try_wait(bar, parity)) return;
-  const long long t0 = clock64();
-  uint32_t n = 0;
   while (!mbar_try_wait(bar, parity)) {
-    if ((++n & 0xFFFu) == 0 && clock64() - t0 > kMbarTimeoutCycles) asm volatile("trap;");
+  }
+}
+// epilogue warps: one arrival each when their loop is over
+__device__ __forceinline__ void watchdog_arrive(uint32_t* ctr) { atomicAdd(ctr, 1u); }
+// the watchdog warp (all lanes): returns when `need` epilogue warps have arrived, traps on timeout
+__device__ __forceinline__ void watchdog_wait(uint32_t* ctr, uint32_t need) {
+  const long long t0 = clock64();
+  while (*reinterpret_cast<volatile uint32_t*>(ctr) < need) {
+    __nanosleep(20000);
+    if (clock64() - t0 > kWatchdogCycles) asm volatile("trap;");
   }
 }
 
@@ -234,8 +243,7 @@ __device__ __forceinline__ void mbar_arrive_cta0(uint64_t* bar) {
 }
 // wait with acquire at cluster scope: the arrivals come from both CTAs of the pair
 __device__ __forceinline__ void mbar_wait_cluster(uint64_t* bar, uint32_t parity) {
-  uint32_t ok = 0, n = 0;
-  long long t0 = 0;
+  uint32_t ok = 0;
   while (!ok) {
     asm volatile(
         "{\n\t.reg .pred p;\n\t"
@@ -244,10 +252,6 @@ __device__ __forceinline__ void mbar_wait_cluster(uint64_t* bar, uint32_t parity
         : "=r"(ok)
         : "r"(smem_u32(bar)), "r"(parity)
         : "memory");
-    if (!ok) {   // bounded like mbar_wait
-      if (n == 0) t0 = clock64();
-      if ((++n & 0xFFFu) == 0 && clock64() - t0 > kMbarTimeoutCycles) asm volatile("trap;");
-    }
   }
 }
 // 2-D tiled load into THIS CTA's shared memory; the bytes are counted on CTA 0's mbarrier

@@ -26,6 +26,7 @@
 #include <cuda_fp16.h>
 #include <string.h>
 
+#include "tts_adam.cuh"
 #include "tts_common.cuh"
 #include "tts_tc_ptx.cuh"
 #include "tts_tc_state.h"
@@ -36,10 +37,12 @@ namespace {
 constexpr int kWJ = 128;                 // stripe width = MMA M = TMEM lanes
 constexpr int kWSV = 8;                  // vocabulary rows per state stage
 constexpr int kWTensorBytes = kWSV * kWJ * 4;   // 4 KB per tensor per stage
-constexpr int kWStageBytes = 3 * kWTensorBytes; // 12 KB
+constexpr int kWStageBytes = 3 * kWTensorBytes; // 12 KB (fp32 moments)
+constexpr int kWMomBytesLp = kWSV * kWJ * 2;    // 2 KB per bf16 moment tensor per stage
+constexpr int kWStageBytesLp = kWTensorBytes + 2 * kWMomBytesLp;   // 8 KB (bf16 moments, TTS_MOMENT_BF16)
 constexpr int kWWoBytes = kWSV * kWJ * 2;       // 2 KB: bf16 staging of one sub-tile (one per epilogue group)
 constexpr int kWThreads = 384;           // warp 0 state TMA, 1 MMA, 2 TMEM alloc, 3 operand TMA, 4-11 epilogue
-constexpr int kWMaxStages = 16;
+constexpr int kWMaxStages = 24;
 constexpr int kWOpStagesMax = 4;         // dl band ring (depth chosen per launch)
 constexpr int kWSmemBudget = 225 * 1024;
 constexpr int kWAccCols = 64;            // TMEM columns reserved for the two gW accumulators (NV <= 32)
@@ -57,6 +60,8 @@ struct WideParams {
   int V, d, Kp;
   int n_stripes, n_bands, n_win, stages, op_stages;
   const float* step_scalars;  // device {1 / (1 - b1^n), 1 / sqrt(1 - b2^n)} of this step
+  const unsigned long long* step_count;   // device: Adam's count n of this step (keys the stochastic rounding of v)
+  uint32_t sr_seed;
   float lr, b1, b2, eps, decay;   // decay = 1 - lr wd
 };
 
@@ -70,6 +75,7 @@ struct WideBars {
   uint64_t a_full;
   uint64_t wt_full, wt_empty, gh_full, gh_empty;   // GH
   uint32_t tmem_slot;
+  uint32_t done_ctr;   // epilogue warps finished (watchdog)
 };
 
 // The sequence of (stripe, band) units of this CTA: window by window, a contiguous range of each window's units --
@@ -116,7 +122,8 @@ __device__ __forceinline__ uint64_t desc64(uint32_t hi, uint32_t lo) { return (s
 // written to shared memory as fp16(16 W) (the A operand), the dl band already in shared memory is read a second
 // time as the MN-major B operand, and the stripe's accumulators [128 j x planes T16] persist in tensor memory until
 // the CTA leaves the stripe.  No gh kernel, no second pass over W.
-template <bool ADAM, int NV, bool GH>
+// MOM: 1 = bf16 moments (TTS_MOMENT_BF16; stages of 8 KB; m nearest-even, v stochastic rounding: tts_adam.cuh)
+template <bool ADAM, int NV, bool GH, int MOM>
 __global__ void __launch_bounds__(kWThreads, 1)
 tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
                       const __grid_constant__ CUtensorMap tm_master, const __grid_constant__ CUtensorMap tm_m,
@@ -125,11 +132,13 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   constexpr int kSubs = NV / kWSV;
+  constexpr int kStageB = MOM ? kWStageBytesLp : kWStageBytes;
+  constexpr int kMomB = MOM ? kWMomBytesLp : kWTensorBytes;
   const int b_bytes = NV * p.Kp * 2;                   // [Kp / 64][NV v][64 k] fp16, 128-byte swizzle
   uint8_t* sB = smem;
   const int kWOpStages = p.op_stages;
   uint8_t* st = sB + kWOpStages * b_bytes;             // [stages][3][8 v][128 j] fp32
-  uint8_t* wo = st + p.stages * kWStageBytes;          // [2 groups][8 v][128 j] bf16
+  uint8_t* wo = st + p.stages * kStageB;               // [2 groups][8 v][128 j] bf16
   uint8_t* wt = wo + 2 * kWWoBytes;                    // GH: [4 v-groups][16 j-groups][8 j][8 v] fp16, K-major core matrices
   WideBars* bars = reinterpret_cast<WideBars*>(wt + (GH ? kWWtBytes : 0));
 
@@ -153,6 +162,7 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
     ptx::mbar_init(&bars->wt_empty, 1);
     ptx::mbar_init(&bars->gh_full, 1);
     ptx::mbar_init(&bars->gh_empty, 4);
+    bars->done_ctr = 0;
     ptx::fence_barrier_init();
   }
   if (warp == 2) {
@@ -181,13 +191,13 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
           if (GH) { s = ps; ph = pph; if (++ps == p.stages) { ps = 0; pph ^= 1; } }
           else { s = n % p.stages; ph = (n / p.stages) & 1; }   // see the epilogue for why the two instances differ
           ptx::mbar_wait(&bars->st_empty[s], ph ^ 1);
-          uint8_t* dst = st + s * kWStageBytes;
-          ptx::mbar_expect_tx(&bars->st_full[s], (ADAM ? 3 : 1) * kWTensorBytes);
+          uint8_t* dst = st + s * kStageB;
+          ptx::mbar_expect_tx(&bars->st_full[s], ADAM ? kWTensorBytes + 2 * kMomB : kWTensorBytes);
           const int r0 = v0 + sub * kWSV;
           ptx::tma_load_2d_hint(dst, &tm_master, &bars->st_full[s], j0, r0, pol);
           if (ADAM) {
             ptx::tma_load_2d_hint(dst + kWTensorBytes, &tm_m, &bars->st_full[s], j0, r0, pol);
-            ptx::tma_load_2d_hint(dst + 2 * kWTensorBytes, &tm_v, &bars->st_full[s], j0, r0, pol);
+            ptx::tma_load_2d_hint(dst + kWTensorBytes + kMomB, &tm_v, &bars->st_full[s], j0, r0, pol);
           }
         }
       }
@@ -290,6 +300,7 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
     __nv_bfloat16* wo_g = reinterpret_cast<__nv_bfloat16*>(wo + g * kWWoBytes);
     const float inv_s = p.dl_scale[1] * p.dl_scale[3];
     const float c1 = ADAM ? p.lr * p.step_scalars[0] : 0.f, inv_sqrt_bc2 = ADAM ? p.step_scalars[1] : 0.f;
+    const uint32_t key = MOM ? sr_key(static_cast<uint32_t>(*p.step_count), p.sr_seed) : 0u;
     WideWalk w(p);
     uint32_t i = 0, n_flush = 0;
     int stripe, band, cur = -1, prev_s = -1;
@@ -373,12 +384,17 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
         uint32_t gr[kWSV];
         ptx::tmem_ld_32x32b_x8(tmem_base + ab * NV + sub * kWSV + lane_bits, gr);
         ptx::mbar_wait(&bars->st_full[s], st_par);
-        float* sM = reinterpret_cast<float*>(st + s * kWStageBytes) + jj;
+        float* sM = reinterpret_cast<float*>(st + s * kStageB) + jj;
+        uint16_t* sLm = reinterpret_cast<uint16_t*>(st + s * kStageB + kWTensorBytes) + jj;   // MOM: bf16 m, then v
+        uint16_t* sLv = reinterpret_cast<uint16_t*>(st + s * kStageB + kWTensorBytes + kMomB) + jj;
         float M[kWSV], mm[kWSV], vv[kWSV];
 #pragma unroll
         for (int r = 0; r < kWSV; ++r) {
           M[r] = sM[r * kWJ];
-          if (ADAM) { mm[r] = sM[kWSV * kWJ + r * kWJ]; vv[r] = sM[2 * kWSV * kWJ + r * kWJ]; }
+          if (ADAM) {
+            if (MOM) { mm[r] = bf16_bits_widen(sLm[r * kWJ]); vv[r] = bf16_bits_widen(sLv[r * kWJ]); }
+            else { mm[r] = sM[kWSV * kWJ + r * kWJ]; vv[r] = sM[2 * kWSV * kWJ + r * kWJ]; }
+          }
         }
         if (GH) {
           // a5 operand: W_in[v, j] = rn_bf16(master[v, j]), as fp16(16 W): rows 8 sub .. 8 sub + 7 of this thread's column
@@ -409,9 +425,16 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
             const float m1 = p.b1 * mm[r] + (1.f - p.b1) * gg;
             const float v1 = p.b2 * vv[r] + (1.f - p.b2) * gg * gg;
             const float den = __fsqrt_rn(v1) * inv_sqrt_bc2 + p.eps;
-            M[r] = M[r] * p.decay - __fdividef(c1 * m1, den);
-            sM[kWSV * kWJ + r * kWJ] = m1;
-            sM[2 * kWSV * kWJ + r * kWJ] = v1;
+            M[r] = M[r] * p.decay - __fdividef(c1 * m1, den);     // the step uses the unrounded moments
+            if (MOM) {
+              const unsigned long long idx =
+                  (unsigned long long)(v0 + sub * kWSV + r) * (unsigned long long)p.d + (j0 + jj);
+              sLm[r * kWJ] = bf16_bits_rn(m1);
+              sLv[r * kWJ] = bf16_bits_sr(v1, sr_bits16(idx, key));
+            } else {
+              sM[kWSV * kWJ + r * kWJ] = m1;
+              sM[2 * kWSV * kWJ + r * kWJ] = v1;
+            }
           } else {
             M[r] = M[r] - p.lr * gg;
           }
@@ -434,11 +457,11 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
         ptx::named_barrier_sync(1 + g, 128);
         if (leader) {
           const int r0 = v0 + sub * kWSV;
-          const float* sT = reinterpret_cast<const float*>(st + s * kWStageBytes);
+          const uint8_t* sT = st + s * kStageB;
           ptx::tma_store_2d(&tm_master, sT, j0, r0);
           if (ADAM) {
-            ptx::tma_store_2d(&tm_m, sT + kWSV * kWJ, j0, r0);
-            ptx::tma_store_2d(&tm_v, sT + 2 * kWSV * kWJ, j0, r0);
+            ptx::tma_store_2d(&tm_m, sT + kWTensorBytes, j0, r0);
+            ptx::tma_store_2d(&tm_v, sT + kWTensorBytes + kMomB, j0, r0);
           }
           ptx::tma_store_2d(&tm_wout, wo_g, j0, r0);
           ptx::bulk_commit_group();
@@ -452,6 +475,9 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
     }
     if (GH && cur >= 0) flush_gh(cur);
     if (leader) ptx::bulk_wait_group_read<0>();   // shared memory must outlive the last stores' reads
+    if (lane == 0) ptx::watchdog_arrive(&bars->done_ctr);
+  } else if (warp == 2) {
+    ptx::watchdog_wait(&bars->done_ctr, 8);
   }
   ptx::tc_fence_before();
   __syncthreads();
@@ -604,18 +630,18 @@ __global__ void __launch_bounds__(256) tc_prep_dl_wide_kernel(const void* __rest
   }
 }
 
-template <bool ADAM, int NV, bool GH>
+template <bool ADAM, int NV, bool GH, int MOM>
 cudaError_t launch_wide(int grid, size_t smem, cudaStream_t s, const CUtensorMap& tm_dlT,
                         const CUtensorMap& tm_master, const CUtensorMap& tm_m, const CUtensorMap& tm_v,
                         const CUtensorMap& tm_wout, const WideParams& p) {
-  tc_update_wide_kernel<ADAM, NV, GH><<<grid, kWThreads, smem, s>>>(tm_dlT, tm_master, tm_m, tm_v, tm_wout, p);
+  tc_update_wide_kernel<ADAM, NV, GH, MOM><<<grid, kWThreads, smem, s>>>(tm_dlT, tm_master, tm_m, tm_v, tm_wout, p);
   return cudaGetLastError();
 }
 
 
-template <bool ADAM, int NV, bool GH>
+template <bool ADAM, int NV, bool GH, int MOM>
 cudaError_t wide_attr() {
-  return cudaFuncSetAttribute(tc_update_wide_kernel<ADAM, NV, GH>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  return cudaFuncSetAttribute(tc_update_wide_kernel<ADAM, NV, GH, MOM>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                               kWSmemBudget + 2048);
 }
 
@@ -623,10 +649,12 @@ cudaError_t wide_attr() {
 
 cudaError_t tc_wide_init(tts_ctx*) {
   cudaError_t e;
-  if ((e = wide_attr<true, 32, false>()) != cudaSuccess) return e;
-  if ((e = wide_attr<false, 32, false>()) != cudaSuccess) return e;
-  if ((e = wide_attr<true, 32, true>()) != cudaSuccess) return e;
-  return wide_attr<false, 32, true>();
+  if ((e = wide_attr<true, 32, false, 0>()) != cudaSuccess) return e;
+  if ((e = wide_attr<false, 32, false, 0>()) != cudaSuccess) return e;
+  if ((e = wide_attr<true, 32, true, 0>()) != cudaSuccess) return e;
+  if ((e = wide_attr<false, 32, true, 0>()) != cudaSuccess) return e;
+  if ((e = wide_attr<true, 32, false, 1>()) != cudaSuccess) return e;
+  return wide_attr<true, 32, true, 1>();
 }
 
 // dl planes of the wide path: hi + lo while both fit the 64-wide K chunk (T16 <= 32), one plane beyond
@@ -689,12 +717,13 @@ cudaError_t tc_launch_update_wide(tts_ctx* c, const StepArgs& a, cudaStream_t s,
     return cudaErrorInvalidValue;
   tm_m = tm_master;
   tm_v = tm_master;
+  const bool lowp = adam && c->cfg.moment_dtype == TTS_MOMENT_BF16;
   if (adam) {
-    if (make_map_2d(st, &tm_m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, a.adam_m, d, V, kWJ, kWSV,
-                    CU_TENSOR_MAP_SWIZZLE_NONE) != CUDA_SUCCESS)
+    const CUtensorMapDataType mdt = lowp ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
+    const int msz = lowp ? 2 : 4;
+    if (make_map_2d(st, &tm_m, mdt, msz, a.adam_m, d, V, kWJ, kWSV, CU_TENSOR_MAP_SWIZZLE_NONE) != CUDA_SUCCESS)
       return cudaErrorInvalidValue;
-    if (make_map_2d(st, &tm_v, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, a.adam_v, d, V, kWJ, kWSV,
-                    CU_TENSOR_MAP_SWIZZLE_NONE) != CUDA_SUCCESS)
+    if (make_map_2d(st, &tm_v, mdt, msz, a.adam_v, d, V, kWJ, kWSV, CU_TENSOR_MAP_SWIZZLE_NONE) != CUDA_SUCCESS)
       return cudaErrorInvalidValue;
   }
   WideParams p;
@@ -715,22 +744,28 @@ cudaError_t tc_launch_update_wide(tts_ctx* c, const StepArgs& a, cudaStream_t s,
   if (gh_here && (e = cudaMemsetAsync(a.gh_out, 0, (size_t)T * d * sizeof(float), s)) != cudaSuccess) return e;
   p.op_stages = gh_here ? 3 : 2;   // with gh a band's dl rows stay until the gh MMAs issued one band later have read them
   const int fixed = 1024 + p.op_stages * NV * Kp * 2 + 2 * kWWoBytes + (gh_here ? kWWtBytes : 0) + (int)sizeof(WideBars);
-  p.stages = (kWSmemBudget - fixed) / kWStageBytes;
-  if (p.stages > kWMaxStages) p.stages = kWMaxStages;
+  const int stage_bytes = lowp ? kWStageBytesLp : kWStageBytes;
+  p.stages = (kWSmemBudget - fixed) / stage_bytes;
+  if (p.stages > (lowp ? kWMaxStages : 16)) p.stages = lowp ? kWMaxStages : 16;
   if (p.stages < 2) return cudaErrorInvalidConfiguration;
   p.lr = a.lr; p.b1 = a.beta1; p.b2 = a.beta2; p.eps = a.eps;
   p.decay = 1.f - a.lr * a.wd;
   p.step_scalars = a.step_scalars;
+  p.step_count = c->step_count_dev;
+  p.sr_seed = static_cast<uint32_t>(c->cfg.sr_seed);
   const long units = (long)p.n_stripes * (p.n_bands / p.n_win);
   int grid = c->cfg.max_ctas > 0 ? c->cfg.max_ctas : c->sm_count;
   if (grid > units) grid = (int)units;
-  const size_t smem = (size_t)fixed + (size_t)p.stages * kWStageBytes;
-  if (gh_here)
-    e = adam ? launch_wide<true, NV, true>(grid, smem, s, tm_dlT, tm_master, tm_m, tm_v, tm_wout, p)
-             : launch_wide<false, NV, true>(grid, smem, s, tm_dlT, tm_master, tm_m, tm_v, tm_wout, p);
+  const size_t smem = (size_t)fixed + (size_t)p.stages * stage_bytes;
+  if (lowp)
+    e = gh_here ? launch_wide<true, NV, true, 1>(grid, smem, s, tm_dlT, tm_master, tm_m, tm_v, tm_wout, p)
+                : launch_wide<true, NV, false, 1>(grid, smem, s, tm_dlT, tm_master, tm_m, tm_v, tm_wout, p);
+  else if (gh_here)
+    e = adam ? launch_wide<true, NV, true, 0>(grid, smem, s, tm_dlT, tm_master, tm_m, tm_v, tm_wout, p)
+             : launch_wide<false, NV, true, 0>(grid, smem, s, tm_dlT, tm_master, tm_m, tm_v, tm_wout, p);
   else
-    e = adam ? launch_wide<true, NV, false>(grid, smem, s, tm_dlT, tm_master, tm_m, tm_v, tm_wout, p)
-             : launch_wide<false, NV, false>(grid, smem, s, tm_dlT, tm_master, tm_m, tm_v, tm_wout, p);
+    e = adam ? launch_wide<true, NV, false, 0>(grid, smem, s, tm_dlT, tm_master, tm_m, tm_v, tm_wout, p)
+             : launch_wide<false, NV, false, 0>(grid, smem, s, tm_dlT, tm_master, tm_m, tm_v, tm_wout, p);
   *launches += 1;
   return e;
 }

@@ -22,7 +22,7 @@ class DraftHeadUpdater:
     def __init__(self, W, master, adam_m, adam_v, *, seg_len, T_max, stride=1, lr=1e-5, beta1=0.9, beta2=0.999,
                  eps=1e-8, weight_decay=0.0, optimizer=tts.TTS_ADAMW, logits_dtype=tts.TTS_BF16,
                  mask_mode=tts.TTS_ROWS_ALL, max_ctas=0, host_barrier=False, want_gh=True, keep_snapshot=False,
-                 use_graph=False):
+                 use_graph=False, moment_dtype=tts.TTS_MOMENT_F32, flags=0, priority=None):
         assert stride >= 1
         V, d = W.shape
         self.V, self.d, self.seg_len, self.T_max, self.stride = V, d, seg_len, T_max, int(stride)
@@ -31,9 +31,11 @@ class DraftHeadUpdater:
         self.cur = 0
         self.master, self.m, self.v = master, adam_m, adam_v
         self.host_barrier = host_barrier          # CPU-side barrier in front of CUDA-graph replay
-        self.side = torch.cuda.Stream(device=self.device)
+        # priority: CUDA stream priority of the side stream (None = default; -1 = high, 0 = low on this device)
+        self.side = (torch.cuda.Stream(device=self.device) if priority is None else
+                     torch.cuda.Stream(device=self.device, priority=priority))
         cfg = tts.make_config(V, d, T_max, seg_len, tts.TTS_BF16, logits_dtype, optimizer, lr, beta1, beta2, eps,
-                              weight_decay, mask_mode, max_ctas)
+                              weight_decay, mask_mode, max_ctas, moment_dtype=moment_dtype, flags=flags)
         self.ctx = tts.tts_ctx_create(cfg, self.device.index or 0)
         self.mask = torch.zeros(T_max, dtype=torch.uint8, device=self.device)
         self.tau = torch.zeros(T_max // seg_len, dtype=torch.int32, device=self.device)

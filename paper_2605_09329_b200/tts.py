@@ -37,7 +37,7 @@ class tts_config(C.Structure):
                 ("lr", C.c_float), ("beta1", C.c_float), ("beta2", C.c_float), ("eps", C.c_float),
                 ("weight_decay", C.c_float), ("mask_mode", C.c_int32), ("max_ctas", C.c_int32),
                 ("kernel_path", C.c_int32), ("moment_dtype", C.c_int32), ("max_inner_steps", C.c_int32),
-                ("flags", C.c_int32)]
+                ("flags", C.c_int32), ("sr_seed", C.c_int32)]
 
 
 EXPORTS = {
@@ -53,6 +53,7 @@ EXPORTS = {
     "tts_get_step_count_on": (C.c_int64, [C.c_void_p, C.c_void_p]),
     "tts_last_device_status": (C.c_int32, [C.c_void_p]),
     "tts_check_preconditions": (C.c_int32, [C.c_void_p] * 5 + [C.c_int32, C.c_void_p]),
+    "tts_debug_trip_watchdog": (C.c_int32, [C.c_void_p, C.c_void_p]),
     "tts_last_cuda_error": (C.c_int32, [C.c_void_p]),
     "tts_last_step_used_tensor_path": (C.c_int32, [C.c_void_p]),
     "tts_last_launch_count": (C.c_int32, [C.c_void_p]),
@@ -181,6 +182,11 @@ def tts_check_preconditions(ctx, teacher_logits, h, W_in, W_master, T, stream=No
     st = lib().tts_check_preconditions(ctx, _ptr(teacher_logits), _ptr(h), _ptr(W_in), _ptr(W_master), T,
                                        _stream(stream, ctx))
     _check(ctx, st, "tts_check_preconditions")
+
+
+def tts_debug_trip_watchdog(ctx, stream=None) -> int:
+    """Returns the status (TTS_ERR_CUDA expected); the CUDA context is dead afterwards."""
+    return lib().tts_debug_trip_watchdog(ctx, _stream(stream, ctx))
 
 
 def tts_last_cuda_error(ctx) -> int:
@@ -312,6 +318,7 @@ def tts_shard_accept_mask(ctx, val_all, idx_all, n_shards, draft_tokens, T, mask
 
 def make_config(V, d, T_max, seg_len, param_dtype=TTS_BF16, logits_dtype=TTS_BF16, optimizer=TTS_ADAMW, lr=1e-5,
                 beta1=0.9, beta2=0.999, eps=1e-8, weight_decay=0.0, mask_mode=TTS_ROWS_ALL, max_ctas=0,
-                kernel_path=TTS_PATH_AUTO, moment_dtype=TTS_MOMENT_F32, max_inner_steps=0, flags=0) -> tts_config:
+                kernel_path=TTS_PATH_AUTO, moment_dtype=TTS_MOMENT_F32, max_inner_steps=0, flags=0,
+                sr_seed=0) -> tts_config:
     return tts_config(V, d, T_max, seg_len, param_dtype, logits_dtype, optimizer, lr, beta1, beta2, eps,
-                      weight_decay, mask_mode, max_ctas, kernel_path, moment_dtype, max_inner_steps, flags)
+                      weight_decay, mask_mode, max_ctas, kernel_path, moment_dtype, max_inner_steps, flags, sr_seed)

@@ -34,12 +34,15 @@ def config_for(case, *, mask_mode=tts.TTS_ROWS_ALL, kernel_path=tts.TTS_PATH_AUT
 
 
 def run_gpu(case, *, mask_mode=tts.TTS_ROWS_ALL, kernel_path=tts.TTS_PATH_AUTO, want_gW=True, want_gh=True,
-            alias_w=False, side_stream=True, max_ctas=0, flags=0):
+            alias_w=False, side_stream=True, max_ctas=0, flags=0, moments="f32", sr_seed=0):
     """One tts_accept_mask + tts_distill_step on cuda:0.  Returns a dict of numpy results."""
     T, V, d = case["T"], case["V"], case["d"]
     bf = case["cfg"]["param"] == synth.BF16
-    ctx = tts.tts_ctx_create(config_for(case, mask_mode=mask_mode, kernel_path=kernel_path, max_ctas=max_ctas,
-                                        flags=flags), 0)
+    lowp = moments == "bf16"
+    cfg = config_for(case, mask_mode=mask_mode, kernel_path=kernel_path, max_ctas=max_ctas, flags=flags,
+                     moment_dtype=tts.TTS_MOMENT_BF16 if lowp else tts.TTS_MOMENT_F32)
+    cfg.sr_seed = sr_seed
+    ctx = tts.tts_ctx_create(cfg, 0)
     try:
         if case.get("step", 1) > 1:
             tts.tts_set_step_count(ctx, case["step"] - 1)
@@ -47,7 +50,10 @@ def run_gpu(case, *, mask_mode=tts.TTS_ROWS_ALL, kernel_path=tts.TTS_PATH_AUTO, 
         W_in = _dev(case["W"])
         W_out = W_in if alias_w else torch.empty_like(W_in)
         master = _dev(case["master"]) if bf else None
-        m, v = _dev(case["m"]), _dev(case["v"])
+        if lowp:     # bf16 moment storage: the case's fp32 moments rounded to nearest (uint16 bits -> bf16 tensors)
+            m, v = _dev(synth.f32_to_bf16_bits(case["m"])), _dev(synth.f32_to_bf16_bits(case["v"]))
+        else:
+            m, v = _dev(case["m"]), _dev(case["v"])
         pw = _dev(case["pos_weight"])
         mask = torch.zeros(T, dtype=torch.uint8, device="cuda")
         tau = torch.zeros(T // case["seg_len"], dtype=torch.int32, device="cuda")
@@ -77,21 +83,28 @@ def run_gpu(case, *, mask_mode=tts.TTS_ROWS_ALL, kernel_path=tts.TTS_PATH_AUTO, 
         else:
             out["master"] = W_out.cpu().numpy()
             out["W_out"] = out["master"]
-        out["m"] = m.cpu().numpy() if m is not None else None
-        out["v"] = v.cpu().numpy() if v is not None else None
+        if lowp:
+            out["m_bits"], out["v_bits"] = bits(m), bits(v)
+            out["m"], out["v"] = synth.bf16_bits_to_f32(out["m_bits"]), synth.bf16_bits_to_f32(out["v_bits"])
+        else:
+            out["m"] = m.cpu().numpy() if m is not None else None
+            out["v"] = v.cpu().numpy() if v is not None else None
         return out
     finally:
         tts.tts_ctx_destroy(ctx)
 
 
-def run_oracle(case, *, mask_mode=O.ROWS_ALL):
+def run_oracle(case, *, mask_mode=O.ROWS_ALL, moments="f32", sr_seed=0):
     c = case["cfg"]
     mask, tau, am = O.accept_mask(case["teacher"], case["draft_tokens"], case["seg_len"])
-    r = O.distill_step(case["teacher"], case["h"], case["W"], case["master"], case["m"], case["v"],
+    m_in, v_in = case["m"], case["v"]
+    if moments == "bf16":
+        m_in, v_in = O.f32_to_bf16_bits(m_in), O.f32_to_bf16_bits(v_in)
+    r = O.distill_step(case["teacher"], case["h"], case["W"], case["master"], m_in, v_in,
                        case["pos_weight"], mask, seg_len=case["seg_len"], mask_mode=mask_mode,
                        loss_scale=case["loss_scale"], optimizer="sgd" if c["optimizer"] == synth.SGD else "adamw",
                        lr=c["lr"], beta1=c["beta1"], beta2=c["beta2"], eps=c["eps"], weight_decay=c["weight_decay"],
-                       step=case.get("step", 1))
+                       step=case.get("step", 1), moments=moments, sr_seed=sr_seed)
     r.update(mask=mask, tau=tau, argmax=am)
     return r
 

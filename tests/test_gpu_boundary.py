@@ -207,3 +207,31 @@ def test_default_mode_weights_are_bit_reproducible(V, d, n_seq):
     assert a["loss"] == b["loss"]
     for k in ("master", "m", "v", "W_out", "kl_rows"):
         np.testing.assert_array_equal(a[k], b[k], err_msg=k)
+
+
+def test_a_stalled_pipeline_traps_instead_of_hanging():
+    """A protocol slip inside a tensor-path kernel (a wait nobody satisfies) ends in TTS_ERR_CUDA after the watchdog's
+    ~9 s, not in a hung GPU.  The trap kills the CUDA context, so the probe runs in a process of its own."""
+    import os
+    import subprocess
+    import sys
+    import time
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    code = ("import sys; sys.path.insert(0, %r)\n"
+            "import torch\n"
+            "from paper_2605_09329_b200 import tts\n"
+            "ctx = tts.tts_ctx_create(tts.make_config(2048, 128, 16, 16), 0)\n"
+            "st = tts.tts_debug_trip_watchdog(ctx, torch.cuda.Stream())\n"
+            "print('STATUS', st, tts.tts_last_cuda_error(ctx))\n" % root)
+    t0 = time.time()
+    r = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=120)
+    dt = time.time() - t0
+    line = [l for l in r.stdout.splitlines() if l.startswith("STATUS")]
+    assert line, (r.stdout, r.stderr[-500:])
+    _, st, cuda_err = line[0].split()
+    assert int(st) == tts.TTS_ERR_CUDA and int(cuda_err) != 0
+    assert 4.0 < dt < 60.0, dt
+    # this process's context is untouched: a step still runs
+    case = synth.make_case(3, V=2048, d=256)
+    g, o = run_gpu(case), run_oracle(case)
+    check_step(g, o, case)

@@ -1,0 +1,133 @@
+"""f4: the step with Adam's moments STORED in bf16 (TTS_MOMENT_BF16, R26; the paper fixes only
+"Adam"), against oracle.adamw_update_lowp on the same seeded inputs, through every update kernel.
+
+What is compared, and why at these tolerances.  The parameter step uses the unrounded new moments, so loss, gh, the
+master, the working copy and the update itself (R13) keep the fp32-moment tolerances.  What is STORED is a rounding
+decision on an fp32 value: the GPU's fp32 moments differ from the oracle's by the gradient's tolerance (bf16 / fp16
+operand planes), so a stored code may land on the neighbouring bf16: values within one bf16 ulp (half for m) plus
+the gradient tolerance.  The rounding RULE itself (nearest-even for m, the counter-based stochastic rounding for v)
+is pinned bit for bit where the gradient is exactly zero (teacher == given draft logits): then both sides round the
+same fp32 number."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import tts_oracle as O
+from paper_2605_09329_b200 import tts
+from workloads import synth
+
+from gpu_util import _dev, bits, check_step, config_for, max_abs, run_gpu, run_oracle
+
+pytestmark = pytest.mark.gpu
+
+SHAPES = [(4096, 1024, 1), (4096, 256, 1), (2048 + 128, 256, 4), (2048, 256, 16), (2048 + 384, 256, 32)]
+
+
+def _check_stored(g, o):
+    """stored moments: within half a bf16 ulp (m) / one ulp (v) of the oracle's unrounded moments, plus the gradient
+    tolerance; most codes identical"""
+    m_ref, v_ref = o["m"], o["v"]
+    gm, gv = g["m"].astype(np.float64), g["v"].astype(np.float64)
+    assert np.all(np.abs(gm - m_ref) <= 2.0 ** -8 * np.abs(m_ref) + 2e-3 * max_abs(m_ref))
+    assert np.all(np.abs(gv - v_ref) <= 2.0 ** -7 * np.abs(v_ref) + 2e-3 * max_abs(v_ref))
+    dm = np.abs(g["m_bits"].astype(np.int32) - o["m_bits"].astype(np.int32))
+    dv = np.abs(g["v_bits"].astype(np.int32) - o["v_bits"].astype(np.int32))
+    return float((dm == 0).mean()), float((dv == 0).mean()), int(dm.max()), int(dv.max())
+
+
+@pytest.mark.parametrize("V,d,n_seq", SHAPES)
+@pytest.mark.parametrize("kind,step", [(None, 1), ("mix", 5), ("const10", 11)])
+def test_bf16_moments_match_oracle(V, d, n_seq, kind, step):
+    case = synth.make_case(3 if n_seq == 1 else 4, V=V, d=d, n_seq=n_seq, nonzero_state=kind or False, step=step)
+    # the state both sides start from is the bf16-rounded one
+    case["m"] = synth.bf16_bits_to_f32(synth.f32_to_bf16_bits(case["m"]))
+    case["v"] = synth.bf16_bits_to_f32(synth.f32_to_bf16_bits(case["v"]))
+    g = run_gpu(case, moments="bf16", sr_seed=7)
+    o = run_oracle(case, moments="bf16", sr_seed=7)
+    assert g["used_tensor"] == 1
+    gm, gv = g.pop("m"), g.pop("v")            # check_step: everything but the stored moments (fp32-moment tolerances)
+    g["m"] = g["v"] = None
+    check_step(g, o, case)
+    g["m"], g["v"] = gm, gv
+    eq_m, eq_v, worst_m, worst_v = _check_stored(g, o)
+    print("stored codes identical: m %.4f, v %.4f; worst code distance m %d, v %d" % (eq_m, eq_v, worst_m, worst_v))
+    assert eq_m >= 0.7 and eq_v >= 0.5
+
+
+@pytest.mark.parametrize("V,d,n_seq", SHAPES)
+def test_rounding_rule_is_bit_exact_at_zero_gradient(V, d, n_seq):
+    """teacher (fp32) == the given draft logits bit for bit: dl, gW are exactly 0, the new moments are beta * old,
+    computed in fp32 on both sides (the oracle is handed fp32(beta)), and the stored bf16 codes -- nearest-even m,
+    stochastically rounded v with the draws of (element, n = 9, seed = 12345) -- must agree on EVERY element."""
+    case = synth.make_case(3 if n_seq == 1 else 4, V=V, d=d, n_seq=n_seq, nonzero_state="mix", step=9)
+    T = case["T"]
+    z = (O.widen(case["h"]) @ O.widen(case["W"]).T).astype(np.float32)
+    case["teacher"] = z.copy()
+    case["cfg"]["logits"] = synth.F32
+    m_bits, v_bits = synth.f32_to_bf16_bits(case["m"]), synth.f32_to_bf16_bits(case["v"])
+    c = case["cfg"]
+    cfg = config_for(case, moment_dtype=tts.TTS_MOMENT_BF16)
+    cfg.sr_seed = 12345
+    ctx = tts.tts_ctx_create(cfg, 0)
+    try:
+        tts.tts_set_step_count(ctx, 8)
+        W_in, master = _dev(case["W"]), _dev(case["master"])
+        W_out = torch.empty_like(W_in)
+        m, v = _dev(m_bits), _dev(v_bits)
+        loss = torch.zeros(1, device="cuda")
+        tts.tts_distill_step_ex(ctx, _dev(case["teacher"]), _dev(case["h"]), W_in, W_out, master, m, v,
+                                _dev(case["pos_weight"]), None, T, case["loss_scale"], loss, None, None, None,
+                                draft_logits=_dev(z))
+        tts.tts_sync_step(ctx)
+        assert float(loss.item()) == 0.0
+        b1, b2 = float(np.float32(c["beta1"])), float(np.float32(c["beta2"]))
+        idx = np.arange(V, dtype=np.uint64)[:, None] * np.uint64(d) + np.arange(d, dtype=np.uint64)[None, :]
+        _, mq, vq, _, _ = O.adamw_update_lowp(O.widen(case["master"]), m_bits, v_bits, np.zeros((V, d)), 9, c["lr"], b1,
+                                              b2, c["eps"], c["weight_decay"], idx=idx, seed=12345)
+        np.testing.assert_array_equal(bits(m), mq)
+        np.testing.assert_array_equal(bits(v), vq)
+        assert (bits(v) != v_bits).mean() > 0.05          # the decay is visible: codes moved, none frozen en bloc
+    finally:
+        tts.tts_ctx_destroy(ctx)
+
+
+def test_bf16_moments_300_round_drift_against_fp32_moments():
+    """The same 300-round stream (config 5 scaled down) with fp32 and with bf16 moments on the GPU: the head moves the
+    same way (the quantisation noise of v is unbiased and enters the step through sqrt(v): ~0.2% of lr per step)."""
+    from paper_2605_09329_b200.scheduler import DraftHeadUpdater
+    V, d, rounds_n = 4096, 1024, 300
+    case0, rounds = synth.make_stream(V=V, d=d, rounds=rounds_n)
+    c = case0["cfg"]
+    finals, losses = {}, {}
+    for mom in ("f32", "bf16"):
+        W0, master = _dev(case0["W"]), _dev(case0["master"])
+        if mom == "bf16":
+            m = torch.zeros(V, d, dtype=torch.bfloat16, device="cuda")
+            v = torch.zeros(V, d, dtype=torch.bfloat16, device="cuda")
+        else:
+            m, v = _dev(case0["m"]), _dev(case0["v"])
+        up = DraftHeadUpdater(W0, master, m, v, seg_len=16, T_max=16, stride=1, lr=c["lr"], beta1=c["beta1"],
+                              beta2=c["beta2"], eps=c["eps"], weight_decay=c["weight_decay"],
+                              moment_dtype=tts.TTS_MOMENT_BF16 if mom == "bf16" else tts.TTS_MOMENT_F32)
+        pw = _dev(case0["pos_weight"])
+        ls = []
+        try:
+            for r in rounds:
+                rd = (_dev(r["teacher"]), _dev(r["h"]), _dev(r["draft_tokens"]))
+                up.on_round_end(rd[0], rd[1], rd[2], pw, 16)
+                tts.tts_sync_step(up.ctx)
+                ls.append(float(up.loss.item()))
+            torch.cuda.synchronize()
+            finals[mom] = master.cpu().numpy().astype(np.float64)
+            losses[mom] = np.array(ls)
+            if mom == "bf16":
+                assert bool(torch.isfinite(v.float()).all()) and bool((v.float() >= 0).all())
+        finally:
+            up.close()
+    M0 = case0["master"].astype(np.float64)
+    d32, d16 = finals["f32"] - M0, finals["bf16"] - M0
+    rel = np.abs(d16 - d32).mean() / np.abs(d32).mean()
+    print("mean |dM_bf16 - dM_f32| / mean |dM_f32| after %d rounds: %.4f; max |.| / lr %.2f" % (
+        rounds_n, rel, np.abs(d16 - d32).max() / c["lr"]))
+    assert rel <= 0.05
+    assert np.all(np.abs(losses["bf16"] - losses["f32"]) <= 2e-3 * np.abs(losses["f32"]) + 1e-6)
