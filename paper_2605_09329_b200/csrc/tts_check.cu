@@ -42,15 +42,15 @@ __global__ void __launch_bounds__(256) check_finite_kernel(const T* __restrict__
 // tensor-path kernels), so the "epilogue" never reports and the watchdog warp must trap.
 __global__ void __launch_bounds__(96) stalled_pipeline_kernel() {
   __shared__ uint64_t bar;
-  __shared__ uint32_t done_ctr;
+  __shared__ uint64_t done;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  if (threadIdx.x == 0) { ptx::mbar_init(&bar, 1); done_ctr = 0; ptx::fence_barrier_init(); }
+  if (threadIdx.x == 0) { ptx::mbar_init(&bar, 1); ptx::mbar_init(&done, 1); ptx::fence_barrier_init(); }
   __syncthreads();
   if (warp == 1) {
     ptx::mbar_wait(&bar, 0);
-    if (lane == 0) ptx::watchdog_arrive(&done_ctr);
+    if (lane == 0) ptx::watchdog_arrive(&done);
   } else if (warp == 2) {
-    ptx::watchdog_wait(&done_ctr, 1);
+    ptx::watchdog_wait(&done);
   }
   __syncthreads();
 }

@@ -146,8 +146,8 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
   uint64_t* wt_empty = wt_full + 1;            // [1]
   uint64_t* gh_full = wt_empty + 1;            // [1]
   uint64_t* gh_empty = gh_full + 1;            // [1]
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(gh_empty + 1);
-  uint32_t* done_ctr = tmem_slot + 1;          // epilogue warps finished (watchdog)
+  uint64_t* done_bar = gh_empty + 1;           // [1] epilogue warps finished (watchdog)
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(done_bar + 1);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const bool do_gh = p.gh != nullptr;
@@ -167,7 +167,7 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
     ptx::mbar_init(wt_empty, 1);
     ptx::mbar_init(gh_full, 1);
     ptx::mbar_init(gh_empty, 4);
-    *done_ctr = 0;
+    ptx::mbar_init(done_bar, 8);
     ptx::fence_barrier_init();
   }
   if (warp == 2) {
@@ -441,9 +441,9 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
     }
     }   // segments
     if (leader) ptx::bulk_wait_group_read<0>();   // shared memory must outlive the last stores' reads
-    if (lane == 0) ptx::watchdog_arrive(done_ctr);
+    if (lane == 0) ptx::watchdog_arrive(done_bar);
   } else if (warp == 2) {
-    ptx::watchdog_wait(done_ctr, 8);
+    ptx::watchdog_wait(done_bar);
   }
   ptx::tc_fence_before();
   __syncthreads();

@@ -42,8 +42,8 @@ struct Bars {
   uint64_t acc_full[2];
   uint64_t acc_empty[2];
   uint64_t conv[kMaxStages];   // gh: the stage's W tile is fp16 now
+  uint64_t done;               // epilogue warps finished (watchdog)
   uint32_t tmem_slot;
-  uint32_t done_ctr;           // epilogue warps finished (watchdog)
 };
 
 // ------------------------------------------------------------------ a2: draft logits
@@ -117,7 +117,7 @@ tc_logits_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant
   if (warp == 1 && lane == 0) {
     for (int i = 0; i < p.stages; ++i) { ptx::mbar_init(&bars->full[i], 1); ptx::mbar_init(&bars->empty[i], 1); }
     for (int i = 0; i < 2; ++i) { ptx::mbar_init(&bars->acc_full[i], 1); ptx::mbar_init(&bars->acc_empty[i], 4); }
-    bars->done_ctr = 0;
+    ptx::mbar_init(&bars->done, 4);
     ptx::fence_barrier_init();
   }
   if (warp == 2) {
@@ -205,23 +205,30 @@ tc_logits_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant
         ptx::tmem_ld_32x32b_x16(tmem_base + ab * p.T16 + c0 + (static_cast<uint32_t>(q * 32) << 16), r);
         ptx::tmem_ld_wait();
         // rows T .. T16 exist only as MMA padding: a caller's draft_logits_out has exactly T rows
-        if (partial) {
+        if (c0 + 16 <= p.T) {
+          if (partial) {
 #pragma unroll
-          for (int i = 0; i < 16; ++i)
-            if (c0 + i < p.T) atomicAdd(zc + (size_t)(c0 + i) * p.z_ld, __uint_as_float(r[i]));
+            for (int i = 0; i < 16; ++i) atomicAdd(zc + (size_t)(c0 + i) * p.z_ld, __uint_as_float(r[i]));
+          } else {
+#pragma unroll
+            for (int i = 0; i < 16; ++i) zc[(size_t)(c0 + i) * p.z_ld] = __uint_as_float(r[i]);
+          }
         } else {
 #pragma unroll
           for (int i = 0; i < 16; ++i)
-            if (c0 + i < p.T) zc[(size_t)(c0 + i) * p.z_ld] = __uint_as_float(r[i]);
+            if (c0 + i < p.T) {
+              if (partial) atomicAdd(zc + (size_t)(c0 + i) * p.z_ld, __uint_as_float(r[i]));
+              else zc[(size_t)(c0 + i) * p.z_ld] = __uint_as_float(r[i]);
+            }
         }
       }
       ptx::tc_fence_before();
       __syncwarp();
       if (lane == 0) ptx::mbar_arrive(&bars->acc_empty[ab]);
     }
-    if (lane == 0) ptx::watchdog_arrive(&bars->done_ctr);
+    if (lane == 0) ptx::watchdog_arrive(&bars->done);
   } else if (warp == 2) {
-    ptx::watchdog_wait(&bars->done_ctr, 4);
+    ptx::watchdog_wait(&bars->done);
   }
   ptx::tc_fence_before();
   __syncthreads();
@@ -285,7 +292,7 @@ tc_gh_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant__ C
       ptx::mbar_init(&bars->full[i], 1); ptx::mbar_init(&bars->empty[i], MC ? 2 : 1); ptx::mbar_init(&bars->conv[i], 128);
     }
     for (int i = 0; i < 2; ++i) { ptx::mbar_init(&bars->acc_full[i], 1); ptx::mbar_init(&bars->acc_empty[i], 4); }
-    bars->done_ctr = 0;
+    ptx::mbar_init(&bars->done, 4);
     ptx::fence_barrier_init();
   }
   if (warp == 2) {
@@ -418,9 +425,9 @@ tc_gh_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant__ C
       __syncwarp();
       if (lane == 0) ptx::mbar_arrive(&bars->acc_empty[ab]);
     }
-    if (lane == 0) ptx::watchdog_arrive(&bars->done_ctr);
+    if (lane == 0) ptx::watchdog_arrive(&bars->done);
   } else if (warp == 2) {
-    ptx::watchdog_wait(&bars->done_ctr, 4);
+    ptx::watchdog_wait(&bars->done);
   }
   ptx::tc_fence_before();
   if (MC) ptx::cluster_sync(); else __syncthreads();

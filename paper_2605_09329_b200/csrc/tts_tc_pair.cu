@@ -42,8 +42,8 @@ struct PairBars {
   uint64_t empty[kPMaxStages];
   uint64_t acc_full;
   uint64_t acc_empty;
+  uint64_t done;       // epilogue warps finished (watchdog)
   uint32_t tmem_slot;
-  uint32_t done_ctr;   // epilogue warps finished (watchdog)
 };
 
 struct PairLogitsParams {
@@ -120,7 +120,7 @@ tc_logits_pair_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_con
     for (int i = 0; i < p.stages; ++i) { ptx::mbar_init(&bars->full[i], 1); ptx::mbar_init(&bars->empty[i], 1); }
     ptx::mbar_init(&bars->acc_full, 1);
     ptx::mbar_init(&bars->acc_empty, 8);
-    bars->done_ctr = 0;
+    ptx::mbar_init(&bars->done, 4);
     ptx::fence_barrier_init();
   }
   if (warp == 2) {
@@ -216,9 +216,9 @@ tc_logits_pair_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_con
       __syncwarp();
       if (lane == 0) ptx::mbar_arrive_cta0(&bars->acc_empty);
     }
-    if (lane == 0) ptx::watchdog_arrive(&bars->done_ctr);
+    if (lane == 0) ptx::watchdog_arrive(&bars->done);
   } else if (warp == 2) {
-    ptx::watchdog_wait(&bars->done_ctr, 4);
+    ptx::watchdog_wait(&bars->done);
   }
   ptx::tc_fence_before();
   ptx::cluster_sync();

@@ -74,8 +74,8 @@ struct WideBars {
   uint64_t acc_empty[2];
   uint64_t a_full;
   uint64_t wt_full, wt_empty, gh_full, gh_empty;   // GH
+  uint64_t done;       // epilogue warps finished (watchdog)
   uint32_t tmem_slot;
-  uint32_t done_ctr;   // epilogue warps finished (watchdog)
 };
 
 // The sequence of (stripe, band) units of this CTA: window by window, a contiguous range of each window's units --
@@ -162,7 +162,7 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
     ptx::mbar_init(&bars->wt_empty, 1);
     ptx::mbar_init(&bars->gh_full, 1);
     ptx::mbar_init(&bars->gh_empty, 4);
-    bars->done_ctr = 0;
+    ptx::mbar_init(&bars->done, 8);
     ptx::fence_barrier_init();
   }
   if (warp == 2) {
@@ -475,9 +475,9 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
     }
     if (GH && cur >= 0) flush_gh(cur);
     if (leader) ptx::bulk_wait_group_read<0>();   // shared memory must outlive the last stores' reads
-    if (lane == 0) ptx::watchdog_arrive(&bars->done_ctr);
+    if (lane == 0) ptx::watchdog_arrive(&bars->done);
   } else if (warp == 2) {
-    ptx::watchdog_wait(&bars->done_ctr, 8);
+    ptx::watchdog_wait(&bars->done);
   }
   ptx::tc_fence_before();
   __syncthreads();
