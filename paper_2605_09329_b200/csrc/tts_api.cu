@@ -31,6 +31,7 @@ void free_all(tts_ctx* c) {
   cudaFree(c->step_count_dev); cudaFree(c->step_scalars); cudaFree(c->dev_status);
   if (c->host_slot) cudaFreeHost(c->host_slot);
   cudaFree(c->z); cudaFree(c->z_ref_buf); cudaFree(c->dl32); cudaFree(c->stat_part); cudaFree(c->row_stats);
+  cudaFree(c->row_loss); cudaFree(c->merge_ticket);
   cudaFree(c->arg_val); cudaFree(c->arg_idx); cudaFree(c->argmax_tmp);
   cudaFree(c->acc_rows); cudaFree(c->acc_rej); cudaFree(c->acc_rpart);
   cudaFree(c->st_teacher); cudaFree(c->st_h); cudaFree(c->st_tok); cudaFree(c->st_pw);
@@ -108,8 +109,11 @@ int32_t tts_ctx_create(const tts_config* cfg, int32_t device, tts_ctx** out) {
   // K > 1 inner steps keep step 1's logits as z_ref: reserved here so that no step call allocates
   if (cfg->max_inner_steps > 1) ok = ok && dmalloc(&c->z_ref_buf, Tp * V) == cudaSuccess;
   if (!c->tensor_ok) ok = ok && dmalloc(&c->dl32, Tm * V) == cudaSuccess;   // fp32 dlogits: CUDA-core kernels only
-  ok = ok && dmalloc(&c->stat_part, Tm * tts::kStatSplitsMax * tts::kStatFields) == cudaSuccess;
+  ok = ok && dmalloc(&c->stat_part, Tm * tts::kStatTuplesMax * tts::kStatFields) == cudaSuccess;
   ok = ok && dmalloc(&c->row_stats, tts::kRowStatFields * Tm) == cudaSuccess;
+  ok = ok && dmalloc(&c->row_loss, Tm) == cudaSuccess;
+  ok = ok && dmalloc(&c->merge_ticket, 1) == cudaSuccess;
+  ok = ok && cudaMemset(c->merge_ticket, 0, sizeof(unsigned int)) == cudaSuccess;
   ok = ok && dmalloc(&c->arg_val, Tm * tts::kArgSplitsMax) == cudaSuccess;
   ok = ok && dmalloc(&c->arg_idx, Tm * tts::kArgSplitsMax) == cudaSuccess;
   ok = ok && dmalloc(&c->argmax_tmp, Tm) == cudaSuccess;

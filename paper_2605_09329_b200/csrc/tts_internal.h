@@ -11,6 +11,8 @@
 namespace tts {
 
 constexpr int kStatSplitsMax = 64;   // V-splits per row in the row-statistics sweep
+constexpr int kStatFixMax = 160;     // tiles whose statistics come from the fix-up sweep (cut by a stream-K walk)
+constexpr int kStatTuplesMax = 320;  // tuples per canvas row in stat_part: one per CTA of a logits kernel + the fix-ups
 constexpr int kArgSplitsMax = 64;    // V-splits per row in the argmax sweep
 constexpr int kStatFields = 8;       // (m_t, s_t, a, m_z, s_z) of SURVEY §8(a) a3 + (m_ref, s_ref, b) of the lambda term
 constexpr int kRowStatFields = 5;    // row_stats planes: lse_t, lse_z, kl, coef, lse_ref
@@ -85,6 +87,8 @@ struct tts_ctx {
   float* dl32;            // [T_max, V] fp32 dlogits                (CUDA-core path)
   float* stat_part;       // [T_max, kStatSplitsMax, 5]
   float* row_stats;       // [kRowStatFields, T_max]: lse_t, lse_z, kl, coef (= loss_scale * omega), lse_ref
+  double* row_loss;       // [T_max] omega_r (KL_r + lambda KL_ref,r): summed in a fixed order by the merge kernel's last CTA
+  unsigned int* merge_ticket;
   float* z_ref_buf;       // [T_pad_max, V] fp32, allocated by the first tts_distill_inner_steps call
   float* arg_val;         // [T_max, kArgSplitsMax]
   int32_t* arg_idx;       // [T_max, kArgSplitsMax]
@@ -144,6 +148,13 @@ cudaError_t launch_row_stats_shard(tts_ctx* c, const StepArgs& a, const float* z
                                    cudaStream_t s, int* launches);
 cudaError_t launch_row_stats_merge_shards(tts_ctx* c, const StepArgs& a, const float* stats_all, int n_shards,
                                           cudaStream_t s, int* launches);
+// a3 fused into a2 (tts_tc_epi.cuh): the logits kernel left `splits` tuples per row in c->stat_part.
+//   tiles:  the fix-up sweep over n 128-column tiles whose z was completed by fp32 RED (tuples slot0 .. slot0 + n - 1)
+//   finish: merge -> normalisers, KL, omega, loss (whole step) or -> one tuple per row in stats_out (shard, phase 1)
+cudaError_t launch_row_stats_tiles(tts_ctx* c, const StepArgs& a, const float* z, int z_ld, const int* col0, int n,
+                                   int slot0, int splits, cudaStream_t s, int* launches);
+cudaError_t launch_row_stats_finish(tts_ctx* c, const StepArgs& a, int splits, float* shard_stats_out, cudaStream_t s,
+                                    int* launches);
 // a2 + a3 of either path for the phase of `a`: returns after phase 1, or leaves the row normalisers in c->row_stats
 enum { kPhaseAll = 0, kPhaseBegin = 1, kPhaseFinish = 2 };
 // tts_simt.cu

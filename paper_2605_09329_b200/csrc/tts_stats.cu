@@ -177,39 +177,27 @@ __global__ void __launch_bounds__(256) row_stats_partial_kernel(const void* __re
   }
 }
 
-// One CTA of 32 warps; a warp merges one row at a time with its lanes spread over the V-splits.
+// A warp merges one row with its lanes spread over the row's tuples (8 rows per CTA); with few tuples and many rows
+// (several canvases from the unfused sweep; vocabulary shards) a THREAD merges one row (256 rows per CTA).
 // row_stats planes ([kRowStatFields][T_max]): 0 = lse_t, 1 = lse_z, 2 = kl, 3 = coef (= loss_scale * omega), 4 = lse_ref.
 // The maxima are exact in fp32; the rescaled sums and the final a / s_t - lse_t + lse_z (a difference of numbers
 // ~10 for a result that can be ~0.01) are formed in double.  With z_ref (has_ref) the loss gains
 // lambda * sum_r omega_r K~L(q_ref || q)_r.
-__global__ void __launch_bounds__(1024) row_stats_merge_kernel(const float* __restrict__ part, int splits,
-                                                               long row_stride, long split_stride, int T,
-                                                               int T_max, int seg_len, int mask_mode,
-                                                               const float* __restrict__ pos_weight,
-                                                               const uint8_t* __restrict__ mask, float loss_scale,
-                                                               int has_ref, float lambda,
-                                                               float* __restrict__ row_stats,
-                                                               float* __restrict__ kl_rows_out,
-                                                               float* __restrict__ loss_out,
-                                                               unsigned long long* __restrict__ step_count,
-                                                               float* __restrict__ step_scalars, float b1, float b2,
-                                                               int* __restrict__ dev_status) {
-  __shared__ double red[32];
-  if (threadIdx.x == 0) {
-    // Adam's count and bias corrections live on the device (a replayed CUDA graph of the step keeps counting):
-    // n <- n + 1, {1 / (1 - b1^n), 1 / sqrt(1 - b2^n)} in double, read by the update kernel later in the stream
-    const unsigned long long n = *step_count + 1ull;
-    *step_count = n;
-    step_scalars[0] = (float)(1.0 / (1.0 - pow((double)b1, (double)n)));
-    step_scalars[1] = (float)(1.0 / sqrt(1.0 - pow((double)b2, (double)n)));
-  }
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
-  double local = 0.0;
-  // many rows, few splits (several canvases; vocabulary shards): a THREAD per row, otherwise a warp per row
-  const bool thread_rows = splits <= 8 && T > n_warps;
-  const int r_first = thread_rows ? (int)threadIdx.x : warp, r_step = thread_rows ? (int)blockDim.x : n_warps;
+// The loss is a sum over rows in a FIXED order: every CTA leaves omega_r (KL_r + lambda KL_ref,r) per row, and the CTA
+// that finishes last (a ticket) adds them up, advances Adam's count and resets the ticket for the next launch.
+constexpr int kMergeThreads = 256;
+__global__ void __launch_bounds__(kMergeThreads) row_stats_merge_kernel(
+    const float* __restrict__ part, int splits, long row_stride, long split_stride, int T, int T_max, int seg_len,
+    int mask_mode, const float* __restrict__ pos_weight, const uint8_t* __restrict__ mask, float loss_scale, int has_ref,
+    float lambda, float* __restrict__ row_stats, float* __restrict__ kl_rows_out, float* __restrict__ loss_out,
+    unsigned long long* __restrict__ step_count, float* __restrict__ step_scalars, float b1, float b2,
+    int* __restrict__ dev_status, double* __restrict__ row_loss, unsigned int* __restrict__ ticket, int thread_rows) {
+  __shared__ double red[kMergeThreads / 32];
+  __shared__ int is_last;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = kMergeThreads >> 5;
+  const int r = thread_rows ? blockIdx.x * kMergeThreads + (int)threadIdx.x : blockIdx.x * n_warps + warp;
   const int l_first = thread_rows ? 0 : lane, l_step = thread_rows ? 1 : 32;
-  for (int r = r_first; r < T; r += r_step) {
+  if (r < T) {
     const float* pr = part + (size_t)r * row_stride;
     float mt = -CUDART_INF_F, mz = -CUDART_INF_F, mr = -CUDART_INF_F;
     for (int s = l_first; s < splits; s += l_step) {
@@ -220,13 +208,14 @@ __global__ void __launch_bounds__(1024) row_stats_merge_kernel(const float* __re
     double st = 0.0, a = 0.0, sz = 0.0, sr = 0.0, b = 0.0;
     for (int s = l_first; s < splits; s += l_step) {
       const float* p = pr + s * split_stride;
+      // rescale factors in fp32 (expf, ~1 ulp: 6e-8 relative per term, against a loss tolerance of 1e-3), sums in double
       if (p[0] != -CUDART_INF_F) {
-        const double e = exp((double)p[0] - (double)mt);
+        const double e = (double)expf(p[0] - mt);
         st += (double)p[1] * e; a += (double)p[2] * e;
       }
-      if (p[3] != -CUDART_INF_F) sz += (double)p[4] * exp((double)p[3] - (double)mz);
+      if (p[3] != -CUDART_INF_F) sz += (double)p[4] * (double)expf(p[3] - mz);
       if (has_ref && p[5] != -CUDART_INF_F) {
-        const double e = exp((double)p[5] - (double)mr);
+        const double e = (double)expf(p[5] - mr);
         sr += (double)p[6] * e; b += (double)p[7] * e;
       }
     }
@@ -258,10 +247,18 @@ __global__ void __launch_bounds__(1024) row_stats_merge_kernel(const float* __re
       row_stats[3 * T_max + r] = (float)((double)loss_scale * omega);
       row_stats[4 * T_max + r] = (float)lse_ref;
       if (kl_rows_out) kl_rows_out[r] = (float)kl;
-      local += omega * (kl + (double)lambda * kl_ref);
+      row_loss[r] = omega * (kl + (double)lambda * kl_ref);
     }
   }
-  if (thread_rows) local = warp_sum(local);   // fixed shuffle tree: deterministic
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x == 0) is_last = atomicAdd(ticket, 1u) == gridDim.x - 1;
+  __syncthreads();
+  if (!is_last) return;
+  __threadfence();
+  double local = 0.0;
+  for (int q = threadIdx.x; q < T; q += kMergeThreads) local += __ldcg(row_loss + q);   // fixed order per thread
+  local = warp_sum(local);                                                              // fixed shuffle tree
   if (lane == 0) red[warp] = local;
   __syncthreads();
   if (threadIdx.x == 0) {
@@ -270,6 +267,13 @@ __global__ void __launch_bounds__(1024) row_stats_merge_kernel(const float* __re
     const float loss = (float)((double)loss_scale * sum);
     loss_out[0] = loss;
     if (!isfinite(loss)) atomicOr(dev_status, TTS_DEV_NONFINITE_LOSS);
+    // Adam's count and bias corrections live on the device (a replayed CUDA graph of the step keeps counting):
+    // n <- n + 1, {1 / (1 - b1^n), 1 / sqrt(1 - b2^n)} in double, read by the update kernel later in the stream
+    const unsigned long long n = *step_count + 1ull;
+    *step_count = n;
+    step_scalars[0] = (float)(1.0 / (1.0 - pow((double)b1, (double)n)));
+    step_scalars[1] = (float)(1.0 / sqrt(1.0 - pow((double)b2, (double)n)));
+    *ticket = 0u;
   }
 }
 
@@ -309,6 +313,32 @@ __global__ void __launch_bounds__(1024) row_stats_reduce_kernel(const float* __r
   }
 }
 
+// Fix-up sweep of the fused a2 + a3 path: block (k, r) takes the 128 columns [col0[k], col0[k] + 128) of canvas row r
+// (tiles whose z was completed by fp32 RED from two CTAs, so that neither epilogue saw whole logits) and writes the
+// row's tuple slot0 + k.  One element per thread, shuffle merge.
+struct FixTiles { int col0[kStatFixMax]; };
+template <bool BF16>
+__global__ void __launch_bounds__(128) row_stats_tiles_kernel(const void* __restrict__ teacher,
+                                                              const float* __restrict__ z, int V, int z_ld,
+                                                              const FixTiles tiles, int slot0, int splits,
+                                                              float* __restrict__ part) {
+  const int r = blockIdx.y, v = tiles.col0[blockIdx.x] + threadIdx.x;
+  RowStat s;
+  stat_init(s);
+  const float t = BF16 ? __bfloat162float(static_cast<const __nv_bfloat16*>(teacher)[(size_t)r * V + v])
+                       : static_cast<const float*>(teacher)[(size_t)r * V + v];
+  stat_push(s, t, z[(size_t)r * z_ld + v]);
+  __shared__ RowStat sh[4];
+  s = warp_stat(s);
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = s;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    RowStat q = stat_merge(stat_merge(sh[0], sh[1]), stat_merge(sh[2], sh[3]));
+    float* o = part + ((size_t)r * splits + slot0 + blockIdx.x) * kStatFields;
+    o[0] = q.mt; o[1] = q.st; o[2] = q.a; o[3] = q.mz; o[4] = q.sz; o[5] = -CUDART_INF_F; o[6] = 0.f; o[7] = 0.f;
+  }
+}
+
 static int launch_partial(tts_ctx* c, const StepArgs& a, const float* z, int z_ld, cudaStream_t s) {
   const int V = c->cfg.V, T = a.T;
   int splits = (2 * c->sm_count + T - 1) / T;
@@ -327,12 +357,12 @@ static int launch_partial(tts_ctx* c, const StepArgs& a, const float* z, int z_l
 static void launch_merge(tts_ctx* c, const StepArgs& a, const float* part, int splits, long row_stride,
                          long split_stride, cudaStream_t s) {
   const int T = a.T;
-  row_stats_merge_kernel<<<1, T >= 32 ? 1024 : 32 * T, 0, s>>>(part, splits, row_stride, split_stride, T, c->cfg.T_max,
-                                                              c->cfg.seg_len, c->cfg.mask_mode, a.pos_weight, a.mask,
-                                                              a.loss_scale, a.z_ref != nullptr, a.lambda, c->row_stats,
-                                                              a.kl_rows_out, a.loss_out, c->step_count_dev,
-                                                              c->step_scalars, c->cfg.beta1, c->cfg.beta2,
-                                                              c->dev_status);
+  const int thread_rows = splits <= 8 && T > kMergeThreads / 32;
+  const int rows_per_cta = thread_rows ? kMergeThreads : kMergeThreads / 32;
+  row_stats_merge_kernel<<<(T + rows_per_cta - 1) / rows_per_cta, kMergeThreads, 0, s>>>(
+      part, splits, row_stride, split_stride, T, c->cfg.T_max, c->cfg.seg_len, c->cfg.mask_mode, a.pos_weight, a.mask,
+      a.loss_scale, a.z_ref != nullptr, a.lambda, c->row_stats, a.kl_rows_out, a.loss_out, c->step_count_dev,
+      c->step_scalars, c->cfg.beta1, c->cfg.beta2, c->dev_status, c->row_loss, c->merge_ticket, thread_rows);
 }
 
 cudaError_t launch_row_stats(tts_ctx* c, const StepArgs& a, const float* z, int z_ld, cudaStream_t s, int* launches) {
@@ -348,6 +378,29 @@ cudaError_t launch_row_stats_shard(tts_ctx* c, const StepArgs& a, const float* z
   const int splits = launch_partial(c, a, z, z_ld, s);
   row_stats_reduce_kernel<<<1, a.T >= 32 ? 1024 : 32 * a.T, 0, s>>>(c->stat_part, splits, a.T, stats_out);
   *launches += 2;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_row_stats_tiles(tts_ctx* c, const StepArgs& a, const float* z, int z_ld, const int* col0, int n,
+                                   int slot0, int splits, cudaStream_t s, int* launches) {
+  FixTiles ft;
+  for (int i = 0; i < n; ++i) ft.col0[i] = col0[i];
+  const dim3 grid(n, a.T);
+  if (c->cfg.logits_dtype == TTS_BF16)
+    row_stats_tiles_kernel<true><<<grid, 128, 0, s>>>(a.teacher, z, c->cfg.V, z_ld, ft, slot0, splits, c->stat_part);
+  else
+    row_stats_tiles_kernel<false><<<grid, 128, 0, s>>>(a.teacher, z, c->cfg.V, z_ld, ft, slot0, splits, c->stat_part);
+  *launches += 1;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_row_stats_finish(tts_ctx* c, const StepArgs& a, int splits, float* shard_stats_out, cudaStream_t s,
+                                    int* launches) {
+  if (shard_stats_out)
+    row_stats_reduce_kernel<<<1, a.T >= 32 ? 1024 : 32 * a.T, 0, s>>>(c->stat_part, splits, a.T, shard_stats_out);
+  else
+    launch_merge(c, a, c->stat_part, splits, (long)splits * kStatFields, kStatFields, s);
+  *launches += 1;
   return cudaGetLastError();
 }
 

@@ -69,14 +69,23 @@ cudaError_t tc_step(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches
   // a2: draft logits on tcgen05 (skipped when the caller supplies them), a3: row statistics + loss
   const float* z = z_src(a, c->z);
   if (a.phase != kPhaseFinish) {
+    // a3 rides in a2's epilogue (north_star (1): one TMA-staged sweep, no second pass over [T, V]) unless the lambda
+    // term needs the reference distribution's statistics too (K > 1 inner steps) or the caller supplies z
+    int n_tuples = 0;
     if (!a.z_given) {
-      e = tc_pair_eligible(c, T16) ? tc_launch_logits_pair(c, a, z_dst(a, c->z), s, launches)
-                                   : tc_launch_logits(c, a, z_dst(a, c->z), s, launches);
+      const bool fuse = a.z_ref == nullptr;
+      e = tc_pair_eligible(c, T16) ? tc_launch_logits_pair(c, a, z_dst(a, c->z), fuse, s, launches, &n_tuples)
+                                   : tc_launch_logits(c, a, z_dst(a, c->z), fuse, s, launches, &n_tuples);
       if (e != cudaSuccess) return e;
     }
     prof_mark(c, 0, s);
-    if (a.phase == kPhaseBegin) return launch_row_stats_shard(c, a, z, V, a.shard_stats_out, s, launches);
-    if ((e = launch_row_stats(c, a, z, V, s, launches)) != cudaSuccess) return e;
+    if (n_tuples > 0) {
+      if (a.phase == kPhaseBegin) return launch_row_stats_finish(c, a, n_tuples, a.shard_stats_out, s, launches);
+      if ((e = launch_row_stats_finish(c, a, n_tuples, nullptr, s, launches)) != cudaSuccess) return e;
+    } else {
+      if (a.phase == kPhaseBegin) return launch_row_stats_shard(c, a, z, V, a.shard_stats_out, s, launches);
+      if ((e = launch_row_stats(c, a, z, V, s, launches)) != cudaSuccess) return e;
+    }
   } else {
     prof_mark(c, 0, s);
     if ((e = launch_row_stats_merge_shards(c, a, a.shard_stats_all, a.n_shards, s, launches)) != cudaSuccess) return e;

@@ -16,6 +16,7 @@
 #include <string.h>
 
 #include "tts_common.cuh"
+#include "tts_tc_epi.cuh"
 #include "tts_tc_ptx.cuh"
 #include "tts_tc_state.h"
 
@@ -28,6 +29,7 @@ constexpr float kGhWScale = 16.f;   // bf16 -> fp16 scale of W: exact for 2^-18 
 constexpr int kATile = kTileMN * kKC * 2;   // 16 KB: [128 x 64] bf16 (K-major) or 2 x [64 k x 64 mn] (MN-major)
 constexpr int kMaxStages = 8;
 constexpr int kSmemBudget = 200 * 1024;
+constexpr int kSmemLimit = 232448;  // 227 KB: the most dynamic shared memory a CTA can have on sm_100
 constexpr int kNMax = 256;          // largest MMA N
 
 __host__ __device__ inline int pow2_cols(int n) {
@@ -99,20 +101,23 @@ __device__ __forceinline__ uint64_t desc64(uint32_t hi, uint32_t lo) { return (s
 // WIDE = false: T16 <= 256, one MMA per 16-element K step.  The single issuing thread is the pipeline's narrowest
 // point at T = 16 (a [128 x 16 x 16] MMA finishes in a few cycles): with descriptors rebuilt per instruction the
 // kernel ran at 3.7 TB/s, MMA-issue-bound; the loop below is 2 integer adds per MMA.
-template <bool WIDE>
+// TB: the teacher is bf16 (its tiles are staged by TMA for the fused a3 statistics; fp32 teachers use vector loads)
+template <bool WIDE, bool TB>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 tc_logits_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant__ CUtensorMap tm_h,
-                 const LogitsParams p) {
+                 const __grid_constant__ CUtensorMap tm_teacher, const LogitsParams p, const epi::Params ep) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const int b_bytes = p.n_boxes * p.box_rows * kKC * 2;
   const int stage_bytes = kATile + b_bytes;
   Bars* bars = reinterpret_cast<Bars*>(smem + p.stages * stage_bytes);
+  uint8_t* epi_base = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(bars + 1) + 127) & ~uintptr_t(127));
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
   if (warp == 0 && lane == 0) {
     ptx::prefetch_tensormap(&tm_W);
     ptx::prefetch_tensormap(&tm_h);
+    if (TB && ep.enabled) ptx::prefetch_tensormap(&tm_teacher);
   }
   if (warp == 1 && lane == 0) {
     for (int i = 0; i < p.stages; ++i) { ptx::mbar_init(&bars->full[i], 1); ptx::mbar_init(&bars->empty[i], 1); }
@@ -189,9 +194,14 @@ tc_logits_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant
       __syncwarp();
     }
   } else if (warp >= 4) {
-    // ===== epilogue: thread = one vocabulary row (TMEM lane); a warp's access to one canvas row is 128 contiguous bytes =====
+    // ===== epilogue: thread = one vocabulary row (TMEM lane); a warp's access to one canvas row is 128 contiguous bytes.
+    // Whole tiles also feed the fused a3 statistics (tts_tc_epi.cuh); a tile cut by a stream-K range boundary is only
+    // accumulated into z here (its statistics come from the small fix-up sweep of tts_stats.cu) =====
     const int q = warp & 3;
-    uint32_t it = 0;
+    const int tid_e = threadIdx.x - 128;
+    const epi::Shared esh(epi_base, p.T16);
+    if (ep.enabled) epi::init(esh, p.T16, tid_e);
+    uint32_t it = 0, g = 0;
     int vt, c_beg, c_end;
     for (LogitsWalk w(p); !w.done(); w.next(p, c_beg, c_end), ++it) {
       w.piece(vt, c_beg, c_end);
@@ -199,10 +209,20 @@ tc_logits_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant
       const int ab = it % p.n_acc;
       ptx::mbar_wait(&bars->acc_full[ab], (it / p.n_acc) & 1);
       ptx::tc_fence_after();
+      const uint32_t tmem_tile = tmem_base + ab * p.T16 + (static_cast<uint32_t>(q * 32) << 16);
+      auto release = [&]() {
+        ptx::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(&bars->acc_empty[ab]);
+      };
+      if (ep.enabled && !partial) {
+        epi::tile<TB>(ep, esh, &tm_teacher, tmem_tile, vt * kTileMN, p.T16, p.z, p.z_ld, tid_e, g, release);
+        continue;
+      }
       float* zc = p.z + vt * kTileMN + q * 32 + lane;
       for (int c0 = 0; c0 < p.T16; c0 += 16) {
         uint32_t r[16];
-        ptx::tmem_ld_32x32b_x16(tmem_base + ab * p.T16 + c0 + (static_cast<uint32_t>(q * 32) << 16), r);
+        ptx::tmem_ld_32x32b_x16(tmem_tile + c0, r);
         ptx::tmem_ld_wait();
         // rows T .. T16 exist only as MMA padding: a caller's draft_logits_out has exactly T rows
         if (c0 + 16 <= p.T) {
@@ -222,10 +242,9 @@ tc_logits_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant
             }
         }
       }
-      ptx::tc_fence_before();
-      __syncwarp();
-      if (lane == 0) ptx::mbar_arrive(&bars->acc_empty[ab]);
+      release();
     }
+    if (ep.enabled) epi::flush(ep, esh, blockIdx.x, tid_e);
     if (lane == 0) ptx::watchdog_arrive(&bars->done);
   } else if (warp == 2) {
     ptx::watchdog_wait(&bars->done);
@@ -478,8 +497,8 @@ GhPlan gh_plan(const tts_ctx* c, int T16) {
   return g;
 }
 
-int pick_stages(int stage_bytes) {
-  int s = (kSmemBudget - (int)sizeof(Bars) - 1024) / stage_bytes;
+int pick_stages(int stage_bytes, int extra = 0) {
+  int s = ((extra ? kSmemLimit : kSmemBudget) - (int)sizeof(Bars) - 1024 - extra) / stage_bytes;
   return s < 1 ? 1 : (s > kMaxStages ? kMaxStages : s);
 }
 
@@ -487,33 +506,36 @@ int pick_stages(int stage_bytes) {
 
 cudaError_t tc_gemm_init(tts_ctx*) {
   cudaError_t e;
+  const auto attr = cudaFuncAttributeMaxDynamicSharedMemorySize;
+  if ((e = cudaFuncSetAttribute(tc_logits_kernel<false, true>, attr, kSmemLimit)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(tc_logits_kernel<false, false>, attr, kSmemLimit)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(tc_logits_kernel<true, true>, attr, kSmemLimit)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(tc_logits_kernel<true, false>, attr, kSmemLimit)) != cudaSuccess) return e;
   const int smem_max = kSmemBudget + 16 * 1024;
-  if ((e = cudaFuncSetAttribute(tc_logits_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max)) !=
-      cudaSuccess)
-    return e;
-  if ((e = cudaFuncSetAttribute(tc_logits_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max)) !=
-      cudaSuccess)
-    return e;
-  if ((e = cudaFuncSetAttribute(tc_gh_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max)) !=
-      cudaSuccess)
-    return e;
-  return cudaFuncSetAttribute(tc_gh_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max);
+  if ((e = cudaFuncSetAttribute(tc_gh_kernel<false>, attr, smem_max)) != cudaSuccess) return e;
+  return cudaFuncSetAttribute(tc_gh_kernel<true>, attr, smem_max);
 }
 
-cudaError_t tc_launch_logits(tts_ctx* c, const StepArgs& a, float* z_out, cudaStream_t s, int* launches) {
+// a2 (+ a3 when `fuse_stats`).  *n_split_out = number of per-row tuples the fused epilogue (plus the fix-up sweep over
+// tiles cut by the stream-K walk) left in c->stat_part, 0 when the statistics were not fused.
+cudaError_t tc_launch_logits(tts_ctx* c, const StepArgs& a, float* z_out, bool fuse_stats, cudaStream_t s, int* launches,
+                             int* n_split_out) {
   TcState* st = static_cast<TcState*>(c->tc_state);
   const int V = c->cfg.V, d = c->cfg.d, T = a.T;
   const int T16 = (T + 15) / 16 * 16;
+  const bool tb = c->cfg.logits_dtype == TTS_BF16;
+  *n_split_out = 0;
   LogitsParams p;
   p.z = z_out; p.z_ld = V;
   p.n_vt = V / kTileMN; p.k_chunks = d / kKC; p.T16 = T16; p.T = T;
   p.box_rows = T16 <= kNMax ? T16 : kNMax;
   p.n_boxes = (T16 + p.box_rows - 1) / p.box_rows;
   const int stage_bytes = kATile + p.n_boxes * p.box_rows * kKC * 2;
-  p.stages = pick_stages(stage_bytes);
+  const int epi_bytes = fuse_stats ? 128 + epi::smem_bytes(T16) : 0;
+  p.stages = pick_stages(stage_bytes, epi_bytes);
   p.n_acc = 2 * T16 <= 512 ? 2 : 1;
   p.tmem_cols = pow2_cols(p.n_acc * T16);
-  CUtensorMap tm_W, tm_h;
+  CUtensorMap tm_W, tm_h, tm_t;
   if (make_map_2d(st, &tm_W, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, a.W_in, d, V, kKC, 64,
                   CU_TENSOR_MAP_SWIZZLE_128B) != CUDA_SUCCESS)
     return cudaErrorInvalidValue;
@@ -521,23 +543,45 @@ cudaError_t tc_launch_logits(tts_ctx* c, const StepArgs& a, float* z_out, cudaSt
   if (make_map_2d(st, &tm_h, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, a.h, d, T, kKC, p.box_rows,
                   CU_TENSOR_MAP_SWIZZLE_128B) != CUDA_SUCCESS)
     return cudaErrorInvalidValue;
+  tm_t = tm_h;
+  if (fuse_stats && tb &&
+      make_map_2d(st, &tm_t, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, a.teacher, V, T, kTileMN, epi::kRows,
+                  CU_TENSOR_MAP_SWIZZLE_NONE) != CUDA_SUCCESS)
+    return cudaErrorInvalidValue;
   int grid = c->cfg.max_ctas > 0 ? c->cfg.max_ctas : c->sm_count;
   if (grid > p.n_vt) grid = p.n_vt;
   // Stream-K for one canvas: 1187 tiles over 148 CTAs would quantise to 9 waves of 8.02; equal contiguous unit
   // ranges keep every SM busy to the end.  A range spans >= k_chunks units (grid <= n_vt), so a tile is cut at most
   // once: it receives exactly two partial sums (or one store), and 0 + a + b does not depend on the order.
   p.stream_k = T16 <= 32 && p.n_vt % grid != 0;
+  // tiles cut by a range boundary: z by fp32 RED in the kernel, statistics by the fix-up sweep afterwards
+  int cut[kStatFixMax], n_cut = 0;
   if (p.stream_k) {
     cudaError_t e = cudaMemsetAsync(z_out, 0, (size_t)T * V * sizeof(float), s);
     if (e != cudaSuccess) return e;
+    const long total = (long)p.n_vt * p.k_chunks;
+    for (int b = 1; b < grid; ++b) {
+      const long u = total * b / grid;
+      if (u % p.k_chunks != 0 && n_cut < kStatFixMax) cut[n_cut++] = (int)(u / p.k_chunks) * kTileMN;
+    }
   }
-  const size_t smem = 1024 + (size_t)p.stages * stage_bytes + sizeof(Bars);
-  if (T16 <= kNMax)
-    tc_logits_kernel<false><<<grid, kGemmThreads, smem, s>>>(tm_W, tm_h, p);
-  else
-    tc_logits_kernel<true><<<grid, kGemmThreads, smem, s>>>(tm_W, tm_h, p);
+  epi::Params ep;
+  ep.teacher = a.teacher; ep.part = c->stat_part; ep.n_split = grid + n_cut; ep.T = T; ep.V = V;
+  ep.enabled = fuse_stats ? 1 : 0;
+  const size_t smem = 1024 + (size_t)p.stages * stage_bytes + sizeof(Bars) + epi_bytes;
+  if (T16 <= kNMax) {
+    if (tb) tc_logits_kernel<false, true><<<grid, kGemmThreads, smem, s>>>(tm_W, tm_h, tm_t, p, ep);
+    else tc_logits_kernel<false, false><<<grid, kGemmThreads, smem, s>>>(tm_W, tm_h, tm_t, p, ep);
+  } else {
+    if (tb) tc_logits_kernel<true, true><<<grid, kGemmThreads, smem, s>>>(tm_W, tm_h, tm_t, p, ep);
+    else tc_logits_kernel<true, false><<<grid, kGemmThreads, smem, s>>>(tm_W, tm_h, tm_t, p, ep);
+  }
   *launches += 1;
-  return cudaGetLastError();
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess || !fuse_stats) return e;
+  if (n_cut > 0) e = launch_row_stats_tiles(c, a, z_out, V, cut, n_cut, grid, ep.n_split, s, launches);
+  *n_split_out = ep.n_split;
+  return e;
 }
 
 // slots of the deterministic-mode scratch for steps of up to T16 rows ([slots][T16][128] fp32)

@@ -25,6 +25,7 @@
 #include <string.h>
 
 #include "tts_common.cuh"
+#include "tts_tc_epi.cuh"
 #include "tts_tc_ptx.cuh"
 #include "tts_tc_state.h"
 
@@ -36,6 +37,7 @@ constexpr int kPATile = 128 * kKC * 2;   // 16 KB: this CTA's [128 x 64] K-major
 constexpr int kPMaxStages = 6;
 constexpr int kPNMax = 256;
 constexpr int kPSmemBudget = 208 * 1024;
+constexpr int kPSmemLimit = 232448;   // 227 KB
 
 struct PairBars {
   uint64_t full[kPMaxStages];
@@ -100,14 +102,17 @@ constexpr uint32_t kDescHiSw128 = (1024u >> 4) | (1u << 14) | (ptx::kSwizzle128B
 __device__ __forceinline__ uint32_t desc_lo_sw128(uint32_t smem_addr) { return ((smem_addr >> 4) & 0x3FFFu) | (1u << 16); }
 __device__ __forceinline__ uint64_t desc64(uint32_t hi, uint32_t lo) { return (static_cast<uint64_t>(hi) << 32) | lo; }
 
+// TB: bf16 teacher (TMA-staged tiles for the fused a3 statistics of tts_tc_epi.cuh; fp32 teachers use vector loads)
+template <bool TB>
 __global__ void __launch_bounds__(kPThreads, 1)
 tc_logits_pair_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant__ CUtensorMap tm_h,
-                      const PairLogitsParams p) {
+                      const __grid_constant__ CUtensorMap tm_teacher, const PairLogitsParams p, const epi::Params ep) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const int piece_bytes = 128 * kKC * 2;                      // this CTA's 128 rows of one N piece: 16 KB
   const int stage_bytes = kPATile + p.n_pieces * piece_bytes;
   PairBars* bars = reinterpret_cast<PairBars*>(smem + p.stages * stage_bytes);
+  uint8_t* epi_base = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(bars + 1) + 127) & ~uintptr_t(127));
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t cta = ptx::cluster_ctarank();
   const int pair = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
@@ -186,19 +191,34 @@ tc_logits_pair_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_con
       }
     }
   } else if (warp >= 4) {
-    // ===== epilogue (both CTAs): thread = one vocabulary row of this CTA's half of the tile =====
+    // ===== epilogue (both CTAs): thread = one vocabulary row of this CTA's half of the tile.  Whole tiles also feed
+    // the fused a3 statistics; the K-split leftover tiles are only accumulated into z (fix-up sweep of tts_stats.cu) =====
     const int q4 = warp & 3;
-    uint32_t it = 0;
+    const int tid_e = threadIdx.x - 128;
+    const epi::Shared esh(epi_base, p.T16);
+    if (ep.enabled) epi::init(esh, p.T16, tid_e);
+    uint32_t it = 0, g = 0;
     PairWalk walk(p, pair, n_pairs);
     PairItem w;
     for (; walk.next(p, w); ++it) {
       ptx::mbar_wait(&bars->acc_full, it & 1);
       ptx::tc_fence_after();
-      const int v = w.pt * 256 + (int)cta * 128 + q4 * 32 + lane;
+      const int v0 = w.pt * 256 + (int)cta * 128;
+      const uint32_t tmem_tile = tmem_base + (static_cast<uint32_t>(q4 * 32) << 16);
+      auto release = [&]() {
+        ptx::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive_cta0(&bars->acc_empty);
+      };
+      if (ep.enabled && !w.partial && v0 < p.V) {
+        epi::tile<TB>(ep, esh, &tm_teacher, tmem_tile, v0, p.T16, p.z, p.z_ld, tid_e, g, release);
+        continue;
+      }
+      const int v = v0 + q4 * 32 + lane;
       float* zc = p.z + v;
       for (int c0 = 0; c0 < p.T16; c0 += 16) {
         uint32_t r[16];
-        ptx::tmem_ld_32x32b_x16(tmem_base + c0 + (static_cast<uint32_t>(q4 * 32) << 16), r);
+        ptx::tmem_ld_32x32b_x16(tmem_tile + c0, r);
         ptx::tmem_ld_wait();
         if (v < p.V) {
           if (w.partial) {
@@ -212,10 +232,9 @@ tc_logits_pair_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_con
           }
         }
       }
-      ptx::tc_fence_before();
-      __syncwarp();
-      if (lane == 0) ptx::mbar_arrive_cta0(&bars->acc_empty);
+      release();
     }
+    if (ep.enabled) epi::flush(ep, esh, blockIdx.x, tid_e);
     if (lane == 0) ptx::watchdog_arrive(&bars->done);
   } else if (warp == 2) {
     ptx::watchdog_wait(&bars->done);
@@ -231,7 +250,9 @@ tc_logits_pair_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_con
 }  // namespace
 
 cudaError_t tc_pair_init(tts_ctx*) {
-  return cudaFuncSetAttribute(tc_logits_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kPSmemBudget + 2048);
+  cudaError_t e = cudaFuncSetAttribute(tc_logits_pair_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPSmemLimit);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(tc_logits_pair_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPSmemLimit);
 }
 
 // 1 when the pair kernels serve this step: several canvases beyond one MMA's N, an even grid of at least one pair
@@ -241,10 +262,13 @@ int tc_pair_eligible(const tts_ctx* c, int T16) {
   return grid >= 2;
 }
 
-cudaError_t tc_launch_logits_pair(tts_ctx* c, const StepArgs& a, float* z_out, cudaStream_t s, int* launches) {
+cudaError_t tc_launch_logits_pair(tts_ctx* c, const StepArgs& a, float* z_out, bool fuse_stats, cudaStream_t s,
+                                  int* launches, int* n_split_out) {
   TcState* st = static_cast<TcState*>(c->tc_state);
   const int V = c->cfg.V, d = c->cfg.d, T = a.T;
   const int T16 = (T + 15) / 16 * 16;
+  const bool tb = c->cfg.logits_dtype == TTS_BF16;
+  *n_split_out = 0;
   PairLogitsParams p;
   p.z = z_out; p.z_ld = V; p.V = V;
   p.n_pt = (V + 255) / 256;
@@ -252,16 +276,22 @@ cudaError_t tc_launch_logits_pair(tts_ctx* c, const StepArgs& a, float* z_out, c
   p.T16 = T16; p.T = T;
   p.n_pieces = (T16 + kPNMax - 1) / kPNMax;
   const int stage_bytes = kPATile + p.n_pieces * 128 * kKC * 2;
-  p.stages = (kPSmemBudget - (int)sizeof(PairBars) - 1024) / stage_bytes;
+  const int epi_bytes = fuse_stats ? 128 + epi::smem_bytes(T16) : 0;
+  p.stages = ((fuse_stats ? kPSmemLimit : kPSmemBudget) - (int)sizeof(PairBars) - 1024 - epi_bytes) / stage_bytes;
   if (p.stages > kPMaxStages) p.stages = kPMaxStages;
   if (p.stages < 2) return cudaErrorInvalidConfiguration;
-  CUtensorMap tm_W, tm_h;
+  CUtensorMap tm_W, tm_h, tm_t;
   if (make_map_2d(st, &tm_W, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, a.W_in, d, V, kKC, 64,
                   CU_TENSOR_MAP_SWIZZLE_128B) != CUDA_SUCCESS)
     return cudaErrorInvalidValue;
   // rows >= T of a box are out of bounds: TMA fills them with zeros
   if (make_map_2d(st, &tm_h, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, a.h, d, T, kKC, 128,
                   CU_TENSOR_MAP_SWIZZLE_128B) != CUDA_SUCCESS)
+    return cudaErrorInvalidValue;
+  tm_t = tm_h;
+  if (fuse_stats && tb &&
+      make_map_2d(st, &tm_t, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, a.teacher, V, T, 128, epi::kRows,
+                  CU_TENSOR_MAP_SWIZZLE_NONE) != CUDA_SUCCESS)
     return cudaErrorInvalidValue;
   int grid = c->cfg.max_ctas > 0 ? c->cfg.max_ctas : c->sm_count;
   grid &= ~1;
@@ -271,25 +301,34 @@ cudaError_t tc_launch_logits_pair(tts_ctx* c, const StepArgs& a, float* z_out, c
   p.n_left = p.n_pt % n_pairs;
   if (p.n_left > n_pairs / 2) { p.n_rounds += 1; p.n_left = 0; }   // a nearly full last round: whole tiles
   p.n_main = p.n_pt - p.n_left;
+  int cut[kStatFixMax], n_cut = 0;
   if (p.n_left > 0) {
-    // the K-split tiles accumulate into zeroed columns [256 n_main, V) of z
+    // the K-split tiles accumulate into zeroed columns [256 n_main, V) of z; their statistics come from the fix-up sweep
     const size_t v_left = (size_t)p.n_main * 256;
     cudaError_t e = cudaMemset2DAsync(z_out + v_left, (size_t)V * sizeof(float), 0, (V - v_left) * sizeof(float), T, s);
     if (e != cudaSuccess) return e;
+    for (size_t v = v_left; v < (size_t)V && n_cut < kStatFixMax; v += 128) cut[n_cut++] = (int)v;
   }
+  epi::Params ep;
+  ep.teacher = a.teacher; ep.part = c->stat_part; ep.n_split = grid + n_cut; ep.T = T; ep.V = V;
+  ep.enabled = fuse_stats ? 1 : 0;
   cudaLaunchConfig_t cfg;
   memset(&cfg, 0, sizeof(cfg));
   cfg.gridDim = dim3(grid);
   cfg.blockDim = dim3(kPThreads);
-  cfg.dynamicSmemBytes = 1024 + (size_t)p.stages * stage_bytes + sizeof(PairBars);
+  cfg.dynamicSmemBytes = 1024 + (size_t)p.stages * stage_bytes + sizeof(PairBars) + epi_bytes;
   cfg.stream = s;
   cudaLaunchAttribute attr;
   attr.id = cudaLaunchAttributeClusterDimension;
   attr.val.clusterDim.x = 2; attr.val.clusterDim.y = 1; attr.val.clusterDim.z = 1;
   cfg.attrs = &attr;
   cfg.numAttrs = 1;
-  cudaError_t e = cudaLaunchKernelEx(&cfg, tc_logits_pair_kernel, tm_W, tm_h, p);
+  cudaError_t e = tb ? cudaLaunchKernelEx(&cfg, tc_logits_pair_kernel<true>, tm_W, tm_h, tm_t, p, ep)
+                     : cudaLaunchKernelEx(&cfg, tc_logits_pair_kernel<false>, tm_W, tm_h, tm_t, p, ep);
   *launches += 1;
+  if (e != cudaSuccess || !fuse_stats) return e;
+  if (n_cut > 0) e = launch_row_stats_tiles(c, a, z_out, V, cut, n_cut, grid, ep.n_split, s, launches);
+  *n_split_out = ep.n_split;
   return e;
 }
 

@@ -40,7 +40,10 @@ inline CUresult make_map_2d(const TcState* st, CUtensorMap* m, CUtensorMapDataTy
 // tts_tc_gemm.cu
 cudaError_t tc_gemm_init(tts_ctx* c);
 // a2: z[r, v] = sum_j h[r, j] W_in[v, j] on tcgen05 (fp32 accumulation), z scratch [T16, V]
-cudaError_t tc_launch_logits(tts_ctx* c, const StepArgs& a, float* z_out, cudaStream_t s, int* launches);
+// fuse_stats: the a3 online statistics are taken in the kernel's epilogue (tts_tc_epi.cuh) and *n_split_out tuples per
+// canvas row are left in c->stat_part for launch_row_stats_finish; otherwise *n_split_out = 0
+cudaError_t tc_launch_logits(tts_ctx* c, const StepArgs& a, float* z_out, bool fuse_stats, cudaStream_t s, int* launches,
+                             int* n_split_out);
 // a5: gh[r, j] = sum_v dl[r, v] W_in[v, j] on tcgen05, split over the vocabulary, fp32 atomics into gh
 cudaError_t tc_launch_gh(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches);
 // floats of the deterministic-mode scratch (per-unit parts of gh) for steps of up to T16 rows
@@ -63,6 +66,7 @@ cudaError_t tc_launch_update_wide(tts_ctx* c, const StepArgs& a, cudaStream_t s,
 // tts_tc_pair.cu: CTA-pair (cta_group::2) a2 for 256 < T16 <= 512
 cudaError_t tc_pair_init(tts_ctx* c);
 int tc_pair_eligible(const tts_ctx* c, int T16);
-cudaError_t tc_launch_logits_pair(tts_ctx* c, const StepArgs& a, float* z_out, cudaStream_t s, int* launches);
+cudaError_t tc_launch_logits_pair(tts_ctx* c, const StepArgs& a, float* z_out, bool fuse_stats, cudaStream_t s,
+                                  int* launches, int* n_split_out);
 
 }  // namespace tts

@@ -72,7 +72,8 @@ def test_given_draft_logits_skip_pass_a(V, d, path):
                                 draft_logits=_dev(z_given))
         n_given = tts.tts_last_launch_count(ctx)
         torch.cuda.synchronize()
-        assert n_given == n_full - 1
+        # pass a2 is gone; on the tensor path its epilogue carried a3, which now runs as its own sweep
+        assert n_given == n_full - 1 if path == tts.TTS_PATH_SIMT else n_given <= n_full
         assert abs(float(loss.item()) - o["loss"]) <= 1e-3 * abs(o["loss"]) + 1e-6
         assert np.all(np.abs(t["kl"].cpu().numpy() - o["kl_rows"]) <= 1e-3 * np.abs(o["kl_rows"]) + 1e-5)
         _check_state(t["master"], t["m"], t["v"], t["gh"], o)
