@@ -68,6 +68,9 @@ def parse_args():
     ap.add_argument("--max-ctas", type=int, default=0,
                     help="SM budget of the step's persistent kernels (tts_config.max_ctas; 0 = all SMs): what the main "
                          "stream keeps while the update overlaps it (PAPER.md:426)")
+    ap.add_argument("--side-priority", default="default", choices=["default", "high", "low"],
+                    help="--stream: CUDA priority of the update's side stream relative to the main stream (low = the "
+                         "harness's main stream is created with high priority instead)")
     ap.add_argument("--stream", action="store_true",
                     help="also run the long-generation stream protocol (BASELINE.json configs[4]; use --config 5)")
     ap.add_argument("--rounds", type=int, default=4000, help="--stream: speculation rounds per pass")
@@ -515,6 +518,13 @@ def run_ours(args, rank, world, local_rank):
             "gpu_launches": launches[0], "roofline": roof, "cpu_baseline": cpu}
     if stream is not None:
         line["stream"] = stream
+    # what crosses the fabric per step, for the driver's rank check: replicas exchange nothing on the data path
+    if world > 1:
+        line["comm"] = ({"ranks": world, "backend": shard.exchange.backend, "pattern": "vocabulary shards",
+                         "per_rank_bytes_per_step": shard.exchange.bytes_per_step(T, d)} if vocab else
+                        {"ranks": world, "backend": "nccl", "pattern": "replicas: no data-path collective; one "
+                         "max-over-ranks / sum-over-ranks scalar reduction around the timed region",
+                         "per_rank_bytes_per_step": {}})
     print(json.dumps(line), flush=True)
 
 
@@ -539,7 +549,10 @@ def run_stream(args, case, dev):
     V, d, C = case["V"], case["d"], case["seg_len"]
     T = C
     tdev = torch.device(dev)
+    if args.side_priority == "low":       # the main stream outranks the side stream
+        torch.cuda.set_stream(torch.cuda.Stream(device=tdev, priority=-1))
     main = torch.cuda.current_stream()
+    side_prio = -1 if args.side_priority == "high" else None
     W0, master0 = case["W"].clone(), case["master"].clone()
     u = torch.from_numpy(synth.stream_direction(V, c["seed"])).to(tdev)
     pw = case["pos_weight"][:T].contiguous()
@@ -590,7 +603,7 @@ def run_stream(args, case, dev):
         master, W = master0.clone(), W0.clone()
         up = DraftHeadUpdater(W, master, m, v, seg_len=C, T_max=T, stride=stride, lr=c["lr"], beta1=c["beta1"],
                               beta2=c["beta2"], eps=c["eps"], weight_decay=c["weight_decay"], want_gh=True,
-                              max_ctas=args.max_ctas)
+                              max_ctas=args.max_ctas, priority=side_prio)
         g = torch.Generator(device=tdev)
         g.manual_seed(1000003 * (c["seed"] + 1))
         fn = standins[kind][0]
@@ -629,7 +642,8 @@ def run_stream(args, case, dev):
         up.close()
         return out
 
-    res = {"rounds": rounds, "timed_rounds": rounds - skip, "runs": []}
+    res = {"rounds": rounds, "timed_rounds": rounds - skip, "max_ctas": args.max_ctas,
+           "side_priority": args.side_priority, "runs": []}
     for kind in [k for k in args.standins.split(",") if k in standins]:
         base = one_pass(kind, 1, False)
         for S in [int(x) for x in args.strides.split(",")]:

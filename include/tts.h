@@ -327,6 +327,8 @@ int32_t tts_sync_step(tts_ctx* ctx);
  * from (preferably pinned) host memory into ctx-owned staging buffers, runs tts_accept_mask and
  * tts_distill_step on `stream`, copies loss / tau / mask back and synchronises the stream.
  * The persistent draft state (W, master, m, v) stays resident on the device: device pointers.
+ * The teacher logits (the bulk of the bytes: 160 MB at 512 rows) travel on a copy stream owned by the ctx while pass
+ * a2, which needs only h and W_in, already runs on `stream` (tensor path); a1 and a3 wait for the copy.
  */
 int32_t tts_round_host(tts_ctx* ctx,
                        const void* teacher_logits_host, /* host [T,V] logits_dtype */

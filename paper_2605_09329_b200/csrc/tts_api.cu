@@ -37,6 +37,9 @@ void free_all(tts_ctx* c) {
   cudaFree(c->st_teacher); cudaFree(c->st_h); cudaFree(c->st_tok); cudaFree(c->st_pw);
   cudaFree(c->st_mask); cudaFree(c->st_tau); cudaFree(c->st_loss);
   if (c->done_event) cudaEventDestroy(c->done_event);
+  if (c->copy_fork) cudaEventDestroy(c->copy_fork);
+  if (c->copy_done) cudaEventDestroy(c->copy_done);
+  if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
   if (c->prof_events) {
     for (int i = 0; i < tts::kProfSlots * (TTS_NUM_PHASES + 1); ++i) cudaEventDestroy(c->prof_events[i]);
     free(c->prof_events);
@@ -99,6 +102,9 @@ int32_t tts_ctx_create(const tts_config* cfg, int32_t device, tts_ctx** out) {
   const size_t V = cfg->V, Tm = cfg->T_max, Tp = c->T_pad_max;
   bool ok = true;
   ok = ok && cudaEventCreateWithFlags(&c->done_event, cudaEventDisableTiming) == cudaSuccess;
+  ok = ok && cudaEventCreateWithFlags(&c->copy_fork, cudaEventDisableTiming) == cudaSuccess;
+  ok = ok && cudaEventCreateWithFlags(&c->copy_done, cudaEventDisableTiming) == cudaSuccess;
+  ok = ok && cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) == cudaSuccess;
   ok = ok && dmalloc(&c->step_count_dev, 1) == cudaSuccess;
   ok = ok && dmalloc(&c->step_scalars, 2) == cudaSuccess;
   ok = ok && cudaMemset(c->step_count_dev, 0, sizeof(unsigned long long)) == cudaSuccess;
@@ -509,21 +515,38 @@ int32_t tts_round_host(tts_ctx* c, const void* teacher_host, const void* h_host,
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const size_t V = cfg.V, d = cfg.d;
   cudaError_t e;
-  if ((e = cudaMemcpyAsync(c->st_teacher, teacher_host, (size_t)T * V * elem_size(cfg.logits_dtype),
-                           cudaMemcpyHostToDevice, s)) != cudaSuccess) return cuda_fail(c, e);
+  // The small inputs go first on the caller's stream; the teacher logits (the bulk: 160 MB at 512 rows, ~3 ms of
+  // PCIe) are copied on the ctx's copy stream while pass a2, which needs only h and W_in, runs on the caller's stream
+  // (tensor path).  a1, a3 and the rest wait for the copy; a3 then runs as its own sweep over the finished z.
   if ((e = cudaMemcpyAsync(c->st_h, h_host, (size_t)T * d * elem_size(cfg.param_dtype),
                            cudaMemcpyHostToDevice, s)) != cudaSuccess) return cuda_fail(c, e);
   if ((e = cudaMemcpyAsync(c->st_tok, tok_host, (size_t)T * 4, cudaMemcpyHostToDevice, s)) != cudaSuccess)
     return cuda_fail(c, e);
   if ((e = cudaMemcpyAsync(c->st_pw, pw_host, (size_t)T * 4, cudaMemcpyHostToDevice, s)) != cudaSuccess)
     return cuda_fail(c, e);
+  if ((e = cudaEventRecord(c->copy_fork, s)) != cudaSuccess) return cuda_fail(c, e);
+  if ((e = cudaStreamWaitEvent(c->copy_stream, c->copy_fork, 0)) != cudaSuccess) return cuda_fail(c, e);
+  if ((e = cudaMemcpyAsync(c->st_teacher, teacher_host, (size_t)T * V * elem_size(cfg.logits_dtype),
+                           cudaMemcpyHostToDevice, c->copy_stream)) != cudaSuccess) return cuda_fail(c, e);
+  if ((e = cudaEventRecord(c->copy_done, c->copy_stream)) != cudaSuccess) return cuda_fail(c, e);
+  int early_launches = 0;
+  tts_step_extras ex;
+  ex.draft_logits = nullptr; ex.draft_logits_out = nullptr; ex.ref_logits = nullptr; ex.lambda = 0.f;
+  if (c->tensor_ok && aligned16(W_in)) {
+    tts::StepArgs a0;
+    memset(&a0, 0, sizeof(a0));
+    a0.h = c->st_h; a0.W_in = W_in; a0.T = T;
+    if ((e = tts::tc_logits_only(c, a0, s, &early_launches)) != cudaSuccess) return cuda_fail(c, e);
+    ex.draft_logits = c->z;                          // the step below takes z as given: a2 is done
+  }
+  if ((e = cudaStreamWaitEvent(s, c->copy_done, 0)) != cudaSuccess) return cuda_fail(c, e);
   int32_t st = tts_accept_mask(c, c->st_teacher, c->st_tok, T, c->st_mask, c->st_tau, nullptr, stream);
   if (st != TTS_OK) return st;
   const int mask_launches = c->last_launches;
-  st = tts_distill_step(c, c->st_teacher, c->st_h, W_in, W_out, W_master, adam_m, adam_v, c->st_pw, c->st_mask, T,
-                        loss_scale, c->st_loss, nullptr, gh_dev, nullptr, stream);
+  st = tts_distill_step_ex(c, c->st_teacher, c->st_h, W_in, W_out, W_master, adam_m, adam_v, c->st_pw, c->st_mask, T,
+                           loss_scale, c->st_loss, nullptr, gh_dev, nullptr, &ex, stream);
   if (st != TTS_OK) return st;
-  c->last_launches += mask_launches;
+  c->last_launches += mask_launches + early_launches;
   if ((e = cudaMemcpyAsync(loss_host, c->st_loss, 4, cudaMemcpyDeviceToHost, s)) != cudaSuccess) return cuda_fail(c, e);
   if ((e = cudaMemcpyAsync(tau_host, c->st_tau, (size_t)(T / cfg.seg_len) * 4, cudaMemcpyDeviceToHost, s)) !=
       cudaSuccess)

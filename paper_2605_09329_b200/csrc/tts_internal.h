@@ -107,6 +107,8 @@ struct tts_ctx {
   uint8_t* st_mask;
   int32_t* st_tau;
   float* st_loss;
+  cudaStream_t copy_stream;   // tts_round_host: the teacher's H2D copy runs here, next to a2 on the caller's stream
+  cudaEvent_t copy_fork, copy_done;
   // ---- per-phase profiling (tts_profile_*) ----
   bool prof_on;
   int prof_count;                                   // steps recorded since the last read
@@ -164,5 +166,8 @@ bool tc_supported(const tts_config& cfg);
 cudaError_t tc_init(tts_ctx* c);
 void tc_destroy(tts_ctx* c);
 cudaError_t tc_step(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches);
+// a2 alone into the ctx's z scratch (no statistics): what tts_round_host runs while the round's teacher logits are
+// still on their way from the host
+cudaError_t tc_logits_only(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches);
 
 }  // namespace tts

@@ -61,6 +61,13 @@ void tc_destroy(tts_ctx* c) {
   c->tc_state = nullptr;
 }
 
+cudaError_t tc_logits_only(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches) {
+  const int T16 = (a.T + 15) / 16 * 16;
+  int n_tuples = 0;
+  return tc_pair_eligible(c, T16) ? tc_launch_logits_pair(c, a, c->z, false, s, launches, &n_tuples)
+                                  : tc_launch_logits(c, a, c->z, false, s, launches, &n_tuples);
+}
+
 cudaError_t tc_step(tts_ctx* c, const StepArgs& a, cudaStream_t s, int* launches) {
   const int V = c->cfg.V, T = a.T;
   const int T16 = (T + 15) / 16 * 16;

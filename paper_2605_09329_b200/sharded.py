@@ -47,11 +47,52 @@ def all_reduce_sum_(x: torch.Tensor, group=None) -> torch.Tensor:
     return x
 
 
+class ShardExchange:
+    """What vocabulary shards exchange per round, as an interface: three tiny collectives between library calls.
+    `TorchDistExchange` (NCCL on GPUs, gloo in the CPU tests) is the implementation shipped; a one-shot multimem /
+    NVLS reduction over NVSwitch peer memory can replace it later without touching VocabShardedStep or the C ABI.
+    `bytes_per_step(T, d)` is the traffic per rank and round, for bench.py's `comm` record."""
+
+    n_shards = 1
+
+    def gather_stats(self, stats):        # [T, 8] fp32 -> [n_shards, T, 8], rank order
+        raise NotImplementedError
+
+    def reduce_gh(self, gh):              # [T, d] fp32, summed over shards in place
+        raise NotImplementedError
+
+    def gather_argmax(self, val, idx):    # ([T] fp32, [T] i32) -> ([n_shards, T], [n_shards, T])
+        raise NotImplementedError
+
+    def bytes_per_step(self, T, d):
+        n = self.n_shards
+        return {"all_gather_row_tuples": {"send": 32 * T, "recv": 32 * T * n},
+                "all_reduce_gh": {"bytes": 4 * T * d},
+                "all_gather_argmax": {"send": 8 * T, "recv": 8 * T * n}}
+
+
+class TorchDistExchange(ShardExchange):
+    def __init__(self, group=None):
+        self.group = group
+        self.n_shards = dist.get_world_size(group) if dist.is_initialized() else 1
+        self.backend = dist.get_backend(group) if dist.is_initialized() else "none"
+
+    def gather_stats(self, stats):
+        return all_gather_rows(stats, self.group)
+
+    def reduce_gh(self, gh):
+        return all_reduce_sum_(gh, self.group)
+
+    def gather_argmax(self, val, idx):
+        return all_gather_rows(val, self.group), all_gather_rows(idx, self.group)
+
+
 class VocabShardedStep:
     """One rank's half of the sharded round.  `cfg_local` is this rank's tts_config (its V is the shard's row count)."""
 
-    def __init__(self, cfg_local: tts.tts_config, v_offset: int, device: int = 0, group=None):
+    def __init__(self, cfg_local: tts.tts_config, v_offset: int, device: int = 0, group=None, exchange=None):
         self.cfg, self.v_offset, self.group = cfg_local, v_offset, group
+        self.exchange = exchange if exchange is not None else TorchDistExchange(group)
         self.dev = torch.device("cuda", device)
         self.ctx = tts.tts_ctx_create(cfg_local, device)
         T = cfg_local.T_max
@@ -68,8 +109,7 @@ class VocabShardedStep:
         s = stream if stream is not None else torch.cuda.current_stream(self.dev)
         with torch.cuda.stream(s):
             tts.tts_shard_argmax(self.ctx, teacher_local, T, self.v_offset, self.am_val, self.am_idx, s)
-            val_all = all_gather_rows(self.am_val[:T], self.group)
-            idx_all = all_gather_rows(self.am_idx[:T], self.group)
+            val_all, idx_all = self.exchange.gather_argmax(self.am_val[:T], self.am_idx[:T])
             tts.tts_shard_accept_mask(self.ctx, val_all, idx_all, val_all.shape[0], draft_tokens, T, mask_out, tau_out,
                                       teacher_argmax_out, s)
         return val_all.shape[0]
@@ -80,10 +120,10 @@ class VocabShardedStep:
         s = stream if stream is not None else torch.cuda.current_stream(self.dev)
         with torch.cuda.stream(s):
             tts.tts_shard_begin_step(self.ctx, teacher_local, h, W_in, T, self.stats, side_stream=s, **extras)
-            stats_all = all_gather_rows(self.stats[:T], self.group)
+            stats_all = self.exchange.gather_stats(self.stats[:T])
             tts.tts_shard_finish_step(self.ctx, stats_all, stats_all.shape[0], teacher_local, h, W_in, W_out, W_master,
                                       adam_m, adam_v, pos_weight, mask, T, loss_scale, loss_out, kl_rows_out, gh_out,
                                       gW_debug_out, side_stream=s, **extras)
             if gh_out is not None:
-                all_reduce_sum_(gh_out, self.group)
+                self.exchange.reduce_gh(gh_out)
         return stats_all.shape[0]
