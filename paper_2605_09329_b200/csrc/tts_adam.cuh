@@ -9,6 +9,24 @@
 
 namespace tts {
 
+// sqrt(v) of Adam's denominator as ONE MUFU instruction.  __fsqrt_rn expands to a reciprocal square root, a Newton
+// step and a branch to a slow path per element; the branch keeps ptxas from interleaving the elements a thread
+// updates, and the update kernels' epilogues (the per-SM bound of every variant that is not HBM-bound) then stall on
+// fixed instruction latencies: ncu, round 2.  Relative error 2^-22 against tolerances of 2e-3 (R12, R13).  The
+// non-ftz approximations (and __fdividef) wrap every MUFU in a subnormal test and two scalings: 6 more instructions
+// per element for inputs that cannot change the result.
+__device__ __forceinline__ float adam_sqrt(float x) {
+  float y;
+  asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));   // ftz: a subnormal v gives 0, i.e. den = eps (sqrt(v) < 1.1e-19 << eps)
+  return y;
+}
+// 1 / den for den = sqrt(v) / sqrt(1 - b2^n) + eps >= eps: one MUFU, no subnormal scaling (den is normal whenever eps is)
+__device__ __forceinline__ float adam_rcp(float x) {
+  float y;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+
 // 16 pseudo-random bits for element idx = v * d + j at Adam count n:
 //   x = lo32(idx) ^ (n * 0x9E3779B9) ^ (seed * 0x85EBCA6B) ^ (hi32(idx) * 0xC2B2AE35)
 //   x ^= x >> 16;  x *= 0x7FEB352D;  x ^= x >> 15;  x *= 0x846CA68B;  x ^= x >> 16;   bits = x >> 16

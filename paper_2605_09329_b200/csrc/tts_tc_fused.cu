@@ -125,7 +125,7 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
                     const __grid_constant__ CUtensorMap tm_v, const __grid_constant__ CUtensorMap tm_wout,
                     const FusedParams p) {
   extern __shared__ uint8_t smem_raw[];
-  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  uint8_t* smem = ptx::align_smem_1024(smem_raw);
   const int kStages = p.stages;
   constexpr int kStageB = MOM ? kStageBytesLp : kStageBytes;
   constexpr int kMomB = MOM ? kMomBytesLp : kTensorBytes;            // bytes of one moment tensor in a stage
@@ -365,8 +365,8 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
             if (ADAM) {
               const float m1 = p.b1 * mm[jb][v] + (1.f - p.b1) * gg;
               const float v1 = p.b2 * vv[jb][v] + (1.f - p.b2) * gg * gg;
-              const float den = __fsqrt_rn(v1) * inv_sqrt_bc2 + p.eps;
-              M[jb][v] = M[jb][v] * p.decay - __fdividef(c1 * m1, den);     // the step uses the unrounded moments
+              const float den = adam_sqrt(v1) * inv_sqrt_bc2 + p.eps;
+              M[jb][v] = fmaf(-(c1 * m1), adam_rcp(den), M[jb][v] * p.decay);     // the step uses the unrounded moments
               if (MOM) {
                 const unsigned long long idx =
                     (unsigned long long)(v0 + sub * kSV + v) * (unsigned long long)p.d + (j_stripe + jb * kMJ + jj);
@@ -453,7 +453,7 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
   }
 }
 
-constexpr int kStagesF32 = 7, kStagesLp = 10;
+constexpr int kStagesF32 = 6, kStagesLp = 6;
 size_t fused_smem(bool lowp) {
   return 1024 + (lowp ? (size_t)kStagesLp * kStageBytesLp : (size_t)kStagesF32 * kStageBytes) + kWtBytes +
          2 * (size_t)kWoBytes + (size_t)kOpStages * kDlBytes + 512;
@@ -534,12 +534,13 @@ int tc_fused_grid(const tts_ctx* c, int T16) {
   if (T16 > kT16 || c->cfg.d % kSW != 0 || c->cfg.V % kTV != 0) return 0;
   const int n_stripes = c->cfg.d / kSW;
   const long n_tiles = (long)(c->cfg.V / kTV) * n_stripes;
-  int grid = c->cfg.max_ctas > 0 ? c->cfg.max_ctas : c->sm_count;
+  const bool lowp = c->cfg.optimizer == TTS_ADAMW && c->cfg.moment_dtype == TTS_MOMENT_BF16;
+  int grid = tc_update_ctas(c, lowp);
   if (grid < n_stripes) return 0;
   if (grid > n_tiles) grid = (int)n_tiles;
   // A grid that is a multiple of the stripe count lets every CTA own ONE stripe for the whole pass (no second h^T load,
-  // one gh flush, the walk known at compile time).  d = 5120: 145 = 5 x 29 of 148 CTAs measured 3.06 ms against 3.21 ms
-  // for the stream-K walk over all 148 (and 3.15 ms at 140), so a few idle SMs are the better deal.
+  // one gh flush, the walk known at compile time): d = 4096 runs 132 = 4 x 33 CTAs, d = 5120 130 = 5 x 26 (measured
+  // 3.11 ms; 135, 140 and 145 CTAs 3.36-3.38 ms, the stream-K walk over all 148 3.21 ms).
   const int whole = grid - grid % n_stripes;
   if (whole >= n_stripes && 10 * whole >= 9 * grid) grid = whole;
   return grid;

@@ -107,7 +107,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1)
 tc_logits_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant__ CUtensorMap tm_h,
                  const __grid_constant__ CUtensorMap tm_teacher, const LogitsParams p, const epi::Params ep) {
   extern __shared__ uint8_t smem_raw[];
-  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  uint8_t* smem = ptx::align_smem_1024(smem_raw);
   const int b_bytes = p.n_boxes * p.box_rows * kKC * 2;
   const int stage_bytes = kATile + b_bytes;
   Bars* bars = reinterpret_cast<Bars*>(smem + p.stages * stage_bytes);
@@ -291,7 +291,7 @@ template <bool MC>
 __global__ void __launch_bounds__(kGhThreads, 1)
 tc_gh_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant__ CUtensorMap tm_dl, const GhParams p) {
   extern __shared__ uint8_t smem_raw[];
-  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  uint8_t* smem = ptx::align_smem_1024(smem_raw);
   const int b_bytes = p.n_boxes * p.box_rows * kKC * 2;
   const int stage_bytes = kATile + b_bytes;
   Bars* bars = reinterpret_cast<Bars*>(smem + p.stages * stage_bytes);

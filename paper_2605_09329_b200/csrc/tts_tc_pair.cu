@@ -108,7 +108,7 @@ __global__ void __launch_bounds__(kPThreads, 1)
 tc_logits_pair_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_constant__ CUtensorMap tm_h,
                       const __grid_constant__ CUtensorMap tm_teacher, const PairLogitsParams p, const epi::Params ep) {
   extern __shared__ uint8_t smem_raw[];
-  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  uint8_t* smem = ptx::align_smem_1024(smem_raw);
   const int piece_bytes = 128 * kKC * 2;                      // this CTA's 128 rows of one N piece: 16 KB
   const int stage_bytes = kPATile + p.n_pieces * piece_bytes;
   PairBars* bars = reinterpret_cast<PairBars*>(smem + p.stages * stage_bytes);

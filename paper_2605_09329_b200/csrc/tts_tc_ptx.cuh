@@ -13,6 +13,14 @@ __device__ __forceinline__ uint32_t smem_u32(const void* p) {
   return static_cast<uint32_t>(__cvta_generic_to_shared(p));
 }
 
+// 1024-byte aligned start of the dynamic shared memory (what the 128-byte swizzle atoms want), formed as an OFFSET on
+// the __shared__ array: an integer round trip of the pointer loses the address space, and every access derived from it
+// becomes a generic LD / ST (64-bit addresses, window check) instead of LDS / STS -- ncu showed exactly that in the
+// update kernels' epilogues.
+__device__ __forceinline__ uint8_t* align_smem_1024(uint8_t* raw) {
+  return raw + ((1024u - (smem_u32(raw) & 1023u)) & 1023u);
+}
+
 __device__ __forceinline__ bool elect_one() {
   uint32_t pred;
   asm volatile(

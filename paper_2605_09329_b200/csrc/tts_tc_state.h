@@ -37,6 +37,20 @@ inline CUresult make_map_2d(const TcState* st, CUtensorMap* m, CUtensorMapDataTy
                     CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
 }
 
+// CTAs of an update pass (tc_update_gh_kernel, tc_update_wide_kernel) when the caller sets no SM budget.
+// With fp32 moments the pass is HBM-bound and the memory system, not the SM count, sets its speed: measured on B200
+// (Qwen3-8B head, profiles/r2_README.md) the one-canvas pass runs 2.46 ms on 132 CTAs whatever the ring depth (5-7
+// stages) and 2.51 / 2.68 / 2.74 ms on 148 CTAs with 5 / 6 / 7 stages; every grid of 136 CTAs and more shows that
+// cliff, every grid from 124 to 132 does not; the several-canvas pass behaves the same way (2.69 against 2.73-2.91 ms
+// at 64 rows).  So those passes leave a tenth of the SMs idle.  With bf16 moments the pass is bound by its epilogue
+// warps (18 bytes per parameter) and wants every SM.
+inline int tc_update_ctas(const tts_ctx* c, bool lowp_moments) {
+  if (c->cfg.max_ctas > 0) return c->cfg.max_ctas < c->sm_count ? c->cfg.max_ctas : c->sm_count;
+  if (lowp_moments) return c->sm_count;
+  const int g = (c->sm_count * 229) >> 8;   // 0.895 x SMs: 132 of 148
+  return g < 1 ? 1 : g;
+}
+
 // tts_tc_gemm.cu
 cudaError_t tc_gemm_init(tts_ctx* c);
 // a2: z[r, v] = sum_j h[r, j] W_in[v, j] on tcgen05 (fp32 accumulation), z scratch [T16, V]

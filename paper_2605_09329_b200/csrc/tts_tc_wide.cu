@@ -130,7 +130,7 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
                       const __grid_constant__ CUtensorMap tm_v, const __grid_constant__ CUtensorMap tm_wout,
                       const WideParams p) {
   extern __shared__ uint8_t smem_raw[];
-  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  uint8_t* smem = ptx::align_smem_1024(smem_raw);
   constexpr int kSubs = NV / kWSV;
   constexpr int kStageB = MOM ? kWStageBytesLp : kWStageBytes;
   constexpr int kMomB = MOM ? kWMomBytesLp : kWTensorBytes;
@@ -424,8 +424,8 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
           if (ADAM) {
             const float m1 = p.b1 * mm[r] + (1.f - p.b1) * gg;
             const float v1 = p.b2 * vv[r] + (1.f - p.b2) * gg * gg;
-            const float den = __fsqrt_rn(v1) * inv_sqrt_bc2 + p.eps;
-            M[r] = M[r] * p.decay - __fdividef(c1 * m1, den);     // the step uses the unrounded moments
+            const float den = adam_sqrt(v1) * inv_sqrt_bc2 + p.eps;
+            M[r] = fmaf(-(c1 * m1), adam_rcp(den), M[r] * p.decay);     // the step uses the unrounded moments
             if (MOM) {
               const unsigned long long idx =
                   (unsigned long long)(v0 + sub * kWSV + r) * (unsigned long long)p.d + (j0 + jj);
@@ -746,7 +746,9 @@ cudaError_t tc_launch_update_wide(tts_ctx* c, const StepArgs& a, cudaStream_t s,
   const int fixed = 1024 + p.op_stages * NV * Kp * 2 + 2 * kWWoBytes + (gh_here ? kWWtBytes : 0) + (int)sizeof(WideBars);
   const int stage_bytes = lowp ? kWStageBytesLp : kWStageBytes;
   p.stages = (kWSmemBudget - fixed) / stage_bytes;
-  if (p.stages > (lowp ? kWMaxStages : 16)) p.stages = lowp ? kWMaxStages : 16;
+  // ring depth: the pass's speed is flat from 7 stages up at the grid tc_update_ctas picks (8: 2.68 ms at 64 rows,
+  // 2.78 at 256, 2.83 at 512; 6: 3.04 / 3.13 / 3.12), deeper rings only take shared memory
+  if (p.stages > (lowp ? kWMaxStages : 8)) p.stages = lowp ? kWMaxStages : 8;
   if (p.stages < 2) return cudaErrorInvalidConfiguration;
   p.lr = a.lr; p.b1 = a.beta1; p.b2 = a.beta2; p.eps = a.eps;
   p.decay = 1.f - a.lr * a.wd;
@@ -754,7 +756,7 @@ cudaError_t tc_launch_update_wide(tts_ctx* c, const StepArgs& a, cudaStream_t s,
   p.step_count = c->step_count_dev;
   p.sr_seed = static_cast<uint32_t>(c->cfg.sr_seed);
   const long units = (long)p.n_stripes * (p.n_bands / p.n_win);
-  int grid = c->cfg.max_ctas > 0 ? c->cfg.max_ctas : c->sm_count;
+  int grid = tc_update_ctas(c, lowp);
   if (grid > units) grid = (int)units;
   const size_t smem = (size_t)fixed + (size_t)p.stages * stage_bytes;
   if (lowp)
