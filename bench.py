@@ -95,9 +95,9 @@ def measured_peaks():
 
 def profiled_traffic(cfg_id):
     """dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed
-    `ncu --set full` capture of this workload (profiles/r1e_README.md has the command); None when there is none."""
+    `ncu --set full` capture of this workload (profiles/r2_README.md has the command); None when there is none."""
     import csv
-    p = os.path.join(ROOT, "profiles", "r1e_ncu_full_config%d.csv" % cfg_id)
+    p = os.path.join(ROOT, "profiles", "r2_ncu_full_config%d.csv" % cfg_id)
     if not os.path.exists(p):
         return None
     try:
