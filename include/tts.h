@@ -214,10 +214,13 @@ int32_t tts_accept_stochastic(tts_ctx* ctx,
  *            pass).  Per element: widen m, v exactly; update as above with the UNROUNDED new moments; store
  *            m = rn_bf16(m_new) and v = bf16 by STOCHASTIC rounding of v_new (beta2 = 0.999 decays v by 0.1% per
  *            step, below half a bf16 ulp: nearest rounding would freeze it): the 16 discarded fp32 bits f round
- *            away from zero iff f + r >= 65536, r = the 16 bits of a counter-based generator keyed by the element
- *            index v * d + j (LOCAL rows on a vocabulary shard), Adam's count n and cfg.sr_seed:
- *              x = lo32(idx) ^ (n * 0x9E3779B9) ^ (sr_seed * 0x85EBCA6B) ^ (hi32(idx) * 0xC2B2AE35)
- *              x ^= x >> 16; x *= 0x7FEB352D; x ^= x >> 15; x *= 0x846CA68B; x ^= x >> 16;  r = x >> 16
+ *            away from zero iff f + r >= 65536, r = 16 bits of a counter-based generator keyed by the element's
+ *            position (v, j) (LOCAL rows on a vocabulary shard), Adam's count n and cfg.sr_seed.  One 32-bit hash
+ *            serves the two vertically adjacent elements (2k, j) and (2k + 1, j):
+ *              pidx = (v >> 1) * d + j
+ *              x = lo32(pidx) ^ (n * 0x9E3779B9) ^ (sr_seed * 0x85EBCA6B) ^ (hi32(pidx) * 0xC2B2AE35)
+ *              x ^= x >> 16; x *= 0x7FEB352D; x ^= x >> 15; x *= 0x846CA68B; x ^= x >> 16
+ *              r = x >> 16 for even v, x & 0xFFFF for odd v
  *            TTS_MOMENT_Q8 (8-bit block-scaled moments) is reserved: tts_ctx_create returns TTS_ERR_UNSUPPORTED.
  *
  * Preconditions: for TTS_BF16, W_in == rn_bf16(W_master) element-wise at entry; teacher_logits

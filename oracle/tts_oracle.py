@@ -292,19 +292,27 @@ def adamw_update(M, m, v, g, step, lr, beta1, beta2, eps, weight_decay):
 # f4: Adam with low-precision moment storage (R26; PAPER.md:393 names only "Adam")
 # ----------------------------------------------------------------------------
 
-def sr_bits16(idx, step, seed):
+def sr_bits16(idx, step, seed, d):
     """16 pseudo-random bits per element for stochastic rounding: a counter-based generator, so that the GPU and the
     oracle draw the same bits without exchanging them (each side implements it on its own).  Key: the element's
-    linear index idx = v * d + j (64-bit), Adam's count n of the step being taken, a caller seed.
+    position (v, j) in the [V, d] matrix (given as the linear index idx = v * d + j, 64-bit, and the row length d),
+    Adam's count n of the step being taken, a caller seed.  ONE 32-bit hash serves the two vertically adjacent
+    elements (2k, j) and (2k + 1, j) -- the even row takes its high half, the odd row its low half (R26: the
+    hash is a third of the bf16-moment kernel's instructions, and every thread of the update kernels owns such pairs):
 
-        x = lo32(idx) ^ (n * 0x9E3779B9) ^ (seed * 0x85EBCA6B) ^ (hi32(idx) * 0xC2B2AE35)        (mod 2^32)
-        x ^= x >> 16;  x *= 0x7FEB352D;  x ^= x >> 15;  x *= 0x846CA68B;  x ^= x >> 16           (an integer mixer)
-        bits = x >> 16
+        pidx = (v >> 1) * d + j                                                                     (64-bit)
+        x = lo32(pidx) ^ (n * 0x9E3779B9) ^ (seed * 0x85EBCA6B) ^ (hi32(pidx) * 0xC2B2AE35)       (mod 2^32)
+        x ^= x >> 16;  x *= 0x7FEB352D;  x ^= x >> 15;  x *= 0x846CA68B;  x ^= x >> 16            (an integer mixer)
+        bits = x >> 16 if v is even else x & 0xFFFF
     """
     idx = np.asarray(idx, dtype=np.uint64)
+    d64 = np.uint64(d)
+    v = idx // d64
+    j = idx - v * d64
+    pidx = (v >> np.uint64(1)) * d64 + j
     m32 = np.uint64(0xFFFFFFFF)
-    lo = idx & m32
-    hi = idx >> np.uint64(32)
+    lo = pidx & m32
+    hi = pidx >> np.uint64(32)
     x = lo ^ ((np.uint64(step) * np.uint64(0x9E3779B9)) & m32) ^ ((np.uint64(seed) * np.uint64(0x85EBCA6B)) & m32) \
         ^ ((hi * np.uint64(0xC2B2AE35)) & m32)
     x ^= x >> np.uint64(16)
@@ -312,7 +320,8 @@ def sr_bits16(idx, step, seed):
     x ^= x >> np.uint64(15)
     x = (x * np.uint64(0x846CA68B)) & m32
     x ^= x >> np.uint64(16)
-    return (x >> np.uint64(16)).astype(np.uint32)
+    odd = (v & np.uint64(1)).astype(bool)
+    return np.where(odd, x & np.uint64(0xFFFF), x >> np.uint64(16)).astype(np.uint32)
 
 
 def f32_to_bf16_bits_sr(x, r16):
@@ -323,13 +332,13 @@ def f32_to_bf16_bits_sr(x, r16):
     return ((u + np.asarray(r16, dtype=np.uint64)) >> np.uint64(16)).astype(np.uint16)
 
 
-def adamw_update_lowp(M, m_bits, v_bits, g, step, lr, beta1, beta2, eps, weight_decay, *, idx, seed):
+def adamw_update_lowp(M, m_bits, v_bits, g, step, lr, beta1, beta2, eps, weight_decay, *, idx, seed, d):
     """Adam (conventions of ``adamw_update``, R5) with m and v STORED as bf16 (R26):
 
       1. dequantise        m = widen(m_bits), v = widen(v_bits)                      (exact)
       2. update            M, m_new, v_new exactly as adamw_update: the parameter step uses the UNROUNDED m_new, v_new
       3. requantise        m_bits' = rn_bf16(rn_fp32(m_new))                         round to nearest even
-                           v_bits' = sr_bf16(rn_fp32(v_new), sr_bits16(idx, step, seed))   stochastic rounding:
+                           v_bits' = sr_bf16(rn_fp32(v_new), sr_bits16(idx, step, seed, d))   stochastic rounding:
                            beta2 = 0.999 decays v by 0.1% per step, below half a bf16 ulp (0.2-0.4%), so nearest
                            rounding would freeze v whenever g^2 << v; stochastic rounding keeps E[v] exact.
     The quantisation decisions are taken on the fp32 value (the precision the kernel computes in).
@@ -338,7 +347,7 @@ def adamw_update_lowp(M, m_bits, v_bits, g, step, lr, beta1, beta2, eps, weight_
     v = bf16_bits_to_f64(v_bits)
     M_new, m_new, v_new = adamw_update(M, m, v, g, step, lr, beta1, beta2, eps, weight_decay)
     m_q = f32_to_bf16_bits(m_new.astype(np.float32))
-    v_q = f32_to_bf16_bits_sr(v_new.astype(np.float32), sr_bits16(idx, step, seed))
+    v_q = f32_to_bf16_bits_sr(v_new.astype(np.float32), sr_bits16(idx, step, seed, d))
     return M_new, m_q, v_q, m_new, v_new
 
 
@@ -379,7 +388,7 @@ def distill_step(teacher_logits, h, W_in, W_master, adam_m, adam_v, pos_weight, 
         V_, d_ = M.shape
         idx = np.arange(V_, dtype=np.uint64)[:, None] * np.uint64(d_) + np.arange(d_, dtype=np.uint64)[None, :]
         M_new, m_q, v_q, m_new, v_new = adamw_update_lowp(M, adam_m, adam_v, r["gW"], step, lr, beta1, beta2, eps,
-                                                          weight_decay, idx=idx, seed=sr_seed)
+                                                          weight_decay, idx=idx, seed=sr_seed, d=d_)
     else:
         M_new, m_new, v_new = adamw_update(M, widen(adam_m), widen(adam_v), r["gW"], step,
                                            lr, beta1, beta2, eps, weight_decay)
@@ -456,7 +465,7 @@ def distill_step_rows(rows, z, lse_t, lse_z, teacher_logits, h, W_in_rows, W_mas
         d_ = M.shape[1]
         idx = np.asarray(rows, dtype=np.uint64)[:, None] * np.uint64(d_) + np.arange(d_, dtype=np.uint64)[None, :]
         M_new, m_q, v_q, m_new, v_new = adamw_update_lowp(M, adam_m_rows, adam_v_rows, gW, step, lr, beta1, beta2, eps,
-                                                          weight_decay, idx=idx, seed=sr_seed)
+                                                          weight_decay, idx=idx, seed=sr_seed, d=d_)
         out.update(m_bits=m_q, v_bits=v_q)
     else:
         M_new, m_new, v_new = adamw_update(M, widen(adam_m_rows), widen(adam_v_rows), gW, step,

@@ -27,15 +27,18 @@ __device__ __forceinline__ float adam_rcp(float x) {
   return y;
 }
 
-// 16 pseudo-random bits for element idx = v * d + j at Adam count n:
-//   x = lo32(idx) ^ (n * 0x9E3779B9) ^ (seed * 0x85EBCA6B) ^ (hi32(idx) * 0xC2B2AE35)
-//   x ^= x >> 16;  x *= 0x7FEB352D;  x ^= x >> 15;  x *= 0x846CA68B;  x ^= x >> 16;   bits = x >> 16
+// 32 pseudo-random bits for the PAIR of vertically adjacent elements (2k, j), (2k + 1, j) at Adam count n -- the even
+// row rounds with the high half, the odd row with the low half (every thread of the update kernels owns such pairs, so
+// one hash serves two elements: the hash was a third of the bf16-moment pass's instructions):
+//   pidx = (v >> 1) * d + j
+//   x = lo32(pidx) ^ (n * 0x9E3779B9) ^ (seed * 0x85EBCA6B) ^ (hi32(pidx) * 0xC2B2AE35)
+//   x ^= x >> 16;  x *= 0x7FEB352D;  x ^= x >> 15;  x *= 0x846CA68B;  x ^= x >> 16
 // `key` = (n * 0x9E3779B9) ^ (seed * 0x85EBCA6B) is formed once per thread.
 __device__ __forceinline__ uint32_t sr_key(uint32_t n, uint32_t seed) { return (n * 0x9E3779B9u) ^ (seed * 0x85EBCA6Bu); }
-__device__ __forceinline__ uint32_t sr_bits16(unsigned long long idx, uint32_t key) {
-  uint32_t x = static_cast<uint32_t>(idx) ^ key ^ (static_cast<uint32_t>(idx >> 32) * 0xC2B2AE35u);
+__device__ __forceinline__ uint32_t sr_bits32(unsigned long long pidx, uint32_t key) {
+  uint32_t x = static_cast<uint32_t>(pidx) ^ key ^ (static_cast<uint32_t>(pidx >> 32) * 0xC2B2AE35u);
   x ^= x >> 16; x *= 0x7FEB352Du; x ^= x >> 15; x *= 0x846CA68Bu; x ^= x >> 16;
-  return x >> 16;
+  return x;
 }
 // stochastic rounding: the 16 discarded bits f round away from zero iff f + r >= 65536, so E_r[result] = x
 __device__ __forceinline__ uint16_t bf16_bits_sr(float x, uint32_t r16) {

@@ -357,7 +357,10 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
         ptx::tmem_ld_wait();
         // a7 in place: the thread rewrites exactly the shared-memory words it read
 #pragma unroll
-        for (int jb = 0; jb < kJB; ++jb)
+        for (int jb = 0; jb < kJB; ++jb) {
+          // MOM: one hash for the two rows (even, odd) of this column (tts_adam.cuh)
+          const uint32_t rnd = MOM ? sr_bits32((unsigned long long)((v0 + sub * kSV) >> 1) * (unsigned long long)p.d +
+                                                   (j_stripe + jb * kMJ + jj), key) : 0u;
 #pragma unroll
           for (int v = 0; v < 2; ++v) {
             const int e = (jb >> 1) * 512 + v * 256 + (jb & 1) * 128;
@@ -368,10 +371,8 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
               const float den = adam_sqrt(v1) * inv_sqrt_bc2 + p.eps;
               M[jb][v] = fmaf(-(c1 * m1), adam_rcp(den), M[jb][v] * p.decay);     // the step uses the unrounded moments
               if (MOM) {
-                const unsigned long long idx =
-                    (unsigned long long)(v0 + sub * kSV + v) * (unsigned long long)p.d + (j_stripe + jb * kMJ + jj);
                 sLm[e] = bf16_bits_rn(m1);
-                sLv[e] = bf16_bits_sr(v1, sr_bits16(idx, key));
+                sLv[e] = bf16_bits_sr(v1, v == 0 ? rnd >> 16 : rnd & 0xFFFFu);
               } else {
                 sM[kSV * kSW + e] = m1;
                 sM[2 * kSV * kSW + e] = v1;
@@ -381,6 +382,7 @@ tc_update_gh_kernel(const __grid_constant__ CUtensorMap tm_master, const __grid_
             }
             sM[e] = M[jb][v];
           }
+        }
         if (p.gW_debug) {
 #pragma unroll
           for (int jb = 0; jb < kJB; ++jb)

@@ -417,20 +417,22 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
         }
         ptx::tmem_ld_wait();
         // a7 in place: the thread rewrites exactly the shared-memory words it read
+        uint32_t rnd = 0u;
 #pragma unroll
         for (int r = 0; r < kWSV; ++r) {
           const float gg = __uint_as_float(gr[r]) * inv_s;
           gr[r] = __float_as_uint(gg);
+          // MOM: one hash for the two rows (even, odd) of this column (tts_adam.cuh)
+          if (MOM && (r & 1) == 0)
+            rnd = sr_bits32((unsigned long long)((v0 + sub * kWSV + r) >> 1) * (unsigned long long)p.d + (j0 + jj), key);
           if (ADAM) {
             const float m1 = p.b1 * mm[r] + (1.f - p.b1) * gg;
             const float v1 = p.b2 * vv[r] + (1.f - p.b2) * gg * gg;
             const float den = adam_sqrt(v1) * inv_sqrt_bc2 + p.eps;
             M[r] = fmaf(-(c1 * m1), adam_rcp(den), M[r] * p.decay);     // the step uses the unrounded moments
             if (MOM) {
-              const unsigned long long idx =
-                  (unsigned long long)(v0 + sub * kWSV + r) * (unsigned long long)p.d + (j0 + jj);
               sLm[r * kWJ] = bf16_bits_rn(m1);
-              sLv[r * kWJ] = bf16_bits_sr(v1, sr_bits16(idx, key));
+              sLv[r * kWJ] = bf16_bits_sr(v1, (r & 1) == 0 ? rnd >> 16 : rnd & 0xFFFFu);
             } else {
               sM[kWSV * kWJ + r * kWJ] = m1;
               sM[2 * kWSV * kWJ + r * kWJ] = v1;

@@ -83,7 +83,7 @@ def test_rounding_rule_is_bit_exact_at_zero_gradient(V, d, n_seq):
         b1, b2 = float(np.float32(c["beta1"])), float(np.float32(c["beta2"]))
         idx = np.arange(V, dtype=np.uint64)[:, None] * np.uint64(d) + np.arange(d, dtype=np.uint64)[None, :]
         _, mq, vq, _, _ = O.adamw_update_lowp(O.widen(case["master"]), m_bits, v_bits, np.zeros((V, d)), 9, c["lr"], b1,
-                                              b2, c["eps"], c["weight_decay"], idx=idx, seed=12345)
+                                              b2, c["eps"], c["weight_decay"], idx=idx, seed=12345, d=d)
         np.testing.assert_array_equal(bits(m), mq)
         np.testing.assert_array_equal(bits(v), vq)
         assert (bits(v) != v_bits).mean() > 0.05          # the decay is visible: codes moved, none frozen en bloc

@@ -586,9 +586,9 @@ def test_stochastic_rounding_is_exactly_unbiased_over_all_16_bit_draws():
 def test_sr_bits_are_uniform_and_decorrelated():
     """The counter-based generator has no paper value to hit; what the method needs from it is uniform 16-bit draws that
     are independent across elements, steps and seeds."""
-    n = 1 << 20
+    n, d = 1 << 20, 1024
     idx = np.arange(n, dtype=np.uint64)
-    a = O.sr_bits16(idx, 1, 0).astype(np.float64)
+    a = O.sr_bits16(idx, 1, 0, d).astype(np.float64)
     assert a.min() >= 0 and a.max() <= 65535
     assert abs(a.mean() - 32767.5) < 4 * 18918.0 / np.sqrt(n)        # sd of U{0..65535} = 18918
     counts = np.bincount((a.astype(np.int64) >> 8), minlength=256)    # chi-square over the top byte
@@ -596,13 +596,27 @@ def test_sr_bits_are_uniform_and_decorrelated():
     assert chi2 < 255 + 6 * np.sqrt(2 * 255)
     for bit in range(16):                                             # every bit is fair
         assert abs(((a.astype(np.int64) >> bit) & 1).mean() - 0.5) < 4 * 0.5 / np.sqrt(n)
-    b = O.sr_bits16(idx, 2, 0).astype(np.float64)                     # next step, same elements
-    c = O.sr_bits16(idx, 1, 1).astype(np.float64)                     # another seed
-    d = O.sr_bits16(idx + np.uint64(1), 1, 0).astype(np.float64)      # neighbouring elements
-    e = O.sr_bits16(idx + np.uint64(1 << 32), 1, 0).astype(np.float64)  # beyond 2^32 elements: the high word counts
-    for other in (b, c, d, e):
+    b = O.sr_bits16(idx, 2, 0, d).astype(np.float64)                  # next step, same elements
+    c = O.sr_bits16(idx, 1, 1, d).astype(np.float64)                  # another seed
+    e1 = O.sr_bits16(idx + np.uint64(1), 1, 0, d).astype(np.float64)  # neighbours along the row
+    e2 = O.sr_bits16(idx + np.uint64(d), 1, 0, d).astype(np.float64)  # neighbours along the column: rows 2k and 2k + 1
+    #                                                                 # share ONE hash and take different halves of it
+    e3 = O.sr_bits16(idx + np.uint64(2 * d), 1, 0, d).astype(np.float64)   # the next pair of rows
+    e4 = O.sr_bits16(idx + np.uint64(1 << 33), 1, 0, d).astype(np.float64)  # beyond 2^32 pairs: the high word counts
+    for other in (b, c, e1, e2, e3, e4):
         assert abs(np.corrcoef(a, other)[0, 1]) < 5.0 / np.sqrt(n)
         assert (a == other).mean() < 4.0 / 65536
+    # the definition, written out once more with Python integers on a few elements (a transposed v / j or a swapped
+    # half fails here)
+    def mix(x):
+        x ^= x >> 16; x = (x * 0x7FEB352D) & 0xFFFFFFFF; x ^= x >> 15; x = (x * 0x846CA68B) & 0xFFFFFFFF; x ^= x >> 16
+        return x
+    for v, j, dd, step, seed in ((0, 0, 8, 1, 0), (1, 0, 8, 1, 0), (6, 5, 8, 3, 7), (7, 5, 8, 3, 7), (2 ** 31 + 1, 77, 4096, 9, 12345)):
+        pidx = (v >> 1) * dd + j
+        x = mix((pidx & 0xFFFFFFFF) ^ ((step * 0x9E3779B9) & 0xFFFFFFFF) ^ ((seed * 0x85EBCA6B) & 0xFFFFFFFF)
+                ^ (((pidx >> 32) * 0xC2B2AE35) & 0xFFFFFFFF))
+        want = (x & 0xFFFF) if (v & 1) else (x >> 16)
+        assert int(O.sr_bits16(np.array([v * dd + j], dtype=np.uint64), step, seed, dd)[0]) == want
 
 
 def test_lowp_adam_matches_a_scalar_loop_in_the_stated_order():
@@ -616,8 +630,8 @@ def test_lowp_adam_matches_a_scalar_loop_in_the_stated_order():
     v_bits = O.f32_to_bf16_bits((rng.standard_normal((V, d)) ** 2 * 1e-8).astype(np.float32))
     idx = np.arange(V, dtype=np.uint64)[:, None] * np.uint64(d) + np.arange(d, dtype=np.uint64)[None, :]
     lr, b1, b2, eps, wd, n, seed = 1e-3, 0.9, 0.999, 1e-8, 0.01, 4, 9
-    Mn, mq, vq, m_new, v_new = O.adamw_update_lowp(M, m_bits, v_bits, g, n, lr, b1, b2, eps, wd, idx=idx, seed=seed)
-    bits = O.sr_bits16(idx, n, seed)
+    Mn, mq, vq, m_new, v_new = O.adamw_update_lowp(M, m_bits, v_bits, g, n, lr, b1, b2, eps, wd, idx=idx, seed=seed, d=d)
+    bits = O.sr_bits16(idx, n, seed, d)
     for i in range(V):
         for j in range(d):
             m0, v0 = _bf16_val_py(int(m_bits[i, j])), _bf16_val_py(int(v_bits[i, j]))
@@ -649,7 +663,7 @@ def test_lowp_v_decays_in_expectation_where_nearest_rounding_freezes():
     g = np.zeros((1, nel))
     start = O.bf16_bits_to_f64(v_bits).mean()
     for n in range(1, steps + 1):
-        _, m_bits, v_bits, _, _ = O.adamw_update_lowp(M, m_bits, v_bits, g, n, 1e-5, 0.9, b2, 1e-8, 0.0, idx=idx, seed=3)
+        _, m_bits, v_bits, _, _ = O.adamw_update_lowp(M, m_bits, v_bits, g, n, 1e-5, 0.9, b2, 1e-8, 0.0, idx=idx, seed=3, d=nel)
         v_rne = O.f32_to_bf16_bits((b2 * O.bf16_bits_to_f64(v_rne)).astype(np.float32))
     got = O.bf16_bits_to_f64(v_bits).mean() / start
     assert got == pytest.approx(b2 ** steps, rel=5e-3)               # 0.8186
