@@ -332,6 +332,14 @@ int32_t tts_sync_step(tts_ctx* ctx);
  * The persistent draft state (W, master, m, v) stays resident on the device: device pointers.
  * The teacher logits (the bulk of the bytes: 160 MB at 512 rows) travel on a copy stream owned by the ctx while pass
  * a2, which needs only h and W_in, already runs on `stream` (tensor path); a1 and a3 wait for the copy.
+ *
+ * tts_round_host_begin / tts_round_host_end are the same round split into "enqueue" and "wait for the results": begin
+ * returns at once; the ctx has two staging slots, so a second round may be begun before the first is ended, and its
+ * teacher logits then travel while the first round's step still runs (the updates are asynchronous by design,
+ * round n + 1's verification does not wait for round n's update).  At most two rounds may be pending
+ * (else TTS_ERR_INVALID_ARG); rounds end in the order they were begun; the host buffers of a round -- inputs and
+ * outputs -- must stay untouched until its end call returns; every pending round must use the same `stream`.
+ * tts_round_host == begin + end and refuses to run while begun rounds are pending.
  */
 int32_t tts_round_host(tts_ctx* ctx,
                        const void* teacher_logits_host, /* host [T,V] logits_dtype */
@@ -345,6 +353,11 @@ int32_t tts_round_host(tts_ctx* ctx,
                        int32_t* tau_host,               /* host [T/seg_len]        */
                        uint8_t* mask_host,              /* host [T] or NULL        */
                        void* stream);
+int32_t tts_round_host_begin(tts_ctx* ctx, const void* teacher_logits_host, const void* h_host,
+                             const int32_t* draft_tokens_host, const float* pos_weight_host, int32_t T, float loss_scale,
+                             const void* W_in, void* W_out, float* W_master, void* adam_m, void* adam_v, float* gh_dev,
+                             float* loss_host, int32_t* tau_host, uint8_t* mask_host, void* stream);
+int32_t tts_round_host_end(tts_ctx* ctx);
 
 /*
  * f4.  The step sharded over the VOCABULARY across n_shards GPUs, one process per GPU.  Shard g owns

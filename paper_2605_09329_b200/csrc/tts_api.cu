@@ -34,11 +34,13 @@ void free_all(tts_ctx* c) {
   cudaFree(c->row_loss); cudaFree(c->merge_ticket);
   cudaFree(c->arg_val); cudaFree(c->arg_idx); cudaFree(c->argmax_tmp);
   cudaFree(c->acc_rows); cudaFree(c->acc_rej); cudaFree(c->acc_rpart);
-  cudaFree(c->st_teacher); cudaFree(c->st_h); cudaFree(c->st_tok); cudaFree(c->st_pw);
-  cudaFree(c->st_mask); cudaFree(c->st_tau); cudaFree(c->st_loss);
+  for (int k = 0; k < 2; ++k) {
+    tts_ctx::RoundSlot& r = c->rs[k];
+    cudaFree(r.teacher); cudaFree(r.h); cudaFree(r.tok); cudaFree(r.pw); cudaFree(r.mask); cudaFree(r.tau); cudaFree(r.loss);
+    if (r.copy_done) cudaEventDestroy(r.copy_done);
+    if (r.round_done) cudaEventDestroy(r.round_done);
+  }
   if (c->done_event) cudaEventDestroy(c->done_event);
-  if (c->copy_fork) cudaEventDestroy(c->copy_fork);
-  if (c->copy_done) cudaEventDestroy(c->copy_done);
   if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
   if (c->prof_events) {
     for (int i = 0; i < tts::kProfSlots * (TTS_NUM_PHASES + 1); ++i) cudaEventDestroy(c->prof_events[i]);
@@ -102,8 +104,6 @@ int32_t tts_ctx_create(const tts_config* cfg, int32_t device, tts_ctx** out) {
   const size_t V = cfg->V, Tm = cfg->T_max, Tp = c->T_pad_max;
   bool ok = true;
   ok = ok && cudaEventCreateWithFlags(&c->done_event, cudaEventDisableTiming) == cudaSuccess;
-  ok = ok && cudaEventCreateWithFlags(&c->copy_fork, cudaEventDisableTiming) == cudaSuccess;
-  ok = ok && cudaEventCreateWithFlags(&c->copy_done, cudaEventDisableTiming) == cudaSuccess;
   ok = ok && cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) == cudaSuccess;
   ok = ok && dmalloc(&c->step_count_dev, 1) == cudaSuccess;
   ok = ok && dmalloc(&c->step_scalars, 2) == cudaSuccess;
@@ -127,13 +127,18 @@ int32_t tts_ctx_create(const tts_config* cfg, int32_t device, tts_ctx** out) {
   ok = ok && dmalloc(&c->acc_rej, Tm / cfg->seg_len) == cudaSuccess;
   ok = ok && dmalloc(&c->acc_rpart, (Tm / cfg->seg_len) * tts::kStatSplitsMax) == cudaSuccess;
   // staging for tts_round_host
-  ok = ok && cudaMalloc(&c->st_teacher, Tm * V * elem_size(cfg->logits_dtype)) == cudaSuccess;
-  ok = ok && cudaMalloc(&c->st_h, Tm * cfg->d * elem_size(cfg->param_dtype)) == cudaSuccess;
-  ok = ok && dmalloc(&c->st_tok, Tm) == cudaSuccess;
-  ok = ok && dmalloc(&c->st_pw, Tm) == cudaSuccess;
-  ok = ok && dmalloc(&c->st_mask, Tm) == cudaSuccess;
-  ok = ok && dmalloc(&c->st_tau, Tm / cfg->seg_len) == cudaSuccess;
-  ok = ok && dmalloc(&c->st_loss, 1) == cudaSuccess;
+  for (int k = 0; k < 2; ++k) {
+    tts_ctx::RoundSlot& r = c->rs[k];
+    ok = ok && cudaMalloc(&r.teacher, Tm * V * elem_size(cfg->logits_dtype)) == cudaSuccess;
+    ok = ok && cudaMalloc(&r.h, Tm * cfg->d * elem_size(cfg->param_dtype)) == cudaSuccess;
+    ok = ok && dmalloc(&r.tok, Tm) == cudaSuccess;
+    ok = ok && dmalloc(&r.pw, Tm) == cudaSuccess;
+    ok = ok && dmalloc(&r.mask, Tm) == cudaSuccess;
+    ok = ok && dmalloc(&r.tau, Tm / cfg->seg_len) == cudaSuccess;
+    ok = ok && dmalloc(&r.loss, 1) == cudaSuccess;
+    ok = ok && cudaEventCreateWithFlags(&r.copy_done, cudaEventDisableTiming) == cudaSuccess;
+    ok = ok && cudaEventCreateWithFlags(&r.round_done, cudaEventDisableTiming) == cudaSuccess;
+  }
   // the low-precision moment formats live in the tcgen05 update kernels only
   if (ok && !c->tensor_ok && cfg->moment_dtype != TTS_MOMENT_F32) {
     free_all(c);
@@ -504,58 +509,89 @@ int32_t tts_sync_step(tts_ctx* c) {
   return e == cudaSuccess ? TTS_OK : cuda_fail(c, e);
 }
 
-int32_t tts_round_host(tts_ctx* c, const void* teacher_host, const void* h_host, const int32_t* tok_host,
-                       const float* pw_host, int32_t T, float loss_scale, const void* W_in, void* W_out,
-                       float* W_master, void* adam_m, void* adam_v, float* gh_dev, float* loss_host,
-                       int32_t* tau_host, uint8_t* mask_host, void* stream) {
+// One round through host buffers, enqueued only: inputs into staging slot (rounds begun & 1), a1 + the step on `stream`,
+// results back into the caller's host buffers, the slot's round_done event behind them.
+static int32_t round_host_enqueue(tts_ctx* c, const void* teacher_host, const void* h_host, const int32_t* tok_host,
+                                  const float* pw_host, int32_t T, float loss_scale, const void* W_in, void* W_out,
+                                  float* W_master, void* adam_m, void* adam_v, float* gh_dev, float* loss_host,
+                                  int32_t* tau_host, uint8_t* mask_host, void* stream) {
   if (!c || !teacher_host || !h_host || !tok_host || !pw_host || !loss_host || !tau_host) return TTS_ERR_INVALID_ARG;
   const tts_config& cfg = c->cfg;
   if (T <= 0 || T > cfg.T_max || T % cfg.seg_len != 0) return TTS_ERR_INVALID_ARG;
+  if (c->rh_begun - c->rh_ended >= 2) return TTS_ERR_INVALID_ARG;   // both slots are in flight: end a round first
   tts_device_guard guard(c->device);
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const size_t V = cfg.V, d = cfg.d;
+  const bool reused = c->rh_begun >= 2;
+  tts_ctx::RoundSlot& r = c->rs[c->rh_begun & 1];
   cudaError_t e;
-  // The small inputs go first on the caller's stream; the teacher logits (the bulk: 160 MB at 512 rows, ~3 ms of
-  // PCIe) are copied on the ctx's copy stream while pass a2, which needs only h and W_in, runs on the caller's stream
-  // (tensor path).  a1, a3 and the rest wait for the copy; a3 then runs as its own sweep over the finished z.
-  if ((e = cudaMemcpyAsync(c->st_h, h_host, (size_t)T * d * elem_size(cfg.param_dtype),
-                           cudaMemcpyHostToDevice, s)) != cudaSuccess) return cuda_fail(c, e);
-  if ((e = cudaMemcpyAsync(c->st_tok, tok_host, (size_t)T * 4, cudaMemcpyHostToDevice, s)) != cudaSuccess)
-    return cuda_fail(c, e);
-  if ((e = cudaMemcpyAsync(c->st_pw, pw_host, (size_t)T * 4, cudaMemcpyHostToDevice, s)) != cudaSuccess)
-    return cuda_fail(c, e);
-  if ((e = cudaEventRecord(c->copy_fork, s)) != cudaSuccess) return cuda_fail(c, e);
-  if ((e = cudaStreamWaitEvent(c->copy_stream, c->copy_fork, 0)) != cudaSuccess) return cuda_fail(c, e);
-  if ((e = cudaMemcpyAsync(c->st_teacher, teacher_host, (size_t)T * V * elem_size(cfg.logits_dtype),
+  // The teacher logits (the bulk: 160 MB at 512 rows, ~3 ms of PCIe) travel on the ctx's copy stream.  That copy waits
+  // only for the round that used this slot two rounds ago, NOT for the caller's stream: it runs under the previous
+  // round's step and under this round's pass a2, which needs only h and W_in (tensor path).  The small inputs go on
+  // the caller's stream (their slot's last readers are earlier kernels of that stream).
+  if (reused && (e = cudaStreamWaitEvent(c->copy_stream, r.round_done, 0)) != cudaSuccess) return cuda_fail(c, e);
+  if ((e = cudaMemcpyAsync(r.teacher, teacher_host, (size_t)T * V * elem_size(cfg.logits_dtype),
                            cudaMemcpyHostToDevice, c->copy_stream)) != cudaSuccess) return cuda_fail(c, e);
-  if ((e = cudaEventRecord(c->copy_done, c->copy_stream)) != cudaSuccess) return cuda_fail(c, e);
+  if ((e = cudaEventRecord(r.copy_done, c->copy_stream)) != cudaSuccess) return cuda_fail(c, e);
+  if ((e = cudaMemcpyAsync(r.h, h_host, (size_t)T * d * elem_size(cfg.param_dtype), cudaMemcpyHostToDevice, s)) !=
+      cudaSuccess)
+    return cuda_fail(c, e);
+  if ((e = cudaMemcpyAsync(r.tok, tok_host, (size_t)T * 4, cudaMemcpyHostToDevice, s)) != cudaSuccess)
+    return cuda_fail(c, e);
+  if ((e = cudaMemcpyAsync(r.pw, pw_host, (size_t)T * 4, cudaMemcpyHostToDevice, s)) != cudaSuccess)
+    return cuda_fail(c, e);
   int early_launches = 0;
   tts_step_extras ex;
   ex.draft_logits = nullptr; ex.draft_logits_out = nullptr; ex.ref_logits = nullptr; ex.lambda = 0.f;
   if (c->tensor_ok && aligned16(W_in)) {
     tts::StepArgs a0;
     memset(&a0, 0, sizeof(a0));
-    a0.h = c->st_h; a0.W_in = W_in; a0.T = T;
+    a0.h = r.h; a0.W_in = W_in; a0.T = T;
     if ((e = tts::tc_logits_only(c, a0, s, &early_launches)) != cudaSuccess) return cuda_fail(c, e);
     ex.draft_logits = c->z;                          // the step below takes z as given: a2 is done
   }
-  if ((e = cudaStreamWaitEvent(s, c->copy_done, 0)) != cudaSuccess) return cuda_fail(c, e);
-  int32_t st = tts_accept_mask(c, c->st_teacher, c->st_tok, T, c->st_mask, c->st_tau, nullptr, stream);
+  if ((e = cudaStreamWaitEvent(s, r.copy_done, 0)) != cudaSuccess) return cuda_fail(c, e);
+  int32_t st = tts_accept_mask(c, r.teacher, r.tok, T, r.mask, r.tau, nullptr, stream);
   if (st != TTS_OK) return st;
   const int mask_launches = c->last_launches;
-  st = tts_distill_step_ex(c, c->st_teacher, c->st_h, W_in, W_out, W_master, adam_m, adam_v, c->st_pw, c->st_mask, T,
-                           loss_scale, c->st_loss, nullptr, gh_dev, nullptr, &ex, stream);
+  st = tts_distill_step_ex(c, r.teacher, r.h, W_in, W_out, W_master, adam_m, adam_v, r.pw, r.mask, T, loss_scale, r.loss,
+                           nullptr, gh_dev, nullptr, &ex, stream);
   if (st != TTS_OK) return st;
   c->last_launches += mask_launches + early_launches;
-  if ((e = cudaMemcpyAsync(loss_host, c->st_loss, 4, cudaMemcpyDeviceToHost, s)) != cudaSuccess) return cuda_fail(c, e);
-  if ((e = cudaMemcpyAsync(tau_host, c->st_tau, (size_t)(T / cfg.seg_len) * 4, cudaMemcpyDeviceToHost, s)) !=
-      cudaSuccess)
+  if ((e = cudaMemcpyAsync(loss_host, r.loss, 4, cudaMemcpyDeviceToHost, s)) != cudaSuccess) return cuda_fail(c, e);
+  if ((e = cudaMemcpyAsync(tau_host, r.tau, (size_t)(T / cfg.seg_len) * 4, cudaMemcpyDeviceToHost, s)) != cudaSuccess)
     return cuda_fail(c, e);
-  if (mask_host &&
-      (e = cudaMemcpyAsync(mask_host, c->st_mask, (size_t)T, cudaMemcpyDeviceToHost, s)) != cudaSuccess)
+  if (mask_host && (e = cudaMemcpyAsync(mask_host, r.mask, (size_t)T, cudaMemcpyDeviceToHost, s)) != cudaSuccess)
     return cuda_fail(c, e);
-  if ((e = cudaStreamSynchronize(s)) != cudaSuccess) return cuda_fail(c, e);
+  if ((e = cudaEventRecord(r.round_done, s)) != cudaSuccess) return cuda_fail(c, e);
+  ++c->rh_begun;
   return TTS_OK;
+}
+
+int32_t tts_round_host_begin(tts_ctx* c, const void* teacher_host, const void* h_host, const int32_t* tok_host,
+                             const float* pw_host, int32_t T, float loss_scale, const void* W_in, void* W_out,
+                             float* W_master, void* adam_m, void* adam_v, float* gh_dev, float* loss_host,
+                             int32_t* tau_host, uint8_t* mask_host, void* stream) {
+  return round_host_enqueue(c, teacher_host, h_host, tok_host, pw_host, T, loss_scale, W_in, W_out, W_master, adam_m,
+                            adam_v, gh_dev, loss_host, tau_host, mask_host, stream);
+}
+
+int32_t tts_round_host_end(tts_ctx* c) {
+  if (!c || c->rh_begun == c->rh_ended) return TTS_ERR_INVALID_ARG;
+  tts_device_guard guard(c->device);
+  const cudaError_t e = cudaEventSynchronize(c->rs[c->rh_ended & 1].round_done);
+  ++c->rh_ended;
+  return e == cudaSuccess ? TTS_OK : cuda_fail(c, e);
+}
+
+int32_t tts_round_host(tts_ctx* c, const void* teacher_host, const void* h_host, const int32_t* tok_host,
+                       const float* pw_host, int32_t T, float loss_scale, const void* W_in, void* W_out,
+                       float* W_master, void* adam_m, void* adam_v, float* gh_dev, float* loss_host,
+                       int32_t* tau_host, uint8_t* mask_host, void* stream) {
+  if (c && c->rh_begun != c->rh_ended) return TTS_ERR_INVALID_ARG;   // rounds begun with tts_round_host_begin are pending
+  const int32_t st = round_host_enqueue(c, teacher_host, h_host, tok_host, pw_host, T, loss_scale, W_in, W_out,
+                                        W_master, adam_m, adam_v, gh_dev, loss_host, tau_host, mask_host, stream);
+  return st != TTS_OK ? st : tts_round_host_end(c);
 }
 
 }  // extern "C"

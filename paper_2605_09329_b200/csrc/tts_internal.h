@@ -99,16 +99,21 @@ struct tts_ctx {
   float* acc_rows;        // [T_max, 2] lse_t, lse_z of tts_accept_stochastic
   int32_t* acc_rej;       // [T_max / seg_len] first rejected row per sequence
   double* acc_rpart;      // [T_max / seg_len, kStatSplitsMax] residual mass per slice
-  // ---- staging for tts_round_host ----
-  void* st_teacher;
-  void* st_h;
-  int32_t* st_tok;
-  float* st_pw;
-  uint8_t* st_mask;
-  int32_t* st_tau;
-  float* st_loss;
-  cudaStream_t copy_stream;   // tts_round_host: the teacher's H2D copy runs here, next to a2 on the caller's stream
-  cudaEvent_t copy_fork, copy_done;
+  // ---- staging for tts_round_host / tts_round_host_begin: two slots, so that the next round's inputs can travel while
+  // this round's step runs ----
+  struct RoundSlot {
+    void* teacher;
+    void* h;
+    int32_t* tok;
+    float* pw;
+    uint8_t* mask;
+    int32_t* tau;
+    float* loss;
+    cudaEvent_t copy_done;    // the teacher's H2D copy into this slot has landed
+    cudaEvent_t round_done;   // the round that used this slot has finished (results copied back): the slot is free
+  } rs[2];
+  unsigned rh_begun, rh_ended;  // rounds begun / ended through the host API (slot = count & 1; at most 2 outstanding)
+  cudaStream_t copy_stream;   // the teacher's H2D copy runs here, next to a2 (and the previous round) on the caller's stream
   // ---- per-phase profiling (tts_profile_*) ----
   bool prof_on;
   int prof_count;                                   // steps recorded since the last read

@@ -69,6 +69,8 @@ EXPORTS = {
     "tts_sync_step": (C.c_int32, [C.c_void_p]),
     "tts_record_done": (C.c_int32, [C.c_void_p, C.c_void_p]),
     "tts_round_host": (C.c_int32, [C.c_void_p] * 5 + [C.c_int32, C.c_float] + [C.c_void_p] * 10),
+    "tts_round_host_begin": (C.c_int32, [C.c_void_p] * 5 + [C.c_int32, C.c_float] + [C.c_void_p] * 10),
+    "tts_round_host_end": (C.c_int32, [C.c_void_p]),
     "tts_shard_begin_step": (C.c_int32, [C.c_void_p] * 4 + [C.c_int32] + [C.c_void_p] * 3),
     "tts_shard_finish_step": (C.c_int32, [C.c_void_p] * 2 + [C.c_int32] + [C.c_void_p] * 9 + [C.c_int32, C.c_float] +
                               [C.c_void_p] * 6),
@@ -276,6 +278,19 @@ def tts_round_host(ctx, teacher_logits_host, h_host, draft_tokens_host, pos_weig
                               _ptr(adam_m), _ptr(adam_v), _ptr(gh_dev), _ptr(loss_host), _ptr(tau_host),
                               _ptr(mask_host), _stream(stream, ctx))
     _check(ctx, st, "tts_round_host")
+
+
+def tts_round_host_begin(ctx, teacher_logits_host, h_host, draft_tokens_host, pos_weight_host, T, loss_scale, W_in,
+                         W_out, W_master, adam_m, adam_v, gh_dev, loss_host, tau_host, mask_host=None, stream=None):
+    st = lib().tts_round_host_begin(ctx, _ptr(teacher_logits_host), _ptr(h_host), _ptr(draft_tokens_host),
+                                    _ptr(pos_weight_host), T, loss_scale, _ptr(W_in), _ptr(W_out), _ptr(W_master),
+                                    _ptr(adam_m), _ptr(adam_v), _ptr(gh_dev), _ptr(loss_host), _ptr(tau_host),
+                                    _ptr(mask_host), _stream(stream, ctx))
+    _check(ctx, st, "tts_round_host_begin")
+
+
+def tts_round_host_end(ctx):
+    _check(ctx, lib().tts_round_host_end(ctx), "tts_round_host_end")
 
 
 def _extras(draft_logits, draft_logits_out, ref_logits, lam):

@@ -235,3 +235,71 @@ def test_a_stalled_pipeline_traps_instead_of_hanging():
     case = synth.make_case(3, V=2048, d=256)
     g, o = run_gpu(case), run_oracle(case)
     check_step(g, o, case)
+
+
+@pytest.mark.parametrize("V,d,n_seq", [(4096, 1024, 1), (2048 + 128, 256, 32)])
+def test_pipelined_host_rounds_equal_serial_host_rounds(V, d, n_seq):
+    """tts_round_host_begin / _end with two rounds in flight (the next round's teacher logits travel under this round's
+    step) give the rounds of tts_round_host bit for bit: per-round loss, tau and mask, and the final
+    master / m / v / working copy.  Also: a third pending round and a plain tts_round_host next to pending rounds are
+    refused."""
+    n_rounds = 5
+    cases = [synth.make_case(4 if n_seq > 1 else 3, V=V, d=d, n_seq=n_seq, seed=900 + r) for r in range(n_rounds)]
+    c0 = cases[0]
+    T, C = c0["T"], c0["seg_len"]
+    host = []
+    for c in cases:
+        host.append(dict(teacher=torch.from_numpy(c["teacher"].view(np.int16)).pin_memory(),
+                         h=torch.from_numpy(c["h"].view(np.int16)).pin_memory(),
+                         tok=torch.from_numpy(c["draft_tokens"]).pin_memory(),
+                         pw=torch.from_numpy(c["pos_weight"]).pin_memory()))
+
+    def run(pipelined):
+        ctx = tts.tts_ctx_create(config_for(c0), 0)
+        try:
+            W = [_dev(c0["W"]), torch.empty_like(_dev(c0["W"]))]
+            master, m, v = _dev(c0["master"]), _dev(c0["m"]), _dev(c0["v"])
+            out = [dict(loss=torch.zeros(1).pin_memory(), tau=torch.zeros(T // C, dtype=torch.int32).pin_memory(),
+                        mask=torch.zeros(T, dtype=torch.uint8).pin_memory()) for _ in range(n_rounds)]
+            side = torch.cuda.Stream()
+
+            def args(r):
+                hb, ob = host[r], out[r]
+                return (ctx, hb["teacher"], hb["h"], hb["tok"], hb["pw"], T, c0["loss_scale"], W[r & 1], W[1 - (r & 1)],
+                        master, m, v, None, ob["loss"], ob["tau"], ob["mask"], side)
+
+            if not pipelined:
+                for r in range(n_rounds):
+                    tts.tts_round_host(*args(r))
+            else:
+                tts.tts_round_host_begin(*args(0))
+                for r in range(1, n_rounds):
+                    tts.tts_round_host_begin(*args(r))
+                    if r == 1:
+                        with pytest.raises(tts.TTSError):          # both slots are in flight
+                            tts.tts_round_host_begin(*args(2))
+                        with pytest.raises(tts.TTSError):          # the synchronous form next to pending rounds
+                            tts.tts_round_host(*args(2))
+                    tts.tts_round_host_end(ctx)
+                tts.tts_round_host_end(ctx)
+                with pytest.raises(tts.TTSError):                  # nothing pending
+                    tts.tts_round_host_end(ctx)
+            torch.cuda.synchronize()
+            res = dict(loss=[float(o["loss"][0]) for o in out], tau=[o["tau"].numpy().copy() for o in out],
+                       mask=[o["mask"].numpy().copy() for o in out], master=master.cpu().numpy(),
+                       m=m.cpu().numpy(), v=v.cpu().numpy(), W=W[n_rounds & 1].cpu().view(torch.int16).numpy())
+            return res
+        finally:
+            tts.tts_ctx_destroy(ctx)
+
+    a, b = run(False), run(True)
+    assert a["loss"] == b["loss"] and all(np.isfinite(a["loss"])) and len(set(a["loss"])) == n_rounds
+    for r in range(n_rounds):
+        np.testing.assert_array_equal(a["tau"][r], b["tau"][r])
+        np.testing.assert_array_equal(a["mask"][r], b["mask"][r])
+    for k in ("master", "m", "v", "W"):
+        np.testing.assert_array_equal(a[k], b[k])
+    # and the first round is the oracle's
+    o = run_oracle(cases[0])
+    assert abs(a["loss"][0] - o["loss"]) <= 1e-3 * abs(o["loss"]) + 1e-6
+    np.testing.assert_array_equal(a["tau"][0], o["tau"])
