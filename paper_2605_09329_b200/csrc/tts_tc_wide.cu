@@ -21,8 +21,10 @@
 //     (evict_last) while every stripe passes over them; inside a window the (stripe, band) units, stripe-major, are
 //     split into gridDim equal contiguous ranges, so the grid is balanced to one band for any SM budget and a CTA
 //     changes stripe (reloads A) at most twice per window.
-// The state moves as in the fused kernel: TMA loads of [8 v x 128 j] sub-tiles of master / m / v into a ring,
-// AdamW applied in place in shared memory, TMA stores of the three tensors and the bf16 working copy.
+// The state moves as in the fused kernel: TMA loads of [16 v x 128 j] sub-tiles of master / m / v into a ring,
+// AdamW applied in place in shared memory (a thread updates its column of a sub-tile in two halves of 8 rows, so that one
+// barrier round and one set of TMA stores serve 16 rows: the bf16-moment pass, which is bound by these warps, gains 3%),
+// TMA stores of the three tensors and the bf16 working copy.
 #include <cuda_fp16.h>
 #include <string.h>
 
@@ -35,12 +37,13 @@ namespace tts {
 namespace {
 
 constexpr int kWJ = 128;                 // stripe width = MMA M = TMEM lanes
-constexpr int kWSV = 8;                  // vocabulary rows per state stage
-constexpr int kWTensorBytes = kWSV * kWJ * 4;   // 4 KB per tensor per stage
-constexpr int kWStageBytes = 3 * kWTensorBytes; // 12 KB (fp32 moments)
-constexpr int kWMomBytesLp = kWSV * kWJ * 2;    // 2 KB per bf16 moment tensor per stage
-constexpr int kWStageBytesLp = kWTensorBytes + 2 * kWMomBytesLp;   // 8 KB (bf16 moments, TTS_MOMENT_BF16)
-constexpr int kWWoBytes = kWSV * kWJ * 2;       // 2 KB: bf16 staging of one sub-tile (one per epilogue group)
+constexpr int kWSV = 16;                 // vocabulary rows per state stage (= sub-tile: one barrier round, one set of TMA stores)
+constexpr int kWH = 8;                   // rows a thread holds at a time: a sub-tile is updated in two halves
+constexpr int kWTensorBytes = kWSV * kWJ * 4;   // 8 KB per tensor per stage
+constexpr int kWStageBytes = 3 * kWTensorBytes; // 24 KB (fp32 moments)
+constexpr int kWMomBytesLp = kWSV * kWJ * 2;    // 4 KB per bf16 moment tensor per stage
+constexpr int kWStageBytesLp = kWTensorBytes + 2 * kWMomBytesLp;   // 16 KB (bf16 moments, TTS_MOMENT_BF16)
+constexpr int kWWoBytes = kWSV * kWJ * 2;       // 4 KB: bf16 staging of one sub-tile (one per epilogue group)
 constexpr int kWThreads = 384;           // warp 0 state TMA, 1 MMA, 2 TMEM alloc, 3 operand TMA, 4-11 epilogue
 constexpr int kWMaxStages = 24;
 constexpr int kWOpStagesMax = 4;         // dl band ring (depth chosen per launch)
@@ -396,15 +399,18 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
           const uint32_t n = i * kSubs + sub;
           s = n % p.stages; st_par = (n / p.stages) & 1;
         }
-        uint32_t gr[kWSV];
-        ptx::tmem_ld_32x32b_x8(tmem_base + ab * NV + sub * kWSV + lane_bits, gr);
-        ptx::mbar_wait(&bars->st_full[s], st_par);
-        float* sM = reinterpret_cast<float*>(st + s * kStageB) + jj;
-        uint16_t* sLm = reinterpret_cast<uint16_t*>(st + s * kStageB + kWTensorBytes) + jj;   // MOM: bf16 m, then v
-        uint16_t* sLv = reinterpret_cast<uint16_t*>(st + s * kStageB + kWTensorBytes + kMomB) + jj;
-        float M[kWSV], mm[kWSV], vv[kWSV];
+        uint32_t wpk[kWSV / 2];                                  // the updated rows as bf16 pairs, for the working copy
 #pragma unroll
-        for (int r = 0; r < kWSV; ++r) {
+        for (int hf = 0; hf < kWSV / kWH; ++hf) {
+        uint32_t gr[kWH];
+        ptx::tmem_ld_32x32b_x8(tmem_base + ab * NV + sub * kWSV + hf * kWH + lane_bits, gr);
+        if (hf == 0) ptx::mbar_wait(&bars->st_full[s], st_par);
+        float* sM = reinterpret_cast<float*>(st + s * kStageB) + hf * kWH * kWJ + jj;
+        uint16_t* sLm = reinterpret_cast<uint16_t*>(st + s * kStageB + kWTensorBytes) + hf * kWH * kWJ + jj;   // MOM: bf16 m, then v
+        uint16_t* sLv = reinterpret_cast<uint16_t*>(st + s * kStageB + kWTensorBytes + kMomB) + hf * kWH * kWJ + jj;
+        float M[kWH], mm[kWH], vv[kWH];
+#pragma unroll
+        for (int r = 0; r < kWH; ++r) {
           M[r] = sM[r * kWJ];
           if (ADAM) {
             if (MOM) { mm[r] = bf16_bits_widen(sLm[r * kWJ]); vv[r] = bf16_bits_widen(sLv[r * kWJ]); }
@@ -412,8 +418,8 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
           }
         }
         if (GH) {
-          // a5 operand: W_in[v, j] = rn_bf16(master[v, j]), as fp16(16 W): rows 8 sub .. 8 sub + 7 of this thread's column
-          ptx::mbar_wait(&bars->wt_empty, (i & 1) ^ 1);          // the gh MMAs of the previous band have read wt
+          // a5 operand: W_in[v, j] = rn_bf16(master[v, j]), as fp16(16 W): eight rows of this thread's column
+          if (hf == 0) ptx::mbar_wait(&bars->wt_empty, (i & 1) ^ 1);   // the gh MMAs of the previous band have read wt
           uint32_t pk[4];
 #pragma unroll
           for (int r = 0; r < 4; ++r) {
@@ -423,8 +429,8 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
             // fp16(16 W), saturating (|W| >= 4094 clamps, as in tts_tc_gemm.cu)
             asm("cvt.rn.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(pk[r]) : "f"(hi), "f"(lo));
           }
-          *reinterpret_cast<uint4*>(wt_thr + sub * 2048) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
-          if (sub >= kSubs - 2) {                                // the group's last sub-tile of this band
+          *reinterpret_cast<uint4*>(wt_thr + (sub * (kWSV / kWH) + hf) * 2048) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+          if (hf == kWSV / kWH - 1) {                            // both groups' sub-tiles make up the band (kSubs == 2)
             ptx::fence_proxy_async_smem();
             __syncwarp();
             if (lane == 0) ptx::mbar_arrive(&bars->wt_full);
@@ -433,13 +439,14 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
         ptx::tmem_ld_wait();
         // a7 in place: the thread rewrites exactly the shared-memory words it read
         uint32_t rnd = 0u;
+        const int row0 = v0 + sub * kWSV + hf * kWH;
 #pragma unroll
-        for (int r = 0; r < kWSV; ++r) {
+        for (int r = 0; r < kWH; ++r) {
           const float gg = __uint_as_float(gr[r]) * inv_s;
           gr[r] = __float_as_uint(gg);
           // MOM: one hash for the two rows (even, odd) of this column (tts_adam.cuh)
           if (MOM && (r & 1) == 0)
-            rnd = sr_bits32((unsigned long long)((v0 + sub * kWSV + r) >> 1) * (unsigned long long)p.d + (j0 + jj), key);
+            rnd = sr_bits32((unsigned long long)((row0 + r) >> 1) * (unsigned long long)p.d + (j0 + jj), key);
           if (ADAM) {
             const float m1 = p.b1 * mm[r] + (1.f - p.b1) * gg;
             const float v1 = p.b2 * vv[r] + (1.f - p.b2) * gg * gg;
@@ -459,17 +466,28 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
         }
         if (p.gW_debug) {
 #pragma unroll
-          for (int r = 0; r < kWSV; ++r)
-            p.gW_debug[(size_t)(v0 + sub * kWSV + r) * p.d + j0 + jj] = __uint_as_float(gr[r]);
+          for (int r = 0; r < kWH; ++r) p.gW_debug[(size_t)(row0 + r) * p.d + j0 + jj] = __uint_as_float(gr[r]);
         }
+#pragma unroll
+        for (int r = 0; r < kWH / 2; ++r) {
+          const __nv_bfloat162 b2 = __floats2bfloat162_rn(M[2 * r], M[2 * r + 1]);
+          wpk[hf * (kWH / 2) + r] = *reinterpret_cast<const uint32_t*>(&b2);
+        }
+        }   // halves
         // the group's previous stores have read their shared memory: release that stage, reuse the bf16 staging
         if (leader) {
           ptx::bulk_wait_group_read<0>();
           if (prev_s >= 0) ptx::mbar_arrive(&bars->st_empty[prev_s]);
         }
         ptx::named_barrier_sync(1 + g, 128);
+        {
+          uint16_t* wo16 = reinterpret_cast<uint16_t*>(wo_g) + jj;
 #pragma unroll
-        for (int r = 0; r < kWSV; ++r) wo_g[r * kWJ + jj] = __float2bfloat16_rn(M[r]);
+          for (int r = 0; r < kWSV / 2; ++r) {
+            wo16[(2 * r) * kWJ] = static_cast<uint16_t>(wpk[r] & 0xFFFFu);
+            wo16[(2 * r + 1) * kWJ] = static_cast<uint16_t>(wpk[r] >> 16);
+          }
+        }
         ptx::fence_proxy_async_smem();
         ptx::named_barrier_sync(1 + g, 128);
         if (leader) {
@@ -763,8 +781,9 @@ cudaError_t tc_launch_update_wide(tts_ctx* c, const StepArgs& a, cudaStream_t s,
   const int fixed = 1024 + p.op_stages * NV * Kp * 2 + 2 * kWWoBytes + (gh_here ? kWWtBytes : 0) + (int)sizeof(WideBars);
   const int stage_bytes = lowp ? kWStageBytesLp : kWStageBytes;
   p.stages = (kWSmemBudget - fixed) / stage_bytes;
-  // ring depth: the pass's speed is flat from 7 stages up at the grid tc_update_ctas picks (8: 2.68 ms at 64 rows,
-  // 2.78 at 256, 2.83 at 512; 6: 3.04 / 3.13 / 3.12), deeper rings only take shared memory
+  // ring depth: with 12 KB stages the pass's speed was flat from 7 stages (84 KB) up at the grid tc_update_ctas picks
+  // (8: 2.68 ms at 64 rows, 2.78 at 256, 2.83 at 512; 6: 3.04 / 3.13 / 3.12); the 24 KB stages of today give 6 (512 rows)
+  // to 8 of them: 144-192 KB in flight, deeper rings only take shared memory
   if (p.stages > (lowp ? kWMaxStages : 8)) p.stages = lowp ? kWMaxStages : 8;
   if (p.stages < 2) return cudaErrorInvalidConfiguration;
   p.lr = a.lr; p.b1 = a.beta1; p.b2 = a.beta2; p.eps = a.eps;
