@@ -17,7 +17,10 @@
 //     2^-28 max|h| lose bits).  The epilogue multiplies the accumulator by 1 / (S S_h) (exact);
 //   * per band of NV vocabulary rows the only operand traffic is the band's dl rows [NV x Kp] (8 B per parameter
 //     at T = 512 against 26 B of state);
-//   * work is cut as windowed stream-K: the vocabulary is cut into windows whose dl rows (<= 12 MB) stay in L2
+//   * work is cut in one of two ways (tc_launch_update_wide): a FIXED-STRIPE walk when the grid is (nearly) a multiple of
+//     the stripe count -- every CTA keeps one stripe for the whole pass and takes every (grid / n_stripes)-th band, so
+//     the CTAs of a phase sweep the same vocabulary rows and their 512-byte row segments add up to whole rows at the
+//     memory controllers --, else windowed stream-K: the vocabulary is cut into windows whose dl rows (<= 12 MB) stay in L2
 //     (evict_last) while every stripe passes over them; inside a window the (stripe, band) units, stripe-major, are
 //     split into gridDim equal contiguous ranges, so the grid is balanced to one band for any SM budget and a CTA
 //     changes stripe (reloads A) at most twice per window.
@@ -155,8 +158,8 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
   const int b_bytes = NV * p.Kp * 2;                   // [Kp / 64][NV v][64 k] fp16, 128-byte swizzle
   uint8_t* sB = smem;
   const int kWOpStages = p.op_stages;
-  uint8_t* st = sB + kWOpStages * b_bytes;             // [stages][3][8 v][128 j] fp32
-  uint8_t* wo = st + p.stages * kStageB;               // [2 groups][8 v][128 j] bf16
+  uint8_t* st = sB + kWOpStages * b_bytes;             // [stages][3][16 v][128 j] fp32
+  uint8_t* wo = st + p.stages * kStageB;               // [2 groups][16 v][128 j] bf16
   uint8_t* wt = wo + 2 * kWWoBytes;                    // GH: [4 v-groups][16 j-groups][8 j][8 v] fp16, K-major core matrices
   WideBars* bars = reinterpret_cast<WideBars*>(wt + (GH ? kWWtBytes : 0));
 
@@ -194,7 +197,7 @@ tc_update_wide_kernel(const __grid_constant__ CUtensorMap tm_dlT,
   const uint32_t tmem_A = tmem_base + kWAccCols;       // Kp / 2 columns: h^T of the stripe, K packed in pairs
 
   if (warp == 0) {
-    // ===== optimiser-state producer: [8 v x 128 j] of master / m / v per stage =====
+    // ===== optimiser-state producer: [16 v x 128 j] of master / m / v per stage =====
     if (lane == 0) {
       const uint64_t pol = ptx::policy_evict_first();
       WideWalk w(p);
