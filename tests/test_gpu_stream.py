@@ -139,6 +139,26 @@ def test_300_round_stream_drift_stays_bounded(d):
         print("max |M_gpu - M_ref| / lr at updates", worst)
     finally:
         up.close()
+    # SURVEY 8(d), end-of-stream invariant: the adapted head sits closer to the drifting teacher than a frozen one.  The
+    # same rounds once more with lr = 0 (every kernel runs, nothing moves): paired round by round, the frozen head's loss
+    # is the higher one over the last 100 rounds, and by a growing margin.
+    W0, master, m, v = _dev(case0["W"]), _dev(case0["master"]), _dev(case0["m"]), _dev(case0["v"])
+    frozen = DraftHeadUpdater(W0, master, m, v, seg_len=16, T_max=16, stride=1, lr=0.0, beta1=c["beta1"], beta2=c["beta2"],
+                              eps=c["eps"], weight_decay=c["weight_decay"])
+    try:
+        gain = []
+        for t, r in enumerate(rounds):
+            rd = (_dev(r["teacher"]), _dev(r["h"]), _dev(r["draft_tokens"]))
+            frozen.on_round_end(rd[0], rd[1], rd[2], pw, 16)
+            tts.tts_sync_step(frozen.ctx)
+            gain.append(float(frozen.loss.item()) - o["losses"][t])
+        np.testing.assert_array_equal(master.cpu().numpy(), case0["master"])          # lr = 0: nothing moved
+        gain = np.array(gain)
+        assert abs(gain[0]) <= 1e-3 * abs(o["losses"][0]) + 1e-6                        # round 0: the same head
+        assert gain[-100:].mean() > 0 and gain[-100:].mean() > gain[:100].mean()
+        print("loss(frozen) - loss(adapted): first 100 rounds %.4g, last 100 rounds %.4g" % (gain[:100].mean(), gain[-100:].mean()))
+    finally:
+        frozen.close()
 
 
 @pytest.mark.parametrize("n_seq,d", [(32, 256), (4, 256), (1, 1024)])
