@@ -172,6 +172,42 @@ int32_t tts_accept_mask(tts_ctx* ctx,
                         void* stream);
 
 /*
+ * a1 without a ctx and without any allocation.  Same operation, same readings and same outputs as tts_accept_mask
+ * (R8, R9, R11), for callers that cannot allocate device memory when they need the mask: a
+ * serving process whose own pool already holds the whole GPU, code inside a region where cudaMalloc is off limits
+ * because it synchronises the device and would stall the decode stream, or an embedder that routes every GPU byte
+ * through its own allocator.  Such a caller cannot use tts_ctx_create (it cudaMallocs the ctx's scratch), so this call
+ * takes the shapes directly and keeps the per-(row, slice) argmax candidates in a fixed array of
+ * TTS_STATIC_SCRATCH_BYTES that is part of the library image: every GPU on which the library's code is loaded holds
+ * one copy until the process exits, whether or not this call is ever made.
+ *   limits     T <= TTS_STATIC_T_MAX; a larger T returns TTS_ERR_INVALID_ARG and enqueues nothing.  V <= 2^30, rows
+ *              16-byte aligned (V % 8 == 0 for bf16, V % 4 == 0 for fp32), T % seg_len == 0, as tts_accept_mask.
+ *   device     the calling thread's CURRENT device; `stream` and every pointer must belong to it (device pointers).
+ *   first call on each device also resolves the array's address on that device (cudaGetSymbolAddress, under a lock)
+ *              and reads two device attributes; make that first call outside any stream capture.  Later calls only
+ *              launch two kernels on `stream`.  No call here uses cudaMalloc, cudaFree or an allocating library routine.
+ *   sharing    all calls on one device use the same array.  Nothing in it has to start at zero (each call writes every
+ *              slot it later reads), and it keeps the last call's candidates afterwards.  Two calls whose kernels can
+ *              run at the same time on one GPU (different streams without an ordering between them, or two host
+ *              threads) race on it and may both return wrong masks: order them, e.g. keep them on one stream.
+ *   errors     INVALID_ARG (NULL, sizes, T over the limit, misaligned teacher), UNSUPPORTED (dtype, row alignment,
+ *              device ordinal >= 64), ARCH (current device is not sm_10x), CUDA (code in tts_static_last_cuda_error).
+ */
+#define TTS_STATIC_T_MAX 512
+#define TTS_STATIC_SCRATCH_BYTES 264192 /* 512 rows x 64 slices x (fp32 value + int32 index) + 512 x int32 */
+int32_t tts_accept_mask_static(const void* teacher_logits,  /* [T,V] logits_dtype, device                      */
+                               int32_t logits_dtype,        /* TTS_BF16 | TTS_F32                              */
+                               int32_t V, int32_t seg_len,
+                               const int32_t* draft_tokens, /* [T]                                             */
+                               int32_t T,                   /* multiple of seg_len, 1..TTS_STATIC_T_MAX        */
+                               uint8_t* mask_out,           /* [T]                                             */
+                               int32_t* tau_out,            /* [T/seg_len]                                     */
+                               int32_t* teacher_argmax_out, /* [T] or NULL                                     */
+                               void* stream);
+/* cudaError_t (as int) of the last failed CUDA call that tts_accept_mask_static made on the calling thread, 0 if none */
+int32_t tts_static_last_cuda_error(void);
+
+/*
  * f2.  The paper's own accept rule, "standard speculative rejection sampling" (Alg. 1):
  * canvas tokens are considered left to right, x_{t+k} is accepted with probability min{1, p(x_{t+k}) / q(x_{t+k})},
  * and the loop breaks at the first rejection.  p = softmax(teacher_logits[r]), q =

@@ -17,8 +17,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libtts_b200.so")
-SOURCES = ["tts_api.cu", "tts_mask.cu", "tts_accept.cu", "tts_stats.cu", "tts_simt.cu", "tts_check.cu", "tts_tc.cu",
-           "tts_tc_gemm.cu", "tts_tc_fused.cu", "tts_tc_wide.cu", "tts_tc_pair.cu"]
+SOURCES = ["tts_api.cu", "tts_mask.cu", "tts_static.cu", "tts_accept.cu", "tts_stats.cu", "tts_simt.cu", "tts_check.cu",
+           "tts_tc.cu", "tts_tc_gemm.cu", "tts_tc_fused.cu", "tts_tc_wide.cu", "tts_tc_pair.cu"]
 HEADERS = ["tts_internal.h", "tts_common.cuh", "tts_tc_ptx.cuh", "tts_tc_state.h", "tts_adam.cuh", "tts_tc_epi.cuh",
            os.path.join("..", "..", "include", "tts.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC",

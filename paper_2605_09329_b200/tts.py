@@ -23,6 +23,7 @@ TTS_FLAG_CHECK_PRECONDITIONS, TTS_FLAG_DETERMINISTIC, TTS_FLAG_SEPARATE_GH = 1, 
 TTS_DEV_W_MISMATCH, TTS_DEV_NONFINITE_TEACHER, TTS_DEV_NONFINITE_H, TTS_DEV_BAD_TOKEN, TTS_DEV_NONFINITE_LOSS = 1, 2, 4, 8, 16
 TTS_NUM_PHASES = 5
 TTS_SHARD_STAT_FIELDS = 8
+TTS_STATIC_T_MAX, TTS_STATIC_SCRATCH_BYTES = 512, 264192
 PHASE_NAMES = ("a2_logits", "a3_row_stats", "a4_dlogits", "a5_gh", "a6a7_gW_update")
 
 
@@ -58,6 +59,8 @@ EXPORTS = {
     "tts_last_step_used_tensor_path": (C.c_int32, [C.c_void_p]),
     "tts_last_launch_count": (C.c_int32, [C.c_void_p]),
     "tts_accept_mask": (C.c_int32, [C.c_void_p] * 3 + [C.c_int32] + [C.c_void_p] * 4),
+    "tts_accept_mask_static": (C.c_int32, [C.c_void_p] + [C.c_int32] * 3 + [C.c_void_p, C.c_int32] + [C.c_void_p] * 4),
+    "tts_static_last_cuda_error": (C.c_int32, []),
     "tts_accept_stochastic": (C.c_int32, [C.c_void_p] * 6 + [C.c_int32] + [C.c_void_p] * 5),
     "tts_distill_step": (C.c_int32, [C.c_void_p] * 10 + [C.c_int32, C.c_float] + [C.c_void_p] * 5),
     "tts_distill_step_ex": (C.c_int32, [C.c_void_p] * 10 + [C.c_int32, C.c_float] + [C.c_void_p] * 6),
@@ -207,6 +210,22 @@ def tts_accept_mask(ctx, teacher_logits, draft_tokens, T, mask_out, tau_out, tea
     st = lib().tts_accept_mask(ctx, _ptr(teacher_logits), _ptr(draft_tokens), T, _ptr(mask_out), _ptr(tau_out),
                                _ptr(teacher_argmax_out), _stream(stream, ctx))
     _check(ctx, st, "tts_accept_mask")
+
+
+def tts_accept_mask_static(teacher_logits, logits_dtype, V, seg_len, draft_tokens, T, mask_out, tau_out,
+                           teacher_argmax_out=None, stream=None):
+    """tts_accept_mask for callers that may not allocate on the GPU (no ctx: tts_ctx_create calls cudaMalloc, which a
+    process whose pool owns the whole GPU, or code that must not synchronise the device, cannot afford).  Runs on the
+    CURRENT device with the library's built-in scratch; T <= TTS_STATIC_T_MAX.  Calls on one device share that
+    scratch, so keep them ordered (one stream)."""
+    st = lib().tts_accept_mask_static(_ptr(teacher_logits), logits_dtype, V, seg_len, _ptr(draft_tokens), T,
+                                      _ptr(mask_out), _ptr(tau_out), _ptr(teacher_argmax_out), _stream(stream))
+    if st != TTS_OK:
+        raise TTSError(st, "tts_accept_mask_static", lib().tts_static_last_cuda_error())
+
+
+def tts_static_last_cuda_error() -> int:
+    return lib().tts_static_last_cuda_error()
 
 
 def tts_accept_stochastic(ctx, teacher_logits, draft_logits, draft_tokens, uniforms, uniforms_resample, T, mask_out,
