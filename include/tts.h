@@ -61,9 +61,10 @@ enum { TTS_ROWS_ALL = 0, TTS_ROWS_ACCEPTED = 1, TTS_ROWS_ACCEPTED_PLUS_ONE = 2 }
  * (fp32 parameters, e.g. BASELINE config 1; other shapes).  SIMT forces the CUDA-core kernels. */
 enum { TTS_PATH_AUTO = 0, TTS_PATH_SIMT = 1 };
 /* precision of Adam's moments m, v (the paper fixes only "Adam"; R6, R26).  F32 is the default and what
- * every BASELINE.json configuration uses.  BF16 / Q8 are opt-in variants that cut the step's bytes (tensor path, AdamW
- * only); their layouts and rounding rules are given at tts_distill_step. */
-enum { TTS_MOMENT_F32 = 0, TTS_MOMENT_BF16 = 1, TTS_MOMENT_Q8 = 2 };
+ * every BASELINE.json configuration uses.  BF16 is an opt-in variant that cuts the step's bytes (tensor path, AdamW
+ * only); its layout and rounding rules are given at tts_distill_step.  (Value 2 was TTS_MOMENT_Q8 up to version 0.2.0:
+ * declared, never implemented; it is gone and tts_ctx_create refuses the value like any other unknown one.) */
+enum { TTS_MOMENT_F32 = 0, TTS_MOMENT_BF16 = 1 };
 /* tts_config.flags */
 enum {
   TTS_FLAG_CHECK_PRECONDITIONS = 1, /* every step also runs the checks behind tts_last_device_status (debug mode)  */
@@ -127,21 +128,37 @@ int64_t tts_get_step_count(const tts_ctx* ctx);   /* returns the count (-1 on er
  * stream between two steps); the get enqueues a copy on `stream` and blocks the host on THAT stream only. */
 int32_t tts_set_step_count_async(tts_ctx* ctx, int64_t n, void* stream);
 int64_t tts_get_step_count_on(tts_ctx* ctx, void* stream);
-/* Device status word (bits TTS_DEV_*), accumulated by the kernels since the last read: blocks the host until the last
- * step on this ctx is done (as tts_sync_step), returns the bits (-1 on error) and clears them.  Which checks run:
+/* Device status word (bits TTS_DEV_*), accumulated by the kernels since the last read.  Which checks run:
  *   always                       TTS_DEV_BAD_TOKEN, TTS_DEV_NONFINITE_LOSS
  *   TTS_FLAG_CHECK_PRECONDITIONS TTS_DEV_W_MISMATCH (every element of W_in against rn_bf16(W_master)),
  *                                TTS_DEV_NONFINITE_TEACHER, TTS_DEV_NONFINITE_H (complete scans); +0.6 ms at the
- *                                Qwen3-8B head: a debug mode.  tts_check_preconditions runs the same checks once. */
+ *                                Qwen3-8B head: a debug mode.  tts_check_preconditions runs the same checks once.
+ * tts_last_device_status blocks the host until the last step on this ctx is done (as tts_sync_step) AND until the last
+ * tts_check_preconditions / tts_accept_stochastic call is done, whatever stream each was enqueued on (non-blocking
+ * streams included); it then takes the word (one atomic exchange with 0, on a stream of the ctx's own -- no other
+ * stream of the process is touched) and returns the bits, -1 on error.  Checks enqueued on a THIRD stream before those
+ * two calls are covered only if that stream was ordered before one of them.
+ * tts_device_status_on is the stream-ordered form for a serving loop: the exchange is enqueued on `stream`, behind
+ * whatever the caller enqueued there, and the host blocks on that stream only.  Not inside a stream capture (-1). */
 int32_t tts_last_device_status(tts_ctx* ctx);
+int32_t tts_device_status_on(tts_ctx* ctx, void* stream);
 int32_t tts_check_preconditions(tts_ctx* ctx, const void* teacher_logits, const void* h, const void* W_in,
                                 const float* W_master, int32_t T, void* stream);
 /* A tensor-path kernel whose internal pipeline stalls (a protocol error, never a legal state) does not hang the GPU:
- * a watchdog warp in every persistent kernel traps after ~9 s without progress, the launch fails with
- * cudaErrorLaunchFailed and the next call that synchronises (tts_sync_step, tts_round_host, tts_last_device_status, ...)
- * returns TTS_ERR_CUDA.  tts_debug_trip_watchdog proves it: it launches a deliberately stalled pipeline on `stream`,
- * blocks until the launch has failed and returns TTS_ERR_CUDA; the process's CUDA context is unusable afterwards
- * (run it in a process of its own). */
+ * a watchdog warp in every persistent kernel traps once the kernel has been running for more than a limit, the launch
+ * fails with cudaErrorLaunchFailed and the next call that synchronises (tts_sync_step, tts_round_host,
+ * tts_last_device_status, ...) returns TTS_ERR_CUDA.  A trap ends the PROCESS's CUDA context on that GPU -- everything
+ * the process holds there, a co-resident target model included.
+ *   what is measured  SM cycles since the kernel's own launch, NOT since its last progress: a healthy kernel that is
+ *                     stretched past the limit trips it too (cuda-gdb, compute-sanitizer, time-slicing with another
+ *                     process; a step takes milliseconds, so this needs a slowdown of three orders of magnitude).
+ *   the limit         2^34 cycles (8.7 s at 1.965 GHz) by default.  The environment variable TTS_WATCHDOG_CYCLES, read
+ *                     by tts_ctx_create, replaces it: a decimal cycle count, 0 = never trap (use that under a debugger
+ *                     or sanitizer); anything else that does not parse makes tts_ctx_create return INVALID_ARG.  The
+ *                     value is stored once per GPU for the whole process: the last ctx created on a GPU decides.
+ * tts_debug_trip_watchdog proves the mechanism: it launches a deliberately stalled pipeline on `stream`, blocks until
+ * the launch has failed and returns TTS_ERR_CUDA; the process's CUDA context is unusable afterwards (run it in a process
+ * of its own). */
 int32_t tts_debug_trip_watchdog(tts_ctx* ctx, void* stream);
 /* CUDA error code (cudaError_t as int) of the last failed CUDA call on this ctx, 0 if none. */
 int32_t tts_last_cuda_error(const tts_ctx* ctx);
@@ -247,7 +264,7 @@ int32_t tts_accept_stochastic(tts_ctx* ctx,
  *            M <- M - lr (m / (1-b1^n)) / (sqrt(v / (1-b2^n)) + eps)      (R5)
  *   W_out  = rn_bf16(M)   (TTS_BF16)   |   W_out = M   (TTS_F32, W_master == NULL)
  *   TTS_MOMENT_BF16 (opt-in, R26): adam_m / adam_v hold bf16 [V,d] (18 instead of 26 bytes per parameter in the update
- *            pass).  Per element: widen m, v exactly; update as above with the UNROUNDED new moments; store
+ *            pass; with a2's read of W_in, 20 instead of 28 per step).  Per element: widen m, v exactly; update as above with the UNROUNDED new moments; store
  *            m = rn_bf16(m_new) and v = bf16 by STOCHASTIC rounding of v_new (beta2 = 0.999 decays v by 0.1% per
  *            step, below half a bf16 ulp: nearest rounding would freeze it): the 16 discarded fp32 bits f round
  *            away from zero iff f + r >= 65536, r = 16 bits of a counter-based generator keyed by the element's
@@ -257,7 +274,6 @@ int32_t tts_accept_stochastic(tts_ctx* ctx,
  *              x = lo32(pidx) ^ (n * 0x9E3779B9) ^ (sr_seed * 0x85EBCA6B) ^ (hi32(pidx) * 0xC2B2AE35)
  *              x ^= x >> 16; x *= 0x7FEB352D; x ^= x >> 15; x *= 0x846CA68B; x ^= x >> 16
  *              r = x >> 16 for even v, x & 0xFFFF for odd v
- *            TTS_MOMENT_Q8 (8-bit block-scaled moments) is reserved: tts_ctx_create returns TTS_ERR_UNSUPPORTED.
  *
  * Preconditions: for TTS_BF16, W_in == rn_bf16(W_master) element-wise at entry; teacher_logits
  * and h must stay untouched until the done-event (the step consumes the buffers captured at
@@ -363,7 +379,9 @@ int32_t tts_sync_step(tts_ctx* ctx);
 
 /*
  * One whole round through HOST buffers (used for end-to-end timing): copies the round's inputs
- * from (preferably pinned) host memory into ctx-owned staging buffers, runs tts_accept_mask and
+ * from (preferably pinned) host memory into ctx-owned staging buffers (two slots of T_max x (V + d) inputs, allocated
+ * by the FIRST tts_round_host / tts_round_host_begin call on the ctx -- the one exception to "only tts_ctx_create
+ * allocates", so that callers who never use these calls do not hold 311 MB at T_max = 512), runs tts_accept_mask and
  * tts_distill_step on `stream`, copies loss / tau / mask back and synchronises the stream.
  * The persistent draft state (W, master, m, v) stays resident on the device: device pointers.
  * The teacher logits (the bulk of the bytes: 160 MB at 512 rows) travel on a copy stream owned by the ctx while pass
@@ -376,6 +394,14 @@ int32_t tts_sync_step(tts_ctx* ctx);
  * (else TTS_ERR_INVALID_ARG); rounds end in the order they were begun; the host buffers of a round -- inputs and
  * outputs -- must stay untouched until its end call returns; every pending round must use the same `stream`.
  * tts_round_host == begin + end and refuses to run while begun rounds are pending.
+ *
+ * Ordering of the inputs: the teacher copy does NOT wait for `stream` (that is what lets it run under the previous
+ * round's step), so the host input buffers must be complete ON THE HOST when begin is called; a caller that fills them
+ * with work enqueued on `stream` (a D2H of the verifier's logits, say) synchronises that work first.
+ * Errors: every argument the step could refuse (NULL or misaligned parameter tensors, T, a master / moment pointer that
+ * does not fit the ctx's dtype and optimiser) is refused before anything is enqueued.  If a CUDA call fails after that,
+ * the call blocks until whatever it had already enqueued on `stream` and on the copy stream has drained, returns
+ * TTS_ERR_CUDA, and the round does not count as begun: the host buffers are free again and the slot is reusable.
  */
 int32_t tts_round_host(tts_ctx* ctx,
                        const void* teacher_logits_host, /* host [T,V] logits_dtype */

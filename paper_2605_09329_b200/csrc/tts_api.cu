@@ -41,11 +41,46 @@ void free_all(tts_ctx* c) {
     if (r.round_done) cudaEventDestroy(r.round_done);
   }
   if (c->done_event) cudaEventDestroy(c->done_event);
+  if (c->status_event) cudaEventDestroy(c->status_event);
+  if (c->status_stream) cudaStreamDestroy(c->status_stream);
   if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
   if (c->prof_events) {
     for (int i = 0; i < tts::kProfSlots * (TTS_NUM_PHASES + 1); ++i) cudaEventDestroy(c->prof_events[i]);
     free(c->prof_events);
   }
+}
+
+// Staging of the host-buffer rounds, allocated on first use (the one place outside tts_ctx_create that allocates;
+// include/tts.h says so at tts_round_host).
+cudaError_t ensure_round_slots(tts_ctx* c) {
+  if (c->rs_ready) return cudaSuccess;
+  const tts_config& cfg = c->cfg;
+  const size_t V = cfg.V, Tm = cfg.T_max;
+  cudaError_t e = cudaSuccess;
+  for (int k = 0; k < 2 && e == cudaSuccess; ++k) {
+    tts_ctx::RoundSlot& r = c->rs[k];
+    if (e == cudaSuccess) e = cudaMalloc(&r.teacher, Tm * V * elem_size(cfg.logits_dtype));
+    if (e == cudaSuccess) e = cudaMalloc(&r.h, Tm * cfg.d * elem_size(cfg.param_dtype));
+    if (e == cudaSuccess) e = dmalloc(&r.tok, Tm);
+    if (e == cudaSuccess) e = dmalloc(&r.pw, Tm);
+    if (e == cudaSuccess) e = dmalloc(&r.mask, Tm);
+    if (e == cudaSuccess) e = dmalloc(&r.tau, Tm / cfg.seg_len);
+    if (e == cudaSuccess) e = dmalloc(&r.loss, 1);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&r.copy_done, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&r.round_done, cudaEventDisableTiming);
+  }
+  if (e != cudaSuccess) {   // all or nothing: a later call may try again
+    for (int k = 0; k < 2; ++k) {
+      tts_ctx::RoundSlot& r = c->rs[k];
+      cudaFree(r.teacher); cudaFree(r.h); cudaFree(r.tok); cudaFree(r.pw); cudaFree(r.mask); cudaFree(r.tau); cudaFree(r.loss);
+      if (r.copy_done) cudaEventDestroy(r.copy_done);
+      if (r.round_done) cudaEventDestroy(r.round_done);
+      memset(&r, 0, sizeof(r));
+    }
+    return e;
+  }
+  c->rs_ready = true;
+  return cudaSuccess;
 }
 
 }  // namespace
@@ -63,7 +98,7 @@ const char* tts_status_string(int32_t s) {
   }
 }
 
-int32_t tts_version(void) { return 200; /* 0.2.0 */ }
+int32_t tts_version(void) { return 300; /* 0.3.0 */ }
 
 int32_t tts_ctx_create(const tts_config* cfg, int32_t device, tts_ctx** out) {
   if (!cfg || !out) return TTS_ERR_INVALID_ARG;
@@ -77,7 +112,7 @@ int32_t tts_ctx_create(const tts_config* cfg, int32_t device, tts_ctx** out) {
   if (cfg->kernel_path != TTS_PATH_AUTO && cfg->kernel_path != TTS_PATH_SIMT) return TTS_ERR_UNSUPPORTED;
   if (cfg->max_ctas < 0 || cfg->max_inner_steps < 0) return TTS_ERR_INVALID_ARG;
   if (cfg->flags & ~(TTS_FLAG_CHECK_PRECONDITIONS | TTS_FLAG_DETERMINISTIC | TTS_FLAG_SEPARATE_GH)) return TTS_ERR_INVALID_ARG;
-  if (cfg->moment_dtype != TTS_MOMENT_F32 && cfg->moment_dtype != TTS_MOMENT_BF16) return TTS_ERR_UNSUPPORTED;   // Q8: reserved
+  if (cfg->moment_dtype != TTS_MOMENT_F32 && cfg->moment_dtype != TTS_MOMENT_BF16) return TTS_ERR_UNSUPPORTED;
   if (cfg->moment_dtype != TTS_MOMENT_F32 && cfg->optimizer != TTS_ADAMW) return TTS_ERR_UNSUPPORTED;
   // rows of every [*, V] / [*, d] tensor must start 16-byte aligned
   if ((static_cast<size_t>(cfg->V) * elem_size(cfg->logits_dtype)) % 16 != 0) return TTS_ERR_UNSUPPORTED;
@@ -100,16 +135,25 @@ int32_t tts_ctx_create(const tts_config* cfg, int32_t device, tts_ctx** out) {
   c->sm_count = prop.multiProcessorCount;
   c->T_pad_max = (cfg->T_max + 15) / 16 * 16;
   c->tensor_ok = cfg->kernel_path == TTS_PATH_AUTO && tts::tc_supported(*cfg);
+  c->watchdog_cycles = 1ll << 34;
+  if (const char* w = getenv("TTS_WATCHDOG_CYCLES")) {   // include/tts.h, tts_debug_trip_watchdog
+    char* end = nullptr;
+    const long long v = strtoll(w, &end, 10);
+    if (end == w || *end != '\0' || v < 0) { delete c; return TTS_ERR_INVALID_ARG; }
+    c->watchdog_cycles = v;
+  }
 
   const size_t V = cfg->V, Tm = cfg->T_max, Tp = c->T_pad_max;
   bool ok = true;
   ok = ok && cudaEventCreateWithFlags(&c->done_event, cudaEventDisableTiming) == cudaSuccess;
+  ok = ok && cudaEventCreateWithFlags(&c->status_event, cudaEventDisableTiming) == cudaSuccess;
   ok = ok && cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) == cudaSuccess;
+  ok = ok && cudaStreamCreateWithFlags(&c->status_stream, cudaStreamNonBlocking) == cudaSuccess;
   ok = ok && dmalloc(&c->step_count_dev, 1) == cudaSuccess;
   ok = ok && dmalloc(&c->step_scalars, 2) == cudaSuccess;
   ok = ok && cudaMemset(c->step_count_dev, 0, sizeof(unsigned long long)) == cudaSuccess;
-  ok = ok && dmalloc(&c->dev_status, 1) == cudaSuccess;
-  ok = ok && cudaMemset(c->dev_status, 0, sizeof(int)) == cudaSuccess;
+  ok = ok && dmalloc(&c->dev_status, 2) == cudaSuccess;
+  ok = ok && cudaMemset(c->dev_status, 0, 2 * sizeof(int)) == cudaSuccess;
   ok = ok && cudaHostAlloc(reinterpret_cast<void**>(&c->host_slot), 16, cudaHostAllocDefault) == cudaSuccess;
   ok = ok && dmalloc(&c->z, Tp * V) == cudaSuccess;
   // K > 1 inner steps keep step 1's logits as z_ref: reserved here so that no step call allocates
@@ -126,25 +170,15 @@ int32_t tts_ctx_create(const tts_config* cfg, int32_t device, tts_ctx** out) {
   ok = ok && dmalloc(&c->acc_rows, 2 * Tm) == cudaSuccess;
   ok = ok && dmalloc(&c->acc_rej, Tm / cfg->seg_len) == cudaSuccess;
   ok = ok && dmalloc(&c->acc_rpart, (Tm / cfg->seg_len) * tts::kStatSplitsMax) == cudaSuccess;
-  // staging for tts_round_host
-  for (int k = 0; k < 2; ++k) {
-    tts_ctx::RoundSlot& r = c->rs[k];
-    ok = ok && cudaMalloc(&r.teacher, Tm * V * elem_size(cfg->logits_dtype)) == cudaSuccess;
-    ok = ok && cudaMalloc(&r.h, Tm * cfg->d * elem_size(cfg->param_dtype)) == cudaSuccess;
-    ok = ok && dmalloc(&r.tok, Tm) == cudaSuccess;
-    ok = ok && dmalloc(&r.pw, Tm) == cudaSuccess;
-    ok = ok && dmalloc(&r.mask, Tm) == cudaSuccess;
-    ok = ok && dmalloc(&r.tau, Tm / cfg->seg_len) == cudaSuccess;
-    ok = ok && dmalloc(&r.loss, 1) == cudaSuccess;
-    ok = ok && cudaEventCreateWithFlags(&r.copy_done, cudaEventDisableTiming) == cudaSuccess;
-    ok = ok && cudaEventCreateWithFlags(&r.round_done, cudaEventDisableTiming) == cudaSuccess;
-  }
+  // the staging slots of tts_round_host* (2 x T_max x V logits: 311 MB at T_max = 512) are allocated by the first
+  // such call (ensure_round_slots): callers that keep their data on the device never pay for them
   // the low-precision moment formats live in the tcgen05 update kernels only
   if (ok && !c->tensor_ok && cfg->moment_dtype != TTS_MOMENT_F32) {
     free_all(c);
     delete c;
     return TTS_ERR_UNSUPPORTED;
   }
+  if (ok) ok = tts::check_init(c) == cudaSuccess;
   if (ok && c->tensor_ok) ok = tts::tc_init(c) == cudaSuccess;
   if (!ok) {
     cudaGetLastError();
@@ -206,18 +240,46 @@ int64_t tts_get_step_count_on(tts_ctx* c, void* stream) {
   return static_cast<int64_t>(*slot);
 }
 
+// The word is exchanged with 0 by a one-thread kernel on `s` and copied into the pinned slot behind it; the host then
+// waits for `s` alone.
+static int32_t take_status(tts_ctx* c, cudaStream_t s) {
+  int* slot = c->host_slot + 2;   // the step-count read uses the first 8 bytes of the 16-byte slot
+  cudaError_t e = tts::launch_take_status(c, s);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(slot, c->dev_status + 1, sizeof(int), cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  if (e != cudaSuccess) { cuda_fail(c, e); return -1; }
+  return *slot;
+}
+
 int32_t tts_last_device_status(tts_ctx* c) {
   if (!c) return -1;
   tts_device_guard g(c->device);
+  // Host-side waits on the two events that stand behind every kernel able to set a bit: the last step's done-event and
+  // the event of the last tts_check_preconditions / tts_accept_stochastic.  (The legacy default stream would NOT order
+  // this read after work on cudaStreamNonBlocking streams, which is what every torch.cuda.Stream is.)
   cudaError_t e = cudaSuccess;
   if (c->done_recorded) e = cudaEventSynchronize(c->done_event);
-  int bits = 0;
-  // the word is only ever written by kernels of finished steps at this point; the copy and the clear use the
-  // legacy default stream, which orders them after everything enqueued before this call
-  if (e == cudaSuccess) e = cudaMemcpy(&bits, c->dev_status, sizeof(int), cudaMemcpyDeviceToHost);
-  if (e == cudaSuccess) e = cudaMemset(c->dev_status, 0, sizeof(int));
+  if (e == cudaSuccess && c->status_recorded) e = cudaEventSynchronize(c->status_event);
   if (e != cudaSuccess) { cuda_fail(c, e); return -1; }
-  return bits;
+  return take_status(c, c->status_stream);
+}
+
+int32_t tts_device_status_on(tts_ctx* c, void* stream) {
+  if (!c) return -1;
+  tts_device_guard g(c->device);
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing(s, &cap) != cudaSuccess || cap != cudaStreamCaptureStatusNone) return -1;
+  return take_status(c, s);
+}
+
+// status bits can also come from calls that are not steps: an event behind them for tts_last_device_status
+static cudaError_t mark_status_source(tts_ctx* c, cudaStream_t s) {
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  cudaError_t e = cudaStreamIsCapturing(s, &cap);
+  if (e != cudaSuccess || cap != cudaStreamCaptureStatusNone) return e;   // inside a capture: see tts_record_done
+  if ((e = cudaEventRecord(c->status_event, s)) == cudaSuccess) c->status_recorded = true;
+  return e;
 }
 
 int32_t tts_check_preconditions(tts_ctx* c, const void* teacher, const void* h, const void* W_in, const float* W_master,
@@ -230,6 +292,7 @@ int32_t tts_check_preconditions(tts_ctx* c, const void* teacher, const void* h, 
   cudaError_t e = tts::launch_check_preconditions(c, teacher, h, W_in, W_master, T, static_cast<cudaStream_t>(stream),
                                                   &launches);
   c->last_launches = launches;
+  if (e == cudaSuccess) e = mark_status_source(c, static_cast<cudaStream_t>(stream));
   return e == cudaSuccess ? TTS_OK : cuda_fail(c, e);
 }
 
@@ -275,6 +338,7 @@ int32_t tts_accept_stochastic(tts_ctx* c, const void* teacher, const float* draf
                                                 mask_out, tau_out, next_token_out, diag_out,
                                                 static_cast<cudaStream_t>(stream), &launches);
   c->last_launches = launches;
+  if (e == cudaSuccess) e = mark_status_source(c, static_cast<cudaStream_t>(stream));
   if (e != cudaSuccess) return cuda_fail(c, e);
   return TTS_OK;
 }
@@ -287,12 +351,13 @@ int32_t tts_distill_step(tts_ctx* c, const void* teacher, const void* h, const v
                              loss_out, kl_rows_out, gh_out, gW_debug_out, nullptr, side_stream);
 }
 
-// The step of include/tts.h in one piece (phase 0) or as the two halves of the vocabulary-sharded step.
-static int32_t run_step(tts_ctx* c, const void* teacher, const void* h, const void* W_in, void* W_out,
-                        float* W_master, void* adam_m, void* adam_v, const float* pos_weight,
-                        const uint8_t* mask, int32_t T, float loss_scale, float* loss_out, float* kl_rows_out,
-                        float* gh_out, float* gW_debug_out, const tts_step_extras* ex, void* side_stream, int phase,
-                        float* stats_out, const float* stats_all, int32_t n_shards) {
+// Everything a step call can reject without touching the GPU (so that callers which enqueue other work first, like
+// tts_round_host, can ask BEFORE their first enqueue).
+static int32_t check_step_args(const tts_ctx* c, const void* teacher, const void* h, const void* W_in, const void* W_out,
+                               const float* W_master, const void* adam_m, const void* adam_v, const float* pos_weight,
+                               const uint8_t* mask, int32_t T, const float* loss_out, const float* gh_out,
+                               const float* gW_debug_out, const tts_step_extras* ex, int phase, const float* stats_out,
+                               const float* stats_all, int32_t n_shards) {
   if (!c || !teacher || !h || !W_in) return TTS_ERR_INVALID_ARG;
   if (phase != tts::kPhaseBegin && (!W_out || !pos_weight || !loss_out)) return TTS_ERR_INVALID_ARG;
   if (phase == tts::kPhaseBegin && !stats_out) return TTS_ERR_INVALID_ARG;
@@ -314,6 +379,19 @@ static int32_t run_step(tts_ctx* c, const void* teacher, const void* h, const vo
   if (!aligned16(teacher) || !aligned16(h) || !aligned16(W_in) || !aligned16(W_out) || !aligned16(W_master) ||
       !aligned16(adam_m) || !aligned16(adam_v) || !aligned16(gh_out) || !aligned16(gW_debug_out))
     return TTS_ERR_INVALID_ARG;
+  return TTS_OK;
+}
+
+// The step of include/tts.h in one piece (phase 0) or as the two halves of the vocabulary-sharded step.
+static int32_t run_step(tts_ctx* c, const void* teacher, const void* h, const void* W_in, void* W_out,
+                        float* W_master, void* adam_m, void* adam_v, const float* pos_weight,
+                        const uint8_t* mask, int32_t T, float loss_scale, float* loss_out, float* kl_rows_out,
+                        float* gh_out, float* gW_debug_out, const tts_step_extras* ex, void* side_stream, int phase,
+                        float* stats_out, const float* stats_all, int32_t n_shards) {
+  const int32_t ok = check_step_args(c, teacher, h, W_in, W_out, W_master, adam_m, adam_v, pos_weight, mask, T, loss_out,
+                                     gh_out, gW_debug_out, ex, phase, stats_out, stats_all, n_shards);
+  if (ok != TTS_OK) return ok;
+  const tts_config& cfg = c->cfg;
 
   tts_device_guard guard(c->device);
   cudaStream_t s = static_cast<cudaStream_t>(side_stream);
@@ -511,24 +589,20 @@ int32_t tts_sync_step(tts_ctx* c) {
 
 // One round through host buffers, enqueued only: inputs into staging slot (rounds begun & 1), a1 + the step on `stream`,
 // results back into the caller's host buffers, the slot's round_done event behind them.
-static int32_t round_host_enqueue(tts_ctx* c, const void* teacher_host, const void* h_host, const int32_t* tok_host,
-                                  const float* pw_host, int32_t T, float loss_scale, const void* W_in, void* W_out,
-                                  float* W_master, void* adam_m, void* adam_v, float* gh_dev, float* loss_host,
-                                  int32_t* tau_host, uint8_t* mask_host, void* stream) {
-  if (!c || !teacher_host || !h_host || !tok_host || !pw_host || !loss_host || !tau_host) return TTS_ERR_INVALID_ARG;
+static int32_t round_host_body(tts_ctx* c, tts_ctx::RoundSlot& r, bool reused, const void* teacher_host,
+                               const void* h_host, const int32_t* tok_host, const float* pw_host, int32_t T,
+                               float loss_scale, const void* W_in, void* W_out, float* W_master, void* adam_m,
+                               void* adam_v, float* gh_dev, float* loss_host, int32_t* tau_host, uint8_t* mask_host,
+                               void* stream) {
   const tts_config& cfg = c->cfg;
-  if (T <= 0 || T > cfg.T_max || T % cfg.seg_len != 0) return TTS_ERR_INVALID_ARG;
-  if (c->rh_begun - c->rh_ended >= 2) return TTS_ERR_INVALID_ARG;   // both slots are in flight: end a round first
-  tts_device_guard guard(c->device);
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const size_t V = cfg.V, d = cfg.d;
-  const bool reused = c->rh_begun >= 2;
-  tts_ctx::RoundSlot& r = c->rs[c->rh_begun & 1];
   cudaError_t e;
   // The teacher logits (the bulk: 160 MB at 512 rows, ~3 ms of PCIe) travel on the ctx's copy stream.  That copy waits
   // only for the round that used this slot two rounds ago, NOT for the caller's stream: it runs under the previous
-  // round's step and under this round's pass a2, which needs only h and W_in (tensor path).  The small inputs go on
-  // the caller's stream (their slot's last readers are earlier kernels of that stream).
+  // round's step and under this round's pass a2, which needs only h and W_in (tensor path).  That is why the host
+  // buffers must be complete ON THE HOST when this is called (include/tts.h).  The small inputs go on the caller's
+  // stream (their slot's last readers are earlier kernels of that stream).
   if (reused && (e = cudaStreamWaitEvent(c->copy_stream, r.round_done, 0)) != cudaSuccess) return cuda_fail(c, e);
   if ((e = cudaMemcpyAsync(r.teacher, teacher_host, (size_t)T * V * elem_size(cfg.logits_dtype),
                            cudaMemcpyHostToDevice, c->copy_stream)) != cudaSuccess) return cuda_fail(c, e);
@@ -543,7 +617,7 @@ static int32_t round_host_enqueue(tts_ctx* c, const void* teacher_host, const vo
   int early_launches = 0;
   tts_step_extras ex;
   ex.draft_logits = nullptr; ex.draft_logits_out = nullptr; ex.ref_logits = nullptr; ex.lambda = 0.f;
-  if (c->tensor_ok && aligned16(W_in)) {
+  if (c->tensor_ok) {
     tts::StepArgs a0;
     memset(&a0, 0, sizeof(a0));
     a0.h = r.h; a0.W_in = W_in; a0.T = T;
@@ -564,6 +638,41 @@ static int32_t round_host_enqueue(tts_ctx* c, const void* teacher_host, const vo
   if (mask_host && (e = cudaMemcpyAsync(mask_host, r.mask, (size_t)T, cudaMemcpyDeviceToHost, s)) != cudaSuccess)
     return cuda_fail(c, e);
   if ((e = cudaEventRecord(r.round_done, s)) != cudaSuccess) return cuda_fail(c, e);
+  return TTS_OK;
+}
+
+static int32_t round_host_enqueue(tts_ctx* c, const void* teacher_host, const void* h_host, const int32_t* tok_host,
+                                  const float* pw_host, int32_t T, float loss_scale, const void* W_in, void* W_out,
+                                  float* W_master, void* adam_m, void* adam_v, float* gh_dev, float* loss_host,
+                                  int32_t* tau_host, uint8_t* mask_host, void* stream) {
+  if (!c || !teacher_host || !h_host || !tok_host || !pw_host || !loss_host || !tau_host) return TTS_ERR_INVALID_ARG;
+  if (c->rh_begun - c->rh_ended >= 2) return TTS_ERR_INVALID_ARG;   // both slots are in flight: end a round first
+  // Everything the step could refuse is refused here, BEFORE anything is allocated or enqueued.  The step's device
+  // inputs will be a slot's staging buffers (never NULL, cudaMalloc-aligned: `staged` stands in for them, it is only
+  // compared, never dereferenced) and the caller's parameter tensors.
+  alignas(16) static const unsigned char staged[16] = {0};
+  const float* sf = reinterpret_cast<const float*>(staged);
+  const int32_t ok = check_step_args(c, staged, staged, W_in, W_out, W_master, adam_m, adam_v, sf, staged, T, sf, gh_dev,
+                                     nullptr, nullptr, tts::kPhaseAll, nullptr, nullptr, 0);
+  if (ok != TTS_OK) return ok;
+  tts_device_guard guard(c->device);
+  if (!c->rs_ready) {   // first host-buffer round on this ctx: allocate the two staging slots (nothing is in flight yet)
+    const cudaError_t ea = ensure_round_slots(c);
+    if (ea != cudaSuccess) return cuda_fail(c, ea);
+  }
+  tts_ctx::RoundSlot& r = c->rs[c->rh_begun & 1];
+  const int32_t st = round_host_body(c, r, c->rh_begun >= 2, teacher_host, h_host, tok_host, pw_host, T, loss_scale,
+                                     W_in, W_out, W_master, adam_m, adam_v, gh_dev, loss_host, tau_host, mask_host,
+                                     stream);
+  if (st != TTS_OK) {
+    // A CUDA call failed after copies / kernels of this round were enqueued.  The round does not count (rh_begun stays),
+    // so nothing would ever wait for them: drain both streams here, while the caller's host buffers and this slot are
+    // still what the in-flight work expects, and leave the slot's events in a state the next begin can wait on.
+    cudaStreamSynchronize(c->copy_stream);
+    cudaStreamSynchronize(static_cast<cudaStream_t>(stream));
+    cudaEventRecord(r.round_done, static_cast<cudaStream_t>(stream));
+    return st;
+  }
   ++c->rh_begun;
   return TTS_OK;
 }

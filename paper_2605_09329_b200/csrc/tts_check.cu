@@ -57,6 +57,9 @@ __global__ void __launch_bounds__(96) stalled_pipeline_kernel() {
 
 __global__ void set_count_kernel(unsigned long long* p, unsigned long long n) { *p = n; }
 
+// read-and-clear in one atomic: a bit that a still-running kernel sets around it lands either in this read or in the next
+__global__ void take_status_kernel(int* status) { status[1] = atomicExch(status, 0); }
+
 }  // namespace
 
 cudaError_t launch_check_preconditions(tts_ctx* c, const void* teacher, const void* h, const void* W_in,
@@ -89,8 +92,15 @@ cudaError_t launch_check_preconditions(tts_ctx* c, const void* teacher, const vo
   return cudaGetLastError();
 }
 
+cudaError_t check_init(tts_ctx* c) { return ptx::set_watchdog_cycles(c->watchdog_cycles); }
+
 cudaError_t launch_stalled_pipeline(cudaStream_t s) {
   stalled_pipeline_kernel<<<1, 96, 0, s>>>();
+  return cudaGetLastError();
+}
+
+cudaError_t launch_take_status(tts_ctx* c, cudaStream_t s) {
+  take_status_kernel<<<1, 1, 0, s>>>(c->dev_status);
   return cudaGetLastError();
 }
 

@@ -79,21 +79,25 @@ struct tts_ctx {
   int last_used_tensor;
   int last_launches;
   int T_pad_max;          // T_max rounded up to 16
+  long long watchdog_cycles;   // limit of the kernels' watchdog (TTS_WATCHDOG_CYCLES at create; 0 = off)
   bool tensor_ok;         // shape/dtype qualifies for the tcgen05 kernels
   cudaEvent_t done_event;
   bool done_recorded;
+  cudaEvent_t status_event;   // behind the last tts_check_preconditions / tts_accept_stochastic (they set status bits too)
+  bool status_recorded;
+  cudaStream_t status_stream; // non-blocking: the read-and-clear of the status word runs here, never on the legacy stream
   // ---- scratch (device) ----
   float* z;               // [T_pad_max, V] draft logits (fp32)
   float* dl32;            // [T_max, V] fp32 dlogits                (CUDA-core path)
-  float* stat_part;       // [T_max, kStatSplitsMax, 5]
+  float* stat_part;       // [T_max, kStatTuplesMax, kStatFields]
   float* row_stats;       // [kRowStatFields, T_max]: lse_t, lse_z, kl, coef (= loss_scale * omega), lse_ref
   double* row_loss;       // [T_max] omega_r (KL_r + lambda KL_ref,r): summed in a fixed order by the merge kernel's last CTA
   unsigned int* merge_ticket;
-  float* z_ref_buf;       // [T_pad_max, V] fp32, allocated by the first tts_distill_inner_steps call
+  float* z_ref_buf;       // [T_pad_max, V] fp32, reserved by tts_ctx_create when cfg.max_inner_steps > 1, else NULL
   float* arg_val;         // [T_max, kArgSplitsMax]
   int32_t* arg_idx;       // [T_max, kArgSplitsMax]
   int32_t* argmax_tmp;    // [T_max]
-  int* dev_status;        // device status word (bits TTS_DEV_*), read and cleared by tts_last_device_status
+  int* dev_status;        // [2]: device status word (bits TTS_DEV_*) + the slot its read-and-clear exchanges it into
   int* host_slot;         // pinned host scratch (16 bytes) for the stream-ordered status / step-count reads
   float* gh_part;         // TTS_FLAG_DETERMINISTIC: [units][T16][128] per-unit parts of gh (tts_tc_gemm.cu)
   float* acc_rows;        // [T_max, 2] lse_t, lse_z of tts_accept_stochastic
@@ -112,6 +116,7 @@ struct tts_ctx {
     cudaEvent_t copy_done;    // the teacher's H2D copy into this slot has landed
     cudaEvent_t round_done;   // the round that used this slot has finished (results copied back): the slot is free
   } rs[2];
+  bool rs_ready;                // the slots exist (allocated by the first tts_round_host* call, not by tts_ctx_create)
   unsigned rh_begun, rh_ended;  // rounds begun / ended through the host API (slot = count & 1; at most 2 outstanding)
   cudaStream_t copy_stream;   // the teacher's H2D copy runs here, next to a2 (and the previous round) on the caller's stream
   // ---- per-phase profiling (tts_profile_*) ----
@@ -135,7 +140,9 @@ inline void prof_mark(tts_ctx* c, int phase, cudaStream_t s) {
 cudaError_t launch_check_preconditions(tts_ctx* c, const void* teacher, const void* h, const void* W_in,
                                        const float* master, int T, cudaStream_t s, int* launches);
 cudaError_t launch_set_count(tts_ctx* c, unsigned long long n, cudaStream_t s);
+cudaError_t launch_take_status(tts_ctx* c, cudaStream_t s);   // dev_status[1] = atomicExch(&dev_status[0], 0)
 cudaError_t launch_stalled_pipeline(cudaStream_t s);
+cudaError_t check_init(tts_ctx* c);   // this unit's copy of the watchdog limit (tts_tc_ptx.cuh)
 // tts_mask.cu
 cudaError_t launch_accept_mask(tts_ctx* c, const void* teacher, const int32_t* tok, int T, uint8_t* mask,
                                int32_t* tau, int32_t* am_out, cudaStream_t s, int* launches);

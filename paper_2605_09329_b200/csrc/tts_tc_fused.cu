@@ -515,6 +515,7 @@ __global__ void __launch_bounds__(256) tc_prep_dlc_kernel(const void* __restrict
 }  // namespace
 
 cudaError_t tc_fused_init(tts_ctx* c) {
+  if (cudaError_t w = ptx::set_watchdog_cycles(c->watchdog_cycles)) return w;
   cudaError_t e;
   TcState* st = static_cast<TcState*>(c->tc_state);
   if ((e = cudaMalloc(&st->hTc, (size_t)c->cfg.d * kT16 * 2)) != cudaSuccess) return e;

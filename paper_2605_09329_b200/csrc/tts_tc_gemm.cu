@@ -476,7 +476,7 @@ struct GhPlan {
 GhPlan gh_plan(const tts_ctx* c, int T16) {
   GhPlan g;
   const int n_jt = c->cfg.d / kTileMN, chunks_total = c->cfg.V / kKC;
-  g.grid = c->cfg.max_ctas > 0 ? c->cfg.max_ctas : c->sm_count;
+  g.grid = (c->cfg.max_ctas > 0 && c->cfg.max_ctas < c->sm_count) ? c->cfg.max_ctas : c->sm_count;
   g.planes = tc_wide_planes(T16);
   g.N = g.planes * T16;
   g.box_rows = g.N <= kNMax ? g.N : kNMax;
@@ -504,7 +504,8 @@ int pick_stages(int stage_bytes, int extra = 0) {
 
 }  // namespace
 
-cudaError_t tc_gemm_init(tts_ctx*) {
+cudaError_t tc_gemm_init(tts_ctx* c) {
+  if (cudaError_t w = ptx::set_watchdog_cycles(c->watchdog_cycles)) return w;
   cudaError_t e;
   const auto attr = cudaFuncAttributeMaxDynamicSharedMemorySize;
   if ((e = cudaFuncSetAttribute(tc_logits_kernel<false, true>, attr, kSmemLimit)) != cudaSuccess) return e;
@@ -548,7 +549,7 @@ cudaError_t tc_launch_logits(tts_ctx* c, const StepArgs& a, float* z_out, bool f
       make_map_2d(st, &tm_t, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, a.teacher, V, T, kTileMN, epi::kRows,
                   CU_TENSOR_MAP_SWIZZLE_NONE) != CUDA_SUCCESS)
     return cudaErrorInvalidValue;
-  int grid = c->cfg.max_ctas > 0 ? c->cfg.max_ctas : c->sm_count;
+  int grid = tc_logits_ctas(c);
   if (grid > p.n_vt) grid = p.n_vt;
   // Stream-K for one canvas: 1187 tiles over 148 CTAs would quantise to 9 waves of 8.02; equal contiguous unit
   // ranges keep every SM busy to the end.  A range spans >= k_chunks units (grid <= n_vt), so a tile is cut at most
@@ -562,7 +563,9 @@ cudaError_t tc_launch_logits(tts_ctx* c, const StepArgs& a, float* z_out, bool f
     const long total = (long)p.n_vt * p.k_chunks;
     for (int b = 1; b < grid; ++b) {
       const long u = total * b / grid;
-      if (u % p.k_chunks != 0 && n_cut < kStatFixMax) cut[n_cut++] = (int)(u / p.k_chunks) * kTileMN;
+      if (u % p.k_chunks == 0) continue;
+      if (n_cut == kStatFixMax) return cudaErrorInvalidConfiguration;   // unreachable: grid <= kStatFixMax (tc_logits_ctas)
+      cut[n_cut++] = (int)(u / p.k_chunks) * kTileMN;
     }
   }
   epi::Params ep;

@@ -249,7 +249,8 @@ tc_logits_pair_kernel(const __grid_constant__ CUtensorMap tm_W, const __grid_con
 
 }  // namespace
 
-cudaError_t tc_pair_init(tts_ctx*) {
+cudaError_t tc_pair_init(tts_ctx* c) {
+  if (cudaError_t w = ptx::set_watchdog_cycles(c->watchdog_cycles)) return w;
   cudaError_t e = cudaFuncSetAttribute(tc_logits_pair_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPSmemLimit);
   if (e != cudaSuccess) return e;
   return cudaFuncSetAttribute(tc_logits_pair_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPSmemLimit);
@@ -293,7 +294,7 @@ cudaError_t tc_launch_logits_pair(tts_ctx* c, const StepArgs& a, float* z_out, b
       make_map_2d(st, &tm_t, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, a.teacher, V, T, 128, epi::kRows,
                   CU_TENSOR_MAP_SWIZZLE_NONE) != CUDA_SUCCESS)
     return cudaErrorInvalidValue;
-  int grid = c->cfg.max_ctas > 0 ? c->cfg.max_ctas : c->sm_count;
+  int grid = tc_logits_ctas(c);
   grid &= ~1;
   if (grid > 2 * p.n_pt) grid = 2 * p.n_pt;
   const int n_pairs = grid / 2;
@@ -307,7 +308,10 @@ cudaError_t tc_launch_logits_pair(tts_ctx* c, const StepArgs& a, float* z_out, b
     const size_t v_left = (size_t)p.n_main * 256;
     cudaError_t e = cudaMemset2DAsync(z_out + v_left, (size_t)V * sizeof(float), 0, (V - v_left) * sizeof(float), T, s);
     if (e != cudaSuccess) return e;
-    for (size_t v = v_left; v < (size_t)V && n_cut < kStatFixMax; v += 128) cut[n_cut++] = (int)v;
+    for (size_t v = v_left; v < (size_t)V; v += 128) {
+      if (n_cut == kStatFixMax) return cudaErrorInvalidConfiguration;   // unreachable: <= grid / 2 tiles, grid <= kStatFixMax
+      cut[n_cut++] = (int)v;
+    }
   }
   epi::Params ep;
   ep.teacher = a.teacher; ep.part = c->stat_part; ep.n_split = grid + n_cut; ep.T = T; ep.V = V;

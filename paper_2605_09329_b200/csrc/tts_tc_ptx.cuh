@@ -61,9 +61,18 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
 // an iteration counter) cost the one-canvas update kernel 1.7 - 5% through ptxas' schedule of its epilogue (measured
 // A/B on one box, profiles/r2_README.md).  A stalled pipeline is caught by a WATCHDOG instead: the warp that only
 // allocates tensor memory sleeps until every epilogue warp (the last stage of each kernel's pipeline) has finished, and
-// traps if that takes more than ~2^34 cycles (8.7 s at 1.965 GHz; a step takes milliseconds).  The launch then fails
-// with cudaErrorLaunchFailed and the host sees TTS_ERR_CUDA instead of a hung GPU.
+// traps if the kernel has by then been running for more than the limit below, counted in SM cycles FROM THE MOMENT
+// THE WATCHDOG WARP STARTED (i.e. since the CTA's launch, not since the last progress).  The launch then fails with
+// cudaErrorLaunchFailed and the host sees TTS_ERR_CUDA instead of a hung GPU.
+// The limit is a device variable, one copy per translation unit (the library is built without relocatable device
+// code): default 2^34 cycles (8.7 s at 1.965 GHz; a step takes milliseconds), 0 = never trap.  tts_ctx_create sets
+// every copy from the environment variable TTS_WATCHDOG_CYCLES (include/tts.h) through set_watchdog_cycles below.
 constexpr long long kWatchdogCycles = 1ll << 34;
+static __device__ long long g_watchdog_cycles = kWatchdogCycles;
+// host: sets THIS translation unit's copy on the current device (synchronous; call it from the unit's init function)
+static inline cudaError_t set_watchdog_cycles(long long cycles) {
+  return cudaMemcpyToSymbol(g_watchdog_cycles, &cycles, sizeof(cycles));
+}
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   while (!mbar_try_wait(bar, parity)) {
   }
@@ -76,9 +85,10 @@ __device__ __forceinline__ void watchdog_wait(uint64_t* done_bar) {
 #ifdef TTS_NO_WATCHDOG   // build-time measurement option (profiles/r2_README.md)
   return;
 #endif
+  const long long limit = *reinterpret_cast<volatile const long long*>(&g_watchdog_cycles);
   const long long t0 = clock64();
   while (!mbar_try_wait(done_bar, 0)) {
-    if (clock64() - t0 > kWatchdogCycles) asm volatile("trap;");
+    if (limit > 0 && clock64() - t0 > limit) asm volatile("trap;");
   }
 }
 

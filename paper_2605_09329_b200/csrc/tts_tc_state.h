@@ -42,13 +42,26 @@ inline CUresult make_map_2d(const TcState* st, CUtensorMap* m, CUtensorMapDataTy
 // (Qwen3-8B head, profiles/r2_README.md) the one-canvas pass runs 2.46 ms on 132 CTAs whatever the ring depth (5-7
 // stages) and 2.51 / 2.68 / 2.74 ms on 148 CTAs with 5 / 6 / 7 stages; every grid of 136 CTAs and more shows that
 // cliff, every grid from 124 to 132 does not; the several-canvas pass behaves the same way (2.69 against 2.73-2.91 ms
-// at 64 rows).  So those passes leave a tenth of the SMs idle.  With bf16 moments the pass is bound by its epilogue
-// warps (18 bytes per parameter) and wants every SM.
+// at 64 rows).  So those passes leave a tenth of the SMs idle ON THAT PART: the figure is one measurement of the
+// 148-SM B200 (and the driver's box of round 2 ran 2.66 ms at the same 132 CTAs), not a rule, so any other
+// SM count gets one CTA per SM and a caller's max_ctas always wins.  With bf16 moments the pass is bound by its
+// epilogue warps (18 bytes per parameter in this pass, 20 per step with a2's read of W_in) and wants every SM.
+constexpr int kB200Sms = 148, kB200UpdateCtas = 132;
 inline int tc_update_ctas(const tts_ctx* c, bool lowp_moments) {
   if (c->cfg.max_ctas > 0) return c->cfg.max_ctas < c->sm_count ? c->cfg.max_ctas : c->sm_count;
-  if (lowp_moments) return c->sm_count;
-  const int g = (c->sm_count * 229) >> 8;   // 0.895 x SMs: 132 of 148
-  return g < 1 ? 1 : g;
+  if (lowp_moments || c->sm_count != kB200Sms) return c->sm_count;
+  return kB200UpdateCtas;
+}
+
+// CTAs of a logits kernel (tc_logits_kernel, tc_logits_pair_kernel): the caller's SM budget, never more than the SMs
+// there are, and never more than the per-row statistics scratch can describe.  A stream-K walk over `grid` ranges cuts
+// at most grid - 1 tiles (the pair kernel's K-split tail: at most grid / 2), each cut tile adds one fix-up tuple, so
+// grid <= kStatFixMax keeps the fix-up list within kStatFixMax entries and grid + cuts within kStatTuplesMax tuples
+// on any part (B200: 148 + 147 = 295).
+static_assert(2 * kStatFixMax <= kStatTuplesMax, "stat_part holds one tuple per CTA plus one per cut tile");
+inline int tc_logits_ctas(const tts_ctx* c) {
+  const int g = (c->cfg.max_ctas > 0 && c->cfg.max_ctas < c->sm_count) ? c->cfg.max_ctas : c->sm_count;
+  return g < kStatFixMax ? g : kStatFixMax;
 }
 
 // tts_tc_gemm.cu

@@ -685,7 +685,8 @@ cudaError_t wide_attr() {
 
 }  // namespace
 
-cudaError_t tc_wide_init(tts_ctx*) {
+cudaError_t tc_wide_init(tts_ctx* c) {
+  if (cudaError_t w = ptx::set_watchdog_cycles(c->watchdog_cycles)) return w;
   cudaError_t e;
   if ((e = wide_attr<true, 32, false, 0>()) != cudaSuccess) return e;
   if ((e = wide_attr<false, 32, false, 0>()) != cudaSuccess) return e;

@@ -18,7 +18,7 @@ TTS_F32, TTS_BF16 = 0, 1
 TTS_SGD, TTS_ADAMW = 0, 1
 TTS_ROWS_ALL, TTS_ROWS_ACCEPTED, TTS_ROWS_ACCEPTED_PLUS_ONE = 0, 1, 2
 TTS_PATH_AUTO, TTS_PATH_SIMT = 0, 1
-TTS_MOMENT_F32, TTS_MOMENT_BF16, TTS_MOMENT_Q8 = 0, 1, 2
+TTS_MOMENT_F32, TTS_MOMENT_BF16 = 0, 1
 TTS_FLAG_CHECK_PRECONDITIONS, TTS_FLAG_DETERMINISTIC, TTS_FLAG_SEPARATE_GH = 1, 2, 4
 TTS_DEV_W_MISMATCH, TTS_DEV_NONFINITE_TEACHER, TTS_DEV_NONFINITE_H, TTS_DEV_BAD_TOKEN, TTS_DEV_NONFINITE_LOSS = 1, 2, 4, 8, 16
 TTS_NUM_PHASES = 5
@@ -53,6 +53,7 @@ EXPORTS = {
     "tts_set_step_count_async": (C.c_int32, [C.c_void_p, C.c_int64, C.c_void_p]),
     "tts_get_step_count_on": (C.c_int64, [C.c_void_p, C.c_void_p]),
     "tts_last_device_status": (C.c_int32, [C.c_void_p]),
+    "tts_device_status_on": (C.c_int32, [C.c_void_p, C.c_void_p]),
     "tts_check_preconditions": (C.c_int32, [C.c_void_p] * 5 + [C.c_int32, C.c_void_p]),
     "tts_debug_trip_watchdog": (C.c_int32, [C.c_void_p, C.c_void_p]),
     "tts_last_cuda_error": (C.c_int32, [C.c_void_p]),
@@ -181,6 +182,10 @@ def tts_get_step_count_on(ctx, stream=None) -> int:
 
 def tts_last_device_status(ctx) -> int:
     return lib().tts_last_device_status(ctx)
+
+
+def tts_device_status_on(ctx, stream=None) -> int:
+    return lib().tts_device_status_on(ctx, _stream(stream, ctx))
 
 
 def tts_check_preconditions(ctx, teacher_logits, h, W_in, W_master, T, stream=None):

@@ -101,3 +101,14 @@ def test_product_does_not_import_oracle():
         if f.endswith(".py"):
             assert "paper_2605_09329_b200" not in open(os.path.join(ROOT, "oracle", f)).read().replace(
                 "``paper_2605_09329_b200/``", ""), f
+
+
+def test_unknown_moment_format_is_refused_without_a_gpu(built):
+    """The 8-bit moment format was a declared-but-unbuilt enum value (2) up to 0.2.0; it is gone from header and
+    binding, and the value is refused by argument checking alone (before any CUDA call)."""
+    from paper_2605_09329_b200 import tts
+    assert not hasattr(tts, "TTS_MOMENT_Q8") and "TTS_MOMENT_Q8 =" not in open(os.path.join(ROOT, "include", "tts.h")).read()
+    with pytest.raises(tts.TTSError) as e:
+        tts.tts_ctx_create(tts.make_config(1024, 128, 16, 16, moment_dtype=2), 0)
+    assert e.value.status == tts.TTS_ERR_UNSUPPORTED
+    assert tts.tts_version() >= 300

@@ -86,6 +86,81 @@ def test_precondition_checks_report_into_the_status_word():
         tts.tts_ctx_destroy(ctx)
 
 
+def test_status_word_sees_work_queued_on_a_non_blocking_stream():
+    """A torch.cuda.Stream is cudaStreamNonBlocking: the legacy default stream does not order after it.  The status
+    read must still wait for a check (or a stochastic accept) that sits on such a stream behind ~0.1 s of other work,
+    through both forms of the call."""
+    case = synth.make_case(3, V=4096, d=1024)
+    ctx = tts.tts_ctx_create(config_for(case), 0)
+    try:
+        T, V = case["T"], case["V"]
+        t = _buffers(case)
+        t["h"][2, 5] = float("inf")
+        side = torch.cuda.Stream()
+        torch.cuda.synchronize()
+
+        def delayed_check():
+            with torch.cuda.stream(side):
+                torch.cuda._sleep(200_000_000)    # the check below is still queued when the status is asked for
+            tts.tts_check_preconditions(ctx, t["teacher"], t["h"], t["W_in"], t["master"], T, side)
+
+        delayed_check()
+        assert tts.tts_last_device_status(ctx) == tts.TTS_DEV_NONFINITE_H
+        assert tts.tts_last_device_status(ctx) == 0            # taken: read-and-clear
+        delayed_check()
+        assert tts.tts_device_status_on(ctx, side) == tts.TTS_DEV_NONFINITE_H
+        assert tts.tts_device_status_on(ctx, side) == 0
+        # TTS_DEV_BAD_TOKEN from the stochastic accept, same situation
+        tok = t["tok"].clone()
+        tok[1] = V + 5
+        z = torch.randn(T, V, device="cuda")
+        u, u2 = torch.rand(T, device="cuda"), torch.rand(T // case["seg_len"], device="cuda")
+        mask = torch.zeros(T, dtype=torch.uint8, device="cuda")
+        tau = torch.zeros(T // case["seg_len"], dtype=torch.int32, device="cuda")
+        nxt = torch.zeros(T // case["seg_len"], dtype=torch.int32, device="cuda")
+        torch.cuda.synchronize()
+        with torch.cuda.stream(side):
+            torch.cuda._sleep(200_000_000)
+        tts.tts_accept_stochastic(ctx, t["teacher"], z, tok, u, u2, T, mask, tau, nxt, None, side)
+        assert tts.tts_last_device_status(ctx) == tts.TTS_DEV_BAD_TOKEN
+        assert tts.tts_last_device_status(ctx) == 0
+    finally:
+        tts.tts_ctx_destroy(ctx)
+
+
+def test_host_round_staging_is_allocated_by_the_first_host_round_only():
+    """tts_ctx_create no longer reserves the two staging slots of tts_round_host* (2 x T_max x V logits): device-buffer
+    steps never pay for them; the first host round allocates them once."""
+    case = synth.make_case(4, V=16384, d=256, n_seq=32)
+    T, V = case["T"], case["V"]
+    slots = 2 * T * V * 2
+    ctx = tts.tts_ctx_create(config_for(case), 0)
+    try:
+        t = _buffers(case)
+        mask = torch.zeros(T, dtype=torch.uint8, device="cuda")
+        torch.cuda.synchronize()
+        free0 = torch.cuda.mem_get_info()[0]
+        tts.tts_distill_step(ctx, t["teacher"], t["h"], t["W_in"], t["W_out"], t["master"], t["m"], t["v"], t["pw"],
+                             mask, T, 1.0, t["loss"], None, t["gh"], None)
+        tts.tts_sync_step(ctx)
+        assert torch.cuda.mem_get_info()[0] == free0                     # a step allocates nothing
+        host = [torch.from_numpy(case[k].view(np.int16)).pin_memory() for k in ("teacher", "h")]
+        tok, pw = torch.from_numpy(case["draft_tokens"]).pin_memory(), torch.from_numpy(case["pos_weight"]).pin_memory()
+        loss, tau = torch.zeros(1).pin_memory(), torch.zeros(T // case["seg_len"], dtype=torch.int32).pin_memory()
+
+        def host_round(a, b):
+            tts.tts_round_host(ctx, host[0], host[1], tok, pw, T, 1.0, a, b, t["master"], t["m"], t["v"], None, loss,
+                               tau, None, None)
+
+        host_round(t["W_out"], t["W_in"])
+        free1 = torch.cuda.mem_get_info()[0]
+        assert free0 - free1 >= slots                                    # the first host round brought the slots
+        host_round(t["W_in"], t["W_out"])
+        assert torch.cuda.mem_get_info()[0] == free1                     # and only the first
+    finally:
+        tts.tts_ctx_destroy(ctx)
+
+
 def test_checks_are_off_by_default_and_loss_bit_is_always_on():
     case = synth.make_case(3, V=2048, d=256)
     ctx = tts.tts_ctx_create(config_for(case), 0)
@@ -211,7 +286,9 @@ def test_default_mode_weights_are_bit_reproducible(V, d, n_seq):
 
 def test_a_stalled_pipeline_traps_instead_of_hanging():
     """A protocol slip inside a tensor-path kernel (a wait nobody satisfies) ends in TTS_ERR_CUDA after the watchdog's
-    ~9 s, not in a hung GPU.  The trap kills the CUDA context, so the probe runs in a process of its own."""
+    limit, not in a hung GPU.  The trap kills the CUDA context, so the probe runs in a process of its own, with the
+    limit lowered through TTS_WATCHDOG_CYCLES to 2^31 cycles (~1.1 s) so that the GPU is held only that long; a value
+    that is not a cycle count is refused by tts_ctx_create."""
     import os
     import subprocess
     import sys
@@ -221,16 +298,23 @@ def test_a_stalled_pipeline_traps_instead_of_hanging():
             "import torch\n"
             "from paper_2605_09329_b200 import tts\n"
             "ctx = tts.tts_ctx_create(tts.make_config(2048, 128, 16, 16), 0)\n"
+            "torch.cuda.synchronize(); import time; t0 = time.time()\n"
             "st = tts.tts_debug_trip_watchdog(ctx, torch.cuda.Stream())\n"
-            "print('STATUS', st, tts.tts_last_cuda_error(ctx))\n" % root)
-    t0 = time.time()
-    r = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=120)
-    dt = time.time() - t0
+            "print('STATUS', st, tts.tts_last_cuda_error(ctx), time.time() - t0)\n" % root)
+    env = dict(os.environ, TTS_WATCHDOG_CYCLES=str(1 << 31))
+    r = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=120, env=env)
     line = [l for l in r.stdout.splitlines() if l.startswith("STATUS")]
     assert line, (r.stdout, r.stderr[-500:])
-    _, st, cuda_err = line[0].split()
+    _, st, cuda_err, dt = line[0].split()
     assert int(st) == tts.TTS_ERR_CUDA and int(cuda_err) != 0
-    assert 4.0 < dt < 60.0, dt
+    assert 0.5 < float(dt) < 5.0, dt          # 2^31 cycles at 1.0 - 2.0 GHz
+    os.environ["TTS_WATCHDOG_CYCLES"] = "soon"
+    try:
+        with pytest.raises(tts.TTSError) as e:
+            tts.tts_ctx_create(tts.make_config(2048, 128, 16, 16), 0)
+        assert e.value.status == tts.TTS_ERR_INVALID_ARG
+    finally:
+        del os.environ["TTS_WATCHDOG_CYCLES"]
     # this process's context is untouched: a step still runs
     case = synth.make_case(3, V=2048, d=256)
     g, o = run_gpu(case), run_oracle(case)

@@ -267,6 +267,47 @@ def test_round_host_matches_device_calls():
         tts.tts_ctx_destroy(ctx)
 
 
+def test_round_host_refuses_bad_arguments_before_it_enqueues_anything():
+    """A NULL / misaligned parameter tensor or a bad T comes back as TTS_ERR_INVALID_ARG (not as a CUDA error out of
+    the tensor-map encoder), with no copy or kernel in flight: the state is untouched, and the very next good round on
+    the same slot gives the oracle's step."""
+    case = synth.make_case(3, V=4096, d=256)
+    o = run_oracle(case)
+    from gpu_util import config_for
+    ctx = tts.tts_ctx_create(config_for(case), 0)
+    try:
+        W_in, master = _dev(case["W"]), _dev(case["master"])
+        W_out = torch.empty_like(W_in)
+        m, v = _dev(case["m"]), _dev(case["v"])
+        teacher = torch.from_numpy(case["teacher"].view(np.int16)).pin_memory()
+        h = torch.from_numpy(case["h"].view(np.int16)).pin_memory()
+        tok = torch.from_numpy(case["draft_tokens"]).pin_memory()
+        pw = torch.from_numpy(case["pos_weight"]).pin_memory()
+        loss = torch.full((1,), -1.0).pin_memory()
+        tau = torch.full((1,), -1, dtype=torch.int32).pin_memory()
+        T, ls = case["T"], case["loss_scale"]
+        before = master.clone()
+        bad = [dict(W_in=None), dict(W_out=W_out.view(torch.int16).view(-1)[1:].data_ptr()), dict(master=None),
+               dict(m=None), dict(T=T + 1)]
+        for b in bad:
+            a = dict(W_in=W_in, W_out=W_out, master=master, m=m, T=T)
+            a.update(b)
+            with pytest.raises(tts.TTSError) as e:
+                tts.tts_round_host_begin(ctx, teacher, h, tok, pw, a["T"], ls, a["W_in"], a["W_out"], a["master"],
+                                         a["m"], v, None, loss, tau, None, None)
+            assert e.value.status == tts.TTS_ERR_INVALID_ARG, b
+        torch.cuda.synchronize()
+        assert torch.equal(master, before) and float(loss[0]) == -1.0 and int(tau[0]) == -1
+        with pytest.raises(tts.TTSError):
+            tts.tts_round_host_end(ctx)                      # nothing was begun
+        tts.tts_round_host(ctx, teacher, h, tok, pw, T, ls, W_in, W_out, master, m, v, None, loss, tau, None, None)
+        assert abs(float(loss[0]) - o["loss"]) <= 1e-3 * abs(o["loss"]) + 1e-6
+        np.testing.assert_array_equal(tau.numpy(), o["tau"])
+        assert np.abs(master.cpu().numpy().astype(np.float64) - o["master"]).max() <= 2e-3 * np.abs(o["master"]).max()
+    finally:
+        tts.tts_ctx_destroy(ctx)
+
+
 # R12 / VERDICT r1: the non-zero optimiser state spans the whole reachable band |m| / sqrt(v) <= 7.27, including the
 # most ordinary state of all (a constant gradient for n steps), through every update kernel: the one-canvas stripe
 # kernel (T = 16, d % 1024 == 0), the wide kernel at 16 rows (d = 256), with gh formed in the pass (64 and 256 rows)
