@@ -44,6 +44,9 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=30)
     ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--blocks", type=int, default=5,
+                    help="timed blocks of --steps steps each (barrier + events around every block); ms_per_step is the "
+                         "MEDIAN block, ms_per_step_min / _max the spread (VERDICT r2: one block hid an 8%% box-to-box spread)")
     ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--kernel-path", default="auto", choices=["auto", "simt"])
@@ -418,19 +421,35 @@ def run_ours(args, rank, world, local_rank):
     launches[0] = 0
     sampler = ClockSampler(local_rank)
     sampler.start()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    e0.record(side)
-    for _ in range(args.steps):
-        step()
-    e1.record(side)
-    barrier()
+    # B blocks of exactly K steps, each bracketed by a barrier (which synchronises) and by CUDA events on the stream the
+    # step runs on; per block the max over ranks.  The reported step time is the median block.
+    block_ms, block_phase, n_prof = [], [], 0
+    for _ in range(max(1, args.blocks)):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record(side)
+        for _ in range(args.steps):
+            step()
+        e1.record(side)
+        barrier()
+        block_ms.append(dist_util.max_over_ranks(e0.elapsed_time(e1), tdev))
+        if not vocab:
+            ph, n = tts.tts_profile_read(ctx)      # mean per phase over this block's steps; resets the recorder
+            if n > 0:
+                block_phase.append(ph)
+                n_prof += n
     clocks = sampler.stop()
-    ms_total = e0.elapsed_time(e1)
-    phase_ms, n_prof = tts.tts_profile_read(ctx) if not vocab else ([0.0] * tts.TTS_NUM_PHASES, 0)
     tts.tts_profile_enable(ctx, 0)
     loss_val = float(loss.item())
-    ms_total = dist_util.max_over_ranks(ms_total, tdev)
+
+    def med(xs):
+        s = sorted(xs)
+        return s[len(s) // 2] if len(s) % 2 else 0.5 * (s[len(s) // 2 - 1] + s[len(s) // 2])
+
+    ms_total = med(block_ms)
+    phase_ms = [med([b[i] for b in block_phase]) for i in range(tts.TTS_NUM_PHASES)] if block_phase else \
+        [0.0] * tts.TTS_NUM_PHASES
+    upd_blocks = [b[4] for b in block_phase]
 
     # ---- end to end through HOST buffers: tts_round_host (H2D of the round's inputs, D2H of loss/tau/mask) ----
     e2e = None
@@ -524,19 +543,27 @@ def run_ours(args, rank, world, local_rank):
             "achieved": (upd_bytes / (upd_ms * 1e-3) / 1e9) if upd_ms else None, "peak": peak, "unit": "GB/s",
             "frac": (upd_bytes / (upd_ms * 1e-3) / 1e9 / peak) if upd_ms else None,
             "traffic": profiled_traffic(args.config) if (z_given is None and not vocab and args.moments == "f32") else None,
+            "traffic_source": "NOT measured by this run: dram__bytes_read.sum + dram__bytes_write.sum of one launch from "
+                              "the committed ncu --set full capture profiles/r2_ncu_full_config%d.csv (commit d9a41c9, "
+                              "2026-11-05; the update kernels' data movement is unchanged since)" % args.config,
             "peak_source": peak_src, "algorithmic_bytes_per_launch": upd_bytes, "kernel_ms": upd_ms,
             "step_algorithmic_bytes": step_bytes, "step_achieved": step_bytes / (ms_step * 1e-3) / 1e9,
             "step_frac_of_measured_copy": step_bytes / (ms_step * 1e-3) / 1e9 / peak,
             "step_frac_of_nominal_8TBs": step_bytes / (ms_step * 1e-3) / 1e9 / 8000.0,
+            "kernel_ms_min": min(upd_blocks) if upd_blocks else None,
+            "kernel_ms_max": max(upd_blocks) if upd_blocks else None,
             "phase_ms": dict(zip(tts.PHASE_NAMES, phase_ms)), "profiled_steps": n_prof}
     line = {"metric": "distill_steps_per_sec", "value": sps, "unit": "steps/s", "n_gpus": world,
-            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step,
+            "blocks": len(block_ms), "ms_per_step_min": min(block_ms) / args.steps,
+            "ms_per_step_max": max(block_ms) / args.steps, "higher_is_better": True,
             "scaling": "strong" if vocab else "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
             "config": dict(workload_config(args.config, world, "tcgen05+tma" if used_tensor else "cuda-core",
                                            args.parallelism), **({"T": T, "n_seq_override": args.n_seq} if args.n_seq else {}),
                            draft_logits=args.draft_logits, adam_moments=args.moments),
             "rows_V_per_sec": sps * T * V, "loss": loss_val, "clocks": clocks, "e2e": e2e,
-            "gpu_launches": launches[0], "roofline": roof, "cpu_baseline": cpu}
+            "gpu_launches": launches[0] // len(block_ms), "gpu_launches_all_blocks": launches[0],
+            "roofline": roof, "cpu_baseline": cpu}
     if stream is not None:
         line["stream"] = stream
     # what crosses the fabric per step, for the driver's rank check: replicas exchange nothing on the data path
@@ -801,11 +828,36 @@ def run_tiny(args):
     print(json.dumps(line), flush=True)
 
 
+def launch_ranks(n, argv, device_count, script=None, run=None):
+    """`bench.py --gpus N` started as ONE plain process (no torchrun around it, WORLD_SIZE unset): start the N ranks
+    here, one per GPU, the way the contract's torchrun line does, and return their exit code.  Refuses, loudly, to
+    pretend: with fewer than N devices there is no N-GPU number to print."""
+    import socket
+    import subprocess
+    if device_count < n:
+        raise SystemExit("bench.py --gpus %d: this node has %d CUDA device(s); refusing to run %d ranks on fewer GPUs "
+                         "(a rank per GPU is the only configuration this bench measures)" % (n, device_count, n))
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(n),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), script or os.path.abspath(__file__)] + list(argv)
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")      # the communicator / transport lines the driver's rank check reads
+    return (run or subprocess.call)(cmd, env=env)
+
+
 def main():
     args = parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl != "reference":
+        import torch
+        sys.exit(launch_ranks(args.gpus, sys.argv[1:], torch.cuda.device_count()))
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus and args.impl != "reference" and rank == 0:
+        sys.stderr.write("bench.py: --gpus %d but WORLD_SIZE=%d; n_gpus in the line is the ranks that joined (%d)\n"
+                         % (args.gpus, world, world))
     if args.impl == "reference":
         run_reference(args, rank, world)
     elif args.config == 1:
