@@ -42,7 +42,7 @@ def _free_port():
     return p
 
 
-def _worker(rank, world, port, q):
+def _worker(rank, world, port, q, V=1024):
     os.environ.update(RANK=str(rank), WORLD_SIZE=str(world), LOCAL_RANK=str(rank), MASTER_ADDR="127.0.0.1",
                       MASTER_PORT=str(port))
     import torch.distributed as dist
@@ -50,8 +50,8 @@ def _worker(rank, world, port, q):
     from paper_2605_09329_b200 import dist_util as D
     from workloads import synth
     D.init("gloo")
-    case = synth.make_case(3, V=1024, d=64)            # every rank draws the same seeded case
-    T, V = case["T"], case["V"]
+    case = synth.make_case(3, V=V, d=64)               # every rank draws the same seeded case
+    T = case["T"]
     v0, v1 = sharded.shard_range(V, rank, world)
     t = O.widen(synth.bf16_bits_to_f32(case["teacher"]))
     h = O.widen(synth.bf16_bits_to_f32(case["h"]))
@@ -82,20 +82,24 @@ def _worker(rank, world, port, q):
     dist.destroy_process_group()
 
 
-def test_two_rank_exchange_reproduces_the_unsharded_step():
+@pytest.mark.parametrize("world,V", [(2, 1024), (8, 1152)])
+def test_two_rank_exchange_reproduces_the_unsharded_step(world, V):
+    """world_size 2, and the node size the driver's scaling run uses (8) with a vocabulary whose 128-row blocks do not
+    divide among the ranks (9 blocks over 8 ranks: one shard is twice the others, as 1187 blocks over 8 are uneven)."""
     from oracle import tts_oracle as O
     from workloads import synth
-    world, port = 2, _free_port()
+    port = _free_port()
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
-    ps = [ctx.Process(target=_worker, args=(r, world, port, q)) for r in range(world)]
+    ps = [ctx.Process(target=_worker, args=(r, world, port, q, V)) for r in range(world)]
     for p in ps:
         p.start()
     out = sorted((q.get(timeout=180) for _ in range(world)), key=lambda x: x[0])
     for p in ps:
         p.join(timeout=60)
         assert p.exitcode == 0
-    case = synth.make_case(3, V=1024, d=64)
+    assert len({o[2] - o[1] for o in out}) == (1 if V % (128 * world) == 0 else 2)      # even / uneven shards
+    case = synth.make_case(3, V=V, d=64)
     mask, tau, am = O.accept_mask(case["teacher"], case["draft_tokens"], case["seg_len"])
     ref = O.distill_step(case["teacher"], case["h"], case["W"], case["master"], case["m"], case["v"],
                          case["pos_weight"], mask, seg_len=case["seg_len"], loss_scale=case["loss_scale"],
@@ -107,5 +111,7 @@ def test_two_rank_exchange_reproduces_the_unsharded_step():
         assert abs(loss - ref["loss"]) <= 1e-10 * abs(ref["loss"])
         np.testing.assert_allclose(gh, ref["gh"], rtol=0, atol=1e-12 * np.abs(ref["gh"]).max() + 1e-15)
         # lowest global index among the shards' maxima = the unsharded argmax
-        best = np.where(val_all[0] >= val_all[1], idx_all[0], idx_all[1])
+        assert val_all.shape == idx_all.shape == (world, case["T"])
+        top = val_all.max(axis=0)
+        best = np.where(val_all == top[None, :], idx_all, np.iinfo(np.int32).max).min(axis=0)
         np.testing.assert_array_equal(best, am)
