@@ -121,7 +121,9 @@ int32_t tts_set_lr(tts_ctx* ctx, float lr);
 /* Adam's bias-correction step count n lives in DEVICE memory of the ctx: 0 after create, incremented by the first
  * kernel of every tts_distill_step on the step's stream (so the first step uses n = 1, and a replayed CUDA graph of
  * the step keeps counting).  Set it to resume a stream or after restoring a snapshot (the paper resets the
- * speculator between requests).  Both calls synchronise the device. */
+ * speculator between requests).  Both calls synchronise the WHOLE DEVICE (every stream of every
+ * process on it, a co-resident target model's included): set-up and debugging only.  A running service uses the
+ * stream-ordered forms below. */
 int32_t tts_set_step_count(tts_ctx* ctx, int64_t n);
 int64_t tts_get_step_count(const tts_ctx* ctx);   /* returns the count (-1 on error), not a status */
 /* Stream-ordered forms that do NOT synchronise the device: the set is enqueued on `stream` (put it on the step's side
