@@ -57,7 +57,7 @@ def test_bf16_moments_match_oracle(V, d, n_seq, kind, step):
                                 stored_m_worst_code_distance=worst_m, stored_v_worst_code_distance=worst_v)
     # These two floors are a sanity check only (a code flips wherever the two sides' fp32 moments straddle a rounding
     # boundary, which the gradient tolerance allows); the PIN of the rounding rule is the bit-exact test below.
-    assert eq_m >= 0.7 and eq_v >= 0.5
+    assert eq_m >= 0.88 and eq_v >= 0.80   # observed over the 17 cases (B200, round 3): >= 0.913 / >= 0.852
 
 
 @pytest.mark.parametrize("max_ctas", [3, 7])
@@ -77,7 +77,7 @@ def test_bf16_moments_under_an_sm_budget(max_ctas):
     g["m"], g["v"] = gm, gv
     eq_m, eq_v, worst_m, worst_v = _check_stored(g, o)
     gpu_util.METRICS[-1].update(moments="bf16", max_ctas=max_ctas, stored_m_identical=eq_m, stored_v_identical=eq_v)
-    assert eq_m >= 0.7 and eq_v >= 0.5
+    assert eq_m >= 0.88 and eq_v >= 0.80   # observed over the 17 cases (B200, round 3): >= 0.913 / >= 0.852
     # and the walk does not change what is stored: the unbudgeted grid gives the same codes almost everywhere
     g0 = run_gpu(case, moments="bf16", sr_seed=7)
     assert (g0["m_bits"] == g["m_bits"]).mean() >= 0.999 and (g0["v_bits"] == g["v_bits"]).mean() >= 0.999
